@@ -1,0 +1,220 @@
+/* =====================================================================================
+ * ng.h — C-ABI of libng.so: the per-time-step hot path of a clock-driven spiking-network
+ * simulator as arXiv 2007.14236 defines it, hand-written CUDA for sm_100a.
+ *
+ * What the path computes, per step n (t_n -> t_{n+1}, h = dt):
+ *   a1  LIF (iaf_psc_exp) exact-integration update fused with a Poisson background drive
+ *       PAPER.md:93-102 Eqs. (1)-(2); "integrated by the exact integration scheme
+ *       described in [20] on the time grid"; PAPER.md:187 refractory time; C7, C11
+ *   a2  spike collection into the global spike array          PAPER.md:69, Fig. 1(b)
+ *   a3  spike delivery: every connection (j -> i, w, d) of a neuron j that spiked in step n
+ *       adds w to ring slot (n + d) mod D of target i          PAPER.md:69 (delay-ordered
+ *       connection groups; "when the time index t_s matches the connection-group delay")
+ *   a0  (setup) fixed-indegree / fixed-outdegree connection rules, built directly
+ *       in GPU memory (PAPER.md:292 names this as the fix for the build-time bottleneck)
+ *
+ * Conventions
+ *   - every function returns an int32 status (NG_OK = 0, negatives below); nothing throws or aborts.
+ *     ng_last_error() gives a message owned by the handle, valid until the next call on it.
+ *   - one handle per host thread; no global state.  All device work is enqueued on the CUDA stream
+ *     given to ng_create (NULL = the legacy default stream).
+ *   - pointers named *_host must be host memory; pointers named `data`/`out` in ng_set_state,
+ *     ng_get_state and ng_copy_* may be host OR device memory (unified addressing decides).
+ *     Every buffer passed in is caller-owned; the library never frees caller memory.
+ *   - device memory comes from the ng_allocator callbacks (the Python harness backs them with
+ *     torch tensors); with a NULL allocator cudaMalloc/cudaFree are used.  Everything is released
+ *     by ng_destroy.
+ *   - neuron ids are global, contiguous, assigned in ng_create_population order.
+ *   - time: a spike reported with step n happened at t = (n+1)*h.  A delay of d steps makes the
+ *     synaptic current of the target jump at t = (n+1+d)*h (C10).  1 <= d <= ring_slots.
+ * ===================================================================================== */
+#ifndef NG_H_
+#define NG_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ng_sim ng_sim;
+
+/* status codes */
+enum {
+    NG_OK = 0,
+    NG_ERR_INVALID_ARG = -1,
+    NG_ERR_STATE = -2,      /* call not legal in this state (e.g. connect after prepare) */
+    NG_ERR_OOM = -3,
+    NG_ERR_CUDA = -4,
+    NG_ERR_OVERFLOW = -5    /* spike record full, or a drawn delay outside [1, ring_slots] */
+};
+
+/* ng_config.flags */
+enum {
+    NG_RECORD_SPIKES = 1u << 0,   /* keep (step, id) of every spike on the device until ng_get_spikes */
+    NG_DEBUG_INPUT = 1u << 1      /* keep the ring plane consumed by the last step (field NG_FIELD_LAST_INPUT) */
+};
+
+/* state fields for ng_set_state / ng_get_state */
+enum {
+    NG_FIELD_V = 0,           /* float  [N]   membrane potential, mV                               */
+    NG_FIELD_I_SYN = 1,       /* float  [N]   synaptic current, pA                                 */
+    NG_FIELD_REFR = 2,        /* int32  [N]   remaining refractory steps                           */
+    NG_FIELD_RING = 3,        /* float  [D*N] input ring buffer, slot-major: ring[slot*N + i]      */
+    NG_FIELD_STEP = 4,        /* int64  [1]   index n of the next step                             */
+    NG_FIELD_LAST_INPUT = 5   /* float  [N]   in_i consumed by the last step (needs NG_DEBUG_INPUT; get only) */
+};
+
+/* distribution kinds for weights and delays ("fixed values ... or probability distributions") */
+enum {
+    NG_DIST_CONST = 0,          /* value a                                                          */
+    NG_DIST_NORMAL_CLIPPED = 1, /* a + b*z, z ~ N(0,1) (fp64 Box-Muller, C4), clipped to [lo, hi];
+                                   as a delay: floor(a + b*z + 0.5) clipped to [lo, hi] (C5)   */
+    NG_DIST_UNIFORM_INT = 2     /* integer uniform on [lo, hi] (C5)                       */
+};
+
+/* options for ng_set_option */
+enum {
+    NG_OPT_STEP_MODE = 0,        /* 0 = CUDA graph of NG_OPT_STEPS_PER_GRAPH steps (default),
+                                    1 = plain kernel launches, 2 = one persistent cooperative kernel  */
+    NG_OPT_STEPS_PER_GRAPH = 1,  /* default 100 */
+    NG_OPT_DELIVERY_KERNEL = 2,  /* 0 = auto, 1 = row-chunk walk, 2 = delay-major segment walk        */
+    NG_OPT_DELIVER_BLOCKS = 3,   /* grid size of the delivery kernel, 0 = auto                         */
+    NG_OPT_PROFILE = 4,          /* 1 = time every kernel with CUDA events (forces plain launches);
+                                    results in ng_stats.ms_update / ms_deliver                       */
+    NG_OPT_ASYNC = 5,            /* 1 = ng_simulate returns after enqueueing (no stream synchronise)   */
+    NG_OPT_SORT_SEGMENTS = 6     /* 1 = order records inside each (source, delay) group by target id
+                                    after the build (default 1; must be set before ng_prepare)        */
+};
+
+typedef struct {
+    double dt_ms;                 /* h, PAPER.md:181 uses 0.1 ms                                      */
+    int32_t ring_slots;           /* D >= largest delay in steps (C9), 1..255               */
+    uint32_t flags;               /* NG_RECORD_SPIKES | NG_DEBUG_INPUT                                */
+    uint64_t seed;                /* Philox4x32-10 key (C1)                                 */
+    int64_t max_recorded_spikes;  /* capacity of the device spike record (used with NG_RECORD_SPIKES) */
+    int32_t device;               /* CUDA device ordinal                                              */
+    int32_t reserved;
+} ng_config;
+
+typedef struct {
+    void* (*alloc)(size_t bytes, void* user);   /* returns device memory, 256-byte aligned, or NULL */
+    void (*free)(void* ptr, void* user);
+    void* user;
+} ng_allocator;
+
+/* iaf_psc_exp parameters, symbols of PAPER.md:93-102.  Units: pF, ms, mV, pA, Hz. */
+typedef struct {
+    double C_m, tau_m, tau_syn, E_L, V_th, V_reset, t_ref_ms, I_e;
+    double poisson_rate_hz;   /* total rate of the background drive per neuron (e.g. 8 Hz * K_ext) */
+    double poisson_weight;    /* pA per background event                                           */
+} ng_lif_params;
+
+typedef struct {
+    int32_t kind;   /* NG_DIST_* */
+    int32_t pad;
+    double a, b, lo, hi;
+} ng_dist;
+
+typedef struct {
+    uint64_t steps;              /* steps simulated since ng_create                                 */
+    uint64_t spikes;             /* spikes emitted                                                   */
+    uint64_t events;             /* synaptic events delivered = sum over spikes of the out-degree    */
+    uint64_t recorded_dropped;   /* spikes not recorded because the record was full                  */
+    int64_t n_neurons;
+    int64_t n_connections;       /* S, records drawn                                                 */
+    int64_t n_records_padded;    /* records stored (rows padded to a multiple of 4)                  */
+    int64_t max_row_records;     /* longest padded row                                               */
+    double build_ms;             /* device time of the connection build                              */
+    double ms_update;            /* with NG_OPT_PROFILE: summed device time of the update kernel     */
+    double ms_deliver;           /* with NG_OPT_PROFILE: summed device time of the delivery kernel   */
+    uint64_t launches_update;    /* kernel launches (or graph kernel nodes executed) since create    */
+    uint64_t launches_deliver;
+    uint64_t launches_other;     /* builder and bookkeeping kernels                                  */
+    int32_t delivery_kernel;     /* the delivery kernel in use (1 or 2)                              */
+    int32_t step_mode;
+} ng_stats;
+
+/* Create a simulator on cfg->device.  `alloc` may be NULL.  `cuda_stream` is a cudaStream_t (or NULL).
+ * Errors: INVALID_ARG (dt <= 0, ring_slots outside 1..255, out == NULL), CUDA. */
+int32_t ng_create(const ng_config* cfg, const ng_allocator* alloc, void* cuda_stream, ng_sim** out);
+
+/* Release every device allocation and the handle.  NULL is accepted. */
+int32_t ng_destroy(ng_sim* sim);
+
+/* Message for the last error on this handle ("" if none).  Never NULL. */
+const char* ng_last_error(const ng_sim* sim);
+
+/* Add n neurons sharing one parameter set (PAPER.md:39-48 `Create`, `SetStatus`).  first_id_out (nullable)
+ * receives the id of the first one.  Initial state: V = E_L, I_syn = 0, not refractory.
+ * Errors: STATE after ng_prepare; INVALID_ARG for n <= 0, more than 255 populations, non-positive C_m /
+ * tau_m / tau_syn / dt, |tau_m - tau_syn| < 1e-9 ms (C19), Poisson rate*h too large for the
+ * 64-entry integer CDF table. */
+int32_t ng_create_population(ng_sim* sim, int32_t n, const ng_lif_params* params, int32_t* first_id_out);
+
+/* PAPER.md:37 rule "fixed indegree": every target in [tgt_first, tgt_first+tgt_n) receives exactly K
+ * connections whose sources are drawn uniformly with replacement from [src_first, src_first+src_n)
+ * (autapses and multapses allowed, C3).  Draw (target i, k) of call c is a pure function of
+ * (seed, c, i, k) (C1-C5); call order defines c.  Nothing is built until ng_prepare.
+ * Errors: STATE after ng_prepare; INVALID_ARG for ranges outside the created neurons, K < 0, bad dist. */
+int32_t ng_connect_fixed_indegree(ng_sim* sim, int32_t src_first, int32_t src_n, int32_t tgt_first,
+                                  int32_t tgt_n, int32_t K, const ng_dist* weight, const ng_dist* delay_steps);
+
+/* PAPER.md:37 rule "fixed outdegree": every source sends exactly K connections to targets drawn uniformly
+ * with replacement; draw (source j, k).  Same errors. */
+int32_t ng_connect_fixed_outdegree(ng_sim* sim, int32_t src_first, int32_t src_n, int32_t tgt_first,
+                                   int32_t tgt_n, int32_t K, const ng_dist* weight, const ng_dist* delay_steps);
+
+/* Delivery-only mode (BASELINE.json configs[3], C8): the neuron update is bypassed and source s
+ * fires in step n iff Philox(INJECT; s, n).x0 < floor(fraction * 2^32).  Before ng_prepare only. */
+int32_t ng_set_bypass(ng_sim* sim, int32_t bypass, double inject_fraction);
+
+/* Tuning / instrumentation knobs (NG_OPT_*).  Errors: INVALID_ARG, STATE. */
+int32_t ng_set_option(ng_sim* sim, int32_t option, int64_t value);
+
+/* Build the connection structure on the device (source-major rows, each ordered into groups of equal
+ * delay, PAPER.md:69 / Fig. 1a) and allocate state.  Implied by the first ng_simulate.
+ * Errors: OOM, CUDA, OVERFLOW (a drawn delay outside [1, ring_slots]); STATE if no population exists. */
+int32_t ng_prepare(ng_sim* sim);
+
+/* Copy `count` elements of a state field starting at element `first` from/to `data` (host or device).
+ * Element types and lengths are listed at NG_FIELD_*.  Synchronises the stream.
+ * Errors: STATE before ng_prepare; INVALID_ARG for a bad field or range. */
+int32_t ng_set_state(ng_sim* sim, int32_t field, const void* data, int64_t count, int64_t first);
+int32_t ng_get_state(ng_sim* sim, int32_t field, void* out, int64_t count, int64_t first);
+
+/* Advance n_steps time steps (a1 -> a2 -> a3 each step).  Synchronises the stream before returning unless
+ * NG_OPT_ASYNC is set.  Returns OVERFLOW if the spike record filled up during the call (the simulation
+ * state stays valid; only recording stopped). */
+int32_t ng_simulate(ng_sim* sim, int64_t n_steps);
+
+/* Copy up to `capacity` recorded spikes (ordered by step; ids unordered within a step) into caller HOST
+ * arrays and drain what was copied.  count_out always receives the number currently recorded BEFORE the
+ * copy, so a call with capacity 0 sizes the buffers.  Errors: STATE (recording not enabled). */
+int32_t ng_get_spikes(ng_sim* sim, int32_t* steps_host, int32_t* ids_host, int64_t capacity, int64_t* count_out);
+
+/* Ids that spiked in the most recent step (the spike array of PAPER.md:69), into a HOST array. */
+int32_t ng_get_last_spikes(ng_sim* sim, int32_t* ids_host, int64_t capacity, int64_t* count_out);
+
+/* Connection structure read-back for parity checks (host or device destinations, any may be NULL).
+ *   ng_copy_row_offsets: int64[N+1]; row j holds records [off[j], off[j+1]), padded to a multiple of 4
+ *                        with records whose target is -1.
+ *   ng_copy_group_offsets: uint32[N*(D+1)]; group of delay d (1-based) of source j is records
+ *                        off[j] + g[j*(D+1)+d-1] .. off[j] + g[j*(D+1)+d]  (exclusive).
+ *   ng_copy_records: records [first, first+count): int32 target, float weight, uint8 delay. */
+int32_t ng_copy_row_offsets(ng_sim* sim, int64_t* out);
+int32_t ng_copy_group_offsets(ng_sim* sim, uint32_t* out);
+int32_t ng_copy_records(ng_sim* sim, int64_t first, int64_t count, int32_t* tgt, float* w, uint8_t* delay);
+
+/* Outgoing connections of one source into HOST arrays (padding removed); count_out = its out-degree. */
+int32_t ng_get_connections(ng_sim* sim, int32_t src_id, int32_t* tgt_host, float* w_host, uint8_t* delay_host,
+                           int64_t capacity, int64_t* count_out);
+
+/* Counters and timings.  Synchronises the stream. */
+int32_t ng_get_stats(ng_sim* sim, ng_stats* out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NG_H_ */

@@ -1,0 +1,681 @@
+// =====================================================================================
+// ng.cu — host side of libng.so: the C-ABI declared in include/ng.h.
+//
+// Holds the population table and the list of connect calls, runs the on-device connection builder
+// (ng_prepare) and enqueues the per-step kernels of ng_device.cuh (ng_simulate), either as a replayed CUDA
+// graph of `steps_per_graph` steps, as plain launches, or as one persistent cooperative kernel.
+//
+// Update/deliver handshake without host round trips: update(n) reads ctl.step_u and writes ctl.step_d;
+// deliver(n) reads ctl.step_d and ctl.spike_cnt[n&1], and one of its threads writes ctl.step_u = n+1 and
+// clears ctl.spike_cnt[(n+1)&1].  Each kernel only reads words the other kind of kernel writes, so a captured
+// graph replays unchanged for any step index.
+//
+// No CPU fallback exists: every entry point that computes needs a CUDA device and fails with NG_ERR_CUDA otherwise.
+// =====================================================================================
+#include "../../include/ng.h"
+#include "ng_device.cuh"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+using namespace ng;
+
+struct HostPop { int32_t first, n; ng_lif_params p; PopDev dev; };
+
+struct ng_sim {
+    ng_config cfg{};
+    ng_allocator alloc{};
+    bool has_alloc = false;
+    cudaStream_t stream = nullptr;
+    bool own_stream = false;
+    std::string err;
+    std::vector<HostPop> pops;
+    std::vector<CallDev> calls;
+    int32_t N = 0;
+    int64_t S = 0;
+    bool prepared = false;
+    int32_t bypass = 0; uint32_t inject_thr = 0;
+    // options
+    int step_mode = 0; int steps_per_graph = 100; int delivery_kernel_opt = 0; int deliver_blocks_opt = 0;
+    int profile = 0; int async = 0; int sort_segments = 1;
+    // device
+    std::vector<void*> allocs;
+    StepArgs a{};
+    uint32_t* d_cnt = nullptr; long long* d_row_len = nullptr; long long* d_row_off = nullptr;
+    uint32_t* d_grp_rel = nullptr; int32_t* d_tgt = nullptr; float* d_w = nullptr; uint8_t* d_dly = nullptr;
+    CallDev* d_calls = nullptr; PopDev* d_pops = nullptr; uint8_t* d_pop_of = nullptr; Ctl* d_ctl = nullptr;
+    int64_t n_padded = 0; int64_t max_row_records = 0;
+    int sm_count = 148; size_t l2_bytes = 0;
+    int delivery_kernel = 1; int deliver_blocks = 0; int update_blocks = 0; int persistent_blocks = 0;
+    cudaGraphExec_t graph_exec = nullptr; int graph_steps = 0;
+    // stats
+    double build_ms = 0, ms_update = 0, ms_deliver = 0;
+    uint64_t launches_update = 0, launches_deliver = 0, launches_other = 0;
+    uint64_t rec_dropped = 0;
+    uint64_t steps_done = 0;
+};
+
+namespace {
+
+int32_t fail(ng_sim* s, int32_t code, const std::string& msg) {
+    if (s) s->err = msg;
+    return code;
+}
+#define NG_CUDA(s, expr)                                                                              \
+    do {                                                                                              \
+        cudaError_t e_ = (expr);                                                                      \
+        if (e_ != cudaSuccess)                                                                        \
+            return fail((s), e_ == cudaErrorMemoryAllocation ? NG_ERR_OOM : NG_ERR_CUDA,              \
+                        std::string(#expr) + ": " + cudaGetErrorString(e_));                          \
+    } while (0)
+
+void* dev_alloc(ng_sim* s, size_t bytes) {
+    if (bytes == 0) bytes = 256;
+    void* p = nullptr;
+    if (s->has_alloc) p = s->alloc.alloc(bytes, s->alloc.user);
+    else if (cudaMalloc(&p, bytes) != cudaSuccess) { cudaGetLastError(); p = nullptr; }
+    if (p) s->allocs.push_back(p);
+    return p;
+}
+void dev_free(ng_sim* s, void* p) {
+    if (!p) return;
+    auto it = std::find(s->allocs.begin(), s->allocs.end(), p);
+    if (it != s->allocs.end()) s->allocs.erase(it);
+    if (s->has_alloc) s->alloc.free(p, s->alloc.user);
+    else cudaFree(p);
+}
+template <typename T>
+bool dev_alloc_t(ng_sim* s, T** out, size_t count) {
+    *out = (T*)dev_alloc(s, count * sizeof(T));
+    return *out != nullptr;
+}
+
+// Exact-integration propagators of PAPER.md Eqs. (1)-(2) over one step h (ref. 20), fp64:
+// x = (I, V - E_L), dx/dt = A x, A = [[-1/tau_syn, 0], [1/C_m, -1/tau_m]]; exp(A h) = [[P11, 0], [P21, P22]].
+void make_pop_dev(const ng_lif_params& p, double h, PopDev& d) {
+    const double P11 = std::exp(-h / p.tau_syn);
+    const double P22 = std::exp(-h / p.tau_m);
+    const double P21 = p.tau_m * p.tau_syn / (p.C_m * (p.tau_m - p.tau_syn)) * (P22 - P11);
+    const double P20 = p.tau_m / p.C_m * (1.0 - P22);
+    d.P11 = (float)P11; d.P22 = (float)P22; d.P21 = (float)P21; d.P20Ie = (float)(P20 * p.I_e);
+    d.E_L = (float)p.E_L; d.V_th = (float)p.V_th; d.V_reset = (float)p.V_reset; d.w_ext = (float)p.poisson_weight;
+    d.refr_steps = (int32_t)std::floor(p.t_ref_ms / h + 0.5);
+}
+
+// DESIGN.md C7: T[m] = floor(CDF_Poisson(lambda)(m) * 2^32), saturating at 2^32-1, with the pmf recurrence
+// p_0 = exp(-lambda), p_{m+1} = (p_m * lambda) / (m+1), CDF accumulated in that order in fp64.
+bool make_poisson_table(double lam, PopDev& d) {
+    d.n_T = 0;
+    if (!(lam > 0.0)) return true;
+    double p = std::exp(-lam), c = p;
+    for (int m = 0; m < kMaxPoissonTable; ++m) {
+        const double s = std::floor(c * 4294967296.0);
+        const uint32_t t = s >= 4294967295.0 ? 4294967295u : (uint32_t)s;
+        d.T[d.n_T++] = t;
+        if (t == 4294967295u) return true;
+        const double pl = p * lam;
+        p = pl / (double)(m + 1);
+        c = c + p;
+    }
+    return false;
+}
+
+bool valid_dist(const ng_dist* d) {
+    return d && d->kind >= NG_DIST_CONST && d->kind <= NG_DIST_UNIFORM_INT;
+}
+
+int32_t add_call(ng_sim* s, int32_t rule, int32_t src_first, int32_t src_n, int32_t tgt_first, int32_t tgt_n, int32_t K,
+                 const ng_dist* w, const ng_dist* d) {
+    if (!s) return NG_ERR_INVALID_ARG;
+    if (s->prepared) return fail(s, NG_ERR_STATE, "connect after ng_prepare");
+    if (!valid_dist(w) || !valid_dist(d)) return fail(s, NG_ERR_INVALID_ARG, "bad distribution");
+    if (src_n <= 0 || tgt_n <= 0 || K < 0 || src_first < 0 || tgt_first < 0 ||
+        (int64_t)src_first + src_n > s->N || (int64_t)tgt_first + tgt_n > s->N)
+        return fail(s, NG_ERR_INVALID_ARG, "population range outside the created neurons, or K < 0");
+    CallDev c{};
+    c.rule = rule; c.src_first = src_first; c.src_n = src_n; c.tgt_first = tgt_first; c.tgt_n = tgt_n; c.K = K;
+    c.call_index = (int32_t)s->calls.size();
+    c.w = DistDev{w->kind, 0, w->a, w->b, w->lo, w->hi};
+    c.d = DistDev{d->kind, 0, d->a, d->b, d->lo, d->hi};
+    s->calls.push_back(c);
+    return NG_OK;
+}
+
+int grid_for(long long work, int threads, int cap) {
+    long long b = (work + threads - 1) / threads;
+    if (b < 1) b = 1;
+    if (b > cap) b = cap;
+    return (int)b;
+}
+
+void destroy_graph(ng_sim* s) {
+    if (s->graph_exec) { cudaGraphExecDestroy(s->graph_exec); s->graph_exec = nullptr; s->graph_steps = 0; }
+}
+
+void launch_update(ng_sim* s) {
+    update_kernel<<<s->update_blocks, kUpdateThreads, 0, s->stream>>>(s->a);
+}
+void launch_deliver(ng_sim* s) {
+    if (s->delivery_kernel == 2) deliver_kernel<2><<<s->deliver_blocks, kDeliverThreads, 0, s->stream>>>(s->a);
+    else deliver_kernel<1><<<s->deliver_blocks, kDeliverThreads, 0, s->stream>>>(s->a);
+}
+
+// choose launch shapes from the built network (static per simulation; no per-step host decisions)
+void configure_launch(ng_sim* s) {
+    const int sm = s->sm_count;
+    s->update_blocks = grid_for(s->N, kUpdateThreads, sm * 32);
+    // delivery kernel: delay-major segment walk pays off when the ring is too big to stay in L2 next to the
+    // streamed records and groups are long enough to fill a warp's 128-bit loads; otherwise walk whole rows.
+    const double ring_bytes = (double)s->N * s->cfg.ring_slots * 4.0;
+    const double mean_group = s->N > 0 ? (double)s->S / ((double)s->N * s->cfg.ring_slots) : 0.0;
+    int k = s->delivery_kernel_opt;
+    if (k == 0) k = (ring_bytes > 0.5 * (double)s->l2_bytes && mean_group >= 64.0) ? 2 : 1;
+    s->delivery_kernel = k;
+    int blocks = s->deliver_blocks_opt;
+    if (blocks <= 0) {
+        // enough warps to cover the expected items of a step, between one and eight CTAs per SM
+        const double mean_row = s->N > 0 ? (double)s->n_padded / s->N : 0.0;
+        const double work_warps = std::max(1.0, mean_row / kChunkRecords) * std::max(1.0, s->N * 0.002);
+        long long b = (long long)(work_warps / (kDeliverThreads / 32)) + 1;
+        b = ((b + sm - 1) / sm) * sm;
+        blocks = (int)std::min<long long>(std::max<long long>(b, sm), (long long)sm * 8);
+    }
+    s->deliver_blocks = blocks;
+    s->a.max_row_chunks = (int32_t)((s->max_row_records + kChunkRecords - 1) / kChunkRecords);
+    if (s->a.max_row_chunks < 1) s->a.max_row_chunks = 1;
+    int occ = 0;
+    if (s->delivery_kernel == 2) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, persistent_kernel<2>, kUpdateThreads, 0);
+    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, persistent_kernel<1>, kUpdateThreads, 0);
+    if (occ < 1) occ = 1;
+    // a small grid makes the grid-wide barrier cheap; large networks want every resident warp
+    const long long want = std::max<long long>((s->N + kUpdateThreads - 1) / kUpdateThreads, s->deliver_blocks);
+    long long pb = std::min<long long>((long long)sm * occ, std::max<long long>(want, sm));
+    pb = (pb / sm) * sm; if (pb < sm) pb = sm;
+    s->persistent_blocks = (int)pb;
+    destroy_graph(s);
+}
+
+int32_t build_graph(ng_sim* s, int steps) {
+    destroy_graph(s);
+    cudaGraph_t graph = nullptr;
+    NG_CUDA(s, cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeThreadLocal));
+    for (int i = 0; i < steps; ++i) { launch_update(s); launch_deliver(s); }
+    NG_CUDA(s, cudaStreamEndCapture(s->stream, &graph));
+    cudaError_t e = cudaGraphInstantiate(&s->graph_exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e != cudaSuccess) return fail(s, NG_ERR_CUDA, std::string("cudaGraphInstantiate: ") + cudaGetErrorString(e));
+    s->graph_steps = steps;
+    return NG_OK;
+}
+
+int32_t read_ctl(ng_sim* s, Ctl* out) {
+    NG_CUDA(s, cudaMemcpyAsync(out, s->d_ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, s->stream));
+    NG_CUDA(s, cudaStreamSynchronize(s->stream));
+    return NG_OK;
+}
+
+int32_t field_info(ng_sim* s, int32_t field, void** base, size_t* elem, int64_t* len) {
+    switch (field) {
+        case NG_FIELD_V: *base = s->a.V; *elem = 4; *len = s->N; return NG_OK;
+        case NG_FIELD_I_SYN: *base = s->a.I; *elem = 4; *len = s->N; return NG_OK;
+        case NG_FIELD_REFR: *base = s->a.refr; *elem = 4; *len = s->N; return NG_OK;
+        case NG_FIELD_RING: *base = s->a.ring; *elem = 4; *len = (int64_t)s->N * s->cfg.ring_slots; return NG_OK;
+        case NG_FIELD_LAST_INPUT:
+            if (!s->a.last_input) return fail(s, NG_ERR_STATE, "NG_FIELD_LAST_INPUT needs NG_DEBUG_INPUT");
+            *base = s->a.last_input; *elem = 4; *len = s->N; return NG_OK;
+        default: return fail(s, NG_ERR_INVALID_ARG, "unknown field");
+    }
+}
+
+}  // namespace
+
+extern "C" {
+
+int32_t ng_create(const ng_config* cfg, const ng_allocator* alloc, void* cuda_stream, ng_sim** out) {
+    if (!out) return NG_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!cfg || !(cfg->dt_ms > 0.0) || cfg->ring_slots < 1 || cfg->ring_slots > 255 || cfg->max_recorded_spikes < 0)
+        return NG_ERR_INVALID_ARG;
+    if (cudaSetDevice(cfg->device) != cudaSuccess) { cudaGetLastError(); return NG_ERR_CUDA; }
+    ng_sim* s = new ng_sim();
+    s->cfg = *cfg;
+    if (alloc && alloc->alloc && alloc->free) { s->alloc = *alloc; s->has_alloc = true; }
+    if (cuda_stream) s->stream = (cudaStream_t)cuda_stream;
+    else {
+        if (cudaStreamCreateWithFlags(&s->stream, cudaStreamNonBlocking) != cudaSuccess) { delete s; return NG_ERR_CUDA; }
+        s->own_stream = true;
+    }
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, cfg->device) == cudaSuccess) {
+        s->sm_count = prop.multiProcessorCount;
+        s->l2_bytes = (size_t)prop.l2CacheSize;
+    }
+    *out = s;
+    return NG_OK;
+}
+
+int32_t ng_destroy(ng_sim* s) {
+    if (!s) return NG_OK;
+    cudaSetDevice(s->cfg.device);
+    if (s->stream) cudaStreamSynchronize(s->stream);
+    destroy_graph(s);
+    std::vector<void*> all = s->allocs;
+    for (void* p : all) dev_free(s, p);
+    if (s->own_stream) cudaStreamDestroy(s->stream);
+    delete s;
+    return NG_OK;
+}
+
+const char* ng_last_error(const ng_sim* s) { return s ? s->err.c_str() : "null handle"; }
+
+int32_t ng_create_population(ng_sim* s, int32_t n, const ng_lif_params* p, int32_t* first_id_out) {
+    if (!s || !p) return NG_ERR_INVALID_ARG;
+    if (s->prepared) return fail(s, NG_ERR_STATE, "population after ng_prepare");
+    if (n <= 0 || (int64_t)s->N + n > 2147483000LL) return fail(s, NG_ERR_INVALID_ARG, "n <= 0 or too many neurons");
+    if (s->pops.size() >= 255) return fail(s, NG_ERR_INVALID_ARG, "more than 255 populations");
+    if (!(p->C_m > 0.0) || !(p->tau_m > 0.0) || !(p->tau_syn > 0.0) || p->t_ref_ms < 0.0 || p->poisson_rate_hz < 0.0)
+        return fail(s, NG_ERR_INVALID_ARG, "non-positive C_m, tau_m or tau_syn, or negative t_ref / rate");
+    if (std::fabs(p->tau_m - p->tau_syn) < 1e-9) return fail(s, NG_ERR_INVALID_ARG, "tau_m == tau_syn (DESIGN.md C19)");
+    HostPop hp{};
+    hp.first = s->N; hp.n = n; hp.p = *p;
+    make_pop_dev(*p, s->cfg.dt_ms, hp.dev);
+    if (!make_poisson_table(p->poisson_rate_hz * s->cfg.dt_ms * 1e-3, hp.dev))
+        return fail(s, NG_ERR_INVALID_ARG, "Poisson rate * h too large for the 64-entry CDF table");
+    s->pops.push_back(hp);
+    s->N += n;
+    if (first_id_out) *first_id_out = hp.first;
+    return NG_OK;
+}
+
+int32_t ng_connect_fixed_indegree(ng_sim* s, int32_t src_first, int32_t src_n, int32_t tgt_first, int32_t tgt_n, int32_t K,
+                                  const ng_dist* w, const ng_dist* d) {
+    return add_call(s, kRuleIndegree, src_first, src_n, tgt_first, tgt_n, K, w, d);
+}
+int32_t ng_connect_fixed_outdegree(ng_sim* s, int32_t src_first, int32_t src_n, int32_t tgt_first, int32_t tgt_n, int32_t K,
+                                   const ng_dist* w, const ng_dist* d) {
+    return add_call(s, kRuleOutdegree, src_first, src_n, tgt_first, tgt_n, K, w, d);
+}
+
+int32_t ng_set_bypass(ng_sim* s, int32_t bypass, double fraction) {
+    if (!s) return NG_ERR_INVALID_ARG;
+    if (s->prepared) return fail(s, NG_ERR_STATE, "ng_set_bypass after ng_prepare");
+    if (!(fraction >= 0.0) || fraction > 1.0) return fail(s, NG_ERR_INVALID_ARG, "fraction outside [0, 1]");
+    s->bypass = bypass ? 1 : 0;
+    double t = std::floor(fraction * 4294967296.0);
+    if (t > 4294967295.0) t = 4294967295.0;
+    s->inject_thr = (uint32_t)t;
+    return NG_OK;
+}
+
+int32_t ng_set_option(ng_sim* s, int32_t option, int64_t value) {
+    if (!s) return NG_ERR_INVALID_ARG;
+    switch (option) {
+        case NG_OPT_STEP_MODE:
+            if (value < 0 || value > 2) return fail(s, NG_ERR_INVALID_ARG, "step mode is 0, 1 or 2");
+            s->step_mode = (int)value; break;
+        case NG_OPT_STEPS_PER_GRAPH:
+            if (value < 1 || value > 10000) return fail(s, NG_ERR_INVALID_ARG, "steps per graph in 1..10000");
+            s->steps_per_graph = (int)value; destroy_graph(s); break;
+        case NG_OPT_DELIVERY_KERNEL:
+            if (value < 0 || value > 2) return fail(s, NG_ERR_INVALID_ARG, "delivery kernel is 0, 1 or 2");
+            s->delivery_kernel_opt = (int)value; if (s->prepared) configure_launch(s); break;
+        case NG_OPT_DELIVER_BLOCKS:
+            if (value < 0 || value > (1 << 20)) return fail(s, NG_ERR_INVALID_ARG, "deliver blocks out of range");
+            s->deliver_blocks_opt = (int)value; if (s->prepared) configure_launch(s); break;
+        case NG_OPT_PROFILE: s->profile = value ? 1 : 0; break;
+        case NG_OPT_ASYNC: s->async = value ? 1 : 0; break;
+        case NG_OPT_SORT_SEGMENTS:
+            if (s->prepared) return fail(s, NG_ERR_STATE, "NG_OPT_SORT_SEGMENTS after ng_prepare");
+            s->sort_segments = value ? 1 : 0; break;
+        default: return fail(s, NG_ERR_INVALID_ARG, "unknown option");
+    }
+    return NG_OK;
+}
+
+int32_t ng_prepare(ng_sim* s) {
+    if (!s) return NG_ERR_INVALID_ARG;
+    if (s->prepared) return NG_OK;
+    if (s->N <= 0) return fail(s, NG_ERR_STATE, "no population");
+    NG_CUDA(s, cudaSetDevice(s->cfg.device));
+    const int N = s->N, D = s->cfg.ring_slots;
+    cudaStream_t st = s->stream;
+    s->S = 0;
+    for (const CallDev& c : s->calls) s->S += (int64_t)(c.rule == kRuleIndegree ? c.tgt_n : c.src_n) * c.K;
+
+    cudaEvent_t e0, e1;
+    NG_CUDA(s, cudaEventCreate(&e0));
+    NG_CUDA(s, cudaEventCreate(&e1));
+    NG_CUDA(s, cudaEventRecord(e0, st));
+
+    // ---- control block, populations, state ----
+    bool ok = dev_alloc_t(s, &s->d_ctl, 1) && dev_alloc_t(s, &s->d_pops, s->pops.size()) &&
+              dev_alloc_t(s, &s->d_pop_of, (size_t)N) && dev_alloc_t(s, &s->a.V, (size_t)N) &&
+              dev_alloc_t(s, &s->a.I, (size_t)N) && dev_alloc_t(s, &s->a.refr, (size_t)N) &&
+              dev_alloc_t(s, &s->a.ring, (size_t)N * D) && dev_alloc_t(s, &s->a.spike_list, (size_t)2 * N) &&
+              dev_alloc_t(s, &s->d_calls, std::max<size_t>(1, s->calls.size())) &&
+              dev_alloc_t(s, &s->d_cnt, (size_t)N * D) && dev_alloc_t(s, &s->d_row_len, (size_t)N) &&
+              dev_alloc_t(s, &s->d_row_off, (size_t)N + 1) && dev_alloc_t(s, &s->d_grp_rel, (size_t)N * (D + 1));
+    if (ok && (s->cfg.flags & NG_DEBUG_INPUT)) ok = dev_alloc_t(s, &s->a.last_input, (size_t)N);
+    if (ok && (s->cfg.flags & NG_RECORD_SPIKES) && s->cfg.max_recorded_spikes > 0) {
+        ok = dev_alloc_t(s, &s->a.rec_step, (size_t)s->cfg.max_recorded_spikes) &&
+             dev_alloc_t(s, &s->a.rec_id, (size_t)s->cfg.max_recorded_spikes);
+        s->a.rec_cap = s->cfg.max_recorded_spikes;
+    }
+    if (!ok) return fail(s, NG_ERR_OOM, "device allocation failed (state)");
+    NG_CUDA(s, cudaMemsetAsync(s->d_ctl, 0, sizeof(Ctl), st));
+    NG_CUDA(s, cudaMemsetAsync(s->a.I, 0, (size_t)N * 4, st));
+    NG_CUDA(s, cudaMemsetAsync(s->a.refr, 0, (size_t)N * 4, st));
+    NG_CUDA(s, cudaMemsetAsync(s->a.ring, 0, (size_t)N * D * 4, st));
+    NG_CUDA(s, cudaMemsetAsync(s->d_cnt, 0, (size_t)N * D * 4, st));
+    if (s->a.last_input) NG_CUDA(s, cudaMemsetAsync(s->a.last_input, 0, (size_t)N * 4, st));
+    std::vector<PopDev> pd(s->pops.size());
+    for (size_t i = 0; i < s->pops.size(); ++i) pd[i] = s->pops[i].dev;
+    NG_CUDA(s, cudaMemcpyAsync(s->d_pops, pd.data(), pd.size() * sizeof(PopDev), cudaMemcpyHostToDevice, st));
+    if (!s->calls.empty())
+        NG_CUDA(s, cudaMemcpyAsync(s->d_calls, s->calls.data(), s->calls.size() * sizeof(CallDev), cudaMemcpyHostToDevice, st));
+    for (size_t i = 0; i < s->pops.size(); ++i) {
+        const HostPop& hp = s->pops[i];
+        fill_pop_of_kernel<<<(hp.n + 255) / 256, 256, 0, st>>>(s->d_pop_of, s->a.V, hp.first, hp.n, (uint8_t)i, hp.dev.E_L);
+        s->launches_other++;
+    }
+
+    // ---- connection build (a0) ----
+    const uint32_t seed_lo = (uint32_t)s->cfg.seed, seed_hi = (uint32_t)(s->cfg.seed >> 32);
+    const int cap = s->sm_count * 16;
+    for (size_t ci = 0; ci < s->calls.size(); ++ci) {
+        const CallDev& c = s->calls[ci];
+        const long long total = (long long)(c.rule == kRuleIndegree ? c.tgt_n : c.src_n) * c.K;
+        if (total == 0) continue;
+        build_count_kernel<<<grid_for(total, 256, cap), 256, 0, st>>>(s->d_calls, (int)ci, seed_lo, seed_hi, D, s->d_cnt, s->d_ctl);
+        s->launches_other++;
+    }
+    build_rowlen_kernel<<<(N + 255) / 256, 256, 0, st>>>(s->d_cnt, N, D, s->d_row_len, s->d_ctl);
+    scan_exclusive_kernel<<<1, 1024, 0, st>>>(s->d_row_len, s->d_row_off, N, s->d_ctl);
+    build_groups_kernel<<<(N + 255) / 256, 256, 0, st>>>(s->d_cnt, N, D, s->d_grp_rel);
+    s->launches_other += 3;
+    Ctl h{};
+    int32_t rc = read_ctl(s, &h);
+    if (rc) return rc;
+    NG_CUDA(s, cudaGetLastError());
+    if (h.err_delay) return fail(s, NG_ERR_OVERFLOW, "a drawn delay fell outside [1, ring_slots]");
+    s->n_padded = (int64_t)h.n_padded;
+    s->max_row_records = h.max_row_records;
+    const size_t np = (size_t)std::max<int64_t>(s->n_padded, 4);
+    if (!(dev_alloc_t(s, &s->d_tgt, np) && dev_alloc_t(s, &s->d_w, np) && dev_alloc_t(s, &s->d_dly, np)))
+        return fail(s, NG_ERR_OOM, "device allocation failed (connection records)");
+    NG_CUDA(s, cudaMemsetAsync(s->d_tgt, 0xFF, np * 4, st));       // padding records: target -1, weight 0, delay 0
+    NG_CUDA(s, cudaMemsetAsync(s->d_w, 0, np * 4, st));
+    NG_CUDA(s, cudaMemsetAsync(s->d_dly, 0, np, st));
+    for (size_t ci = 0; ci < s->calls.size(); ++ci) {
+        const CallDev& c = s->calls[ci];
+        const long long total = (long long)(c.rule == kRuleIndegree ? c.tgt_n : c.src_n) * c.K;
+        if (total == 0) continue;
+        build_fill_kernel<<<grid_for(total, 256, cap), 256, 0, st>>>(s->d_calls, (int)ci, seed_lo, seed_hi, D, s->d_cnt,
+                                                                   s->d_row_off, s->d_grp_rel, s->d_tgt, s->d_w, s->d_dly);
+        s->launches_other++;
+    }
+    if (s->sort_segments) {
+        build_sort_groups_kernel<<<s->sm_count * 8, 256, 0, st>>>(N, D, s->d_row_off, s->d_grp_rel, s->d_tgt, s->d_w);
+        s->launches_other++;
+    }
+    NG_CUDA(s, cudaEventRecord(e1, st));
+    NG_CUDA(s, cudaStreamSynchronize(st));
+    NG_CUDA(s, cudaGetLastError());
+    float ms = 0;
+    cudaEventElapsedTime(&ms, e0, e1);
+    s->build_ms = ms;
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    // the per-(source, delay) counters and the row lengths are builder scratch
+    dev_free(s, s->d_cnt); s->d_cnt = nullptr;
+    dev_free(s, s->d_row_len); s->d_row_len = nullptr;
+
+    // ---- step arguments ----
+    s->a.N = N; s->a.D = D; s->a.seed_lo = seed_lo; s->a.seed_hi = seed_hi;
+    s->a.pop_of = s->d_pop_of; s->a.pops = s->d_pops;
+    s->a.row_off = s->d_row_off; s->a.grp_rel = s->d_grp_rel; s->a.tgt = s->d_tgt; s->a.w = s->d_w; s->a.dly = s->d_dly;
+    s->a.ctl = s->d_ctl; s->a.bypass = s->bypass; s->a.inject_thr = s->inject_thr;
+    s->prepared = true;
+    configure_launch(s);
+    return NG_OK;
+}
+
+int32_t ng_set_state(ng_sim* s, int32_t field, const void* data, int64_t count, int64_t first) {
+    if (!s || !data) return NG_ERR_INVALID_ARG;
+    if (!s->prepared) return fail(s, NG_ERR_STATE, "ng_set_state before ng_prepare");
+    NG_CUDA(s, cudaSetDevice(s->cfg.device));
+    if (field == NG_FIELD_STEP) {
+        if (count != 1 || first != 0) return fail(s, NG_ERR_INVALID_ARG, "NG_FIELD_STEP is one int64");
+        long long n = 0;
+        NG_CUDA(s, cudaMemcpy(&n, data, 8, cudaMemcpyDefault));
+        if (n < 0) return fail(s, NG_ERR_INVALID_ARG, "negative step");
+        Ctl h{};
+        int32_t rc = read_ctl(s, &h);
+        if (rc) return rc;
+        const unsigned long long recorded = h.rec_total[h.step_u & 1];
+        h.step_u = n; h.step_d = n; h.spike_cnt[0] = h.spike_cnt[1] = 0;
+        h.rec_total[0] = h.rec_total[1] = recorded;
+        NG_CUDA(s, cudaMemcpyAsync(s->d_ctl, &h, sizeof(Ctl), cudaMemcpyHostToDevice, s->stream));
+        NG_CUDA(s, cudaStreamSynchronize(s->stream));
+        return NG_OK;
+    }
+    if (field == NG_FIELD_LAST_INPUT) return fail(s, NG_ERR_INVALID_ARG, "NG_FIELD_LAST_INPUT is read-only");
+    void* base; size_t elem; int64_t len;
+    int32_t rc = field_info(s, field, &base, &elem, &len);
+    if (rc) return rc;
+    if (count < 0 || first < 0 || first + count > len) return fail(s, NG_ERR_INVALID_ARG, "range outside the field");
+    NG_CUDA(s, cudaMemcpyAsync((char*)base + first * elem, data, (size_t)count * elem, cudaMemcpyDefault, s->stream));
+    NG_CUDA(s, cudaStreamSynchronize(s->stream));
+    return NG_OK;
+}
+
+int32_t ng_get_state(ng_sim* s, int32_t field, void* out, int64_t count, int64_t first) {
+    if (!s || !out) return NG_ERR_INVALID_ARG;
+    if (!s->prepared) return fail(s, NG_ERR_STATE, "ng_get_state before ng_prepare");
+    NG_CUDA(s, cudaSetDevice(s->cfg.device));
+    if (field == NG_FIELD_STEP) {
+        if (count != 1 || first != 0) return fail(s, NG_ERR_INVALID_ARG, "NG_FIELD_STEP is one int64");
+        Ctl h{};
+        int32_t rc = read_ctl(s, &h);
+        if (rc) return rc;
+        long long n = h.step_u;
+        NG_CUDA(s, cudaMemcpy(out, &n, 8, cudaMemcpyDefault));
+        return NG_OK;
+    }
+    void* base; size_t elem; int64_t len;
+    int32_t rc = field_info(s, field, &base, &elem, &len);
+    if (rc) return rc;
+    if (count < 0 || first < 0 || first + count > len) return fail(s, NG_ERR_INVALID_ARG, "range outside the field");
+    NG_CUDA(s, cudaMemcpyAsync(out, (char*)base + first * elem, (size_t)count * elem, cudaMemcpyDefault, s->stream));
+    NG_CUDA(s, cudaStreamSynchronize(s->stream));
+    return NG_OK;
+}
+
+int32_t ng_simulate(ng_sim* s, int64_t n_steps) {
+    if (!s) return NG_ERR_INVALID_ARG;
+    if (n_steps < 0) return fail(s, NG_ERR_INVALID_ARG, "n_steps < 0");
+    int32_t rc = ng_prepare(s);
+    if (rc) return rc;
+    NG_CUDA(s, cudaSetDevice(s->cfg.device));
+    if (n_steps == 0) return NG_OK;
+    cudaStream_t st = s->stream;
+    if (s->profile) {
+        // per-kernel device times: events around every launch, read back in batches
+        const int kBatch = 128;
+        std::vector<cudaEvent_t> ev(3 * kBatch);
+        for (auto& e : ev) NG_CUDA(s, cudaEventCreate(&e));
+        for (int64_t done = 0; done < n_steps;) {
+            const int b = (int)std::min<int64_t>(kBatch, n_steps - done);
+            for (int i = 0; i < b; ++i) {
+                cudaEventRecord(ev[3 * i], st);
+                launch_update(s);
+                cudaEventRecord(ev[3 * i + 1], st);
+                launch_deliver(s);
+                cudaEventRecord(ev[3 * i + 2], st);
+            }
+            NG_CUDA(s, cudaStreamSynchronize(st));
+            for (int i = 0; i < b; ++i) {
+                float m0 = 0, m1 = 0;
+                cudaEventElapsedTime(&m0, ev[3 * i], ev[3 * i + 1]);
+                cudaEventElapsedTime(&m1, ev[3 * i + 1], ev[3 * i + 2]);
+                s->ms_update += m0; s->ms_deliver += m1;
+            }
+            done += b;
+        }
+        for (auto& e : ev) cudaEventDestroy(e);
+        s->launches_update += n_steps; s->launches_deliver += n_steps;
+    } else if (s->step_mode == 2) {
+        long long ns = n_steps;
+        void* args[] = {(void*)&s->a, (void*)&ns};
+        const void* fn = s->delivery_kernel == 2 ? (const void*)persistent_kernel<2> : (const void*)persistent_kernel<1>;
+        NG_CUDA(s, cudaLaunchCooperativeKernel(fn, dim3(s->persistent_blocks), dim3(kUpdateThreads), args, 0, st));
+        s->launches_update += 1;
+    } else if (s->step_mode == 1) {
+        for (int64_t i = 0; i < n_steps; ++i) { launch_update(s); launch_deliver(s); }
+        s->launches_update += n_steps; s->launches_deliver += n_steps;
+    } else {
+        int64_t left = n_steps;
+        const int G = s->steps_per_graph;
+        if (left >= G) {
+            if (!s->graph_exec || s->graph_steps != G) { rc = build_graph(s, G); if (rc) return rc; }
+            while (left >= G) { NG_CUDA(s, cudaGraphLaunch(s->graph_exec, st)); left -= G; }
+        }
+        for (int64_t i = 0; i < left; ++i) { launch_update(s); launch_deliver(s); }
+        s->launches_update += n_steps; s->launches_deliver += n_steps;
+    }
+    NG_CUDA(s, cudaGetLastError());
+    s->steps_done += (uint64_t)n_steps;
+    if (s->async) return NG_OK;
+    NG_CUDA(s, cudaStreamSynchronize(st));
+    if (s->a.rec_cap > 0) {
+        Ctl h{};
+        rc = read_ctl(s, &h);
+        if (rc) return rc;
+        const unsigned long long total = h.rec_total[h.step_u & 1];
+        if (total > (unsigned long long)s->a.rec_cap) return fail(s, NG_ERR_OVERFLOW, "spike record full; later spikes were not recorded");
+    }
+    return NG_OK;
+}
+
+int32_t ng_get_spikes(ng_sim* s, int32_t* steps_host, int32_t* ids_host, int64_t capacity, int64_t* count_out) {
+    if (!s || !count_out || capacity < 0) return NG_ERR_INVALID_ARG;
+    *count_out = 0;
+    if (!s->prepared) return fail(s, NG_ERR_STATE, "ng_get_spikes before ng_prepare");
+    if (s->a.rec_cap <= 0) return fail(s, NG_ERR_STATE, "spike recording is not enabled (NG_RECORD_SPIKES)");
+    NG_CUDA(s, cudaSetDevice(s->cfg.device));
+    Ctl h{};
+    int32_t rc = read_ctl(s, &h);
+    if (rc) return rc;
+    const unsigned long long total = h.rec_total[h.step_u & 1];
+    const int64_t have = (int64_t)std::min<unsigned long long>(total, (unsigned long long)s->a.rec_cap);
+    if (total > (unsigned long long)s->a.rec_cap) s->rec_dropped += total - (unsigned long long)s->a.rec_cap;
+    *count_out = have;
+    const int64_t m = std::min(have, capacity);
+    if (m == 0 || !steps_host || !ids_host) {
+        if (total > (unsigned long long)s->a.rec_cap) {       // forget the uncounted tail so it is not double-counted
+            h.rec_total[0] = h.rec_total[1] = (unsigned long long)have;
+            NG_CUDA(s, cudaMemcpy(s->d_ctl, &h, sizeof(Ctl), cudaMemcpyHostToDevice));
+        }
+        return NG_OK;
+    }
+    NG_CUDA(s, cudaMemcpy(steps_host, s->a.rec_step, (size_t)m * 4, cudaMemcpyDeviceToHost));
+    NG_CUDA(s, cudaMemcpy(ids_host, s->a.rec_id, (size_t)m * 4, cudaMemcpyDeviceToHost));
+    const int64_t rest = have - m;
+    if (rest > 0) {                                           // partial drain: move the tail to the front via scratch
+        int32_t* tmp = nullptr;
+        if (!dev_alloc_t(s, &tmp, (size_t)rest)) return fail(s, NG_ERR_OOM, "scratch for partial drain");
+        NG_CUDA(s, cudaMemcpy(tmp, s->a.rec_step + m, (size_t)rest * 4, cudaMemcpyDeviceToDevice));
+        NG_CUDA(s, cudaMemcpy(s->a.rec_step, tmp, (size_t)rest * 4, cudaMemcpyDeviceToDevice));
+        NG_CUDA(s, cudaMemcpy(tmp, s->a.rec_id + m, (size_t)rest * 4, cudaMemcpyDeviceToDevice));
+        NG_CUDA(s, cudaMemcpy(s->a.rec_id, tmp, (size_t)rest * 4, cudaMemcpyDeviceToDevice));
+        dev_free(s, tmp);
+    }
+    h.rec_total[0] = h.rec_total[1] = (unsigned long long)rest;
+    NG_CUDA(s, cudaMemcpy(s->d_ctl, &h, sizeof(Ctl), cudaMemcpyHostToDevice));
+    return NG_OK;
+}
+
+int32_t ng_get_last_spikes(ng_sim* s, int32_t* ids_host, int64_t capacity, int64_t* count_out) {
+    if (!s || !count_out || capacity < 0) return NG_ERR_INVALID_ARG;
+    *count_out = 0;
+    if (!s->prepared) return fail(s, NG_ERR_STATE, "ng_get_last_spikes before ng_prepare");
+    NG_CUDA(s, cudaSetDevice(s->cfg.device));
+    Ctl h{};
+    int32_t rc = read_ctl(s, &h);
+    if (rc) return rc;
+    if (h.step_u == 0) return NG_OK;
+    const long long n = h.step_u - 1;
+    // spike_cnt[n&1] is cleared only by deliver(n+1); after deliver(n) it still holds step n's count
+    const int64_t M = h.spike_cnt[n & 1];
+    *count_out = M;
+    const int64_t m = std::min(M, capacity);
+    if (m > 0 && ids_host)
+        NG_CUDA(s, cudaMemcpy(ids_host, s->a.spike_list + (size_t)(n & 1) * s->N, (size_t)m * 4, cudaMemcpyDeviceToHost));
+    return NG_OK;
+}
+
+int32_t ng_copy_row_offsets(ng_sim* s, int64_t* out) {
+    if (!s || !out) return NG_ERR_INVALID_ARG;
+    if (!s->prepared) return fail(s, NG_ERR_STATE, "before ng_prepare");
+    NG_CUDA(s, cudaMemcpy(out, s->d_row_off, ((size_t)s->N + 1) * 8, cudaMemcpyDefault));
+    return NG_OK;
+}
+int32_t ng_copy_group_offsets(ng_sim* s, uint32_t* out) {
+    if (!s || !out) return NG_ERR_INVALID_ARG;
+    if (!s->prepared) return fail(s, NG_ERR_STATE, "before ng_prepare");
+    NG_CUDA(s, cudaMemcpy(out, s->d_grp_rel, (size_t)s->N * (s->cfg.ring_slots + 1) * 4, cudaMemcpyDefault));
+    return NG_OK;
+}
+int32_t ng_copy_records(ng_sim* s, int64_t first, int64_t count, int32_t* tgt, float* w, uint8_t* delay) {
+    if (!s) return NG_ERR_INVALID_ARG;
+    if (!s->prepared) return fail(s, NG_ERR_STATE, "before ng_prepare");
+    if (first < 0 || count < 0 || first + count > s->n_padded) return fail(s, NG_ERR_INVALID_ARG, "record range");
+    if (count == 0) return NG_OK;
+    if (tgt) NG_CUDA(s, cudaMemcpy(tgt, s->d_tgt + first, (size_t)count * 4, cudaMemcpyDefault));
+    if (w) NG_CUDA(s, cudaMemcpy(w, s->d_w + first, (size_t)count * 4, cudaMemcpyDefault));
+    if (delay) NG_CUDA(s, cudaMemcpy(delay, s->d_dly + first, (size_t)count, cudaMemcpyDefault));
+    return NG_OK;
+}
+
+int32_t ng_get_connections(ng_sim* s, int32_t src_id, int32_t* tgt_host, float* w_host, uint8_t* delay_host, int64_t capacity,
+                           int64_t* count_out) {
+    if (!s || !count_out || capacity < 0) return NG_ERR_INVALID_ARG;
+    *count_out = 0;
+    if (!s->prepared) return fail(s, NG_ERR_STATE, "before ng_prepare");
+    if (src_id < 0 || src_id >= s->N) return fail(s, NG_ERR_INVALID_ARG, "source id");
+    long long off = 0; uint32_t deg = 0;
+    NG_CUDA(s, cudaMemcpy(&off, s->d_row_off + src_id, 8, cudaMemcpyDeviceToHost));
+    NG_CUDA(s, cudaMemcpy(&deg, s->d_grp_rel + (size_t)src_id * (s->cfg.ring_slots + 1) + s->cfg.ring_slots, 4, cudaMemcpyDeviceToHost));
+    *count_out = deg;
+    const int64_t m = std::min<int64_t>(deg, capacity);
+    if (m == 0) return NG_OK;
+    if (tgt_host) NG_CUDA(s, cudaMemcpy(tgt_host, s->d_tgt + off, (size_t)m * 4, cudaMemcpyDeviceToHost));
+    if (w_host) NG_CUDA(s, cudaMemcpy(w_host, s->d_w + off, (size_t)m * 4, cudaMemcpyDeviceToHost));
+    if (delay_host) NG_CUDA(s, cudaMemcpy(delay_host, s->d_dly + off, (size_t)m, cudaMemcpyDeviceToHost));
+    return NG_OK;
+}
+
+int32_t ng_get_stats(ng_sim* s, ng_stats* out) {
+    if (!s || !out) return NG_ERR_INVALID_ARG;
+    std::memset(out, 0, sizeof(*out));
+    out->n_neurons = s->N;
+    out->step_mode = s->step_mode;
+    if (!s->prepared) return NG_OK;
+    NG_CUDA(s, cudaSetDevice(s->cfg.device));
+    Ctl h{};
+    int32_t rc = read_ctl(s, &h);
+    if (rc) return rc;
+    out->steps = s->steps_done; out->spikes = h.spikes; out->events = h.events;
+    const unsigned long long total = h.rec_total[h.step_u & 1];
+    out->recorded_dropped = s->rec_dropped + (s->a.rec_cap > 0 && total > (unsigned long long)s->a.rec_cap ? total - s->a.rec_cap : 0);
+    out->n_connections = s->S; out->n_records_padded = s->n_padded; out->max_row_records = s->max_row_records;
+    out->build_ms = s->build_ms; out->ms_update = s->ms_update; out->ms_deliver = s->ms_deliver;
+    out->launches_update = s->launches_update; out->launches_deliver = s->launches_deliver; out->launches_other = s->launches_other;
+    out->delivery_kernel = s->delivery_kernel;
+    return NG_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,530 @@
+// =====================================================================================
+// ng_device.cuh — device code of libng.so (sm_100a): Philox, samplers, connection builder,
+// fused LIF + Poisson neuron update with spike collection, spike delivery.
+// Shares nothing with oracle/ (test infrastructure).  Citations are PAPER.md lines and the
+// readings C1..C20 of DESIGN.md.
+// =====================================================================================
+#pragma once
+#include <cooperative_groups.h>
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace ng {
+namespace cg = cooperative_groups;
+
+// counter word 3 of the Philox stream (C1)
+enum : uint32_t { kTagConn = 1, kTagPoisson = 2, kTagInject = 3 };
+enum : int32_t { kRuleIndegree = 0, kRuleOutdegree = 1 };
+enum : int32_t { kDistConst = 0, kDistNormalClipped = 1, kDistUniformInt = 2 };
+
+constexpr int kMaxPoissonTable = 64;
+constexpr int kUpdateThreads = 256;
+constexpr int kDeliverThreads = 256;
+constexpr int kChunkRecords = 128;   // records one warp consumes per iteration of the row walk: 32 lanes x 4
+
+struct DistDev { int32_t kind; int32_t pad; double a, b, lo, hi; };
+
+struct CallDev {               // one ng_connect_* call
+    int32_t rule, src_first, src_n, tgt_first, tgt_n, K;
+    int32_t call_index, pad;
+    DistDev w, d;
+};
+
+struct PopDev {                // per-population constants of the update (fp32 copies of fp64 host values)
+    float P11, P22, P21, P20Ie;            // exact-integration propagators; P20Ie = P20 * I_e
+    float E_L, V_th, V_reset, w_ext;
+    int32_t refr_steps, n_T;
+    uint32_t T[kMaxPoissonTable];          // integer Poisson CDF table (C7)
+};
+
+struct Ctl {                   // device-resident control block; see ng.cu for the update/deliver handshake
+    long long step_u;                      // written by deliver, read by update: index of the next step
+    long long step_d;                      // written by update, read by deliver: index of the step being delivered
+    int32_t spike_cnt[2];                  // length of spike_list[parity]
+    unsigned long long rec_total[2];       // spikes recorded before step of this parity
+    unsigned long long spikes, events;
+    int32_t err_delay;                     // builder: a drawn delay fell outside [1, D]
+    int32_t max_row_records;               // builder: longest padded row
+    unsigned long long n_padded;           // builder: total records stored
+};
+
+// ---------------------------------------------------------------------------------------
+// Philox4x32-10 (Salmon et al., SC'11).  key = 64-bit seed (lo, hi), C1.
+// ---------------------------------------------------------------------------------------
+__device__ __forceinline__ uint4 philox4x32_10(uint32_t k0, uint32_t k1, uint32_t c0, uint32_t c1, uint32_t c2,
+                                               uint32_t c3) {
+    constexpr uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u, W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t hi0 = __umulhi(M0, c0), lo0 = M0 * c0;
+        const uint32_t hi1 = __umulhi(M1, c2), lo1 = M1 * c2;
+        const uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+        k0 += W0; k1 += W1;
+    }
+    return make_uint4(c0, c1, c2, c3);
+}
+
+__device__ __forceinline__ int32_t mulhi_range(uint32_t x, uint32_t n) {   // DESIGN.md C2
+    return (int32_t)__umulhi(x, n);
+}
+
+// One connection draw, a pure function of (seed, call, endpoint, k) — DESIGN.md C1-C5.
+// Every fp64 operation is an explicitly rounded intrinsic so no FMA contraction can change a bit.
+struct Draw { int32_t src, tgt, delay; float w; };
+
+template <bool kNeedWeight>
+__device__ __forceinline__ Draw draw_connection(const CallDev& c, uint32_t seed_lo, uint32_t seed_hi, int32_t endpoint,
+                                                int32_t k) {
+    const uint4 x = philox4x32_10(seed_lo, seed_hi, (uint32_t)k, (uint32_t)endpoint, (uint32_t)c.call_index, kTagConn);
+    Draw out;
+    if (c.rule == kRuleIndegree) {
+        out.tgt = endpoint;
+        out.src = c.src_first + mulhi_range(x.x, (uint32_t)c.src_n);
+    } else {
+        out.src = endpoint;
+        out.tgt = c.tgt_first + mulhi_range(x.x, (uint32_t)c.tgt_n);
+    }
+    double z_w = 0.0, z_d = 0.0;
+    const bool normal_w = kNeedWeight && c.w.kind == kDistNormalClipped;
+    const bool normal_d = c.d.kind == kDistNormalClipped;
+    if (normal_w || normal_d) {                                          // C4: fp64 Box-Muller from (x1, x2)
+        const double u1 = __dmul_rn(__dadd_rn((double)x.y, 0.5), 1.0 / 4294967296.0);
+        const double u2 = __dmul_rn(__dadd_rn((double)x.z, 0.5), 1.0 / 4294967296.0);
+        const double r = sqrt(__dmul_rn(-2.0, log(u1)));
+        const double a = __dmul_rn(6.283185307179586476925286766559, u2);
+        double sa, ca;
+        sincos(a, &sa, &ca);
+        z_w = __dmul_rn(r, ca);
+        z_d = __dmul_rn(r, sa);
+    }
+    out.w = 0.f;
+    if (kNeedWeight) {
+        double w;
+        if (c.w.kind == kDistConst) w = c.w.a;
+        else if (c.w.kind == kDistNormalClipped) {
+            w = __dadd_rn(c.w.a, __dmul_rn(c.w.b, z_w));
+            if (w < c.w.lo) w = c.w.lo;
+            if (w > c.w.hi) w = c.w.hi;
+        } else {
+            const double span = __dadd_rn(__dsub_rn(c.w.hi, c.w.lo), 1.0);
+            w = __dadd_rn(c.w.lo, (double)(((uint64_t)x.w * (uint64_t)span) >> 32));
+        }
+        out.w = (float)w;                                                // the record stores fp32
+    }
+    long long d;
+    if (c.d.kind == kDistConst) d = (long long)c.d.a;
+    else if (c.d.kind == kDistUniformInt) {                              // C5
+        const uint64_t span = (uint64_t)((long long)c.d.hi - (long long)c.d.lo + 1);
+        d = (long long)c.d.lo + (long long)(((uint64_t)x.w * span) >> 32);
+    } else {                                                             // C5: round half up, then clip
+        double f = floor(__dadd_rn(__dadd_rn(c.d.a, __dmul_rn(c.d.b, z_d)), 0.5));
+        if (f < c.d.lo) f = c.d.lo;
+        if (f > c.d.hi) f = c.d.hi;
+        d = (long long)f;
+    }
+    out.delay = (int32_t)d;
+    return out;
+}
+
+// ---------------------------------------------------------------------------------------
+// a0. Connection builder (PAPER.md:37 rules, built in GPU memory as PAPER.md:292 proposes).
+//   pass 1  count records per (source, delay)                    build_count_kernel
+//           row lengths (padded to 4), exclusive scan            build_rowlen_kernel, scan kernels
+//           group offsets inside each row                        build_groups_kernel
+//   pass 2  regenerate every draw and scatter it into its group  build_fill_kernel
+// The rows come out source-major with groups of equal delay in increasing delay order — the
+// layout of PAPER.md:69 / Fig. 1(a).
+// ---------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+build_count_kernel(const CallDev* __restrict__ calls, int call_idx, uint32_t seed_lo, uint32_t seed_hi, int D,
+                   uint32_t* __restrict__ cnt, Ctl* __restrict__ ctl) {
+    const CallDev c = calls[call_idx];
+    const int32_t e_first = c.rule == kRuleIndegree ? c.tgt_first : c.src_first;
+    const int32_t e_n = c.rule == kRuleIndegree ? c.tgt_n : c.src_n;
+    const long long total = (long long)e_n * c.K;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += stride) {
+        const int32_t e = e_first + (int32_t)(idx / c.K);
+        const int32_t k = (int32_t)(idx % c.K);
+        const Draw dr = draw_connection<false>(c, seed_lo, seed_hi, e, k);
+        if (dr.delay < 1 || dr.delay > D) { ctl->err_delay = 1; continue; }
+        atomicAdd(&cnt[(size_t)dr.src * D + (dr.delay - 1)], 1u);
+    }
+}
+
+// row_len[j] = out-degree of j padded to a multiple of 4 records (so every row starts 16-byte aligned
+// in the tgt / w arrays and can be read with 128-bit loads)
+__global__ void build_rowlen_kernel(const uint32_t* __restrict__ cnt, int N, int D, long long* __restrict__ row_len,
+                                    Ctl* __restrict__ ctl) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    int len = 0;
+    if (j < N) {
+        for (int d = 0; d < D; ++d) len += (int)cnt[(size_t)j * D + d];
+        len = (len + 3) & ~3;
+        row_len[j] = len;
+    }
+    // block max -> one atomic per block
+    __shared__ int smax;
+    if (threadIdx.x == 0) smax = 0;
+    __syncthreads();
+    atomicMax(&smax, len);
+    __syncthreads();
+    if (threadIdx.x == 0) atomicMax(&ctl->max_row_records, smax);
+}
+
+// Exclusive scan of int64 values, one CTA of 1024 threads walking the array tile by tile.  N <= a few 1e6
+// and this runs once, so a single-CTA scan is simple and fast enough (~1 ms at N = 1e6).
+__global__ void __launch_bounds__(1024)
+scan_exclusive_kernel(const long long* __restrict__ in, long long* __restrict__ out, int N, Ctl* __restrict__ ctl) {
+    __shared__ long long warp_sum[32];
+    __shared__ long long carry_s;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    if (threadIdx.x == 0) carry_s = 0;
+    __syncthreads();
+    for (int base = 0; base < N; base += 1024) {
+        const int i = base + threadIdx.x;
+        const long long v = i < N ? in[i] : 0;
+        long long x = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const long long y = __shfl_up_sync(0xffffffffu, x, o);
+            if (lane >= o) x += y;
+        }
+        if (lane == 31) warp_sum[wid] = x;
+        __syncthreads();
+        if (wid == 0) {
+            long long s = warp_sum[lane];
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const long long y = __shfl_up_sync(0xffffffffu, s, o);
+                if (lane >= o) s += y;
+            }
+            warp_sum[lane] = s;
+        }
+        __syncthreads();
+        const long long carry = carry_s;
+        const long long incl = x + (wid > 0 ? warp_sum[wid - 1] : 0) + carry;
+        if (i < N) out[i] = incl - v;
+        __syncthreads();
+        if (threadIdx.x == 1023) carry_s = incl;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) { out[N] = carry_s; ctl->n_padded = (unsigned long long)carry_s; }
+}
+
+// grp_rel[j*(D+1) + d] = offset inside row j of the first record with delay d+1; entry D = out-degree.
+// Also clears cnt so that pass 2 can use it as the per-group fill cursor.
+__global__ void build_groups_kernel(uint32_t* __restrict__ cnt, int N, int D, uint32_t* __restrict__ grp_rel) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= N) return;
+    uint32_t run = 0;
+    for (int d = 0; d < D; ++d) {
+        grp_rel[(size_t)j * (D + 1) + d] = run;
+        run += cnt[(size_t)j * D + d];
+        cnt[(size_t)j * D + d] = 0;
+    }
+    grp_rel[(size_t)j * (D + 1) + D] = run;
+}
+
+__global__ void __launch_bounds__(256)
+build_fill_kernel(const CallDev* __restrict__ calls, int call_idx, uint32_t seed_lo, uint32_t seed_hi, int D,
+                  uint32_t* __restrict__ cursor, const long long* __restrict__ row_off,
+                  const uint32_t* __restrict__ grp_rel, int32_t* __restrict__ tgt, float* __restrict__ w,
+                  uint8_t* __restrict__ dly) {
+    const CallDev c = calls[call_idx];
+    const int32_t e_first = c.rule == kRuleIndegree ? c.tgt_first : c.src_first;
+    const int32_t e_n = c.rule == kRuleIndegree ? c.tgt_n : c.src_n;
+    const long long total = (long long)e_n * c.K;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += stride) {
+        const int32_t e = e_first + (int32_t)(idx / c.K);
+        const int32_t k = (int32_t)(idx % c.K);
+        const Draw dr = draw_connection<true>(c, seed_lo, seed_hi, e, k);
+        if (dr.delay < 1 || dr.delay > D) continue;
+        const uint32_t p = atomicAdd(&cursor[(size_t)dr.src * D + (dr.delay - 1)], 1u);
+        const long long pos = row_off[dr.src] + grp_rel[(size_t)dr.src * (D + 1) + (dr.delay - 1)] + p;
+        tgt[pos] = dr.tgt;
+        w[pos] = dr.w;
+        dly[pos] = (uint8_t)dr.delay;
+    }
+}
+
+// Order the records of every (source, delay) group by (target, weight bits): the fill order above depends on
+// atomic arrival order; after this pass the structure is a deterministic function of the seed.
+// One warp per group; groups are short (1..~1e3 records), so an in-place odd-even transposition over
+// lane-strided elements is enough.  Groups longer than kSortMax records are left as filled.
+constexpr int kSortMax = 768;    // 8 warps x 768 x 8 B = 48 KB of static shared memory
+__global__ void __launch_bounds__(256)
+build_sort_groups_kernel(int N, int D, const long long* __restrict__ row_off, const uint32_t* __restrict__ grp_rel,
+                         int32_t* __restrict__ tgt, float* __restrict__ w) {
+    __shared__ unsigned long long keys[8][kSortMax];
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const long long n_groups = (long long)N * D;
+    const long long warps = ((long long)gridDim.x * blockDim.x) >> 5;
+    for (long long g = (((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5); g < n_groups; g += warps) {
+        const int j = (int)(g / D), d = (int)(g % D);
+        const uint32_t a = grp_rel[(size_t)j * (D + 1) + d], b = grp_rel[(size_t)j * (D + 1) + d + 1];
+        const int len = (int)(b - a);
+        if (len < 2 || len > kSortMax) continue;
+        const long long base = row_off[j] + a;
+        unsigned long long* K = keys[wib];
+        for (int i = lane; i < len; i += 32)
+            K[i] = ((unsigned long long)(uint32_t)tgt[base + i] << 32) | (unsigned long long)__float_as_uint(w[base + i]);
+        __syncwarp();
+        for (int pass = 0; pass < len; ++pass) {
+            for (int i = (pass & 1) + 2 * lane; i + 1 < len; i += 64) {
+                const unsigned long long x = K[i], y = K[i + 1];
+                if (x > y) { K[i] = y; K[i + 1] = x; }
+            }
+            __syncwarp();
+        }
+        for (int i = lane; i < len; i += 32) {
+            tgt[base + i] = (int32_t)(uint32_t)(K[i] >> 32);
+            w[base + i] = __uint_as_float((uint32_t)K[i]);
+        }
+        __syncwarp();
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// Warp-aggregated append to the spike array (Fig. 1b: "the spike is sent to the spike
+// array"; its maximum size is the number of nodes).  One atomicAdd per warp that holds a spike.
+// Every lane of the warp must call this.
+// ---------------------------------------------------------------------------------------
+__device__ __forceinline__ void append_spike(bool spk, int32_t id, int32_t* __restrict__ list, int32_t* cnt) {
+    const unsigned m = __ballot_sync(0xffffffffu, spk);
+    if (m == 0) return;
+    const int lane = threadIdx.x & 31;
+    const int leader = __ffs(m) - 1;
+    int base = 0;
+    if (lane == leader) base = atomicAdd(cnt, __popc(m));
+    base = __shfl_sync(0xffffffffu, base, leader);
+    if (spk) list[base + __popc(m & ((1u << lane) - 1u))] = id;
+}
+
+struct StepArgs {
+    int32_t N, D;
+    uint32_t seed_lo, seed_hi;
+    // neuron state (SoA) and parameters
+    float* V; float* I; int32_t* refr; const uint8_t* pop_of; const PopDev* pops;
+    float* ring;                 // [D][N] slot-major
+    float* last_input;           // [N] or nullptr (NG_DEBUG_INPUT)
+    // spike array, double-buffered by step parity, and the spike record
+    int32_t* spike_list;         // [2][N]
+    int32_t* rec_step; int32_t* rec_id; long long rec_cap;   // rec_cap = 0: recording off
+    // connection structure
+    const long long* row_off; const uint32_t* grp_rel;
+    const int32_t* tgt; const float* w; const uint8_t* dly;
+    Ctl* ctl;
+    int32_t bypass; uint32_t inject_thr;
+    int32_t max_row_chunks;      // ceil(longest padded row / kChunkRecords)
+};
+
+// ---------------------------------------------------------------------------------------
+// a1 + a2. Neuron update fused with the Poisson drive and spike collection — one thread per neuron.
+//   PAPER.md:93-102 Eqs. (1)-(2), exact integration PAPER.md:37; order of operations DESIGN.md C11:
+//     in  = ring[n mod D][i], slot cleared                                       (C9)
+//     k   ~ Poisson(lambda_pop) from Philox(seed; i, n, POISSON)                 (C7)
+//     V  <- E_L + P22 (V - E_L) + P21 I + P20 I_e    if not refractory, else refr--
+//     I  <- P11 I + in + w_ext k
+//     V >= V_th: spike, V <- V_reset, refr <- t_ref/h
+// `gtid`/`gthreads` let the same body serve the stand-alone kernel and the persistent kernel.
+// ---------------------------------------------------------------------------------------
+__device__ __forceinline__ void update_phase(const StepArgs& a, long long n, long long gtid, long long gthreads) {
+    const int N = a.N;
+    const int slot = (int)(n % a.D);
+    float* __restrict__ plane = a.ring + (size_t)slot * N;
+    int32_t* __restrict__ list = a.spike_list + (size_t)(n & 1) * N;
+    int32_t* cnt = &a.ctl->spike_cnt[n & 1];
+    const long long n_round = ((long long)N + 31) & ~31LL;      // keep warps whole for the ballot
+    for (long long ii = gtid; ii < n_round; ii += gthreads) {
+        const int i = (int)ii;
+        bool spk = false;
+        if (i < N) {
+            const float in = __ldcg(plane + i);      // written by red.global from other SMs: read at L2
+            plane[i] = 0.f;
+            if (a.last_input) a.last_input[i] = in;
+            if (a.bypass) {                                      // DESIGN.md C8: delivery-only mode
+                const uint4 x = philox4x32_10(a.seed_lo, a.seed_hi, (uint32_t)i, (uint32_t)n, (uint32_t)(n >> 32), kTagInject);
+                spk = x.x < a.inject_thr;
+            } else {
+                const PopDev* __restrict__ p = a.pops + a.pop_of[i];
+                int k = 0;
+                const int nT = p->n_T;
+                if (nT > 0) {
+                    const uint4 x = philox4x32_10(a.seed_lo, a.seed_hi, (uint32_t)i, (uint32_t)n, (uint32_t)(n >> 32), kTagPoisson);
+                    while (k < nT && x.x >= __ldg(&p->T[k])) ++k;   // T is non-decreasing: k = #{m : x0 >= T[m]}
+                }
+                float V = a.V[i], I = a.I[i];
+                int r = a.refr[i];
+                const float E_L = p->E_L;
+                if (r == 0) V = E_L + fmaf(p->P22, V - E_L, fmaf(p->P21, I, p->P20Ie));
+                else r -= 1;
+                I = fmaf(p->P11, I, in) + p->w_ext * (float)k;
+                if (V >= p->V_th) { spk = true; V = p->V_reset; r = p->refr_steps; }
+                a.V[i] = V; a.I[i] = I; a.refr[i] = r;
+            }
+        }
+        append_spike(spk, i, list, cnt);
+    }
+    if (gtid == 0) a.ctl->step_d = n;
+}
+
+__device__ __forceinline__ void red_add_f32(float* addr, float v) {
+    asm volatile("red.global.add.f32 [%0], %1;" ::"l"(addr), "f"(v) : "memory");
+}
+__device__ __forceinline__ int4 ld_stream_s32x4(const int32_t* p) {
+    int4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.s32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ float4 ld_stream_f32x4(const float* p) {
+    float4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];"
+                 : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ uint32_t ld_stream_u32(const void* p) {
+    uint32_t r;
+    asm volatile("ld.global.nc.L1::no_allocate.u32 %0, [%1];" : "=r"(r) : "l"(p));
+    return r;
+}
+
+// Step bookkeeping shared by both delivery kernels (a4): one thread publishes the next step index, clears the
+// other parity's spike counter and advances the record cursor; all threads copy the spike array into the
+// spike record (a2, "all spike times of all neurons recorded").
+__device__ __forceinline__ void bookkeeping_phase(const StepArgs& a, long long n, int M, long long gtid, long long gthreads) {
+    const unsigned long long rec_base = __ldcg(&a.ctl->rec_total[n & 1]);
+    if (a.rec_cap > 0) {
+        const int32_t* __restrict__ list = a.spike_list + (size_t)(n & 1) * a.N;
+        for (long long i = gtid; i < M; i += gthreads) {
+            const unsigned long long pos = rec_base + (unsigned long long)i;
+            if (pos < (unsigned long long)a.rec_cap) { a.rec_id[pos] = __ldcg(list + i); a.rec_step[pos] = (int32_t)n; }
+        }
+    }
+    if (gtid == 0) {
+        a.ctl->rec_total[(n + 1) & 1] = rec_base + (unsigned long long)M;
+        a.ctl->spike_cnt[(n + 1) & 1] = 0;
+        a.ctl->spikes += (unsigned long long)M;
+        a.ctl->step_u = n + 1;
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// a3. Spike delivery, kernel 1: row-chunk walk.
+//   work item = (spike index i, chunk c of kChunkRecords records of row(spike i)), chunk fastest, one warp per
+//   item; lane l reads records [4l, 4l+4) of the chunk with one 128-bit load of targets, one of weights and one
+//   32-bit load of delays, then issues up to four red.global.add.f32 into ring[(n + d) mod D][target].
+//   Rows are delay-grouped, so consecutive records mostly hit the same ring plane.
+// ---------------------------------------------------------------------------------------
+__device__ __forceinline__ void deliver_rows_phase(const StepArgs& a, long long n, int M, long long gwarp, long long gwarps,
+                                                   int lane) {
+    const int N = a.N, D = a.D;
+    const int nmod = (int)(n % D);
+    const int32_t* __restrict__ list = a.spike_list + (size_t)(n & 1) * N;
+    const int chunks = a.max_row_chunks;
+    const long long items = (long long)M * chunks;
+    unsigned long long ev = 0;
+    for (long long it = gwarp; it < items; it += gwarps) {
+        const int si = (int)(it / chunks), c = (int)(it % chunks);
+        const int j = __ldcg(list + si);
+        const long long r0 = a.row_off[j], r1 = a.row_off[j + 1];
+        if (c == 0 && lane == 0) ev += a.grp_rel[(size_t)j * (D + 1) + D];
+        const long long p = r0 + (long long)c * kChunkRecords + lane * 4;
+        if (p < r1) {
+            const int4 t = ld_stream_s32x4(a.tgt + p);
+            const float4 ww = ld_stream_f32x4(a.w + p);
+            const uint32_t dd = ld_stream_u32(a.dly + p);
+            int s;
+            if (t.x >= 0) { s = nmod + (int)(dd & 0xff); if (s >= D) s -= D; red_add_f32(a.ring + (size_t)s * N + t.x, ww.x); }
+            if (t.y >= 0) { s = nmod + (int)((dd >> 8) & 0xff); if (s >= D) s -= D; red_add_f32(a.ring + (size_t)s * N + t.y, ww.y); }
+            if (t.z >= 0) { s = nmod + (int)((dd >> 16) & 0xff); if (s >= D) s -= D; red_add_f32(a.ring + (size_t)s * N + t.z, ww.z); }
+            if (t.w >= 0) { s = nmod + (int)(dd >> 24); if (s >= D) s -= D; red_add_f32(a.ring + (size_t)s * N + t.w, ww.w); }
+        }
+    }
+    if (ev) atomicAdd(&a.ctl->events, ev);
+}
+
+// ---------------------------------------------------------------------------------------
+// a3. Spike delivery, kernel 2: delay-major segment walk.
+//   work item = (delay d, spike index i), spike fastest, one warp per (source, delay-group) segment: all warps
+//   running at one time add into the same one or two ring planes (N*4 bytes each), which keeps the reduction
+//   target L2-resident when the whole ring (D*N*4 bytes) is larger than L2.  The delay comes from the group
+//   table, so a record costs 8 bytes of reads.  Segments are walked with 128-bit loads from the first 4-aligned
+//   record at or below the segment start; records outside [start, end) are masked.
+// ---------------------------------------------------------------------------------------
+__device__ __forceinline__ void deliver_groups_phase(const StepArgs& a, long long n, int M, long long gwarp, long long gwarps,
+                                                     int lane) {
+    const int N = a.N, D = a.D;
+    const int nmod = (int)(n % D);
+    const int32_t* __restrict__ list = a.spike_list + (size_t)(n & 1) * N;
+    const long long items = (long long)M * D;
+    unsigned long long ev = 0;
+    for (long long it = gwarp; it < items; it += gwarps) {
+        const int d = (int)(it / M), si = (int)(it % M);          // d = delay - 1
+        const int j = __ldcg(list + si);
+        const uint32_t* __restrict__ g = a.grp_rel + (size_t)j * (D + 1);
+        const uint32_t ga = g[d], gb = g[d + 1];
+        if (d == 0 && lane == 0) ev += g[D];
+        if (ga == gb) continue;
+        int s = nmod + d + 1; if (s >= D) s -= D;
+        float* __restrict__ plane = a.ring + (size_t)s * N;
+        const long long r0 = a.row_off[j];
+        const long long lo = r0 + ga, hi = r0 + gb;
+        for (long long p = (lo & ~3LL) + lane * 4; p < hi; p += 128) {
+            const int4 t = ld_stream_s32x4(a.tgt + p);
+            const float4 ww = ld_stream_f32x4(a.w + p);
+            if (p >= lo && p < hi) red_add_f32(plane + t.x, ww.x);
+            if (p + 1 >= lo && p + 1 < hi) red_add_f32(plane + t.y, ww.y);
+            if (p + 2 >= lo && p + 2 < hi) red_add_f32(plane + t.z, ww.z);
+            if (p + 3 >= lo && p + 3 < hi) red_add_f32(plane + t.w, ww.w);
+        }
+    }
+    if (ev) atomicAdd(&a.ctl->events, ev);
+}
+
+// ------------------------------- stand-alone kernels ---------------------------------
+__global__ void __launch_bounds__(kUpdateThreads) update_kernel(const StepArgs a) {
+    const long long n = __ldcg(&a.ctl->step_u);
+    update_phase(a, n, (long long)blockIdx.x * blockDim.x + threadIdx.x, (long long)gridDim.x * blockDim.x);
+}
+
+template <int kKernel>
+__global__ void __launch_bounds__(kDeliverThreads) deliver_kernel(const StepArgs a) {
+    const long long n = __ldcg(&a.ctl->step_d);
+    const int M = __ldcg(&a.ctl->spike_cnt[n & 1]);
+    const long long gtid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long gthreads = (long long)gridDim.x * blockDim.x;
+    if (kKernel == 1) deliver_rows_phase(a, n, M, gtid >> 5, gthreads >> 5, threadIdx.x & 31);
+    else deliver_groups_phase(a, n, M, gtid >> 5, gthreads >> 5, threadIdx.x & 31);
+    bookkeeping_phase(a, n, M, gtid, gthreads);
+}
+
+// One persistent cooperative kernel for n_steps steps: the two phases separated by grid-wide barriers instead of
+// kernel boundaries (the per-step work of the microcircuit is a few microseconds).
+template <int kKernel>
+__global__ void __launch_bounds__(kUpdateThreads) persistent_kernel(const StepArgs a, long long n_steps) {
+    cg::grid_group grid = cg::this_grid();
+    const long long gtid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long gthreads = (long long)gridDim.x * blockDim.x;
+    long long n = __ldcg(&a.ctl->step_u);
+    grid.sync();                                   // everyone has read step_u before anyone moves it
+    for (long long s = 0; s < n_steps; ++s, ++n) {
+        update_phase(a, n, gtid, gthreads);
+        grid.sync();
+        const int M = __ldcg(&a.ctl->spike_cnt[n & 1]);
+        if (kKernel == 1) deliver_rows_phase(a, n, M, gtid >> 5, gthreads >> 5, threadIdx.x & 31);
+        else deliver_groups_phase(a, n, M, gtid >> 5, gthreads >> 5, threadIdx.x & 31);
+        bookkeeping_phase(a, n, M, gtid, gthreads);
+        grid.sync();
+    }
+}
+
+__global__ void fill_pop_of_kernel(uint8_t* pop_of, float* V, int first, int n, uint8_t pop, float E_L) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) { pop_of[first + i] = pop; V[first + i] = E_L; }
+}
+
+}  // namespace ng
