@@ -1,0 +1,306 @@
+"""Thin ctypes binding of libng.so (include/ng.h).  Argument marshalling only: every step of the hot path runs in
+the CUDA kernels behind the C-ABI.  PyTorch supplies device memory (allocator callbacks) and the CUDA stream.
+
+There is no CPU fallback: importing this module loads libng.so and raises if it is missing or cannot be built.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+NG_OK, NG_ERR_INVALID_ARG, NG_ERR_STATE, NG_ERR_OOM, NG_ERR_CUDA, NG_ERR_OVERFLOW = 0, -1, -2, -3, -4, -5
+NG_RECORD_SPIKES, NG_DEBUG_INPUT = 1, 2
+FIELD_V, FIELD_I_SYN, FIELD_REFR, FIELD_RING, FIELD_STEP, FIELD_LAST_INPUT = 0, 1, 2, 3, 4, 5
+DIST_CONST, DIST_NORMAL_CLIPPED, DIST_UNIFORM_INT = 0, 1, 2
+(OPT_STEP_MODE, OPT_STEPS_PER_GRAPH, OPT_DELIVERY_KERNEL, OPT_DELIVER_BLOCKS, OPT_PROFILE, OPT_ASYNC,
+ OPT_SORT_SEGMENTS) = range(7)
+STEP_GRAPH, STEP_LAUNCH, STEP_PERSISTENT = 0, 1, 2
+
+EXPORTS = ["ng_create", "ng_destroy", "ng_last_error", "ng_create_population", "ng_connect_fixed_indegree",
+           "ng_connect_fixed_outdegree", "ng_set_bypass", "ng_set_option", "ng_prepare", "ng_set_state",
+           "ng_get_state", "ng_simulate", "ng_get_spikes", "ng_get_last_spikes", "ng_copy_row_offsets",
+           "ng_copy_group_offsets", "ng_copy_records", "ng_get_connections", "ng_get_stats"]
+
+
+class NgConfig(C.Structure):
+    _fields_ = [("dt_ms", C.c_double), ("ring_slots", C.c_int32), ("flags", C.c_uint32), ("seed", C.c_uint64),
+                ("max_recorded_spikes", C.c_int64), ("device", C.c_int32), ("reserved", C.c_int32)]
+
+
+_ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
+_FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)
+
+
+class NgAllocator(C.Structure):
+    _fields_ = [("alloc", _ALLOC_FN), ("free", _FREE_FN), ("user", C.c_void_p)]
+
+
+class NgLifParams(C.Structure):
+    _fields_ = [(k, C.c_double) for k in
+                ("C_m", "tau_m", "tau_syn", "E_L", "V_th", "V_reset", "t_ref_ms", "I_e",
+                 "poisson_rate_hz", "poisson_weight")]
+
+
+class NgDist(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("pad", C.c_int32), ("a", C.c_double), ("b", C.c_double),
+                ("lo", C.c_double), ("hi", C.c_double)]
+
+
+class NgStats(C.Structure):
+    _fields_ = [("steps", C.c_uint64), ("spikes", C.c_uint64), ("events", C.c_uint64),
+                ("recorded_dropped", C.c_uint64), ("n_neurons", C.c_int64), ("n_connections", C.c_int64),
+                ("n_records_padded", C.c_int64), ("max_row_records", C.c_int64), ("build_ms", C.c_double),
+                ("ms_update", C.c_double), ("ms_deliver", C.c_double), ("launches_update", C.c_uint64),
+                ("launches_deliver", C.c_uint64), ("launches_other", C.c_uint64), ("delivery_kernel", C.c_int32),
+                ("step_mode", C.c_int32)]
+
+
+class NgError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"ng error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def load_library(path: str | None = None):
+    """Load libng.so (building it with nvcc if it is missing or stale).  Raises on failure — no fallback."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    p = path or _build.build_lib()
+    if not os.path.exists(p):
+        raise ImportError(f"libng.so not found at {p}; run `python -m paper_2007_14236_b200.build`")
+    L = C.CDLL(p)
+    vp, i32, i64 = C.c_void_p, C.c_int32, C.c_int64
+    L.ng_create.argtypes = [C.POINTER(NgConfig), C.POINTER(NgAllocator), vp, C.POINTER(vp)]
+    L.ng_destroy.argtypes = [vp]
+    L.ng_last_error.argtypes = [vp]
+    L.ng_last_error.restype = C.c_char_p
+    L.ng_create_population.argtypes = [vp, i32, C.POINTER(NgLifParams), C.POINTER(i32)]
+    for fn in (L.ng_connect_fixed_indegree, L.ng_connect_fixed_outdegree):
+        fn.argtypes = [vp, i32, i32, i32, i32, i32, C.POINTER(NgDist), C.POINTER(NgDist)]
+    L.ng_set_bypass.argtypes = [vp, i32, C.c_double]
+    L.ng_set_option.argtypes = [vp, i32, i64]
+    L.ng_prepare.argtypes = [vp]
+    L.ng_set_state.argtypes = [vp, i32, vp, i64, i64]
+    L.ng_get_state.argtypes = [vp, i32, vp, i64, i64]
+    L.ng_simulate.argtypes = [vp, i64]
+    L.ng_get_spikes.argtypes = [vp, vp, vp, i64, C.POINTER(i64)]
+    L.ng_get_last_spikes.argtypes = [vp, vp, i64, C.POINTER(i64)]
+    L.ng_copy_row_offsets.argtypes = [vp, vp]
+    L.ng_copy_group_offsets.argtypes = [vp, vp]
+    L.ng_copy_records.argtypes = [vp, i64, i64, vp, vp, vp]
+    L.ng_get_connections.argtypes = [vp, i32, vp, vp, vp, i64, C.POINTER(i64)]
+    L.ng_get_stats.argtypes = [vp, C.POINTER(NgStats)]
+    for name in EXPORTS:
+        if name != "ng_last_error":
+            getattr(L, name).restype = i32
+    if path is None:
+        _lib = L
+    return L
+
+
+def _lif(params: dict) -> NgLifParams:
+    return NgLifParams(**{k: float(params.get(k, 0.0)) for k, _ in NgLifParams._fields_})
+
+
+def _dist(d) -> NgDist:
+    """d = ("const", a) | ("normal", mean, sd[, lo, hi]) | ("uniform_int", lo, hi)."""
+    kind = d[0]
+    if kind == "const":
+        return NgDist(DIST_CONST, 0, float(d[1]), 0.0, 0.0, 0.0)
+    if kind == "normal":
+        lo = float(d[3]) if len(d) > 3 else -np.inf
+        hi = float(d[4]) if len(d) > 4 else np.inf
+        return NgDist(DIST_NORMAL_CLIPPED, 0, float(d[1]), float(d[2]), lo, hi)
+    if kind == "uniform_int":
+        return NgDist(DIST_UNIFORM_INT, 0, 0.0, 0.0, float(d[1]), float(d[2]))
+    raise ValueError(kind)
+
+
+def _ptr(x):
+    """Host numpy array or torch tensor (host or device) -> raw address."""
+    if isinstance(x, np.ndarray):
+        assert x.flags["C_CONTIGUOUS"]
+        return x.ctypes.data
+    return x.data_ptr()          # torch tensor
+
+
+class Sim:
+    """One simulator handle.  Method names mirror the C-ABI (ng_ prefix dropped)."""
+
+    def __init__(self, dt_ms: float = 0.1, ring_slots: int = 64, seed: int = 1, record_spikes: bool = True,
+                 max_recorded_spikes: int = 1 << 22, debug_input: bool = False, device: int = 0,
+                 torch_alloc: bool = True):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2007_14236_b200 needs a CUDA device; there is no CPU fallback")
+        self._L = load_library()
+        self._torch = torch
+        self.device = device
+        self.dt_ms, self.D, self.seed = dt_ms, ring_slots, seed
+        self.stream = torch.cuda.Stream(device=device)
+        self._tensors = {}
+        self._alloc_struct = None
+        if torch_alloc:
+            def _alloc(nbytes, _user):
+                try:
+                    t = torch.empty(int(nbytes), dtype=torch.uint8, device=f"cuda:{device}")
+                except Exception:
+                    return None
+                self._tensors[t.data_ptr()] = t
+                return t.data_ptr()
+
+            def _free(ptr, _user):
+                self._tensors.pop(ptr, None)
+
+            self._alloc_cb, self._free_cb = _ALLOC_FN(_alloc), _FREE_FN(_free)
+            self._alloc_struct = NgAllocator(self._alloc_cb, self._free_cb, None)
+        flags = (NG_RECORD_SPIKES if record_spikes else 0) | (NG_DEBUG_INPUT if debug_input else 0)
+        cfg = NgConfig(dt_ms, ring_slots, flags, seed, max_recorded_spikes if record_spikes else 0, device, 0)
+        h = C.c_void_p()
+        rc = self._L.ng_create(C.byref(cfg), C.byref(self._alloc_struct) if self._alloc_struct else None,
+                               C.c_void_p(self.stream.cuda_stream), C.byref(h))
+        if rc != NG_OK:
+            raise NgError(rc, "ng_create failed")
+        self._h = h
+
+    # ---- lifetime -------------------------------------------------------------------------------------------
+    def close(self):
+        if getattr(self, "_h", None):
+            self._L.ng_destroy(self._h)
+            self._h = None
+            self._tensors.clear()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _chk(self, rc, allow=()):
+        if rc != NG_OK and rc not in allow:
+            raise NgError(rc, self._L.ng_last_error(self._h).decode())
+        return rc
+
+    # ---- network description --------------------------------------------------------------------------------
+    def create_population(self, n: int, params: dict) -> int:
+        first = C.c_int32()
+        p = _lif(params)
+        self._chk(self._L.ng_create_population(self._h, n, C.byref(p), C.byref(first)))
+        return first.value
+
+    def connect_fixed_indegree(self, src_first, src_n, tgt_first, tgt_n, K, weight, delay):
+        w, d = _dist(weight), _dist(delay)
+        self._chk(self._L.ng_connect_fixed_indegree(self._h, src_first, src_n, tgt_first, tgt_n, K,
+                                                    C.byref(w), C.byref(d)))
+
+    def connect_fixed_outdegree(self, src_first, src_n, tgt_first, tgt_n, K, weight, delay):
+        w, d = _dist(weight), _dist(delay)
+        self._chk(self._L.ng_connect_fixed_outdegree(self._h, src_first, src_n, tgt_first, tgt_n, K,
+                                                     C.byref(w), C.byref(d)))
+
+    def set_bypass(self, bypass: bool, inject_fraction: float = 0.0):
+        self._chk(self._L.ng_set_bypass(self._h, int(bypass), float(inject_fraction)))
+
+    def set_option(self, option: int, value: int):
+        self._chk(self._L.ng_set_option(self._h, option, int(value)))
+
+    def prepare(self):
+        self._chk(self._L.ng_prepare(self._h))
+
+    # ---- state ----------------------------------------------------------------------------------------------
+    def stats(self) -> NgStats:
+        st = NgStats()
+        self._chk(self._L.ng_get_stats(self._h, C.byref(st)))
+        return st
+
+    @property
+    def n_neurons(self) -> int:
+        return int(self.stats().n_neurons)
+
+    @property
+    def n_connections(self) -> int:
+        return int(self.stats().n_connections)
+
+    def set_state(self, field: int, data, first: int = 0):
+        """data: numpy array or torch tensor (host or device) of the field's element type."""
+        if field == FIELD_STEP:
+            a = np.asarray([data], dtype=np.int64)
+        elif isinstance(data, np.ndarray) or not hasattr(data, "data_ptr"):
+            a = np.ascontiguousarray(data, dtype=np.int32 if field == FIELD_REFR else np.float32)
+        else:
+            a = data.contiguous()
+        n = a.size if isinstance(a, np.ndarray) else a.numel()
+        self._chk(self._L.ng_set_state(self._h, field, _ptr(a), n, first))
+
+    def get_state(self, field: int, n: int | None = None, first: int = 0, out=None):
+        if field == FIELD_STEP:
+            a = np.zeros(1, np.int64)
+            self._chk(self._L.ng_get_state(self._h, field, a.ctypes.data, 1, 0))
+            return int(a[0])
+        if out is None:
+            if n is None:
+                n = self.n_neurons * (self.D if field == FIELD_RING else 1) - first
+            out = np.empty(n, np.int32 if field == FIELD_REFR else np.float32)
+        cnt = out.size if isinstance(out, np.ndarray) else out.numel()
+        self._chk(self._L.ng_get_state(self._h, field, _ptr(out), cnt, first))
+        return out
+
+    # ---- run ------------------------------------------------------------------------------------------------
+    def simulate(self, n_steps: int, allow_overflow: bool = False):
+        return self._chk(self._L.ng_simulate(self._h, n_steps), allow=(NG_ERR_OVERFLOW,) if allow_overflow else ())
+
+    def get_spikes(self, steps_out=None, ids_out=None):
+        """(steps, ids) of every recorded spike as host int32 arrays; drains the device record."""
+        cnt = C.c_int64()
+        self._chk(self._L.ng_get_spikes(self._h, None, None, 0, C.byref(cnt)))
+        n = cnt.value
+        steps = steps_out if steps_out is not None else np.empty(n, np.int32)
+        ids = ids_out if ids_out is not None else np.empty(n, np.int32)
+        cap = min(n, steps.size if isinstance(steps, np.ndarray) else steps.numel())
+        if cap > 0:
+            self._chk(self._L.ng_get_spikes(self._h, _ptr(steps), _ptr(ids), cap, C.byref(cnt)))
+        return steps[:cap], ids[:cap]
+
+    def last_spikes(self) -> np.ndarray:
+        cnt = C.c_int64()
+        self._chk(self._L.ng_get_last_spikes(self._h, None, 0, C.byref(cnt)))
+        ids = np.empty(cnt.value, np.int32)
+        if cnt.value:
+            self._chk(self._L.ng_get_last_spikes(self._h, ids.ctypes.data, cnt.value, C.byref(cnt)))
+        return ids
+
+    # ---- connection structure read-back (parity checks) --------------------------------------------------------
+    def row_offsets(self) -> np.ndarray:
+        out = np.empty(self.n_neurons + 1, np.int64)
+        self._chk(self._L.ng_copy_row_offsets(self._h, out.ctypes.data))
+        return out
+
+    def group_offsets(self) -> np.ndarray:
+        out = np.empty((self.n_neurons, self.D + 1), np.uint32)
+        self._chk(self._L.ng_copy_group_offsets(self._h, out.ctypes.data))
+        return out
+
+    def records(self, first: int = 0, count: int | None = None):
+        if count is None:
+            count = int(self.stats().n_records_padded) - first
+        tgt = np.empty(count, np.int32); w = np.empty(count, np.float32); d = np.empty(count, np.uint8)
+        self._chk(self._L.ng_copy_records(self._h, first, count, tgt.ctypes.data, w.ctypes.data, d.ctypes.data))
+        return tgt, w, d
+
+    def connections_of(self, src_id: int):
+        cnt = C.c_int64()
+        self._chk(self._L.ng_get_connections(self._h, src_id, None, None, None, 0, C.byref(cnt)))
+        n = cnt.value
+        tgt = np.empty(n, np.int32); w = np.empty(n, np.float32); d = np.empty(n, np.uint8)
+        if n:
+            self._chk(self._L.ng_get_connections(self._h, src_id, tgt.ctypes.data, w.ctypes.data, d.ctypes.data, n,
+                                                 C.byref(cnt)))
+        return tgt, w, d

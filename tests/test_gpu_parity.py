@@ -1,0 +1,169 @@
+"""GPU parity tests: the CUDA path (through the C-ABI binding) against the fp64 CPU oracle on the same seeded inputs.
+
+Bars (BASELINE.json north_star):
+  * connectivity and delivery indexing bit-exact (weights: <= 1 fp32 ulp on a handful of records, reading C4)
+  * lockstep: per-step spike lists bit-exact except neurons within 1e-4 mV of threshold (logged, reading C11)
+  * per-step input currents within 1e-5 relative to their L1 mass (reading C12); V within 1e-4 mV
+  * free-running population rates within 5 % (reading C17)
+"""
+import numpy as np
+import pytest
+
+from paper_2007_14236_b200 import workloads as W
+
+from helpers import Shadow, check_structure, make_pair, raw_layout_ok
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2007_14236_b200 import binding
+    return binding
+
+
+def lockstep(o, g, wl, oracle_mod, B, n_steps, check_input=True):
+    """DESIGN.md lockstep protocol.  Returns (near-threshold log, number of spikes compared)."""
+    N, D = o.n_neurons, wl.ring_slots
+    sh = Shadow(o, wl, oracle_mod)
+    log, n_spk = [], 0
+    n0 = o.get_state(oracle_mod.FIELD_STEP)
+    for n in range(n0, n0 + n_steps):
+        V = o.get_state(oracle_mod.FIELD_V); I = o.get_state(oracle_mod.FIELD_I_SYN); R = o.get_state(oracle_mod.FIELD_REFR)
+        V32, I32 = V.astype(np.float32), I.astype(np.float32)
+        g.set_state(B.FIELD_V, V32); g.set_state(B.FIELD_I_SYN, I32); g.set_state(B.FIELD_REFR, R)
+        in_or = o.get_state(oracle_mod.FIELD_RING, N, first=(n % D) * N)
+        abs_in = sh.consume(n)
+        v_pre = np.where(R == 0, sh.E_L + sh.P22 * (V32.astype(np.float64) - sh.E_L) + sh.P21 * I32.astype(np.float64), -1e9)
+        near = np.abs(v_pre - sh.V_th) < 1e-4
+        g.simulate(1)
+        o.simulate(1, record=False)
+        gs = np.sort(g.last_spikes()); os_ = np.sort(o.last_spikes())
+        diff = np.setxor1d(gs, os_)
+        assert np.all(near[diff]), f"step {n}: spike lists differ away from threshold: {diff[~near[diff]][:10]}"
+        n_spk += os_.size
+        gin = g.get_state(B.FIELD_LAST_INPUT).astype(np.float64)
+        if check_input:
+            err = np.abs(gin - in_or)
+            assert np.all(err <= 1e-5 * abs_in + 1e-12), f"step {n}: input current off by {err.max()} (mass {abs_in[err.argmax()]})"
+        Vo = o.get_state(oracle_mod.FIELD_V); Io = o.get_state(oracle_mod.FIELD_I_SYN)
+        gV = g.get_state(B.FIELD_V).astype(np.float64); gI = g.get_state(B.FIELD_I_SYN).astype(np.float64)
+        keep = np.ones(N, bool); keep[diff] = False
+        assert np.all(np.abs(gV - Vo)[keep] <= 1e-4), f"step {n}: V off by {np.abs(gV - Vo)[keep].max()}"
+        k_abs = np.abs(Io - sh.P11 * I - in_or)                      # = w_ext * k up to rounding
+        sh.abs_I = sh.P11 * sh.abs_I + abs_in + k_abs
+        assert np.all(np.abs(gI - Io) <= 1e-5 * sh.abs_I + 1e-9), f"step {n}: I_syn off by {np.abs(gI - Io).max()}"
+        assert np.array_equal(g.get_state(B.FIELD_REFR)[keep], o.get_state(oracle_mod.FIELD_REFR)[keep])
+        sh.deliver(n, os_)
+        if diff.size:                                                    # logged divergence: re-feed the ring (C11)
+            log.append((n, diff.tolist()))
+            g.set_state(B.FIELD_RING, o.get_state(oracle_mod.FIELD_RING).astype(np.float32))
+    return log, n_spk
+
+
+# ------------------------------------------------------------------------------------------------------------
+# config 0: tiny Brunel-style net
+# ------------------------------------------------------------------------------------------------------------
+def test_cfg0_structure_bit_exact(oracle_mod, B):
+    wl = W.brunel_tiny()
+    o, g = make_pair(wl, oracle_mod)
+    assert check_structure(g, o) == 0          # constant weights: no tolerance at all
+    assert raw_layout_ok(g)
+    st = g.stats()
+    assert st.n_connections == 100_000 and st.n_neurons == 1000
+    # O(1) spot regeneration of single draws against per-source read-back
+    for call, e, k in [(0, 5, 3), (1, 900, 79), (2, 17, 0), (3, 999, 19)]:
+        s, t, d, w = o.draw_connection(call, e, k)
+        tg, wg, dg = g.connections_of(s)
+        assert np.any((tg == t) & (dg == d) & (wg == w))
+    g.close()
+
+
+@pytest.mark.parametrize("mode", [0, 1, 2])
+def test_cfg0_lockstep_1000_steps(oracle_mod, B, mode):
+    wl = W.brunel_tiny()
+    o, g = make_pair(wl, oracle_mod)
+    g.set_option(B.OPT_STEP_MODE, mode)
+    log, n_spk = lockstep(o, g, wl, oracle_mod, B, 1000)
+    assert n_spk > 200                          # the initial volley (~21 % start above threshold)
+    assert len(log) <= 3, log
+    if not log:
+        assert g.stats().events == o.n_events
+    g.close()
+
+
+@pytest.mark.parametrize("mode,kernel", [(0, 1), (0, 2), (2, 1), (2, 2), (1, 1)])
+def test_cfg0_free_running_spikes_and_rates(oracle_mod, B, mode, kernel):
+    """Free run.  The first steps must agree spike for spike; afterwards rates per population (C17)."""
+    wl = W.brunel_tiny(n_steps=20000)
+    o, g = make_pair(wl, oracle_mod, debug_input=False)
+    g.set_option(B.OPT_STEP_MODE, mode)
+    g.set_option(B.OPT_DELIVERY_KERNEL, kernel)
+    g.simulate(wl.n_steps)
+    o.simulate(wl.n_steps)
+    gs, gi = g.get_spikes()
+    os_, oi = o.get_spikes()
+    assert np.all(np.diff(gs) >= 0)
+    first = 30                                  # before fp32/fp64 trajectories can separate
+    a = sorted(zip(gs[gs < first].tolist(), gi[gs < first].tolist()))
+    b = sorted(zip(os_[os_ < first].tolist(), oi[os_ < first].tolist()))
+    assert a == b and len(a) > 150
+    for first_id, n in wl.pop_ranges():
+        t = (wl.n_steps - 1000) * 1e-4
+        rg = np.sum((gi >= first_id) & (gi < first_id + n) & (gs >= 1000)) / n / t
+        ro = np.sum((oi >= first_id) & (oi < first_id + n) & (os_ >= 1000)) / n / t
+        assert abs(rg - ro) <= max(0.05 * ro, 0.1), (rg, ro)
+    assert g.stats().spikes == gs.size
+    g.close()
+
+
+# ------------------------------------------------------------------------------------------------------------
+# microcircuit-shaped nets (normal weights and delays, 8 populations, up to 54 connect calls)
+# ------------------------------------------------------------------------------------------------------------
+def test_microcircuit_small_structure_and_lockstep(oracle_mod, B):
+    wl = W.microcircuit(scale_div=40, n_steps=300, indegree_div=8)
+    o, g = make_pair(wl, oracle_mod)
+    nbad = check_structure(g, o, max_weight_ulp_mismatch=4)
+    assert raw_layout_ok(g)
+    log, n_spk = lockstep(o, g, wl, oracle_mod, B, 300)
+    assert n_spk > 100 and len(log) <= 3, (n_spk, log, nbad)
+    g.close()
+
+
+@pytest.fixture(scope="module")
+def cfg1(oracle_mod):
+    wl = W.microcircuit(10, 10000)
+    o, g = make_pair(wl, oracle_mod)
+    yield wl, o, g
+    g.close()
+
+
+def test_cfg1_structure_bit_exact(oracle_mod, B, cfg1):
+    wl, o, g = cfg1
+    assert g.stats().n_connections == 29_892_043
+    nbad = check_structure(g, o, max_weight_ulp_mismatch=16)     # C4: expected O(1) per 3e7 draws
+    print("cfg1 weight 1-ulp mismatches:", nbad)
+
+
+def test_cfg1_lockstep_200_steps(oracle_mod, B, cfg1):
+    wl, o, g = cfg1
+    log, n_spk = lockstep(o, g, wl, oracle_mod, B, 200)
+    print("cfg1 lockstep near-threshold log:", log, "spikes:", n_spk)
+    assert n_spk > 300 and len(log) <= 5
+
+
+def test_cfg1_free_running_rates_10s(oracle_mod, B):
+    """Population rates over 10 s of biological time, first 1 s discarded as the paper does."""
+    wl = W.microcircuit(10, 100_000)
+    o, g = make_pair(wl, oracle_mod, debug_input=False, max_recorded_spikes=1 << 24)
+    g.simulate(wl.n_steps)
+    o.simulate(wl.n_steps)
+    gs, gi = g.get_spikes()
+    os_, oi = o.get_spikes()
+    t = (wl.n_steps - 10000) * 1e-4
+    for (first_id, n), name in zip(wl.pop_ranges(), W.PD_NAMES):
+        rg = np.sum((gi >= first_id) & (gi < first_id + n) & (gs >= 10000)) / n / t
+        ro = np.sum((oi >= first_id) & (oi < first_id + n) & (os_ >= 10000)) / n / t
+        print(f"{name}: gpu {rg:.3f} Hz oracle {ro:.3f} Hz")
+        assert abs(rg - ro) <= max(0.05 * ro, 0.1), (name, rg, ro)
+    g.close()
