@@ -173,7 +173,7 @@ void configure_launch(ng_sim* s) {
     const double ring_bytes = (double)s->N * s->cfg.ring_slots * 4.0;
     const double mean_group = s->N > 0 ? (double)s->S / ((double)s->N * s->cfg.ring_slots) : 0.0;
     int k = s->delivery_kernel_opt;
-    if (k == 0) k = (ring_bytes > 0.5 * (double)s->l2_bytes && mean_group >= 64.0) ? 2 : 1;
+    if (k == 0) k = (ring_bytes > 0.5 * (double)s->l2_bytes && mean_group >= 4.0) ? 2 : 1;
     s->delivery_kernel = k;
     int blocks = s->deliver_blocks_opt;
     if (blocks <= 0) {

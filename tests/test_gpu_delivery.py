@@ -1,0 +1,97 @@
+"""GPU parity of the delivery stage alone (BASELINE.json configs[3] shape, neuron update bypassed, reading C8):
+spike injection bit-exact, ring contents equal to the oracle's within the L1-mass tolerance (C12), for both delivery
+kernels and all three step modes; plus the per-plane weight-sum invariants at a size the oracle cannot hold."""
+import numpy as np
+import pytest
+
+from paper_2007_14236_b200 import workloads as W
+
+from helpers import make_pair
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2007_14236_b200 import binding
+    return binding
+
+
+def ring_mass(o, wl, oracle_mod, n_steps, spikes_by_step):
+    """L1 mass of every ring cell after n_steps (|w| delivered and not yet consumed)."""
+    src, tgt, w, d, ro = o.get_connections()
+    N, D = o.n_neurons, wl.ring_slots
+    mass = np.zeros((D, N))
+    for n in range(n_steps):
+        mass[n % D] = 0.0
+        for j in spikes_by_step.get(n, ()):
+            lo, hi = ro[j], ro[j + 1]
+            np.add.at(mass, ((n + d[lo:hi].astype(np.int64)) % D, tgt[lo:hi]), np.abs(w[lo:hi]).astype(np.float64))
+    return mass.reshape(-1)
+
+
+@pytest.mark.parametrize("K,fraction,kernel,mode", [
+    (100, 0.05, 1, 0), (100, 0.05, 2, 0), (100, 0.01, 2, 2), (1000, 0.01, 1, 0), (1000, 0.01, 2, 0),
+    (1000, 0.05, 2, 1), (1000, 0.002, 2, 2), (1000, 0.002, 1, 2), (37, 0.03, 2, 0), (3, 0.5, 2, 0),
+])
+def test_delivery_only_matches_oracle(oracle_mod, B, K, fraction, kernel, mode):
+    n, steps = 20000, 70                       # 70 > D = 64: the ring wraps
+    wl = W.delivery_microbench(n=n, K=K, fraction=fraction, n_steps=steps, seed=5)
+    o, g = make_pair(wl, oracle_mod, debug_input=False)
+    g.set_option(B.OPT_DELIVERY_KERNEL, kernel)
+    g.set_option(B.OPT_STEP_MODE, mode)
+    g.simulate(steps)
+    o.simulate(steps)
+    gs, gi = g.get_spikes()
+    os_, oi = o.get_spikes()
+    assert gs.size == os_.size and gs.size > 0
+    go = np.lexsort((gi, gs)); oo = np.lexsort((oi, os_))
+    assert np.array_equal(gs[go], os_[oo]) and np.array_equal(gi[go], oi[oo])      # injection bit-exact
+    assert g.stats().events == o.n_events == gs.size * K
+    by_step = {}
+    for s_, i_ in zip(os_.tolist(), oi.tolist()):
+        by_step.setdefault(s_, []).append(i_)
+    mass = ring_mass(o, wl, oracle_mod, steps, by_step)
+    gr = g.get_state(B.FIELD_RING).astype(np.float64)
+    orr = o.get_state(oracle_mod.FIELD_RING)
+    assert np.count_nonzero(orr) > 0
+    assert np.array_equal(gr != 0, orr != 0)                                         # same cells touched
+    assert np.all(np.abs(gr - orr) <= 1e-5 * mass + 1e-12), float(np.abs(gr - orr).max())
+    g.close()
+
+
+@pytest.mark.parametrize("kernel", [1, 2])
+def test_delivery_invariants_large(B, kernel):
+    """200,000 sources x out-degree 1000 (2e8 records): per step, the weight arriving in every ring plane equals the sum
+    over spiking sources of their outgoing weights with that delay (fp64 on the host from the read-back rows), and
+    the event counter equals spikes x K.  No oracle involved: these are identities of the plain definition."""
+    n, K, steps = 200_000, 1000, 5
+    wl = W.delivery_microbench(n=n, K=K, fraction=0.01, n_steps=steps, seed=9)
+    g = B.Sim(0.1, wl.ring_slots, wl.seed, record_spikes=True)
+    wl.apply(g); g.prepare()
+    g.set_option(B.OPT_DELIVERY_KERNEL, kernel)
+    ro = g.row_offsets()
+    assert np.all(np.diff(ro) == K) and g.stats().n_records_padded == n * K
+    D = wl.ring_slots
+    total = np.zeros(D)
+    for n_step in range(steps):
+        ring_before = g.get_state(B.FIELD_RING).astype(np.float64).reshape(D, n)
+        g.simulate(1)
+        ids = g.last_spikes()
+        ring_after = g.get_state(B.FIELD_RING).astype(np.float64).reshape(D, n)
+        ring_before[n_step % D] = 0.0                       # consumed and cleared by this step
+        delta = (ring_after - ring_before).sum(axis=1)
+        expect = np.zeros(D)
+        absmass = np.zeros(D)
+        for j in ids[:400]:                                 # read back a bounded number of rows
+            tg, w, d = g.connections_of(int(j))
+            assert tg.size == K and tg.min() >= 0 and tg.max() < n and d.min() >= 1 and d.max() <= D
+        for j in ids:
+            tg, w, d = g.records(int(ro[j]), K)
+            np.add.at(expect, (n_step + d.astype(np.int64)) % D, w.astype(np.float64))
+            np.add.at(absmass, (n_step + d.astype(np.int64)) % D, np.abs(w.astype(np.float64)))
+        assert np.all(np.abs(delta - expect) <= 1e-5 * absmass + 1e-9), (delta - expect)
+        total += expect
+    st = g.stats()
+    assert st.events == st.spikes * K
+    g.close()
