@@ -459,15 +459,30 @@ __device__ __forceinline__ void deliver_rows_phase(const StepArgs& a, long long 
 //   segment length (1.6 records for out-degree 100, 156 for out-degree 10,000).
 //   `batch` shrinks to 1 when there are fewer items than warps, so a quiet step still spreads over the whole grid.
 // ---------------------------------------------------------------------------------------
-__device__ __forceinline__ void deliver_vec(const StepArgs& a, long long pbase, int q, int rel_lo, int len, int slot) {
-    const long long p = pbase + q;
-    const int4 t = ld_stream_s32x4(a.tgt + p);
-    const float4 ww = ld_stream_f32x4(a.w + p);
-    float* __restrict__ plane = a.ring + (size_t)slot * a.N;
-    if (q >= rel_lo && q < len) red_add_f32(plane + t.x, ww.x);
-    if (q + 1 >= rel_lo && q + 1 < len) red_add_f32(plane + t.y, ww.y);
-    if (q + 2 >= rel_lo && q + 2 < len) red_add_f32(plane + t.z, ww.z);
-    if (q + 3 >= rel_lo && q + 3 < len) red_add_f32(plane + t.w, ww.w);
+struct VecRef { long long pb; int q, rel_lo, len, slot; bool on; };
+
+// segment of vector v (in the batch-wide numbering) by a 5-step shuffle search over the exclusive prefix `pre`
+__device__ __forceinline__ VecRef locate_vec(int v, int total, int pre, long long pbase, int meta, int slot) {
+    int k = 0;
+#pragma unroll
+    for (int st = 16; st > 0; st >>= 1) {
+        const int t = __shfl_sync(0xffffffffu, pre, k + st);
+        if (t <= v) k += st;
+    }
+    VecRef r;
+    r.pb = __shfl_sync(0xffffffffu, pbase, k);
+    const int mt = __shfl_sync(0xffffffffu, meta, k);
+    r.slot = __shfl_sync(0xffffffffu, slot, k);
+    r.q = (v - __shfl_sync(0xffffffffu, pre, k)) << 2;
+    r.rel_lo = mt & 3; r.len = mt >> 2; r.on = v < total;
+    return r;
+}
+__device__ __forceinline__ void red_vec(const StepArgs& a, const VecRef& r, const int4& t, const float4& ww) {
+    float* __restrict__ plane = a.ring + (size_t)r.slot * a.N;
+    if (r.q >= r.rel_lo && r.q < r.len) red_add_f32(plane + t.x, ww.x);
+    if (r.q + 1 >= r.rel_lo && r.q + 1 < r.len) red_add_f32(plane + t.y, ww.y);
+    if (r.q + 2 >= r.rel_lo && r.q + 2 < r.len) red_add_f32(plane + t.z, ww.z);
+    if (r.q + 3 >= r.rel_lo && r.q + 3 < r.len) red_add_f32(plane + t.w, ww.w);
 }
 
 __device__ __forceinline__ void deliver_groups_phase(const StepArgs& a, long long n, int M, long long gwarp, long long gwarps,
@@ -477,31 +492,56 @@ __device__ __forceinline__ void deliver_groups_phase(const StepArgs& a, long lon
     const int32_t* __restrict__ list = a.spike_list + (size_t)(n & 1) * N;
     const long long items = (long long)M * D;
     if (items == 0) return;
-    long long bsz = (items + gwarps - 1) / gwarps;
+    const long long bsz = (items + gwarps - 1) / gwarps;
     const int batch = bsz > 32 ? 32 : (int)bsz;
     const long long n_batches = (items + batch - 1) / batch;
+    const bool small = items < 0x7fffffffLL;                         // 32-bit div/mod is enough (uniform branch)
     unsigned long long ev = 0;
-    for (long long b = gwarp; b < n_batches; b += gwarps) {
-        // ---- header of item (b*batch + lane) ----
+
+    // Three-stage software pipeline over this warp's batches b, b+gwarps, ...: while batch k is delivered, the group
+    // bounds of batch k+1 and the spike ids of batch k+2 are already in flight (the header chain
+    // list -> grp_rel/row_off -> records is three dependent DRAM/L2 round trips otherwise paid per batch).
+    auto item_of = [&](long long b, int& d, int& si) -> bool {
         const long long it = b * batch + lane;
-        long long pbase = 0; int rel_lo = 0, len = 0, slot = 0, nvec = 0;
-        if (lane < batch && it < items) {
-            const int d = (int)(it / M), si = (int)(it % M);          // d = delay - 1
-            const int j = __ldcg(list + si);
+        if (b >= n_batches || lane >= batch || it >= items) return false;
+        if (small) { d = (int)((uint32_t)it / (uint32_t)M); si = (int)((uint32_t)it - (uint32_t)d * (uint32_t)M); }
+        else { d = (int)(it / M); si = (int)(it - (long long)d * M); }
+        return true;
+    };
+    auto load_j = [&](long long b) -> int {
+        int d, si;
+        return item_of(b, d, si) ? __ldcg(list + si) : -1;
+    };
+    int d_cur = 0, d_nxt = 0, si_unused;
+    uint32_t ga_cur = 0, gb_cur = 0, ga_nxt = 0, gb_nxt = 0;
+    long long r0_cur = 0, r0_nxt = 0;
+    auto load_g = [&](long long b, int j, int& d, uint32_t& ga, uint32_t& gb, long long& r0) {
+        ga = gb = 0; r0 = 0; d = 0;
+        if (j >= 0 && item_of(b, d, si_unused)) {
             const uint32_t* __restrict__ g = a.grp_rel + (size_t)j * (D + 1);
-            const uint32_t ga = g[d], gb = g[d + 1];
+            ga = g[d]; gb = g[d + 1];
+            r0 = a.row_off[j];
             if (d == 0) ev += g[D];
-            if (gb > ga) {
-                const long long lo = a.row_off[j] + ga;
-                pbase = lo & ~3LL;
-                rel_lo = (int)(lo - pbase);
-                len = rel_lo + (int)(gb - ga);
-                nvec = (len + 3) >> 2;
-                slot = nmod + d + 1; if (slot >= D) slot -= D;
-            }
         }
-        // ---- lay the vectors of the batch end to end ----
-        int incl = nvec;
+    };
+    long long b = gwarp;
+    int j_nxt = load_j(b);
+    load_g(b, j_nxt, d_cur, ga_cur, gb_cur, r0_cur);
+    j_nxt = load_j(b + gwarps);
+    for (; b < n_batches; b += gwarps) {
+        load_g(b + gwarps, j_nxt, d_nxt, ga_nxt, gb_nxt, r0_nxt);       // stage B for the next batch
+        j_nxt = load_j(b + 2 * gwarps);                                 // stage A for the one after
+        // ---- stage C: header of this lane's item of batch b ----
+        long long pbase = 0; int rel_lo = 0, len = 0, slot = 0, nvec = 0;
+        if (gb_cur > ga_cur) {
+            const long long lo = r0_cur + ga_cur;
+            pbase = lo & ~3LL;
+            rel_lo = (int)(lo - pbase);
+            len = rel_lo + (int)(gb_cur - ga_cur);
+            nvec = (len + 3) >> 2;
+            slot = nmod + d_cur + 1; if (slot >= D) slot -= D;
+        }
+        int incl = nvec;                                                // lay the vectors of the batch end to end
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
             const int y = __shfl_up_sync(0xffffffffu, incl, o);
@@ -509,21 +549,17 @@ __device__ __forceinline__ void deliver_groups_phase(const StepArgs& a, long lon
         }
         const int pre = incl - nvec;
         const int total = __shfl_sync(0xffffffffu, incl, 31);
-        const int meta = (len << 2) | rel_lo;                         // len < 2^29
-        for (int base = 0; base < total; base += 32) {
-            const int v = base + lane;
-            int k = 0;
-#pragma unroll
-            for (int st = 16; st > 0; st >>= 1) {
-                const int t = __shfl_sync(0xffffffffu, pre, k + st);
-                if (t <= v) k += st;
-            }
-            const long long pb = __shfl_sync(0xffffffffu, pbase, k);
-            const int mt = __shfl_sync(0xffffffffu, meta, k);
-            const int sl = __shfl_sync(0xffffffffu, slot, k);
-            const int pk = __shfl_sync(0xffffffffu, pre, k);
-            if (v < total) deliver_vec(a, pb, (v - pk) << 2, mt & 3, mt >> 2, sl);
+        const int meta = (len << 2) | rel_lo;                           // len < 2^29
+        for (int base = 0; base < total; base += 64) {                  // two vectors per lane in flight
+            const VecRef r0v = locate_vec(base + lane, total, pre, pbase, meta, slot);
+            const VecRef r1v = locate_vec(base + 32 + lane, total, pre, pbase, meta, slot);
+            int4 t0 = make_int4(0, 0, 0, 0), t1 = t0; float4 w0 = make_float4(0.f, 0.f, 0.f, 0.f), w1 = w0;
+            if (r0v.on) { t0 = ld_stream_s32x4(a.tgt + r0v.pb + r0v.q); w0 = ld_stream_f32x4(a.w + r0v.pb + r0v.q); }
+            if (r1v.on) { t1 = ld_stream_s32x4(a.tgt + r1v.pb + r1v.q); w1 = ld_stream_f32x4(a.w + r1v.pb + r1v.q); }
+            if (r0v.on) red_vec(a, r0v, t0, w0);
+            if (r1v.on) red_vec(a, r1v, t1, w1);
         }
+        d_cur = d_nxt; ga_cur = ga_nxt; gb_cur = gb_nxt; r0_cur = r0_nxt;
     }
     if (ev) atomicAdd(&a.ctl->events, ev);
 }
