@@ -185,6 +185,16 @@ def delivery_microbench(device, peak_gbs, K=10000, fraction=0.05, steps=30, warm
     return {"error": err}
 
 
+def run_probes(device=0):
+    """Measured ceilings for the access shapes of the delivery stage."""
+    from paper_2007_14236_b200 import binding as B
+    out = {"stream_read_GBps": B.probe(0, 4 << 20, device) / 1e9}
+    for mb in (4, 16, 64, 256):
+        out[f"scattered_red_per_s_{mb}MB"] = B.probe(1, mb << 20, device)
+        out[f"records_plus_red_events_per_s_{mb}MB"] = B.probe(2, mb << 20, device)
+    return out
+
+
 def run_ours(args):
     import torch
     if not torch.cuda.is_available():
@@ -378,13 +388,16 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip timing the oracle")
     ap.add_argument("--only-microbench", action="store_true",
                     help="run only the configs[3] delivery microbenchmark and print its JSON object (used for ncu captures)")
+    ap.add_argument("--probe", action="store_true", help="run the ceiling probes (ng_probe) and print them as JSON")
     ap.add_argument("--micro-k", type=int, default=10000)
     ap.add_argument("--micro-fraction", type=float, default=0.05)
     ap.add_argument("--micro-steps", type=int, default=30)
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
-    if args.only_microbench:
+    if args.probe:
+        print(json.dumps(run_probes()), flush=True)
+    elif args.only_microbench:
         print(json.dumps(delivery_microbench(0, measured_peak_gbs()[0], K=args.micro_k, fraction=args.micro_fraction,
                                              steps=args.micro_steps)), flush=True)
     elif args.impl == "reference":

@@ -214,6 +214,14 @@ int32_t ng_get_connections(ng_sim* sim, int32_t src_id, int32_t* tgt_host, float
 /* Counters and timings.  Synchronises the stream. */
 int32_t ng_get_stats(ng_sim* sim, ng_stats* out);
 
+/* Ceiling probe for the roofline report (not on the hot path).  Measures, with the load and
+ * reduction instructions the delivery kernels use, what this GPU sustains for
+ *   kind 0: a coalesced 128-bit read stream over 2 GiB                        -> bytes per second
+ *   kind 1: red.global.add.f32 to uniformly random cells of a footprint_bytes array -> reductions per second
+ *   kind 2: streamed 8-byte records + one random reduction per record (the shape of a3) -> events per second
+ * Allocates its own scratch with cudaMalloc and frees it.  Errors: INVALID_ARG, OOM, CUDA. */
+int32_t ng_probe(int32_t device, int32_t kind, int64_t footprint_bytes, double* per_second_out);
+
 #ifdef __cplusplus
 }
 #endif

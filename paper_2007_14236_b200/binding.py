@@ -23,7 +23,7 @@ STEP_GRAPH, STEP_LAUNCH, STEP_PERSISTENT = 0, 1, 2
 EXPORTS = ["ng_create", "ng_destroy", "ng_last_error", "ng_create_population", "ng_connect_fixed_indegree",
            "ng_connect_fixed_outdegree", "ng_set_bypass", "ng_set_option", "ng_prepare", "ng_set_state",
            "ng_get_state", "ng_simulate", "ng_get_spikes", "ng_get_last_spikes", "ng_copy_row_offsets",
-           "ng_copy_group_offsets", "ng_copy_records", "ng_get_connections", "ng_get_stats"]
+           "ng_copy_group_offsets", "ng_copy_records", "ng_get_connections", "ng_get_stats", "ng_probe"]
 
 
 class NgConfig(C.Structure):
@@ -98,12 +98,22 @@ def load_library(path: str | None = None):
     L.ng_copy_records.argtypes = [vp, i64, i64, vp, vp, vp]
     L.ng_get_connections.argtypes = [vp, i32, vp, vp, vp, i64, C.POINTER(i64)]
     L.ng_get_stats.argtypes = [vp, C.POINTER(NgStats)]
+    L.ng_probe.argtypes = [i32, i32, i64, C.POINTER(C.c_double)]
     for name in EXPORTS:
         if name != "ng_last_error":
             getattr(L, name).restype = i32
     if path is None:
         _lib = L
     return L
+
+
+def probe(kind: int, footprint_bytes: int = 4 << 20, device: int = 0) -> float:
+    """ng_probe: kind 0 stream bytes/s, 1 scattered reductions/s, 2 streamed records + reductions events/s."""
+    out = C.c_double()
+    rc = load_library().ng_probe(device, kind, footprint_bytes, C.byref(out))
+    if rc != NG_OK:
+        raise NgError(rc, "ng_probe failed")
+    return out.value
 
 
 def _lif(params: dict) -> NgLifParams:

@@ -679,3 +679,55 @@ int32_t ng_get_stats(ng_sim* s, ng_stats* out) {
 }
 
 }  // extern "C"
+
+// ng_probe: see include/ng.h.  Allocates with cudaMalloc, runs on the legacy stream, frees everything.
+extern "C" int32_t ng_probe(int32_t device, int32_t kind, int64_t footprint_bytes, double* per_second_out) {
+    if (!per_second_out || kind < 0 || kind > 2 || footprint_bytes < 4096) return NG_ERR_INVALID_ARG;
+    if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return NG_ERR_CUDA; }
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return NG_ERR_CUDA;
+    const int blocks = prop.multiProcessorCount * 8, thr = 256;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    float ms = 0; double units = 0; int32_t rc = NG_OK;
+    float* ring = nullptr; int32_t* tgt = nullptr; float* w = nullptr; int* sink = nullptr;
+    const long long n_rec = 1LL << 28;                                  // 2 GiB of records for kinds 0 and 2
+    const uint32_t M = (uint32_t)std::min<int64_t>(footprint_bytes / 4, 0x7fffffff);
+    do {
+        if (cudaMalloc(&sink, 4) != cudaSuccess) { rc = NG_ERR_OOM; break; }
+        if (kind == 0) {
+            if (cudaMalloc(&tgt, n_rec * 8) != cudaSuccess) { rc = NG_ERR_OOM; break; }
+            cudaMemset(tgt, 0, n_rec * 8);
+            probe_stream_kernel<<<blocks * 2, thr>>>((const int4*)tgt, n_rec / 2, sink);
+            cudaEventRecord(e0);
+            probe_stream_kernel<<<blocks * 2, thr>>>((const int4*)tgt, n_rec / 2, sink);
+            cudaEventRecord(e1);
+            units = (double)n_rec * 8;                                  // bytes
+        } else if (kind == 1) {
+            if (cudaMalloc(&ring, (size_t)M * 4) != cudaSuccess) { rc = NG_ERR_OOM; break; }
+            cudaMemset(ring, 0, (size_t)M * 4);
+            probe_red_kernel<<<blocks, thr>>>(ring, M, 100);
+            cudaEventRecord(e0);
+            probe_red_kernel<<<blocks, thr>>>(ring, M, 2000);
+            cudaEventRecord(e1);
+            units = (double)blocks * thr * 2000;                        // reductions
+        } else {
+            if (cudaMalloc(&ring, (size_t)M * 4) != cudaSuccess || cudaMalloc(&tgt, n_rec * 4) != cudaSuccess ||
+                cudaMalloc(&w, n_rec * 4) != cudaSuccess) { rc = NG_ERR_OOM; break; }
+            cudaMemset(ring, 0, (size_t)M * 4); cudaMemset(w, 0, n_rec * 4);
+            probe_fill_targets_kernel<<<blocks, thr>>>(tgt, n_rec, M);
+            probe_deliver_kernel<<<blocks, thr>>>((const int4*)tgt, (const float4*)w, ring, n_rec / 32);
+            cudaEventRecord(e0);
+            probe_deliver_kernel<<<blocks, thr>>>((const int4*)tgt, (const float4*)w, ring, n_rec / 4);
+            cudaEventRecord(e1);
+            units = (double)n_rec;                                      // events
+        }
+        if (cudaDeviceSynchronize() != cudaSuccess) { rc = NG_ERR_CUDA; break; }
+        cudaEventElapsedTime(&ms, e0, e1);
+        *per_second_out = units / (ms * 1e-3);
+    } while (0);
+    cudaGetLastError();
+    cudaFree(ring); cudaFree(tgt); cudaFree(w); cudaFree(sink);
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    return rc;
+}

@@ -607,3 +607,46 @@ __global__ void fill_pop_of_kernel(uint8_t* pop_of, float* V, int first, int n, 
 }
 
 }  // namespace ng
+
+// ---------------------------------------------------------------------------------------
+// Ceiling probes (ng_probe): what the memory system of this GPU sustains for the access shapes of a3, measured
+// with the same instructions the delivery kernels use.  Not on the hot path; bench.py --probe reports them.
+// ---------------------------------------------------------------------------------------
+namespace ng {
+__device__ __forceinline__ uint32_t probe_hash(uint32_t x) {
+    x ^= x >> 16; x *= 0x7feb352dU; x ^= x >> 15; x *= 0x846ca68bU; x ^= x >> 16; return x;
+}
+// kind 0: coalesced 128-bit read stream over `n4` int4 elements
+__global__ void probe_stream_kernel(const int4* __restrict__ a, long long n4, int* sink) {
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    int acc = 0;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += stride) {
+        const int4 t = ld_stream_s32x4((const int32_t*)(a + i));
+        acc += t.x ^ t.y ^ t.z ^ t.w;
+    }
+    if (acc == 0x12345) *sink = acc;
+}
+// kind 1: `per_thread` red.global.add.f32 per thread to uniformly random cells of ring[0..M)
+__global__ void probe_red_kernel(float* ring, uint32_t M, int per_thread) {
+    uint32_t s = probe_hash((blockIdx.x * blockDim.x + threadIdx.x) * 2654435761u + 1u);
+    for (int i = 0; i < per_thread; ++i) {
+        s = s * 1664525u + 1013904223u;
+        red_add_f32(ring + __umulhi(probe_hash(s), M), 1.0f);
+    }
+}
+// kind 2: streamed records (int4 targets + float4 weights, 8 B per event) with one red per event
+__global__ void probe_deliver_kernel(const int4* __restrict__ tgt, const float4* __restrict__ w, float* ring, long long n4) {
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += stride) {
+        const int4 t = ld_stream_s32x4((const int32_t*)(tgt + i));
+        const float4 ww = ld_stream_f32x4((const float*)(w + i));
+        red_add_f32(ring + t.x, ww.x); red_add_f32(ring + t.y, ww.y);
+        red_add_f32(ring + t.z, ww.z); red_add_f32(ring + t.w, ww.w);
+    }
+}
+__global__ void probe_fill_targets_kernel(int32_t* t, long long n, uint32_t M) {
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
+        t[i] = (int32_t)__umulhi(probe_hash((uint32_t)i * 2654435761u + (uint32_t)(i >> 32) + 7u), M);
+}
+}  // namespace ng
