@@ -210,6 +210,8 @@ def run_ours(args):
     g = B.Sim(DT_MS, wl.ring_slots, wl.seed, record_spikes=True, max_recorded_spikes=1 << 24, device=local)
     wl.apply(g)
     t0 = time.time(); g.prepare(); build_wall = time.time() - t0
+    g.set_option(B.OPT_STEP_MODE, args.step_mode)
+    g.set_option(B.OPT_DELIVERY_KERNEL, args.delivery_kernel)
     g.set_state(B.FIELD_V, wl.initial_v())
     N = wl.n_neurons
 
@@ -269,7 +271,9 @@ def run_ours(args):
     us_upd = (p1.ms_update - p0.ms_update) * 1e3 / n_launch
     us_del = (p1.ms_deliver - p0.ms_deliver) * 1e3 / n_launch
     ev_per_launch = (p1.events - p0.events) / n_launch
-    if us_del >= us_upd:
+    if int(p1.delivery_kernel) == 3:          # fused step kernel: update + collection + delivery in one launch
+        kern, alg_bytes, us = "fused_step_kernel", N * BYTES_PER_NEURON_STEP + ev_per_launch * BYTES_PER_EVENT, us_upd
+    elif us_del >= us_upd:
         kern, alg_bytes, us = f"deliver_kernel<{int(p1.delivery_kernel)}>", ev_per_launch * BYTES_PER_EVENT, us_del
     else:
         kern, alg_bytes, us = "update_kernel", N * BYTES_PER_NEURON_STEP, us_upd
@@ -296,7 +300,9 @@ def run_ours(args):
                    "parallelism": "replicas only (independent seeds per rank, no collective)" if world > 1 else "1 GPU",
                    "l2": "no flush: 2.7 GB of connection records (>> 126 MB L2) read by data-dependent rows; neuron "
                          "state and ring stay resident as in any long simulation",
-                   "step_mode": "cuda graph, 100 time steps per graph", "seed": wl.seed},
+                   "step_mode": {0: "cuda graph, 100 time steps per graph", 1: "plain launches",
+                                 2: "one persistent cooperative kernel per ng_simulate call"}[args.step_mode],
+                   "delivery_kernel": int(s1.delivery_kernel), "seed": wl.seed},
         "synaptic_events_per_s": events / (ms_total * 1e-3), "spikes_per_time_step": spikes / (args.steps * T * world),
         "mean_rate_hz": spikes / world / N / bio_s, "us_per_time_step": ms_total * 1e3 / (args.steps * T),
         "build_s": build_wall, "gpu_launches": launches,
@@ -389,6 +395,8 @@ def main():
     ap.add_argument("--only-microbench", action="store_true",
                     help="run only the configs[3] delivery microbenchmark and print its JSON object (used for ncu captures)")
     ap.add_argument("--probe", action="store_true", help="run the ceiling probes (ng_probe) and print them as JSON")
+    ap.add_argument("--step-mode", type=int, default=0, choices=[0, 1, 2], help="NG_OPT_STEP_MODE")
+    ap.add_argument("--delivery-kernel", type=int, default=0, choices=[0, 1, 2, 3], help="NG_OPT_DELIVERY_KERNEL (0 = auto)")
     ap.add_argument("--micro-k", type=int, default=10000)
     ap.add_argument("--micro-fraction", type=float, default=0.05)
     ap.add_argument("--micro-steps", type=int, default=30)

@@ -51,6 +51,7 @@ struct ng_sim {
     int64_t n_padded = 0; int64_t max_row_records = 0;
     int sm_count = 148; size_t l2_bytes = 0;
     int delivery_kernel = 1; int deliver_blocks = 0; int update_blocks = 0; int persistent_blocks = 0;
+    int fused_blocks = 0; int persistent_fused_blocks = 0;
     cudaGraphExec_t graph_exec = nullptr; int graph_steps = 0;
     // stats
     double build_ms = 0, ms_update = 0, ms_deliver = 0;
@@ -164,6 +165,14 @@ void launch_deliver(ng_sim* s) {
     else deliver_kernel<1><<<s->deliver_blocks, kDeliverThreads, 0, s->stream>>>(s->a);
 }
 
+void launch_fused(ng_sim* s) {
+    fused_step_kernel<<<s->fused_blocks, kFusedThreads, 0, s->stream>>>(s->a);
+}
+// one time step: two kernels (update, deliver) or the fused step kernel
+void launch_step(ng_sim* s) {
+    if (s->delivery_kernel == 3) launch_fused(s);
+    else { launch_update(s); launch_deliver(s); }
+}
 // choose launch shapes from the built network (static per simulation; no per-step host decisions)
 void configure_launch(ng_sim* s) {
     const int sm = s->sm_count;
@@ -173,8 +182,18 @@ void configure_launch(ng_sim* s) {
     const double ring_bytes = (double)s->N * s->cfg.ring_slots * 4.0;
     const double mean_group = s->N > 0 ? (double)s->S / ((double)s->N * s->cfg.ring_slots) : 0.0;
     int k = s->delivery_kernel_opt;
+    // otherwise the step is latency-bound and the fused step kernel (one launch per step) wins.
     if (k == 0) k = (ring_bytes > 0.5 * (double)s->l2_bytes && mean_group >= 4.0) ? 2 : 1;
     s->delivery_kernel = k;
+    s->fused_blocks = grid_for(s->N, kFusedThreads, sm * 32);
+    {
+        int occf = 0;
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occf, persistent_fused_kernel, kFusedThreads, 0);
+        if (occf < 1) occf = 1;
+        long long pf = std::min<long long>((long long)sm * occf, (long long)s->fused_blocks);
+        if (pf < 1) pf = 1;
+        s->persistent_fused_blocks = (int)pf;
+    }
     int blocks = s->deliver_blocks_opt;
     if (blocks <= 0) {
         // enough warps to cover the expected items of a step, between one and eight CTAs per SM
@@ -203,7 +222,7 @@ int32_t build_graph(ng_sim* s, int steps) {
     destroy_graph(s);
     cudaGraph_t graph = nullptr;
     NG_CUDA(s, cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeThreadLocal));
-    for (int i = 0; i < steps; ++i) { launch_update(s); launch_deliver(s); }
+    for (int i = 0; i < steps; ++i) launch_step(s);
     NG_CUDA(s, cudaStreamEndCapture(s->stream, &graph));
     cudaError_t e = cudaGraphInstantiate(&s->graph_exec, graph, 0);
     cudaGraphDestroy(graph);
@@ -223,12 +242,35 @@ int32_t field_info(ng_sim* s, int32_t field, void** base, size_t* elem, int64_t*
         case NG_FIELD_V: *base = s->a.V; *elem = 4; *len = s->N; return NG_OK;
         case NG_FIELD_I_SYN: *base = s->a.I; *elem = 4; *len = s->N; return NG_OK;
         case NG_FIELD_REFR: *base = s->a.refr; *elem = 4; *len = s->N; return NG_OK;
-        case NG_FIELD_RING: *base = s->a.ring; *elem = 4; *len = (int64_t)s->N * s->cfg.ring_slots; return NG_OK;
+        case NG_FIELD_RING: *base = s->a.ring; *elem = 4; *len = (int64_t)s->N * s->cfg.ring_slots; return NG_OK;   // see ring_copy
         case NG_FIELD_LAST_INPUT:
             if (!s->a.last_input) return fail(s, NG_ERR_STATE, "NG_FIELD_LAST_INPUT needs NG_DEBUG_INPUT");
             *base = s->a.last_input; *elem = 4; *len = s->N; return NG_OK;
         default: return fail(s, NG_ERR_INVALID_ARG, "unknown field");
     }
+}
+
+// NG_FIELD_RING as the C-ABI shows it is [D][N], slot s holding the input of the one pending step n' in [n, n+D) with
+// n' mod D == s (n = index of the next step).  The device stores Dr = D + 1 planes indexed n' mod Dr (see
+// neuron_step in ng_device.cuh); this copies the element range [first, first+count) of the API view plane by plane.
+int32_t ring_copy(ng_sim* s, bool to_device, void* user, int64_t count, int64_t first) {
+    Ctl h{};
+    int32_t rc = read_ctl(s, &h);
+    if (rc) return rc;
+    const int64_t N = s->N, D = s->cfg.ring_slots, Dr = s->a.Dr, n = h.step_u;
+    int64_t done = 0;
+    while (done < count) {
+        const int64_t e = first + done, slot = e / N, i0 = e % N;
+        const int64_t len = std::min<int64_t>(count - done, N - i0);
+        const int64_t np = n + (((slot - n) % D) + D) % D;               // the pending step stored in API slot `slot`
+        float* dev = s->a.ring + (size_t)(np % Dr) * N + i0;
+        char* usr = (char*)user + (size_t)done * 4;
+        if (to_device) NG_CUDA(s, cudaMemcpyAsync(dev, usr, (size_t)len * 4, cudaMemcpyDefault, s->stream));
+        else NG_CUDA(s, cudaMemcpyAsync(usr, dev, (size_t)len * 4, cudaMemcpyDefault, s->stream));
+        done += len;
+    }
+    NG_CUDA(s, cudaStreamSynchronize(s->stream));
+    return NG_OK;
 }
 
 }  // namespace
@@ -321,7 +363,7 @@ int32_t ng_set_option(ng_sim* s, int32_t option, int64_t value) {
             if (value < 1 || value > 10000) return fail(s, NG_ERR_INVALID_ARG, "steps per graph in 1..10000");
             s->steps_per_graph = (int)value; destroy_graph(s); break;
         case NG_OPT_DELIVERY_KERNEL:
-            if (value < 0 || value > 2) return fail(s, NG_ERR_INVALID_ARG, "delivery kernel is 0, 1 or 2");
+            if (value < 0 || value > 3) return fail(s, NG_ERR_INVALID_ARG, "delivery kernel is 0, 1, 2 or 3");
             s->delivery_kernel_opt = (int)value; if (s->prepared) configure_launch(s); break;
         case NG_OPT_DELIVER_BLOCKS:
             if (value < 0 || value > (1 << 20)) return fail(s, NG_ERR_INVALID_ARG, "deliver blocks out of range");
@@ -355,7 +397,7 @@ int32_t ng_prepare(ng_sim* s) {
     bool ok = dev_alloc_t(s, &s->d_ctl, 1) && dev_alloc_t(s, &s->d_pops, s->pops.size()) &&
               dev_alloc_t(s, &s->d_pop_of, (size_t)N) && dev_alloc_t(s, &s->a.V, (size_t)N) &&
               dev_alloc_t(s, &s->a.I, (size_t)N) && dev_alloc_t(s, &s->a.refr, (size_t)N) &&
-              dev_alloc_t(s, &s->a.ring, (size_t)N * D) && dev_alloc_t(s, &s->a.spike_list, (size_t)2 * N) &&
+              dev_alloc_t(s, &s->a.ring, (size_t)N * (D + 1)) && dev_alloc_t(s, &s->a.spike_list, (size_t)2 * N) &&
               dev_alloc_t(s, &s->d_calls, std::max<size_t>(1, s->calls.size())) &&
               dev_alloc_t(s, &s->d_cnt, (size_t)N * D) && dev_alloc_t(s, &s->d_row_len, (size_t)N) &&
               dev_alloc_t(s, &s->d_row_off, (size_t)N + 1) && dev_alloc_t(s, &s->d_grp_rel, (size_t)N * (D + 1));
@@ -369,7 +411,7 @@ int32_t ng_prepare(ng_sim* s) {
     NG_CUDA(s, cudaMemsetAsync(s->d_ctl, 0, sizeof(Ctl), st));
     NG_CUDA(s, cudaMemsetAsync(s->a.I, 0, (size_t)N * 4, st));
     NG_CUDA(s, cudaMemsetAsync(s->a.refr, 0, (size_t)N * 4, st));
-    NG_CUDA(s, cudaMemsetAsync(s->a.ring, 0, (size_t)N * D * 4, st));
+    NG_CUDA(s, cudaMemsetAsync(s->a.ring, 0, (size_t)N * (D + 1) * 4, st));
     NG_CUDA(s, cudaMemsetAsync(s->d_cnt, 0, (size_t)N * D * 4, st));
     if (s->a.last_input) NG_CUDA(s, cudaMemsetAsync(s->a.last_input, 0, (size_t)N * 4, st));
     std::vector<PopDev> pd(s->pops.size());
@@ -434,7 +476,7 @@ int32_t ng_prepare(ng_sim* s) {
     dev_free(s, s->d_row_len); s->d_row_len = nullptr;
 
     // ---- step arguments ----
-    s->a.N = N; s->a.D = D; s->a.seed_lo = seed_lo; s->a.seed_hi = seed_hi;
+    s->a.N = N; s->a.D = D; s->a.Dr = D + 1; s->a.n_pops = (int32_t)s->pops.size(); s->a.seed_lo = seed_lo; s->a.seed_hi = seed_hi;
     s->a.pop_of = s->d_pop_of; s->a.pops = s->d_pops;
     s->a.row_off = s->d_row_off; s->a.grp_rel = s->d_grp_rel; s->a.tgt = s->d_tgt; s->a.w = s->d_w; s->a.dly = s->d_dly;
     s->a.ctl = s->d_ctl; s->a.bypass = s->bypass; s->a.inject_thr = s->inject_thr;
@@ -456,7 +498,7 @@ int32_t ng_set_state(ng_sim* s, int32_t field, const void* data, int64_t count, 
         int32_t rc = read_ctl(s, &h);
         if (rc) return rc;
         const unsigned long long recorded = h.rec_total[h.step_u & 1];
-        h.step_u = n; h.step_d = n; h.spike_cnt[0] = h.spike_cnt[1] = 0;
+        h.step_u = n; h.step_d = n; h.spike_cnt[0] = h.spike_cnt[1] = h.spike_cnt[2] = h.spike_cnt[3] = 0; h.ticket = 0;
         h.rec_total[0] = h.rec_total[1] = recorded;
         NG_CUDA(s, cudaMemcpyAsync(s->d_ctl, &h, sizeof(Ctl), cudaMemcpyHostToDevice, s->stream));
         NG_CUDA(s, cudaStreamSynchronize(s->stream));
@@ -467,6 +509,7 @@ int32_t ng_set_state(ng_sim* s, int32_t field, const void* data, int64_t count, 
     int32_t rc = field_info(s, field, &base, &elem, &len);
     if (rc) return rc;
     if (count < 0 || first < 0 || first + count > len) return fail(s, NG_ERR_INVALID_ARG, "range outside the field");
+    if (field == NG_FIELD_RING) return ring_copy(s, true, const_cast<void*>(data), count, first);
     NG_CUDA(s, cudaMemcpyAsync((char*)base + first * elem, data, (size_t)count * elem, cudaMemcpyDefault, s->stream));
     NG_CUDA(s, cudaStreamSynchronize(s->stream));
     return NG_OK;
@@ -489,6 +532,7 @@ int32_t ng_get_state(ng_sim* s, int32_t field, void* out, int64_t count, int64_t
     int32_t rc = field_info(s, field, &base, &elem, &len);
     if (rc) return rc;
     if (count < 0 || first < 0 || first + count > len) return fail(s, NG_ERR_INVALID_ARG, "range outside the field");
+    if (field == NG_FIELD_RING) return ring_copy(s, false, out, count, first);
     NG_CUDA(s, cudaMemcpyAsync(out, (char*)base + first * elem, (size_t)count * elem, cudaMemcpyDefault, s->stream));
     NG_CUDA(s, cudaStreamSynchronize(s->stream));
     return NG_OK;
@@ -511,9 +555,9 @@ int32_t ng_simulate(ng_sim* s, int64_t n_steps) {
             const int b = (int)std::min<int64_t>(kBatch, n_steps - done);
             for (int i = 0; i < b; ++i) {
                 cudaEventRecord(ev[3 * i], st);
-                launch_update(s);
+                if (s->delivery_kernel == 3) launch_fused(s); else launch_update(s);
                 cudaEventRecord(ev[3 * i + 1], st);
-                launch_deliver(s);
+                if (s->delivery_kernel != 3) launch_deliver(s);
                 cudaEventRecord(ev[3 * i + 2], st);
             }
             NG_CUDA(s, cudaStreamSynchronize(st));
@@ -526,16 +570,22 @@ int32_t ng_simulate(ng_sim* s, int64_t n_steps) {
             done += b;
         }
         for (auto& e : ev) cudaEventDestroy(e);
-        s->launches_update += n_steps; s->launches_deliver += n_steps;
+        s->launches_update += n_steps; s->launches_deliver += s->delivery_kernel == 3 ? 0 : n_steps;
     } else if (s->step_mode == 2) {
         long long ns = n_steps;
         void* args[] = {(void*)&s->a, (void*)&ns};
-        const void* fn = s->delivery_kernel == 2 ? (const void*)persistent_kernel<2> : (const void*)persistent_kernel<1>;
-        NG_CUDA(s, cudaLaunchCooperativeKernel(fn, dim3(s->persistent_blocks), dim3(kUpdateThreads), args, 0, st));
+        if (s->delivery_kernel == 3) {
+            NG_CUDA(s, cudaMemsetAsync(&s->d_ctl->bar, 0, sizeof(unsigned long long), st));
+            NG_CUDA(s, cudaLaunchCooperativeKernel((const void*)persistent_fused_kernel, dim3(s->persistent_fused_blocks),
+                                                   dim3(kFusedThreads), args, 0, st));
+        } else {
+            const void* fn = s->delivery_kernel == 2 ? (const void*)persistent_kernel<2> : (const void*)persistent_kernel<1>;
+            NG_CUDA(s, cudaLaunchCooperativeKernel(fn, dim3(s->persistent_blocks), dim3(kUpdateThreads), args, 0, st));
+        }
         s->launches_update += 1;
     } else if (s->step_mode == 1) {
-        for (int64_t i = 0; i < n_steps; ++i) { launch_update(s); launch_deliver(s); }
-        s->launches_update += n_steps; s->launches_deliver += n_steps;
+        for (int64_t i = 0; i < n_steps; ++i) launch_step(s);
+        s->launches_update += n_steps; s->launches_deliver += s->delivery_kernel == 3 ? 0 : n_steps;
     } else {
         int64_t left = n_steps;
         const int G = s->steps_per_graph;
@@ -543,8 +593,8 @@ int32_t ng_simulate(ng_sim* s, int64_t n_steps) {
             if (!s->graph_exec || s->graph_steps != G) { rc = build_graph(s, G); if (rc) return rc; }
             while (left >= G) { NG_CUDA(s, cudaGraphLaunch(s->graph_exec, st)); left -= G; }
         }
-        for (int64_t i = 0; i < left; ++i) { launch_update(s); launch_deliver(s); }
-        s->launches_update += n_steps; s->launches_deliver += n_steps;
+        for (int64_t i = 0; i < left; ++i) launch_step(s);
+        s->launches_update += n_steps; s->launches_deliver += s->delivery_kernel == 3 ? 0 : n_steps;
     }
     NG_CUDA(s, cudaGetLastError());
     s->steps_done += (uint64_t)n_steps;
@@ -608,8 +658,8 @@ int32_t ng_get_last_spikes(ng_sim* s, int32_t* ids_host, int64_t capacity, int64
     if (rc) return rc;
     if (h.step_u == 0) return NG_OK;
     const long long n = h.step_u - 1;
-    // spike_cnt[n&1] is cleared only by deliver(n+1); after deliver(n) it still holds step n's count
-    const int64_t M = h.spike_cnt[n & 1];
+    // spike_cnt[n&3] is cleared only during step n+3 at the earliest; after step n it still holds step n's count
+    const int64_t M = h.spike_cnt[n & 3];
     *count_out = M;
     const int64_t m = std::min(M, capacity);
     if (m > 0 && ids_host)

@@ -40,12 +40,15 @@ struct PopDev {                // per-population constants of the update (fp32 c
 struct Ctl {                   // device-resident control block; see ng.cu for the update/deliver handshake
     long long step_u;                      // written by deliver, read by update: index of the next step
     long long step_d;                      // written by update, read by deliver: index of the step being delivered
-    int32_t spike_cnt[2];                  // length of spike_list[parity]
+    int32_t spike_cnt[4];                  // length of the spike array of step n, indexed n & 3 (the list itself by n & 1)
     unsigned long long rec_total[2];       // spikes recorded before step of this parity
     unsigned long long spikes, events;
     int32_t err_delay;                     // builder: a drawn delay fell outside [1, D]
     int32_t max_row_records;               // builder: longest padded row
     unsigned long long n_padded;           // builder: total records stored
+    unsigned int ticket;                   // fused step kernel: CTAs that finished the current step
+    unsigned int pad0;
+    unsigned long long bar;                // persistent fused kernel: arrivals at the grid barrier
 };
 
 // ---------------------------------------------------------------------------------------
@@ -304,11 +307,12 @@ __device__ __forceinline__ void append_spike(bool spk, int32_t id, int32_t* __re
 }
 
 struct StepArgs {
-    int32_t N, D;
+    int32_t N, D;                // D = ring_slots of the C-ABI = largest legal delay
+    int32_t Dr, n_pops;          // Dr = D + 1 planes are stored (see update_phase); number of populations
     uint32_t seed_lo, seed_hi;
     // neuron state (SoA) and parameters
     float* V; float* I; int32_t* refr; const uint8_t* pop_of; const PopDev* pops;
-    float* ring;                 // [D][N] slot-major
+    float* ring;                 // [Dr][N] slot-major
     float* last_input;           // [N] or nullptr (NG_DEBUG_INPUT)
     // spike array, double-buffered by step parity, and the spike record
     int32_t* spike_list;         // [2][N]
@@ -331,41 +335,53 @@ struct StepArgs {
 //     V >= V_th: spike, V <- V_reset, refr <- t_ref/h
 // `gtid`/`gthreads` let the same body serve the stand-alone kernel and the persistent kernel.
 // ---------------------------------------------------------------------------------------
-__device__ __forceinline__ void update_phase(const StepArgs& a, long long n, long long gtid, long long gthreads) {
+// One neuron, one step.  `P` is the population table (global memory, or the CTA's shared-memory copy).
+// The ring stores Dr = D + 1 planes: the plane consumed here (n mod Dr) can then never be a delivery target of
+// step n (targets are (n + d) mod Dr, 1 <= d <= D), so the fused step kernel may deliver a spike while other
+// CTAs are still consuming their inputs.
+__device__ __forceinline__ bool neuron_step(const StepArgs& a, const PopDev* __restrict__ P, long long n, int i,
+                                            float* __restrict__ plane) {
+    // all independent loads first: one memory round trip instead of a chain
+    const float in = __ldcg(plane + i);          // written by red.global from other SMs: read at L2
+    if (a.bypass) {                                          // DESIGN.md C8: delivery-only mode
+        plane[i] = 0.f;
+        if (a.last_input) a.last_input[i] = in;
+        const uint4 x = philox4x32_10(a.seed_lo, a.seed_hi, (uint32_t)i, (uint32_t)n, (uint32_t)(n >> 32), kTagInject);
+        return x.x < a.inject_thr;
+    }
+    float V = a.V[i], I = a.I[i];
+    int r = a.refr[i];
+    const int pi = a.pop_of[i];
+    plane[i] = 0.f;
+    if (a.last_input) a.last_input[i] = in;
+    const PopDev* __restrict__ p = P + pi;
+    int k = 0;
+    const int nT = p->n_T;
+    if (nT > 0) {
+        const uint4 x = philox4x32_10(a.seed_lo, a.seed_hi, (uint32_t)i, (uint32_t)n, (uint32_t)(n >> 32), kTagPoisson);
+        while (k < nT && x.x >= p->T[k]) ++k;                // T is non-decreasing: k = #{m : x0 >= T[m]}
+    }
+    const float E_L = p->E_L;
+    bool spk = false;
+    if (r == 0) V = E_L + fmaf(p->P22, V - E_L, fmaf(p->P21, I, p->P20Ie));
+    else r -= 1;
+    I = fmaf(p->P11, I, in) + p->w_ext * (float)k;
+    if (V >= p->V_th) { spk = true; V = p->V_reset; r = p->refr_steps; }
+    a.V[i] = V; a.I[i] = I; a.refr[i] = r;
+    return spk;
+}
+
+__device__ __forceinline__ void update_phase(const StepArgs& a, const PopDev* __restrict__ P, long long n, long long gtid,
+                                             long long gthreads) {
     const int N = a.N;
-    const int slot = (int)(n % a.D);
+    const int slot = (int)(n % a.Dr);
     float* __restrict__ plane = a.ring + (size_t)slot * N;
     int32_t* __restrict__ list = a.spike_list + (size_t)(n & 1) * N;
-    int32_t* cnt = &a.ctl->spike_cnt[n & 1];
+    int32_t* cnt = &a.ctl->spike_cnt[n & 3];
     const long long n_round = ((long long)N + 31) & ~31LL;      // keep warps whole for the ballot
     for (long long ii = gtid; ii < n_round; ii += gthreads) {
         const int i = (int)ii;
-        bool spk = false;
-        if (i < N) {
-            const float in = __ldcg(plane + i);      // written by red.global from other SMs: read at L2
-            plane[i] = 0.f;
-            if (a.last_input) a.last_input[i] = in;
-            if (a.bypass) {                                      // DESIGN.md C8: delivery-only mode
-                const uint4 x = philox4x32_10(a.seed_lo, a.seed_hi, (uint32_t)i, (uint32_t)n, (uint32_t)(n >> 32), kTagInject);
-                spk = x.x < a.inject_thr;
-            } else {
-                const PopDev* __restrict__ p = a.pops + a.pop_of[i];
-                int k = 0;
-                const int nT = p->n_T;
-                if (nT > 0) {
-                    const uint4 x = philox4x32_10(a.seed_lo, a.seed_hi, (uint32_t)i, (uint32_t)n, (uint32_t)(n >> 32), kTagPoisson);
-                    while (k < nT && x.x >= __ldg(&p->T[k])) ++k;   // T is non-decreasing: k = #{m : x0 >= T[m]}
-                }
-                float V = a.V[i], I = a.I[i];
-                int r = a.refr[i];
-                const float E_L = p->E_L;
-                if (r == 0) V = E_L + fmaf(p->P22, V - E_L, fmaf(p->P21, I, p->P20Ie));
-                else r -= 1;
-                I = fmaf(p->P11, I, in) + p->w_ext * (float)k;
-                if (V >= p->V_th) { spk = true; V = p->V_reset; r = p->refr_steps; }
-                a.V[i] = V; a.I[i] = I; a.refr[i] = r;
-            }
-        }
+        const bool spk = i < N && neuron_step(a, P, n, i, plane);
         append_spike(spk, i, list, cnt);
     }
     if (gtid == 0) a.ctl->step_d = n;
@@ -406,7 +422,7 @@ __device__ __forceinline__ void bookkeeping_phase(const StepArgs& a, long long n
     }
     if (gtid == 0) {
         a.ctl->rec_total[(n + 1) & 1] = rec_base + (unsigned long long)M;
-        a.ctl->spike_cnt[(n + 1) & 1] = 0;
+        a.ctl->spike_cnt[(n + 1) & 3] = 0;
         a.ctl->spikes += (unsigned long long)M;
         a.ctl->step_u = n + 1;
     }
@@ -421,8 +437,8 @@ __device__ __forceinline__ void bookkeeping_phase(const StepArgs& a, long long n
 // ---------------------------------------------------------------------------------------
 __device__ __forceinline__ void deliver_rows_phase(const StepArgs& a, long long n, int M, long long gwarp, long long gwarps,
                                                    int lane) {
-    const int N = a.N, D = a.D;
-    const int nmod = (int)(n % D);
+    const int N = a.N, D = a.D, Dr = a.Dr;
+    const int nmod = (int)(n % Dr);
     const int32_t* __restrict__ list = a.spike_list + (size_t)(n & 1) * N;
     const int chunks = a.max_row_chunks;
     const long long items = (long long)M * chunks;
@@ -438,10 +454,10 @@ __device__ __forceinline__ void deliver_rows_phase(const StepArgs& a, long long 
             const float4 ww = ld_stream_f32x4(a.w + p);
             const uint32_t dd = ld_stream_u32(a.dly + p);
             int s;
-            if (t.x >= 0) { s = nmod + (int)(dd & 0xff); if (s >= D) s -= D; red_add_f32(a.ring + (size_t)s * N + t.x, ww.x); }
-            if (t.y >= 0) { s = nmod + (int)((dd >> 8) & 0xff); if (s >= D) s -= D; red_add_f32(a.ring + (size_t)s * N + t.y, ww.y); }
-            if (t.z >= 0) { s = nmod + (int)((dd >> 16) & 0xff); if (s >= D) s -= D; red_add_f32(a.ring + (size_t)s * N + t.z, ww.z); }
-            if (t.w >= 0) { s = nmod + (int)(dd >> 24); if (s >= D) s -= D; red_add_f32(a.ring + (size_t)s * N + t.w, ww.w); }
+            if (t.x >= 0) { s = nmod + (int)(dd & 0xff); if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * N + t.x, ww.x); }
+            if (t.y >= 0) { s = nmod + (int)((dd >> 8) & 0xff); if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * N + t.y, ww.y); }
+            if (t.z >= 0) { s = nmod + (int)((dd >> 16) & 0xff); if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * N + t.z, ww.z); }
+            if (t.w >= 0) { s = nmod + (int)(dd >> 24); if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * N + t.w, ww.w); }
         }
     }
     if (ev) atomicAdd(&a.ctl->events, ev);
@@ -487,8 +503,8 @@ __device__ __forceinline__ void red_vec(const StepArgs& a, const VecRef& r, cons
 
 __device__ __forceinline__ void deliver_groups_phase(const StepArgs& a, long long n, int M, long long gwarp, long long gwarps,
                                                      int lane) {
-    const int N = a.N, D = a.D;
-    const int nmod = (int)(n % D);
+    const int N = a.N, D = a.D, Dr = a.Dr;
+    const int nmod = (int)(n % Dr);
     const int32_t* __restrict__ list = a.spike_list + (size_t)(n & 1) * N;
     const long long items = (long long)M * D;
     if (items == 0) return;
@@ -539,7 +555,7 @@ __device__ __forceinline__ void deliver_groups_phase(const StepArgs& a, long lon
             rel_lo = (int)(lo - pbase);
             len = rel_lo + (int)(gb_cur - ga_cur);
             nvec = (len + 3) >> 2;
-            slot = nmod + d_cur + 1; if (slot >= D) slot -= D;
+            slot = nmod + d_cur + 1; if (slot >= Dr) slot -= Dr;
         }
         int incl = nvec;                                                // lay the vectors of the batch end to end
 #pragma unroll
@@ -564,16 +580,182 @@ __device__ __forceinline__ void deliver_groups_phase(const StepArgs& a, long lon
     if (ev) atomicAdd(&a.ctl->events, ev);
 }
 
+// ---------------------------------------------------------------------------------------
+// Population table staged in shared memory (the Poisson CDF walk and the propagators then cost shared-memory
+// latency instead of a chain of L2 round trips; L1 is invalidated at every kernel boundary).
+// ---------------------------------------------------------------------------------------
+constexpr int kMaxPopsSmem = 16;
+__device__ __forceinline__ const PopDev* stage_pops(const StepArgs& a, PopDev* sh) {
+    if (a.n_pops > kMaxPopsSmem) return a.pops;
+    const uint32_t* __restrict__ src = reinterpret_cast<const uint32_t*>(a.pops);
+    uint32_t* dst = reinterpret_cast<uint32_t*>(sh);
+    const int words = a.n_pops * (int)(sizeof(PopDev) / 4);
+    for (int k = threadIdx.x; k < words; k += blockDim.x) dst[k] = __ldg(src + k);
+    __syncthreads();
+    return sh;
+}
+
+// ---------------------------------------------------------------------------------------
+// a1 + a2 + a3 fused: kernel 3, one kernel per time step (the latency regime: tens of spikes per step).
+//   Every thread updates one neuron; the CTA gathers its own spikes in shared memory (id, row start, padded row
+//   length — the row bounds are fetched by the thread that spiked, so they are in flight while the rest of the CTA
+//   finishes its update), appends them to the global spike array / spike record with ONE atomic per CTA, and then
+//   walks the rows of its own spikes: 128-bit loads of targets and weights, 32-bit loads of delays, two vectors
+//   per thread in flight, red.global.add.f32 into ring[(n + d) mod Dr][target].
+//   No grid-wide dependency exists inside the step (the consumed plane n mod Dr is never a delivery target, see
+//   neuron_step), so a step costs one launch — or one grid barrier in the persistent variant — instead of two.
+// ---------------------------------------------------------------------------------------
+constexpr int kFusedThreads = 256;
+struct FusedShared {
+    PopDev pops[kMaxPopsSmem];
+    long long r0[kFusedThreads];
+    int32_t len[kFusedThreads];
+    int32_t id[kFusedThreads];
+    int32_t cnt, gbase;
+};
+
+__device__ __forceinline__ void red_rec4(const StepArgs& a, int nmod, const int4& t, const float4& ww, uint32_t dd) {
+    const int N = a.N, Dr = a.Dr;
+    int s;
+    if (t.x >= 0) { s = nmod + (int)(dd & 0xff); if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * N + t.x, ww.x); }
+    if (t.y >= 0) { s = nmod + (int)((dd >> 8) & 0xff); if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * N + t.y, ww.y); }
+    if (t.z >= 0) { s = nmod + (int)((dd >> 16) & 0xff); if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * N + t.z, ww.z); }
+    if (t.w >= 0) { s = nmod + (int)(dd >> 24); if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * N + t.w, ww.w); }
+}
+
+__device__ __forceinline__ void fused_phase(const StepArgs& a, const PopDev* __restrict__ P, long long n,
+                                            unsigned long long rec_base, FusedShared& sh) {
+    const int N = a.N, D = a.D;
+    const int nmod = (int)(n % a.Dr);
+    float* __restrict__ plane = a.ring + (size_t)nmod * N;
+    int32_t* __restrict__ list = a.spike_list + (size_t)(n & 1) * N;
+    const int lane = threadIdx.x & 31;
+    unsigned long long ev = 0;
+    for (long long base = (long long)blockIdx.x * kFusedThreads; base < N; base += (long long)gridDim.x * kFusedThreads) {
+        __syncthreads();                                   // previous round's readers of sh are done
+        if (threadIdx.x == 0) sh.cnt = 0;
+        __syncthreads();
+        const long long ii = base + threadIdx.x;
+        const int i = (int)ii;
+        const bool spk = ii < N && neuron_step(a, P, n, i, plane);
+        const unsigned m = __ballot_sync(0xffffffffu, spk);
+        if (m) {                                           // warp-aggregated append to the CTA's list
+            const int leader = __ffs(m) - 1;
+            int b = 0;
+            if (lane == leader) b = atomicAdd(&sh.cnt, __popc(m));
+            b = __shfl_sync(0xffffffffu, b, leader);
+            if (spk) {
+                const int k = b + __popc(m & ((1u << lane) - 1u));
+                const long long r0 = a.row_off[i], r1 = a.row_off[i + 1];
+                sh.id[k] = i; sh.r0[k] = r0; sh.len[k] = (int)(r1 - r0);
+                ev += a.grp_rel[(size_t)i * (D + 1) + D];
+            }
+        }
+        __syncthreads();
+        const int Ml = sh.cnt;
+        if (Ml == 0) continue;                             // uniform over the CTA
+        if (threadIdx.x == 0) sh.gbase = atomicAdd(&a.ctl->spike_cnt[n & 3], Ml);
+        for (int s = 0; s < Ml; ++s) {                     // a3: walk the rows of this CTA's spikes
+            const long long r0 = sh.r0[s];
+            const int len = sh.len[s];
+            for (int p = threadIdx.x * 4; p < len; p += kFusedThreads * 8) {
+                const int q = p + kFusedThreads * 4;
+                const int4 t0 = ld_stream_s32x4(a.tgt + r0 + p);
+                const float4 w0 = ld_stream_f32x4(a.w + r0 + p);
+                const uint32_t d0 = ld_stream_u32(a.dly + r0 + p);
+                int4 t1 = make_int4(-1, -1, -1, -1); float4 w1 = make_float4(0.f, 0.f, 0.f, 0.f); uint32_t d1 = 0;
+                if (q < len) { t1 = ld_stream_s32x4(a.tgt + r0 + q); w1 = ld_stream_f32x4(a.w + r0 + q); d1 = ld_stream_u32(a.dly + r0 + q); }
+                red_rec4(a, nmod, t0, w0, d0);
+                red_rec4(a, nmod, t1, w1, d1);
+            }
+        }
+        __syncthreads();                                   // sh.gbase
+        const int gb = sh.gbase;
+        for (int k = threadIdx.x; k < Ml; k += kFusedThreads) {    // a2: spike array and spike record
+            const int id = sh.id[k];
+            list[gb + k] = id;
+            const unsigned long long pos = rec_base + (unsigned long long)(gb + k);
+            if (pos < (unsigned long long)a.rec_cap) { a.rec_id[pos] = id; a.rec_step[pos] = (int32_t)n; }
+        }
+    }
+    if (ev) atomicAdd(&a.ctl->events, ev);
+}
+
+// One launch = one time step.  The last CTA to finish publishes the next step index (a4).
+__global__ void __launch_bounds__(kFusedThreads) fused_step_kernel(const StepArgs a) {
+    __shared__ FusedShared sh;
+    const long long n = __ldcg(&a.ctl->step_u);
+    const unsigned long long rec_base = __ldcg(&a.ctl->rec_total[n & 1]);
+    const PopDev* P = stage_pops(a, sh.pops);
+    fused_phase(a, P, n, rec_base, sh);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        const unsigned t = atomicAdd(&a.ctl->ticket, 1u);
+        if (t == gridDim.x - 1) {
+            __threadfence();
+            const int M = __ldcg(&a.ctl->spike_cnt[n & 3]);
+            a.ctl->rec_total[(n + 1) & 1] = rec_base + (unsigned long long)M;
+            a.ctl->spike_cnt[(n + 1) & 3] = 0;
+            a.ctl->spikes += (unsigned long long)M;
+            a.ctl->ticket = 0;
+            a.ctl->step_d = n;
+            a.ctl->step_u = n + 1;
+        }
+    }
+}
+
+// Grid barrier of the persistent fused kernel: one atomic arrival per CTA on a counter that only grows, then a
+// poll.  The kernel is launched cooperatively (all CTAs co-resident); the host clears ctl->bar before the launch.
+__device__ __forceinline__ void grid_barrier(Ctl* ctl, unsigned long long& epoch) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        epoch += gridDim.x;
+        __threadfence();
+        atomicAdd(&ctl->bar, 1ULL);
+        unsigned long long v;
+        do {
+            asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(&ctl->bar) : "memory");
+        } while (v < epoch);
+        __threadfence();
+    }
+    __syncthreads();
+}
+
+__global__ void __launch_bounds__(kFusedThreads) persistent_fused_kernel(const StepArgs a, long long n_steps) {
+    __shared__ FusedShared sh;
+    long long n = __ldcg(&a.ctl->step_u);
+    unsigned long long rec_base = __ldcg(&a.ctl->rec_total[n & 1]);
+    unsigned long long epoch = 0, spikes = 0;
+    const PopDev* P = stage_pops(a, sh.pops);
+    for (long long s = 0; s < n_steps; ++s, ++n) {
+        // the counter of step n+1 was last read (as step n-3's) long before the previous barrier
+        if (blockIdx.x == 0 && threadIdx.x == 0) a.ctl->spike_cnt[(n + 1) & 3] = 0;
+        fused_phase(a, P, n, rec_base, sh);
+        grid_barrier(a.ctl, epoch);
+        const unsigned long long M = (unsigned long long)__ldcg(&a.ctl->spike_cnt[n & 3]);
+        rec_base += M; spikes += M;
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) {             // nobody reads these words any more in this launch
+        a.ctl->rec_total[n & 1] = rec_base;
+        a.ctl->spikes += spikes;
+        a.ctl->step_d = n - 1;
+        a.ctl->step_u = n;
+    }
+}
+
 // ------------------------------- stand-alone kernels ---------------------------------
 __global__ void __launch_bounds__(kUpdateThreads) update_kernel(const StepArgs a) {
+    __shared__ PopDev sh_pops[kMaxPopsSmem];
     const long long n = __ldcg(&a.ctl->step_u);
-    update_phase(a, n, (long long)blockIdx.x * blockDim.x + threadIdx.x, (long long)gridDim.x * blockDim.x);
+    const PopDev* P = stage_pops(a, sh_pops);
+    update_phase(a, P, n, (long long)blockIdx.x * blockDim.x + threadIdx.x, (long long)gridDim.x * blockDim.x);
 }
 
 template <int kKernel>
 __global__ void __launch_bounds__(kDeliverThreads) deliver_kernel(const StepArgs a) {
     const long long n = __ldcg(&a.ctl->step_d);
-    const int M = __ldcg(&a.ctl->spike_cnt[n & 1]);
+    const int M = __ldcg(&a.ctl->spike_cnt[n & 3]);
     const long long gtid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const long long gthreads = (long long)gridDim.x * blockDim.x;
     if (kKernel == 1) deliver_rows_phase(a, n, M, gtid >> 5, gthreads >> 5, threadIdx.x & 31);
@@ -588,12 +770,14 @@ __global__ void __launch_bounds__(kUpdateThreads) persistent_kernel(const StepAr
     cg::grid_group grid = cg::this_grid();
     const long long gtid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const long long gthreads = (long long)gridDim.x * blockDim.x;
+    __shared__ PopDev sh_pops[kMaxPopsSmem];
+    const PopDev* P = stage_pops(a, sh_pops);
     long long n = __ldcg(&a.ctl->step_u);
     grid.sync();                                   // everyone has read step_u before anyone moves it
     for (long long s = 0; s < n_steps; ++s, ++n) {
-        update_phase(a, n, gtid, gthreads);
+        update_phase(a, P, n, gtid, gthreads);
         grid.sync();
-        const int M = __ldcg(&a.ctl->spike_cnt[n & 1]);
+        const int M = __ldcg(&a.ctl->spike_cnt[n & 3]);
         if (kKernel == 1) deliver_rows_phase(a, n, M, gtid >> 5, gthreads >> 5, threadIdx.x & 31);
         else deliver_groups_phase(a, n, M, gtid >> 5, gthreads >> 5, threadIdx.x & 31);
         bookkeeping_phase(a, n, M, gtid, gthreads);

@@ -79,11 +79,12 @@ def test_cfg0_structure_bit_exact(oracle_mod, B):
     g.close()
 
 
-@pytest.mark.parametrize("mode", [0, 1, 2])
-def test_cfg0_lockstep_1000_steps(oracle_mod, B, mode):
+@pytest.mark.parametrize("mode,kernel", [(0, 3), (1, 3), (2, 3), (0, 1), (2, 1), (1, 2)])
+def test_cfg0_lockstep_1000_steps(oracle_mod, B, mode, kernel):
     wl = W.brunel_tiny()
     o, g = make_pair(wl, oracle_mod)
     g.set_option(B.OPT_STEP_MODE, mode)
+    g.set_option(B.OPT_DELIVERY_KERNEL, kernel)
     log, n_spk = lockstep(o, g, wl, oracle_mod, B, 1000)
     assert n_spk > 200                          # the initial volley (~21 % start above threshold)
     assert len(log) <= 3, log
@@ -92,7 +93,7 @@ def test_cfg0_lockstep_1000_steps(oracle_mod, B, mode):
     g.close()
 
 
-@pytest.mark.parametrize("mode,kernel", [(0, 1), (0, 2), (2, 1), (2, 2), (1, 1)])
+@pytest.mark.parametrize("mode,kernel", [(0, 1), (0, 2), (2, 1), (2, 2), (1, 1), (0, 3), (1, 3), (2, 3)])
 def test_cfg0_free_running_spikes_and_rates(oracle_mod, B, mode, kernel):
     """Free run.  The first steps must agree spike for spike; afterwards rates per population (C17)."""
     wl = W.brunel_tiny(n_steps=20000)
