@@ -212,6 +212,7 @@ def run_ours(args):
     t0 = time.time(); g.prepare(); build_wall = time.time() - t0
     g.set_option(B.OPT_STEP_MODE, args.step_mode)
     g.set_option(B.OPT_DELIVERY_KERNEL, args.delivery_kernel)
+    g.set_option(B.OPT_PREFETCH, 0 if args.no_prefetch else 1)
     g.set_state(B.FIELD_V, wl.initial_v())
     N = wl.n_neurons
 
@@ -271,8 +272,8 @@ def run_ours(args):
     us_upd = (p1.ms_update - p0.ms_update) * 1e3 / n_launch
     us_del = (p1.ms_deliver - p0.ms_deliver) * 1e3 / n_launch
     ev_per_launch = (p1.events - p0.events) / n_launch
-    if int(p1.delivery_kernel) == 3:          # fused step kernel: update + collection + delivery in one launch
-        kern, alg_bytes, us = "fused_step_kernel", N * BYTES_PER_NEURON_STEP + ev_per_launch * BYTES_PER_EVENT, us_upd
+    if int(p1.delivery_kernel) == 3:          # pipelined step kernel: update + collection + delivery in one launch
+        kern, alg_bytes, us = "pipe_step_kernel", N * BYTES_PER_NEURON_STEP + ev_per_launch * BYTES_PER_EVENT, us_upd
     elif us_del >= us_upd:
         kern, alg_bytes, us = f"deliver_kernel<{int(p1.delivery_kernel)}>", ev_per_launch * BYTES_PER_EVENT, us_del
     else:
@@ -397,6 +398,7 @@ def main():
     ap.add_argument("--probe", action="store_true", help="run the ceiling probes (ng_probe) and print them as JSON")
     ap.add_argument("--step-mode", type=int, default=0, choices=[0, 1, 2], help="NG_OPT_STEP_MODE")
     ap.add_argument("--delivery-kernel", type=int, default=0, choices=[0, 1, 2, 3], help="NG_OPT_DELIVERY_KERNEL (0 = auto)")
+    ap.add_argument("--no-prefetch", action="store_true", help="NG_OPT_PREFETCH = 0")
     ap.add_argument("--micro-k", type=int, default=10000)
     ap.add_argument("--micro-fraction", type=float, default=0.05)
     ap.add_argument("--micro-steps", type=int, default=30)

@@ -79,13 +79,20 @@ enum {
     NG_OPT_STEP_MODE = 0,        /* 0 = CUDA graph of NG_OPT_STEPS_PER_GRAPH steps (default),
                                     1 = plain kernel launches, 2 = one persistent cooperative kernel  */
     NG_OPT_STEPS_PER_GRAPH = 1,  /* default 100 */
-    NG_OPT_DELIVERY_KERNEL = 2,  /* 0 = auto, 1 = row-chunk walk, 2 = delay-major segment walk        */
+    NG_OPT_DELIVERY_KERNEL = 2,  /* 0 = auto, 1 = row-chunk walk, 2 = delay-major segment walk,
+                                    3 = pipelined step kernel (delay-1 records with the update, the rest
+                                        overlapped with the next step: one grid dependency per step)      */
     NG_OPT_DELIVER_BLOCKS = 3,   /* grid size of the delivery kernel, 0 = auto                         */
     NG_OPT_PROFILE = 4,          /* 1 = time every kernel with CUDA events (forces plain launches);
                                     results in ng_stats.ms_update / ms_deliver                       */
     NG_OPT_ASYNC = 5,            /* 1 = ng_simulate returns after enqueueing (no stream synchronise)   */
-    NG_OPT_SORT_SEGMENTS = 6     /* 1 = order records inside each (source, delay) group by target id
+    NG_OPT_SORT_SEGMENTS = 6,    /* 1 = order records inside each (source, delay) group by target id
                                     after the build (default 1; must be set before ng_prepare)        */
+    NG_OPT_PREFETCH = 7,         /* 1 = the thread that detects a spike bulk-prefetches the spiking row into
+                                    L2 (default 1; ignored by delivery kernel 2)                       */
+    NG_OPT_TRACE = 8,            /* 1 = the persistent kernels (step mode 2) stamp %globaltimer at every phase
+                                    boundary of every CTA; read with ng_get_trace (after ng_prepare)   */
+    NG_OPT_PERSISTENT_THREADS = 9 /* threads per CTA of the persistent kernels: 1024 (default, one CTA per SM) or 512 */
 };
 
 typedef struct {
@@ -132,7 +139,7 @@ typedef struct {
     uint64_t launches_update;    /* kernel launches (or graph kernel nodes executed) since create    */
     uint64_t launches_deliver;
     uint64_t launches_other;     /* builder and bookkeeping kernels                                  */
-    int32_t delivery_kernel;     /* the delivery kernel in use (1 or 2)                              */
+    int32_t delivery_kernel;     /* the delivery kernel in use (1, 2 or 3)                           */
     int32_t step_mode;
 } ng_stats;
 
@@ -213,6 +220,12 @@ int32_t ng_get_connections(ng_sim* sim, int32_t src_id, int32_t* tgt_host, float
 
 /* Counters and timings.  Synchronises the stream. */
 int32_t ng_get_stats(ng_sim* sim, ng_stats* out);
+
+/* Phase stamps of the last persistent launch (NG_OPT_TRACE): uint64 ns, laid out [64 steps][blocks][8 stamps], step
+ * index = step-in-launch mod 64.  Stamps: 0 step start, 1 update (or fused phase) done, 2 after barrier; two-phase
+ * kernels also 3 delivery done, 4 bookkeeping done, 5 after the second barrier.  count_out = words available,
+ * blocks_out = CTAs of that launch; copies only if capacity >= count.  Errors: STATE when no trace exists. */
+int32_t ng_get_trace(ng_sim* sim, uint64_t* out_host, int64_t capacity, int64_t* count_out, int32_t* blocks_out);
 
 /* Ceiling probe for the roofline report (not on the hot path).  Measures, with the load and
  * reduction instructions the delivery kernels use, what this GPU sustains for

@@ -17,13 +17,13 @@ NG_RECORD_SPIKES, NG_DEBUG_INPUT = 1, 2
 FIELD_V, FIELD_I_SYN, FIELD_REFR, FIELD_RING, FIELD_STEP, FIELD_LAST_INPUT = 0, 1, 2, 3, 4, 5
 DIST_CONST, DIST_NORMAL_CLIPPED, DIST_UNIFORM_INT = 0, 1, 2
 (OPT_STEP_MODE, OPT_STEPS_PER_GRAPH, OPT_DELIVERY_KERNEL, OPT_DELIVER_BLOCKS, OPT_PROFILE, OPT_ASYNC,
- OPT_SORT_SEGMENTS) = range(7)
+ OPT_SORT_SEGMENTS, OPT_PREFETCH, OPT_TRACE, OPT_PERSISTENT_THREADS) = range(10)
 STEP_GRAPH, STEP_LAUNCH, STEP_PERSISTENT = 0, 1, 2
 
 EXPORTS = ["ng_create", "ng_destroy", "ng_last_error", "ng_create_population", "ng_connect_fixed_indegree",
            "ng_connect_fixed_outdegree", "ng_set_bypass", "ng_set_option", "ng_prepare", "ng_set_state",
            "ng_get_state", "ng_simulate", "ng_get_spikes", "ng_get_last_spikes", "ng_copy_row_offsets",
-           "ng_copy_group_offsets", "ng_copy_records", "ng_get_connections", "ng_get_stats", "ng_probe"]
+           "ng_copy_group_offsets", "ng_copy_records", "ng_get_connections", "ng_get_stats", "ng_get_trace", "ng_probe"]
 
 
 class NgConfig(C.Structure):
@@ -98,6 +98,7 @@ def load_library(path: str | None = None):
     L.ng_copy_records.argtypes = [vp, i64, i64, vp, vp, vp]
     L.ng_get_connections.argtypes = [vp, i32, vp, vp, vp, i64, C.POINTER(i64)]
     L.ng_get_stats.argtypes = [vp, C.POINTER(NgStats)]
+    L.ng_get_trace.argtypes = [vp, vp, i64, C.POINTER(i64), C.POINTER(i32)]
     L.ng_probe.argtypes = [i32, i32, i64, C.POINTER(C.c_double)]
     for name in EXPORTS:
         if name != "ng_last_error":
@@ -278,6 +279,14 @@ class Sim:
         if cap > 0:
             self._chk(self._L.ng_get_spikes(self._h, _ptr(steps), _ptr(ids), cap, C.byref(cnt)))
         return steps[:cap], ids[:cap]
+
+    def trace(self) -> np.ndarray:
+        """ng_get_trace: uint64 ns stamps [64 steps][blocks][8] of the last persistent launch (OPT_TRACE)."""
+        cnt, blocks = C.c_int64(), C.c_int32()
+        self._chk(self._L.ng_get_trace(self._h, None, 0, C.byref(cnt), C.byref(blocks)))
+        out = np.zeros(cnt.value, np.uint64)
+        self._chk(self._L.ng_get_trace(self._h, out.ctypes.data, cnt.value, C.byref(cnt), C.byref(blocks)))
+        return out.reshape(64, blocks.value, -1)
 
     def last_spikes(self) -> np.ndarray:
         cnt = C.c_int64()

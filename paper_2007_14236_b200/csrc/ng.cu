@@ -41,17 +41,20 @@ struct ng_sim {
     int32_t bypass = 0; uint32_t inject_thr = 0;
     // options
     int step_mode = 0; int steps_per_graph = 100; int delivery_kernel_opt = 0; int deliver_blocks_opt = 0;
-    int profile = 0; int async = 0; int sort_segments = 1;
+    bool trace_on = false; unsigned long long* trace_saved = nullptr; int last_persistent_blocks = 0;
+    int profile = 0; int async = 0; int sort_segments = 1; int prefetch_opt = 1;
     // device
     std::vector<void*> allocs;
     StepArgs a{};
     uint32_t* d_cnt = nullptr; long long* d_row_len = nullptr; long long* d_row_off = nullptr;
     uint32_t* d_grp_rel = nullptr; int32_t* d_tgt = nullptr; float* d_w = nullptr; uint8_t* d_dly = nullptr;
+    RowInfo* d_row_info = nullptr;
     CallDev* d_calls = nullptr; PopDev* d_pops = nullptr; uint8_t* d_pop_of = nullptr; Ctl* d_ctl = nullptr;
     int64_t n_padded = 0; int64_t max_row_records = 0;
     int sm_count = 148; size_t l2_bytes = 0;
     int delivery_kernel = 1; int deliver_blocks = 0; int update_blocks = 0; int persistent_blocks = 0;
-    int fused_blocks = 0; int persistent_fused_blocks = 0;
+    int pipe_blocks = 0; int persistent_pipe_blocks = 0;
+    int persistent_threads = kPersistentThreads;
     cudaGraphExec_t graph_exec = nullptr; int graph_steps = 0;
     // stats
     double build_ms = 0, ms_update = 0, ms_deliver = 0;
@@ -165,12 +168,16 @@ void launch_deliver(ng_sim* s) {
     else deliver_kernel<1><<<s->deliver_blocks, kDeliverThreads, 0, s->stream>>>(s->a);
 }
 
-void launch_fused(ng_sim* s) {
-    fused_step_kernel<<<s->fused_blocks, kFusedThreads, 0, s->stream>>>(s->a);
+// one time step: two kernels (update, deliver) or the pipelined step kernel
+void launch_pipe(ng_sim* s) {
+    pipe_step_kernel<true><<<s->pipe_blocks, kPipeThreads, 0, s->stream>>>(s->a);
 }
-// one time step: two kernels (update, deliver) or the fused step kernel
+// rest pass of the last step of an ng_simulate call (delivery kernel 4): leaves nothing pending between API calls
+void launch_pipe_flush(ng_sim* s) {
+    pipe_step_kernel<false><<<s->pipe_blocks, kPipeThreads, 0, s->stream>>>(s->a);
+}
 void launch_step(ng_sim* s) {
-    if (s->delivery_kernel == 3) launch_fused(s);
+    if (s->delivery_kernel == 3) launch_pipe(s);
     else { launch_update(s); launch_deliver(s); }
 }
 // choose launch shapes from the built network (static per simulation; no per-step host decisions)
@@ -182,17 +189,16 @@ void configure_launch(ng_sim* s) {
     const double ring_bytes = (double)s->N * s->cfg.ring_slots * 4.0;
     const double mean_group = s->N > 0 ? (double)s->S / ((double)s->N * s->cfg.ring_slots) : 0.0;
     int k = s->delivery_kernel_opt;
-    // otherwise the step is latency-bound and the fused step kernel (one launch per step) wins.
+    // otherwise the step is latency-bound: rows are walked whole (kernel 1) or by the pipelined step kernel (3).
     if (k == 0) k = (ring_bytes > 0.5 * (double)s->l2_bytes && mean_group >= 4.0) ? 2 : 1;
     s->delivery_kernel = k;
-    s->fused_blocks = grid_for(s->N, kFusedThreads, sm * 32);
+    s->a.prefetch = (k != 2 && s->prefetch_opt) ? 1 : 0;
+    s->pipe_blocks = grid_for(s->N, kPipeThreads - kEntryTile, sm * 4);   // updaters per CTA = kPipeThreads - kEntryTile
     {
-        int occf = 0;
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occf, persistent_fused_kernel, kFusedThreads, 0);
-        if (occf < 1) occf = 1;
-        long long pf = std::min<long long>((long long)sm * occf, (long long)s->fused_blocks);
-        if (pf < 1) pf = 1;
-        s->persistent_fused_blocks = (int)pf;
+        int occp = 0;
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occp, persistent_pipe_kernel, s->persistent_threads, 0);
+        if (occp < 1) occp = 1;
+        s->persistent_pipe_blocks = sm * std::min(occp, kPersistentThreads / s->persistent_threads);
     }
     int blocks = s->deliver_blocks_opt;
     if (blocks <= 0) {
@@ -206,15 +212,13 @@ void configure_launch(ng_sim* s) {
     s->deliver_blocks = blocks;
     s->a.max_row_chunks = (int32_t)((s->max_row_records + kChunkRecords - 1) / kChunkRecords);
     if (s->a.max_row_chunks < 1) s->a.max_row_chunks = 1;
+    s->a.mean_row_records = (int32_t)std::max<int64_t>(1, s->N > 0 ? s->n_padded / s->N : 1);
+    // persistent kernel: one CTA of persistent_threads per SM slot; few CTAs keep the grid barrier cheap
     int occ = 0;
-    if (s->delivery_kernel == 2) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, persistent_kernel<2>, kUpdateThreads, 0);
-    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, persistent_kernel<1>, kUpdateThreads, 0);
+    if (s->delivery_kernel == 2) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, persistent_kernel<2>, s->persistent_threads, 0);
+    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, persistent_kernel<1>, s->persistent_threads, 0);
     if (occ < 1) occ = 1;
-    // a small grid makes the grid-wide barrier cheap; large networks want every resident warp
-    const long long want = std::max<long long>((s->N + kUpdateThreads - 1) / kUpdateThreads, s->deliver_blocks);
-    long long pb = std::min<long long>((long long)sm * occ, std::max<long long>(want, sm));
-    pb = (pb / sm) * sm; if (pb < sm) pb = sm;
-    s->persistent_blocks = (int)pb;
+    s->persistent_blocks = sm * std::min(occ, kPersistentThreads / s->persistent_threads);
     destroy_graph(s);
 }
 
@@ -252,7 +256,7 @@ int32_t field_info(ng_sim* s, int32_t field, void** base, size_t* elem, int64_t*
 
 // NG_FIELD_RING as the C-ABI shows it is [D][N], slot s holding the input of the one pending step n' in [n, n+D) with
 // n' mod D == s (n = index of the next step).  The device stores Dr = D + 1 planes indexed n' mod Dr (see
-// neuron_step in ng_device.cuh); this copies the element range [first, first+count) of the API view plane by plane.
+// neuron_early in ng_device.cuh); this copies the element range [first, first+count) of the API view plane by plane.
 int32_t ring_copy(ng_sim* s, bool to_device, void* user, int64_t count, int64_t first) {
     Ctl h{};
     int32_t rc = read_ctl(s, &h);
@@ -363,7 +367,7 @@ int32_t ng_set_option(ng_sim* s, int32_t option, int64_t value) {
             if (value < 1 || value > 10000) return fail(s, NG_ERR_INVALID_ARG, "steps per graph in 1..10000");
             s->steps_per_graph = (int)value; destroy_graph(s); break;
         case NG_OPT_DELIVERY_KERNEL:
-            if (value < 0 || value > 3) return fail(s, NG_ERR_INVALID_ARG, "delivery kernel is 0, 1, 2 or 3");
+            if (value < 0 || value > 3) return fail(s, NG_ERR_INVALID_ARG, "delivery kernel is 0 .. 3");
             s->delivery_kernel_opt = (int)value; if (s->prepared) configure_launch(s); break;
         case NG_OPT_DELIVER_BLOCKS:
             if (value < 0 || value > (1 << 20)) return fail(s, NG_ERR_INVALID_ARG, "deliver blocks out of range");
@@ -373,6 +377,21 @@ int32_t ng_set_option(ng_sim* s, int32_t option, int64_t value) {
         case NG_OPT_SORT_SEGMENTS:
             if (s->prepared) return fail(s, NG_ERR_STATE, "NG_OPT_SORT_SEGMENTS after ng_prepare");
             s->sort_segments = value ? 1 : 0; break;
+        case NG_OPT_TRACE:
+            if (value && !s->prepared) return fail(s, NG_ERR_STATE, "NG_OPT_TRACE before ng_prepare");
+            if (value && !s->a.trace) {
+                const size_t words = (size_t)kTraceSteps * (size_t)s->sm_count * 32 * kTraceStamps;
+                if (!dev_alloc_t(s, &s->a.trace, words)) return fail(s, NG_ERR_OOM, "trace buffer");
+                NG_CUDA(s, cudaMemsetAsync(s->a.trace, 0, words * 8, s->stream));
+                s->trace_on = true;
+            }
+            if (!value && s->a.trace) { s->trace_saved = s->a.trace; s->a.trace = nullptr; }
+            else if (value && !s->a.trace) s->a.trace = s->trace_saved;
+            break;
+        case NG_OPT_PERSISTENT_THREADS:
+            if (value != 512 && value != 1024) return fail(s, NG_ERR_INVALID_ARG, "persistent threads: 512 or 1024");
+            s->persistent_threads = (int)value; if (s->prepared) configure_launch(s); break;
+        case NG_OPT_PREFETCH: s->prefetch_opt = value ? 1 : 0; if (s->prepared) configure_launch(s); break;
         default: return fail(s, NG_ERR_INVALID_ARG, "unknown option");
     }
     return NG_OK;
@@ -398,6 +417,7 @@ int32_t ng_prepare(ng_sim* s) {
               dev_alloc_t(s, &s->d_pop_of, (size_t)N) && dev_alloc_t(s, &s->a.V, (size_t)N) &&
               dev_alloc_t(s, &s->a.I, (size_t)N) && dev_alloc_t(s, &s->a.refr, (size_t)N) &&
               dev_alloc_t(s, &s->a.ring, (size_t)N * (D + 1)) && dev_alloc_t(s, &s->a.spike_list, (size_t)2 * N) &&
+              dev_alloc_t(s, &s->a.spike_row, (size_t)2 * N) && dev_alloc_t(s, &s->a.pois_k, (size_t)N) && dev_alloc_t(s, &s->d_row_info, (size_t)N) &&
               dev_alloc_t(s, &s->d_calls, std::max<size_t>(1, s->calls.size())) &&
               dev_alloc_t(s, &s->d_cnt, (size_t)N * D) && dev_alloc_t(s, &s->d_row_len, (size_t)N) &&
               dev_alloc_t(s, &s->d_row_off, (size_t)N + 1) && dev_alloc_t(s, &s->d_grp_rel, (size_t)N * (D + 1));
@@ -438,7 +458,8 @@ int32_t ng_prepare(ng_sim* s) {
     build_rowlen_kernel<<<(N + 255) / 256, 256, 0, st>>>(s->d_cnt, N, D, s->d_row_len, s->d_ctl);
     scan_exclusive_kernel<<<1, 1024, 0, st>>>(s->d_row_len, s->d_row_off, N, s->d_ctl);
     build_groups_kernel<<<(N + 255) / 256, 256, 0, st>>>(s->d_cnt, N, D, s->d_grp_rel);
-    s->launches_other += 3;
+    build_row_info_kernel<<<(N + 255) / 256, 256, 0, st>>>(N, D, s->d_row_off, s->d_grp_rel, s->d_row_info);
+    s->launches_other += 4;
     Ctl h{};
     int32_t rc = read_ctl(s, &h);
     if (rc) return rc;
@@ -447,7 +468,7 @@ int32_t ng_prepare(ng_sim* s) {
     s->n_padded = (int64_t)h.n_padded;
     s->max_row_records = h.max_row_records;
     const size_t np = (size_t)std::max<int64_t>(s->n_padded, 4);
-    if (!(dev_alloc_t(s, &s->d_tgt, np) && dev_alloc_t(s, &s->d_w, np) && dev_alloc_t(s, &s->d_dly, np)))
+    if (!(dev_alloc_t(s, &s->d_tgt, np) && dev_alloc_t(s, &s->d_w, np) && dev_alloc_t(s, &s->d_dly, np + 16)))
         return fail(s, NG_ERR_OOM, "device allocation failed (connection records)");
     NG_CUDA(s, cudaMemsetAsync(s->d_tgt, 0xFF, np * 4, st));       // padding records: target -1, weight 0, delay 0
     NG_CUDA(s, cudaMemsetAsync(s->d_w, 0, np * 4, st));
@@ -478,6 +499,7 @@ int32_t ng_prepare(ng_sim* s) {
     // ---- step arguments ----
     s->a.N = N; s->a.D = D; s->a.Dr = D + 1; s->a.n_pops = (int32_t)s->pops.size(); s->a.seed_lo = seed_lo; s->a.seed_hi = seed_hi;
     s->a.pop_of = s->d_pop_of; s->a.pops = s->d_pops;
+    s->a.row_info = s->d_row_info;
     s->a.row_off = s->d_row_off; s->a.grp_rel = s->d_grp_rel; s->a.tgt = s->d_tgt; s->a.w = s->d_w; s->a.dly = s->d_dly;
     s->a.ctl = s->d_ctl; s->a.bypass = s->bypass; s->a.inject_thr = s->inject_thr;
     s->prepared = true;
@@ -498,7 +520,8 @@ int32_t ng_set_state(ng_sim* s, int32_t field, const void* data, int64_t count, 
         int32_t rc = read_ctl(s, &h);
         if (rc) return rc;
         const unsigned long long recorded = h.rec_total[h.step_u & 1];
-        h.step_u = n; h.step_d = n; h.spike_cnt[0] = h.spike_cnt[1] = h.spike_cnt[2] = h.spike_cnt[3] = 0; h.ticket = 0;
+        h.step_u = n; h.step_d = n; h.spike_cnt[0] = h.spike_cnt[1] = h.spike_cnt[2] = h.spike_cnt[3] = 0; h.ticket = 0; h.pending = 0;
+        h.slot = (int32_t)(n % s->a.Dr);
         h.rec_total[0] = h.rec_total[1] = recorded;
         NG_CUDA(s, cudaMemcpyAsync(s->d_ctl, &h, sizeof(Ctl), cudaMemcpyHostToDevice, s->stream));
         NG_CUDA(s, cudaStreamSynchronize(s->stream));
@@ -555,7 +578,7 @@ int32_t ng_simulate(ng_sim* s, int64_t n_steps) {
             const int b = (int)std::min<int64_t>(kBatch, n_steps - done);
             for (int i = 0; i < b; ++i) {
                 cudaEventRecord(ev[3 * i], st);
-                if (s->delivery_kernel == 3) launch_fused(s); else launch_update(s);
+                if (s->delivery_kernel == 3) launch_pipe(s); else launch_update(s);
                 cudaEventRecord(ev[3 * i + 1], st);
                 if (s->delivery_kernel != 3) launch_deliver(s);
                 cudaEventRecord(ev[3 * i + 2], st);
@@ -574,13 +597,14 @@ int32_t ng_simulate(ng_sim* s, int64_t n_steps) {
     } else if (s->step_mode == 2) {
         long long ns = n_steps;
         void* args[] = {(void*)&s->a, (void*)&ns};
+        NG_CUDA(s, cudaMemsetAsync(&s->d_ctl->bar, 0, sizeof(unsigned long long), st));
+        s->last_persistent_blocks = s->delivery_kernel == 3 ? s->persistent_pipe_blocks : s->persistent_blocks;
         if (s->delivery_kernel == 3) {
-            NG_CUDA(s, cudaMemsetAsync(&s->d_ctl->bar, 0, sizeof(unsigned long long), st));
-            NG_CUDA(s, cudaLaunchCooperativeKernel((const void*)persistent_fused_kernel, dim3(s->persistent_fused_blocks),
-                                                   dim3(kFusedThreads), args, 0, st));
+            NG_CUDA(s, cudaLaunchCooperativeKernel((const void*)persistent_pipe_kernel, dim3(s->persistent_pipe_blocks),
+                                                   dim3(s->persistent_threads), args, 0, st));
         } else {
             const void* fn = s->delivery_kernel == 2 ? (const void*)persistent_kernel<2> : (const void*)persistent_kernel<1>;
-            NG_CUDA(s, cudaLaunchCooperativeKernel(fn, dim3(s->persistent_blocks), dim3(kUpdateThreads), args, 0, st));
+            NG_CUDA(s, cudaLaunchCooperativeKernel(fn, dim3(s->persistent_blocks), dim3(s->persistent_threads), args, 0, st));
         }
         s->launches_update += 1;
     } else if (s->step_mode == 1) {
@@ -596,6 +620,7 @@ int32_t ng_simulate(ng_sim* s, int64_t n_steps) {
         for (int64_t i = 0; i < left; ++i) launch_step(s);
         s->launches_update += n_steps; s->launches_deliver += s->delivery_kernel == 3 ? 0 : n_steps;
     }
+    if (s->delivery_kernel == 3 && (s->profile || s->step_mode != 2)) { launch_pipe_flush(s); s->launches_deliver += 1; }
     NG_CUDA(s, cudaGetLastError());
     s->steps_done += (uint64_t)n_steps;
     if (s->async) return NG_OK;
@@ -725,6 +750,19 @@ int32_t ng_get_stats(ng_sim* s, ng_stats* out) {
     out->build_ms = s->build_ms; out->ms_update = s->ms_update; out->ms_deliver = s->ms_deliver;
     out->launches_update = s->launches_update; out->launches_deliver = s->launches_deliver; out->launches_other = s->launches_other;
     out->delivery_kernel = s->delivery_kernel;
+    return NG_OK;
+}
+
+int32_t ng_get_trace(ng_sim* s, uint64_t* out_host, int64_t capacity, int64_t* count_out, int32_t* blocks_out) {
+    if (!s || !count_out || !blocks_out || capacity < 0) return NG_ERR_INVALID_ARG;
+    *count_out = 0; *blocks_out = 0;
+    unsigned long long* t = s->a.trace ? s->a.trace : s->trace_saved;
+    if (!t || s->last_persistent_blocks <= 0) return fail(s, NG_ERR_STATE, "no trace: set NG_OPT_TRACE and run step mode 2");
+    NG_CUDA(s, cudaSetDevice(s->cfg.device));
+    NG_CUDA(s, cudaStreamSynchronize(s->stream));
+    const int64_t words = (int64_t)kTraceSteps * s->last_persistent_blocks * kTraceStamps;
+    *count_out = words; *blocks_out = s->last_persistent_blocks;
+    if (out_host && capacity >= words) NG_CUDA(s, cudaMemcpy(out_host, t, (size_t)words * 8, cudaMemcpyDeviceToHost));
     return NG_OK;
 }
 

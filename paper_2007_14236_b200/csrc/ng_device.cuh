@@ -18,6 +18,8 @@ enum : int32_t { kRuleIndegree = 0, kRuleOutdegree = 1 };
 enum : int32_t { kDistConst = 0, kDistNormalClipped = 1, kDistUniformInt = 2 };
 
 constexpr int kMaxPoissonTable = 64;
+constexpr int kTraceSteps = 64;      // the persistent kernels keep the phase stamps of the last kTraceSteps steps
+constexpr int kTraceStamps = 16;
 constexpr int kUpdateThreads = 256;
 constexpr int kDeliverThreads = 256;
 constexpr int kChunkRecords = 128;   // records one warp consumes per iteration of the row walk: 32 lanes x 4
@@ -46,8 +48,10 @@ struct Ctl {                   // device-resident control block; see ng.cu for t
     int32_t err_delay;                     // builder: a drawn delay fell outside [1, D]
     int32_t max_row_records;               // builder: longest padded row
     unsigned long long n_padded;           // builder: total records stored
-    unsigned int ticket;                   // fused step kernel: CTAs that finished the current step
-    unsigned int pad0;
+    unsigned int ticket;                   // fused / pipelined step kernels: CTAs that finished the current step
+    int32_t pending;                       // pipelined step kernel: the rest pass of step step_u - 1 is outstanding
+    int32_t slot;                          // step_u mod Dr, kept next to step_u so no kernel divides 64-bit integers
+    int32_t pad1;
     unsigned long long bar;                // persistent fused kernel: arrivals at the grid barrier
 };
 
@@ -230,6 +234,20 @@ __global__ void build_groups_kernel(uint32_t* __restrict__ cnt, int N, int D, ui
     grp_rel[(size_t)j * (D + 1) + D] = run;
 }
 
+// row_info[j] = (first record, out-degree, padded length) of row j in one 16-byte word: the thread that detects a
+// spike fetches everything delivery needs with a single load.
+// deg = out-degree (the stored row is padded to a multiple of 4 records), d1 = records with delay 1 (the first d1 of the row)
+struct __align__(16) RowInfo { long long r0; int32_t deg; int32_t d1; };
+__host__ __device__ __forceinline__ int32_t padded_len(int32_t deg) { return (deg + 3) & ~3; }
+__global__ void build_row_info_kernel(int N, int D, const long long* __restrict__ row_off, const uint32_t* __restrict__ grp_rel,
+                                      RowInfo* __restrict__ row_info) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= N) return;
+    RowInfo r;
+    r.r0 = row_off[j]; r.deg = (int32_t)grp_rel[(size_t)j * (D + 1) + D]; r.d1 = (int32_t)grp_rel[(size_t)j * (D + 1) + 1];
+    row_info[j] = r;
+}
+
 __global__ void __launch_bounds__(256)
 build_fill_kernel(const CallDev* __restrict__ calls, int call_idx, uint32_t seed_lo, uint32_t seed_hi, int D,
                   uint32_t* __restrict__ cursor, const long long* __restrict__ row_off,
@@ -293,18 +311,24 @@ build_sort_groups_kernel(int N, int D, const long long* __restrict__ row_off, co
 // ---------------------------------------------------------------------------------------
 // Warp-aggregated append to the spike array (Fig. 1b: "the spike is sent to the spike
 // array"; its maximum size is the number of nodes).  One atomicAdd per warp that holds a spike.
-// Every lane of the warp must call this.
+// Every lane of the warp must call this.  Next to the id the entry carries the row bounds of the spiking neuron
+// (one 16-byte load from row_info), so delivery starts from the entry without a second dependent lookup.
 // ---------------------------------------------------------------------------------------
-__device__ __forceinline__ void append_spike(bool spk, int32_t id, int32_t* __restrict__ list, int32_t* cnt) {
-    const unsigned m = __ballot_sync(0xffffffffu, spk);
-    if (m == 0) return;
-    const int lane = threadIdx.x & 31;
-    const int leader = __ffs(m) - 1;
-    int base = 0;
-    if (lane == leader) base = atomicAdd(cnt, __popc(m));
-    base = __shfl_sync(0xffffffffu, base, leader);
-    if (spk) list[base + __popc(m & ((1u << lane) - 1u))] = id;
+__device__ __forceinline__ RowInfo ld_row_info(const RowInfo* p) {
+    const int4 v = __ldg(reinterpret_cast<const int4*>(p));
+    RowInfo r;
+    r.r0 = (long long)(((unsigned long long)(uint32_t)v.y << 32) | (uint32_t)v.x); r.deg = v.z; r.d1 = v.w;
+    return r;
 }
+__device__ __forceinline__ void st_row_info(RowInfo* p, const RowInfo& r) {
+    *reinterpret_cast<int4*>(p) = make_int4((int)(uint32_t)(unsigned long long)r.r0, (int)(uint32_t)((unsigned long long)r.r0 >> 32), r.deg, r.d1);
+}
+// TMA-unit bulk prefetch into L2 (no destination): p 16-byte aligned, bytes a multiple of 16
+__device__ __forceinline__ void prefetch_l2_bulk(const void* p, uint32_t bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+struct StepArgs;
+__device__ __forceinline__ void prefetch_row(const StepArgs& a, const RowInfo& r);
 
 struct StepArgs {
     int32_t N, D;                // D = ring_slots of the C-ABI = largest legal delay
@@ -316,6 +340,11 @@ struct StepArgs {
     float* last_input;           // [N] or nullptr (NG_DEBUG_INPUT)
     // spike array, double-buffered by step parity, and the spike record
     int32_t* spike_list;         // [2][N]
+    RowInfo* spike_row;          // [2][N] row bounds of spike_list's entries (same index)
+    const RowInfo* row_info;     // [N]
+    int32_t prefetch;            // 1: a spiking thread bulk-prefetches its row into L2 (row-walk kernels)
+    uint8_t* pois_k;             // [N] Poisson counts of the next step (persistent pipelined kernel)
+    unsigned long long* trace;   // NG_OPT_TRACE: [kTraceSteps][gridDim.x][kTraceStamps] %globaltimer stamps, or nullptr
     int32_t* rec_step; int32_t* rec_id; long long rec_cap;   // rec_cap = 0: recording off
     // connection structure
     const long long* row_off; const uint32_t* grp_rel;
@@ -323,7 +352,51 @@ struct StepArgs {
     Ctl* ctl;
     int32_t bypass; uint32_t inject_thr;
     int32_t max_row_chunks;      // ceil(longest padded row / kChunkRecords)
+    int32_t mean_row_records;    // mean padded row length (>= 1): picks the item size of delivery kernel 1
 };
+
+// The records of a spiking row are requested from DRAM the moment the spike is detected: by the time the delivery
+// phase (after the grid barrier / kernel boundary) asks for them they are L2 hits.  Pieces of at most 32 KB.
+__device__ __forceinline__ void prefetch_row(const StepArgs& a, const RowInfo& r) {
+    const int len = padded_len(r.deg);
+    const long long bytes4 = (long long)len * 4;
+    const uint32_t head = (uint32_t)(((long long)r.d1 * 4 + 15) & ~15LL);      // delay-1 records: needed first (kernel 4)
+    if (head > 0 && head < 32768) {
+        prefetch_l2_bulk(reinterpret_cast<const char*>(a.tgt + r.r0), head);
+        prefetch_l2_bulk(reinterpret_cast<const char*>(a.w + r.r0), head);
+    }
+    for (long long o = 0; o < bytes4; o += 32768) {
+        const uint32_t b = (uint32_t)(bytes4 - o < 32768 ? bytes4 - o : 32768);
+        prefetch_l2_bulk(reinterpret_cast<const char*>(a.tgt + r.r0) + o, b);
+        prefetch_l2_bulk(reinterpret_cast<const char*>(a.w + r.r0) + o, b);
+    }
+    const long long d0 = r.r0 & ~15LL, d1 = (r.r0 + len + 15) & ~15LL;       // delay bytes, 16-byte grid
+    for (long long o = d0; o < d1; o += 32768)
+        prefetch_l2_bulk(a.dly + o, (uint32_t)(d1 - o < 32768 ? d1 - o : 32768));
+}
+
+// `rec_base` = number of spikes recorded before step n: the spiking thread also writes the spike record (a2,
+// PAPER.md:181 "all spike times of all neurons recorded").  The atomic is issued before the row lookup and the
+// prefetches so that all three overlap.
+__device__ __forceinline__ void append_spike(const StepArgs& a, bool spk, int32_t id, long long n, unsigned long long rec_base) {
+    const unsigned m = __ballot_sync(0xffffffffu, spk);
+    if (m == 0) return;
+    const int lane = threadIdx.x & 31;
+    const int leader = __ffs(m) - 1;
+    int base = 0;
+    if (lane == leader) base = atomicAdd(&a.ctl->spike_cnt[n & 3], __popc(m));
+    RowInfo r;
+    if (spk) { r = ld_row_info(a.row_info + id); if (a.prefetch) prefetch_row(a, r); }
+    base = __shfl_sync(0xffffffffu, base, leader);
+    if (spk) {
+        const int idx = base + __popc(m & ((1u << lane) - 1u));
+        const size_t k = (size_t)(n & 1) * a.N + idx;
+        a.spike_list[k] = id;
+        st_row_info(a.spike_row + k, r);
+        const unsigned long long pos = rec_base + (unsigned long long)idx;
+        if (pos < (unsigned long long)a.rec_cap) { a.rec_id[pos] = id; a.rec_step[pos] = (int32_t)n; }
+    }
+}
 
 // ---------------------------------------------------------------------------------------
 // a1 + a2. Neuron update fused with the Poisson drive and spike collection — one thread per neuron.
@@ -339,52 +412,68 @@ struct StepArgs {
 // The ring stores Dr = D + 1 planes: the plane consumed here (n mod Dr) can then never be a delivery target of
 // step n (targets are (n + d) mod Dr, 1 <= d <= D), so the fused step kernel may deliver a spike while other
 // CTAs are still consuming their inputs.
-__device__ __forceinline__ bool neuron_step(const StepArgs& a, const PopDev* __restrict__ P, long long n, int i,
-                                            float* __restrict__ plane) {
-    // all independent loads first: one memory round trip instead of a chain
-    const float in = __ldcg(plane + i);          // written by red.global from other SMs: read at L2
-    if (a.bypass) {                                          // DESIGN.md C8: delivery-only mode
-        plane[i] = 0.f;
-        if (a.last_input) a.last_input[i] = in;
-        const uint4 x = philox4x32_10(a.seed_lo, a.seed_hi, (uint32_t)i, (uint32_t)n, (uint32_t)(n >> 32), kTagInject);
-        return x.x < a.inject_thr;
-    }
-    float V = a.V[i], I = a.I[i];
-    int r = a.refr[i];
-    const int pi = a.pop_of[i];
-    plane[i] = 0.f;
-    if (a.last_input) a.last_input[i] = in;
-    const PopDev* __restrict__ p = P + pi;
+// Split in two so that the spike is known as early as possible: neuron_early needs only V, I_syn, refr (one memory
+// round trip); the caller then starts everything that depends on the spike (row lookup, L2 prefetch of the row,
+// counters) and neuron_late — Philox, Poisson count, I_syn update: most of the arithmetic — overlaps those latencies.
+// The arithmetic and its order are exactly those of the list above (V uses I before its update).
+struct NeuronRegs { float in, I; int pi, kq; };     // kq: Poisson count computed ahead of time, or 0xff
+
+// DESIGN.md C7: k = #{m : x0 >= T[m]}, x0 from Philox(seed; i, n, POISSON); T is non-decreasing.  A pure function of
+// (seed, i, n): the persistent pipelined kernel evaluates it for step n+1 while it waits at the grid barrier.
+__device__ __forceinline__ int poisson_count(const StepArgs& a, const PopDev* __restrict__ p, long long n, int i) {
     int k = 0;
     const int nT = p->n_T;
     if (nT > 0) {
         const uint4 x = philox4x32_10(a.seed_lo, a.seed_hi, (uint32_t)i, (uint32_t)n, (uint32_t)(n >> 32), kTagPoisson);
-        while (k < nT && x.x >= p->T[k]) ++k;                // T is non-decreasing: k = #{m : x0 >= T[m]}
+        while (k < nT && x.x >= p->T[k]) ++k;
     }
+    return k;
+}
+
+__device__ __forceinline__ bool neuron_early(const StepArgs& a, const PopDev* __restrict__ P, long long n, int i,
+                                             float* __restrict__ plane, NeuronRegs& g, bool have_k = false) {
+    g.in = __ldcg(plane + i);                    // written by red.global from other SMs: read at L2
+    g.kq = have_k ? (int)a.pois_k[i] : 0xff;
+    if (a.bypass) {                                          // DESIGN.md C8: delivery-only mode
+        const uint4 x = philox4x32_10(a.seed_lo, a.seed_hi, (uint32_t)i, (uint32_t)n, (uint32_t)(n >> 32), kTagInject);
+        return x.x < a.inject_thr;
+    }
+    float V = a.V[i];
+    g.I = a.I[i];
+    int r = a.refr[i];
+    g.pi = a.pop_of[i];
+    const PopDev* __restrict__ p = P + g.pi;
     const float E_L = p->E_L;
     bool spk = false;
-    if (r == 0) V = E_L + fmaf(p->P22, V - E_L, fmaf(p->P21, I, p->P20Ie));
+    if (r == 0) V = E_L + fmaf(p->P22, V - E_L, fmaf(p->P21, g.I, p->P20Ie));
     else r -= 1;
-    I = fmaf(p->P11, I, in) + p->w_ext * (float)k;
     if (V >= p->V_th) { spk = true; V = p->V_reset; r = p->refr_steps; }
-    a.V[i] = V; a.I[i] = I; a.refr[i] = r;
+    a.V[i] = V; a.refr[i] = r;
     return spk;
 }
 
-__device__ __forceinline__ void update_phase(const StepArgs& a, const PopDev* __restrict__ P, long long n, long long gtid,
-                                             long long gthreads) {
+__device__ __forceinline__ void neuron_late(const StepArgs& a, const PopDev* __restrict__ P, long long n, int i,
+                                            float* __restrict__ plane, const NeuronRegs& g) {
+    plane[i] = 0.f;
+    if (a.last_input) a.last_input[i] = g.in;
+    if (a.bypass) return;
+    const PopDev* __restrict__ p = P + g.pi;
+    const int k = g.kq != 0xff ? g.kq : poisson_count(a, p, n, i);
+    a.I[i] = fmaf(p->P11, g.I, g.in) + p->w_ext * (float)k;
+}
+
+__device__ __forceinline__ void update_phase(const StepArgs& a, const PopDev* __restrict__ P, long long n, int slot,
+                                             unsigned long long rec_base, long long gtid, long long gthreads) {
     const int N = a.N;
-    const int slot = (int)(n % a.Dr);
     float* __restrict__ plane = a.ring + (size_t)slot * N;
-    int32_t* __restrict__ list = a.spike_list + (size_t)(n & 1) * N;
-    int32_t* cnt = &a.ctl->spike_cnt[n & 3];
     const long long n_round = ((long long)N + 31) & ~31LL;      // keep warps whole for the ballot
     for (long long ii = gtid; ii < n_round; ii += gthreads) {
         const int i = (int)ii;
-        const bool spk = i < N && neuron_step(a, P, n, i, plane);
-        append_spike(spk, i, list, cnt);
+        NeuronRegs g;
+        const bool spk = i < N && neuron_early(a, P, n, i, plane, g);
+        append_spike(a, spk, i, n, rec_base);
+        if (i < N) neuron_late(a, P, n, i, plane, g);
     }
-    if (gtid == 0) a.ctl->step_d = n;
 }
 
 __device__ __forceinline__ void red_add_f32(float* addr, float v) {
@@ -408,59 +497,138 @@ __device__ __forceinline__ uint32_t ld_stream_u32(const void* p) {
     return r;
 }
 
-// Step bookkeeping shared by both delivery kernels (a4): one thread publishes the next step index, clears the
-// other parity's spike counter and advances the record cursor; all threads copy the spike array into the
-// spike record (a2, "all spike times of all neurons recorded").
-__device__ __forceinline__ void bookkeeping_phase(const StepArgs& a, long long n, int M, long long gtid, long long gthreads) {
-    const unsigned long long rec_base = __ldcg(&a.ctl->rec_total[n & 1]);
-    if (a.rec_cap > 0) {
-        const int32_t* __restrict__ list = a.spike_list + (size_t)(n & 1) * a.N;
-        for (long long i = gtid; i < M; i += gthreads) {
-            const unsigned long long pos = rec_base + (unsigned long long)i;
-            if (pos < (unsigned long long)a.rec_cap) { a.rec_id[pos] = __ldcg(list + i); a.rec_step[pos] = (int32_t)n; }
-        }
+// Step bookkeeping of the stand-alone delivery kernels (a4), one thread: publish the next step index, clear the
+// spike counter of the next step and advance the record cursor.  (The spike record itself is written by
+// append_spike.)  Per-step scalars are always read by ONE thread per CTA and broadcast through shared memory:
+// thousands of warps asking the same L2 sector after a barrier serialise on that slice for microseconds.
+__device__ __forceinline__ void bookkeeping_scalar(const StepArgs& a, long long n, int slot, int M, unsigned long long rec_base) {
+    a.ctl->rec_total[(n + 1) & 1] = rec_base + (unsigned long long)M;
+    a.ctl->spike_cnt[(n + 1) & 3] = 0;
+    a.ctl->spikes += (unsigned long long)M;
+    a.ctl->slot = slot + 1 == a.Dr ? 0 : slot + 1;
+    a.ctl->step_u = n + 1;
+}
+
+__device__ __forceinline__ void trace_stamp(const StepArgs& a, long long n, int k, int who = 0) {
+    if (a.trace && (int)threadIdx.x == who) {
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+        a.trace[((size_t)(n % kTraceSteps) * gridDim.x + blockIdx.x) * kTraceStamps + k] = t;
     }
-    if (gtid == 0) {
-        a.ctl->rec_total[(n + 1) & 1] = rec_base + (unsigned long long)M;
-        a.ctl->spike_cnt[(n + 1) & 3] = 0;
-        a.ctl->spikes += (unsigned long long)M;
-        a.ctl->step_u = n + 1;
+}
+// ---------------------------------------------------------------------------------------
+// a3. Spike delivery, kernel 1: row-chunk walk.
+//   The CTA stages the spike array's entries (row start, out-degree, padded length — written by append_spike) in
+//   shared memory, tile by tile, and prefix-sums their chunk counts; the flattened list of
+//   (spike, chunk of kChunkRecords records) items is then dealt round-robin to all warps of the grid: exactly the
+//   existing chunks, no per-warp header loads from global memory.  Lane l reads records [4l, 4l+4) of its chunk
+//   with one 128-bit load of targets, one of weights and one 32-bit load of delays, then issues up to four
+//   red.global.add.f32 into ring[(n + d) mod Dr][target].  Rows are delay-grouped, so consecutive
+//   records mostly hit the same ring plane.
+// ---------------------------------------------------------------------------------------
+constexpr int kEntryTile = 256;
+struct DeliverShared {
+    long long r0[kEntryTile];
+    int32_t len[kEntryTile];
+    int32_t pre[kEntryTile + 1];       // pre[k] = chunks of entries [0, k) of the tile
+    int32_t warp_tot[kEntryTile / 32];
+    int32_t M;
+};
+
+// One item: `kPerLane` records per lane (4: 128-bit loads, 1: 32-bit loads) starting at record q of a row.
+// A scattered red (or store) instruction holds its warp for about one L2 round trip (~0.45 us measured on B200
+// with a quiet memory system), so in the latency regime an item is 32 records — one red per warp — and the
+// items are spread over every warp of the grid; under load 128-record items keep the loads 128-bit wide.
+template <int kPerLane>
+__device__ __forceinline__ void deliver_item(const StepArgs& a, int nmod, long long r0, int len, int c, int lane, int skip = 0) {
+    const int N = a.N, Dr = a.Dr;
+    const int q = (c * 32 + lane) * kPerLane;
+    if (q >= len || q + kPerLane <= skip) return;          // records [0, skip) were delivered by the delay-1 pass
+    const long long p = r0 + q;
+    int s;
+    if (kPerLane == 4) {
+        const int4 t = ld_stream_s32x4(a.tgt + p);
+        const float4 ww = ld_stream_f32x4(a.w + p);
+        const uint32_t dd = ld_stream_u32(a.dly + p);
+        if (t.x >= 0 && q >= skip) { s = nmod + (int)(dd & 0xff); if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * N + t.x, ww.x); }
+        if (t.y >= 0 && q + 1 >= skip) { s = nmod + (int)((dd >> 8) & 0xff); if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * N + t.y, ww.y); }
+        if (t.z >= 0 && q + 2 >= skip) { s = nmod + (int)((dd >> 16) & 0xff); if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * N + t.z, ww.z); }
+        if (t.w >= 0 && q + 3 >= skip) { s = nmod + (int)(dd >> 24); if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * N + t.w, ww.w); }
+    } else {
+        int t; float ww; uint32_t dd;
+        asm("ld.global.nc.L1::no_allocate.s32 %0, [%1];" : "=r"(t) : "l"(a.tgt + p));
+        asm("ld.global.nc.L1::no_allocate.f32 %0, [%1];" : "=f"(ww) : "l"(a.w + p));
+        asm("ld.global.nc.L1::no_allocate.u8 %0, [%1];" : "=r"(dd) : "l"(a.dly + p));
+        if (t >= 0) { s = nmod + (int)dd; if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * N + t, ww); }
     }
 }
 
-// ---------------------------------------------------------------------------------------
-// a3. Spike delivery, kernel 1: row-chunk walk.
-//   work item = (spike index i, chunk c of kChunkRecords records of row(spike i)), chunk fastest, one warp per
-//   item; lane l reads records [4l, 4l+4) of the chunk with one 128-bit load of targets, one of weights and one
-//   32-bit load of delays, then issues up to four red.global.add.f32 into ring[(n + d) mod D][target].
-//   Rows are delay-grouped, so consecutive records mostly hit the same ring plane.
-// ---------------------------------------------------------------------------------------
-__device__ __forceinline__ void deliver_rows_phase(const StepArgs& a, long long n, int M, long long gwarp, long long gwarps,
-                                                   int lane) {
-    const int N = a.N, D = a.D, Dr = a.Dr;
-    const int nmod = (int)(n % Dr);
-    const int32_t* __restrict__ list = a.spike_list + (size_t)(n & 1) * N;
-    const int chunks = a.max_row_chunks;
-    const long long items = (long long)M * chunks;
+// Returns M, the number of spikes of step n.  Thread 0 reads M while the first kEntryTile threads already load the
+// first tile of entries speculatively (one L2 round trip instead of two).
+__device__ __forceinline__ int deliver_rows_phase(const StepArgs& a, long long n, int nmod, DeliverShared& sh) {
+    const int N = a.N;
+    const RowInfo* __restrict__ rows = a.spike_row + (size_t)(n & 1) * N;
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5, wpb = blockDim.x >> 5;
+    const int gwarp = blockIdx.x * wpb + wib, gwarps = gridDim.x * wpb;
+    if (threadIdx.x == 0) sh.M = __ldcg(&a.ctl->spike_cnt[n & 3]);
+    int4 e = make_int4(0, 0, 0, 0);
+    if (threadIdx.x < kEntryTile && threadIdx.x < N) e = __ldcg(reinterpret_cast<const int4*>(rows + threadIdx.x));
+    __syncthreads();
+    const int M = sh.M;
+    // latency regime: about two 32-record items per warp or fewer
+    const bool small = (long long)M * a.mean_row_records <= 64LL * gwarps;
+    const int cshift = small ? 5 : 7;
     unsigned long long ev = 0;
-    for (long long it = gwarp; it < items; it += gwarps) {
-        const int si = (int)(it / chunks), c = (int)(it % chunks);
-        const int j = __ldcg(list + si);
-        const long long r0 = a.row_off[j], r1 = a.row_off[j + 1];
-        if (c == 0 && lane == 0) ev += a.grp_rel[(size_t)j * (D + 1) + D];
-        const long long p = r0 + (long long)c * kChunkRecords + lane * 4;
-        if (p < r1) {
-            const int4 t = ld_stream_s32x4(a.tgt + p);
-            const float4 ww = ld_stream_f32x4(a.w + p);
-            const uint32_t dd = ld_stream_u32(a.dly + p);
-            int s;
-            if (t.x >= 0) { s = nmod + (int)(dd & 0xff); if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * N + t.x, ww.x); }
-            if (t.y >= 0) { s = nmod + (int)((dd >> 8) & 0xff); if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * N + t.y, ww.y); }
-            if (t.z >= 0) { s = nmod + (int)((dd >> 16) & 0xff); if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * N + t.z, ww.z); }
-            if (t.w >= 0) { s = nmod + (int)(dd >> 24); if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * N + t.w, ww.w); }
+    int base_mod = 0;                                          // (flattened index of the tile's first item) mod gwarps
+    for (int tile0 = 0; tile0 < M; tile0 += kEntryTile) {
+        const int m = min(kEntryTile, M - tile0);
+        if (tile0 > 0) {
+            __syncthreads();                                   // previous tile's readers are done
+            if (threadIdx.x < m) e = __ldcg(reinterpret_cast<const int4*>(rows + tile0 + threadIdx.x));
         }
+        if (threadIdx.x < kEntryTile) {                        // first 8 warps: stage entries, scan chunk counts
+            int x = 0;
+            if (threadIdx.x < m) {                             // e = r0 (lo, hi), deg, len
+                sh.r0[threadIdx.x] = (long long)(((unsigned long long)(uint32_t)e.y << 32) | (uint32_t)e.x);
+                const int len = padded_len(e.z);
+                sh.len[threadIdx.x] = len;
+                x = (len + (1 << cshift) - 1) >> cshift;
+                if (blockIdx.x == 0) ev += (unsigned long long)e.z;
+            }
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int y = __shfl_up_sync(0xffffffffu, x, o);
+                if (lane >= o) x += y;
+            }
+            if (lane == 31) sh.warp_tot[wib] = x;
+            e.x = x;                                           // inclusive scan inside the warp
+        }
+        __syncthreads();
+        if (threadIdx.x < kEntryTile) {
+            int off = 0;
+            for (int k = 0; k < wib; ++k) off += sh.warp_tot[k];
+            sh.pre[threadIdx.x + 1] = e.x + off;
+            if (threadIdx.x == 0) sh.pre[0] = 0;
+        }
+        __syncthreads();
+        const int total = sh.pre[m];
+        int first = gwarp - base_mod;                          // items are numbered across tiles: round-robin deal
+        if (first < 0) first += gwarps;
+        for (int it = first; it < total; it += gwarps) {
+            int sidx = 0;                                      // number of k in [1, m] with pre[k] <= it
+            for (int j = 0; j < m; j += 32) {
+                const int k = j + lane + 1;
+                const int v = k <= m ? sh.pre[k] : 0x7fffffff;
+                sidx += __popc(__ballot_sync(0xffffffffu, v <= it));
+            }
+            const int c = it - sh.pre[sidx];
+            if (small) deliver_item<1>(a, nmod, sh.r0[sidx], sh.len[sidx], c, lane);
+            else deliver_item<4>(a, nmod, sh.r0[sidx], sh.len[sidx], c, lane);
+        }
+        base_mod = (int)(((long long)base_mod + total) % gwarps);
     }
     if (ev) atomicAdd(&a.ctl->events, ev);
+    return M;
 }
 
 // ---------------------------------------------------------------------------------------
@@ -501,10 +669,9 @@ __device__ __forceinline__ void red_vec(const StepArgs& a, const VecRef& r, cons
     if (r.q + 3 >= r.rel_lo && r.q + 3 < r.len) red_add_f32(plane + t.w, ww.w);
 }
 
-__device__ __forceinline__ void deliver_groups_phase(const StepArgs& a, long long n, int M, long long gwarp, long long gwarps,
-                                                     int lane) {
+__device__ __forceinline__ void deliver_groups_phase(const StepArgs& a, long long n, int nmod, int M, long long gwarp,
+                                                     long long gwarps, int lane) {
     const int N = a.N, D = a.D, Dr = a.Dr;
-    const int nmod = (int)(n % Dr);
     const int32_t* __restrict__ list = a.spike_list + (size_t)(n & 1) * N;
     const long long items = (long long)M * D;
     if (items == 0) return;
@@ -595,151 +762,287 @@ __device__ __forceinline__ const PopDev* stage_pops(const StepArgs& a, PopDev* s
     return sh;
 }
 
+// Grid barrier of the persistent kernels: one release-arrival per CTA on a counter that only grows, then an
+// acquire-poll by the same thread.  The kernels are launched cooperatively (all CTAs co-resident); the host clears
+// ctl->bar before the launch.  Split in two so that work which needs no other CTA's data (the Poisson counts of
+// the next step) runs between arrival and release — the ~1 us a barrier costs on this part (one L2 round trip to
+// drain the CTA's reductions, one for the arrival, one for the poll) is otherwise idle time.
+__device__ __forceinline__ void grid_arrive(Ctl* ctl, unsigned long long& epoch) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        epoch += gridDim.x;
+        asm volatile("red.release.gpu.global.add.u64 [%0], 1;" ::"l"(&ctl->bar) : "memory");
+    }
+}
+__device__ __forceinline__ void grid_wait(Ctl* ctl, unsigned long long epoch) {
+    if (threadIdx.x == 0) {
+        unsigned long long v;
+        do {
+            asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(&ctl->bar) : "memory");
+        } while (v < epoch);
+    }
+    __syncthreads();
+}
+__device__ __forceinline__ void grid_barrier(Ctl* ctl, unsigned long long& epoch) {
+    grid_arrive(ctl, epoch);
+    grid_wait(ctl, epoch);
+}
+
+struct StepScalars { long long n; unsigned long long rec_base; int M; int slot; };
+constexpr int kPersistentThreads = 1024;
+
 // ---------------------------------------------------------------------------------------
-// a1 + a2 + a3 fused: kernel 3, one kernel per time step (the latency regime: tens of spikes per step).
-//   Every thread updates one neuron; the CTA gathers its own spikes in shared memory (id, row start, padded row
-//   length — the row bounds are fetched by the thread that spiked, so they are in flight while the rest of the CTA
-//   finishes its update), appends them to the global spike array / spike record with ONE atomic per CTA, and then
-//   walks the rows of its own spikes: 128-bit loads of targets and weights, 32-bit loads of delays, two vectors
-//   per thread in flight, red.global.add.f32 into ring[(n + d) mod Dr][target].
-//   No grid-wide dependency exists inside the step (the consumed plane n mod Dr is never a delivery target, see
-//   neuron_step), so a step costs one launch — or one grid barrier in the persistent variant — instead of two.
+// Delivery kernel 4: the pipelined step — ONE grid-wide dependency per time step instead of two.
+//   Only the delay-1 records of a spike of step n must land before update(n+1) starts; every other record
+//   (delay d >= 2, slot n+d) is not consumed before step n+2.  A step is therefore cut differently:
+//     phase n = [ update(n), then the CTA delivers the delay-1 records of ITS OWN spikes ]   (critical path)
+//               || [ the whole grid delivers the delay >= 2 records of the spikes of step n-1 ] (overlapped)
+//     barrier / kernel boundary
+//   The delay-1 records are the first RowInfo.d1 records of a row (rows are delay-grouped) —
+//   ~140-200 of ~3900 in the microcircuit — so the serial part per spike is one 32-record item per warp.
+//   Nothing in a phase reads what the same phase writes: update(n) consumes plane n mod Dr, the delay-1 pass
+//   writes plane n+1, the rest pass of step n-1 writes planes n+1 .. n-1+D (Dr = D + 1 planes).
+//   The spike record of step n-1 is written by CTA 0 during the rest pass (coalesced, off the critical path).
 // ---------------------------------------------------------------------------------------
-constexpr int kFusedThreads = 256;
-struct FusedShared {
+constexpr int kD1Cap = 1024;
+struct PipeShared {
     PopDev pops[kMaxPopsSmem];
-    long long r0[kFusedThreads];
-    int32_t len[kFusedThreads];
-    int32_t id[kFusedThreads];
-    int32_t cnt, gbase;
+    DeliverShared d;
+    int32_t skip[kEntryTile];
+    long long d1_r0[kD1Cap];
+    int32_t d1_cnt[kD1Cap];
+    int32_t n_d1;
+    StepScalars sc;
+    int32_t pending;
 };
 
-__device__ __forceinline__ void red_rec4(const StepArgs& a, int nmod, const int4& t, const float4& ww, uint32_t dd) {
-    const int N = a.N, Dr = a.Dr;
-    int s;
-    if (t.x >= 0) { s = nmod + (int)(dd & 0xff); if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * N + t.x, ww.x); }
-    if (t.y >= 0) { s = nmod + (int)((dd >> 8) & 0xff); if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * N + t.y, ww.y); }
-    if (t.z >= 0) { s = nmod + (int)((dd >> 16) & 0xff); if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * N + t.z, ww.z); }
-    if (t.w >= 0) { s = nmod + (int)(dd >> 24); if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * N + t.w, ww.w); }
-}
-
-__device__ __forceinline__ void fused_phase(const StepArgs& a, const PopDev* __restrict__ P, long long n,
-                                            unsigned long long rec_base, FusedShared& sh) {
-    const int N = a.N, D = a.D;
-    const int nmod = (int)(n % a.Dr);
-    float* __restrict__ plane = a.ring + (size_t)nmod * N;
-    int32_t* __restrict__ list = a.spike_list + (size_t)(n & 1) * N;
-    const int lane = threadIdx.x & 31;
-    unsigned long long ev = 0;
-    for (long long base = (long long)blockIdx.x * kFusedThreads; base < N; base += (long long)gridDim.x * kFusedThreads) {
-        __syncthreads();                                   // previous round's readers of sh are done
-        if (threadIdx.x == 0) sh.cnt = 0;
-        __syncthreads();
-        const long long ii = base + threadIdx.x;
-        const int i = (int)ii;
-        const bool spk = ii < N && neuron_step(a, P, n, i, plane);
-        const unsigned m = __ballot_sync(0xffffffffu, spk);
-        if (m) {                                           // warp-aggregated append to the CTA's list
-            const int leader = __ffs(m) - 1;
-            int b = 0;
-            if (lane == leader) b = atomicAdd(&sh.cnt, __popc(m));
-            b = __shfl_sync(0xffffffffu, b, leader);
-            if (spk) {
-                const int k = b + __popc(m & ((1u << lane) - 1u));
-                const long long r0 = a.row_off[i], r1 = a.row_off[i + 1];
-                sh.id[k] = i; sh.r0[k] = r0; sh.len[k] = (int)(r1 - r0);
-                ev += a.grp_rel[(size_t)i * (D + 1) + D];
-            }
-        }
-        __syncthreads();
-        const int Ml = sh.cnt;
-        if (Ml == 0) continue;                             // uniform over the CTA
-        if (threadIdx.x == 0) sh.gbase = atomicAdd(&a.ctl->spike_cnt[n & 3], Ml);
-        for (int s = 0; s < Ml; ++s) {                     // a3: walk the rows of this CTA's spikes
-            const long long r0 = sh.r0[s];
-            const int len = sh.len[s];
-            for (int p = threadIdx.x * 4; p < len; p += kFusedThreads * 8) {
-                const int q = p + kFusedThreads * 4;
-                const int4 t0 = ld_stream_s32x4(a.tgt + r0 + p);
-                const float4 w0 = ld_stream_f32x4(a.w + r0 + p);
-                const uint32_t d0 = ld_stream_u32(a.dly + r0 + p);
-                int4 t1 = make_int4(-1, -1, -1, -1); float4 w1 = make_float4(0.f, 0.f, 0.f, 0.f); uint32_t d1 = 0;
-                if (q < len) { t1 = ld_stream_s32x4(a.tgt + r0 + q); w1 = ld_stream_f32x4(a.w + r0 + q); d1 = ld_stream_u32(a.dly + r0 + q); }
-                red_rec4(a, nmod, t0, w0, d0);
-                red_rec4(a, nmod, t1, w1, d1);
-            }
-        }
-        __syncthreads();                                   // sh.gbase
-        const int gb = sh.gbase;
-        for (int k = threadIdx.x; k < Ml; k += kFusedThreads) {    // a2: spike array and spike record
-            const int id = sh.id[k];
-            list[gb + k] = id;
-            const unsigned long long pos = rec_base + (unsigned long long)(gb + k);
-            if (pos < (unsigned long long)a.rec_cap) { a.rec_id[pos] = id; a.rec_step[pos] = (int32_t)n; }
-        }
+__device__ __forceinline__ void deliver_d1_piece(const StepArgs& a, float* __restrict__ plane1, long long r0, int cnt, int q) {
+    if (q < cnt) {
+        int t; float ww;
+        asm("ld.global.nc.L1::no_allocate.s32 %0, [%1];" : "=r"(t) : "l"(a.tgt + r0 + q));
+        asm("ld.global.nc.L1::no_allocate.f32 %0, [%1];" : "=f"(ww) : "l"(a.w + r0 + q));
+        red_add_f32(plane1 + t, ww);
     }
-    if (ev) atomicAdd(&a.ctl->events, ev);
 }
 
-// One launch = one time step.  The last CTA to finish publishes the next step index (a4).
-__global__ void __launch_bounds__(kFusedThreads) fused_step_kernel(const StepArgs a) {
-    __shared__ FusedShared sh;
-    const long long n = __ldcg(&a.ctl->step_u);
-    const unsigned long long rec_base = __ldcg(&a.ctl->rec_total[n & 1]);
-    const PopDev* P = stage_pops(a, sh.pops);
-    fused_phase(a, P, n, rec_base, sh);
+// Warp-specialised: the last `rest_threads` threads of the CTA run the rest pass of step n-1 while the others run
+// update(n) and the delay-1 pass, each group synchronising on its own named barrier.
+// Returns M_{n-1} (0 if nothing was pending).  `rec_prev` = spikes recorded before step n-1.
+__device__ __forceinline__ void group_sync(int id, int count) {
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory");
+}
+__device__ __forceinline__ int pipe_rest_threads() { return blockDim.x >= 512 ? kEntryTile : 64; }
+
+template <bool kUpdate>
+__device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* __restrict__ P, long long n, int slot, bool pending,
+                                               unsigned long long rec_prev, PipeShared& sh, bool have_k = false) {
+    const int N = a.N, Dr = a.Dr;
+    const int lane = threadIdx.x & 31;
+    const int R = pipe_rest_threads(), U = blockDim.x - R;         // rest group = threads [U, U + R)
+    if (threadIdx.x == 0) sh.n_d1 = 0;
+    if (threadIdx.x == U && !pending) sh.d.M = 0;
     __syncthreads();
+
+    if ((int)threadIdx.x < U) {
+        // ---- update(n), spike collection, then the delay-1 records of this CTA's spikes ----
+        if (kUpdate) {
+            const int wib = threadIdx.x >> 5, wpu = U >> 5;
+            float* __restrict__ plane = a.ring + (size_t)slot * N;
+            float* __restrict__ plane1 = a.ring + (size_t)(slot + 1 == Dr ? 0 : slot + 1) * N;
+            for (long long base = (long long)blockIdx.x * U; base < N; base += (long long)gridDim.x * U) {
+                const long long ii = base + threadIdx.x;
+                const int i = (int)ii;
+                NeuronRegs g;
+                const bool spk = ii < N && neuron_early(a, P, n, i, plane, g, have_k);
+                const unsigned m = __ballot_sync(0xffffffffu, spk);
+                if (m) {
+                    const int leader = __ffs(m) - 1;
+                    int gb = 0, lb = 0;
+                    if (lane == leader) { gb = atomicAdd(&a.ctl->spike_cnt[n & 3], __popc(m)); lb = atomicAdd(&sh.n_d1, __popc(m)); }
+                    RowInfo r;
+                    if (spk) { r = ld_row_info(a.row_info + i); if (a.prefetch) prefetch_row(a, r); }
+                    gb = __shfl_sync(0xffffffffu, gb, leader);
+                    lb = __shfl_sync(0xffffffffu, lb, leader);
+                    if (spk) {
+                        const int rank = __popc(m & ((1u << lane) - 1u));
+                        const size_t k = (size_t)(n & 1) * N + gb + rank;
+                        a.spike_list[k] = i;
+                        st_row_info(a.spike_row + k, r);
+                        if (lb + rank < kD1Cap) { sh.d1_r0[lb + rank] = r.r0; sh.d1_cnt[lb + rank] = r.d1; }
+                        else for (int q = 0; q < r.d1; ++q) deliver_d1_piece(a, plane1, r.r0, r.d1, q);   // list full: serial
+                    }
+                }
+                if (ii < N) neuron_late(a, P, n, i, plane, g);
+            }
+            trace_stamp(a, n, 3);
+            group_sync(1, U);
+            trace_stamp(a, n, 4);
+            const int nd1 = min(sh.n_d1, kD1Cap);
+            for (int s = 0; s < nd1; ++s) {
+                const long long r0 = sh.d1_r0[s];
+                const int cnt = sh.d1_cnt[s];
+                for (int q = wib * 32 + lane; q < cnt; q += wpu * 32) deliver_d1_piece(a, plane1, r0, cnt, q);
+            }
+            trace_stamp(a, n, 6);
+        }
+    } else if (pending) {
+        // ---- rest pass of step n-1: records [d1, deg) of every spike, dealt to the rest warps of the whole grid ----
+        const int t = threadIdx.x - U;                             // index inside the rest group
+        const int wir = t >> 5, wpr = R >> 5;
+        const int gwarp = blockIdx.x * wpr + wir, gwarps = gridDim.x * wpr;
+        const long long np = n - 1;
+        const RowInfo* __restrict__ rows_prev = a.spike_row + (size_t)(np & 1) * N;
+        const int32_t* __restrict__ list_prev = a.spike_list + (size_t)(np & 1) * N;
+        const bool rec_cta = blockIdx.x == 0 && a.rec_cap > 0;
+        if (t == 0) sh.d.M = __ldcg(&a.ctl->spike_cnt[np & 3]);
+        int4 e = make_int4(0, 0, 0, 0);
+        int id_prev = 0;
+        if (t < N) {                                               // speculative: the first tile, before M is known
+            e = __ldcg(reinterpret_cast<const int4*>(rows_prev + t));
+            if (rec_cta) id_prev = __ldcg(list_prev + t);
+        }
+        group_sync(2, R);
+        trace_stamp(a, n, 7, U);
+        const int M = sh.d.M;
+        const int nmod = slot == 0 ? Dr - 1 : slot - 1;             // (n - 1) mod Dr
+        const bool small = (long long)M * a.mean_row_records <= 64LL * gwarps;
+        const int cshift = small ? 5 : 7;
+        unsigned long long ev = 0;
+        int base_mod = 0;
+        for (int tile0 = 0; tile0 < M; tile0 += R) {
+            const int m = min(R, M - tile0);
+            if (tile0 > 0) {
+                group_sync(2, R);
+                if (t < m) {
+                    e = __ldcg(reinterpret_cast<const int4*>(rows_prev + tile0 + t));
+                    if (rec_cta) id_prev = __ldcg(list_prev + tile0 + t);
+                }
+            }
+            int x = 0;
+            if (t < m) {                                           // e = r0 (lo, hi), deg, d1
+                const int len = padded_len(e.z);
+                sh.d.r0[t] = (long long)(((unsigned long long)(uint32_t)e.y << 32) | (uint32_t)e.x);
+                sh.d.len[t] = len;
+                sh.skip[t] = e.w;
+                x = (len + (1 << cshift) - 1) >> cshift;
+                if (blockIdx.x == 0) ev += (unsigned long long)e.z;
+                if (rec_cta) {
+                    const unsigned long long pos = rec_prev + (unsigned long long)(tile0 + t);
+                    if (pos < (unsigned long long)a.rec_cap) { a.rec_id[pos] = id_prev; a.rec_step[pos] = (int32_t)np; }
+                }
+            }
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int y = __shfl_up_sync(0xffffffffu, x, o);
+                if (lane >= o) x += y;
+            }
+            if (lane == 31) sh.d.warp_tot[wir] = x;
+            group_sync(2, R);
+            int off = 0;
+            for (int k = 0; k < wir; ++k) off += sh.d.warp_tot[k];
+            sh.d.pre[t + 1] = x + off;
+            if (t == 0) sh.d.pre[0] = 0;
+            group_sync(2, R);
+            trace_stamp(a, n, 8, U);
+            const int total = sh.d.pre[m];
+            int first = gwarp - base_mod;
+            if (first < 0) first += gwarps;
+            for (int it = first; it < total; it += gwarps) {
+                int sidx = 0;
+                for (int j = 0; j < m; j += 32) {
+                    const int k = j + lane + 1;
+                    const int v = k <= m ? sh.d.pre[k] : 0x7fffffff;
+                    sidx += __popc(__ballot_sync(0xffffffffu, v <= it));
+                }
+                const int c = it - sh.d.pre[sidx];
+                if (small) deliver_item<1>(a, nmod, sh.d.r0[sidx], sh.d.len[sidx], c, lane, sh.skip[sidx]);
+                else deliver_item<4>(a, nmod, sh.d.r0[sidx], sh.d.len[sidx], c, lane, sh.skip[sidx]);
+            }
+            base_mod = (int)(((long long)base_mod + total) % gwarps);
+        }
+        trace_stamp(a, n, 9, U);
+        if (ev) atomicAdd(&a.ctl->events, ev);
+    }
+    __syncthreads();
+    return sh.d.M;
+}
+
+// Graph / plain-launch form: one launch per time step, the kernel boundary is the barrier.  The last CTA to finish
+// publishes the next step index (a4) and marks the rest pass of this step as pending.
+constexpr int kPipeThreads = 512;        // 256 updaters + 256 rest-pass threads
+template <bool kUpdate>
+__global__ void __launch_bounds__(kPipeThreads) pipe_step_kernel(const StepArgs a) {
+    __shared__ PipeShared sh;
+    if (threadIdx.x == 0) {
+        sh.sc.n = __ldcg(&a.ctl->step_u);
+        sh.sc.slot = __ldcg(&a.ctl->slot);
+        sh.pending = __ldcg(&a.ctl->pending);
+        sh.sc.rec_base = __ldcg(&a.ctl->rec_total[(sh.sc.n - 1) & 1]);     // recorded before step n-1
+    }
+    const PopDev* P = stage_pops(a, sh.pops);
+    if (a.n_pops > kMaxPopsSmem) __syncthreads();
+    const long long n = sh.sc.n;
+    const int slot = sh.sc.slot;
+    pipelined_phase<kUpdate>(a, P, n, slot, sh.pending != 0, sh.sc.rec_base, sh);
     if (threadIdx.x == 0) {
         __threadfence();
         const unsigned t = atomicAdd(&a.ctl->ticket, 1u);
         if (t == gridDim.x - 1) {
             __threadfence();
-            const int M = __ldcg(&a.ctl->spike_cnt[n & 3]);
-            a.ctl->rec_total[(n + 1) & 1] = rec_base + (unsigned long long)M;
-            a.ctl->spike_cnt[(n + 1) & 3] = 0;
-            a.ctl->spikes += (unsigned long long)M;
             a.ctl->ticket = 0;
-            a.ctl->step_d = n;
-            a.ctl->step_u = n + 1;
+            if (kUpdate) {
+                const int M = __ldcg(&a.ctl->spike_cnt[n & 3]);
+                a.ctl->rec_total[(n + 1) & 1] = __ldcg(&a.ctl->rec_total[n & 1]) + (unsigned long long)M;
+                a.ctl->spike_cnt[(n + 1) & 3] = 0;
+                a.ctl->spikes += (unsigned long long)M;
+                a.ctl->step_d = n;
+                a.ctl->slot = slot + 1 == a.Dr ? 0 : slot + 1;
+                a.ctl->step_u = n + 1;
+                a.ctl->pending = 1;
+            } else a.ctl->pending = 0;                             // flush launch: rest pass of step n-1 done
         }
     }
 }
 
-// Grid barrier of the persistent fused kernel: one atomic arrival per CTA on a counter that only grows, then a
-// poll.  The kernel is launched cooperatively (all CTAs co-resident); the host clears ctl->bar before the launch.
-__device__ __forceinline__ void grid_barrier(Ctl* ctl, unsigned long long& epoch) {
-    __syncthreads();
+__global__ void __launch_bounds__(kPersistentThreads, 1) persistent_pipe_kernel(const StepArgs a, long long n_steps) {
+    __shared__ PipeShared sh;
     if (threadIdx.x == 0) {
-        epoch += gridDim.x;
-        __threadfence();
-        atomicAdd(&ctl->bar, 1ULL);
-        unsigned long long v;
-        do {
-            asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(&ctl->bar) : "memory");
-        } while (v < epoch);
-        __threadfence();
+        sh.sc.n = __ldcg(&a.ctl->step_u);
+        sh.sc.slot = __ldcg(&a.ctl->slot);
+        sh.sc.rec_base = __ldcg(&a.ctl->rec_total[sh.sc.n & 1]);
     }
-    __syncthreads();
-}
-
-__global__ void __launch_bounds__(kFusedThreads) persistent_fused_kernel(const StepArgs a, long long n_steps) {
-    __shared__ FusedShared sh;
-    long long n = __ldcg(&a.ctl->step_u);
-    unsigned long long rec_base = __ldcg(&a.ctl->rec_total[n & 1]);
-    unsigned long long epoch = 0, spikes = 0;
     const PopDev* P = stage_pops(a, sh.pops);
+    if (a.n_pops > kMaxPopsSmem) __syncthreads();
+    const long long gtid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int U = blockDim.x - pipe_rest_threads();
+    long long n = sh.sc.n;
+    int slot = sh.sc.slot;
+    unsigned long long rec_prev = sh.sc.rec_base, spikes = 0, epoch = 0;       // recorded before step n-1 (nothing pending at entry)
     for (long long s = 0; s < n_steps; ++s, ++n) {
-        // the counter of step n+1 was last read (as step n-3's) long before the previous barrier
-        if (blockIdx.x == 0 && threadIdx.x == 0) a.ctl->spike_cnt[(n + 1) & 3] = 0;
-        fused_phase(a, P, n, rec_base, sh);
-        grid_barrier(a.ctl, epoch);
-        const unsigned long long M = (unsigned long long)__ldcg(&a.ctl->spike_cnt[n & 3]);
-        rec_base += M; spikes += M;
+        if (gtid == 0) a.ctl->spike_cnt[(n + 1) & 3] = 0;          // last read (as step n-3's) in phase n-2
+        trace_stamp(a, n, 0);
+        const int Mp = pipelined_phase<true>(a, P, n, slot, s > 0, rec_prev, sh, s > 0);
+        rec_prev += (unsigned long long)Mp; spikes += (unsigned long long)Mp;
+        trace_stamp(a, n, 1);
+        grid_arrive(a.ctl, epoch);
+        if (s + 1 < n_steps && !a.bypass && (int)threadIdx.x < U) {        // barrier shadow: Poisson counts of step n+1
+            for (long long ii = (long long)blockIdx.x * U + threadIdx.x; ii < a.N; ii += (long long)gridDim.x * U)
+                a.pois_k[ii] = (uint8_t)poisson_count(a, P + a.pop_of[ii], n + 1, (int)ii);
+        }
+        grid_wait(a.ctl, epoch);
+        trace_stamp(a, n, 2);
+        slot = slot + 1 == a.Dr ? 0 : slot + 1;
     }
-    if (blockIdx.x == 0 && threadIdx.x == 0) {             // nobody reads these words any more in this launch
-        a.ctl->rec_total[n & 1] = rec_base;
+    if (n_steps > 0) {                                             // flush: rest pass of the last step
+        const int Mp = pipelined_phase<false>(a, P, n, slot, true, rec_prev, sh);
+        rec_prev += (unsigned long long)Mp; spikes += (unsigned long long)Mp;
+    }
+    if (gtid == 0) {
+        a.ctl->rec_total[n & 1] = rec_prev;
+        a.ctl->rec_total[(n - 1) & 1] = rec_prev;
         a.ctl->spikes += spikes;
         a.ctl->step_d = n - 1;
+        a.ctl->slot = slot;
         a.ctl->step_u = n;
     }
 }
@@ -747,41 +1050,85 @@ __global__ void __launch_bounds__(kFusedThreads) persistent_fused_kernel(const S
 // ------------------------------- stand-alone kernels ---------------------------------
 __global__ void __launch_bounds__(kUpdateThreads) update_kernel(const StepArgs a) {
     __shared__ PopDev sh_pops[kMaxPopsSmem];
-    const long long n = __ldcg(&a.ctl->step_u);
-    const PopDev* P = stage_pops(a, sh_pops);
-    update_phase(a, P, n, (long long)blockIdx.x * blockDim.x + threadIdx.x, (long long)gridDim.x * blockDim.x);
+    __shared__ StepScalars sc;
+    if (threadIdx.x == 0) {
+        sc.n = __ldcg(&a.ctl->step_u);
+        sc.slot = __ldcg(&a.ctl->slot);
+        sc.rec_base = __ldcg(&a.ctl->rec_total[sc.n & 1]);
+        if (blockIdx.x == 0) a.ctl->step_d = sc.n;
+    }
+    const PopDev* P = stage_pops(a, sh_pops);              // contains the __syncthreads that publishes sc
+    if (a.n_pops > kMaxPopsSmem) __syncthreads();
+    update_phase(a, P, sc.n, sc.slot, sc.rec_base, (long long)blockIdx.x * blockDim.x + threadIdx.x, (long long)gridDim.x * blockDim.x);
 }
 
 template <int kKernel>
 __global__ void __launch_bounds__(kDeliverThreads) deliver_kernel(const StepArgs a) {
-    const long long n = __ldcg(&a.ctl->step_d);
-    const int M = __ldcg(&a.ctl->spike_cnt[n & 3]);
+    __shared__ DeliverShared sh;
+    __shared__ StepScalars sc;
+    if (threadIdx.x == 0) {
+        sc.n = __ldcg(&a.ctl->step_d);
+        sc.slot = __ldcg(&a.ctl->slot);
+        if (kKernel != 1) sc.M = __ldcg(&a.ctl->spike_cnt[sc.n & 3]);
+    }
+    __syncthreads();
     const long long gtid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const long long gthreads = (long long)gridDim.x * blockDim.x;
-    if (kKernel == 1) deliver_rows_phase(a, n, M, gtid >> 5, gthreads >> 5, threadIdx.x & 31);
-    else deliver_groups_phase(a, n, M, gtid >> 5, gthreads >> 5, threadIdx.x & 31);
-    bookkeeping_phase(a, n, M, gtid, gthreads);
+    int M;
+    if (kKernel == 1) M = deliver_rows_phase(a, sc.n, sc.slot, sh);
+    else { M = sc.M; deliver_groups_phase(a, sc.n, sc.slot, M, gtid >> 5, gthreads >> 5, threadIdx.x & 31); }
+    if (gtid == 0) bookkeeping_scalar(a, sc.n, sc.slot, M, __ldcg(&a.ctl->rec_total[sc.n & 1]));
 }
 
-// One persistent cooperative kernel for n_steps steps: the two phases separated by grid-wide barriers instead of
-// kernel boundaries (the per-step work of the microcircuit is a few microseconds).
+// One persistent cooperative kernel for n_steps steps: the two phases separated by grid-wide barriers (grid_barrier)
+// instead of kernel boundaries (the per-step work of the microcircuit is a few microseconds).
+// One CTA per SM keeps the number of barrier arrivals (atomics on one address) at the SM count.
 template <int kKernel>
-__global__ void __launch_bounds__(kUpdateThreads) persistent_kernel(const StepArgs a, long long n_steps) {
-    cg::grid_group grid = cg::this_grid();
+__global__ void __launch_bounds__(kPersistentThreads, 1) persistent_kernel(const StepArgs a, long long n_steps) {
     const long long gtid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const long long gthreads = (long long)gridDim.x * blockDim.x;
     __shared__ PopDev sh_pops[kMaxPopsSmem];
+    __shared__ DeliverShared sh;
+    __shared__ StepScalars sc;
+    if (threadIdx.x == 0) {
+        sc.n = __ldcg(&a.ctl->step_u);
+        sc.slot = __ldcg(&a.ctl->slot);
+        sc.rec_base = __ldcg(&a.ctl->rec_total[sc.n & 1]);
+    }
     const PopDev* P = stage_pops(a, sh_pops);
-    long long n = __ldcg(&a.ctl->step_u);
-    grid.sync();                                   // everyone has read step_u before anyone moves it
+    if (a.n_pops > kMaxPopsSmem) __syncthreads();
+    long long n = sc.n;
+    int slot = sc.slot;
+    unsigned long long rec_base = sc.rec_base, spikes = 0, epoch = 0;
     for (long long s = 0; s < n_steps; ++s, ++n) {
-        update_phase(a, P, n, gtid, gthreads);
-        grid.sync();
-        const int M = __ldcg(&a.ctl->spike_cnt[n & 3]);
-        if (kKernel == 1) deliver_rows_phase(a, n, M, gtid >> 5, gthreads >> 5, threadIdx.x & 31);
-        else deliver_groups_phase(a, n, M, gtid >> 5, gthreads >> 5, threadIdx.x & 31);
-        bookkeeping_phase(a, n, M, gtid, gthreads);
-        grid.sync();
+        // the counter of step n+1 was last read (as step n-3's) before the barriers of step n-1
+        if (gtid == 0) a.ctl->spike_cnt[(n + 1) & 3] = 0;
+        trace_stamp(a, n, 0);
+        update_phase(a, P, n, slot, rec_base, gtid, gthreads);
+        trace_stamp(a, n, 1);
+        grid_barrier(a.ctl, epoch);
+        trace_stamp(a, n, 2);
+        int M;
+        if (kKernel == 1) M = deliver_rows_phase(a, n, slot, sh);
+        else {
+            if (threadIdx.x == 0) sc.M = __ldcg(&a.ctl->spike_cnt[n & 3]);
+            __syncthreads();
+            M = sc.M;
+            deliver_groups_phase(a, n, slot, M, gtid >> 5, gthreads >> 5, threadIdx.x & 31);
+            __syncthreads();                               // sc.M is rewritten next step
+        }
+        rec_base += (unsigned long long)M; spikes += (unsigned long long)M;
+        trace_stamp(a, n, 3);
+        grid_barrier(a.ctl, epoch);
+        trace_stamp(a, n, 5);
+        slot = slot + 1 == a.Dr ? 0 : slot + 1;
+    }
+    if (gtid == 0) {                                       // nobody reads these words any more in this launch
+        a.ctl->rec_total[n & 1] = rec_base;
+        a.ctl->spikes += spikes;
+        a.ctl->step_d = n - 1;
+        a.ctl->slot = slot;
+        a.ctl->step_u = n;
     }
 }
 

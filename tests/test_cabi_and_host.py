@@ -40,7 +40,7 @@ def test_struct_layouts_match_header():
             printf("%zu %zu %zu %zu\n", offsetof(ng_config, seed), offsetof(ng_config, device), offsetof(ng_stats, build_ms), offsetof(ng_stats, delivery_kernel));
             printf("%d %d %d %d %d %d\n", NG_OK, NG_ERR_INVALID_ARG, NG_ERR_STATE, NG_ERR_OOM, NG_ERR_CUDA, NG_ERR_OVERFLOW);
             printf("%d %d %d %d %d %d\n", NG_FIELD_V, NG_FIELD_I_SYN, NG_FIELD_REFR, NG_FIELD_RING, NG_FIELD_STEP, NG_FIELD_LAST_INPUT);
-            printf("%d %d %d %d %d %d %d\n", NG_OPT_STEP_MODE, NG_OPT_STEPS_PER_GRAPH, NG_OPT_DELIVERY_KERNEL, NG_OPT_DELIVER_BLOCKS, NG_OPT_PROFILE, NG_OPT_ASYNC, NG_OPT_SORT_SEGMENTS);
+            printf("%d %d %d %d %d %d %d %d %d %d\n", NG_OPT_STEP_MODE, NG_OPT_STEPS_PER_GRAPH, NG_OPT_DELIVERY_KERNEL, NG_OPT_DELIVER_BLOCKS, NG_OPT_PROFILE, NG_OPT_ASYNC, NG_OPT_SORT_SEGMENTS, NG_OPT_PREFETCH, NG_OPT_TRACE, NG_OPT_PERSISTENT_THREADS);
             return 0;
         }''')
     import tempfile
@@ -56,7 +56,7 @@ def test_struct_layouts_match_header():
     assert list(map(int, out[2].split())) == [B.NG_OK, B.NG_ERR_INVALID_ARG, B.NG_ERR_STATE, B.NG_ERR_OOM, B.NG_ERR_CUDA, B.NG_ERR_OVERFLOW]
     assert list(map(int, out[3].split())) == [B.FIELD_V, B.FIELD_I_SYN, B.FIELD_REFR, B.FIELD_RING, B.FIELD_STEP, B.FIELD_LAST_INPUT]
     assert list(map(int, out[4].split())) == [B.OPT_STEP_MODE, B.OPT_STEPS_PER_GRAPH, B.OPT_DELIVERY_KERNEL, B.OPT_DELIVER_BLOCKS,
-                                              B.OPT_PROFILE, B.OPT_ASYNC, B.OPT_SORT_SEGMENTS]
+                                              B.OPT_PROFILE, B.OPT_ASYNC, B.OPT_SORT_SEGMENTS, B.OPT_PREFETCH, B.OPT_TRACE, B.OPT_PERSISTENT_THREADS]
 
 
 def test_argument_validation_without_a_gpu():

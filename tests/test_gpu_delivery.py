@@ -34,6 +34,7 @@ def ring_mass(o, wl, oracle_mod, n_steps, spikes_by_step):
     (100, 0.05, 1, 0), (100, 0.05, 2, 0), (100, 0.01, 2, 2), (1000, 0.01, 1, 0), (1000, 0.01, 2, 0),
     (1000, 0.05, 2, 1), (1000, 0.002, 2, 2), (1000, 0.002, 1, 2), (37, 0.03, 2, 0), (3, 0.5, 2, 0),
     (100, 0.05, 3, 0), (1000, 0.01, 3, 1), (1000, 0.002, 3, 2), (37, 0.03, 3, 2), (3, 0.5, 3, 0), (1500, 0.3, 3, 0),
+    (1500, 0.3, 3, 2), (1000, 0.05, 1, 0),
 ])
 def test_delivery_only_matches_oracle(oracle_mod, B, K, fraction, kernel, mode):
     n, steps = 20000, 70                       # 70 > D = 64: the ring wraps
