@@ -262,29 +262,40 @@ def run_ours(args):
         g.close()
         return
 
-    # ---- roofline of the dominant kernel: per-kernel CUDA-event times over the same number of time steps ----
-    g.set_option(B.OPT_PROFILE, 1)
-    p0 = g.stats()
-    g.simulate(args.steps * T, allow_overflow=True)
-    p1 = g.stats()
-    g.set_option(B.OPT_PROFILE, 0)
-    n_launch = args.steps * T
-    us_upd = (p1.ms_update - p0.ms_update) * 1e3 / n_launch
-    us_del = (p1.ms_deliver - p0.ms_deliver) * 1e3 / n_launch
-    ev_per_launch = (p1.events - p0.events) / n_launch
-    if int(p1.delivery_kernel) == 3:          # pipelined step kernel: update + collection + delivery in one launch
-        kern, alg_bytes, us = "pipe_step_kernel", N * BYTES_PER_NEURON_STEP + ev_per_launch * BYTES_PER_EVENT, us_upd
-    elif us_del >= us_upd:
-        kern, alg_bytes, us = f"deliver_kernel<{int(p1.delivery_kernel)}>", ev_per_launch * BYTES_PER_EVENT, us_del
+    # ---- roofline of the dominant kernel ----
+    if int(s1.step_mode) == 2:
+        # one persistent kernel per bench step: its launch IS the timed region (CUDA events on the simulator's stream)
+        kern = {1: "persistent_kernel<1>", 2: "persistent_kernel<2>", 3: "persistent_pipe_kernel"}[int(s1.delivery_kernel)]
+        us = ms_total * 1e3 / args.steps
+        ev_per_launch = float(s1.events - s0.events) / args.steps
+        alg_bytes = T * N * BYTES_PER_NEURON_STEP + ev_per_launch * BYTES_PER_EVENT
+        share = {"persistent_kernel_share_of_step": 1.0, "time_steps_per_launch": T}
     else:
-        kern, alg_bytes, us = "update_kernel", N * BYTES_PER_NEURON_STEP, us_upd
+        # per-kernel CUDA-event times (NG_OPT_PROFILE, plain launches) over the same number of time steps
+        g.set_option(B.OPT_PROFILE, 1)
+        p0 = g.stats()
+        g.simulate(args.steps * T, allow_overflow=True)
+        p1 = g.stats()
+        g.set_option(B.OPT_PROFILE, 0)
+        n_launch = args.steps * T
+        us_upd = (p1.ms_update - p0.ms_update) * 1e3 / n_launch
+        us_del = (p1.ms_deliver - p0.ms_deliver) * 1e3 / n_launch
+        ev_per_launch = (p1.events - p0.events) / n_launch
+        if int(p1.delivery_kernel) == 3:          # pipelined step kernel: update + collection + delivery in one launch
+            kern, alg_bytes, us = "pipe_step_kernel", N * BYTES_PER_NEURON_STEP + ev_per_launch * BYTES_PER_EVENT, us_upd
+        elif us_del >= us_upd:
+            kern, alg_bytes, us = f"deliver_kernel<{int(p1.delivery_kernel)}>", ev_per_launch * BYTES_PER_EVENT, us_del
+        else:
+            kern, alg_bytes, us = "update_kernel", N * BYTES_PER_NEURON_STEP, us_upd
+        share = {"update_kernel_us": us_upd, "deliver_kernel_us": us_del}
     achieved = alg_bytes / (us * 1e-6) / 1e9
     roofline = {"bound": "hbm", "kernel": kern, "achieved": achieved, "peak": peak_gbs, "unit": "GB/s",
                 "frac": achieved / peak_gbs, "traffic": None, "peak_source": peak_src,
                 "avg_launch_us": us, "algorithmic_bytes_per_launch": alg_bytes,
-                "share_of_step": {"update_kernel_us": us_upd, "deliver_kernel_us": us_del},
-                "note": "latency-bound regime: ~1e5 events (0.8 MB) per launch; see delivery_microbench for the "
-                        "bandwidth-relevant load and DESIGN.md for the scattered-RED ceiling"}
+                "share_of_step": share,
+                "note": "latency-bound regime: ~1e5 events (0.8 MB) + 2.5 MB of neuron state per time step against "
+                        "~5 us of dependent memory round trips and one grid barrier; see delivery_microbench for the "
+                        "bandwidth-relevant load and DESIGN.md for the L2 tag-rate ceiling of scattered reductions"}
     g.close()
     del g
     torch.cuda.empty_cache()
@@ -302,7 +313,7 @@ def run_ours(args):
                    "l2": "no flush: 2.7 GB of connection records (>> 126 MB L2) read by data-dependent rows; neuron "
                          "state and ring stay resident as in any long simulation",
                    "step_mode": {0: "cuda graph, 100 time steps per graph", 1: "plain launches",
-                                 2: "one persistent cooperative kernel per ng_simulate call"}[args.step_mode],
+                                 2: "one persistent cooperative kernel per ng_simulate call"}[int(s1.step_mode)],
                    "delivery_kernel": int(s1.delivery_kernel), "seed": wl.seed},
         "synaptic_events_per_s": events / (ms_total * 1e-3), "spikes_per_time_step": spikes / (args.steps * T * world),
         "mean_rate_hz": spikes / world / N / bio_s, "us_per_time_step": ms_total * 1e3 / (args.steps * T),
@@ -396,7 +407,7 @@ def main():
     ap.add_argument("--only-microbench", action="store_true",
                     help="run only the configs[3] delivery microbenchmark and print its JSON object (used for ncu captures)")
     ap.add_argument("--probe", action="store_true", help="run the ceiling probes (ng_probe) and print them as JSON")
-    ap.add_argument("--step-mode", type=int, default=0, choices=[0, 1, 2], help="NG_OPT_STEP_MODE")
+    ap.add_argument("--step-mode", type=int, default=3, choices=[0, 1, 2, 3], help="NG_OPT_STEP_MODE (3 = auto)")
     ap.add_argument("--delivery-kernel", type=int, default=0, choices=[0, 1, 2, 3], help="NG_OPT_DELIVERY_KERNEL (0 = auto)")
     ap.add_argument("--no-prefetch", action="store_true", help="NG_OPT_PREFETCH = 0")
     ap.add_argument("--micro-k", type=int, default=10000)

@@ -76,8 +76,9 @@ enum {
 
 /* options for ng_set_option */
 enum {
-    NG_OPT_STEP_MODE = 0,        /* 0 = CUDA graph of NG_OPT_STEPS_PER_GRAPH steps (default),
-                                    1 = plain kernel launches, 2 = one persistent cooperative kernel  */
+    NG_OPT_STEP_MODE = 0,        /* 0 = CUDA graph of NG_OPT_STEPS_PER_GRAPH steps, 1 = plain kernel launches,
+                                    2 = one persistent cooperative kernel per ng_simulate call,
+                                    3 = auto (default): 2 for delivery kernels 1 and 3, 0 for kernel 2      */
     NG_OPT_STEPS_PER_GRAPH = 1,  /* default 100 */
     NG_OPT_DELIVERY_KERNEL = 2,  /* 0 = auto, 1 = row-chunk walk, 2 = delay-major segment walk,
                                     3 = pipelined step kernel (delay-1 records with the update, the rest

@@ -18,7 +18,7 @@ FIELD_V, FIELD_I_SYN, FIELD_REFR, FIELD_RING, FIELD_STEP, FIELD_LAST_INPUT = 0, 
 DIST_CONST, DIST_NORMAL_CLIPPED, DIST_UNIFORM_INT = 0, 1, 2
 (OPT_STEP_MODE, OPT_STEPS_PER_GRAPH, OPT_DELIVERY_KERNEL, OPT_DELIVER_BLOCKS, OPT_PROFILE, OPT_ASYNC,
  OPT_SORT_SEGMENTS, OPT_PREFETCH, OPT_TRACE, OPT_PERSISTENT_THREADS) = range(10)
-STEP_GRAPH, STEP_LAUNCH, STEP_PERSISTENT = 0, 1, 2
+STEP_GRAPH, STEP_LAUNCH, STEP_PERSISTENT, STEP_AUTO = 0, 1, 2, 3
 
 EXPORTS = ["ng_create", "ng_destroy", "ng_last_error", "ng_create_population", "ng_connect_fixed_indegree",
            "ng_connect_fixed_outdegree", "ng_set_bypass", "ng_set_option", "ng_prepare", "ng_set_state",

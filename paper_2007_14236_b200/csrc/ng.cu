@@ -40,7 +40,7 @@ struct ng_sim {
     bool prepared = false;
     int32_t bypass = 0; uint32_t inject_thr = 0;
     // options
-    int step_mode = 0; int steps_per_graph = 100; int delivery_kernel_opt = 0; int deliver_blocks_opt = 0;
+    int step_mode_opt = 3; int step_mode = 0; int steps_per_graph = 100; int delivery_kernel_opt = 0; int deliver_blocks_opt = 0;
     bool trace_on = false; unsigned long long* trace_saved = nullptr; int last_persistent_blocks = 0;
     int profile = 0; int async = 0; int sort_segments = 1; int prefetch_opt = 1;
     // device
@@ -51,7 +51,7 @@ struct ng_sim {
     RowInfo* d_row_info = nullptr;
     CallDev* d_calls = nullptr; PopDev* d_pops = nullptr; uint8_t* d_pop_of = nullptr; Ctl* d_ctl = nullptr;
     int64_t n_padded = 0; int64_t max_row_records = 0;
-    int sm_count = 148; size_t l2_bytes = 0;
+    int sm_count = 148; size_t l2_bytes = 0; bool coop_ok = false;
     int delivery_kernel = 1; int deliver_blocks = 0; int update_blocks = 0; int persistent_blocks = 0;
     int pipe_blocks = 0; int persistent_pipe_blocks = 0;
     int persistent_threads = kPersistentThreads;
@@ -190,8 +190,11 @@ void configure_launch(ng_sim* s) {
     const double mean_group = s->N > 0 ? (double)s->S / ((double)s->N * s->cfg.ring_slots) : 0.0;
     int k = s->delivery_kernel_opt;
     // otherwise the step is latency-bound: rows are walked whole (kernel 1) or by the pipelined step kernel (3).
-    if (k == 0) k = (ring_bytes > 0.5 * (double)s->l2_bytes && mean_group >= 4.0) ? 2 : 1;
+    if (k == 0) k = (ring_bytes > 0.8 * (double)s->l2_bytes && mean_group >= 4.0) ? 2 : 3;
     s->delivery_kernel = k;
+    // step mode: the latency-bound kernels run as one persistent cooperative kernel per ng_simulate call; the
+    // bandwidth-bound delay-major kernel keeps its 8 CTAs per SM and runs from a CUDA graph
+    s->step_mode = s->step_mode_opt != 3 ? s->step_mode_opt : (k == 2 || !s->coop_ok) ? 0 : 2;
     s->a.prefetch = (k != 2 && s->prefetch_opt) ? 1 : 0;
     s->pipe_blocks = grid_for(s->N, kPipeThreads - kEntryTile, sm * 4);   // updaters per CTA = kPipeThreads - kEntryTile
     {
@@ -299,6 +302,7 @@ int32_t ng_create(const ng_config* cfg, const ng_allocator* alloc, void* cuda_st
     if (cudaGetDeviceProperties(&prop, cfg->device) == cudaSuccess) {
         s->sm_count = prop.multiProcessorCount;
         s->l2_bytes = (size_t)prop.l2CacheSize;
+        s->coop_ok = prop.cooperativeLaunch != 0;
     }
     *out = s;
     return NG_OK;
@@ -361,8 +365,10 @@ int32_t ng_set_option(ng_sim* s, int32_t option, int64_t value) {
     if (!s) return NG_ERR_INVALID_ARG;
     switch (option) {
         case NG_OPT_STEP_MODE:
-            if (value < 0 || value > 2) return fail(s, NG_ERR_INVALID_ARG, "step mode is 0, 1 or 2");
-            s->step_mode = (int)value; break;
+            if (value < 0 || value > 3) return fail(s, NG_ERR_INVALID_ARG, "step mode is 0, 1, 2 or 3 (auto)");
+            s->step_mode_opt = (int)value;
+            if (s->prepared) configure_launch(s); else if (value != 3) s->step_mode = (int)value;
+            break;
         case NG_OPT_STEPS_PER_GRAPH:
             if (value < 1 || value > 10000) return fail(s, NG_ERR_INVALID_ARG, "steps per graph in 1..10000");
             s->steps_per_graph = (int)value; destroy_graph(s); break;

@@ -811,6 +811,9 @@ struct PipeShared {
     int32_t skip[kEntryTile];
     long long d1_r0[kD1Cap];
     int32_t d1_cnt[kD1Cap];
+    int32_t d1_deg[kD1Cap];
+    int32_t d1_id[kD1Cap];
+    int32_t gbase;
     int32_t n_d1;
     StepScalars sc;
     int32_t pending;
@@ -831,14 +834,35 @@ __device__ __forceinline__ void deliver_d1_piece(const StepArgs& a, float* __res
 __device__ __forceinline__ void group_sync(int id, int count) {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory");
 }
-__device__ __forceinline__ int pipe_rest_threads() { return blockDim.x >= 512 ? kEntryTile : 64; }
+// item `it` of the staged tile: find its entry (number of k in [1, m] with pre[k] <= it) and deliver its chunk
+__device__ __forceinline__ void pipe_one_item(const StepArgs& a, int nmod, PipeShared& sh, int m, int it, bool small, int lane) {
+    int sidx = 0;
+    for (int j = 0; j < m; j += 32) {
+        const int k = j + lane + 1;
+        const int v = k <= m ? sh.d.pre[k] : 0x7fffffff;
+        sidx += __popc(__ballot_sync(0xffffffffu, v <= it));
+    }
+    const int c = it - sh.d.pre[sidx];
+    if (small) deliver_item<1>(a, nmod, sh.d.r0[sidx], sh.d.len[sidx], c, lane, sh.skip[sidx]);
+    else deliver_item<4>(a, nmod, sh.d.r0[sidx], sh.d.len[sidx], c, lane, sh.skip[sidx]);
+}
+// Updaters per CTA: just enough for one neuron per thread when the network is small enough for a single round
+// (every other warp then joins the rest pass), else all but kEntryTile threads.
+__device__ __forceinline__ int pipe_updater_threads(int N) {
+    const unsigned per_cta = ((unsigned)N + gridDim.x - 1u) / gridDim.x;          // 32-bit: no 64-bit division on the step path
+    const int need = (int)((per_cta + 31u) & ~31u);
+    const int cap = (int)blockDim.x - (blockDim.x >= 512 ? kEntryTile : 64);
+    return (int)per_cta <= cap ? max(need, 32) : cap;
+}
 
 template <bool kUpdate>
 __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* __restrict__ P, long long n, int slot, bool pending,
                                                unsigned long long rec_prev, PipeShared& sh, bool have_k = false) {
     const int N = a.N, Dr = a.Dr;
     const int lane = threadIdx.x & 31;
-    const int R = pipe_rest_threads(), U = blockDim.x - R;         // rest group = threads [U, U + R)
+    const int U = pipe_updater_threads(N), R = blockDim.x - U;     // rest group = threads [U, U + R), R >= 64
+    const int RT = min(R, kEntryTile);                             // threads of the rest group that stage entries
+    const int nmod_prev = slot == 0 ? Dr - 1 : slot - 1;           // (n - 1) mod Dr
     if (threadIdx.x == 0) sh.n_d1 = 0;
     if (threadIdx.x == U && !pending) sh.d.M = 0;
     __syncthreads();
@@ -853,23 +877,32 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
                 const long long ii = base + threadIdx.x;
                 const int i = (int)ii;
                 NeuronRegs g;
+                // the row descriptor is fetched for EVERY neuron together with its state (16 B, L2-resident because it
+                // is touched every step): a spiking thread then needs no further memory round trip
+                RowInfo r;
+                if (ii < N) r = ld_row_info(a.row_info + i);
                 const bool spk = ii < N && neuron_early(a, P, n, i, plane, g, have_k);
                 const unsigned m = __ballot_sync(0xffffffffu, spk);
-                if (m) {
+                if (m) {                                           // warp-aggregated append to the CTA's own list
                     const int leader = __ffs(m) - 1;
-                    int gb = 0, lb = 0;
-                    if (lane == leader) { gb = atomicAdd(&a.ctl->spike_cnt[n & 3], __popc(m)); lb = atomicAdd(&sh.n_d1, __popc(m)); }
-                    RowInfo r;
-                    if (spk) { r = ld_row_info(a.row_info + i); if (a.prefetch) prefetch_row(a, r); }
-                    gb = __shfl_sync(0xffffffffu, gb, leader);
+                    int lb = 0;
+                    if (lane == leader) lb = atomicAdd(&sh.n_d1, __popc(m));
+                    if (spk && a.prefetch && r.d1 > 0) {           // delay-1 head of the row: needed within a microsecond
+                        const uint32_t head = (uint32_t)(((long long)r.d1 * 4 + 15) & ~15LL);
+                        prefetch_l2_bulk(reinterpret_cast<const char*>(a.tgt + r.r0), head);
+                        prefetch_l2_bulk(reinterpret_cast<const char*>(a.w + r.r0), head);
+                    }
                     lb = __shfl_sync(0xffffffffu, lb, leader);
                     if (spk) {
-                        const int rank = __popc(m & ((1u << lane) - 1u));
-                        const size_t k = (size_t)(n & 1) * N + gb + rank;
-                        a.spike_list[k] = i;
-                        st_row_info(a.spike_row + k, r);
-                        if (lb + rank < kD1Cap) { sh.d1_r0[lb + rank] = r.r0; sh.d1_cnt[lb + rank] = r.d1; }
-                        else for (int q = 0; q < r.d1; ++q) deliver_d1_piece(a, plane1, r.r0, r.d1, q);   // list full: serial
+                        const int k = lb + __popc(m & ((1u << lane) - 1u));
+                        if (k < kD1Cap) { sh.d1_r0[k] = r.r0; sh.d1_cnt[k] = r.d1; sh.d1_deg[k] = r.deg; sh.d1_id[k] = i; }
+                        else {                                     // CTA list full: this lane does everything alone
+                            for (int q = 0; q < r.d1; ++q) deliver_d1_piece(a, plane1, r.r0, r.d1, q);
+                            if (a.prefetch) prefetch_row(a, r);
+                            const size_t gk = (size_t)(n & 1) * N + atomicAdd(&a.ctl->spike_cnt[n & 3], 1);
+                            a.spike_list[gk] = i;
+                            st_row_info(a.spike_row + gk, r);
+                        }
                     }
                 }
                 if (ii < N) neuron_late(a, P, n, i, plane, g);
@@ -878,18 +911,33 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
             group_sync(1, U);
             trace_stamp(a, n, 4);
             const int nd1 = min(sh.n_d1, kD1Cap);
+            // one atomic per CTA reserves the CTA's slots in the global spike array; its round trip overlaps the
+            // delay-1 pass (nothing on the critical path needs the global index)
+            int gbase = 0;
+            if (threadIdx.x == 0 && nd1 > 0) gbase = atomicAdd(&a.ctl->spike_cnt[n & 3], nd1);
             for (int s = 0; s < nd1; ++s) {
                 const long long r0 = sh.d1_r0[s];
                 const int cnt = sh.d1_cnt[s];
                 for (int q = wib * 32 + lane; q < cnt; q += wpu * 32) deliver_d1_piece(a, plane1, r0, cnt, q);
             }
             trace_stamp(a, n, 6);
+            if (nd1 > 0) {                                         // uniform over the updater group
+                if (threadIdx.x == 0) sh.gbase = gbase;
+                group_sync(1, U);
+                const int gb = sh.gbase;
+                for (int s = threadIdx.x; s < nd1; s += U) {       // a2: global spike array; the rest of the row is read
+                    RowInfo r; r.r0 = sh.d1_r0[s]; r.d1 = sh.d1_cnt[s]; r.deg = sh.d1_deg[s];       // one phase later
+                    const size_t gk = (size_t)(n & 1) * N + gb + s;
+                    a.spike_list[gk] = sh.d1_id[s];
+                    st_row_info(a.spike_row + gk, r);
+                    if (a.prefetch) prefetch_row(a, r);
+                }
+            }
         }
     } else if (pending) {
-        // ---- rest pass of step n-1: records [d1, deg) of every spike, dealt to the rest warps of the whole grid ----
+        // ---- rest pass of step n-1: records [d1, deg) of every spike ----
         const int t = threadIdx.x - U;                             // index inside the rest group
         const int wir = t >> 5, wpr = R >> 5;
-        const int gwarp = blockIdx.x * wpr + wir, gwarps = gridDim.x * wpr;
         const long long np = n - 1;
         const RowInfo* __restrict__ rows_prev = a.spike_row + (size_t)(np & 1) * N;
         const int32_t* __restrict__ list_prev = a.spike_list + (size_t)(np & 1) * N;
@@ -897,20 +945,20 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
         if (t == 0) sh.d.M = __ldcg(&a.ctl->spike_cnt[np & 3]);
         int4 e = make_int4(0, 0, 0, 0);
         int id_prev = 0;
-        if (t < N) {                                               // speculative: the first tile, before M is known
+        if (t < RT && t < N) {                                     // speculative: the first tile, before M is known
             e = __ldcg(reinterpret_cast<const int4*>(rows_prev + t));
             if (rec_cta) id_prev = __ldcg(list_prev + t);
         }
         group_sync(2, R);
         trace_stamp(a, n, 7, U);
         const int M = sh.d.M;
-        const int nmod = slot == 0 ? Dr - 1 : slot - 1;             // (n - 1) mod Dr
+        const int gwarp = blockIdx.x * wpr + wir, gwarps = gridDim.x * wpr;      // items are dealt to the rest warps of the grid
         const bool small = (long long)M * a.mean_row_records <= 64LL * gwarps;
         const int cshift = small ? 5 : 7;
         unsigned long long ev = 0;
         int base_mod = 0;
-        for (int tile0 = 0; tile0 < M; tile0 += R) {
-            const int m = min(R, M - tile0);
+        for (int tile0 = 0; tile0 < M; tile0 += RT) {
+            const int m = min(RT, M - tile0);
             if (tile0 > 0) {
                 group_sync(2, R);
                 if (t < m) {
@@ -931,33 +979,29 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
                     if (pos < (unsigned long long)a.rec_cap) { a.rec_id[pos] = id_prev; a.rec_step[pos] = (int32_t)np; }
                 }
             }
+            if (t < RT) {                                          // whole warps: RT is a multiple of 32
 #pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const int y = __shfl_up_sync(0xffffffffu, x, o);
-                if (lane >= o) x += y;
+                for (int o = 1; o < 32; o <<= 1) {
+                    const int y = __shfl_up_sync(0xffffffffu, x, o);
+                    if (lane >= o) x += y;
+                }
+                if (lane == 31) sh.d.warp_tot[wir] = x;
             }
-            if (lane == 31) sh.d.warp_tot[wir] = x;
-            group_sync(2, R);
-            int off = 0;
-            for (int k = 0; k < wir; ++k) off += sh.d.warp_tot[k];
-            sh.d.pre[t + 1] = x + off;
+            if (m > 32) {                                          // several warps hold entries: add the warp offsets
+                group_sync(2, R);
+                if (t < RT) {
+                    int off = 0;
+                    for (int k = 0; k < wir; ++k) off += sh.d.warp_tot[k];
+                    sh.d.pre[t + 1] = x + off;
+                }
+            } else if (t < 32) sh.d.pre[t + 1] = x;                // latency regime: one warp, one barrier
             if (t == 0) sh.d.pre[0] = 0;
             group_sync(2, R);
             trace_stamp(a, n, 8, U);
             const int total = sh.d.pre[m];
-            int first = gwarp - base_mod;
+            int first = gwarp - base_mod;                          // items are numbered across tiles: round-robin deal
             if (first < 0) first += gwarps;
-            for (int it = first; it < total; it += gwarps) {
-                int sidx = 0;
-                for (int j = 0; j < m; j += 32) {
-                    const int k = j + lane + 1;
-                    const int v = k <= m ? sh.d.pre[k] : 0x7fffffff;
-                    sidx += __popc(__ballot_sync(0xffffffffu, v <= it));
-                }
-                const int c = it - sh.d.pre[sidx];
-                if (small) deliver_item<1>(a, nmod, sh.d.r0[sidx], sh.d.len[sidx], c, lane, sh.skip[sidx]);
-                else deliver_item<4>(a, nmod, sh.d.r0[sidx], sh.d.len[sidx], c, lane, sh.skip[sidx]);
-            }
+            for (int it = first; it < total; it += gwarps) pipe_one_item(a, nmod_prev, sh, m, it, small, lane);
             base_mod = (int)(((long long)base_mod + total) % gwarps);
         }
         trace_stamp(a, n, 9, U);
@@ -1014,7 +1058,7 @@ __global__ void __launch_bounds__(kPersistentThreads, 1) persistent_pipe_kernel(
     const PopDev* P = stage_pops(a, sh.pops);
     if (a.n_pops > kMaxPopsSmem) __syncthreads();
     const long long gtid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const int U = blockDim.x - pipe_rest_threads();
+    const int U = pipe_updater_threads(a.N);
     long long n = sh.sc.n;
     int slot = sh.sc.slot;
     unsigned long long rec_prev = sh.sc.rec_base, spikes = 0, epoch = 0;       // recorded before step n-1 (nothing pending at entry)
