@@ -151,12 +151,12 @@ def barrier(world):
     torch.cuda.synchronize()
 
 
-def delivery_microbench(device, peak_gbs, K=10000, fraction=0.05, steps=30, warm=5):
+def delivery_microbench(device, peak_gbs, K=10000, fraction=0.05, steps=30, warm=5, fallback=True):
     """BASELINE.json configs[3]: delivery kernel alone (neuron update bypassed), 1e6 sources, out-degree K, a random
     fraction of sources firing per step.  Falls back to K = 1000 when 90 GB of records do not fit."""
     import torch
     from paper_2007_14236_b200 import binding as B, workloads as W
-    for k_try in (K, 1000):
+    for k_try in ((K, 1000) if fallback else (K,)):
         g = None
         try:
             wl = W.delivery_microbench(K=k_try, fraction=fraction)
@@ -168,12 +168,15 @@ def delivery_microbench(device, peak_gbs, K=10000, fraction=0.05, steps=30, warm
             g.simulate(steps)
             s1 = g.stats()
             ev = s1.events - s0.events
-            ms = s1.ms_deliver - s0.ms_deliver
-            out = {"workload": f"configs[3] delivery microbenchmark: 1e6 sources, out-degree {k_try}, {fraction:.0%} firing per step, D=64",
+            # kernels 1 and 2: the delivery kernel alone; kernel 3 is one launch per step (spike injection + delivery)
+            ms = (s1.ms_deliver - s0.ms_deliver) if int(s1.delivery_kernel) != 3 else (s1.ms_update - s0.ms_update)
+            out = {"workload": f"configs[3] delivery microbenchmark: 1e6 sources, out-degree {k_try}, {fraction:.1%} firing per step, D=64",
                    "steps": steps, "events_per_step": ev / steps, "deliver_ms_per_step": ms / steps,
                    "events_per_s": ev / (ms * 1e-3), "algorithmic_gbs": ev * BYTES_PER_EVENT / (ms * 1e-3) / 1e9,
                    "frac_of_hbm_peak": ev * BYTES_PER_EVENT / (ms * 1e-3) / 1e9 / peak_gbs,
-                   "delivery_kernel": int(s1.delivery_kernel), "build_ms": s1.build_ms,
+                   "delivery_kernel": int(s1.delivery_kernel),
+                   "timed": "delivery kernel" if int(s1.delivery_kernel) != 3 else "pipelined step kernel (injection + delivery)",
+                   "build_ms": s1.build_ms,
                    "n_connections": int(s1.n_connections)}
             g.close()
             return out
@@ -406,6 +409,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip timing the oracle")
     ap.add_argument("--only-microbench", action="store_true",
                     help="run only the configs[3] delivery microbenchmark and print its JSON object (used for ncu captures)")
+    ap.add_argument("--micro-sweep", action="store_true",
+                    help="run the 3 x 3 sweep of BASELINE.json configs[3] (out-degree 100/1000/10000 x firing 0.1/1/5 %%)")
     ap.add_argument("--probe", action="store_true", help="run the ceiling probes (ng_probe) and print them as JSON")
     ap.add_argument("--step-mode", type=int, default=3, choices=[0, 1, 2, 3], help="NG_OPT_STEP_MODE (3 = auto)")
     ap.add_argument("--delivery-kernel", type=int, default=0, choices=[0, 1, 2, 3], help="NG_OPT_DELIVERY_KERNEL (0 = auto)")
@@ -418,6 +423,12 @@ def main():
         args.warmup = 3
     if args.probe:
         print(json.dumps(run_probes()), flush=True)
+    elif args.micro_sweep:
+        # BASELINE.json configs[3]: out-degree x firing-fraction sweep of the delivery stage alone, one JSON object per line
+        peak = measured_peak_gbs()[0]
+        for k in (100, 1000, 10000):
+            for f in (0.001, 0.01, 0.05):
+                print(json.dumps(delivery_microbench(0, peak, K=k, fraction=f, steps=args.micro_steps, fallback=False)), flush=True)
     elif args.only_microbench:
         print(json.dumps(delivery_microbench(0, measured_peak_gbs()[0], K=args.micro_k, fraction=args.micro_fraction,
                                              steps=args.micro_steps)), flush=True)

@@ -222,10 +222,14 @@ int32_t ng_get_connections(ng_sim* sim, int32_t src_id, int32_t* tgt_host, float
 /* Counters and timings.  Synchronises the stream. */
 int32_t ng_get_stats(ng_sim* sim, ng_stats* out);
 
-/* Phase stamps of the last persistent launch (NG_OPT_TRACE): uint64 ns, laid out [64 steps][blocks][8 stamps], step
- * index = step-in-launch mod 64.  Stamps: 0 step start, 1 update (or fused phase) done, 2 after barrier; two-phase
- * kernels also 3 delivery done, 4 bookkeeping done, 5 after the second barrier.  count_out = words available,
- * blocks_out = CTAs of that launch; copies only if capacity >= count.  Errors: STATE when no trace exists. */
+/* Phase stamps of the last persistent launch (NG_OPT_TRACE): uint64 ns (%globaltimer), laid out
+ * [64 steps][blocks][16 stamps], step index = step mod 64, one stamping thread per CTA and stamp.
+ *   two-phase kernels (delivery kernel 1, 2): 0 step start, 1 update done, 2 after the first barrier, 3 delivery done,
+ *     5 after the second barrier;
+ *   pipelined kernel (3): 0 phase start, 3 update done (warp 0), 4 all updater warps done, 6 delay-1 pass done,
+ *     7 rest pass: spike count known, 8 rest pass: entries staged, 9 rest pass: items done, 1 phase done, 2 after the barrier.
+ * count_out = words available, blocks_out = CTAs of that launch; copies only if capacity >= count.
+ * Errors: STATE when no trace exists. */
 int32_t ng_get_trace(ng_sim* sim, uint64_t* out_host, int64_t capacity, int64_t* count_out, int32_t* blocks_out);
 
 /* Ceiling probe for the roofline report (not on the hot path).  Measures, with the load and

@@ -51,7 +51,8 @@ struct Ctl {                   // device-resident control block; see ng.cu for t
     unsigned int ticket;                   // fused / pipelined step kernels: CTAs that finished the current step
     int32_t pending;                       // pipelined step kernel: the rest pass of step step_u - 1 is outstanding
     int32_t slot;                          // step_u mod Dr, kept next to step_u so no kernel divides 64-bit integers
-    int32_t pad1;
+    int32_t slot_d;                        // step_d mod Dr: written by update, read by deliver (like step_d) — the delivery
+                                           // kernel's bookkeeping advances `slot` while later CTAs of the same launch still start
     unsigned long long bar;                // persistent fused kernel: arrivals at the grid barrier
 };
 
@@ -579,8 +580,13 @@ __device__ __forceinline__ int deliver_rows_phase(const StepArgs& a, long long n
     const bool small = (long long)M * a.mean_row_records <= 64LL * gwarps;
     const int cshift = small ? 5 : 7;
     unsigned long long ev = 0;
-    int base_mod = 0;                                          // (flattened index of the tile's first item) mod gwarps
-    for (int tile0 = 0; tile0 < M; tile0 += kEntryTile) {
+    int base_mod = 0;                                          // (flattened index of the tile's first item) mod gw_n
+    // Many spikes (>= 16 per CTA): every CTA stages only its own tiles of the spike array and deals their items to its
+    // own warps; few spikes: every CTA stages all of them and the items are dealt to all warps of the grid.
+    const bool part = M >= 16 * (int)gridDim.x;
+    const int tile_first = part ? (int)blockIdx.x * kEntryTile : 0, tile_stride = part ? (int)gridDim.x * kEntryTile : kEntryTile;
+    const int gw = part ? wib : gwarp, gw_n = part ? wpb : gwarps;
+    for (int tile0 = tile_first; tile0 < M; tile0 += tile_stride) {
         const int m = min(kEntryTile, M - tile0);
         if (tile0 > 0) {
             __syncthreads();                                   // previous tile's readers are done
@@ -593,7 +599,7 @@ __device__ __forceinline__ int deliver_rows_phase(const StepArgs& a, long long n
                 const int len = padded_len(e.z);
                 sh.len[threadIdx.x] = len;
                 x = (len + (1 << cshift) - 1) >> cshift;
-                if (blockIdx.x == 0) ev += (unsigned long long)e.z;
+                if (blockIdx.x == 0 || part) ev += (unsigned long long)e.z;
             }
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
@@ -612,9 +618,9 @@ __device__ __forceinline__ int deliver_rows_phase(const StepArgs& a, long long n
         }
         __syncthreads();
         const int total = sh.pre[m];
-        int first = gwarp - base_mod;                          // items are numbered across tiles: round-robin deal
-        if (first < 0) first += gwarps;
-        for (int it = first; it < total; it += gwarps) {
+        int first = gw - base_mod;                             // items are numbered across tiles: round-robin deal
+        if (first < 0) first += gw_n;
+        for (int it = first; it < total; it += gw_n) {
             int sidx = 0;                                      // number of k in [1, m] with pre[k] <= it
             for (int j = 0; j < m; j += 32) {
                 const int k = j + lane + 1;
@@ -625,7 +631,7 @@ __device__ __forceinline__ int deliver_rows_phase(const StepArgs& a, long long n
             if (small) deliver_item<1>(a, nmod, sh.r0[sidx], sh.len[sidx], c, lane);
             else deliver_item<4>(a, nmod, sh.r0[sidx], sh.len[sidx], c, lane);
         }
-        base_mod = (int)(((long long)base_mod + total) % gwarps);
+        base_mod = (int)(((long long)base_mod + total) % gw_n);
     }
     if (ev) atomicAdd(&a.ctl->events, ev);
     return M;
@@ -813,6 +819,7 @@ struct PipeShared {
     int32_t d1_cnt[kD1Cap];
     int32_t d1_deg[kD1Cap];
     int32_t d1_id[kD1Cap];
+    int32_t d1_pre[kD1Cap + 32];
     int32_t gbase;
     int32_t n_d1;
     StepScalars sc;
@@ -915,10 +922,34 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
             // delay-1 pass (nothing on the critical path needs the global index)
             int gbase = 0;
             if (threadIdx.x == 0 && nd1 > 0) gbase = atomicAdd(&a.ctl->spike_cnt[n & 3], nd1);
-            for (int s = 0; s < nd1; ++s) {
-                const long long r0 = sh.d1_r0[s];
-                const int cnt = sh.d1_cnt[s];
-                for (int q = wib * 32 + lane; q < cnt; q += wpu * 32) deliver_d1_piece(a, plane1, r0, cnt, q);
+            if (nd1 <= 8) {                                        // latency regime: a few spikes, 32 records per warp
+                for (int s = 0; s < nd1; ++s) {
+                    const long long r0 = sh.d1_r0[s];
+                    const int cnt = sh.d1_cnt[s];
+                    for (int q = wib * 32 + lane; q < cnt; q += wpu * 32) deliver_d1_piece(a, plane1, r0, cnt, q);
+                }
+            } else {                                               // many spikes: flatten (spike, record) over the updaters
+                if (wib == 0) {
+                    int carry = 0;
+                    for (int base = 0; base < nd1; base += 32) {
+                        int x = base + lane < nd1 ? sh.d1_cnt[base + lane] : 0;
+#pragma unroll
+                        for (int o = 1; o < 32; o <<= 1) {
+                            const int y = __shfl_up_sync(0xffffffffu, x, o);
+                            if (lane >= o) x += y;
+                        }
+                        sh.d1_pre[base + lane + 1] = carry + x;
+                        carry += __shfl_sync(0xffffffffu, x, 31);
+                    }
+                    if (lane == 0) sh.d1_pre[0] = 0;
+                }
+                group_sync(1, U);
+                const int T = sh.d1_pre[nd1];
+                for (int f = threadIdx.x; f < T; f += U) {
+                    int lo = 0, hi = nd1;                          // largest s with d1_pre[s] <= f
+                    while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (sh.d1_pre[mid] <= f) lo = mid; else hi = mid; }
+                    deliver_d1_piece(a, plane1, sh.d1_r0[lo], sh.d1_cnt[lo], f - sh.d1_pre[lo]);
+                }
             }
             trace_stamp(a, n, 6);
             if (nd1 > 0) {                                         // uniform over the updater group
@@ -957,13 +988,18 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
         const int cshift = small ? 5 : 7;
         unsigned long long ev = 0;
         int base_mod = 0;
-        for (int tile0 = 0; tile0 < M; tile0 += RT) {
+        // many spikes (>= 16 per CTA): every CTA stages only its own tiles and deals their items to its own rest warps
+        const bool part = M >= 16 * (int)gridDim.x;
+        const int tile_first = part ? (int)blockIdx.x * RT : 0, tile_stride = part ? (int)gridDim.x * RT : RT;
+        const int gw = part ? wir : gwarp, gw_n = part ? wpr : gwarps;
+        const bool rec_here = a.rec_cap > 0 && (blockIdx.x == 0 || part);
+        for (int tile0 = tile_first; tile0 < M; tile0 += tile_stride) {
             const int m = min(RT, M - tile0);
             if (tile0 > 0) {
                 group_sync(2, R);
                 if (t < m) {
                     e = __ldcg(reinterpret_cast<const int4*>(rows_prev + tile0 + t));
-                    if (rec_cta) id_prev = __ldcg(list_prev + tile0 + t);
+                    if (rec_here) id_prev = __ldcg(list_prev + tile0 + t);
                 }
             }
             int x = 0;
@@ -973,8 +1009,8 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
                 sh.d.len[t] = len;
                 sh.skip[t] = e.w;
                 x = (len + (1 << cshift) - 1) >> cshift;
-                if (blockIdx.x == 0) ev += (unsigned long long)e.z;
-                if (rec_cta) {
+                if (blockIdx.x == 0 || part) ev += (unsigned long long)e.z;
+                if (rec_here) {
                     const unsigned long long pos = rec_prev + (unsigned long long)(tile0 + t);
                     if (pos < (unsigned long long)a.rec_cap) { a.rec_id[pos] = id_prev; a.rec_step[pos] = (int32_t)np; }
                 }
@@ -999,10 +1035,10 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
             group_sync(2, R);
             trace_stamp(a, n, 8, U);
             const int total = sh.d.pre[m];
-            int first = gwarp - base_mod;                          // items are numbered across tiles: round-robin deal
-            if (first < 0) first += gwarps;
-            for (int it = first; it < total; it += gwarps) pipe_one_item(a, nmod_prev, sh, m, it, small, lane);
-            base_mod = (int)(((long long)base_mod + total) % gwarps);
+            int first = gw - base_mod;                             // items are numbered across tiles: round-robin deal
+            if (first < 0) first += gw_n;
+            for (int it = first; it < total; it += gw_n) pipe_one_item(a, nmod_prev, sh, m, it, small, lane);
+            base_mod = (int)(((long long)base_mod + total) % gw_n);
         }
         trace_stamp(a, n, 9, U);
         if (ev) atomicAdd(&a.ctl->events, ev);
@@ -1099,7 +1135,7 @@ __global__ void __launch_bounds__(kUpdateThreads) update_kernel(const StepArgs a
         sc.n = __ldcg(&a.ctl->step_u);
         sc.slot = __ldcg(&a.ctl->slot);
         sc.rec_base = __ldcg(&a.ctl->rec_total[sc.n & 1]);
-        if (blockIdx.x == 0) a.ctl->step_d = sc.n;
+        if (blockIdx.x == 0) { a.ctl->step_d = sc.n; a.ctl->slot_d = sc.slot; }
     }
     const PopDev* P = stage_pops(a, sh_pops);              // contains the __syncthreads that publishes sc
     if (a.n_pops > kMaxPopsSmem) __syncthreads();
@@ -1107,12 +1143,12 @@ __global__ void __launch_bounds__(kUpdateThreads) update_kernel(const StepArgs a
 }
 
 template <int kKernel>
-__global__ void __launch_bounds__(kDeliverThreads) deliver_kernel(const StepArgs a) {
+__global__ void __launch_bounds__(kDeliverThreads, 3) deliver_kernel(const StepArgs a) {
     __shared__ DeliverShared sh;
     __shared__ StepScalars sc;
     if (threadIdx.x == 0) {
         sc.n = __ldcg(&a.ctl->step_d);
-        sc.slot = __ldcg(&a.ctl->slot);
+        sc.slot = __ldcg(&a.ctl->slot_d);
         if (kKernel != 1) sc.M = __ldcg(&a.ctl->spike_cnt[sc.n & 3]);
     }
     __syncthreads();

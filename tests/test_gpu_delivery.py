@@ -62,6 +62,26 @@ def test_delivery_only_matches_oracle(oracle_mod, B, K, fraction, kernel, mode):
     g.close()
 
 
+@pytest.mark.parametrize("kernel,mode", [(1, 0), (2, 0), (2, 1)])
+def test_delivery_grid_larger_than_one_wave(oracle_mod, B, kernel, mode):
+    """Stand-alone delivery kernels with more CTAs than are resident at once: CTAs of the second wave start after
+    CTA 0 has already published the next step, so nothing they read may be advanced by that bookkeeping."""
+    n, steps, K = 20000, 70, 1000
+    wl = W.delivery_microbench(n=n, K=K, fraction=0.05, n_steps=steps, seed=6)
+    o, g = make_pair(wl, oracle_mod, debug_input=False)
+    g.set_option(B.OPT_DELIVERY_KERNEL, kernel)
+    g.set_option(B.OPT_STEP_MODE, mode)
+    g.set_option(B.OPT_DELIVER_BLOCKS, 148 * 24)
+    g.simulate(steps)
+    o.simulate(steps)
+    assert g.stats().events == o.n_events
+    gr = g.get_state(B.FIELD_RING).astype(np.float64)
+    orr = o.get_state(oracle_mod.FIELD_RING)
+    assert np.array_equal(gr != 0, orr != 0)
+    assert np.all(np.abs(gr - orr) <= 1e-4 * np.abs(orr) + 1e-9)
+    g.close()
+
+
 @pytest.mark.parametrize("kernel", [1, 2, 3])
 def test_delivery_invariants_large(B, kernel):
     """200,000 sources x out-degree 1000 (2e8 records): per step, the weight arriving in every ring plane equals the sum
@@ -96,4 +116,60 @@ def test_delivery_invariants_large(B, kernel):
         total += expect
     st = g.stats()
     assert st.events == st.spikes * K
+    g.close()
+
+
+@pytest.mark.parametrize("K,fraction", [(10_000, 0.001), (1000, 0.05), (100, 0.05)])
+def test_cfg3_full_size_sampled(oracle_mod, B, K, fraction):
+    """BASELINE.json configs[3] at its full size (10^6 sources, out-degree K, 10^6-neuron pool, D = 64) in the launch
+    configuration bench.py's delivery microbenchmark times (default options: delay-major kernel 2 from a CUDA graph).
+    The oracle cannot hold 10^10 records, so: (a) sampled rows are compared record for record with the oracle's O(1)
+    regeneration of the same draws (fixed-outdegree rule: draws (call 0, source j, k)); (b) the injected spike set of a
+    step equals the oracle's Philox rule on sampled sources; (c) for a sampled set of targets every ring cell (all
+    planes) equals the plain definition evaluated in fp64 from the read-back rows of the sources that spiked, within
+    1e-5 of the L1 mass (reading C12), and the per-plane sums over ALL targets agree; (d) events = spikes x K."""
+    n, D, steps = 1_000_000, 64, 2
+    wl = W.delivery_microbench(n=n, K=K, fraction=fraction, n_steps=steps)
+    g = B.Sim(0.1, D, wl.seed, record_spikes=True, max_recorded_spikes=1 << 22)
+    wl.apply(g); g.prepare()
+    st = g.stats()
+    # auto rule: delay-major kernel 2 from a CUDA graph when groups are long enough, else the pipelined kernel 3
+    assert st.n_connections == n * K
+    assert (st.delivery_kernel, st.step_mode) == ((2, B.STEP_GRAPH) if K >= 1000 else (3, B.STEP_PERSISTENT))
+    oc = oracle_mod.Oracle(0.1, D, wl.seed)
+    wl.apply(oc)                                             # calls only; never prepared
+    rnd = np.random.default_rng(11)
+    ro = g.row_offsets()
+    assert np.all(np.diff(ro) == K)
+    for j in rnd.choice(n, 4, replace=False).tolist():      # (a)
+        tg, w, d = g.connections_of(j)
+        exp = [oc.draw_connection(0, j, k) for k in range(K)]
+        et = np.array([e[1] for e in exp], np.int64); ed = np.array([e[2] for e in exp], np.int64)
+        ew = np.array([e[3] for e in exp], np.float32)
+        assert all(e[0] == j for e in exp)
+        go = np.lexsort((w.view(np.uint32), tg, d)); eo = np.lexsort((ew.view(np.uint32), et, ed))
+        assert np.array_equal(tg[go], et[eo]) and np.array_equal(d[go].astype(np.int64), ed[eo])
+        assert np.all(np.abs(w[go].view(np.uint32).astype(np.int64) - ew[eo].view(np.uint32).astype(np.int64)) <= 1)
+        assert np.all(np.diff(d.astype(np.int64)) >= 0)     # stored delay-grouped
+    thr = int(np.floor(fraction * 4294967296.0))
+    sample_t = rnd.choice(n, 3000, replace=False)
+    is_sampled = np.zeros(n, bool); is_sampled[sample_t] = True
+    expect = np.zeros((D, n)); mass = np.zeros((D, n))
+    for n_step in range(steps):
+        g.simulate(1)
+        ids = np.sort(g.last_spikes())
+        for s in rnd.choice(n, 200, replace=False).tolist():               # (b)
+            x = oracle_mod.philox4x32_10(wl.seed & 0xffffffff, wl.seed >> 32, [s, n_step, 0, 3])
+            assert (int(x[0]) < thr) == bool(np.isin(s, ids))
+        expect[n_step % D] = 0.0; mass[n_step % D] = 0.0                   # consumed and cleared by this step
+        for j in ids.tolist():
+            tg, w, d = g.records(int(ro[j]), K)
+            sl = (n_step + d.astype(np.int64)) % D
+            np.add.at(expect, (sl, tg), w.astype(np.float64))
+            np.add.at(mass, (sl, tg), np.abs(w.astype(np.float64)))
+        ring = g.get_state(B.FIELD_RING).astype(np.float64).reshape(D, n)
+        assert np.all(np.abs(ring - expect)[:, is_sampled] <= 1e-5 * mass[:, is_sampled] + 1e-12)      # (c) cells
+        assert np.all(np.abs(ring.sum(axis=1) - expect.sum(axis=1)) <= 1e-5 * mass.sum(axis=1) + 1e-6)  # (c) planes
+    st = g.stats()
+    assert st.events == st.spikes * K and st.spikes > 0                    # (d)
     g.close()
