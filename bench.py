@@ -151,7 +151,7 @@ def barrier(world):
     torch.cuda.synchronize()
 
 
-def delivery_microbench(device, peak_gbs, K=10000, fraction=0.05, steps=30, warm=5, fallback=True):
+def delivery_microbench(device, peak_gbs, K=10000, fraction=0.05, steps=30, warm=5, fallback=True, kernel=0):
     """BASELINE.json configs[3]: delivery kernel alone (neuron update bypassed), 1e6 sources, out-degree K, a random
     fraction of sources firing per step.  Falls back to K = 1000 when 90 GB of records do not fit."""
     import torch
@@ -162,7 +162,14 @@ def delivery_microbench(device, peak_gbs, K=10000, fraction=0.05, steps=30, warm
             wl = W.delivery_microbench(K=k_try, fraction=fraction)
             g = B.Sim(DT_MS, wl.ring_slots, wl.seed, record_spikes=False, device=device)
             wl.apply(g); g.prepare()
+            g.set_option(B.OPT_DELIVERY_KERNEL, kernel)
             g.simulate(warm)
+            # whole step (spike injection + delivery) in the default step mode, CUDA events on the simulator's stream
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            g.simulate(steps)
+            e0.record(g.stream); g.simulate(steps); e1.record(g.stream); torch.cuda.synchronize()
+            step_ms = e0.elapsed_time(e1) / steps
+            step_mode = int(g.stats().step_mode)
             g.set_option(B.OPT_PROFILE, 1)
             s0 = g.stats()
             g.simulate(steps)
@@ -172,6 +179,7 @@ def delivery_microbench(device, peak_gbs, K=10000, fraction=0.05, steps=30, warm
             ms = (s1.ms_deliver - s0.ms_deliver) if int(s1.delivery_kernel) != 3 else (s1.ms_update - s0.ms_update)
             out = {"workload": f"configs[3] delivery microbenchmark: 1e6 sources, out-degree {k_try}, {fraction:.1%} firing per step, D=64",
                    "steps": steps, "events_per_step": ev / steps, "deliver_ms_per_step": ms / steps,
+                   "step_ms_default_mode": step_ms, "step_mode": step_mode, "events_per_s_whole_step": ev / steps / (step_ms * 1e-3),
                    "events_per_s": ev / (ms * 1e-3), "algorithmic_gbs": ev * BYTES_PER_EVENT / (ms * 1e-3) / 1e9,
                    "frac_of_hbm_peak": ev * BYTES_PER_EVENT / (ms * 1e-3) / 1e9 / peak_gbs,
                    "delivery_kernel": int(s1.delivery_kernel),
@@ -411,6 +419,7 @@ def main():
                     help="run only the configs[3] delivery microbenchmark and print its JSON object (used for ncu captures)")
     ap.add_argument("--micro-sweep", action="store_true",
                     help="run the 3 x 3 sweep of BASELINE.json configs[3] (out-degree 100/1000/10000 x firing 0.1/1/5 %%)")
+    ap.add_argument("--micro-k-only", type=int, default=0, help="restrict --micro-sweep to one out-degree")
     ap.add_argument("--probe", action="store_true", help="run the ceiling probes (ng_probe) and print them as JSON")
     ap.add_argument("--step-mode", type=int, default=3, choices=[0, 1, 2, 3], help="NG_OPT_STEP_MODE (3 = auto)")
     ap.add_argument("--delivery-kernel", type=int, default=0, choices=[0, 1, 2, 3], help="NG_OPT_DELIVERY_KERNEL (0 = auto)")
@@ -426,11 +435,12 @@ def main():
     elif args.micro_sweep:
         # BASELINE.json configs[3]: out-degree x firing-fraction sweep of the delivery stage alone, one JSON object per line
         peak = measured_peak_gbs()[0]
-        for k in (100, 1000, 10000):
+        for k in ((100, 1000, 10000) if args.micro_k_only == 0 else (args.micro_k_only,)):
             for f in (0.001, 0.01, 0.05):
-                print(json.dumps(delivery_microbench(0, peak, K=k, fraction=f, steps=args.micro_steps, fallback=False)), flush=True)
+                print(json.dumps(delivery_microbench(0, peak, K=k, fraction=f, steps=args.micro_steps, fallback=False,
+                                                     kernel=args.delivery_kernel)), flush=True)
     elif args.only_microbench:
-        print(json.dumps(delivery_microbench(0, measured_peak_gbs()[0], K=args.micro_k, fraction=args.micro_fraction,
+        print(json.dumps(delivery_microbench(0, measured_peak_gbs()[0], K=args.micro_k, fraction=args.micro_fraction, kernel=args.delivery_kernel,
                                              steps=args.micro_steps)), flush=True)
     elif args.impl == "reference":
         run_reference(args)
