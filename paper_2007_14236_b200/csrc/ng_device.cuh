@@ -880,15 +880,19 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
             const int wib = threadIdx.x >> 5, wpu = U >> 5;
             float* __restrict__ plane = a.ring + (size_t)slot * N;
             float* __restrict__ plane1 = a.ring + (size_t)(slot + 1 == Dr ? 0 : slot + 1) * N;
+            const bool single_round = (long long)gridDim.x * U >= N;
             for (long long base = (long long)blockIdx.x * U; base < N; base += (long long)gridDim.x * U) {
                 const long long ii = base + threadIdx.x;
                 const int i = (int)ii;
                 NeuronRegs g;
                 // the row descriptor is fetched for EVERY neuron together with its state (16 B, L2-resident because it
                 // is touched every step): a spiking thread then needs no further memory round trip
+                // (only while one round covers the network: for large N the extra 16 B per neuron-step costs more
+                // bandwidth than the round trip of the few spiking threads)
                 RowInfo r;
-                if (ii < N) r = ld_row_info(a.row_info + i);
+                if (single_round && ii < N) r = ld_row_info(a.row_info + i);
                 const bool spk = ii < N && neuron_early(a, P, n, i, plane, g, have_k);
+                if (!single_round && spk) r = ld_row_info(a.row_info + i);
                 const unsigned m = __ballot_sync(0xffffffffu, spk);
                 if (m) {                                           // warp-aggregated append to the CTA's own list
                     const int leader = __ffs(m) - 1;
@@ -1095,17 +1099,18 @@ __global__ void __launch_bounds__(kPersistentThreads, 1) persistent_pipe_kernel(
     if (a.n_pops > kMaxPopsSmem) __syncthreads();
     const long long gtid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const int U = pipe_updater_threads(a.N);
+    const bool single_round = (long long)gridDim.x * U >= a.N;     // else the counts are computed in line, overlapping the loads
     long long n = sh.sc.n;
     int slot = sh.sc.slot;
     unsigned long long rec_prev = sh.sc.rec_base, spikes = 0, epoch = 0;       // recorded before step n-1 (nothing pending at entry)
     for (long long s = 0; s < n_steps; ++s, ++n) {
         if (gtid == 0) a.ctl->spike_cnt[(n + 1) & 3] = 0;          // last read (as step n-3's) in phase n-2
         trace_stamp(a, n, 0);
-        const int Mp = pipelined_phase<true>(a, P, n, slot, s > 0, rec_prev, sh, s > 0);
+        const int Mp = pipelined_phase<true>(a, P, n, slot, s > 0, rec_prev, sh, s > 0 && single_round);
         rec_prev += (unsigned long long)Mp; spikes += (unsigned long long)Mp;
         trace_stamp(a, n, 1);
         grid_arrive(a.ctl, epoch);
-        if (s + 1 < n_steps && !a.bypass && (int)threadIdx.x < U) {        // barrier shadow: Poisson counts of step n+1
+        if (s + 1 < n_steps && !a.bypass && single_round && (int)threadIdx.x < U) {    // barrier shadow: Poisson counts of step n+1
             for (long long ii = (long long)blockIdx.x * U + threadIdx.x; ii < a.N; ii += (long long)gridDim.x * U)
                 a.pois_k[ii] = (uint8_t)poisson_count(a, P + a.pop_of[ii], n + 1, (int)ii);
         }
