@@ -82,7 +82,11 @@ enum {
     NG_OPT_STEPS_PER_GRAPH = 1,  /* default 100 */
     NG_OPT_DELIVERY_KERNEL = 2,  /* 0 = auto, 1 = row-chunk walk, 2 = delay-major segment walk,
                                     3 = pipelined step kernel (delay-1 records with the update, the rest
-                                        overlapped with the next step: one grid dependency per step)      */
+                                        overlapped with the next step: one grid dependency per step),
+                                    4 = spike-buffer backend, the paper's own mechanism: no D-plane
+                                        ring; the spikes of the last ring_slots steps stay buffered and reach their
+                                        delay groups one step at a time.  Must be chosen BEFORE ng_prepare;
+                                        NG_FIELD_RING is then read-only (expanded on demand)                 */
     NG_OPT_DELIVER_BLOCKS = 3,   /* grid size of the delivery kernel, 0 = auto                         */
     NG_OPT_PROFILE = 4,          /* 1 = time every kernel with CUDA events (forces plain launches);
                                     results in ng_stats.ms_update / ms_deliver                       */
@@ -140,7 +144,7 @@ typedef struct {
     uint64_t launches_update;    /* kernel launches (or graph kernel nodes executed) since create    */
     uint64_t launches_deliver;
     uint64_t launches_other;     /* builder and bookkeeping kernels                                  */
-    int32_t delivery_kernel;     /* the delivery kernel in use (1, 2 or 3)                           */
+    int32_t delivery_kernel;     /* the delivery kernel in use (1 .. 4)                           */
     int32_t step_mode;
 } ng_stats;
 

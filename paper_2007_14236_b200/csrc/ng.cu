@@ -55,6 +55,7 @@ struct ng_sim {
     int delivery_kernel = 1; int deliver_blocks = 0; int update_blocks = 0; int persistent_blocks = 0;
     int pipe_blocks = 0; int persistent_pipe_blocks = 0;
     int persistent_threads = kPersistentThreads;
+    bool window_backend = false;           // delivery kernel 4 chosen before ng_prepare: spike window instead of a D-plane ring
     cudaGraphExec_t graph_exec = nullptr; int graph_steps = 0;
     // stats
     double build_ms = 0, ms_update = 0, ms_deliver = 0;
@@ -164,7 +165,8 @@ void launch_update(ng_sim* s) {
     update_kernel<<<s->update_blocks, kUpdateThreads, 0, s->stream>>>(s->a);
 }
 void launch_deliver(ng_sim* s) {
-    if (s->delivery_kernel == 2) deliver_kernel<2><<<s->deliver_blocks, kDeliverThreads, 0, s->stream>>>(s->a);
+    if (s->delivery_kernel == 4) deliver_kernel<4><<<s->deliver_blocks, kDeliverThreads, 0, s->stream>>>(s->a);
+    else if (s->delivery_kernel == 2) deliver_kernel<2><<<s->deliver_blocks, kDeliverThreads, 0, s->stream>>>(s->a);
     else deliver_kernel<1><<<s->deliver_blocks, kDeliverThreads, 0, s->stream>>>(s->a);
 }
 
@@ -190,12 +192,14 @@ void configure_launch(ng_sim* s) {
     const double mean_group = s->N > 0 ? (double)s->S / ((double)s->N * s->cfg.ring_slots) : 0.0;
     int k = s->delivery_kernel_opt;
     // otherwise the step is latency-bound: rows are walked whole (kernel 1) or by the pipelined step kernel (3).
-    if (k == 0) k = (ring_bytes > 0.8 * (double)s->l2_bytes && mean_group >= 4.0) ? 2 : 3;
+    if (k == 0) k = 3;                                              // a ring beyond L2 was given the window backend in ng_prepare
+    (void)mean_group; (void)ring_bytes;
+    if (s->window_backend) k = 4;                                   // fixed at ng_prepare: there is no D-plane ring
     s->delivery_kernel = k;
     // step mode: the latency-bound kernels run as one persistent cooperative kernel per ng_simulate call; the
     // bandwidth-bound delay-major kernel keeps its 8 CTAs per SM and runs from a CUDA graph
-    s->step_mode = s->step_mode_opt != 3 ? s->step_mode_opt : (k == 2 || !s->coop_ok) ? 0 : 2;
-    s->a.prefetch = (k != 2 && s->prefetch_opt) ? 1 : 0;
+    s->step_mode = s->step_mode_opt != 3 ? s->step_mode_opt : (k == 2 || k == 4 || !s->coop_ok) ? 0 : 2;
+    s->a.prefetch = (k != 2 && k != 4 && s->prefetch_opt) ? 1 : 0;
     s->pipe_blocks = grid_for(s->N, kPipeThreads - kEntryTile, sm * 4);   // updaters per CTA = kPipeThreads - kEntryTile
     {
         int occp = 0;
@@ -218,7 +222,8 @@ void configure_launch(ng_sim* s) {
     s->a.mean_row_records = (int32_t)std::max<int64_t>(1, s->N > 0 ? s->n_padded / s->N : 1);
     // persistent kernel: one CTA of persistent_threads per SM slot; few CTAs keep the grid barrier cheap
     int occ = 0;
-    if (s->delivery_kernel == 2) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, persistent_kernel<2>, s->persistent_threads, 0);
+    if (s->delivery_kernel == 4) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, persistent_kernel<4>, s->persistent_threads, 0);
+    else if (s->delivery_kernel == 2) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, persistent_kernel<2>, s->persistent_threads, 0);
     else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, persistent_kernel<1>, s->persistent_threads, 0);
     if (occ < 1) occ = 1;
     s->persistent_blocks = sm * std::min(occ, kPersistentThreads / s->persistent_threads);
@@ -265,6 +270,19 @@ int32_t ring_copy(ng_sim* s, bool to_device, void* user, int64_t count, int64_t 
     int32_t rc = read_ctl(s, &h);
     if (rc) return rc;
     const int64_t N = s->N, D = s->cfg.ring_slots, Dr = s->a.Dr, n = h.step_u;
+    if (s->window_backend) {
+        // no ring exists: the pending inputs live in the spike window.  Read-back expands them into a temporary image.
+        if (to_device) return fail(s, NG_ERR_STATE, "NG_FIELD_RING cannot be set with the spike-buffer backend (delivery kernel 4)");
+        float* img = nullptr;
+        if (!dev_alloc_t(s, &img, (size_t)N * D)) return fail(s, NG_ERR_OOM, "ring image");
+        NG_CUDA(s, cudaMemsetAsync(img, 0, (size_t)N * D * 4, s->stream));
+        NG_CUDA(s, cudaMemcpyAsync(img + (size_t)(n % D) * N, s->a.ring + (size_t)(n % 2) * N, (size_t)N * 4, cudaMemcpyDeviceToDevice, s->stream));
+        materialize_window_kernel<<<s->sm_count * 8, 256, 0, s->stream>>>(s->a, (long long)n, img);
+        NG_CUDA(s, cudaMemcpyAsync(user, img + first, (size_t)count * 4, cudaMemcpyDefault, s->stream));
+        NG_CUDA(s, cudaStreamSynchronize(s->stream));
+        dev_free(s, img);
+        return NG_OK;
+    }
     int64_t done = 0;
     while (done < count) {
         const int64_t e = first + done, slot = e / N, i0 = e % N;
@@ -373,7 +391,9 @@ int32_t ng_set_option(ng_sim* s, int32_t option, int64_t value) {
             if (value < 1 || value > 10000) return fail(s, NG_ERR_INVALID_ARG, "steps per graph in 1..10000");
             s->steps_per_graph = (int)value; destroy_graph(s); break;
         case NG_OPT_DELIVERY_KERNEL:
-            if (value < 0 || value > 3) return fail(s, NG_ERR_INVALID_ARG, "delivery kernel is 0 .. 3");
+            if (value < 0 || value > 4) return fail(s, NG_ERR_INVALID_ARG, "delivery kernel is 0 .. 4");
+            if (s->prepared && value != 0 && (value == 4) != s->window_backend)
+                return fail(s, NG_ERR_STATE, "delivery kernel 4 (spike-buffer backend) must be chosen before ng_prepare and cannot be left after it");
             s->delivery_kernel_opt = (int)value; if (s->prepared) configure_launch(s); break;
         case NG_OPT_DELIVER_BLOCKS:
             if (value < 0 || value > (1 << 20)) return fail(s, NG_ERR_INVALID_ARG, "deliver blocks out of range");
@@ -410,6 +430,12 @@ int32_t ng_prepare(ng_sim* s) {
     NG_CUDA(s, cudaSetDevice(s->cfg.device));
     const int N = s->N, D = s->cfg.ring_slots;
     cudaStream_t st = s->stream;
+    // Ring or spike window?  A ring that cannot stay in L2 (config 3: 65 planes x 4 MB) costs a DRAM round trip per plane
+    // and step; the spike-buffer backend keeps two planes whatever D is and measured faster on every point of the
+    // config 3 sweep, so it is the automatic choice there.
+    s->window_backend = s->delivery_kernel_opt == 4 ||
+                        (s->delivery_kernel_opt == 0 && (double)N * (D + 1) * 4.0 > 0.8 * (double)s->l2_bytes);
+    const int planes = s->window_backend ? 2 : D + 1;               // ring planes actually stored
     s->S = 0;
     for (const CallDev& c : s->calls) s->S += (int64_t)(c.rule == kRuleIndegree ? c.tgt_n : c.src_n) * c.K;
 
@@ -422,7 +448,7 @@ int32_t ng_prepare(ng_sim* s) {
     bool ok = dev_alloc_t(s, &s->d_ctl, 1) && dev_alloc_t(s, &s->d_pops, s->pops.size()) &&
               dev_alloc_t(s, &s->d_pop_of, (size_t)N) && dev_alloc_t(s, &s->a.V, (size_t)N) &&
               dev_alloc_t(s, &s->a.I, (size_t)N) && dev_alloc_t(s, &s->a.refr, (size_t)N) &&
-              dev_alloc_t(s, &s->a.ring, (size_t)N * (D + 1)) && dev_alloc_t(s, &s->a.spike_list, (size_t)2 * N) &&
+              dev_alloc_t(s, &s->a.ring, (size_t)N * planes) && dev_alloc_t(s, &s->a.spike_list, (size_t)2 * N) &&
               dev_alloc_t(s, &s->a.spike_row, (size_t)2 * N) && dev_alloc_t(s, &s->a.pois_k, (size_t)N) && dev_alloc_t(s, &s->d_row_info, (size_t)N) &&
               dev_alloc_t(s, &s->d_calls, std::max<size_t>(1, s->calls.size())) &&
               dev_alloc_t(s, &s->d_cnt, (size_t)N * D) && dev_alloc_t(s, &s->d_row_len, (size_t)N) &&
@@ -437,7 +463,13 @@ int32_t ng_prepare(ng_sim* s) {
     NG_CUDA(s, cudaMemsetAsync(s->d_ctl, 0, sizeof(Ctl), st));
     NG_CUDA(s, cudaMemsetAsync(s->a.I, 0, (size_t)N * 4, st));
     NG_CUDA(s, cudaMemsetAsync(s->a.refr, 0, (size_t)N * 4, st));
-    NG_CUDA(s, cudaMemsetAsync(s->a.ring, 0, (size_t)N * (D + 1) * 4, st));
+    NG_CUDA(s, cudaMemsetAsync(s->a.ring, 0, (size_t)N * planes * 4, st));
+    if (s->window_backend) {
+        // worst case N spikes per step for D steps; beyond 2^26 entries an eighth of that (overflow is detected)
+        const long long worst = (long long)N * D;
+        s->a.win_cap = worst <= (1LL << 26) ? worst : std::max(1LL << 26, worst / 8);
+        if (!dev_alloc_t(s, &s->a.win_id, (size_t)s->a.win_cap)) return fail(s, NG_ERR_OOM, "device allocation failed (spike window)");
+    }
     NG_CUDA(s, cudaMemsetAsync(s->d_cnt, 0, (size_t)N * D * 4, st));
     if (s->a.last_input) NG_CUDA(s, cudaMemsetAsync(s->a.last_input, 0, (size_t)N * 4, st));
     std::vector<PopDev> pd(s->pops.size());
@@ -503,7 +535,7 @@ int32_t ng_prepare(ng_sim* s) {
     dev_free(s, s->d_row_len); s->d_row_len = nullptr;
 
     // ---- step arguments ----
-    s->a.N = N; s->a.D = D; s->a.Dr = D + 1; s->a.n_pops = (int32_t)s->pops.size(); s->a.seed_lo = seed_lo; s->a.seed_hi = seed_hi;
+    s->a.N = N; s->a.D = D; s->a.Dr = planes; s->a.n_pops = (int32_t)s->pops.size(); s->a.seed_lo = seed_lo; s->a.seed_hi = seed_hi;
     s->a.pop_of = s->d_pop_of; s->a.pops = s->d_pops;
     s->a.row_info = s->d_row_info;
     s->a.row_off = s->d_row_off; s->a.grp_rel = s->d_grp_rel; s->a.tgt = s->d_tgt; s->a.w = s->d_w; s->a.dly = s->d_dly;
@@ -527,6 +559,7 @@ int32_t ng_set_state(ng_sim* s, int32_t field, const void* data, int64_t count, 
         if (rc) return rc;
         const unsigned long long recorded = h.rec_total[h.step_u & 1];
         h.step_u = n; h.step_d = n; h.spike_cnt[0] = h.spike_cnt[1] = h.spike_cnt[2] = h.spike_cnt[3] = 0; h.ticket = 0; h.pending = 0;
+        std::memset(h.win_start, 0, sizeof(h.win_start)); h.err_window = 0;
         h.slot = (int32_t)(n % s->a.Dr);
         h.rec_total[0] = h.rec_total[1] = recorded;
         NG_CUDA(s, cudaMemcpyAsync(s->d_ctl, &h, sizeof(Ctl), cudaMemcpyHostToDevice, s->stream));
@@ -609,7 +642,8 @@ int32_t ng_simulate(ng_sim* s, int64_t n_steps) {
             NG_CUDA(s, cudaLaunchCooperativeKernel((const void*)persistent_pipe_kernel, dim3(s->persistent_pipe_blocks),
                                                    dim3(s->persistent_threads), args, 0, st));
         } else {
-            const void* fn = s->delivery_kernel == 2 ? (const void*)persistent_kernel<2> : (const void*)persistent_kernel<1>;
+            const void* fn = s->delivery_kernel == 4 ? (const void*)persistent_kernel<4>
+                             : s->delivery_kernel == 2 ? (const void*)persistent_kernel<2> : (const void*)persistent_kernel<1>;
             NG_CUDA(s, cudaLaunchCooperativeKernel(fn, dim3(s->persistent_blocks), dim3(s->persistent_threads), args, 0, st));
         }
         s->launches_update += 1;
@@ -631,12 +665,13 @@ int32_t ng_simulate(ng_sim* s, int64_t n_steps) {
     s->steps_done += (uint64_t)n_steps;
     if (s->async) return NG_OK;
     NG_CUDA(s, cudaStreamSynchronize(st));
-    if (s->a.rec_cap > 0) {
+    if (s->a.rec_cap > 0 || s->window_backend) {
         Ctl h{};
         rc = read_ctl(s, &h);
         if (rc) return rc;
+        if (h.err_window) return fail(s, NG_ERR_OVERFLOW, "spike window overflowed: more spikes within ring_slots steps than its capacity");
         const unsigned long long total = h.rec_total[h.step_u & 1];
-        if (total > (unsigned long long)s->a.rec_cap) return fail(s, NG_ERR_OVERFLOW, "spike record full; later spikes were not recorded");
+        if (s->a.rec_cap > 0 && total > (unsigned long long)s->a.rec_cap) return fail(s, NG_ERR_OVERFLOW, "spike record full; later spikes were not recorded");
     }
     return NG_OK;
 }

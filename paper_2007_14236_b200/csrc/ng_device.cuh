@@ -18,6 +18,7 @@ enum : int32_t { kRuleIndegree = 0, kRuleOutdegree = 1 };
 enum : int32_t { kDistConst = 0, kDistNormalClipped = 1, kDistUniformInt = 2 };
 
 constexpr int kMaxPoissonTable = 64;
+constexpr int kMaxWindowSteps = 256;     // >= ring_slots (1..255)
 constexpr int kTraceSteps = 64;      // the persistent kernels keep the phase stamps of the last kTraceSteps steps
 constexpr int kTraceStamps = 16;
 constexpr int kUpdateThreads = 256;
@@ -53,7 +54,11 @@ struct Ctl {                   // device-resident control block; see ng.cu for t
     int32_t slot;                          // step_u mod Dr, kept next to step_u so no kernel divides 64-bit integers
     int32_t slot_d;                        // step_d mod Dr: written by update, read by deliver (like step_d) — the delivery
                                            // kernel's bookkeeping advances `slot` while later CTAs of the same launch still start
-    unsigned long long bar;                // persistent fused kernel: arrivals at the grid barrier
+    unsigned long long bar;                // persistent kernels: arrivals at the grid barrier
+    int32_t err_window;                    // spike-buffer backend: the spike window overflowed its capacity
+    int32_t pad2;
+    unsigned long long win_start[kMaxWindowSteps + 1];   // spike-buffer backend: absolute position in the spike window of
+                                           // the first spike of step s, at index s mod (D+1); [s+1] = its end
 };
 
 // ---------------------------------------------------------------------------------------
@@ -345,6 +350,8 @@ struct StepArgs {
     const RowInfo* row_info;     // [N]
     int32_t prefetch;            // 1: a spiking thread bulk-prefetches its row into L2 (row-walk kernels)
     uint8_t* pois_k;             // [N] Poisson counts of the next step (persistent pipelined kernel)
+    int32_t* win_id;             // spike-buffer backend (delivery kernel 4): circular log of the spikes of the last D steps
+    long long win_cap;           //   its capacity in entries; nullptr / 0 for the ring backends
     unsigned long long* trace;   // NG_OPT_TRACE: [kTraceSteps][gridDim.x][kTraceStamps] %globaltimer stamps, or nullptr
     int32_t* rec_step; int32_t* rec_id; long long rec_cap;   // rec_cap = 0: recording off
     // connection structure
@@ -379,7 +386,8 @@ __device__ __forceinline__ void prefetch_row(const StepArgs& a, const RowInfo& r
 // `rec_base` = number of spikes recorded before step n: the spiking thread also writes the spike record (a2,
 // PAPER.md:181 "all spike times of all neurons recorded").  The atomic is issued before the row lookup and the
 // prefetches so that all three overlap.
-__device__ __forceinline__ void append_spike(const StepArgs& a, bool spk, int32_t id, long long n, unsigned long long rec_base) {
+__device__ __forceinline__ void append_spike(const StepArgs& a, bool spk, int32_t id, long long n, unsigned long long rec_base,
+                                             unsigned long long win_base = 0) {
     const unsigned m = __ballot_sync(0xffffffffu, spk);
     if (m == 0) return;
     const int lane = threadIdx.x & 31;
@@ -387,7 +395,7 @@ __device__ __forceinline__ void append_spike(const StepArgs& a, bool spk, int32_
     int base = 0;
     if (lane == leader) base = atomicAdd(&a.ctl->spike_cnt[n & 3], __popc(m));
     RowInfo r;
-    if (spk) { r = ld_row_info(a.row_info + id); if (a.prefetch) prefetch_row(a, r); }
+    if (spk) { r = ld_row_info(a.row_info + id); if (a.prefetch && !a.win_id) prefetch_row(a, r); }
     base = __shfl_sync(0xffffffffu, base, leader);
     if (spk) {
         const int idx = base + __popc(m & ((1u << lane) - 1u));
@@ -396,6 +404,7 @@ __device__ __forceinline__ void append_spike(const StepArgs& a, bool spk, int32_
         st_row_info(a.spike_row + k, r);
         const unsigned long long pos = rec_base + (unsigned long long)idx;
         if (pos < (unsigned long long)a.rec_cap) { a.rec_id[pos] = id; a.rec_step[pos] = (int32_t)n; }
+        if (a.win_id) a.win_id[(win_base + (unsigned long long)idx) % (unsigned long long)a.win_cap] = id;
     }
 }
 
@@ -464,7 +473,8 @@ __device__ __forceinline__ void neuron_late(const StepArgs& a, const PopDev* __r
 }
 
 __device__ __forceinline__ void update_phase(const StepArgs& a, const PopDev* __restrict__ P, long long n, int slot,
-                                             unsigned long long rec_base, long long gtid, long long gthreads) {
+                                             unsigned long long rec_base, long long gtid, long long gthreads,
+                                             unsigned long long win_base = 0) {
     const int N = a.N;
     float* __restrict__ plane = a.ring + (size_t)slot * N;
     const long long n_round = ((long long)N + 31) & ~31LL;      // keep warps whole for the ballot
@@ -472,7 +482,7 @@ __device__ __forceinline__ void update_phase(const StepArgs& a, const PopDev* __
         const int i = (int)ii;
         NeuronRegs g;
         const bool spk = i < N && neuron_early(a, P, n, i, plane, g);
-        append_spike(a, spk, i, n, rec_base);
+        append_spike(a, spk, i, n, rec_base, win_base);
         if (i < N) neuron_late(a, P, n, i, plane, g);
     }
 }
@@ -675,11 +685,16 @@ __device__ __forceinline__ void red_vec(const StepArgs& a, const VecRef& r, cons
     if (r.q + 3 >= r.rel_lo && r.q + 3 < r.len) red_add_f32(plane + t.w, ww.w);
 }
 
+// kWindow (delivery kernel 4, the paper's spike-buffer mechanism): no ring.  The spikes of the last D steps
+// stay in a time-ordered window; a spike of step s "reaches" its connection group of delay d in step n = s + d - 1, so
+// the items of step n are (window entry, delay = age + 1) and every reduction goes into the ONE input plane of step n+1.
+// `off` (shared memory) holds the W + 1 window offsets of steps n-W+1 .. n and the end.
+template <bool kWindow>
 __device__ __forceinline__ void deliver_groups_phase(const StepArgs& a, long long n, int nmod, int M, long long gwarp,
-                                                     long long gwarps, int lane) {
+                                                     long long gwarps, int lane, const unsigned long long* off = nullptr, int W = 0) {
     const int N = a.N, D = a.D, Dr = a.Dr;
     const int32_t* __restrict__ list = a.spike_list + (size_t)(n & 1) * N;
-    const long long items = (long long)M * D;
+    const long long items = kWindow ? (long long)(off[W] - off[0]) : (long long)M * D;
     if (items == 0) return;
     const long long bsz = (items + gwarps - 1) / gwarps;
     const int batch = bsz > 32 ? 32 : (int)bsz;
@@ -693,13 +708,19 @@ __device__ __forceinline__ void deliver_groups_phase(const StepArgs& a, long lon
     auto item_of = [&](long long b, int& d, int& si) -> bool {
         const long long it = b * batch + lane;
         if (b >= n_batches || lane >= batch || it >= items) return false;
-        if (small) { d = (int)((uint32_t)it / (uint32_t)M); si = (int)((uint32_t)it - (uint32_t)d * (uint32_t)M); }
+        if (kWindow) {                                                   // oldest step first: delay-major like the ring walk
+            const unsigned long long pos = off[0] + (unsigned long long)it;
+            int lo = 0, hi = W;                                          // largest k with off[k] <= pos
+            while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (off[mid] <= pos) lo = mid; else hi = mid; }
+            d = W - 1 - lo;                                              // 0-based delay index: age of the spike
+            si = (int)(pos % (unsigned long long)a.win_cap);
+        } else if (small) { d = (int)((uint32_t)it / (uint32_t)M); si = (int)((uint32_t)it - (uint32_t)d * (uint32_t)M); }
         else { d = (int)(it / M); si = (int)(it - (long long)d * M); }
         return true;
     };
     auto load_j = [&](long long b) -> int {
         int d, si;
-        return item_of(b, d, si) ? __ldcg(list + si) : -1;
+        return item_of(b, d, si) ? __ldcg((kWindow ? a.win_id : list) + si) : -1;
     };
     int d_cur = 0, d_nxt = 0, si_unused;
     uint32_t ga_cur = 0, gb_cur = 0, ga_nxt = 0, gb_nxt = 0;
@@ -728,7 +749,8 @@ __device__ __forceinline__ void deliver_groups_phase(const StepArgs& a, long lon
             rel_lo = (int)(lo - pbase);
             len = rel_lo + (int)(gb_cur - ga_cur);
             nvec = (len + 3) >> 2;
-            slot = nmod + d_cur + 1; if (slot >= Dr) slot -= Dr;
+            if (kWindow) slot = nmod == 0 ? 1 : 0;                      // two planes: this step's and the next step's input
+            else { slot = nmod + d_cur + 1; if (slot >= Dr) slot -= Dr; }
         }
         int incl = nvec;                                                // lay the vectors of the batch end to end
 #pragma unroll
@@ -1133,24 +1155,49 @@ __global__ void __launch_bounds__(kPersistentThreads, 1) persistent_pipe_kernel(
 }
 
 // ------------------------------- stand-alone kernels ---------------------------------
+struct WindowShared { unsigned long long off[kMaxWindowSteps + 1]; int W; };
+
+// offsets of the window of step n: steps n-W+1 .. n (W = min(D, n+1)) and the end = start of step n + M
+__device__ __forceinline__ void stage_window(const StepArgs& a, long long n, int M, WindowShared& ws) {
+    const int D = a.D;
+    const int W = (int)(n + 1 < (long long)D ? n + 1 : (long long)D);
+    for (int k = threadIdx.x; k <= W; k += blockDim.x) {
+        const long long s = n - W + 1 + (k < W ? k : W - 1);
+        const unsigned long long v = __ldcg(&a.ctl->win_start[(unsigned long long)s % (unsigned)(D + 1)]);
+        ws.off[k] = k < W ? v : v + (unsigned long long)M;
+    }
+    if (threadIdx.x == 0) ws.W = W;
+    __syncthreads();
+}
+// one thread, after the offsets are staged: publish the start of step n+1 and flag an overflow of the window
+__device__ __forceinline__ void window_bookkeeping(const StepArgs& a, long long n, const WindowShared& ws) {
+    a.ctl->win_start[(unsigned long long)(n + 1) % (unsigned)(a.D + 1)] = ws.off[ws.W];
+    if (ws.off[ws.W] - ws.off[0] > (unsigned long long)a.win_cap) a.ctl->err_window = 1;
+}
+
 __global__ void __launch_bounds__(kUpdateThreads) update_kernel(const StepArgs a) {
     __shared__ PopDev sh_pops[kMaxPopsSmem];
     __shared__ StepScalars sc;
+    __shared__ unsigned long long win_base;
     if (threadIdx.x == 0) {
         sc.n = __ldcg(&a.ctl->step_u);
         sc.slot = __ldcg(&a.ctl->slot);
         sc.rec_base = __ldcg(&a.ctl->rec_total[sc.n & 1]);
+        win_base = a.win_id ? __ldcg(&a.ctl->win_start[(unsigned long long)sc.n % (unsigned)(a.D + 1)]) : 0ULL;
         if (blockIdx.x == 0) { a.ctl->step_d = sc.n; a.ctl->slot_d = sc.slot; }
     }
     const PopDev* P = stage_pops(a, sh_pops);              // contains the __syncthreads that publishes sc
     if (a.n_pops > kMaxPopsSmem) __syncthreads();
-    update_phase(a, P, sc.n, sc.slot, sc.rec_base, (long long)blockIdx.x * blockDim.x + threadIdx.x, (long long)gridDim.x * blockDim.x);
+    update_phase(a, P, sc.n, sc.slot, sc.rec_base, (long long)blockIdx.x * blockDim.x + threadIdx.x, (long long)gridDim.x * blockDim.x,
+                 win_base);
 }
 
+// kKernel 1: row-chunk walk, 2: delay-major segment walk, 4: spike-buffer backend (segment walk over the spike window)
 template <int kKernel>
 __global__ void __launch_bounds__(kDeliverThreads, 3) deliver_kernel(const StepArgs a) {
     __shared__ DeliverShared sh;
     __shared__ StepScalars sc;
+    __shared__ WindowShared ws;
     if (threadIdx.x == 0) {
         sc.n = __ldcg(&a.ctl->step_d);
         sc.slot = __ldcg(&a.ctl->slot_d);
@@ -1161,7 +1208,13 @@ __global__ void __launch_bounds__(kDeliverThreads, 3) deliver_kernel(const StepA
     const long long gthreads = (long long)gridDim.x * blockDim.x;
     int M;
     if (kKernel == 1) M = deliver_rows_phase(a, sc.n, sc.slot, sh);
-    else { M = sc.M; deliver_groups_phase(a, sc.n, sc.slot, M, gtid >> 5, gthreads >> 5, threadIdx.x & 31); }
+    else if (kKernel == 2) { M = sc.M; deliver_groups_phase<false>(a, sc.n, sc.slot, M, gtid >> 5, gthreads >> 5, threadIdx.x & 31); }
+    else {
+        M = sc.M;
+        stage_window(a, sc.n, M, ws);
+        deliver_groups_phase<true>(a, sc.n, sc.slot, M, gtid >> 5, gthreads >> 5, threadIdx.x & 31, ws.off, ws.W);
+        if (gtid == 0) window_bookkeeping(a, sc.n, ws);
+    }
     if (gtid == 0) bookkeeping_scalar(a, sc.n, sc.slot, M, __ldcg(&a.ctl->rec_total[sc.n & 1]));
 }
 
@@ -1175,21 +1228,24 @@ __global__ void __launch_bounds__(kPersistentThreads, 1) persistent_kernel(const
     __shared__ PopDev sh_pops[kMaxPopsSmem];
     __shared__ DeliverShared sh;
     __shared__ StepScalars sc;
+    __shared__ WindowShared ws;
+    __shared__ unsigned long long win_base_sh;
     if (threadIdx.x == 0) {
         sc.n = __ldcg(&a.ctl->step_u);
         sc.slot = __ldcg(&a.ctl->slot);
         sc.rec_base = __ldcg(&a.ctl->rec_total[sc.n & 1]);
+        win_base_sh = a.win_id ? __ldcg(&a.ctl->win_start[(unsigned long long)sc.n % (unsigned)(a.D + 1)]) : 0ULL;
     }
     const PopDev* P = stage_pops(a, sh_pops);
     if (a.n_pops > kMaxPopsSmem) __syncthreads();
     long long n = sc.n;
     int slot = sc.slot;
-    unsigned long long rec_base = sc.rec_base, spikes = 0, epoch = 0;
+    unsigned long long rec_base = sc.rec_base, spikes = 0, epoch = 0, win_base = win_base_sh;
     for (long long s = 0; s < n_steps; ++s, ++n) {
         // the counter of step n+1 was last read (as step n-3's) before the barriers of step n-1
         if (gtid == 0) a.ctl->spike_cnt[(n + 1) & 3] = 0;
         trace_stamp(a, n, 0);
-        update_phase(a, P, n, slot, rec_base, gtid, gthreads);
+        update_phase(a, P, n, slot, rec_base, gtid, gthreads, win_base);
         trace_stamp(a, n, 1);
         grid_barrier(a.ctl, epoch);
         trace_stamp(a, n, 2);
@@ -1199,10 +1255,15 @@ __global__ void __launch_bounds__(kPersistentThreads, 1) persistent_kernel(const
             if (threadIdx.x == 0) sc.M = __ldcg(&a.ctl->spike_cnt[n & 3]);
             __syncthreads();
             M = sc.M;
-            deliver_groups_phase(a, n, slot, M, gtid >> 5, gthreads >> 5, threadIdx.x & 31);
-            __syncthreads();                               // sc.M is rewritten next step
+            if (kKernel == 2) deliver_groups_phase<false>(a, n, slot, M, gtid >> 5, gthreads >> 5, threadIdx.x & 31);
+            else {
+                stage_window(a, n, M, ws);
+                deliver_groups_phase<true>(a, n, slot, M, gtid >> 5, gthreads >> 5, threadIdx.x & 31, ws.off, ws.W);
+                if (gtid == 0) window_bookkeeping(a, n, ws);
+            }
+            __syncthreads();                               // sc.M and the window offsets are rewritten next step
         }
-        rec_base += (unsigned long long)M; spikes += (unsigned long long)M;
+        rec_base += (unsigned long long)M; spikes += (unsigned long long)M; win_base += (unsigned long long)M;
         trace_stamp(a, n, 3);
         grid_barrier(a.ctl, epoch);
         trace_stamp(a, n, 5);
@@ -1214,6 +1275,29 @@ __global__ void __launch_bounds__(kPersistentThreads, 1) persistent_kernel(const
         a.ctl->step_d = n - 1;
         a.ctl->slot = slot;
         a.ctl->step_u = n;
+    }
+}
+
+// Spike-buffer backend, read-back only (NG_FIELD_RING): expand the pending part of the spike window into a [D][N] ring
+// image: entry (step s, source j), record (target, w, d) with s + d > n arrives in step s + d (slot (s+d) mod D).
+__global__ void materialize_window_kernel(const StepArgs a, long long n, float* __restrict__ out) {
+    const int D = a.D, N = a.N;
+    const int W = (int)(n < (long long)D ? n : (long long)D);                      // steps n-W .. n-1 are buffered
+    const int lane = threadIdx.x & 31;
+    const long long gwarp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5, gwarps = ((long long)gridDim.x * blockDim.x) >> 5;
+    for (int k = 0; k < W; ++k) {
+        const long long s = n - W + k;
+        const unsigned long long b0 = a.ctl->win_start[(unsigned long long)s % (unsigned)(D + 1)];
+        const unsigned long long b1 = a.ctl->win_start[(unsigned long long)(s + 1) % (unsigned)(D + 1)];
+        for (unsigned long long pos = b0 + (unsigned long long)gwarp; pos < b1; pos += (unsigned long long)gwarps) {
+            const int j = a.win_id[pos % (unsigned long long)a.win_cap];
+            const long long r0 = a.row_off[j];
+            const int deg = (int)a.grp_rel[(size_t)j * (D + 1) + D];
+            for (int q = lane; q < deg; q += 32) {
+                const int d = a.dly[r0 + q];
+                if (s + d >= n + 1) atomicAdd(out + (size_t)((s + d) % D) * N + a.tgt[r0 + q], a.w[r0 + q]);
+            }
+        }
     }
 }
 

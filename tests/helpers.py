@@ -5,14 +5,17 @@ from __future__ import annotations
 import numpy as np
 
 
-def make_pair(wl, oracle_mod, debug_input=True, record=True, **sim_kw):
-    """(oracle, gpu sim) for workload `wl`, both prepared, same fp32 initial V."""
+def make_pair(wl, oracle_mod, debug_input=True, record=True, pre_options=None, **sim_kw):
+    """(oracle, gpu sim) for workload `wl`, both prepared, same fp32 initial V.  `pre_options`: {option: value} set
+    before ng_prepare (the spike-buffer backend, delivery kernel 4, must be chosen there)."""
     from paper_2007_14236_b200 import binding as B
     o = oracle_mod.Oracle(0.1, wl.ring_slots, wl.seed)
     wl.apply(o)
     o.prepare()
     g = B.Sim(0.1, wl.ring_slots, wl.seed, record_spikes=record, debug_input=debug_input, **sim_kw)
     wl.apply(g)
+    for opt, val in (pre_options or {}).items():
+        g.set_option(opt, val)
     g.prepare()
     if not wl.bypass_neurons:
         v0 = wl.initial_v()

@@ -35,11 +35,12 @@ def ring_mass(o, wl, oracle_mod, n_steps, spikes_by_step):
     (1000, 0.05, 2, 1), (1000, 0.002, 2, 2), (1000, 0.002, 1, 2), (37, 0.03, 2, 0), (3, 0.5, 2, 0),
     (100, 0.05, 3, 0), (1000, 0.01, 3, 1), (1000, 0.002, 3, 2), (37, 0.03, 3, 2), (3, 0.5, 3, 0), (1500, 0.3, 3, 0),
     (1500, 0.3, 3, 2), (1000, 0.05, 1, 0),
+    (100, 0.05, 4, 0), (1000, 0.01, 4, 1), (1000, 0.002, 4, 2), (37, 0.03, 4, 2), (3, 0.5, 4, 0), (1500, 0.3, 4, 0),
 ])
 def test_delivery_only_matches_oracle(oracle_mod, B, K, fraction, kernel, mode):
     n, steps = 20000, 70                       # 70 > D = 64: the ring wraps
     wl = W.delivery_microbench(n=n, K=K, fraction=fraction, n_steps=steps, seed=5)
-    o, g = make_pair(wl, oracle_mod, debug_input=False)
+    o, g = make_pair(wl, oracle_mod, debug_input=False, pre_options={B.OPT_DELIVERY_KERNEL: kernel} if kernel == 4 else None)
     g.set_option(B.OPT_DELIVERY_KERNEL, kernel)
     g.set_option(B.OPT_STEP_MODE, mode)
     g.simulate(steps)
@@ -122,7 +123,8 @@ def test_delivery_invariants_large(B, kernel):
 @pytest.mark.parametrize("K,fraction", [(10_000, 0.001), (1000, 0.05), (100, 0.05)])
 def test_cfg3_full_size_sampled(oracle_mod, B, K, fraction):
     """BASELINE.json configs[3] at its full size (10^6 sources, out-degree K, 10^6-neuron pool, D = 64) in the launch
-    configuration bench.py's delivery microbenchmark times (default options: delay-major kernel 2 from a CUDA graph).
+    configuration bench.py's delivery microbenchmark times (default options: spike-buffer backend, kernel 4, from a CUDA
+    graph; NG_FIELD_RING is then the on-demand expansion of the pending spike window).
     The oracle cannot hold 10^10 records, so: (a) sampled rows are compared record for record with the oracle's O(1)
     regeneration of the same draws (fixed-outdegree rule: draws (call 0, source j, k)); (b) the injected spike set of a
     step equals the oracle's Philox rule on sampled sources; (c) for a sampled set of targets every ring cell (all
@@ -133,9 +135,9 @@ def test_cfg3_full_size_sampled(oracle_mod, B, K, fraction):
     g = B.Sim(0.1, D, wl.seed, record_spikes=True, max_recorded_spikes=1 << 22)
     wl.apply(g); g.prepare()
     st = g.stats()
-    # auto rule: delay-major kernel 2 from a CUDA graph when groups are long enough, else the pipelined kernel 3
+    # auto rule: a ring of 65 x 4 MB cannot stay in L2 -> spike-buffer backend (kernel 4) from a CUDA graph
     assert st.n_connections == n * K
-    assert (st.delivery_kernel, st.step_mode) == ((2, B.STEP_GRAPH) if K >= 1000 else (3, B.STEP_PERSISTENT))
+    assert (st.delivery_kernel, st.step_mode) == (4, B.STEP_GRAPH)
     oc = oracle_mod.Oracle(0.1, D, wl.seed)
     wl.apply(oc)                                             # calls only; never prepared
     rnd = np.random.default_rng(11)
@@ -173,3 +175,24 @@ def test_cfg3_full_size_sampled(oracle_mod, B, K, fraction):
     st = g.stats()
     assert st.events == st.spikes * K and st.spikes > 0                    # (d)
     g.close()
+
+
+def test_spike_buffer_backend_api(B):
+    """Delivery kernel 4 must be chosen before ng_prepare, cannot be left afterwards, and NG_FIELD_RING is read-only."""
+    wl = W.delivery_microbench(n=5000, K=50, fraction=0.05, n_steps=10, seed=2)
+    g = B.Sim(0.1, wl.ring_slots, wl.seed, record_spikes=True)
+    wl.apply(g); g.set_option(B.OPT_DELIVERY_KERNEL, 4); g.prepare()
+    assert g.stats().delivery_kernel == 4
+    with pytest.raises(B.NgError):
+        g.set_option(B.OPT_DELIVERY_KERNEL, 1)
+    g.simulate(5)
+    ring = g.get_state(B.FIELD_RING)
+    assert ring.size == 5000 * wl.ring_slots and np.count_nonzero(ring) > 0
+    with pytest.raises(B.NgError):
+        g.set_state(B.FIELD_RING, ring)
+    g.close()
+    g2 = B.Sim(0.1, wl.ring_slots, wl.seed)
+    wl.apply(g2); g2.prepare()
+    with pytest.raises(B.NgError):
+        g2.set_option(B.OPT_DELIVERY_KERNEL, 4)
+    g2.close()
