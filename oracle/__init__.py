@@ -17,16 +17,18 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "oracle.cpp")
+_HDR = os.path.join(_HERE, "oracle_adex.hpp")
 _LIB = os.path.join(_HERE, "liboracle.so")
 
 FIELD_V, FIELD_I_SYN, FIELD_REFR, FIELD_RING, FIELD_STEP = 0, 1, 2, 3, 4
+FIELD_W, FIELD_G_EX, FIELD_Y_EX, FIELD_G_IN, FIELD_Y_IN, FIELD_H_INT = 6, 7, 8, 9, 10, 11        # AdEx state
 DIST_CONST, DIST_NORMAL_CLIPPED, DIST_UNIFORM_INT = 0, 1, 2
 RULE_FIXED_INDEGREE, RULE_FIXED_OUTDEGREE = 0, 1
 
 
 def build(force: bool = False) -> str:
     """Compile oracle.cpp with g++ (no fast-math, no FMA contraction)."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < max(os.path.getmtime(_SRC), os.path.getmtime(_HDR)):
         cmd = ["g++", "-O2", "-std=c++17", "-ffp-contract=off", "-fno-fast-math", "-shared", "-fPIC",
                _SRC, "-o", _LIB]
         subprocess.check_call(cmd)
@@ -37,6 +39,22 @@ class _LifParams(C.Structure):
     _fields_ = [(k, C.c_double) for k in
                 ("C_m", "tau_m", "tau_syn", "E_L", "V_th", "V_reset", "t_ref_ms", "I_e",
                  "poisson_rate_hz", "poisson_weight")]
+
+
+_ADEX_SCALARS = ("C_m", "g_L", "E_L", "V_T", "Delta_T", "tau_w", "a", "b", "V_reset", "V_peak", "E_ex", "E_in", "tau_syn",
+                 "I_e", "poisson_rate_hz", "poisson_weight")
+
+
+class _AdexParams(C.Structure):
+    _fields_ = [(k, C.c_double) for k in _ADEX_SCALARS] + [("tol", C.c_double * 6), ("h_min", C.c_double)]
+
+
+def _adex(params: dict) -> _AdexParams:
+    p = _AdexParams(**{k: float(params.get(k, 0.0)) for k in _ADEX_SCALARS})
+    for i, t in enumerate(params["tol"]):
+        p.tol[i] = float(t)
+    p.h_min = float(params["h_min"])
+    return p
 
 
 class _Dist(C.Structure):
@@ -59,6 +77,11 @@ def lib():
         L.orc_set_bypass.argtypes = [C.c_void_p, C.c_int32, C.c_double]
         L.orc_create_population.argtypes = [C.c_void_p, C.c_int32, C.POINTER(_LifParams), C.POINTER(C.c_int32)]
         L.orc_connect.argtypes = [C.c_void_p] + [C.c_int32] * 6 + [C.POINTER(_Dist), C.POINTER(_Dist)]
+        L.orc_connect_port.argtypes = [C.c_void_p] + [C.c_int32] * 6 + [C.POINTER(_Dist), C.POINTER(_Dist), C.c_int32]
+        L.orc_create_population_adex.argtypes = [C.c_void_p, C.c_int32, C.POINTER(_AdexParams), C.POINTER(C.c_int32)]
+        L.orc_adex_rhs.argtypes = [C.POINTER(_AdexParams), C.c_void_p, C.c_void_p]
+        L.orc_adex_step.argtypes = [C.POINTER(_AdexParams), C.c_void_p, C.c_void_p, C.c_double]
+        L.orc_num_ports.argtypes = [C.c_void_p]
         L.orc_prepare.argtypes = [C.c_void_p]
         L.orc_num_connections.restype = C.c_int64
         L.orc_num_connections.argtypes = [C.c_void_p]
@@ -117,6 +140,22 @@ def propagators(params: dict, h: float) -> np.ndarray:
     return out
 
 
+def adex_rhs(params: dict, y) -> np.ndarray:
+    """Right-hand side of the AdEx system (oracle_adex.hpp): y = (V, w, g_ex, y_ex, g_in, y_in)."""
+    a = np.ascontiguousarray(y, dtype=np.float64); f = np.zeros(6)
+    p = _adex(params)
+    lib().orc_adex_rhs(C.byref(p), a.ctypes.data, f.ctypes.data)
+    return f
+
+
+def adex_step(params: dict, y, h_int: float, h_step: float):
+    """One time step of the adaptive Cash-Karp integrator: returns (y', h_int', spiked)."""
+    a = np.array(y, dtype=np.float64); h = np.array([h_int], dtype=np.float64)
+    p = _adex(params)
+    spk = lib().orc_adex_step(C.byref(p), a.ctypes.data, h.ctypes.data, float(h_step))
+    return a, float(h[0]), bool(spk)
+
+
 def poisson_table(lam: float) -> np.ndarray:
     out = np.zeros(64, dtype=np.uint32)
     n = lib().orc_poisson_table(lam, out.ctypes.data, 64)
@@ -145,21 +184,33 @@ class Oracle:
     def set_bypass(self, bypass: bool, inject_fraction: float = 0.0):
         self._chk(self._L.orc_set_bypass(self._h, int(bypass), inject_fraction))
 
+    def create_population_adex(self, n: int, params: dict) -> int:
+        first = C.c_int32()
+        p = _adex(params)
+        self._chk(self._L.orc_create_population_adex(self._h, n, C.byref(p), C.byref(first)))
+        return first.value
+
+    @property
+    def n_ports(self) -> int:
+        return self._L.orc_num_ports(self._h)
+
     def create_population(self, n: int, params: dict) -> int:
+        if params.get("model") == "adex":
+            return self.create_population_adex(n, params)
         first = C.c_int32()
         p = _lif(params)
         self._chk(self._L.orc_create_population(self._h, n, C.byref(p), C.byref(first)))
         return first.value
 
-    def connect_fixed_indegree(self, src_first, src_n, tgt_first, tgt_n, K, weight, delay):
+    def connect_fixed_indegree(self, src_first, src_n, tgt_first, tgt_n, K, weight, delay, port: int = 0):
         w, d = _dist(weight), _dist(delay)
-        self._chk(self._L.orc_connect(self._h, RULE_FIXED_INDEGREE, src_first, src_n, tgt_first, tgt_n, K,
-                                      C.byref(w), C.byref(d)))
+        self._chk(self._L.orc_connect_port(self._h, RULE_FIXED_INDEGREE, src_first, src_n, tgt_first, tgt_n, K,
+                                           C.byref(w), C.byref(d), port))
 
-    def connect_fixed_outdegree(self, src_first, src_n, tgt_first, tgt_n, K, weight, delay):
+    def connect_fixed_outdegree(self, src_first, src_n, tgt_first, tgt_n, K, weight, delay, port: int = 0):
         w, d = _dist(weight), _dist(delay)
-        self._chk(self._L.orc_connect(self._h, RULE_FIXED_OUTDEGREE, src_first, src_n, tgt_first, tgt_n, K,
-                                      C.byref(w), C.byref(d)))
+        self._chk(self._L.orc_connect_port(self._h, RULE_FIXED_OUTDEGREE, src_first, src_n, tgt_first, tgt_n, K,
+                                           C.byref(w), C.byref(d), port))
 
     def prepare(self):
         self._chk(self._L.orc_prepare(self._h))
@@ -204,7 +255,7 @@ class Oracle:
             self._chk(self._L.orc_get_state(self._h, field, a.ctypes.data, 1, 0))
             return int(a[0])
         if n is None:
-            n = self.n_neurons * (self.D if field == FIELD_RING else 1) - first
+            n = self.n_neurons * (self.D * self.n_ports if field == FIELD_RING else 1) - first
         a = np.empty(n, np.int32 if field == FIELD_REFR else np.float64)
         self._chk(self._L.orc_get_state(self._h, field, a.ctypes.data, n, first))
         return a

@@ -44,6 +44,8 @@
 #include <string>
 #include <vector>
 
+#include "oracle_adex.hpp"
+
 namespace {
 
 // ---------------------------------------------------------------------------------
@@ -73,7 +75,9 @@ void philox4x32_10(uint32_t key_lo, uint32_t key_hi, const uint32_t ctr[4], uint
 enum { TAG_CONN = 1, TAG_POISSON = 2, TAG_INJECT = 3 };     // counter word 3 (reading C1)
 enum { DIST_CONST = 0, DIST_NORMAL_CLIPPED = 1, DIST_UNIFORM_INT = 2 };
 enum { RULE_FIXED_INDEGREE = 0, RULE_FIXED_OUTDEGREE = 1 };
-enum { FIELD_V = 0, FIELD_I_SYN = 1, FIELD_REFR = 2, FIELD_RING = 3, FIELD_STEP = 4 };
+enum { FIELD_V = 0, FIELD_I_SYN = 1, FIELD_REFR = 2, FIELD_RING = 3, FIELD_STEP = 4,
+       FIELD_W = 6, FIELD_G_EX = 7, FIELD_Y_EX = 8, FIELD_G_IN = 9, FIELD_Y_IN = 10, FIELD_H_INT = 11 };   // AdEx state
+enum { MODEL_LIF = 0, MODEL_ADEX = 1 };
 
 struct LifParams {           // PAPER.md:93-102 symbols; units pF, ms, mV, pA, Hz
     double C_m, tau_m, tau_syn, E_L, V_th, V_reset, t_ref_ms, I_e, poisson_rate_hz, poisson_weight;
@@ -82,6 +86,8 @@ struct Dist { int32_t kind; int32_t pad; double a, b, lo, hi; };
 
 struct Population {
     int32_t first, n;
+    int32_t model = MODEL_LIF;
+    adex::Params ax{};                // MODEL_ADEX (oracle_adex.hpp)
     LifParams p;
     double P11, P22, P21, P20;        // exact-integration propagators
     int32_t refr_steps;
@@ -90,8 +96,9 @@ struct Population {
 struct ConnectCall {
     int32_t rule, src_first, src_n, tgt_first, tgt_n, K;
     Dist w, d;
+    int32_t port = 0;                 // receptor port of the targets: 0 excitatory (and the LIF current), 1 inhibitory
 };
-struct Conn { int32_t src, tgt; int32_t delay; float w; int32_t call; int32_t endpoint; int32_t k; };
+struct Conn { int32_t src, tgt; int32_t delay; float w; int32_t call; int32_t endpoint; int32_t k; int32_t port; };
 
 // Exact-integration propagators of Eqs. (1)-(2) over one step h (ref. 20).
 // State x = (I, V - E_L);  dx/dt = A x,  A = [[-1/tau_syn, 0], [1/C_m, -1/tau_m]]  (R_m = tau_m/C_m).
@@ -133,7 +140,9 @@ struct Sim {
     std::vector<int64_t> row_off;          // N+1
     // state (fp64)
     std::vector<double> V, I; std::vector<int32_t> refr; std::vector<int32_t> pop_of;
-    std::vector<double> ring;              // [D][N], slot-major
+    std::vector<double> ring;              // [D][P][N], slot-major, P = n_ports
+    int32_t P = 1;                         // receptor ports: 2 as soon as an AdEx population exists
+    std::vector<adex::State> ax;           // AdEx state (unused entries for LIF neurons)
     int64_t step = 0;
     std::vector<int32_t> spk_step, spk_id; // spike record
     std::vector<int32_t> last_spikes;      // ids that spiked in the most recent step
@@ -193,7 +202,7 @@ void draw_conn(const Sim& s, int32_t call_idx, int32_t endpoint, int32_t k, Conn
         d = (int64_t)f;
     }
     out.delay = (int32_t)d;
-    out.call = call_idx; out.endpoint = endpoint; out.k = k;
+    out.call = call_idx; out.endpoint = endpoint; out.k = k; out.port = c.port;
 }
 
 int poisson_count(const Sim& s, const Population& pop, int32_t i, int64_t n) {
@@ -251,7 +260,15 @@ int prepare(Sim& s) {
         Population& p = s.pops[pi];
         for (int32_t i = p.first; i < p.first + p.n; ++i) { s.V[i] = p.p.E_L; s.pop_of[i] = pi; }
     }
-    s.ring.assign((size_t)s.D * (size_t)N, 0.0);
+    s.P = 1;
+    for (auto& p : s.pops) if (p.model == MODEL_ADEX) s.P = 2;
+    s.ax.assign(N, adex::State{});
+    for (auto& p : s.pops) if (p.model == MODEL_ADEX)
+        for (int32_t i = p.first; i < p.first + p.n; ++i) {
+            adex::State st{}; st.y[0] = p.ax.E_L; st.h_int = s.dt_ms;
+            s.ax[i] = st; s.V[i] = p.ax.E_L;
+        }
+    s.ring.assign((size_t)s.D * (size_t)s.P * (size_t)N, 0.0);
     s.step = 0;
     s.prepared = true;
     return 0;
@@ -260,18 +277,34 @@ int prepare(Sim& s) {
 // One time step n: t_n -> t_{n+1}.  DESIGN.md oracle algorithm, steps 3a-3d then 4.
 void step_once(Sim& s, bool record) {
     const int32_t N = s.N; const int32_t D = s.D; const int64_t n = s.step;
+    const size_t P = (size_t)s.P;
     const size_t slot = (size_t)(n % D);
     s.last_spikes.clear();
     for (int32_t i = 0; i < N; ++i) {
-        // 3a. consume and clear this step's ring slot
-        double in = s.ring[slot * N + i];
-        s.ring[slot * N + i] = 0.0;
+        // 3a. consume and clear this step's ring slot (port 0; port 1 exists only next to AdEx populations)
+        double in = s.ring[(slot * P) * N + i];
+        s.ring[(slot * P) * N + i] = 0.0;
+        double in1 = 0.0;
+        if (P > 1) { in1 = s.ring[(slot * P + 1) * N + i]; s.ring[(slot * P + 1) * N + i] = 0.0; }
         if (s.bypass_neurons) {                       // config-3 mode, reading C8
             if (inject_fires(s, i, n)) s.last_spikes.push_back(i);
             continue;
         }
         const Population& pop = s.pops[s.pop_of[i]];
         int k = poisson_count(s, pop, i, n);
+        if (pop.model == MODEL_ADEX) {
+            // AdEx + alpha conductances, adaptive RK5 over the step (oracle_adex.hpp), then the
+            // conductance jumps arriving at t_{n+1} (C25): y += W e / tau for both ports, Poisson drive on port 0
+            adex::State& st = s.ax[i];
+            st.y[0] = s.V[i];
+            const bool spk = adex::step(pop.ax, st, s.dt_ms);
+            const double jump = std::exp(1.0) / pop.ax.tau_syn;
+            st.y[3] += jump * (in + pop.ax.poisson_weight * (double)k);
+            st.y[5] += jump * in1;
+            s.V[i] = st.y[0];
+            if (spk) s.last_spikes.push_back(i);
+            continue;
+        }
         // 3b. membrane: exact integration with the current *before* its update (C11)
         if (s.refr[i] == 0) {
             s.V[i] = pop.p.E_L + pop.P22 * (s.V[i] - pop.p.E_L) + pop.P21 * s.I[i] + pop.P20 * pop.p.I_e;
@@ -293,7 +326,7 @@ void step_once(Sim& s, bool record) {
         for (int64_t c = s.row_off[j]; c < s.row_off[(size_t)j + 1]; ++c) {
             const Conn& cn = s.conns[(size_t)c];
             size_t sl = (size_t)((n + cn.delay) % D);
-            s.ring[sl * N + cn.tgt] += (double)cn.w;
+            s.ring[(sl * P + (size_t)cn.port) * N + cn.tgt] += (double)cn.w;
         }
         s.events += (uint64_t)(s.row_off[(size_t)j + 1] - s.row_off[j]);
     }
@@ -358,16 +391,45 @@ int32_t orc_create_population(void* h, int32_t n, const LifParams* p, int32_t* f
     return 0;
 }
 
-int32_t orc_connect(void* h, int32_t rule, int32_t src_first, int32_t src_n, int32_t tgt_first, int32_t tgt_n,
-                    int32_t K, const Dist* w, const Dist* d) {
+int32_t orc_connect_port(void* h, int32_t rule, int32_t src_first, int32_t src_n, int32_t tgt_first, int32_t tgt_n,
+                         int32_t K, const Dist* w, const Dist* d, int32_t port) {
     Sim* s = (Sim*)h;
     if (s->prepared) { s->err = "connect after prepare"; return -2; }
-    if (src_n <= 0 || tgt_n <= 0 || K < 0 || src_first < 0 || tgt_first < 0 ||
+    if (src_n <= 0 || tgt_n <= 0 || K < 0 || src_first < 0 || tgt_first < 0 || port < 0 || port > 1 ||
         src_first + src_n > s->N || tgt_first + tgt_n > s->N) { s->err = "bad range"; return -1; }
-    ConnectCall c{rule, src_first, src_n, tgt_first, tgt_n, K, *w, *d};
+    ConnectCall c{rule, src_first, src_n, tgt_first, tgt_n, K, *w, *d, port};
     s->calls.push_back(c);
     return 0;
 }
+int32_t orc_connect(void* h, int32_t rule, int32_t src_first, int32_t src_n, int32_t tgt_first, int32_t tgt_n,
+                    int32_t K, const Dist* w, const Dist* d) {
+    return orc_connect_port(h, rule, src_first, src_n, tgt_first, tgt_n, K, w, d, 0);
+}
+
+int32_t orc_create_population_adex(void* h, int32_t n, const adex::Params* p, int32_t* first_out) {
+    Sim* s = (Sim*)h;
+    if (s->prepared) { s->err = "population after prepare"; return -2; }
+    if (n <= 0) { s->err = "n <= 0"; return -1; }
+    Population pop;
+    pop.first = s->N; pop.n = n; pop.model = MODEL_ADEX; pop.ax = *p; pop.p = LifParams{};
+    pop.P11 = pop.P22 = pop.P21 = pop.P20 = 0.0; pop.refr_steps = 0;
+    double lam = p->poisson_rate_hz * s->dt_ms * 1e-3;
+    if (poisson_table(lam, pop.poisson_T) != 0) { s->err = "poisson rate too large"; return -1; }
+    s->pops.push_back(pop);
+    s->N += n;
+    if (first_out) *first_out = pop.first;
+    return 0;
+}
+
+// single-neuron helpers for the pins: the right-hand side and one time step of the AdEx integrator
+void orc_adex_rhs(const adex::Params* p, const double* y6, double* f6) { adex::rhs(*p, y6, f6); }
+int32_t orc_adex_step(const adex::Params* p, double* y6, double* h_int, double h_step) {
+    adex::State st; for (int i = 0; i < 6; ++i) st.y[i] = y6[i]; st.h_int = *h_int;
+    const bool spk = adex::step(*p, st, h_step);
+    for (int i = 0; i < 6; ++i) y6[i] = st.y[i]; *h_int = st.h_int;
+    return spk ? 1 : 0;
+}
+int32_t orc_num_ports(void* h) { return ((Sim*)h)->P; }
 
 int32_t orc_prepare(void* h) { return prepare(*(Sim*)h); }
 
@@ -411,6 +473,8 @@ int32_t orc_set_state(void* h, int32_t field, const void* data, int64_t n, int64
     else if (field == FIELD_REFR) { for (int64_t i = 0; i < n; ++i) s->refr[first + i] = ((const int32_t*)data)[i]; }
     else if (field == FIELD_RING) { for (int64_t i = 0; i < n; ++i) s->ring[first + i] = ((const double*)data)[i]; }
     else if (field == FIELD_STEP) { s->step = *(const int64_t*)data; }
+    else if (field >= FIELD_W && field <= FIELD_Y_IN) { for (int64_t i = 0; i < n; ++i) s->ax[first + i].y[field - FIELD_W + 1] = ((const double*)data)[i]; }
+    else if (field == FIELD_H_INT) { for (int64_t i = 0; i < n; ++i) s->ax[first + i].h_int = ((const double*)data)[i]; }
     else return -1;
     return 0;
 }
@@ -422,6 +486,8 @@ int32_t orc_get_state(void* h, int32_t field, void* data, int64_t n, int64_t fir
     else if (field == FIELD_REFR) { for (int64_t i = 0; i < n; ++i) ((int32_t*)data)[i] = s->refr[first + i]; }
     else if (field == FIELD_RING) { for (int64_t i = 0; i < n; ++i) ((double*)data)[i] = s->ring[first + i]; }
     else if (field == FIELD_STEP) { *(int64_t*)data = s->step; }
+    else if (field >= FIELD_W && field <= FIELD_Y_IN) { for (int64_t i = 0; i < n; ++i) ((double*)data)[i] = s->ax[first + i].y[field - FIELD_W + 1]; }
+    else if (field == FIELD_H_INT) { for (int64_t i = 0; i < n; ++i) ((double*)data)[i] = s->ax[first + i].h_int; }
     else return -1;
     return 0;
 }

@@ -57,7 +57,7 @@ class Workload:
     seed: int
     n_steps: int
     populations: list = field(default_factory=list)      # (name, n, lif-params dict)
-    calls: list = field(default_factory=list)            # (rule, src_pop, tgt_pop, K, weight dist, delay dist)
+    calls: list = field(default_factory=list)            # (rule, src_pop, tgt_pop, K, weight dist, delay dist[, port])
     bypass_neurons: bool = False
     inject_fraction: float = 0.0
     v0_mean: float = -58.0
@@ -70,7 +70,7 @@ class Workload:
     @property
     def n_connections(self) -> int:
         tot = 0
-        for rule, sp, tp, K, _, _ in self.calls:
+        for rule, sp, tp, K, *_ in self.calls:
             tot += K * (self.populations[tp][1] if rule == "in" else self.populations[sp][1])
         return tot
 
@@ -86,9 +86,12 @@ class Workload:
         firsts = [sim.create_population(n, params) for _, n, params in self.populations]
         rng = self.pop_ranges()
         assert firsts == [r[0] for r in rng]
-        for rule, sp, tp, K, w, d in self.calls:
+        for rule, sp, tp, K, w, d, *port in self.calls:
             fn = sim.connect_fixed_indegree if rule == "in" else sim.connect_fixed_outdegree
-            fn(rng[sp][0], rng[sp][1], rng[tp][0], rng[tp][1], K, w, d)
+            if port:                                     # receptor port of the targets (AdEx: 0 excitatory, 1 inhibitory)
+                fn(rng[sp][0], rng[sp][1], rng[tp][0], rng[tp][1], K, w, d, port=port[0])
+            else:
+                fn(rng[sp][0], rng[sp][1], rng[tp][0], rng[tp][1], K, w, d)
         if self.bypass_neurons:
             sim.set_bypass(True, self.inject_fraction)
         return sim
@@ -162,6 +165,27 @@ def balanced_large(n=1_000_000, k_total=1000, n_steps=10000, seed=1) -> Workload
     dly = ("uniform_int", 1, 20)
     wl.calls = [("in", 0, 0, k_e, ("const", W_E), dly), ("in", 0, 1, k_e, ("const", W_E), dly),
                 ("in", 1, 0, k_i, ("const", -5.0 * W_E), dly), ("in", 1, 1, k_i, ("const", -5.0 * W_E), dly)]
+    return wl
+
+
+# AdEx parameters of the paper's balanced network (Table II); V_peak, t_ref and the integrator tolerances are
+# not in the paper (readings C23, C24)
+ADEX = dict(model="adex", C_m=281.0, g_L=30.0, E_L=-70.6, V_T=-50.4, Delta_T=2.0, tau_w=144.0, a=4.0, b=80.5, V_reset=-60.0,
+            V_peak=0.0, E_ex=0.0, E_in=-85.0, tau_syn=1.0, I_e=0.0,
+            tol=(2e-4, 2e-3, 2e-5, 2e-4, 2e-5, 2e-4), h_min=1e-3)
+
+
+def balanced_adex(n=1_000_000, k_total=1000, n_steps=10000, seed=1) -> Workload:
+    """The paper's balanced network (Table I): N_in = N_ex / 4, CI = CE / 4, W_ex = 0.05 nS, W_in = 0.35 nS
+    on separate receptor ports, delays 0.5 +- 0.25 ms, Poisson drive 20 kHz x 0.37 nS, AdEx neurons of Table II."""
+    n_e, n_i = (n * 4) // 5, n - (n * 4) // 5
+    k_e, k_i = (k_total * 4) // 5, k_total - (k_total * 4) // 5
+    wl = Workload(f"adex_balanced_n{n}_k{k_total}", ring_slots=20, seed=seed, n_steps=n_steps, v0_mean=-65.0, v0_sd=5.0)
+    ax = dict(ADEX); ax.update(poisson_rate_hz=20000.0, poisson_weight=0.37)
+    wl.populations = [("E", n_e, ax), ("I", n_i, ax)]
+    dly = ("normal", 5.0, 2.5, 1, 20)
+    wl.calls = [("in", 0, 0, k_e, ("const", 0.05), dly, 0), ("in", 0, 1, k_e, ("const", 0.05), dly, 0),
+                ("in", 1, 0, k_i, ("const", 0.35), dly, 1), ("in", 1, 1, k_i, ("const", 0.35), dly, 1)]
     return wl
 
 

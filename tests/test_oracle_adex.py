@@ -1,0 +1,135 @@
+"""Pins of the AdEx part of the oracle (oracle/oracle_adex.hpp) against things other than itself: scipy's stiff ODE
+solvers on the single-neuron protocol the paper itself validates with (one AdEx neuron, 700 pA), the
+closed-form alpha conductance, hand-evaluated right-hand sides, and brute force of the two-port delivery."""
+import numpy as np
+import pytest
+from scipy.integrate import solve_ivp
+
+from paper_2007_14236_b200 import workloads as W
+
+
+def params(**over):
+    p = dict(W.ADEX)
+    p.update(over)
+    return p
+
+
+def scipy_rhs(p, clamp=True):
+    def f(t, y):
+        V = min(y[0], p["V_peak"]) if clamp else y[0]      # the clamp only matters beyond the spike event
+        return [(-p["g_L"] * (V - p["E_L"]) + p["g_L"] * p["Delta_T"] * np.exp((V - p["V_T"]) / p["Delta_T"])
+                 + y[2] * (p["E_ex"] - V) + y[4] * (p["E_in"] - V) - y[1] + p["I_e"]) / p["C_m"],
+                (p["a"] * (V - p["E_L"]) - y[1]) / p["tau_w"],
+                -y[2] / p["tau_syn"] + y[3], -y[3] / p["tau_syn"], -y[4] / p["tau_syn"] + y[5], -y[5] / p["tau_syn"]]
+    return f
+
+
+def test_rhs_hand_values(oracle_mod):
+    p = params(I_e=100.0)
+    y = np.array([-55.0, 20.0, 1.5, 0.3, 0.7, -0.1])
+    f = oracle_mod.adex_rhs(p, y)
+    dV = (-30.0 * (-55.0 + 70.6) + 30.0 * 2.0 * np.exp((-55.0 + 50.4) / 2.0) + 1.5 * (0.0 + 55.0) + 0.7 * (-85.0 + 55.0)
+          - 20.0 + 100.0) / 281.0                                   # Eq. (3) with reading C21, typed out by hand
+    assert f[0] == pytest.approx(dV, rel=1e-14)
+    assert f[1] == pytest.approx((4.0 * (-55.0 + 70.6) - 20.0) / 144.0, rel=1e-14)      # Eq. (5)
+    assert f[2] == pytest.approx(-1.5 + 0.3) and f[3] == pytest.approx(-0.3)
+    assert f[4] == pytest.approx(-0.7 - 0.1) and f[5] == pytest.approx(0.1)
+    # C21: an excitatory conductance depolarises, an inhibitory one hyperpolarises (at rest, between the reversals)
+    rest = np.array([-70.6, 0, 0, 0, 0, 0.0])
+    f0 = oracle_mod.adex_rhs(params(), rest)[0]
+    assert oracle_mod.adex_rhs(params(), rest + [0, 0, 1, 0, 0, 0])[0] > f0 > oracle_mod.adex_rhs(params(), rest + [0, 0, 0, 0, 1, 0])[0]
+    # exponential clamped at V_peak (C24)
+    assert oracle_mod.adex_rhs(params(), [50.0, 0, 0, 0, 0, 0])[0] == oracle_mod.adex_rhs(params(), [0.0, 0, 0, 0, 0, 0])[0]
+
+
+def test_alpha_conductance_closed_form(oracle_mod):
+    """C22: y jumps by W e / tau; g(t) = W (t / tau) exp(1 - t / tau), peak W at t = tau."""
+    p = params()
+    Wn = 0.05
+    y = np.array([-70.6, 0, 0, Wn * np.e / p["tau_syn"], 0, 0.35 * np.e / p["tau_syn"]]); h = 0.1
+    g_ex, g_in = [], []
+    for k in range(60):
+        y, h, _ = oracle_mod.adex_step(p, y, h, 0.1)
+        g_ex.append(y[2]); g_in.append(y[4])
+    t = 0.1 * np.arange(1, 61)
+    assert np.allclose(g_ex, Wn * t * np.exp(1 - t), atol=2e-5)
+    assert np.allclose(g_in, 0.35 * t * np.exp(1 - t), atol=1e-4)
+    assert abs(max(g_ex) - Wn) < 1e-4 and int(np.argmax(g_ex)) == 9          # peak W one tau after the spike
+
+
+def test_single_neuron_700pA_against_scipy(oracle_mod):
+    """PAPER.md:252 protocol.  Reference: scipy DOP853 (rtol 1e-11) with an event at V_peak, reset by hand."""
+    p = params(I_e=700.0)
+    f = scipy_rhs(p, clamp=False)
+    ev = lambda t, y: y[0] - p["V_peak"]
+    ev.terminal = True; ev.direction = 1
+    T = 300.0
+    t0, y0, ref_spikes, segs = 0.0, [p["E_L"], 0, 0, 0, 0, 0], [], []
+    while t0 < T:
+        sol = solve_ivp(f, (t0, T), y0, method="DOP853", rtol=1e-11, atol=1e-12, events=ev, dense_output=True)
+        segs.append((t0, sol.t[-1], sol.sol))
+        if sol.status == 1:
+            t0 = sol.t_events[0][0]; ref_spikes.append(t0)
+            y0 = sol.y[:, -1].copy(); y0[0] = p["V_reset"]; y0[1] += p["b"]
+        else:
+            break
+    y = np.array([p["E_L"], 0, 0, 0, 0, 0.0]); h = 0.1
+    spikes, Vs = [], []
+    for k in range(int(T / 0.1)):
+        y, h, s = oracle_mod.adex_step(p, y, h, 0.1)
+        Vs.append(y[0])
+        if s:
+            spikes.append(k)
+    assert len(ref_spikes) >= 4 and len(spikes) == len(ref_spikes)
+    # a spike is found in the step that contains the reference crossing (resets happen on sub-step boundaries, so the
+    # trajectories after the first spike are shifted by less than one sub-step)
+    assert all(abs(k - int(tr / 0.1)) <= 1 for k, tr in zip(spikes, ref_spikes))
+    # before the first spike the trajectory is the same ODE: compare away from the upswing
+    k1 = spikes[0]
+    tg = 0.1 * np.arange(1, k1 - 5)
+    ref = segs[0][2](tg)[0]
+    sel = ref < -45.0
+    assert np.max(np.abs(np.array(Vs[:k1 - 6]) - ref)[sel]) < 2e-3
+    # adaptation: inter-spike intervals grow (w accumulates b per spike)
+    assert np.all(np.diff(np.diff(spikes)) > 0)
+
+
+def test_fixed_point_and_step_size_state(oracle_mod):
+    """No drive: the resting point of Eqs. (3), (5) is stationary; the sub-step size grows to the whole step."""
+    p = params()
+    root = solve_ivp(scipy_rhs(p), (0, 5000.0), [p["E_L"], 0, 0, 0, 0, 0], method="Radau", rtol=1e-10, atol=1e-12).y[:, -1]
+    y, h = root.copy(), 0.01
+    for _ in range(50):
+        y, h, s = oracle_mod.adex_step(p, y, h, 0.1)
+        assert not s
+    assert np.allclose(y, root, atol=1e-6) and h == pytest.approx(0.1)
+
+
+def test_two_port_network_brute_force(oracle_mod):
+    """Delivery with receptor ports: ring[slot][port][target] equals the plain definition per port (dense brute force)."""
+    wl = W.balanced_adex(n=40, k_total=10, n_steps=60, seed=4)
+    o = oracle_mod.Oracle(0.1, wl.ring_slots, wl.seed)
+    wl.apply(o); o.prepare()
+    assert o.n_ports == 2
+    N, D = 40, wl.ring_slots
+    v0 = wl.initial_v(); v0[:8] = -30.0; v0[32:36] = -30.0  # a few E and I neurons start on the upswing and fire at once
+    o.set_state(oracle_mod.FIELD_V, v0.astype(np.float64))
+    src, tgt, w, d, ro = o.get_connections()
+    port = np.where(src < 32, 0, 1)                          # E sources -> port 0, I sources -> port 1 (the recipe)
+    hist = np.zeros((200, N), bool)
+    seen_ports = set()
+    for n in range(60):
+        ring_before = o.get_state(oracle_mod.FIELD_RING).reshape(D, 2, N).copy()
+        o.simulate(1)
+        hist[n, o.last_spikes()] = True
+        ring = o.get_state(oracle_mod.FIELD_RING).reshape(D, 2, N)
+        # plain definition of every pending cell: sum over connections of w * S_src(n' - d), n' in (n, n + D]
+        for npend in range(n + 1, n + 1 + D):
+            exp = np.zeros((2, N))
+            for c in range(src.size):
+                m = npend - int(d[c])
+                if 0 <= m <= n and hist[m, src[c]]:
+                    exp[port[c], tgt[c]] += float(w[c])
+            assert np.allclose(ring[npend % D], exp, atol=1e-12), (n, npend)
+            seen_ports |= {pt for pt in (0, 1) if exp[pt].any()}
+    assert hist.sum() >= 12 and seen_ports == {0, 1}
