@@ -63,8 +63,18 @@ enum {
     NG_FIELD_REFR = 2,        /* int32  [N]   remaining refractory steps                           */
     NG_FIELD_RING = 3,        /* float  [D*N] input ring buffer, slot-major: ring[slot*N + i]      */
     NG_FIELD_STEP = 4,        /* int64  [1]   index n of the next step                             */
-    NG_FIELD_LAST_INPUT = 5   /* float  [N]   in_i consumed by the last step (needs NG_DEBUG_INPUT; get only) */
+    NG_FIELD_LAST_INPUT = 5,  /* float  [P*N] in_i consumed by the last step (needs NG_DEBUG_INPUT; get only) */
+    /* AdEx state (only with AdEx populations), float [N] each; V is NG_FIELD_V */
+    NG_FIELD_ADEX_W = 6,      /* adaptation current w, pA                                           */
+    NG_FIELD_ADEX_G_EX = 7,   /* excitatory conductance g_ex, nS                                    */
+    NG_FIELD_ADEX_Y_EX = 8,   /* its alpha-function companion y_ex, nS/ms                           */
+    NG_FIELD_ADEX_G_IN = 9,   /* inhibitory conductance g_in, nS                                    */
+    NG_FIELD_ADEX_Y_IN = 10,  /* y_in, nS/ms                                                        */
+    NG_FIELD_ADEX_H = 11      /* current sub-step size of the adaptive integrator, ms               */
 };
+/* Receptor ports: P = 1, or 2 as soon as an AdEx population exists (port 0 excitatory — also the LIF input current —,
+ * port 1 inhibitory).  NG_FIELD_RING is then [D][P][N], NG_FIELD_LAST_INPUT [P][N], and the stored target of a
+ * connection record (ng_copy_records, ng_get_connections) is target id + port * N. */
 
 /* distribution kinds for weights and delays ("fixed values ... or probability distributions") */
 enum {
@@ -123,6 +133,17 @@ typedef struct {
     double poisson_weight;    /* pA per background event                                           */
 } ng_lif_params;
 
+/* AdEx neuron with conductance-based alpha synapses, the model of the paper's balanced network (PAPER.md:110-161,
+ * Eqs. (3)-(5), Table II symbols).  Units: pF, nS, mV, ms, pA, Hz; weights of connections onto AdEx neurons are peak
+ * conductances in nS.  V_peak, tol and h_min are not in the paper (readings C23, C24). */
+typedef struct {
+    double C_m, g_L, E_L, V_T, Delta_T, tau_w, a, b, V_reset, V_peak, E_ex, E_in, tau_syn, I_e;
+    double poisson_rate_hz;   /* background drive onto the excitatory port                           */
+    double poisson_weight;    /* nS per background event                                             */
+    double tol[6];            /* absolute tolerances of (V, w, g_ex, y_ex, g_in, y_in) for the step-size control */
+    double h_min;             /* smallest sub-step of the adaptive Runge-Kutta integrator, ms        */
+} ng_adex_params;
+
 typedef struct {
     int32_t kind;   /* NG_DIST_* */
     int32_t pad;
@@ -177,6 +198,18 @@ int32_t ng_connect_fixed_indegree(ng_sim* sim, int32_t src_first, int32_t src_n,
  * with replacement; draw (source j, k).  Same errors. */
 int32_t ng_connect_fixed_outdegree(ng_sim* sim, int32_t src_first, int32_t src_n, int32_t tgt_first,
                                    int32_t tgt_n, int32_t K, const ng_dist* weight, const ng_dist* delay_steps);
+
+/* Same rules with an explicit receptor port of the targets (0 or 1; see "Receptor ports" above).  The plain calls use
+ * port 0.  Errors as above, INVALID_ARG for another port. */
+int32_t ng_connect_fixed_indegree_port(ng_sim* sim, int32_t src_first, int32_t src_n, int32_t tgt_first, int32_t tgt_n,
+                                       int32_t K, const ng_dist* weight, const ng_dist* delay_steps, int32_t port);
+int32_t ng_connect_fixed_outdegree_port(ng_sim* sim, int32_t src_first, int32_t src_n, int32_t tgt_first, int32_t tgt_n,
+                                        int32_t K, const ng_dist* weight, const ng_dist* delay_steps, int32_t port);
+
+/* Add n AdEx neurons (Eqs. (3)-(5), alpha conductances, adaptive 5th-order Runge-Kutta).
+ * Initial state: V = E_L, w = 0, conductances 0.  Errors: STATE after ng_prepare; INVALID_ARG for non-positive
+ * C_m, g_L, Delta_T, tau_w, tau_syn, h_min or tolerances, too many populations, Poisson rate*h too large. */
+int32_t ng_create_population_adex(ng_sim* sim, int32_t n, const ng_adex_params* params, int32_t* first_id_out);
 
 /* Delivery-only mode (BASELINE.json configs[3], C8): the neuron update is bypassed and source s
  * fires in step n iff Philox(INJECT; s, n).x0 < floor(fraction * 2^32).  Before ng_prepare only. */

@@ -15,6 +15,7 @@ from . import build as _build
 NG_OK, NG_ERR_INVALID_ARG, NG_ERR_STATE, NG_ERR_OOM, NG_ERR_CUDA, NG_ERR_OVERFLOW = 0, -1, -2, -3, -4, -5
 NG_RECORD_SPIKES, NG_DEBUG_INPUT = 1, 2
 FIELD_V, FIELD_I_SYN, FIELD_REFR, FIELD_RING, FIELD_STEP, FIELD_LAST_INPUT = 0, 1, 2, 3, 4, 5
+FIELD_ADEX_W, FIELD_ADEX_G_EX, FIELD_ADEX_Y_EX, FIELD_ADEX_G_IN, FIELD_ADEX_Y_IN, FIELD_ADEX_H = 6, 7, 8, 9, 10, 11
 DIST_CONST, DIST_NORMAL_CLIPPED, DIST_UNIFORM_INT = 0, 1, 2
 (OPT_STEP_MODE, OPT_STEPS_PER_GRAPH, OPT_DELIVERY_KERNEL, OPT_DELIVER_BLOCKS, OPT_PROFILE, OPT_ASYNC,
  OPT_SORT_SEGMENTS, OPT_PREFETCH, OPT_TRACE, OPT_PERSISTENT_THREADS) = range(10)
@@ -23,7 +24,8 @@ STEP_GRAPH, STEP_LAUNCH, STEP_PERSISTENT, STEP_AUTO = 0, 1, 2, 3
 EXPORTS = ["ng_create", "ng_destroy", "ng_last_error", "ng_create_population", "ng_connect_fixed_indegree",
            "ng_connect_fixed_outdegree", "ng_set_bypass", "ng_set_option", "ng_prepare", "ng_set_state",
            "ng_get_state", "ng_simulate", "ng_get_spikes", "ng_get_last_spikes", "ng_copy_row_offsets",
-           "ng_copy_group_offsets", "ng_copy_records", "ng_get_connections", "ng_get_stats", "ng_get_trace", "ng_probe"]
+           "ng_copy_group_offsets", "ng_copy_records", "ng_get_connections", "ng_get_stats", "ng_get_trace", "ng_probe",
+           "ng_create_population_adex", "ng_connect_fixed_indegree_port", "ng_connect_fixed_outdegree_port"]
 
 
 class NgConfig(C.Structure):
@@ -43,6 +45,22 @@ class NgLifParams(C.Structure):
     _fields_ = [(k, C.c_double) for k in
                 ("C_m", "tau_m", "tau_syn", "E_L", "V_th", "V_reset", "t_ref_ms", "I_e",
                  "poisson_rate_hz", "poisson_weight")]
+
+
+_ADEX_SCALARS = ("C_m", "g_L", "E_L", "V_T", "Delta_T", "tau_w", "a", "b", "V_reset", "V_peak", "E_ex", "E_in", "tau_syn",
+                 "I_e", "poisson_rate_hz", "poisson_weight")
+
+
+class NgAdexParams(C.Structure):
+    _fields_ = [(k, C.c_double) for k in _ADEX_SCALARS] + [("tol", C.c_double * 6), ("h_min", C.c_double)]
+
+
+def _adex(params: dict) -> NgAdexParams:
+    p = NgAdexParams(**{k: float(params.get(k, 0.0)) for k in _ADEX_SCALARS})
+    for i, t in enumerate(params["tol"]):
+        p.tol[i] = float(t)
+    p.h_min = float(params["h_min"])
+    return p
 
 
 class NgDist(C.Structure):
@@ -85,6 +103,9 @@ def load_library(path: str | None = None):
     L.ng_create_population.argtypes = [vp, i32, C.POINTER(NgLifParams), C.POINTER(i32)]
     for fn in (L.ng_connect_fixed_indegree, L.ng_connect_fixed_outdegree):
         fn.argtypes = [vp, i32, i32, i32, i32, i32, C.POINTER(NgDist), C.POINTER(NgDist)]
+    for fn in (L.ng_connect_fixed_indegree_port, L.ng_connect_fixed_outdegree_port):
+        fn.argtypes = [vp, i32, i32, i32, i32, i32, C.POINTER(NgDist), C.POINTER(NgDist), i32]
+    L.ng_create_population_adex.argtypes = [vp, i32, C.POINTER(NgAdexParams), C.POINTER(i32)]
     L.ng_set_bypass.argtypes = [vp, i32, C.c_double]
     L.ng_set_option.argtypes = [vp, i32, i64]
     L.ng_prepare.argtypes = [vp]
@@ -156,6 +177,7 @@ class Sim:
         self._torch = torch
         self.device = device
         self.dt_ms, self.D, self.seed = dt_ms, ring_slots, seed
+        self.n_ports = 1                          # 2 as soon as an AdEx population is created
         self.stream = torch.cuda.Stream(device=device)
         self._tensors = {}
         self._alloc_struct = None
@@ -202,20 +224,26 @@ class Sim:
 
     # ---- network description --------------------------------------------------------------------------------
     def create_population(self, n: int, params: dict) -> int:
+        """params: LIF dict (ng_lif_params fields) or, with params["model"] == "adex", an AdEx dict (ng_adex_params)."""
         first = C.c_int32()
-        p = _lif(params)
-        self._chk(self._L.ng_create_population(self._h, n, C.byref(p), C.byref(first)))
+        if params.get("model") == "adex":
+            p = _adex(params)
+            self._chk(self._L.ng_create_population_adex(self._h, n, C.byref(p), C.byref(first)))
+            self.n_ports = 2
+        else:
+            p = _lif(params)
+            self._chk(self._L.ng_create_population(self._h, n, C.byref(p), C.byref(first)))
         return first.value
 
-    def connect_fixed_indegree(self, src_first, src_n, tgt_first, tgt_n, K, weight, delay):
+    def connect_fixed_indegree(self, src_first, src_n, tgt_first, tgt_n, K, weight, delay, port: int = 0):
         w, d = _dist(weight), _dist(delay)
-        self._chk(self._L.ng_connect_fixed_indegree(self._h, src_first, src_n, tgt_first, tgt_n, K,
-                                                    C.byref(w), C.byref(d)))
+        self._chk(self._L.ng_connect_fixed_indegree_port(self._h, src_first, src_n, tgt_first, tgt_n, K,
+                                                         C.byref(w), C.byref(d), port))
 
-    def connect_fixed_outdegree(self, src_first, src_n, tgt_first, tgt_n, K, weight, delay):
+    def connect_fixed_outdegree(self, src_first, src_n, tgt_first, tgt_n, K, weight, delay, port: int = 0):
         w, d = _dist(weight), _dist(delay)
-        self._chk(self._L.ng_connect_fixed_outdegree(self._h, src_first, src_n, tgt_first, tgt_n, K,
-                                                     C.byref(w), C.byref(d)))
+        self._chk(self._L.ng_connect_fixed_outdegree_port(self._h, src_first, src_n, tgt_first, tgt_n, K,
+                                                          C.byref(w), C.byref(d), port))
 
     def set_bypass(self, bypass: bool, inject_fraction: float = 0.0):
         self._chk(self._L.ng_set_bypass(self._h, int(bypass), float(inject_fraction)))
@@ -258,7 +286,8 @@ class Sim:
             return int(a[0])
         if out is None:
             if n is None:
-                n = self.n_neurons * (self.D if field == FIELD_RING else 1) - first
+                n = self.n_neurons * (self.D * self.n_ports if field == FIELD_RING else
+                                      self.n_ports if field == FIELD_LAST_INPUT else 1) - first
             out = np.empty(n, np.int32 if field == FIELD_REFR else np.float32)
         cnt = out.size if isinstance(out, np.ndarray) else out.numel()
         self._chk(self._L.ng_get_state(self._h, field, _ptr(out), cnt, first))

@@ -24,7 +24,7 @@
 
 using namespace ng;
 
-struct HostPop { int32_t first, n; ng_lif_params p; PopDev dev; };
+struct HostPop { int32_t first, n; ng_lif_params p; PopDev dev; };     // dev.model tells LIF from AdEx
 
 struct ng_sim {
     ng_config cfg{};
@@ -55,6 +55,8 @@ struct ng_sim {
     int delivery_kernel = 1; int deliver_blocks = 0; int update_blocks = 0; int persistent_blocks = 0;
     int pipe_blocks = 0; int persistent_pipe_blocks = 0;
     int persistent_threads = kPersistentThreads;
+    bool has_adex = false;                 // any AdEx population: two receptor ports, AdEx state arrays, <true> kernels
+    int64_t NR = 0;                        // ring row length = N * ports
     bool window_backend = false;           // delivery kernel 4 chosen before ng_prepare: spike window instead of a D-plane ring
     cudaGraphExec_t graph_exec = nullptr; int graph_steps = 0;
     // stats
@@ -134,7 +136,7 @@ bool valid_dist(const ng_dist* d) {
 }
 
 int32_t add_call(ng_sim* s, int32_t rule, int32_t src_first, int32_t src_n, int32_t tgt_first, int32_t tgt_n, int32_t K,
-                 const ng_dist* w, const ng_dist* d) {
+                 const ng_dist* w, const ng_dist* d, int32_t port = 0) {
     if (!s) return NG_ERR_INVALID_ARG;
     if (s->prepared) return fail(s, NG_ERR_STATE, "connect after ng_prepare");
     if (!valid_dist(w) || !valid_dist(d)) return fail(s, NG_ERR_INVALID_ARG, "bad distribution");
@@ -143,7 +145,8 @@ int32_t add_call(ng_sim* s, int32_t rule, int32_t src_first, int32_t src_n, int3
         return fail(s, NG_ERR_INVALID_ARG, "population range outside the created neurons, or K < 0");
     CallDev c{};
     c.rule = rule; c.src_first = src_first; c.src_n = src_n; c.tgt_first = tgt_first; c.tgt_n = tgt_n; c.K = K;
-    c.call_index = (int32_t)s->calls.size();
+    if (port < 0 || port > 1) return fail(s, NG_ERR_INVALID_ARG, "receptor port is 0 or 1");
+    c.call_index = (int32_t)s->calls.size(); c.port = port;
     c.w = DistDev{w->kind, 0, w->a, w->b, w->lo, w->hi};
     c.d = DistDev{d->kind, 0, d->a, d->b, d->lo, d->hi};
     s->calls.push_back(c);
@@ -162,7 +165,8 @@ void destroy_graph(ng_sim* s) {
 }
 
 void launch_update(ng_sim* s) {
-    update_kernel<<<s->update_blocks, kUpdateThreads, 0, s->stream>>>(s->a);
+    if (s->has_adex) update_kernel<true><<<s->update_blocks, kUpdateThreads, 0, s->stream>>>(s->a);
+    else update_kernel<false><<<s->update_blocks, kUpdateThreads, 0, s->stream>>>(s->a);
 }
 void launch_deliver(ng_sim* s) {
     if (s->delivery_kernel == 4) deliver_kernel<4><<<s->deliver_blocks, kDeliverThreads, 0, s->stream>>>(s->a);
@@ -172,11 +176,13 @@ void launch_deliver(ng_sim* s) {
 
 // one time step: two kernels (update, deliver) or the pipelined step kernel
 void launch_pipe(ng_sim* s) {
-    pipe_step_kernel<true><<<s->pipe_blocks, kPipeThreads, 0, s->stream>>>(s->a);
+    if (s->has_adex) pipe_step_kernel<true, true><<<s->pipe_blocks, kPipeThreads, 0, s->stream>>>(s->a);
+    else pipe_step_kernel<true, false><<<s->pipe_blocks, kPipeThreads, 0, s->stream>>>(s->a);
 }
 // rest pass of the last step of an ng_simulate call (delivery kernel 4): leaves nothing pending between API calls
 void launch_pipe_flush(ng_sim* s) {
-    pipe_step_kernel<false><<<s->pipe_blocks, kPipeThreads, 0, s->stream>>>(s->a);
+    if (s->has_adex) pipe_step_kernel<false, true><<<s->pipe_blocks, kPipeThreads, 0, s->stream>>>(s->a);
+    else pipe_step_kernel<false, false><<<s->pipe_blocks, kPipeThreads, 0, s->stream>>>(s->a);
 }
 void launch_step(ng_sim* s) {
     if (s->delivery_kernel == 3) launch_pipe(s);
@@ -199,13 +205,16 @@ void configure_launch(ng_sim* s) {
     // step mode: the latency-bound kernels run as one persistent cooperative kernel per ng_simulate call; the
     // bandwidth-bound delay-major kernel keeps its 8 CTAs per SM and runs from a CUDA graph
     s->step_mode = s->step_mode_opt != 3 ? s->step_mode_opt : (k == 2 || k == 4 || !s->coop_ok) ? 0 : 2;
+    if (s->has_adex && s->step_mode == 2 && k != 3) s->step_mode = 0;   // the two-phase persistent kernels are LIF only
     s->a.prefetch = (k != 2 && k != 4 && s->prefetch_opt) ? 1 : 0;
     s->pipe_blocks = grid_for(s->N, kPipeThreads - kEntryTile, sm * 4);   // updaters per CTA = kPipeThreads - kEntryTile
     {
         int occp = 0;
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occp, persistent_pipe_kernel, s->persistent_threads, 0);
+        const int pt = s->has_adex ? 512 : s->persistent_threads;      // AdEx kernels are compiled for 512-thread CTAs
+        if (s->has_adex) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occp, persistent_pipe_kernel<true>, pt, 0);
+        else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occp, persistent_pipe_kernel<false>, pt, 0);
         if (occp < 1) occp = 1;
-        s->persistent_pipe_blocks = sm * std::min(occp, kPersistentThreads / s->persistent_threads);
+        s->persistent_pipe_blocks = sm * std::min(occp, kPersistentThreads / pt);
     }
     int blocks = s->deliver_blocks_opt;
     if (blocks <= 0) {
@@ -254,10 +263,16 @@ int32_t field_info(ng_sim* s, int32_t field, void** base, size_t* elem, int64_t*
         case NG_FIELD_V: *base = s->a.V; *elem = 4; *len = s->N; return NG_OK;
         case NG_FIELD_I_SYN: *base = s->a.I; *elem = 4; *len = s->N; return NG_OK;
         case NG_FIELD_REFR: *base = s->a.refr; *elem = 4; *len = s->N; return NG_OK;
-        case NG_FIELD_RING: *base = s->a.ring; *elem = 4; *len = (int64_t)s->N * s->cfg.ring_slots; return NG_OK;   // see ring_copy
+        case NG_FIELD_RING: *base = s->a.ring; *elem = 4; *len = s->NR * s->cfg.ring_slots; return NG_OK;   // see ring_copy
         case NG_FIELD_LAST_INPUT:
             if (!s->a.last_input) return fail(s, NG_ERR_STATE, "NG_FIELD_LAST_INPUT needs NG_DEBUG_INPUT");
-            *base = s->a.last_input; *elem = 4; *len = s->N; return NG_OK;
+            *base = s->a.last_input; *elem = 4; *len = s->NR; return NG_OK;
+        case NG_FIELD_ADEX_W: case NG_FIELD_ADEX_G_EX: case NG_FIELD_ADEX_Y_EX: case NG_FIELD_ADEX_G_IN: case NG_FIELD_ADEX_Y_IN:
+        case NG_FIELD_ADEX_H: {
+            if (!s->has_adex) return fail(s, NG_ERR_STATE, "no AdEx population");
+            float* arr[] = {s->a.ax_w, s->a.ax_gx, s->a.ax_yx, s->a.ax_gi, s->a.ax_yi, s->a.ax_h};
+            *base = arr[field - NG_FIELD_ADEX_W]; *elem = 4; *len = s->N; return NG_OK;
+        }
         default: return fail(s, NG_ERR_INVALID_ARG, "unknown field");
     }
 }
@@ -269,7 +284,7 @@ int32_t ring_copy(ng_sim* s, bool to_device, void* user, int64_t count, int64_t 
     Ctl h{};
     int32_t rc = read_ctl(s, &h);
     if (rc) return rc;
-    const int64_t N = s->N, D = s->cfg.ring_slots, Dr = s->a.Dr, n = h.step_u;
+    const int64_t N = s->NR, D = s->cfg.ring_slots, Dr = s->a.Dr, n = h.step_u;      // N: plane length (all ports)
     if (s->window_backend) {
         // no ring exists: the pending inputs live in the spike window.  Read-back expands them into a temporary image.
         if (to_device) return fail(s, NG_ERR_STATE, "NG_FIELD_RING cannot be set with the spike-buffer backend (delivery kernel 4)");
@@ -368,6 +383,46 @@ int32_t ng_connect_fixed_outdegree(ng_sim* s, int32_t src_first, int32_t src_n, 
     return add_call(s, kRuleOutdegree, src_first, src_n, tgt_first, tgt_n, K, w, d);
 }
 
+int32_t ng_connect_fixed_indegree_port(ng_sim* s, int32_t src_first, int32_t src_n, int32_t tgt_first, int32_t tgt_n, int32_t K,
+                                       const ng_dist* w, const ng_dist* d, int32_t port) {
+    return add_call(s, kRuleIndegree, src_first, src_n, tgt_first, tgt_n, K, w, d, port);
+}
+int32_t ng_connect_fixed_outdegree_port(ng_sim* s, int32_t src_first, int32_t src_n, int32_t tgt_first, int32_t tgt_n, int32_t K,
+                                        const ng_dist* w, const ng_dist* d, int32_t port) {
+    return add_call(s, kRuleOutdegree, src_first, src_n, tgt_first, tgt_n, K, w, d, port);
+}
+
+int32_t ng_create_population_adex(ng_sim* s, int32_t n, const ng_adex_params* p, int32_t* first_id_out) {
+    if (!s || !p) return NG_ERR_INVALID_ARG;
+    if (s->prepared) return fail(s, NG_ERR_STATE, "population after ng_prepare");
+    if (n <= 0 || (int64_t)s->N + n > 1073741000LL) return fail(s, NG_ERR_INVALID_ARG, "n <= 0 or too many neurons");
+    if (s->pops.size() >= 255) return fail(s, NG_ERR_INVALID_ARG, "more than 255 populations");
+    if (!(p->C_m > 0.0) || !(p->g_L > 0.0) || !(p->Delta_T > 0.0) || !(p->tau_w > 0.0) || !(p->tau_syn > 0.0) ||
+        !(p->h_min > 0.0) || p->poisson_rate_hz < 0.0)
+        return fail(s, NG_ERR_INVALID_ARG, "non-positive C_m, g_L, Delta_T, tau_w, tau_syn or h_min, or negative rate");
+    for (int i = 0; i < 6; ++i) if (!(p->tol[i] > 0.0)) return fail(s, NG_ERR_INVALID_ARG, "non-positive tolerance");
+    HostPop hp{};
+    hp.first = s->N; hp.n = n;
+    PopDev& d = hp.dev;
+    d.model = 1;
+    d.E_L = (float)p->E_L;                                 // initial V
+    d.w_ext = (float)p->poisson_weight;
+    AdexDev& x = d.ax;
+    x.g_L = (float)p->g_L; x.E_L = (float)p->E_L; x.V_T = (float)p->V_T; x.inv_DeltaT = (float)(1.0 / p->Delta_T);
+    x.gL_DeltaT = (float)(p->g_L * p->Delta_T); x.inv_C = (float)(1.0 / p->C_m); x.inv_tau_w = (float)(1.0 / p->tau_w);
+    x.a = (float)p->a; x.b = (float)p->b; x.V_reset = (float)p->V_reset; x.V_peak = (float)p->V_peak;
+    x.E_ex = (float)p->E_ex; x.E_in = (float)p->E_in; x.inv_tau_syn = (float)(1.0 / p->tau_syn); x.I_e = (float)p->I_e;
+    x.jump = (float)(std::exp(1.0) / p->tau_syn);
+    for (int i = 0; i < 6; ++i) x.inv_tol[i] = (float)(1.0 / p->tol[i]);
+    x.h_min = (float)p->h_min;
+    if (!make_poisson_table(p->poisson_rate_hz * s->cfg.dt_ms * 1e-3, d))
+        return fail(s, NG_ERR_INVALID_ARG, "Poisson rate * h too large for the 64-entry CDF table");
+    s->pops.push_back(hp);
+    s->N += n;
+    if (first_id_out) *first_id_out = hp.first;
+    return NG_OK;
+}
+
 int32_t ng_set_bypass(ng_sim* s, int32_t bypass, double fraction) {
     if (!s) return NG_ERR_INVALID_ARG;
     if (s->prepared) return fail(s, NG_ERR_STATE, "ng_set_bypass after ng_prepare");
@@ -436,6 +491,10 @@ int32_t ng_prepare(ng_sim* s) {
     s->window_backend = s->delivery_kernel_opt == 4 ||
                         (s->delivery_kernel_opt == 0 && (double)N * (D + 1) * 4.0 > 0.8 * (double)s->l2_bytes);
     const int planes = s->window_backend ? 2 : D + 1;               // ring planes actually stored
+    s->has_adex = false;
+    for (const HostPop& hp : s->pops) s->has_adex = s->has_adex || hp.dev.model == 1;
+    s->NR = (int64_t)N * (s->has_adex ? 2 : 1);
+    const size_t NRs = (size_t)s->NR;
     s->S = 0;
     for (const CallDev& c : s->calls) s->S += (int64_t)(c.rule == kRuleIndegree ? c.tgt_n : c.src_n) * c.K;
 
@@ -448,12 +507,15 @@ int32_t ng_prepare(ng_sim* s) {
     bool ok = dev_alloc_t(s, &s->d_ctl, 1) && dev_alloc_t(s, &s->d_pops, s->pops.size()) &&
               dev_alloc_t(s, &s->d_pop_of, (size_t)N) && dev_alloc_t(s, &s->a.V, (size_t)N) &&
               dev_alloc_t(s, &s->a.I, (size_t)N) && dev_alloc_t(s, &s->a.refr, (size_t)N) &&
-              dev_alloc_t(s, &s->a.ring, (size_t)N * planes) && dev_alloc_t(s, &s->a.spike_list, (size_t)2 * N) &&
+              dev_alloc_t(s, &s->a.ring, NRs * planes) && dev_alloc_t(s, &s->a.spike_list, (size_t)2 * N) &&
               dev_alloc_t(s, &s->a.spike_row, (size_t)2 * N) && dev_alloc_t(s, &s->a.pois_k, (size_t)N) && dev_alloc_t(s, &s->d_row_info, (size_t)N) &&
               dev_alloc_t(s, &s->d_calls, std::max<size_t>(1, s->calls.size())) &&
               dev_alloc_t(s, &s->d_cnt, (size_t)N * D) && dev_alloc_t(s, &s->d_row_len, (size_t)N) &&
               dev_alloc_t(s, &s->d_row_off, (size_t)N + 1) && dev_alloc_t(s, &s->d_grp_rel, (size_t)N * (D + 1));
-    if (ok && (s->cfg.flags & NG_DEBUG_INPUT)) ok = dev_alloc_t(s, &s->a.last_input, (size_t)N);
+    if (ok && (s->cfg.flags & NG_DEBUG_INPUT)) ok = dev_alloc_t(s, &s->a.last_input, NRs);
+    if (ok && s->has_adex)
+        ok = dev_alloc_t(s, &s->a.ax_w, (size_t)N) && dev_alloc_t(s, &s->a.ax_gx, (size_t)N) && dev_alloc_t(s, &s->a.ax_yx, (size_t)N) &&
+             dev_alloc_t(s, &s->a.ax_gi, (size_t)N) && dev_alloc_t(s, &s->a.ax_yi, (size_t)N) && dev_alloc_t(s, &s->a.ax_h, (size_t)N);
     if (ok && (s->cfg.flags & NG_RECORD_SPIKES) && s->cfg.max_recorded_spikes > 0) {
         ok = dev_alloc_t(s, &s->a.rec_step, (size_t)s->cfg.max_recorded_spikes) &&
              dev_alloc_t(s, &s->a.rec_id, (size_t)s->cfg.max_recorded_spikes);
@@ -463,7 +525,13 @@ int32_t ng_prepare(ng_sim* s) {
     NG_CUDA(s, cudaMemsetAsync(s->d_ctl, 0, sizeof(Ctl), st));
     NG_CUDA(s, cudaMemsetAsync(s->a.I, 0, (size_t)N * 4, st));
     NG_CUDA(s, cudaMemsetAsync(s->a.refr, 0, (size_t)N * 4, st));
-    NG_CUDA(s, cudaMemsetAsync(s->a.ring, 0, (size_t)N * planes * 4, st));
+    NG_CUDA(s, cudaMemsetAsync(s->a.ring, 0, NRs * planes * 4, st));
+    if (s->has_adex) {
+        for (float* p : {s->a.ax_w, s->a.ax_gx, s->a.ax_yx, s->a.ax_gi, s->a.ax_yi}) NG_CUDA(s, cudaMemsetAsync(p, 0, (size_t)N * 4, st));
+        std::vector<float> h0((size_t)N, (float)s->cfg.dt_ms);     // sub-step size starts at the whole time step
+        NG_CUDA(s, cudaMemcpyAsync(s->a.ax_h, h0.data(), (size_t)N * 4, cudaMemcpyHostToDevice, st));
+        NG_CUDA(s, cudaStreamSynchronize(st));
+    }
     if (s->window_backend) {
         // worst case N spikes per step for D steps; beyond 2^26 entries an eighth of that (overflow is detected)
         const long long worst = (long long)N * D;
@@ -471,7 +539,7 @@ int32_t ng_prepare(ng_sim* s) {
         if (!dev_alloc_t(s, &s->a.win_id, (size_t)s->a.win_cap)) return fail(s, NG_ERR_OOM, "device allocation failed (spike window)");
     }
     NG_CUDA(s, cudaMemsetAsync(s->d_cnt, 0, (size_t)N * D * 4, st));
-    if (s->a.last_input) NG_CUDA(s, cudaMemsetAsync(s->a.last_input, 0, (size_t)N * 4, st));
+    if (s->a.last_input) NG_CUDA(s, cudaMemsetAsync(s->a.last_input, 0, NRs * 4, st));
     std::vector<PopDev> pd(s->pops.size());
     for (size_t i = 0; i < s->pops.size(); ++i) pd[i] = s->pops[i].dev;
     NG_CUDA(s, cudaMemcpyAsync(s->d_pops, pd.data(), pd.size() * sizeof(PopDev), cudaMemcpyHostToDevice, st));
@@ -516,7 +584,7 @@ int32_t ng_prepare(ng_sim* s) {
         const long long total = (long long)(c.rule == kRuleIndegree ? c.tgt_n : c.src_n) * c.K;
         if (total == 0) continue;
         build_fill_kernel<<<grid_for(total, 256, cap), 256, 0, st>>>(s->d_calls, (int)ci, seed_lo, seed_hi, D, s->d_cnt,
-                                                                   s->d_row_off, s->d_grp_rel, s->d_tgt, s->d_w, s->d_dly);
+                                                                   s->d_row_off, s->d_grp_rel, s->d_tgt, s->d_w, s->d_dly, N);
         s->launches_other++;
     }
     if (s->sort_segments) {
@@ -535,6 +603,7 @@ int32_t ng_prepare(ng_sim* s) {
     dev_free(s, s->d_row_len); s->d_row_len = nullptr;
 
     // ---- step arguments ----
+    s->a.NR = (int32_t)s->NR; s->a.dt_ms = (float)s->cfg.dt_ms; s->a.has_adex = s->has_adex ? 1 : 0;
     s->a.N = N; s->a.D = D; s->a.Dr = planes; s->a.n_pops = (int32_t)s->pops.size(); s->a.seed_lo = seed_lo; s->a.seed_hi = seed_hi;
     s->a.pop_of = s->d_pop_of; s->a.pops = s->d_pops;
     s->a.row_info = s->d_row_info;
@@ -639,8 +708,9 @@ int32_t ng_simulate(ng_sim* s, int64_t n_steps) {
         NG_CUDA(s, cudaMemsetAsync(&s->d_ctl->bar, 0, sizeof(unsigned long long), st));
         s->last_persistent_blocks = s->delivery_kernel == 3 ? s->persistent_pipe_blocks : s->persistent_blocks;
         if (s->delivery_kernel == 3) {
-            NG_CUDA(s, cudaLaunchCooperativeKernel((const void*)persistent_pipe_kernel, dim3(s->persistent_pipe_blocks),
-                                                   dim3(s->persistent_threads), args, 0, st));
+            const void* fn = s->has_adex ? (const void*)persistent_pipe_kernel<true> : (const void*)persistent_pipe_kernel<false>;
+            NG_CUDA(s, cudaLaunchCooperativeKernel(fn, dim3(s->persistent_pipe_blocks),
+                                                   dim3(s->has_adex ? 512 : s->persistent_threads), args, 0, st));
         } else {
             const void* fn = s->delivery_kernel == 4 ? (const void*)persistent_kernel<4>
                              : s->delivery_kernel == 2 ? (const void*)persistent_kernel<2> : (const void*)persistent_kernel<1>;

@@ -29,15 +29,23 @@ struct DistDev { int32_t kind; int32_t pad; double a, b, lo, hi; };
 
 struct CallDev {               // one ng_connect_* call
     int32_t rule, src_first, src_n, tgt_first, tgt_n, K;
-    int32_t call_index, pad;
+    int32_t call_index, port;              // port: receptor port of the targets (0, or 1 = inhibitory conductance of AdEx)
     DistDev w, d;
 };
 
+struct AdexDev {               // AdEx constants (fp32 copies of the fp64 host values), Table II symbols
+    float g_L, E_L, V_T, inv_DeltaT, gL_DeltaT, inv_C, inv_tau_w, a, b, V_reset, V_peak, E_ex, E_in, inv_tau_syn, I_e;
+    float jump;                            // e / tau_syn: conductance-derivative jump per unit weight (reading C22)
+    float inv_tol[6];                      // 1 / absolute tolerance of (V, w, g_ex, y_ex, g_in, y_in)
+    float h_min;
+};
 struct PopDev {                // per-population constants of the update (fp32 copies of fp64 host values)
     float P11, P22, P21, P20Ie;            // exact-integration propagators; P20Ie = P20 * I_e
     float E_L, V_th, V_reset, w_ext;
     int32_t refr_steps, n_T;
     uint32_t T[kMaxPoissonTable];          // integer Poisson CDF table (C7)
+    int32_t model, pad;                    // 0 = LIF (iaf_psc_exp), 1 = AdEx with alpha conductances
+    AdexDev ax;
 };
 
 struct Ctl {                   // device-resident control block; see ng.cu for the update/deliver handshake
@@ -258,7 +266,7 @@ __global__ void __launch_bounds__(256)
 build_fill_kernel(const CallDev* __restrict__ calls, int call_idx, uint32_t seed_lo, uint32_t seed_hi, int D,
                   uint32_t* __restrict__ cursor, const long long* __restrict__ row_off,
                   const uint32_t* __restrict__ grp_rel, int32_t* __restrict__ tgt, float* __restrict__ w,
-                  uint8_t* __restrict__ dly) {
+                  uint8_t* __restrict__ dly, int n_neurons) {
     const CallDev c = calls[call_idx];
     const int32_t e_first = c.rule == kRuleIndegree ? c.tgt_first : c.src_first;
     const int32_t e_n = c.rule == kRuleIndegree ? c.tgt_n : c.src_n;
@@ -271,7 +279,7 @@ build_fill_kernel(const CallDev* __restrict__ calls, int call_idx, uint32_t seed
         if (dr.delay < 1 || dr.delay > D) continue;
         const uint32_t p = atomicAdd(&cursor[(size_t)dr.src * D + (dr.delay - 1)], 1u);
         const long long pos = row_off[dr.src] + grp_rel[(size_t)dr.src * (D + 1) + (dr.delay - 1)] + p;
-        tgt[pos] = dr.tgt;
+        tgt[pos] = dr.tgt + c.port * n_neurons;             // receptor port folded into the ring column
         w[pos] = dr.w;
         dly[pos] = (uint8_t)dr.delay;
     }
@@ -339,6 +347,9 @@ __device__ __forceinline__ void prefetch_row(const StepArgs& a, const RowInfo& r
 struct StepArgs {
     int32_t N, D;                // D = ring_slots of the C-ABI = largest legal delay
     int32_t Dr, n_pops;          // Dr = D + 1 planes are stored (see update_phase); number of populations
+    int32_t NR, pad_nr;          // ring row length = N * receptor ports (2 as soon as an AdEx population exists):
+                                 // plane of (slot, port) = ring + (slot * NR + port * N); records store target + port * N
+    float *ax_w, *ax_gx, *ax_yx, *ax_gi, *ax_yi, *ax_h;     // AdEx state, [N] each (nullptr without AdEx populations)
     uint32_t seed_lo, seed_hi;
     // neuron state (SoA) and parameters
     float* V; float* I; int32_t* refr; const uint8_t* pop_of; const PopDev* pops;
@@ -359,6 +370,7 @@ struct StepArgs {
     const int32_t* tgt; const float* w; const uint8_t* dly;
     Ctl* ctl;
     int32_t bypass; uint32_t inject_thr;
+    float dt_ms; int32_t has_adex;
     int32_t max_row_chunks;      // ceil(longest padded row / kChunkRecords)
     int32_t mean_row_records;    // mean padded row length (>= 1): picks the item size of delivery kernel 1
 };
@@ -426,7 +438,8 @@ __device__ __forceinline__ void append_spike(const StepArgs& a, bool spk, int32_
 // round trip); the caller then starts everything that depends on the spike (row lookup, L2 prefetch of the row,
 // counters) and neuron_late — Philox, Poisson count, I_syn update: most of the arithmetic — overlaps those latencies.
 // The arithmetic and its order are exactly those of the list above (V uses I before its update).
-struct NeuronRegs { float in, I; int pi, kq; };     // kq: Poisson count computed ahead of time, or 0xff
+struct NeuronRegs { float in, I; int pi, kq; float in1; bool adex; };     // kq: Poisson count computed ahead of time, or 0xff
+
 
 // DESIGN.md C7: k = #{m : x0 >= T[m]}, x0 from Philox(seed; i, n, POISSON); T is non-decreasing.  A pure function of
 // (seed, i, n): the persistent pipelined kernel evaluates it for step n+1 while it waits at the grid barrier.
@@ -440,10 +453,94 @@ __device__ __forceinline__ int poisson_count(const StepArgs& a, const PopDev* __
     return k;
 }
 
+// ---------------------------------------------------------------------------------------
+// AdEx neuron with conductance-based alpha synapses — the model of the paper's balanced network:
+//   Eq. (3)  C dV/dt = -g_L (V - E_L) + g_L Delta_T exp((V - V_T)/Delta_T) + I_syn - w + I_e
+//   Eq. (4)  I_syn = sum_i g_i (E_rev,i - V)                 (sign: DESIGN.md reading C21)
+//   Eq. (5)  tau_w dw/dt = a (V - E_L) - w;   spike: V -> V_r, w -> w + b
+//   alpha conductances g' = -g/tau + y, y' = -y/tau, a spike of weight W raises y by W e / tau   (C22)
+// integrated with "the 5th order Runge-Kutta method with adaptive control of the step size": embedded
+// Cash-Karp 5(4), controller and spike rule as readings C23-C25 state them.  fp32 throughout.
+// ---------------------------------------------------------------------------------------
+struct AdexY { float V, w, gx, yx, gi, yi; };
+
+__device__ __forceinline__ AdexY adex_rhs(const AdexDev& p, const AdexY& y) {
+    const float V = fminf(y.V, p.V_peak);                                           // C24
+    const float I_spike = p.gL_DeltaT * __expf((V - p.V_T) * p.inv_DeltaT);
+    const float I_syn = fmaf(y.gx, p.E_ex - V, y.gi * (p.E_in - V));                // C21
+    AdexY f;
+    f.V = (fmaf(-p.g_L, V - p.E_L, I_spike) + I_syn - y.w + p.I_e) * p.inv_C;
+    f.w = (p.a * (V - p.E_L) - y.w) * p.inv_tau_w;
+    f.gx = fmaf(-y.gx, p.inv_tau_syn, y.yx);
+    f.yx = -y.yx * p.inv_tau_syn;
+    f.gi = fmaf(-y.gi, p.inv_tau_syn, y.yi);
+    f.yi = -y.yi * p.inv_tau_syn;
+    return f;
+}
+#define NG_AXPY(out, y, h, expr) \
+    out.V = fmaf(h, expr(V), y.V); out.w = fmaf(h, expr(w), y.w); out.gx = fmaf(h, expr(gx), y.gx); \
+    out.yx = fmaf(h, expr(yx), y.yx); out.gi = fmaf(h, expr(gi), y.gi); out.yi = fmaf(h, expr(yi), y.yi);
+
+// One time step of one neuron (C23, C24): returns true if it spiked; y and h_int are updated in place.
+__device__ __forceinline__ bool adex_step(const AdexDev& p, AdexY& y, float& h_int, float h_step) {
+    float t = 0.f;
+    bool spiked = false;
+    while (t < h_step) {
+        const float h = fmaxf(h_int, p.h_min);
+        const bool clipped = h > h_step - t;
+        const float ht = clipped ? h_step - t : h;
+        AdexY k1 = adex_rhs(p, y), tmp, k2, k3, k4, k5, k6;
+#define E2(c) (0.2f * k1.c)
+        NG_AXPY(tmp, y, ht, E2) k2 = adex_rhs(p, tmp);
+#define E3(c) (0.075f * k1.c + 0.225f * k2.c)
+        NG_AXPY(tmp, y, ht, E3) k3 = adex_rhs(p, tmp);
+#define E4(c) (0.3f * k1.c - 0.9f * k2.c + 1.2f * k3.c)
+        NG_AXPY(tmp, y, ht, E4) k4 = adex_rhs(p, tmp);
+#define E5(c) ((-11.f / 54.f) * k1.c + 2.5f * k2.c - (70.f / 27.f) * k3.c + (35.f / 27.f) * k4.c)
+        NG_AXPY(tmp, y, ht, E5) k5 = adex_rhs(p, tmp);
+#define E6(c) ((1631.f / 55296.f) * k1.c + (175.f / 512.f) * k2.c + (575.f / 13824.f) * k3.c + (44275.f / 110592.f) * k4.c + (253.f / 4096.f) * k5.c)
+        NG_AXPY(tmp, y, ht, E6) k6 = adex_rhs(p, tmp);
+        // 5th-order weights and the difference to the embedded 4th-order ones
+#define Y5(c) ((37.f / 378.f) * k1.c + (250.f / 621.f) * k3.c + (125.f / 594.f) * k4.c + (512.f / 1771.f) * k6.c)
+#define ER(c) ((37.f / 378.f - 2825.f / 27648.f) * k1.c + (250.f / 621.f - 18575.f / 48384.f) * k3.c + \
+               (125.f / 594.f - 13525.f / 55296.f) * k4.c - (277.f / 14336.f) * k5.c + (512.f / 1771.f - 0.25f) * k6.c)
+        float e = fabsf(ht * ER(V)) * p.inv_tol[0];
+        e = fmaxf(e, fabsf(ht * ER(w)) * p.inv_tol[1]);
+        e = fmaxf(e, fabsf(ht * ER(gx)) * p.inv_tol[2]);
+        e = fmaxf(e, fabsf(ht * ER(yx)) * p.inv_tol[3]);
+        e = fmaxf(e, fabsf(ht * ER(gi)) * p.inv_tol[4]);
+        e = fmaxf(e, fabsf(ht * ER(yi)) * p.inv_tol[5]);
+        const bool accept = e <= 1.f || ht <= p.h_min;
+        float fac = e > 0.f ? 0.9f * __powf(e, -0.2f) : 5.f;
+        fac = fminf(5.f, fmaxf(0.2f, fac));
+        if (!clipped || !accept) h_int = fminf(h_step, ht * fac);
+        if (accept) {
+            NG_AXPY(tmp, y, ht, Y5)
+            y = tmp;
+            t = clipped ? h_step : t + ht;
+            if (y.V >= p.V_peak) { y.V = p.V_reset; y.w += p.b; spiked = true; }     // C24; a 2nd crossing is not recorded (C20)
+        }
+#undef E2
+#undef E3
+#undef E4
+#undef E5
+#undef E6
+#undef Y5
+#undef ER
+    }
+    return spiked;
+}
+#undef NG_AXPY
+
+// kAdex: the network holds AdEx populations (second receptor port, AdEx state arrays); LIF-only networks compile to
+// exactly the code without it.
+template <bool kAdex>
 __device__ __forceinline__ bool neuron_early(const StepArgs& a, const PopDev* __restrict__ P, long long n, int i,
                                              float* __restrict__ plane, NeuronRegs& g, bool have_k = false) {
     g.in = __ldcg(plane + i);                    // written by red.global from other SMs: read at L2
     g.kq = have_k ? (int)a.pois_k[i] : 0xff;
+    g.adex = false;
+    if (kAdex) g.in1 = __ldcg(plane + a.N + i);  // inhibitory port
     if (a.bypass) {                                          // DESIGN.md C8: delivery-only mode
         const uint4 x = philox4x32_10(a.seed_lo, a.seed_hi, (uint32_t)i, (uint32_t)n, (uint32_t)(n >> 32), kTagInject);
         return x.x < a.inject_thr;
@@ -453,6 +550,16 @@ __device__ __forceinline__ bool neuron_early(const StepArgs& a, const PopDev* __
     int r = a.refr[i];
     g.pi = a.pop_of[i];
     const PopDev* __restrict__ p = P + g.pi;
+    if (kAdex && p->model == 1) {                // AdEx: the whole step is integrated here; neuron_late applies the jumps
+        g.adex = true;
+        AdexY y; y.V = V; y.w = a.ax_w[i]; y.gx = a.ax_gx[i]; y.yx = a.ax_yx[i]; y.gi = a.ax_gi[i]; y.yi = a.ax_yi[i];
+        float h_int = a.ax_h[i];
+        const bool s = adex_step(p->ax, y, h_int, a.dt_ms);
+        a.V[i] = y.V; a.ax_w[i] = y.w; a.ax_gx[i] = y.gx; a.ax_gi[i] = y.gi; a.ax_h[i] = h_int;
+        g.I = y.yx;
+        a.ax_yi[i] = fmaf(p->ax.jump, g.in1, y.yi);          // C25: jumps arriving at t_{n+1}
+        return s;
+    }
     const float E_L = p->E_L;
     bool spk = false;
     if (r == 0) V = E_L + fmaf(p->P22, V - E_L, fmaf(p->P21, g.I, p->P20Ie));
@@ -462,28 +569,35 @@ __device__ __forceinline__ bool neuron_early(const StepArgs& a, const PopDev* __
     return spk;
 }
 
+template <bool kAdex>
 __device__ __forceinline__ void neuron_late(const StepArgs& a, const PopDev* __restrict__ P, long long n, int i,
                                             float* __restrict__ plane, const NeuronRegs& g) {
     plane[i] = 0.f;
-    if (a.last_input) a.last_input[i] = g.in;
+    if (kAdex) plane[a.N + i] = 0.f;
+    if (a.last_input) { a.last_input[i] = g.in; if (kAdex) a.last_input[a.N + i] = g.in1; }
     if (a.bypass) return;
     const PopDev* __restrict__ p = P + g.pi;
     const int k = g.kq != 0xff ? g.kq : poisson_count(a, p, n, i);
+    if (kAdex && g.adex) {                       // g.I carries y_ex after the integration; Poisson drive on the excitatory port
+        a.ax_yx[i] = fmaf(p->ax.jump, fmaf(p->w_ext, (float)k, g.in), g.I);
+        return;
+    }
     a.I[i] = fmaf(p->P11, g.I, g.in) + p->w_ext * (float)k;
 }
 
+template <bool kAdex>
 __device__ __forceinline__ void update_phase(const StepArgs& a, const PopDev* __restrict__ P, long long n, int slot,
                                              unsigned long long rec_base, long long gtid, long long gthreads,
                                              unsigned long long win_base = 0) {
     const int N = a.N;
-    float* __restrict__ plane = a.ring + (size_t)slot * N;
+    float* __restrict__ plane = a.ring + (size_t)slot * a.NR;
     const long long n_round = ((long long)N + 31) & ~31LL;      // keep warps whole for the ballot
     for (long long ii = gtid; ii < n_round; ii += gthreads) {
         const int i = (int)ii;
         NeuronRegs g;
-        const bool spk = i < N && neuron_early(a, P, n, i, plane, g);
+        const bool spk = i < N && neuron_early<kAdex>(a, P, n, i, plane, g);
         append_spike(a, spk, i, n, rec_base, win_base);
-        if (i < N) neuron_late(a, P, n, i, plane, g);
+        if (i < N) neuron_late<kAdex>(a, P, n, i, plane, g);
     }
 }
 
@@ -552,7 +666,7 @@ struct DeliverShared {
 // items are spread over every warp of the grid; under load 128-record items keep the loads 128-bit wide.
 template <int kPerLane>
 __device__ __forceinline__ void deliver_item(const StepArgs& a, int nmod, long long r0, int len, int c, int lane, int skip = 0) {
-    const int N = a.N, Dr = a.Dr;
+    const int Dr = a.Dr;
     const int q = (c * 32 + lane) * kPerLane;
     if (q >= len || q + kPerLane <= skip) return;          // records [0, skip) were delivered by the delay-1 pass
     const long long p = r0 + q;
@@ -561,16 +675,16 @@ __device__ __forceinline__ void deliver_item(const StepArgs& a, int nmod, long l
         const int4 t = ld_stream_s32x4(a.tgt + p);
         const float4 ww = ld_stream_f32x4(a.w + p);
         const uint32_t dd = ld_stream_u32(a.dly + p);
-        if (t.x >= 0 && q >= skip) { s = nmod + (int)(dd & 0xff); if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * N + t.x, ww.x); }
-        if (t.y >= 0 && q + 1 >= skip) { s = nmod + (int)((dd >> 8) & 0xff); if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * N + t.y, ww.y); }
-        if (t.z >= 0 && q + 2 >= skip) { s = nmod + (int)((dd >> 16) & 0xff); if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * N + t.z, ww.z); }
-        if (t.w >= 0 && q + 3 >= skip) { s = nmod + (int)(dd >> 24); if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * N + t.w, ww.w); }
+        if (t.x >= 0 && q >= skip) { s = nmod + (int)(dd & 0xff); if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * a.NR + t.x, ww.x); }
+        if (t.y >= 0 && q + 1 >= skip) { s = nmod + (int)((dd >> 8) & 0xff); if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * a.NR + t.y, ww.y); }
+        if (t.z >= 0 && q + 2 >= skip) { s = nmod + (int)((dd >> 16) & 0xff); if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * a.NR + t.z, ww.z); }
+        if (t.w >= 0 && q + 3 >= skip) { s = nmod + (int)(dd >> 24); if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * a.NR + t.w, ww.w); }
     } else {
         int t; float ww; uint32_t dd;
         asm("ld.global.nc.L1::no_allocate.s32 %0, [%1];" : "=r"(t) : "l"(a.tgt + p));
         asm("ld.global.nc.L1::no_allocate.f32 %0, [%1];" : "=f"(ww) : "l"(a.w + p));
         asm("ld.global.nc.L1::no_allocate.u8 %0, [%1];" : "=r"(dd) : "l"(a.dly + p));
-        if (t >= 0) { s = nmod + (int)dd; if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * N + t, ww); }
+        if (t >= 0) { s = nmod + (int)dd; if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * a.NR + t, ww); }
     }
 }
 
@@ -678,7 +792,7 @@ __device__ __forceinline__ VecRef locate_vec(int v, int total, int pre, long lon
     return r;
 }
 __device__ __forceinline__ void red_vec(const StepArgs& a, const VecRef& r, const int4& t, const float4& ww) {
-    float* __restrict__ plane = a.ring + (size_t)r.slot * a.N;
+    float* __restrict__ plane = a.ring + (size_t)r.slot * a.NR;
     if (r.q >= r.rel_lo && r.q < r.len) red_add_f32(plane + t.x, ww.x);
     if (r.q + 1 >= r.rel_lo && r.q + 1 < r.len) red_add_f32(plane + t.y, ww.y);
     if (r.q + 2 >= r.rel_lo && r.q + 2 < r.len) red_add_f32(plane + t.z, ww.z);
@@ -884,7 +998,7 @@ __device__ __forceinline__ int pipe_updater_threads(int N) {
     return (int)per_cta <= cap ? max(need, 32) : cap;
 }
 
-template <bool kUpdate>
+template <bool kUpdate, bool kAdex>
 __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* __restrict__ P, long long n, int slot, bool pending,
                                                unsigned long long rec_prev, PipeShared& sh, bool have_k = false) {
     const int N = a.N, Dr = a.Dr;
@@ -900,8 +1014,8 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
         // ---- update(n), spike collection, then the delay-1 records of this CTA's spikes ----
         if (kUpdate) {
             const int wib = threadIdx.x >> 5, wpu = U >> 5;
-            float* __restrict__ plane = a.ring + (size_t)slot * N;
-            float* __restrict__ plane1 = a.ring + (size_t)(slot + 1 == Dr ? 0 : slot + 1) * N;
+            float* __restrict__ plane = a.ring + (size_t)slot * a.NR;
+            float* __restrict__ plane1 = a.ring + (size_t)(slot + 1 == Dr ? 0 : slot + 1) * a.NR;
             const bool single_round = (long long)gridDim.x * U >= N;
             for (long long base = (long long)blockIdx.x * U; base < N; base += (long long)gridDim.x * U) {
                 const long long ii = base + threadIdx.x;
@@ -913,7 +1027,7 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
                 // bandwidth than the round trip of the few spiking threads)
                 RowInfo r;
                 if (single_round && ii < N) r = ld_row_info(a.row_info + i);
-                const bool spk = ii < N && neuron_early(a, P, n, i, plane, g, have_k);
+                const bool spk = ii < N && neuron_early<kAdex>(a, P, n, i, plane, g, have_k);
                 if (!single_round && spk) r = ld_row_info(a.row_info + i);
                 const unsigned m = __ballot_sync(0xffffffffu, spk);
                 if (m) {                                           // warp-aggregated append to the CTA's own list
@@ -938,7 +1052,7 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
                         }
                     }
                 }
-                if (ii < N) neuron_late(a, P, n, i, plane, g);
+                if (ii < N) neuron_late<kAdex>(a, P, n, i, plane, g);
             }
             trace_stamp(a, n, 3);
             group_sync(1, U);
@@ -1076,7 +1190,7 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
 // Graph / plain-launch form: one launch per time step, the kernel boundary is the barrier.  The last CTA to finish
 // publishes the next step index (a4) and marks the rest pass of this step as pending.
 constexpr int kPipeThreads = 512;        // 256 updaters + 256 rest-pass threads
-template <bool kUpdate>
+template <bool kUpdate, bool kAdex>
 __global__ void __launch_bounds__(kPipeThreads) pipe_step_kernel(const StepArgs a) {
     __shared__ PipeShared sh;
     if (threadIdx.x == 0) {
@@ -1089,7 +1203,7 @@ __global__ void __launch_bounds__(kPipeThreads) pipe_step_kernel(const StepArgs 
     if (a.n_pops > kMaxPopsSmem) __syncthreads();
     const long long n = sh.sc.n;
     const int slot = sh.sc.slot;
-    pipelined_phase<kUpdate>(a, P, n, slot, sh.pending != 0, sh.sc.rec_base, sh);
+    pipelined_phase<kUpdate, kAdex>(a, P, n, slot, sh.pending != 0, sh.sc.rec_base, sh);
     if (threadIdx.x == 0) {
         __threadfence();
         const unsigned t = atomicAdd(&a.ctl->ticket, 1u);
@@ -1110,7 +1224,9 @@ __global__ void __launch_bounds__(kPipeThreads) pipe_step_kernel(const StepArgs 
     }
 }
 
-__global__ void __launch_bounds__(kPersistentThreads, 1) persistent_pipe_kernel(const StepArgs a, long long n_steps) {
+// kAdex: the AdEx integrator needs more than the 64 registers a 1024-thread CTA leaves: 512-thread CTAs, two per SM at most
+template <bool kAdex>
+__global__ void __launch_bounds__(kAdex ? 512 : kPersistentThreads, 1) persistent_pipe_kernel(const StepArgs a, long long n_steps) {
     __shared__ PipeShared sh;
     if (threadIdx.x == 0) {
         sh.sc.n = __ldcg(&a.ctl->step_u);
@@ -1128,7 +1244,7 @@ __global__ void __launch_bounds__(kPersistentThreads, 1) persistent_pipe_kernel(
     for (long long s = 0; s < n_steps; ++s, ++n) {
         if (gtid == 0) a.ctl->spike_cnt[(n + 1) & 3] = 0;          // last read (as step n-3's) in phase n-2
         trace_stamp(a, n, 0);
-        const int Mp = pipelined_phase<true>(a, P, n, slot, s > 0, rec_prev, sh, s > 0 && single_round);
+        const int Mp = pipelined_phase<true, kAdex>(a, P, n, slot, s > 0, rec_prev, sh, s > 0 && single_round);
         rec_prev += (unsigned long long)Mp; spikes += (unsigned long long)Mp;
         trace_stamp(a, n, 1);
         grid_arrive(a.ctl, epoch);
@@ -1141,7 +1257,7 @@ __global__ void __launch_bounds__(kPersistentThreads, 1) persistent_pipe_kernel(
         slot = slot + 1 == a.Dr ? 0 : slot + 1;
     }
     if (n_steps > 0) {                                             // flush: rest pass of the last step
-        const int Mp = pipelined_phase<false>(a, P, n, slot, true, rec_prev, sh);
+        const int Mp = pipelined_phase<false, kAdex>(a, P, n, slot, true, rec_prev, sh);
         rec_prev += (unsigned long long)Mp; spikes += (unsigned long long)Mp;
     }
     if (gtid == 0) {
@@ -1175,6 +1291,7 @@ __device__ __forceinline__ void window_bookkeeping(const StepArgs& a, long long 
     if (ws.off[ws.W] - ws.off[0] > (unsigned long long)a.win_cap) a.ctl->err_window = 1;
 }
 
+template <bool kAdex>
 __global__ void __launch_bounds__(kUpdateThreads) update_kernel(const StepArgs a) {
     __shared__ PopDev sh_pops[kMaxPopsSmem];
     __shared__ StepScalars sc;
@@ -1188,7 +1305,7 @@ __global__ void __launch_bounds__(kUpdateThreads) update_kernel(const StepArgs a
     }
     const PopDev* P = stage_pops(a, sh_pops);              // contains the __syncthreads that publishes sc
     if (a.n_pops > kMaxPopsSmem) __syncthreads();
-    update_phase(a, P, sc.n, sc.slot, sc.rec_base, (long long)blockIdx.x * blockDim.x + threadIdx.x, (long long)gridDim.x * blockDim.x,
+    update_phase<kAdex>(a, P, sc.n, sc.slot, sc.rec_base, (long long)blockIdx.x * blockDim.x + threadIdx.x, (long long)gridDim.x * blockDim.x,
                  win_base);
 }
 
@@ -1245,7 +1362,7 @@ __global__ void __launch_bounds__(kPersistentThreads, 1) persistent_kernel(const
         // the counter of step n+1 was last read (as step n-3's) before the barriers of step n-1
         if (gtid == 0) a.ctl->spike_cnt[(n + 1) & 3] = 0;
         trace_stamp(a, n, 0);
-        update_phase(a, P, n, slot, rec_base, gtid, gthreads, win_base);
+        update_phase<false>(a, P, n, slot, rec_base, gtid, gthreads, win_base);      // two-phase persistent kernels: LIF only
         trace_stamp(a, n, 1);
         grid_barrier(a.ctl, epoch);
         trace_stamp(a, n, 2);
@@ -1281,7 +1398,7 @@ __global__ void __launch_bounds__(kPersistentThreads, 1) persistent_kernel(const
 // Spike-buffer backend, read-back only (NG_FIELD_RING): expand the pending part of the spike window into a [D][N] ring
 // image: entry (step s, source j), record (target, w, d) with s + d > n arrives in step s + d (slot (s+d) mod D).
 __global__ void materialize_window_kernel(const StepArgs a, long long n, float* __restrict__ out) {
-    const int D = a.D, N = a.N;
+    const int D = a.D;
     const int W = (int)(n < (long long)D ? n : (long long)D);                      // steps n-W .. n-1 are buffered
     const int lane = threadIdx.x & 31;
     const long long gwarp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5, gwarps = ((long long)gridDim.x * blockDim.x) >> 5;
@@ -1295,7 +1412,7 @@ __global__ void materialize_window_kernel(const StepArgs a, long long n, float* 
             const int deg = (int)a.grp_rel[(size_t)j * (D + 1) + D];
             for (int q = lane; q < deg; q += 32) {
                 const int d = a.dly[r0 + q];
-                if (s + d >= n + 1) atomicAdd(out + (size_t)((s + d) % D) * N + a.tgt[r0 + q], a.w[r0 + q]);
+                if (s + d >= n + 1) atomicAdd(out + (size_t)((s + d) % D) * a.NR + a.tgt[r0 + q], a.w[r0 + q]);
             }
         }
     }
