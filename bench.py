@@ -30,6 +30,7 @@ import numpy as np
 TIME_STEPS_PER_BENCH_STEP = 1000
 DT_MS = 0.1
 PAPER_RTF_2080TI = 1.055          # PAPER.md:248, full-scale microcircuit, NeuronGPU on RTX 2080 Ti (context, other hardware)
+PAPER_RTF_ADEX_1M = 70.0          # PAPER.md:16, balanced network of 1e6 AdEx neurons / 1e9 synapses on an RTX 2080 Ti (context)
 BYTES_PER_EVENT = 8               # 4 B target + 4 B weight per synaptic event
 BYTES_PER_NEURON_STEP = 33        # V, I_syn, refr read+write (24 B) + ring slot read+zero (8 B) + population index (1 B)
 
@@ -98,7 +99,7 @@ class ClockSampler:
 def make_workload(name, seed_offset=0):
     from paper_2007_14236_b200 import workloads as W
     wl = {"cfg0": W.brunel_tiny, "cfg1": lambda: W.microcircuit(10), "cfg2": lambda: W.microcircuit(1),
-          "cfg4": W.balanced_large}[name]()
+          "cfg4": W.balanced_large, "adex1m": W.balanced_adex, "adex100k": lambda: W.balanced_adex(n=100_000)}[name]()
     wl.seed += seed_offset
     return wl
 
@@ -107,7 +108,10 @@ def workload_label(name):
     return {"cfg0": "configs[0] tiny Brunel-style LIF net, 1,000 neurons",
             "cfg1": "configs[1] cortical microcircuit at 10% neuron scale, full in-degrees, 7,718 neurons / 29,892,043 synapses",
             "cfg2": "configs[2] full-scale cortical microcircuit, 77,169 LIF neurons / 298,905,266 synapses",
-            "cfg4": "configs[4] balanced E/I network, 1,000,000 LIF neurons / 1e9 synapses"}[name]
+            "cfg4": "configs[4] balanced E/I network, 1,000,000 LIF neurons / 1e9 synapses",
+            "adex1m": "the paper's balanced network (PAPER.md:110-128, Tables I-II): 1,000,000 AdEx neurons with alpha conductances, "
+                      "1000 inputs each (1e9 synapses), adaptive RK5",
+            "adex100k": "the paper's balanced network at 100,000 AdEx neurons, 1000 inputs each (1e8 synapses)"}[name]
 
 
 def dist_setup(n_gpus):
@@ -282,7 +286,9 @@ def run_ours(args):
         kern = {1: "persistent_kernel<1>", 2: "persistent_kernel<2>", 3: "persistent_pipe_kernel"}[int(s1.delivery_kernel)]
         us = ms_total * 1e3 / args.steps
         ev_per_launch = float(s1.events - s0.events) / args.steps
-        alg_bytes = T * N * BYTES_PER_NEURON_STEP + ev_per_launch * BYTES_PER_EVENT
+        # AdEx: seven state words and two input ports per neuron instead of three and one
+        bpn = 73 if args.workload.startswith("adex") else BYTES_PER_NEURON_STEP
+        alg_bytes = T * N * bpn + ev_per_launch * BYTES_PER_EVENT
         share = {"persistent_kernel_share_of_step": 1.0, "time_steps_per_launch": T}
     else:
         # per-kernel CUDA-event times (NG_OPT_PROFILE, plain launches) over the same number of time steps
@@ -320,7 +326,7 @@ def run_ours(args):
     line = {
         "metric": "real_time_factor", "value": rtf, "unit": "wall_s_per_bio_s", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": False, "scaling": "weak",
-        "vs_baseline": rtf / PAPER_RTF_2080TI if args.workload == "cfg2" else None,
+        "vs_baseline": rtf / PAPER_RTF_2080TI if args.workload == "cfg2" else rtf / PAPER_RTF_ADEX_1M if args.workload == "adex1m" else None,
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": workload_label(args.workload), "time_steps_per_bench_step": T, "dt_ms": DT_MS,
                    "parallelism": "replicas only (independent seeds per rank, no collective)" if world > 1 else "1 GPU",
@@ -415,7 +421,7 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=["cfg0", "cfg1", "cfg2", "cfg4"])
+    ap.add_argument("--workload", default="cfg2", choices=["cfg0", "cfg1", "cfg2", "cfg4", "adex1m", "adex100k"])
     ap.add_argument("--no-microbench", action="store_true", help="skip the configs[3] delivery microbenchmark")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip timing the oracle")
     ap.add_argument("--only-microbench", action="store_true",
