@@ -207,7 +207,7 @@ void configure_launch(ng_sim* s) {
     s->step_mode = s->step_mode_opt != 3 ? s->step_mode_opt : (k == 2 || k == 4 || !s->coop_ok) ? 0 : 2;
     if (s->has_adex && s->step_mode == 2 && k != 3) s->step_mode = 0;   // the two-phase persistent kernels are LIF only
     s->a.prefetch = (k != 2 && k != 4 && s->prefetch_opt) ? 1 : 0;
-    s->pipe_blocks = grid_for(s->N, kPipeThreads - kEntryTile, sm * 4);   // updaters per CTA = kPipeThreads - kEntryTile
+    s->pipe_blocks = grid_for(s->N, kPipeThreads - (s->has_adex ? 128 : kEntryTile), sm * 4);   // updaters per CTA
     {
         int occp = 0;
         const int pt = s->has_adex ? 512 : s->persistent_threads;      // AdEx kernels are compiled for 512-thread CTAs

@@ -705,13 +705,15 @@ __device__ __forceinline__ int deliver_rows_phase(const StepArgs& a, long long n
     const int cshift = small ? 5 : 7;
     unsigned long long ev = 0;
     int base_mod = 0;                                          // (flattened index of the tile's first item) mod gw_n
-    // Many spikes (>= 16 per CTA): every CTA stages only its own tiles of the spike array and deals their items to its
+    // Many spikes (>= 8 per CTA): every CTA stages only its own tiles of the spike array and deals their items to its
     // own warps; few spikes: every CTA stages all of them and the items are dealt to all warps of the grid.
-    const bool part = M >= 16 * (int)gridDim.x;
-    const int tile_first = part ? (int)blockIdx.x * kEntryTile : 0, tile_stride = part ? (int)gridDim.x * kEntryTile : kEntryTile;
+    const bool part = M >= 8 * (int)gridDim.x;
+    // a CTA's tile holds about M / gridDim entries, so that every CTA has one
+    const int tile_len = part ? min(kEntryTile, (M + (int)gridDim.x - 1) / (int)gridDim.x) : kEntryTile;
+    const int tile_first = part ? (int)blockIdx.x * tile_len : 0, tile_stride = part ? (int)gridDim.x * tile_len : kEntryTile;
     const int gw = part ? wib : gwarp, gw_n = part ? wpb : gwarps;
     for (int tile0 = tile_first; tile0 < M; tile0 += tile_stride) {
-        const int m = min(kEntryTile, M - tile0);
+        const int m = min(tile_len, M - tile0);
         if (tile0 > 0) {
             __syncthreads();                                   // previous tile's readers are done
             if (threadIdx.x < m) e = __ldcg(reinterpret_cast<const int4*>(rows + tile0 + threadIdx.x));
@@ -991,10 +993,11 @@ __device__ __forceinline__ void pipe_one_item(const StepArgs& a, int nmod, PipeS
 }
 // Updaters per CTA: just enough for one neuron per thread when the network is small enough for a single round
 // (every other warp then joins the rest pass), else all but kEntryTile threads.
-__device__ __forceinline__ int pipe_updater_threads(int N) {
+// AdEx networks spend their step in the integrator: only four warps are set aside for the rest pass there.
+__device__ __forceinline__ int pipe_updater_threads(int N, bool heavy_update) {
     const unsigned per_cta = ((unsigned)N + gridDim.x - 1u) / gridDim.x;          // 32-bit: no 64-bit division on the step path
     const int need = (int)((per_cta + 31u) & ~31u);
-    const int cap = (int)blockDim.x - (blockDim.x >= 512 ? kEntryTile : 64);
+    const int cap = (int)blockDim.x - (blockDim.x < 512 ? 64 : heavy_update ? 128 : kEntryTile);
     return (int)per_cta <= cap ? max(need, 32) : cap;
 }
 
@@ -1003,7 +1006,7 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
                                                unsigned long long rec_prev, PipeShared& sh, bool have_k = false) {
     const int N = a.N, Dr = a.Dr;
     const int lane = threadIdx.x & 31;
-    const int U = pipe_updater_threads(N), R = blockDim.x - U;     // rest group = threads [U, U + R), R >= 64
+    const int U = pipe_updater_threads(N, kAdex), R = blockDim.x - U;     // rest group = threads [U, U + R), R >= 64
     const int RT = min(R, kEntryTile);                             // threads of the rest group that stage entries
     const int nmod_prev = slot == 0 ? Dr - 1 : slot - 1;           // (n - 1) mod Dr
     if (threadIdx.x == 0) sh.n_d1 = 0;
@@ -1128,13 +1131,15 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
         const int cshift = small ? 5 : 7;
         unsigned long long ev = 0;
         int base_mod = 0;
-        // many spikes (>= 16 per CTA): every CTA stages only its own tiles and deals their items to its own rest warps
-        const bool part = M >= 16 * (int)gridDim.x;
-        const int tile_first = part ? (int)blockIdx.x * RT : 0, tile_stride = part ? (int)gridDim.x * RT : RT;
+        // many spikes (>= 8 per CTA): every CTA stages only its own tiles and deals their items to its own rest warps
+        const bool part = M >= 8 * (int)gridDim.x;
+        // a CTA's tile holds about M / gridDim entries, so that every CTA has one
+        const int tile_len = part ? min(RT, (M + (int)gridDim.x - 1) / (int)gridDim.x) : RT;
+        const int tile_first = part ? (int)blockIdx.x * tile_len : 0, tile_stride = part ? (int)gridDim.x * tile_len : RT;
         const int gw = part ? wir : gwarp, gw_n = part ? wpr : gwarps;
         const bool rec_here = a.rec_cap > 0 && (blockIdx.x == 0 || part);
         for (int tile0 = tile_first; tile0 < M; tile0 += tile_stride) {
-            const int m = min(RT, M - tile0);
+            const int m = min(tile_len, M - tile0);
             if (tile0 > 0) {
                 group_sync(2, R);
                 if (t < m) {
@@ -1226,7 +1231,7 @@ __global__ void __launch_bounds__(kPipeThreads) pipe_step_kernel(const StepArgs 
 
 // kAdex: the AdEx integrator needs more than the 64 registers a 1024-thread CTA leaves: 512-thread CTAs, two per SM at most
 template <bool kAdex>
-__global__ void __launch_bounds__(kAdex ? 512 : kPersistentThreads, 1) persistent_pipe_kernel(const StepArgs a, long long n_steps) {
+__global__ void __launch_bounds__(kAdex ? 512 : kPersistentThreads, kAdex ? 2 : 1) persistent_pipe_kernel(const StepArgs a, long long n_steps) {
     __shared__ PipeShared sh;
     if (threadIdx.x == 0) {
         sh.sc.n = __ldcg(&a.ctl->step_u);
@@ -1236,7 +1241,7 @@ __global__ void __launch_bounds__(kAdex ? 512 : kPersistentThreads, 1) persisten
     const PopDev* P = stage_pops(a, sh.pops);
     if (a.n_pops > kMaxPopsSmem) __syncthreads();
     const long long gtid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const int U = pipe_updater_threads(a.N);
+    const int U = pipe_updater_threads(a.N, kAdex);
     const bool single_round = (long long)gridDim.x * U >= a.N;     // else the counts are computed in line, overlapping the loads
     long long n = sh.sc.n;
     int slot = sh.sc.slot;
