@@ -259,6 +259,22 @@ int32_t ng_get_connections(ng_sim* sim, int32_t src_id, int32_t* tgt_host, float
 /* Counters and timings.  Synchronises the stream. */
 int32_t ng_get_stats(ng_sim* sim, ng_stats* out);
 
+/* On-device spike statistics, the three quantities the paper validates its simulations with: per
+ * neuron the average firing rate and the coefficient of variation of the inter-spike interval (standard deviation over
+ * mean), and per population the Pearson correlation matrix of the spike trains of a sample of neurons re-binned to
+ * bin_steps time steps (the paper: 200 neurons, 2 ms).  Accumulated at spike time inside the step kernels from
+ * start_step on (the paper discards the first second); no spike record or host round trip is needed.
+ *   ng_enable_statistics: after ng_prepare, once.  The sample of a population is its first sample_per_pop neurons.
+ *     Spikes in bins >= max_bins are not binned (rates and CVs still count them).
+ *   ng_get_rate_cv: rate_hz[N], cv_isi[N] (NaN with fewer than two intervals) into host or device arrays.
+ *   ng_get_correlations: corr[ns*ns] row-major over the complete bins so far (NaN for a silent train); n_sample_out = ns
+ *     and n_bins_out are always set, the matrix is written only if capacity >= ns*ns.
+ * Errors: STATE (before ng_prepare, not enabled, enabled twice, nothing simulated yet), INVALID_ARG, OOM. */
+int32_t ng_enable_statistics(ng_sim* sim, int64_t start_step, int32_t bin_steps, int32_t sample_per_pop, int32_t max_bins);
+int32_t ng_get_rate_cv(ng_sim* sim, float* rate_hz, float* cv_isi, int64_t count);
+int32_t ng_get_correlations(ng_sim* sim, int32_t population, float* corr, int64_t capacity, int32_t* n_sample_out,
+                            int32_t* n_bins_out);
+
 /* Phase stamps of the last persistent launch (NG_OPT_TRACE): uint64 ns (%globaltimer), laid out
  * [64 steps][blocks][16 stamps], step index = step mod 64, one stamping thread per CTA and stamp.
  *   two-phase kernels (delivery kernel 1, 2): 0 step start, 1 update done, 2 after the first barrier, 3 delivery done,

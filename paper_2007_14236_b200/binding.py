@@ -25,7 +25,8 @@ EXPORTS = ["ng_create", "ng_destroy", "ng_last_error", "ng_create_population", "
            "ng_connect_fixed_outdegree", "ng_set_bypass", "ng_set_option", "ng_prepare", "ng_set_state",
            "ng_get_state", "ng_simulate", "ng_get_spikes", "ng_get_last_spikes", "ng_copy_row_offsets",
            "ng_copy_group_offsets", "ng_copy_records", "ng_get_connections", "ng_get_stats", "ng_get_trace", "ng_probe",
-           "ng_create_population_adex", "ng_connect_fixed_indegree_port", "ng_connect_fixed_outdegree_port"]
+           "ng_create_population_adex", "ng_connect_fixed_indegree_port", "ng_connect_fixed_outdegree_port",
+           "ng_enable_statistics", "ng_get_rate_cv", "ng_get_correlations"]
 
 
 class NgConfig(C.Structure):
@@ -120,6 +121,9 @@ def load_library(path: str | None = None):
     L.ng_get_connections.argtypes = [vp, i32, vp, vp, vp, i64, C.POINTER(i64)]
     L.ng_get_stats.argtypes = [vp, C.POINTER(NgStats)]
     L.ng_get_trace.argtypes = [vp, vp, i64, C.POINTER(i64), C.POINTER(i32)]
+    L.ng_enable_statistics.argtypes = [vp, i64, i32, i32, i32]
+    L.ng_get_rate_cv.argtypes = [vp, vp, vp, i64]
+    L.ng_get_correlations.argtypes = [vp, i32, vp, i64, C.POINTER(i32), C.POINTER(i32)]
     L.ng_probe.argtypes = [i32, i32, i64, C.POINTER(C.c_double)]
     for name in EXPORTS:
         if name != "ng_last_error":
@@ -308,6 +312,25 @@ class Sim:
         if cap > 0:
             self._chk(self._L.ng_get_spikes(self._h, _ptr(steps), _ptr(ids), cap, C.byref(cnt)))
         return steps[:cap], ids[:cap]
+
+    def enable_statistics(self, start_step: int = 0, bin_steps: int = 20, sample_per_pop: int = 200, max_bins: int = 8192):
+        self._chk(self._L.ng_enable_statistics(self._h, start_step, bin_steps, sample_per_pop, max_bins))
+
+    def rate_cv(self):
+        """(rate_hz[N], cv_isi[N]) computed on the device from the spike-time accumulators."""
+        n = self.n_neurons
+        rate = np.empty(n, np.float32); cv = np.empty(n, np.float32)
+        self._chk(self._L.ng_get_rate_cv(self._h, rate.ctypes.data, cv.ctypes.data, n))
+        return rate, cv
+
+    def correlations(self, population: int) -> np.ndarray:
+        """Pearson correlation matrix [ns, ns] of the binned spike trains of the population's sample."""
+        ns, nb = C.c_int32(), C.c_int32()
+        self._chk(self._L.ng_get_correlations(self._h, population, None, 0, C.byref(ns), C.byref(nb)))
+        out = np.empty((ns.value, ns.value), np.float32)
+        if ns.value and nb.value:
+            self._chk(self._L.ng_get_correlations(self._h, population, out.ctypes.data, out.size, C.byref(ns), C.byref(nb)))
+        return out
 
     def trace(self) -> np.ndarray:
         """ng_get_trace: uint64 ns stamps [64 steps][blocks][8] of the last persistent launch (OPT_TRACE)."""

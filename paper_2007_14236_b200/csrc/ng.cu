@@ -55,6 +55,8 @@ struct ng_sim {
     int delivery_kernel = 1; int deliver_blocks = 0; int update_blocks = 0; int persistent_blocks = 0;
     int pipe_blocks = 0; int persistent_pipe_blocks = 0;
     int persistent_threads = kPersistentThreads;
+    // statistics (ng_enable_statistics)
+    int32_t* d_st_sample = nullptr; int st_sample_per_pop = 0; int st_slots = 0;
     bool has_adex = false;                 // any AdEx population: two receptor ports, AdEx state arrays, <true> kernels
     int64_t NR = 0;                        // ring row length = N * ports
     bool window_backend = false;           // delivery kernel 4 chosen before ng_prepare: spike window instead of a D-plane ring
@@ -861,6 +863,84 @@ int32_t ng_get_stats(ng_sim* s, ng_stats* out) {
     out->build_ms = s->build_ms; out->ms_update = s->ms_update; out->ms_deliver = s->ms_deliver;
     out->launches_update = s->launches_update; out->launches_deliver = s->launches_deliver; out->launches_other = s->launches_other;
     out->delivery_kernel = s->delivery_kernel;
+    return NG_OK;
+}
+
+int32_t ng_enable_statistics(ng_sim* s, int64_t start_step, int32_t bin_steps, int32_t sample_per_pop, int32_t max_bins) {
+    if (!s) return NG_ERR_INVALID_ARG;
+    if (!s->prepared) return fail(s, NG_ERR_STATE, "ng_enable_statistics before ng_prepare");
+    if (s->a.st_cnt) return fail(s, NG_ERR_STATE, "statistics are already enabled");
+    if (start_step < 0 || bin_steps < 1 || sample_per_pop < 0 || max_bins < 1 || max_bins > (1 << 24))
+        return fail(s, NG_ERR_INVALID_ARG, "start_step < 0, bin_steps < 1, sample_per_pop < 0 or max_bins outside 1..2^24");
+    NG_CUDA(s, cudaSetDevice(s->cfg.device));
+    const size_t N = (size_t)s->N;
+    // the sample of a population = its first sample_per_pop neurons (C27); slot = population * sample_per_pop + k
+    std::vector<int32_t> sample(N, -1);
+    for (size_t p = 0; p < s->pops.size(); ++p)
+        for (int k = 0; k < std::min(sample_per_pop, s->pops[p].n); ++k) sample[(size_t)s->pops[p].first + k] = (int32_t)(p * sample_per_pop + k);
+    const size_t slots = std::max<size_t>(1, s->pops.size() * (size_t)sample_per_pop);
+    uint16_t* bins = nullptr;
+    if (!(dev_alloc_t(s, &s->a.st_last, N) && dev_alloc_t(s, &s->a.st_cnt, N) && dev_alloc_t(s, &s->a.st_sum, N) &&
+          dev_alloc_t(s, &s->a.st_sumsq, N) && dev_alloc_t(s, &s->d_st_sample, N) && dev_alloc_t(s, &bins, slots * (size_t)max_bins))) {
+        s->a.st_cnt = nullptr;
+        return fail(s, NG_ERR_OOM, "device allocation failed (statistics)");
+    }
+    cudaStream_t st = s->stream;
+    NG_CUDA(s, cudaMemsetAsync(s->a.st_last, 0xFF, N * 4, st));           // -1: no spike yet
+    NG_CUDA(s, cudaMemsetAsync(s->a.st_cnt, 0, N * 4, st));
+    NG_CUDA(s, cudaMemsetAsync(s->a.st_sum, 0, N * 8, st));
+    NG_CUDA(s, cudaMemsetAsync(s->a.st_sumsq, 0, N * 8, st));
+    NG_CUDA(s, cudaMemsetAsync(bins, 0, slots * (size_t)max_bins * 2, st));
+    NG_CUDA(s, cudaMemcpyAsync(s->d_st_sample, sample.data(), N * 4, cudaMemcpyHostToDevice, st));
+    NG_CUDA(s, cudaStreamSynchronize(st));
+    s->a.st_sample = s->d_st_sample; s->a.st_bins = bins;
+    s->a.st_start = start_step; s->a.st_bin_steps = bin_steps; s->a.st_max_bins = max_bins;
+    s->st_sample_per_pop = sample_per_pop; s->st_slots = (int)slots;
+    destroy_graph(s);                                                   // the kernels' argument block changed
+    return NG_OK;
+}
+
+int32_t ng_get_rate_cv(ng_sim* s, float* rate_hz, float* cv_isi, int64_t count) {
+    if (!s || !rate_hz || !cv_isi) return NG_ERR_INVALID_ARG;
+    if (!s->prepared || !s->a.st_cnt) return fail(s, NG_ERR_STATE, "statistics are not enabled");
+    if (count != s->N) return fail(s, NG_ERR_INVALID_ARG, "count must be the number of neurons");
+    NG_CUDA(s, cudaSetDevice(s->cfg.device));
+    Ctl h{};
+    int32_t rc = read_ctl(s, &h);
+    if (rc) return rc;
+    const double T_s = (double)(h.step_u - s->a.st_start) * s->cfg.dt_ms * 1e-3;
+    if (!(T_s > 0.0)) return fail(s, NG_ERR_STATE, "no step after the statistics start step yet");
+    float *d_rate = nullptr, *d_cv = nullptr;
+    if (!(dev_alloc_t(s, &d_rate, (size_t)s->N) && dev_alloc_t(s, &d_cv, (size_t)s->N))) return fail(s, NG_ERR_OOM, "scratch");
+    stat_rate_cv_kernel<<<(s->N + 255) / 256, 256, 0, s->stream>>>(s->N, s->a.st_cnt, s->a.st_sum, s->a.st_sumsq, T_s, d_rate, d_cv);
+    NG_CUDA(s, cudaMemcpyAsync(rate_hz, d_rate, (size_t)s->N * 4, cudaMemcpyDefault, s->stream));
+    NG_CUDA(s, cudaMemcpyAsync(cv_isi, d_cv, (size_t)s->N * 4, cudaMemcpyDefault, s->stream));
+    NG_CUDA(s, cudaStreamSynchronize(s->stream));
+    dev_free(s, d_rate); dev_free(s, d_cv);
+    return NG_OK;
+}
+
+int32_t ng_get_correlations(ng_sim* s, int32_t population, float* corr, int64_t capacity, int32_t* n_sample_out, int32_t* n_bins_out) {
+    if (!s || !n_sample_out || !n_bins_out || capacity < 0) return NG_ERR_INVALID_ARG;
+    *n_sample_out = 0; *n_bins_out = 0;
+    if (!s->prepared || !s->a.st_cnt) return fail(s, NG_ERR_STATE, "statistics are not enabled");
+    if (population < 0 || population >= (int32_t)s->pops.size()) return fail(s, NG_ERR_INVALID_ARG, "population index");
+    NG_CUDA(s, cudaSetDevice(s->cfg.device));
+    Ctl h{};
+    int32_t rc = read_ctl(s, &h);
+    if (rc) return rc;
+    const int ns = std::min(s->st_sample_per_pop, s->pops[population].n);
+    const long long full = (h.step_u - s->a.st_start) / s->a.st_bin_steps;            // complete bins only
+    const int nb = (int)std::max<long long>(0, std::min<long long>(full, s->a.st_max_bins));
+    *n_sample_out = ns; *n_bins_out = nb;
+    if (!corr || capacity < (int64_t)ns * ns || ns == 0 || nb == 0) return NG_OK;
+    float* d_c = nullptr;
+    if (!dev_alloc_t(s, &d_c, (size_t)ns * ns)) return fail(s, NG_ERR_OOM, "scratch");
+    stat_corr_kernel<<<s->sm_count * 4, 256, 0, s->stream>>>(s->a.st_bins + (size_t)population * s->st_sample_per_pop * s->a.st_max_bins,
+                                                             ns, nb, s->a.st_max_bins, d_c);
+    NG_CUDA(s, cudaMemcpyAsync(corr, d_c, (size_t)ns * ns * 4, cudaMemcpyDefault, s->stream));
+    NG_CUDA(s, cudaStreamSynchronize(s->stream));
+    dev_free(s, d_c);
     return NG_OK;
 }
 

@@ -361,6 +361,11 @@ struct StepArgs {
     const RowInfo* row_info;     // [N]
     int32_t prefetch;            // 1: a spiking thread bulk-prefetches its row into L2 (row-walk kernels)
     uint8_t* pois_k;             // [N] Poisson counts of the next step (persistent pipelined kernel)
+    // on-device spike statistics, nullptr until ng_enable_statistics: accumulated by the thread that
+    // detects the spike — a neuron spikes at most once per step and always in one thread, so no atomics are needed
+    int32_t* st_last; int32_t* st_cnt; double* st_sum; double* st_sumsq;       // [N]: last spike step, spikes, sum ISI, sum ISI^2
+    const int32_t* st_sample; uint16_t* st_bins;                                // [N] sample slot or -1; [slots][st_max_bins] binned trains
+    long long st_start; int32_t st_bin_steps, st_max_bins;
     int32_t* win_id;             // spike-buffer backend (delivery kernel 4): circular log of the spikes of the last D steps
     long long win_cap;           //   its capacity in entries; nullptr / 0 for the ring backends
     unsigned long long* trace;   // NG_OPT_TRACE: [kTraceSteps][gridDim.x][kTraceStamps] %globaltimer stamps, or nullptr
@@ -374,6 +379,21 @@ struct StepArgs {
     int32_t max_row_chunks;      // ceil(longest padded row / kChunkRecords)
     int32_t mean_row_records;    // mean padded row length (>= 1): picks the item size of delivery kernel 1
 };
+
+// Spike statistics at spike time: per neuron the spike count and the first two moments of the
+// inter-spike interval (in steps, exact in fp64), and for the sampled neurons the spike train re-binned to st_bin_steps.
+__device__ __forceinline__ void stat_on_spike(const StepArgs& a, int i, long long n) {
+    if (!a.st_cnt || n < a.st_start) return;
+    const int last = a.st_last[i];
+    a.st_last[i] = (int)n;
+    a.st_cnt[i] += 1;
+    if (last >= 0) { const double isi = (double)((int)n - last); a.st_sum[i] += isi; a.st_sumsq[i] += isi * isi; }
+    const int slot = a.st_sample[i];
+    if (slot >= 0) {
+        const long long bin = (n - a.st_start) / a.st_bin_steps;
+        if (bin < a.st_max_bins) a.st_bins[(size_t)slot * a.st_max_bins + bin] += 1;
+    }
+}
 
 // The records of a spiking row are requested from DRAM the moment the spike is detected: by the time the delivery
 // phase (after the grid barrier / kernel boundary) asks for them they are L2 hits.  Pieces of at most 32 KB.
@@ -417,6 +437,7 @@ __device__ __forceinline__ void append_spike(const StepArgs& a, bool spk, int32_
         const unsigned long long pos = rec_base + (unsigned long long)idx;
         if (pos < (unsigned long long)a.rec_cap) { a.rec_id[pos] = id; a.rec_step[pos] = (int32_t)n; }
         if (a.win_id) a.win_id[(win_base + (unsigned long long)idx) % (unsigned long long)a.win_cap] = id;
+        stat_on_spike(a, id, n);
     }
 }
 
@@ -1044,6 +1065,7 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
                     }
                     lb = __shfl_sync(0xffffffffu, lb, leader);
                     if (spk) {
+                        stat_on_spike(a, i, n);
                         const int k = lb + __popc(m & ((1u << lane) - 1u));
                         if (k < kD1Cap) { sh.d1_r0[k] = r.r0; sh.d1_cnt[k] = r.d1; sh.d1_deg[k] = r.deg; sh.d1_id[k] = i; }
                         else {                                     // CTA list full: this lane does everything alone
@@ -1419,6 +1441,48 @@ __global__ void materialize_window_kernel(const StepArgs a, long long n, float* 
                 const int d = a.dly[r0 + q];
                 if (s + d >= n + 1) atomicAdd(out + (size_t)((s + d) % D) * a.NR + a.tgt[r0 + q], a.w[r0 + q]);
             }
+        }
+    }
+}
+
+// Statistics read-out.  rate = spikes / T; CV ISI = std / mean of the inter-spike intervals (population standard deviation,
+// PAPER.md:185), NaN with fewer than two intervals.
+__global__ void stat_rate_cv_kernel(int N, const int32_t* __restrict__ cnt, const double* __restrict__ sum,
+                                    const double* __restrict__ sumsq, double T_s, float* __restrict__ rate, float* __restrict__ cv) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const int c = cnt[i];
+    rate[i] = (float)((double)c / T_s);
+    const int m = c - 1;
+    float out = __int_as_float(0x7fc00000);
+    if (m >= 2) {
+        const double mean = sum[i] / m, var = sumsq[i] / m - mean * mean;
+        out = (float)(sqrt(var > 0.0 ? var : 0.0) / mean);
+    }
+    cv[i] = out;
+}
+// Pearson correlation of the binned trains of one population's sample:
+// C[i,j] = <b_i - mu_i, b_j - mu_j> / sqrt(<b_i - mu_i, b_i - mu_i> <b_j - mu_j, b_j - mu_j>).  One warp per pair.
+__global__ void stat_corr_kernel(const uint16_t* __restrict__ bins, int ns, int nb, int stride, float* __restrict__ C) {
+    const int lane = threadIdx.x & 31;
+    const long long gw = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = ((long long)gridDim.x * blockDim.x) >> 5;
+    for (long long pair = gw; pair < (long long)ns * ns; pair += nw) {
+        const int i = (int)(pair / ns), j = (int)(pair % ns);
+        const uint16_t* __restrict__ bi = bins + (size_t)i * stride;
+        const uint16_t* __restrict__ bj = bins + (size_t)j * stride;
+        double si = 0, sj = 0, sii = 0, sjj = 0, sij = 0;
+        for (int b = lane; b < nb; b += 32) {
+            const double x = bi[b], y = bj[b];
+            si += x; sj += y; sii += x * x; sjj += y * y; sij += x * y;
+        }
+        for (int o = 16; o > 0; o >>= 1) {
+            si += __shfl_xor_sync(0xffffffffu, si, o); sj += __shfl_xor_sync(0xffffffffu, sj, o);
+            sii += __shfl_xor_sync(0xffffffffu, sii, o); sjj += __shfl_xor_sync(0xffffffffu, sjj, o);
+            sij += __shfl_xor_sync(0xffffffffu, sij, o);
+        }
+        if (lane == 0) {
+            const double cov = sij - si * sj / nb, vi = sii - si * si / nb, vj = sjj - sj * sj / nb;
+            C[pair] = (vi > 0 && vj > 0) ? (float)(cov / sqrt(vi * vj)) : __int_as_float(0x7fc00000);
         }
     }
 }
