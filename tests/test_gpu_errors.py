@@ -1,0 +1,67 @@
+"""Error behaviour of the C-ABI on a device (include/ng.h states it per entry point): status codes instead of aborts,
+messages from ng_last_error, and a simulator that stays usable afterwards."""
+import numpy as np
+import pytest
+
+from paper_2007_14236_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2007_14236_b200 import binding
+    return binding
+
+
+def code(B, fn, *a, **k):
+    with pytest.raises(B.NgError) as e:
+        fn(*a, **k)
+    return e.value.code
+
+
+def test_argument_and_state_errors(B):
+    g = B.Sim(0.1, 20, 1)
+    assert code(B, g.prepare) == B.NG_ERR_STATE                                         # no population
+    assert code(B, g.create_population, 0, W.LIF | dict(poisson_rate_hz=0, poisson_weight=0)) == B.NG_ERR_INVALID_ARG
+    assert code(B, g.create_population, 10, W.LIF | dict(tau_syn=10.0)) == B.NG_ERR_INVALID_ARG    # tau_m == tau_syn (C19)
+    assert code(B, g.create_population, 10, W.LIF | dict(poisson_rate_hz=1e7)) == B.NG_ERR_INVALID_ARG   # Poisson table too short
+    first = g.create_population(100, W.LIF | dict(poisson_rate_hz=800.0, poisson_weight=87.8))
+    assert first == 0
+    assert code(B, g.connect_fixed_indegree, 0, 200, 0, 100, 5, ("const", 1.0), ("const", 1)) == B.NG_ERR_INVALID_ARG   # range
+    assert code(B, g.connect_fixed_indegree, 0, 100, 0, 100, 5, ("const", 1.0), ("const", 1), port=2) == B.NG_ERR_INVALID_ARG
+    assert code(B, g.get_state, B.FIELD_V) == B.NG_ERR_STATE                            # before prepare
+    assert code(B, g.set_option, B.OPT_STEP_MODE, 9) == B.NG_ERR_INVALID_ARG
+    g.connect_fixed_indegree(0, 100, 0, 100, 5, ("const", 50.0), ("uniform_int", 1, 20))
+    g.prepare()
+    assert code(B, g.connect_fixed_indegree, 0, 100, 0, 100, 5, ("const", 1.0), ("const", 1)) == B.NG_ERR_STATE         # after prepare
+    assert code(B, g.create_population, 5, W.LIF) == B.NG_ERR_STATE
+    assert code(B, g.set_state, B.FIELD_V, np.zeros(101, np.float32)) == B.NG_ERR_INVALID_ARG      # range outside the field
+    assert code(B, g.get_state, B.FIELD_LAST_INPUT) == B.NG_ERR_STATE                   # needs NG_DEBUG_INPUT
+    assert code(B, g.get_state, B.FIELD_ADEX_W) == B.NG_ERR_STATE                       # no AdEx population
+    assert code(B, g.rate_cv) == B.NG_ERR_STATE                                         # statistics not enabled
+    g.simulate(50)                                                                      # still usable
+    assert g.get_state(B.FIELD_STEP) == 50
+    g.close()
+
+
+def test_delay_beyond_ring_is_overflow(B):
+    g = B.Sim(0.1, 8, 1)
+    g.create_population(50, W.LIF | dict(poisson_rate_hz=0.0, poisson_weight=0.0))
+    g.connect_fixed_indegree(0, 50, 0, 50, 4, ("const", 1.0), ("uniform_int", 1, 9))    # 9 > ring_slots = 8
+    assert code(B, g.prepare) == B.NG_ERR_OVERFLOW
+    g.close()
+
+
+def test_spike_record_overflow_keeps_simulating(B):
+    wl = W.delivery_microbench(n=2000, K=10, fraction=0.5, n_steps=10, seed=3)
+    g = B.Sim(0.1, wl.ring_slots, wl.seed, record_spikes=True, max_recorded_spikes=1500)
+    wl.apply(g); g.prepare()
+    assert code(B, g.simulate, 5) == B.NG_ERR_OVERFLOW                                 # ~1000 spikes per step
+    st = g.stats()
+    assert st.steps == 5 and st.spikes > 3000 and st.recorded_dropped > 0
+    s, i = g.get_spikes()
+    assert s.size == 1500 and np.all(np.diff(s) >= 0)
+    g.simulate(2, allow_overflow=True)
+    assert g.get_state(B.FIELD_STEP) == 7 and g.stats().events == g.stats().spikes * 10
+    g.close()
