@@ -555,21 +555,33 @@ __device__ __forceinline__ bool adex_step(const AdexDev& p, AdexY& y, float& h_i
 
 // kAdex: the network holds AdEx populations (second receptor port, AdEx state arrays); LIF-only networks compile to
 // exactly the code without it.
+// neuron_load: every load of one neuron-step, issued together (one memory round trip).  Networks that need several
+// rounds per step (config 4) issue the loads of the next round before they compute the current one.
+struct NeuronLoad { float in, in1, V, I; int r, pi, kq; };
+
+template <bool kAdex>
+__device__ __forceinline__ NeuronLoad neuron_load(const StepArgs& a, const float* __restrict__ plane, int i, bool have_k) {
+    NeuronLoad L;
+    L.in = __ldcg(plane + i);                    // written by red.global from other SMs: read at L2
+    L.in1 = kAdex ? __ldcg(plane + a.N + i) : 0.f;          // inhibitory port
+    L.kq = have_k ? (int)a.pois_k[i] : 0xff;
+    L.V = 0.f; L.I = 0.f; L.r = 0; L.pi = 0;
+    if (!a.bypass) { L.V = a.V[i]; L.I = a.I[i]; L.r = a.refr[i]; L.pi = a.pop_of[i]; }
+    return L;
+}
+
 template <bool kAdex>
 __device__ __forceinline__ bool neuron_early(const StepArgs& a, const PopDev* __restrict__ P, long long n, int i,
-                                             float* __restrict__ plane, NeuronRegs& g, bool have_k = false) {
-    g.in = __ldcg(plane + i);                    // written by red.global from other SMs: read at L2
-    g.kq = have_k ? (int)a.pois_k[i] : 0xff;
-    g.adex = false;
-    if (kAdex) g.in1 = __ldcg(plane + a.N + i);  // inhibitory port
+                                             NeuronRegs& g, const NeuronLoad& L) {
+    g.in = L.in; g.in1 = L.in1; g.kq = L.kq; g.adex = false;
     if (a.bypass) {                                          // DESIGN.md C8: delivery-only mode
         const uint4 x = philox4x32_10(a.seed_lo, a.seed_hi, (uint32_t)i, (uint32_t)n, (uint32_t)(n >> 32), kTagInject);
         return x.x < a.inject_thr;
     }
-    float V = a.V[i];
-    g.I = a.I[i];
-    int r = a.refr[i];
-    g.pi = a.pop_of[i];
+    float V = L.V;
+    g.I = L.I;
+    int r = L.r;
+    g.pi = L.pi;
     const PopDev* __restrict__ p = P + g.pi;
     if (kAdex && p->model == 1) {                // AdEx: the whole step is integrated here; neuron_late applies the jumps
         g.adex = true;
@@ -616,7 +628,9 @@ __device__ __forceinline__ void update_phase(const StepArgs& a, const PopDev* __
     for (long long ii = gtid; ii < n_round; ii += gthreads) {
         const int i = (int)ii;
         NeuronRegs g;
-        const bool spk = i < N && neuron_early<kAdex>(a, P, n, i, plane, g);
+        NeuronLoad L;
+        if (i < N) L = neuron_load<kAdex>(a, plane, i, false);
+        const bool spk = i < N && neuron_early<kAdex>(a, P, n, i, g, L);
         append_spike(a, spk, i, n, rec_base, win_base);
         if (i < N) neuron_late<kAdex>(a, P, n, i, plane, g);
     }
@@ -1041,17 +1055,22 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
             float* __restrict__ plane = a.ring + (size_t)slot * a.NR;
             float* __restrict__ plane1 = a.ring + (size_t)(slot + 1 == Dr ? 0 : slot + 1) * a.NR;
             const bool single_round = (long long)gridDim.x * U >= N;
-            for (long long base = (long long)blockIdx.x * U; base < N; base += (long long)gridDim.x * U) {
+            const long long stride = (long long)gridDim.x * U;
+            NeuronLoad L, Ln;
+            if (!kAdex) { const long long i0 = (long long)blockIdx.x * U + threadIdx.x; if (i0 < N) L = neuron_load<kAdex>(a, plane, (int)i0, have_k); }
+            for (long long base = (long long)blockIdx.x * U; base < N; base += stride) {
                 const long long ii = base + threadIdx.x;
                 const int i = (int)ii;
                 NeuronRegs g;
+                if (kAdex) { if (ii < N) L = neuron_load<kAdex>(a, plane, i, have_k); }
+                else if (ii + stride < N) Ln = neuron_load<kAdex>(a, plane, (int)(ii + stride), have_k);   // next round's loads in flight
                 // the row descriptor is fetched for EVERY neuron together with its state (16 B, L2-resident because it
                 // is touched every step): a spiking thread then needs no further memory round trip
                 // (only while one round covers the network: for large N the extra 16 B per neuron-step costs more
                 // bandwidth than the round trip of the few spiking threads)
                 RowInfo r;
                 if (single_round && ii < N) r = ld_row_info(a.row_info + i);
-                const bool spk = ii < N && neuron_early<kAdex>(a, P, n, i, plane, g, have_k);
+                const bool spk = ii < N && neuron_early<kAdex>(a, P, n, i, g, L);
                 if (!single_round && spk) r = ld_row_info(a.row_info + i);
                 const unsigned m = __ballot_sync(0xffffffffu, spk);
                 if (m) {                                           // warp-aggregated append to the CTA's own list
@@ -1078,6 +1097,7 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
                     }
                 }
                 if (ii < N) neuron_late<kAdex>(a, P, n, i, plane, g);
+                if (!kAdex) L = Ln;
             }
             trace_stamp(a, n, 3);
             group_sync(1, U);
@@ -1087,7 +1107,7 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
             // delay-1 pass (nothing on the critical path needs the global index)
             int gbase = 0;
             if (threadIdx.x == 0 && nd1 > 0) gbase = atomicAdd(&a.ctl->spike_cnt[n & 3], nd1);
-            if (nd1 <= 8) {                                        // latency regime: a few spikes, 32 records per warp
+            if (nd1 <= 2) {                                        // latency regime: one or two spikes, 32 records per warp
                 for (int s = 0; s < nd1; ++s) {
                     const long long r0 = sh.d1_r0[s];
                     const int cnt = sh.d1_cnt[s];
