@@ -57,7 +57,7 @@ struct ng_sim {
     int persistent_threads = kPersistentThreads;
     // statistics (ng_enable_statistics)
     int32_t* d_st_sample = nullptr; int st_sample_per_pop = 0; int st_slots = 0;
-    bool adex_two_pass_step = false, adex_two_pass_persistent = false;   // AdEx network covered in one round of updater threads
+    bool one_round_step = false, one_round_persistent = false;   // the network is covered in one round of updater threads
     bool has_adex = false;                 // any AdEx population: two receptor ports, AdEx state arrays, <true> kernels
     int64_t NR = 0;                        // ring row length = N * ports
     bool window_backend = false;           // delivery kernel 4 chosen before ng_prepare: spike window instead of a D-plane ring
@@ -179,9 +179,10 @@ void launch_deliver(ng_sim* s) {
 
 // one time step: two kernels (update, deliver) or the pipelined step kernel
 void launch_pipe(ng_sim* s) {
-    if (s->has_adex && s->adex_two_pass_step) pipe_step_kernel<true, true, true><<<s->pipe_blocks, kPipeThreads, 0, s->stream>>>(s->a);
-    else if (s->has_adex) pipe_step_kernel<true, true><<<s->pipe_blocks, kPipeThreads, 0, s->stream>>>(s->a);
-    else pipe_step_kernel<true, false><<<s->pipe_blocks, kPipeThreads, 0, s->stream>>>(s->a);
+    if (s->has_adex && s->one_round_step) pipe_step_kernel<true, true, true><<<s->pipe_blocks, kPipeThreads, 0, s->stream>>>(s->a);
+    else if (s->has_adex) pipe_step_kernel<true, true, false><<<s->pipe_blocks, kPipeThreads, 0, s->stream>>>(s->a);
+    else if (s->one_round_step) pipe_step_kernel<true, false, true><<<s->pipe_blocks, kPipeThreads, 0, s->stream>>>(s->a);
+    else pipe_step_kernel<true, false, false><<<s->pipe_blocks, kPipeThreads, 0, s->stream>>>(s->a);
 }
 // rest pass of the last step of an ng_simulate call (delivery kernel 4): leaves nothing pending between API calls
 void launch_pipe_flush(ng_sim* s) {
@@ -215,13 +216,13 @@ void configure_launch(ng_sim* s) {
     {
         int occp = 0;
         const int pt = s->has_adex ? 512 : s->persistent_threads;      // AdEx kernels are compiled for 512-thread CTAs
-        if (s->has_adex) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occp, persistent_pipe_kernel<true>, pt, 0);
-        else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occp, persistent_pipe_kernel<false>, pt, 0);
+        if (s->has_adex) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occp, persistent_pipe_kernel<true, false>, pt, 0);
+        else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occp, persistent_pipe_kernel<false, false>, pt, 0);
         if (occp < 1) occp = 1;
         s->persistent_pipe_blocks = sm * std::min(occp, kPersistentThreads / pt);
         // updater threads per CTA of the AdEx kernels: all but four warps (pipe_updater_threads in ng_device.cuh)
-        s->adex_two_pass_persistent = s->has_adex && (long long)s->persistent_pipe_blocks * (512 - 128) >= s->N;
-        s->adex_two_pass_step = s->has_adex && (long long)s->pipe_blocks * (kPipeThreads - 128) >= s->N;
+        s->one_round_persistent = (long long)s->persistent_pipe_blocks * (pt - (s->has_adex ? 128 : (pt >= 512 ? kEntryTile : 64))) >= s->N;
+        s->one_round_step = (long long)s->pipe_blocks * (kPipeThreads - (s->has_adex ? 128 : kEntryTile)) >= s->N;
     }
     int blocks = s->deliver_blocks_opt;
     if (blocks <= 0) {
@@ -715,9 +716,10 @@ int32_t ng_simulate(ng_sim* s, int64_t n_steps) {
         NG_CUDA(s, cudaMemsetAsync(&s->d_ctl->bar, 0, sizeof(unsigned long long), st));
         s->last_persistent_blocks = s->delivery_kernel == 3 ? s->persistent_pipe_blocks : s->persistent_blocks;
         if (s->delivery_kernel == 3) {
-            const void* fn = s->has_adex ? (s->adex_two_pass_persistent ? (const void*)persistent_pipe_kernel<true, true>
-                                                                         : (const void*)persistent_pipe_kernel<true>)
-                                         : (const void*)persistent_pipe_kernel<false>;
+            const void* fn = s->has_adex ? (s->one_round_persistent ? (const void*)persistent_pipe_kernel<true, true>
+                                                                     : (const void*)persistent_pipe_kernel<true, false>)
+                                         : (s->one_round_persistent ? (const void*)persistent_pipe_kernel<false, true>
+                                                                    : (const void*)persistent_pipe_kernel<false, false>);
             NG_CUDA(s, cudaLaunchCooperativeKernel(fn, dim3(s->persistent_pipe_blocks),
                                                    dim3(s->has_adex ? 512 : s->persistent_threads), args, 0, st));
         } else {

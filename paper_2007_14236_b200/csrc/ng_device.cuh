@@ -1048,6 +1048,32 @@ __device__ __forceinline__ void deliver_d1_piece(const StepArgs& a, float* __res
 __device__ __forceinline__ void group_sync(int id, int count) {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory");
 }
+// Delay-1 pass for many spikes per CTA: (spike, record) pairs flattened over the updater threads.
+__device__ __noinline__ void d1_flat_pass(const StepArgs& a, PipeShared& sh, float* __restrict__ plane1, int nd1, int U) {
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    if (wib == 0) {
+        int carry = 0;
+        for (int base = 0; base < nd1; base += 32) {
+            int x = base + lane < nd1 ? sh.d1_cnt[base + lane] : 0;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int y = __shfl_up_sync(0xffffffffu, x, o);
+                if (lane >= o) x += y;
+            }
+            sh.d1_pre[base + lane + 1] = carry + x;
+            carry += __shfl_sync(0xffffffffu, x, 31);
+        }
+        if (lane == 0) sh.d1_pre[0] = 0;
+    }
+    group_sync(1, U);
+    const int T = sh.d1_pre[nd1];
+    for (int f = threadIdx.x; f < T; f += U) {
+        int lo = 0, hi = nd1;                          // largest s with d1_pre[s] <= f
+        while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (sh.d1_pre[mid] <= f) lo = mid; else hi = mid; }
+        deliver_d1_piece(a, plane1, sh.d1_r0[lo], sh.d1_cnt[lo], f - sh.d1_pre[lo]);
+    }
+}
+
 // item `it` of the staged tile: find its entry (number of k in [1, m] with pre[k] <= it) and deliver its chunk
 __device__ __forceinline__ void pipe_one_item(const StepArgs& a, int nmod, PipeShared& sh, int m, int it, bool small, int lane) {
     int sidx = 0;
@@ -1070,10 +1096,13 @@ __device__ __forceinline__ int pipe_updater_threads(int N, bool heavy_update) {
     return (int)per_cta <= cap ? max(need, 32) : cap;
 }
 
-// kTwoPass (AdEx networks covered in one round): one integration attempt per lane, the unfinished neurons in a second,
-// dense pass (10^5 neurons: 33 -> 19 us per step).  With many rounds per step the update is bound by its memory round
-// trips and the second pass only adds register pressure and traffic, so every lane finishes in place there.
-template <bool kUpdate, bool kAdex, bool kTwoPass = false>
+// kOneRound: one round of updater threads covers the network (the host knows the grid: one neuron per thread).  The
+// kernel is then compiled without the multi-round machinery (loads of the next round in flight) and with the row
+// descriptor fetched speculatively for every neuron; AdEx networks additionally use the two-pass update: one
+// integration attempt per lane, the unfinished neurons in a second, dense pass (10^5 neurons: 33 -> 19 us per step).
+// With many rounds per step the update is bound by its memory round trips and the second pass only adds register
+// pressure and traffic, so every lane finishes in place there.
+template <bool kUpdate, bool kAdex, bool kOneRound = false>
 __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* __restrict__ P, long long n, int slot, bool pending,
                                                unsigned long long rec_prev, PipeShared& sh, bool have_k = false) {
     const int N = a.N, Dr = a.Dr;
@@ -1091,7 +1120,7 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
             const int wib = threadIdx.x >> 5, wpu = U >> 5;
             float* __restrict__ plane = a.ring + (size_t)slot * a.NR;
             float* __restrict__ plane1 = a.ring + (size_t)(slot + 1 == Dr ? 0 : slot + 1) * a.NR;
-            const bool single_round = (long long)gridDim.x * U >= N;
+            const bool single_round = kOneRound;
             const long long stride = (long long)gridDim.x * U;
             NeuronLoad L, Ln;
             if (!kAdex) { const long long i0 = (long long)blockIdx.x * U + threadIdx.x; if (i0 < N) L = neuron_load<kAdex>(a, plane, (int)i0, have_k); }
@@ -1100,15 +1129,15 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
                 const int i = (int)ii;
                 NeuronRegs g;
                 if (kAdex) { if (ii < N) L = neuron_load<kAdex>(a, plane, i, have_k); }
-                else if (ii + stride < N) Ln = neuron_load<kAdex>(a, plane, (int)(ii + stride), have_k);   // next round's loads in flight
+                else if (!kOneRound && ii + stride < N) Ln = neuron_load<kAdex>(a, plane, (int)(ii + stride), have_k);   // next round's loads in flight
                 // the row descriptor is fetched for EVERY neuron together with its state (16 B, L2-resident because it
                 // is touched every step): a spiking thread then needs no further memory round trip
                 // (only while one round covers the network: for large N the extra 16 B per neuron-step costs more
                 // bandwidth than the round trip of the few spiking threads)
                 RowInfo r;
                 if (single_round && ii < N) r = ld_row_info(a.row_info + i);
-                bool spk = ii < N && neuron_early<kAdex, kAdex && kTwoPass>(a, P, n, i, g, L);
-                if (kAdex && kTwoPass && ii < N && g.pending) {            // first attempt did not finish: second pass, dense warps
+                bool spk = ii < N && neuron_early<kAdex, kAdex && kOneRound>(a, P, n, i, g, L);
+                if (kAdex && kOneRound && ii < N && g.pending) {            // first attempt did not finish: second pass, dense warps
                     const int ks = atomicAdd(&sh.n_slow, 1);
                     if (ks < kSlowCap) { sh.slow_id[ks] = i | (g.spiked ? (1 << 30) : 0); sh.slow_t[ks] = g.t; }
                     else { spk = adex_resume(a, P, n, i, g.t, g.spiked, plane); g.pending = false; g.adex = false; g.pi = -1; }
@@ -1138,10 +1167,10 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
                         }
                     }
                 }
-                if (ii < N && !(kAdex && kTwoPass && (g.pending || g.pi < 0))) neuron_late<kAdex>(a, P, n, i, plane, g);
-                if (!kAdex) L = Ln;
+                if (ii < N && !(kAdex && kOneRound && (g.pending || g.pi < 0))) neuron_late<kAdex>(a, P, n, i, plane, g);
+                if (!kAdex && !kOneRound) L = Ln;
             }
-            if (kAdex && kTwoPass) {                               // second pass over the CTA's slow neurons
+            if (kAdex && kOneRound) {                               // second pass over the CTA's slow neurons
                 group_sync(1, U);
                 const int ns = min(sh.n_slow, kSlowCap);
                 for (int s = threadIdx.x; s < ns; s += U) {
@@ -1180,29 +1209,7 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
                     const int cnt = sh.d1_cnt[s];
                     for (int q = wib * 32 + lane; q < cnt; q += wpu * 32) deliver_d1_piece(a, plane1, r0, cnt, q);
                 }
-            } else {                                               // many spikes: flatten (spike, record) over the updaters
-                if (wib == 0) {
-                    int carry = 0;
-                    for (int base = 0; base < nd1; base += 32) {
-                        int x = base + lane < nd1 ? sh.d1_cnt[base + lane] : 0;
-#pragma unroll
-                        for (int o = 1; o < 32; o <<= 1) {
-                            const int y = __shfl_up_sync(0xffffffffu, x, o);
-                            if (lane >= o) x += y;
-                        }
-                        sh.d1_pre[base + lane + 1] = carry + x;
-                        carry += __shfl_sync(0xffffffffu, x, 31);
-                    }
-                    if (lane == 0) sh.d1_pre[0] = 0;
-                }
-                group_sync(1, U);
-                const int T = sh.d1_pre[nd1];
-                for (int f = threadIdx.x; f < T; f += U) {
-                    int lo = 0, hi = nd1;                          // largest s with d1_pre[s] <= f
-                    while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (sh.d1_pre[mid] <= f) lo = mid; else hi = mid; }
-                    deliver_d1_piece(a, plane1, sh.d1_r0[lo], sh.d1_cnt[lo], f - sh.d1_pre[lo]);
-                }
-            }
+            } else d1_flat_pass(a, sh, plane1, nd1, U);           // many spikes: out of line, off the latency path
             trace_stamp(a, n, 6);
             if (nd1 > 0) {                                         // uniform over the updater group
                 if (threadIdx.x == 0) sh.gbase = gbase;
@@ -1304,7 +1311,7 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
 // Graph / plain-launch form: one launch per time step, the kernel boundary is the barrier.  The last CTA to finish
 // publishes the next step index (a4) and marks the rest pass of this step as pending.
 constexpr int kPipeThreads = 512;        // 256 updaters + 256 rest-pass threads
-template <bool kUpdate, bool kAdex, bool kTwoPass = false>
+template <bool kUpdate, bool kAdex, bool kOneRound = false>
 __global__ void __launch_bounds__(kPipeThreads) pipe_step_kernel(const StepArgs a) {
     __shared__ PipeShared sh;
     if (threadIdx.x == 0) {
@@ -1317,7 +1324,7 @@ __global__ void __launch_bounds__(kPipeThreads) pipe_step_kernel(const StepArgs 
     if (a.n_pops > kMaxPopsSmem) __syncthreads();
     const long long n = sh.sc.n;
     const int slot = sh.sc.slot;
-    pipelined_phase<kUpdate, kAdex, kTwoPass>(a, P, n, slot, sh.pending != 0, sh.sc.rec_base, sh);
+    pipelined_phase<kUpdate, kAdex, kOneRound>(a, P, n, slot, sh.pending != 0, sh.sc.rec_base, sh);
     if (threadIdx.x == 0) {
         __threadfence();
         const unsigned t = atomicAdd(&a.ctl->ticket, 1u);
@@ -1339,7 +1346,7 @@ __global__ void __launch_bounds__(kPipeThreads) pipe_step_kernel(const StepArgs 
 }
 
 // kAdex: the AdEx integrator needs more than the 64 registers a 1024-thread CTA leaves: 512-thread CTAs, two per SM at most
-template <bool kAdex, bool kTwoPass = false>
+template <bool kAdex, bool kOneRound = false>
 __global__ void __launch_bounds__(kAdex ? 512 : kPersistentThreads, kAdex ? 2 : 1) persistent_pipe_kernel(const StepArgs a, long long n_steps) {
     __shared__ PipeShared sh;
     if (threadIdx.x == 0) {
@@ -1351,14 +1358,14 @@ __global__ void __launch_bounds__(kAdex ? 512 : kPersistentThreads, kAdex ? 2 : 
     if (a.n_pops > kMaxPopsSmem) __syncthreads();
     const long long gtid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const int U = pipe_updater_threads(a.N, kAdex);
-    const bool single_round = (long long)gridDim.x * U >= a.N;     // else the counts are computed in line, overlapping the loads
+    const bool single_round = kOneRound;                           // else the counts are computed in line, overlapping the loads
     long long n = sh.sc.n;
     int slot = sh.sc.slot;
     unsigned long long rec_prev = sh.sc.rec_base, spikes = 0, epoch = 0;       // recorded before step n-1 (nothing pending at entry)
     for (long long s = 0; s < n_steps; ++s, ++n) {
         if (gtid == 0) a.ctl->spike_cnt[(n + 1) & 3] = 0;          // last read (as step n-3's) in phase n-2
         trace_stamp(a, n, 0);
-        const int Mp = pipelined_phase<true, kAdex, kTwoPass>(a, P, n, slot, s > 0, rec_prev, sh, s > 0 && single_round);
+        const int Mp = pipelined_phase<true, kAdex, kOneRound>(a, P, n, slot, s > 0, rec_prev, sh, s > 0 && single_round);
         rec_prev += (unsigned long long)Mp; spikes += (unsigned long long)Mp;
         trace_stamp(a, n, 1);
         grid_arrive(a.ctl, epoch);
