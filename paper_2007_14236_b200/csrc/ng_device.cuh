@@ -48,25 +48,33 @@ struct PopDev {                // per-population constants of the update (fp32 c
     AdexDev ax;
 };
 
-struct Ctl {                   // device-resident control block; see ng.cu for the update/deliver handshake
-    long long step_u;                      // written by deliver, read by update: index of the next step
+// Device-resident control block; see ng.cu for the update/deliver handshake.  Words with different traffic live on
+// different 128-byte lines: the barrier counter is polled by every CTA while late CTAs still append spikes
+// (atomics on spike_cnt) and count events — on one line those requests queue at the same L2 slice.
+struct Ctl {
+    // line 0: step bookkeeping, written once per step by one thread
+    alignas(128) long long step_u;         // written by deliver, read by update: index of the next step
     long long step_d;                      // written by update, read by deliver: index of the step being delivered
-    int32_t spike_cnt[4];                  // length of the spike array of step n, indexed n & 3 (the list itself by n & 1)
     unsigned long long rec_total[2];       // spikes recorded before step of this parity
-    unsigned long long spikes, events;
+    unsigned long long spikes;
     int32_t err_delay;                     // builder: a drawn delay fell outside [1, D]
     int32_t max_row_records;               // builder: longest padded row
     unsigned long long n_padded;           // builder: total records stored
-    unsigned int ticket;                   // fused / pipelined step kernels: CTAs that finished the current step
     int32_t pending;                       // pipelined step kernel: the rest pass of step step_u - 1 is outstanding
     int32_t slot;                          // step_u mod Dr, kept next to step_u so no kernel divides 64-bit integers
     int32_t slot_d;                        // step_d mod Dr: written by update, read by deliver (like step_d) — the delivery
                                            // kernel's bookkeeping advances `slot` while later CTAs of the same launch still start
-    unsigned long long bar;                // persistent kernels: arrivals at the grid barrier
     int32_t err_window;                    // spike-buffer backend: the spike window overflowed its capacity
-    int32_t pad2;
-    unsigned long long win_start[kMaxWindowSteps + 1];   // spike-buffer backend: absolute position in the spike window of
-                                           // the first spike of step s, at index s mod (D+1); [s+1] = its end
+    // line 1: spike counters (atomics of the appending warps / CTAs)
+    alignas(128) int32_t spike_cnt[4];     // length of the spike array of step n, indexed n & 3 (the list itself by n & 1)
+    // line 2: event counter (one atomic per CTA and step)
+    alignas(128) unsigned long long events;
+    // line 3: grid barrier of the persistent kernels, and the ticket of the stand-alone pipelined kernel
+    alignas(128) unsigned long long bar;   // arrivals at the grid barrier
+    unsigned int ticket;                   // CTAs that finished the current step
+    // line 4 ..: spike-buffer backend
+    alignas(128) unsigned long long win_start[kMaxWindowSteps + 1];   // absolute position in the spike window of the first
+                                           // spike of step s, at index s mod (D+1); [s+1] = its end
 };
 
 // ---------------------------------------------------------------------------------------
