@@ -1211,6 +1211,13 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
             // delay-1 pass (nothing on the critical path needs the global index)
             int gbase = 0;
             if (threadIdx.x == 0 && nd1 > 0) gbase = atomicAdd(&a.ctl->spike_cnt[n & 3], nd1);
+            // the rest of the spiking rows is read one phase later: request it now, from the LAST updater threads, so
+            // that issuing the bulk prefetches overlaps the delay-1 pass of the first warps instead of following it
+            if (a.prefetch)
+                for (int s = U - 1 - (int)threadIdx.x; s < nd1; s += U) {
+                    RowInfo r; r.r0 = sh.d1_r0[s]; r.d1 = sh.d1_cnt[s]; r.deg = sh.d1_deg[s];
+                    prefetch_row(a, r);
+                }
             if (nd1 <= 2) {                                        // latency regime: one or two spikes, 32 records per warp
                 for (int s = 0; s < nd1; ++s) {
                     const long long r0 = sh.d1_r0[s];
@@ -1228,7 +1235,6 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
                     const size_t gk = (size_t)(n & 1) * N + gb + s;
                     a.spike_list[gk] = sh.d1_id[s];
                     st_row_info(a.spike_row + gk, r);
-                    if (a.prefetch) prefetch_row(a, r);
                 }
             }
         }
