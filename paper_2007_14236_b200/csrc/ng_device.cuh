@@ -752,6 +752,13 @@ __device__ __forceinline__ void deliver_item(const StepArgs& a, int nmod, long l
         if (t.y >= 0 && q + 1 >= skip) { s = nmod + (int)((dd >> 8) & 0xff); if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * a.NR + t.y, ww.y); }
         if (t.z >= 0 && q + 2 >= skip) { s = nmod + (int)((dd >> 16) & 0xff); if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * a.NR + t.z, ww.z); }
         if (t.w >= 0 && q + 3 >= skip) { s = nmod + (int)(dd >> 24); if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * a.NR + t.w, ww.w); }
+    } else if (kPerLane == 2) {
+        int2 t; float2 ww; uint32_t dd;
+        asm("ld.global.nc.L1::no_allocate.v2.s32 {%0,%1}, [%2];" : "=r"(t.x), "=r"(t.y) : "l"(a.tgt + p));
+        asm("ld.global.nc.L1::no_allocate.v2.f32 {%0,%1}, [%2];" : "=f"(ww.x), "=f"(ww.y) : "l"(a.w + p));
+        asm("ld.global.nc.L1::no_allocate.u16 %0, [%1];" : "=r"(dd) : "l"(a.dly + p));
+        if (t.x >= 0 && q >= skip) { s = nmod + (int)(dd & 0xff); if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * a.NR + t.x, ww.x); }
+        if (t.y >= 0 && q + 1 >= skip) { s = nmod + (int)(dd >> 8); if (s >= Dr) s -= Dr; red_add_f32(a.ring + (size_t)s * a.NR + t.y, ww.y); }
     } else {
         int t; float ww; uint32_t dd;
         asm("ld.global.nc.L1::no_allocate.s32 %0, [%1];" : "=r"(t) : "l"(a.tgt + p));
@@ -1083,7 +1090,7 @@ __device__ __noinline__ void d1_flat_pass(const StepArgs& a, PipeShared& sh, flo
 }
 
 // item `it` of the staged tile: find its entry (number of k in [1, m] with pre[k] <= it) and deliver its chunk
-__device__ __forceinline__ void pipe_one_item(const StepArgs& a, int nmod, PipeShared& sh, int m, int it, bool small, int lane) {
+__device__ __forceinline__ void pipe_one_item(const StepArgs& a, int nmod, PipeShared& sh, int m, int it, int cshift, int lane) {
     int sidx = 0;
     for (int j = 0; j < m; j += 32) {
         const int k = j + lane + 1;
@@ -1091,7 +1098,8 @@ __device__ __forceinline__ void pipe_one_item(const StepArgs& a, int nmod, PipeS
         sidx += __popc(__ballot_sync(0xffffffffu, v <= it));
     }
     const int c = it - sh.d.pre[sidx];
-    if (small) deliver_item<1>(a, nmod, sh.d.r0[sidx], sh.d.len[sidx], c, lane, sh.skip[sidx]);
+    if (cshift == 5) deliver_item<1>(a, nmod, sh.d.r0[sidx], sh.d.len[sidx], c, lane, sh.skip[sidx]);
+    else if (cshift == 6) deliver_item<2>(a, nmod, sh.d.r0[sidx], sh.d.len[sidx], c, lane, sh.skip[sidx]);
     else deliver_item<4>(a, nmod, sh.d.r0[sidx], sh.d.len[sidx], c, lane, sh.skip[sidx]);
 }
 // Updaters per CTA: just enough for one neuron per thread when the network is small enough for a single round
@@ -1257,8 +1265,10 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
         trace_stamp(a, n, 7, U);
         const int M = sh.d.M;
         const int gwarp = blockIdx.x * wpr + wir, gwarps = gridDim.x * wpr;      // items are dealt to the rest warps of the grid
-        const bool small = (long long)M * a.mean_row_records <= 64LL * gwarps;
-        const int cshift = small ? 5 : 7;
+        // item size: the smallest of 32 / 64 / 128 records with about one item per rest warp or fewer — a warp's items
+        // are serial (every scattered red holds it for an L2 round trip), so the phase ends with the warp that has most
+        const long long est = (long long)M * a.mean_row_records;
+        const int cshift = est <= 32LL * gwarps ? 5 : est <= 64LL * gwarps ? 6 : 7;
         unsigned long long ev = 0;
         int base_mod = 0;
         // many spikes (>= 8 per CTA): every CTA stages only its own tiles and deals their items to its own rest warps
@@ -1312,7 +1322,7 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
             const int total = sh.d.pre[m];
             int first = gw - base_mod;                             // items are numbered across tiles: round-robin deal
             if (first < 0) first += gw_n;
-            for (int it = first; it < total; it += gw_n) pipe_one_item(a, nmod_prev, sh, m, it, small, lane);
+            for (int it = first; it < total; it += gw_n) pipe_one_item(a, nmod_prev, sh, m, it, cshift, lane);
             base_mod = (int)(((long long)base_mod + total) % gw_n);
         }
         trace_stamp(a, n, 9, U);
