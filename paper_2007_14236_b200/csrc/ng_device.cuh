@@ -1217,8 +1217,9 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
             const int nd1 = min(sh.n_d1, kD1Cap);
             // one atomic per CTA reserves the CTA's slots in the global spike array; its round trip overlaps the
             // delay-1 pass (nothing on the critical path needs the global index)
-            int gbase = 0;
-            if (threadIdx.x == 0 && nd1 > 0) gbase = atomicAdd(&a.ctl->spike_cnt[n & 3], nd1);
+            // (issued by the LAST updater thread, whose warp has no delay-1 records unless a row has thousands: on the
+            // first warps the atomic's round trip was measured in front of the record loads, 0.4 us)
+            if ((int)threadIdx.x == U - 1 && nd1 > 0) sh.gbase = atomicAdd(&a.ctl->spike_cnt[n & 3], nd1);
             // the rest of the spiking rows is read one phase later: request it now, from the LAST updater threads, so
             // that issuing the bulk prefetches overlaps the delay-1 pass of the first warps instead of following it
             if (a.prefetch)
@@ -1235,7 +1236,6 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
             } else d1_flat_pass(a, sh, plane1, nd1, U);           // many spikes: out of line, off the latency path
             trace_stamp(a, n, 6);
             if (nd1 > 0) {                                         // uniform over the updater group
-                if (threadIdx.x == 0) sh.gbase = gbase;
                 group_sync(1, U);
                 const int gb = sh.gbase;
                 for (int s = threadIdx.x; s < nd1; s += U) {       // a2: global spike array; the rest of the row is read
