@@ -718,7 +718,7 @@ int32_t ng_simulate(ng_sim* s, int64_t n_steps) {
         if (s->delivery_kernel == 3) {
             const void* fn = s->has_adex ? (s->one_round_persistent ? (const void*)persistent_pipe_kernel<true, true>
                                                                      : (const void*)persistent_pipe_kernel<true, false>)
-                                         : (s->one_round_persistent ? (const void*)persistent_pipe_kernel<false, true>
+                                         : (s->one_round_persistent && !s->bypass ? (const void*)persistent_pipe_kernel<false, true>
                                                                     : (const void*)persistent_pipe_kernel<false, false>);
             NG_CUDA(s, cudaLaunchCooperativeKernel(fn, dim3(s->persistent_pipe_blocks),
                                                    dim3(s->has_adex ? 512 : s->persistent_threads), args, 0, st));

@@ -1028,7 +1028,8 @@ constexpr int kPersistentThreads = 1024;
 //   writes plane n+1, the rest pass of step n-1 writes planes n+1 .. n-1+D (Dr = D + 1 planes).
 //   The spike record of step n-1 is written by CTA 0 during the rest pass (coalesced, off the critical path).
 // ---------------------------------------------------------------------------------------
-constexpr int kD1Cap = 1024;
+constexpr int kD1Cap = 256;
+constexpr int kResCap = 768;             // updater threads of a 1024-thread CTA at most (pipe_updater_threads)
 constexpr int kSlowCap = 512;
 struct PipeShared {
     PopDev pops[kMaxPopsSmem];
@@ -1041,8 +1042,15 @@ struct PipeShared {
     int32_t d1_pre[kD1Cap + 32];
     int32_t slow_id[kSlowCap];             // AdEx neurons whose first integration attempt did not finish the step
     float slow_t[kSlowCap];                //   (bit 30 of the id: already spiked), and the time they reached
+    // LIF state of the CTA's neurons, resident for a whole persistent launch when one round of updater threads covers
+    // the network (thread t owns neuron blockIdx.x * U + t): read from global memory at entry, written back at exit
+    float res_V[kResCap];
+    float res_I[kResCap];
+    int32_t res_r[kResCap];
+    alignas(16) RowInfo res_row[kResCap];
+    uint8_t res_pi[kResCap];
+    uint8_t res_kq[kResCap];               // Poisson count of the next step (barrier shadow)
     int32_t n_slow;
-    int32_t gbase;
     int32_t n_d1;
     StepScalars sc;
     int32_t pending;
@@ -1118,7 +1126,7 @@ __device__ __forceinline__ int pipe_updater_threads(int N, bool heavy_update) {
 // integration attempt per lane, the unfinished neurons in a second, dense pass (10^5 neurons: 33 -> 19 us per step).
 // With many rounds per step the update is bound by its memory round trips and the second pass only adds register
 // pressure and traffic, so every lane finishes in place there.
-template <bool kUpdate, bool kAdex, bool kOneRound = false>
+template <bool kUpdate, bool kAdex, bool kOneRound = false, bool kRes = false>
 __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* __restrict__ P, long long n, int slot, bool pending,
                                                unsigned long long rec_prev, PipeShared& sh, bool have_k = false) {
     const int N = a.N, Dr = a.Dr;
@@ -1139,7 +1147,7 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
             const bool single_round = kOneRound;
             const long long stride = (long long)gridDim.x * U;
             NeuronLoad L, Ln;
-            if (!kAdex) { const long long i0 = (long long)blockIdx.x * U + threadIdx.x; if (i0 < N) L = neuron_load<kAdex>(a, plane, (int)i0, have_k); }
+            if (!kAdex && !kRes) { const long long i0 = (long long)blockIdx.x * U + threadIdx.x; if (i0 < N) L = neuron_load<kAdex>(a, plane, (int)i0, have_k); }
             for (long long base = (long long)blockIdx.x * U; base < N; base += stride) {
                 const long long ii = base + threadIdx.x;
                 const int i = (int)ii;
@@ -1151,8 +1159,30 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
                 // (only while one round covers the network: for large N the extra 16 B per neuron-step costs more
                 // bandwidth than the round trip of the few spiking threads)
                 RowInfo r;
+                bool spk = false;
+                float res_in = 0.f, res_I = 0.f;
+                if (kRes) {
+                    // Resident LIF state: the membrane update reads nothing but shared memory — V_{n+1} does not depend on
+                    // the input arriving in this step — so the spike is known ~0.1 us into the phase and the delay-1
+                    // records start at once; the one L2 round trip of the step (the input cell, written by other SMs'
+                    // reds) overlaps all of it and is waited for only by the current update at the end.
+                    const int t = threadIdx.x;
+                    if (ii < N) {
+                        res_in = __ldcg(plane + i);
+                        float V = sh.res_V[t];
+                        int rf = sh.res_r[t];
+                        res_I = sh.res_I[t];
+                        const PopDev* __restrict__ p = P + sh.res_pi[t];
+                        const float E_L = p->E_L;
+                        if (rf == 0) V = E_L + fmaf(p->P22, V - E_L, fmaf(p->P21, res_I, p->P20Ie));
+                        else rf -= 1;
+                        if (V >= p->V_th) { spk = true; V = p->V_reset; rf = p->refr_steps; r = sh.res_row[t]; }
+                        sh.res_V[t] = V; sh.res_r[t] = rf;
+                    }
+                } else {
                 if (single_round && ii < N) r = ld_row_info(a.row_info + i);
-                bool spk = ii < N && neuron_early<kAdex, kAdex && kOneRound>(a, P, n, i, g, L);
+                spk = ii < N && neuron_early<kAdex, kAdex && kOneRound>(a, P, n, i, g, L);
+                }
                 if (kAdex && kOneRound && ii < N && g.pending) {            // first attempt did not finish: second pass, dense warps
                     const int ks = atomicAdd(&sh.n_slow, 1);
                     if (ks < kSlowCap) { sh.slow_id[ks] = i | (g.spiked ? (1 << 30) : 0); sh.slow_t[ks] = g.t; }
@@ -1183,6 +1213,16 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
                         }
                     }
                 }
+                if (kRes) {
+                    if (ii < N) {
+                        const int t = threadIdx.x;
+                        const PopDev* __restrict__ p = P + sh.res_pi[t];
+                        plane[i] = 0.f;
+                        if (a.last_input) a.last_input[i] = res_in;
+                        const int k = have_k ? (int)sh.res_kq[t] : poisson_count(a, p, n, i);
+                        sh.res_I[t] = fmaf(p->P11, res_I, res_in) + p->w_ext * (float)k;
+                    }
+                } else
                 if (ii < N && !(kAdex && kOneRound && (g.pending || g.pi < 0))) neuron_late<kAdex>(a, P, n, i, plane, g);
                 if (!kAdex && !kOneRound) L = Ln;
             }
@@ -1219,7 +1259,10 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
             // delay-1 pass (nothing on the critical path needs the global index)
             // (issued by the LAST updater thread, whose warp has no delay-1 records unless a row has thousands: on the
             // first warps the atomic's round trip was measured in front of the record loads, 0.4 us)
-            if ((int)threadIdx.x == U - 1 && nd1 > 0) sh.gbase = atomicAdd(&a.ctl->spike_cnt[n & 3], nd1);
+            // The same warp later writes the CTA's entries of the global spike array: no barrier, nothing after the reds
+            // on the warps that deliver.
+            int gb = 0;
+            if ((int)threadIdx.x == U - 1 && nd1 > 0) gb = atomicAdd(&a.ctl->spike_cnt[n & 3], nd1);
             // the rest of the spiking rows is read one phase later: request it now, from the LAST updater threads, so
             // that issuing the bulk prefetches overlaps the delay-1 pass of the first warps instead of following it
             if (a.prefetch)
@@ -1235,10 +1278,9 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
                 }
             } else d1_flat_pass(a, sh, plane1, nd1, U);           // many spikes: out of line, off the latency path
             trace_stamp(a, n, 6);
-            if (nd1 > 0) {                                         // uniform over the updater group
-                group_sync(1, U);
-                const int gb = sh.gbase;
-                for (int s = threadIdx.x; s < nd1; s += U) {       // a2: global spike array; the rest of the row is read
+            if (nd1 > 0 && (int)threadIdx.x >= U - 32) {           // the last updater warp (U is a multiple of 32)
+                gb = __shfl_sync(0xffffffffu, gb, 31);
+                for (int s = lane; s < nd1; s += 32) {             // a2: global spike array; the rest of the row is read
                     RowInfo r; r.r0 = sh.d1_r0[s]; r.d1 = sh.d1_cnt[s]; r.deg = sh.d1_deg[s];       // one phase later
                     const size_t gk = (size_t)(n & 1) * N + gb + s;
                     a.spike_list[gk] = sh.d1_id[s];
@@ -1383,23 +1425,38 @@ __global__ void __launch_bounds__(kAdex ? 512 : kPersistentThreads, kAdex ? 2 : 
     const long long gtid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const int U = pipe_updater_threads(a.N, kAdex);
     const bool single_round = kOneRound;                           // else the counts are computed in line, overlapping the loads
+    constexpr bool kRes = !kAdex && kOneRound;                     // LIF state resident in shared memory (the host never
+    const long long res_i = (long long)blockIdx.x * U + threadIdx.x;       // picks this instantiation in bypass mode)
+    if (kRes && (int)threadIdx.x < U && res_i < a.N) {
+        const int t = threadIdx.x;
+        sh.res_V[t] = a.V[res_i]; sh.res_I[t] = a.I[res_i]; sh.res_r[t] = a.refr[res_i]; sh.res_pi[t] = a.pop_of[res_i];
+        sh.res_row[t] = ld_row_info(a.row_info + res_i);
+    }
     long long n = sh.sc.n;
     int slot = sh.sc.slot;
     unsigned long long rec_prev = sh.sc.rec_base, spikes = 0, epoch = 0;       // recorded before step n-1 (nothing pending at entry)
     for (long long s = 0; s < n_steps; ++s, ++n) {
         if (gtid == 0) a.ctl->spike_cnt[(n + 1) & 3] = 0;          // last read (as step n-3's) in phase n-2
         trace_stamp(a, n, 0);
-        const int Mp = pipelined_phase<true, kAdex, kOneRound>(a, P, n, slot, s > 0, rec_prev, sh, s > 0 && single_round);
+        const int Mp = pipelined_phase<true, kAdex, kOneRound, kRes>(a, P, n, slot, s > 0, rec_prev, sh, s > 0 && single_round);
         rec_prev += (unsigned long long)Mp; spikes += (unsigned long long)Mp;
         trace_stamp(a, n, 1);
         grid_arrive(a.ctl, epoch);
         if (s + 1 < n_steps && !a.bypass && single_round && (int)threadIdx.x < U) {    // barrier shadow: Poisson counts of step n+1
-            for (long long ii = (long long)blockIdx.x * U + threadIdx.x; ii < a.N; ii += (long long)gridDim.x * U)
-                a.pois_k[ii] = (uint8_t)poisson_count(a, P + a.pop_of[ii], n + 1, (int)ii);
+            if (kRes) {                                            // thread t owns neuron blockIdx.x * U + t for the whole launch
+                const long long ii = (long long)blockIdx.x * U + threadIdx.x;
+                if (ii < a.N) sh.res_kq[threadIdx.x] = (uint8_t)poisson_count(a, P + sh.res_pi[threadIdx.x], n + 1, (int)ii);
+            } else
+                for (long long ii = (long long)blockIdx.x * U + threadIdx.x; ii < a.N; ii += (long long)gridDim.x * U)
+                    a.pois_k[ii] = (uint8_t)poisson_count(a, P + a.pop_of[ii], n + 1, (int)ii);
         }
         grid_wait(a.ctl, epoch);
         trace_stamp(a, n, 2);
         slot = slot + 1 == a.Dr ? 0 : slot + 1;
+    }
+    if (kRes && (int)threadIdx.x < U && res_i < a.N) {
+        const int t = threadIdx.x;
+        a.V[res_i] = sh.res_V[t]; a.I[res_i] = sh.res_I[t]; a.refr[res_i] = sh.res_r[t];
     }
     if (n_steps > 0) {                                             // flush: rest pass of the last step
         const int Mp = pipelined_phase<false, kAdex>(a, P, n, slot, true, rec_prev, sh);
