@@ -1128,10 +1128,12 @@ __device__ __forceinline__ int pipe_updater_threads(int N, bool heavy_update) {
 // pressure and traffic, so every lane finishes in place there.
 template <bool kUpdate, bool kAdex, bool kOneRound = false, bool kRes = false>
 __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* __restrict__ P, long long n, int slot, bool pending,
-                                               unsigned long long rec_prev, PipeShared& sh, bool have_k = false) {
+                                               unsigned long long rec_prev, PipeShared& sh, int U, bool have_k = false) {
     const int N = a.N, Dr = a.Dr;
     const int lane = threadIdx.x & 31;
-    const int U = pipe_updater_threads(N, kAdex), R = blockDim.x - U;     // rest group = threads [U, U + R), R >= 64
+    // U = pipe_updater_threads(N, kAdex), computed once per launch by the caller: its integer division in front of every
+    // phase cost all 32 warps ~50 issue slots each, 0.2 us before the first useful instruction
+    const int R = blockDim.x - U;                                  // rest group = threads [U, U + R), R >= 64
     const int RT = min(R, kEntryTile);                             // threads of the rest group that stage entries
     const int nmod_prev = slot == 0 ? Dr - 1 : slot - 1;           // (n - 1) mod Dr
     if (threadIdx.x == 0) { sh.n_d1 = 0; sh.n_slow = 0; }
@@ -1147,6 +1149,7 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
             const bool single_round = kOneRound;
             const long long stride = (long long)gridDim.x * U;
             NeuronLoad L, Ln;
+            float res_in = 0.f, res_I = 0.f;
             if (!kAdex && !kRes) { const long long i0 = (long long)blockIdx.x * U + threadIdx.x; if (i0 < N) L = neuron_load<kAdex>(a, plane, (int)i0, have_k); }
             for (long long base = (long long)blockIdx.x * U; base < N; base += stride) {
                 const long long ii = base + threadIdx.x;
@@ -1160,7 +1163,6 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
                 // bandwidth than the round trip of the few spiking threads)
                 RowInfo r;
                 bool spk = false;
-                float res_in = 0.f, res_I = 0.f;
                 if (kRes) {
                     // Resident LIF state: the membrane update reads nothing but shared memory — V_{n+1} does not depend on
                     // the input arriving in this step — so the spike is known ~0.1 us into the phase and the delay-1
@@ -1168,7 +1170,7 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
                     // reds) overlaps all of it and is waited for only by the current update at the end.
                     const int t = threadIdx.x;
                     if (ii < N) {
-                        res_in = __ldcg(plane + i);
+                        asm volatile("ld.global.cg.f32 %0, [%1];" : "=f"(res_in) : "l"(plane + i));      // first: the one long latency
                         float V = sh.res_V[t];
                         int rf = sh.res_r[t];
                         res_I = sh.res_I[t];
@@ -1213,17 +1215,7 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
                         }
                     }
                 }
-                if (kRes) {
-                    if (ii < N) {
-                        const int t = threadIdx.x;
-                        const PopDev* __restrict__ p = P + sh.res_pi[t];
-                        plane[i] = 0.f;
-                        if (a.last_input) a.last_input[i] = res_in;
-                        const int k = have_k ? (int)sh.res_kq[t] : poisson_count(a, p, n, i);
-                        sh.res_I[t] = fmaf(p->P11, res_I, res_in) + p->w_ext * (float)k;
-                    }
-                } else
-                if (ii < N && !(kAdex && kOneRound && (g.pending || g.pi < 0))) neuron_late<kAdex>(a, P, n, i, plane, g);
+                if (!kRes && ii < N && !(kAdex && kOneRound && (g.pending || g.pi < 0))) neuron_late<kAdex>(a, P, n, i, plane, g);
                 if (!kAdex && !kOneRound) L = Ln;
             }
             if (kAdex && kOneRound) {                               // second pass over the CTA's slow neurons
@@ -1277,6 +1269,17 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
                     for (int q = wib * 32 + lane; q < cnt; q += wpu * 32) deliver_d1_piece(a, plane1, r0, cnt, q);
                 }
             } else d1_flat_pass(a, sh, plane1, nd1, U);           // many spikes: out of line, off the latency path
+            if (kRes) {                                            // the current update: the only consumer of the input cell
+                const long long ii = (long long)blockIdx.x * U + threadIdx.x;
+                if (ii < N) {
+                    const int t = threadIdx.x, i = (int)ii;
+                    const PopDev* __restrict__ p = P + sh.res_pi[t];
+                    plane[i] = 0.f;
+                    if (a.last_input) a.last_input[i] = res_in;
+                    const int k = have_k ? (int)sh.res_kq[t] : poisson_count(a, p, n, i);
+                    sh.res_I[t] = fmaf(p->P11, res_I, res_in) + p->w_ext * (float)k;
+                }
+            }
             trace_stamp(a, n, 6);
             if (nd1 > 0 && (int)threadIdx.x >= U - 32) {           // the last updater warp (U is a multiple of 32)
                 gb = __shfl_sync(0xffffffffu, gb, 31);
@@ -1390,7 +1393,7 @@ __global__ void __launch_bounds__(kPipeThreads) pipe_step_kernel(const StepArgs 
     if (a.n_pops > kMaxPopsSmem) __syncthreads();
     const long long n = sh.sc.n;
     const int slot = sh.sc.slot;
-    pipelined_phase<kUpdate, kAdex, kOneRound>(a, P, n, slot, sh.pending != 0, sh.sc.rec_base, sh);
+    pipelined_phase<kUpdate, kAdex, kOneRound>(a, P, n, slot, sh.pending != 0, sh.sc.rec_base, sh, pipe_updater_threads(a.N, kAdex));
     if (threadIdx.x == 0) {
         __threadfence();
         const unsigned t = atomicAdd(&a.ctl->ticket, 1u);
@@ -1438,7 +1441,7 @@ __global__ void __launch_bounds__(kAdex ? 512 : kPersistentThreads, kAdex ? 2 : 
     for (long long s = 0; s < n_steps; ++s, ++n) {
         if (gtid == 0) a.ctl->spike_cnt[(n + 1) & 3] = 0;          // last read (as step n-3's) in phase n-2
         trace_stamp(a, n, 0);
-        const int Mp = pipelined_phase<true, kAdex, kOneRound, kRes>(a, P, n, slot, s > 0, rec_prev, sh, s > 0 && single_round);
+        const int Mp = pipelined_phase<true, kAdex, kOneRound, kRes>(a, P, n, slot, s > 0, rec_prev, sh, U, s > 0 && single_round);
         rec_prev += (unsigned long long)Mp; spikes += (unsigned long long)Mp;
         trace_stamp(a, n, 1);
         grid_arrive(a.ctl, epoch);
@@ -1459,7 +1462,7 @@ __global__ void __launch_bounds__(kAdex ? 512 : kPersistentThreads, kAdex ? 2 : 
         a.V[res_i] = sh.res_V[t]; a.I[res_i] = sh.res_I[t]; a.refr[res_i] = sh.res_r[t];
     }
     if (n_steps > 0) {                                             // flush: rest pass of the last step
-        const int Mp = pipelined_phase<false, kAdex>(a, P, n, slot, true, rec_prev, sh);
+        const int Mp = pipelined_phase<false, kAdex>(a, P, n, slot, true, rec_prev, sh, U);
         rec_prev += (unsigned long long)Mp; spikes += (unsigned long long)Mp;
     }
     if (gtid == 0) {
