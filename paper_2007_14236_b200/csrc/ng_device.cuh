@@ -1333,6 +1333,9 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
                 }
             }
             int x = 0;
+            // only the warps that hold entries run the staging code: with all fifteen rest warps in it the few spikes of
+            // a latency-bound step cost ~250 issue slots per warp, 0.5 us, before the first record was requested
+            const int mw = (m + 31) >> 5;
             if (t < m) {                                           // e = r0 (lo, hi), deg, d1
                 const int len = padded_len(e.z);
                 sh.d.r0[t] = (long long)(((unsigned long long)(uint32_t)e.y << 32) | (uint32_t)e.x);
@@ -1345,7 +1348,7 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
                     if (pos < (unsigned long long)a.rec_cap) { a.rec_id[pos] = id_prev; a.rec_step[pos] = (int32_t)np; }
                 }
             }
-            if (t < RT) {                                          // whole warps: RT is a multiple of 32
+            if (wir < mw) {                                        // whole warps (m <= RT, a multiple of 32)
 #pragma unroll
                 for (int o = 1; o < 32; o <<= 1) {
                     const int y = __shfl_up_sync(0xffffffffu, x, o);
@@ -1355,7 +1358,7 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
             }
             if (m > 32) {                                          // several warps hold entries: add the warp offsets
                 group_sync(2, R);
-                if (t < RT) {
+                if (wir < mw) {
                     int off = 0;
                     for (int k = 0; k < wir; ++k) off += sh.d.warp_tot[k];
                     sh.d.pre[t + 1] = x + off;
