@@ -1306,6 +1306,13 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
             e = __ldcg(reinterpret_cast<const int4*>(rows_prev + t));
             if (rec_cta) id_prev = __ldcg(list_prev + t);
         }
+        // the first 32 entries go to shared memory before M is known (entries beyond M are stale but valid memory): the
+        // barrier that publishes M publishes them too
+        if (t < 32 && t < N) {
+            sh.d.r0[t] = (long long)(((unsigned long long)(uint32_t)e.y << 32) | (uint32_t)e.x);
+            sh.d.len[t] = padded_len(e.z);
+            sh.skip[t] = e.w;
+        }
         group_sync(2, R);
         trace_stamp(a, n, 7, U);
         const int M = sh.d.M;
@@ -1323,6 +1330,34 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
         const int tile_first = part ? (int)blockIdx.x * tile_len : 0, tile_stride = part ? (int)gridDim.x * tile_len : RT;
         const int gw = part ? wir : gwarp, gw_n = part ? wpr : gwarps;
         const bool rec_here = a.rec_cap > 0 && (blockIdx.x == 0 || part);
+        if (M <= 32) {
+            // Latency regime (three steps of four in config 2): no second staging round and no second barrier — every
+            // rest warp prefix-sums the chunk counts of the <= 32 entries in its own registers and finds its items by
+            // ballot; the first records are requested ~0.5 us earlier.
+            const int len_l = lane < M ? sh.d.len[lane] : 0;
+            int incl = (len_l + (1 << cshift) - 1) >> cshift;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int y = __shfl_up_sync(0xffffffffu, incl, o);
+                if (lane >= o) incl += y;
+            }
+            const int total = __shfl_sync(0xffffffffu, incl, 31);
+            if (blockIdx.x == 0 && t < M) {                        // warp 0 of CTA 0 still holds the entries: events, spike record
+                ev += (unsigned long long)e.z;
+                if (rec_cta) {
+                    const unsigned long long pos = rec_prev + (unsigned long long)t;
+                    if (pos < (unsigned long long)a.rec_cap) { a.rec_id[pos] = id_prev; a.rec_step[pos] = (int32_t)np; }
+                }
+            }
+            for (int it = gwarp; it < total; it += gwarps) {
+                const int sidx = __popc(__ballot_sync(0xffffffffu, incl <= it));
+                const int before = __shfl_sync(0xffffffffu, incl, sidx > 0 ? sidx - 1 : 0);
+                const int c = it - (sidx > 0 ? before : 0);
+                if (cshift == 5) deliver_item<1>(a, nmod_prev, sh.d.r0[sidx], sh.d.len[sidx], c, lane, sh.skip[sidx]);
+                else if (cshift == 6) deliver_item<2>(a, nmod_prev, sh.d.r0[sidx], sh.d.len[sidx], c, lane, sh.skip[sidx]);
+                else deliver_item<4>(a, nmod_prev, sh.d.r0[sidx], sh.d.len[sidx], c, lane, sh.skip[sidx]);
+            }
+        } else
         for (int tile0 = tile_first; tile0 < M; tile0 += tile_stride) {
             const int m = min(tile_len, M - tile0);
             if (tile0 > 0) {

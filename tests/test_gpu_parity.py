@@ -122,6 +122,38 @@ def test_cfg0_free_running_spikes_and_rates(oracle_mod, B, mode, kernel):
     g.close()
 
 
+@pytest.mark.parametrize("mode,kernel", [(2, 3), (2, 1), (0, 3)])
+def test_cfg0_launch_boundaries_are_invisible(B, mode, kernel):
+    """The persistent pipelined kernel keeps the LIF state in shared memory for a whole launch and writes it back at
+    exit: one call of 240 steps and the same steps cut into calls of 1, 7, 32 and 200 — with a state read-back and a
+    set_state of the same values in between — must give the same spikes and the same state (up to the summation order
+    of the fp32 reductions, which differs from run to run)."""
+    wl = W.brunel_tiny(n_steps=240)
+
+    def run(chunks, roundtrip):
+        g = B.Sim(0.1, wl.ring_slots, wl.seed, record_spikes=True)
+        wl.apply(g); g.prepare(); g.set_state(B.FIELD_V, wl.initial_v())
+        g.set_option(B.OPT_STEP_MODE, mode); g.set_option(B.OPT_DELIVERY_KERNEL, kernel)
+        for c in chunks:
+            g.simulate(c)
+            if roundtrip:
+                for f in (B.FIELD_V, B.FIELD_I_SYN, B.FIELD_REFR):
+                    g.set_state(f, g.get_state(f))
+        st, ids = g.get_spikes()
+        out = (set(zip(st.tolist(), ids.tolist())), g.get_state(B.FIELD_V), g.get_state(B.FIELD_I_SYN), g.get_state(B.FIELD_REFR),
+               g.stats().steps)
+        g.close()
+        return out
+
+    a = run([240], False)
+    b = run([1, 7, 32, 200], True)
+    assert a[4] == b[4] == 240
+    assert len(a[0]) > 150 and len(a[0] ^ b[0]) <= 2, sorted(a[0] ^ b[0])[:10]
+    same = ~np.isin(np.arange(wl.n_neurons), [i for _, i in a[0] ^ b[0]])
+    assert np.mean(np.abs(a[1] - b[1])[same] <= 1e-3) >= 0.99 and np.mean(np.abs(a[2] - b[2])[same] <= 1e-3) >= 0.99
+    assert np.mean(a[3] == b[3]) >= 0.99
+
+
 # ------------------------------------------------------------------------------------------------------------
 # microcircuit-shaped nets (normal weights and delays, 8 populations, up to 54 connect calls)
 # ------------------------------------------------------------------------------------------------------------
