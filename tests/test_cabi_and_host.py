@@ -114,7 +114,7 @@ wl = bench.make_workload("cfg0", seed_offset=rank)      # replicas use independe
 assert wl.seed == 1 + rank
 dist.barrier()
 dist.destroy_process_group()
-print("ok", rank)
+sys.stdout.write("ok %d\n" % rank); sys.stdout.flush()   # one write per rank: the two ranks share a pipe
 '''
 
 
