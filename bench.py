@@ -211,6 +211,9 @@ def run_probes(device=0):
     for mb in (4, 16, 64, 256):
         out[f"scattered_red_per_s_{mb}MB"] = B.probe(1, mb << 20, device)
         out[f"records_plus_red_events_per_s_{mb}MB"] = B.probe(2, mb << 20, device)
+    for cs in (1, 2, 4, 8, 16):                 # reduction target in the distributed shared memory of a cs-CTA cluster (200 KB per CTA)
+        out[f"dsmem_red_per_s_cluster{cs}"] = B.probe(3, cs * 200 * 1024, device)
+        out[f"dsmem_plus_global_red_per_s_cluster{cs}"] = B.probe(4, cs * 200 * 1024, device)
     return out
 
 

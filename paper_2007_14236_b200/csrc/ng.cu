@@ -970,7 +970,7 @@ int32_t ng_get_trace(ng_sim* s, uint64_t* out_host, int64_t capacity, int64_t* c
 
 // ng_probe: see include/ng.h.  Allocates with cudaMalloc, runs on the legacy stream, frees everything.
 extern "C" int32_t ng_probe(int32_t device, int32_t kind, int64_t footprint_bytes, double* per_second_out) {
-    if (!per_second_out || kind < 0 || kind > 2 || footprint_bytes < 4096) return NG_ERR_INVALID_ARG;
+    if (!per_second_out || kind < 0 || kind > 4 || footprint_bytes < 4096) return NG_ERR_INVALID_ARG;
     if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return NG_ERR_CUDA; }
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return NG_ERR_CUDA;
@@ -999,6 +999,30 @@ extern "C" int32_t ng_probe(int32_t device, int32_t kind, int64_t footprint_byte
             probe_red_kernel<<<blocks, thr>>>(ring, M, 2000);
             cudaEventRecord(e1);
             units = (double)blocks * thr * 2000;                        // reductions
+        } else if (kind >= 3) {
+            // plane of footprint_bytes spread over the shared memory of one cluster: 200 KB per CTA, 1..16 CTAs (power of two)
+            const int64_t tile_bytes = 200 * 1024;
+            unsigned csize = 1;
+            while ((int64_t)csize * tile_bytes < footprint_bytes && csize < 32) csize *= 2;
+            if (csize > 16) { rc = NG_ERR_INVALID_ARG; break; }
+            const uint32_t tile = (uint32_t)((footprint_bytes / 4 + csize - 1) / csize), Mg = 1000000;   // global plane: 4 MB
+            const int grid = prop.multiProcessorCount / (int)csize * (int)csize, cthr = 1024, per = 2000;
+            if (cudaMalloc(&ring, (size_t)Mg * 4) != cudaSuccess) { rc = NG_ERR_OOM; break; }
+            cudaMemset(ring, 0, (size_t)Mg * 4);
+            auto kern = kind == 3 ? probe_dsmem_red_kernel<false> : probe_dsmem_red_kernel<true>;
+            cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(tile * 4));
+            cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+            cudaLaunchConfig_t lc = {};
+            lc.gridDim = dim3(grid); lc.blockDim = dim3(cthr); lc.dynamicSmemBytes = (size_t)tile * 4;
+            cudaLaunchAttribute at[1];
+            at[0].id = cudaLaunchAttributeClusterDimension;
+            at[0].val.clusterDim.x = csize; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+            lc.attrs = at; lc.numAttrs = 1;
+            if (cudaLaunchKernelEx(&lc, kern, ring, Mg, tile, (uint32_t)csize, 100) != cudaSuccess) { rc = NG_ERR_CUDA; break; }
+            cudaEventRecord(e0);
+            if (cudaLaunchKernelEx(&lc, kern, ring, Mg, tile, (uint32_t)csize, per) != cudaSuccess) { rc = NG_ERR_CUDA; break; }
+            cudaEventRecord(e1);
+            units = (double)grid * cthr * per;                          // reductions
         } else {
             if (cudaMalloc(&ring, (size_t)M * 4) != cudaSuccess || cudaMalloc(&tgt, n_rec * 4) != cudaSuccess ||
                 cudaMalloc(&w, n_rec * 4) != cudaSuccess) { rc = NG_ERR_OOM; break; }

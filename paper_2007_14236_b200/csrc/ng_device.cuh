@@ -1746,6 +1746,28 @@ __global__ void probe_deliver_kernel(const int4* __restrict__ tgt, const float4*
         red_add_f32(ring + t.z, ww.z); red_add_f32(ring + t.w, ww.w);
     }
 }
+// kinds 3, 4: the reduction target held in the distributed shared memory of a thread-block cluster (`tile` cells per CTA,
+// csize CTAs): `per_thread` red.shared::cluster.add.f32 per thread to uniformly random cells of the cluster's plane;
+// kMix alternates them with red.global.add.f32 into ring[0..M) (do the two reduction paths add up?)
+template <bool kMix>
+__global__ void probe_dsmem_red_kernel(float* ring, uint32_t M, uint32_t tile, uint32_t csize, int per_thread) {
+    extern __shared__ float probe_tile[];
+    for (uint32_t i = threadIdx.x; i < tile; i += blockDim.x) probe_tile[i] = 0.f;
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+    const uint32_t base = (uint32_t)__cvta_generic_to_shared(probe_tile), cells = tile * csize;
+    uint32_t s = probe_hash((blockIdx.x * blockDim.x + threadIdx.x) * 2654435761u + 1u);
+    for (int i = 0; i < per_thread; ++i) {
+        s = s * 1664525u + 1013904223u;
+        const uint32_t r = probe_hash(s);
+        if (kMix && (i & 1)) { red_add_f32(ring + __umulhi(r, M), 1.0f); continue; }
+        const uint32_t c = __umulhi(r, cells), rank = c / tile;
+        uint32_t remote;
+        asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(base + (c - rank * tile) * 4u), "r"(rank));
+        asm volatile("red.shared::cluster.add.f32 [%0], %1;" ::"r"(remote), "f"(1.0f) : "memory");
+    }
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+    if (probe_tile[threadIdx.x % tile] == -1.f) ring[0] = 1.f;
+}
 __global__ void probe_fill_targets_kernel(int32_t* t, long long n, uint32_t M) {
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
