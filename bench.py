@@ -214,6 +214,7 @@ def run_probes(device=0):
     for cs in (1, 2, 4, 8, 16):                 # reduction target in the distributed shared memory of a cs-CTA cluster (200 KB per CTA)
         out[f"dsmem_red_per_s_cluster{cs}"] = B.probe(3, cs * 200 * 1024, device)
         out[f"dsmem_plus_global_red_per_s_cluster{cs}"] = B.probe(4, cs * 200 * 1024, device)
+    out["tiled_delivery_shape_events_per_s"] = B.probe(5, 200 * 1024, device)
     return out
 
 

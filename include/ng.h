@@ -293,6 +293,9 @@ int32_t ng_get_trace(ng_sim* sim, uint64_t* out_host, int64_t capacity, int64_t*
  *   kind 3: red.shared::cluster.add.f32 to uniformly random cells of a footprint_bytes plane spread over the shared
  *           memory of one thread-block cluster (200 KB per CTA, so footprint_bytes <= 3,276,800 = 16 CTAs)  -> reductions per second
  *   kind 4: kind 3 alternating with red.global.add.f32 into a 4 MB plane (whether the two paths add up) -> reductions per second
+ *   kind 5: the access shape of a target-tiled delivery: per item one dependent 4-byte lookup in a 256 MB table, then an
+ *           8-record run (32 B targets + 32 B weights, random place in 2 GiB) reduced into the CTA's own shared-memory tile
+ *           of footprint_bytes (<= 200 KB)                                                     -> events per second
  * Allocates its own scratch with cudaMalloc and frees it.  Errors: INVALID_ARG, OOM, CUDA. */
 int32_t ng_probe(int32_t device, int32_t kind, int64_t footprint_bytes, double* per_second_out);
 

@@ -970,7 +970,7 @@ int32_t ng_get_trace(ng_sim* s, uint64_t* out_host, int64_t capacity, int64_t* c
 
 // ng_probe: see include/ng.h.  Allocates with cudaMalloc, runs on the legacy stream, frees everything.
 extern "C" int32_t ng_probe(int32_t device, int32_t kind, int64_t footprint_bytes, double* per_second_out) {
-    if (!per_second_out || kind < 0 || kind > 4 || footprint_bytes < 4096) return NG_ERR_INVALID_ARG;
+    if (!per_second_out || kind < 0 || kind > 5 || footprint_bytes < 4096) return NG_ERR_INVALID_ARG;
     if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return NG_ERR_CUDA; }
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return NG_ERR_CUDA;
@@ -999,6 +999,22 @@ extern "C" int32_t ng_probe(int32_t device, int32_t kind, int64_t footprint_byte
             probe_red_kernel<<<blocks, thr>>>(ring, M, 2000);
             cudaEventRecord(e1);
             units = (double)blocks * thr * 2000;                        // reductions
+        } else if (kind == 5) {
+            const uint32_t n_offs = 1u << 26, tile = (uint32_t)std::min<int64_t>(footprint_bytes / 4, 50 * 1024);
+            const int grid = prop.multiProcessorCount, cthr = 1024, per = 2000;
+            uint32_t* offs = nullptr;
+            if (cudaMalloc(&ring, (size_t)n_offs * 4) != cudaSuccess || cudaMalloc(&tgt, n_rec * 4) != cudaSuccess ||
+                cudaMalloc(&w, n_rec * 4) != cudaSuccess) { rc = NG_ERR_OOM; break; }
+            offs = (uint32_t*)ring;
+            cudaMemset(w, 0, n_rec * 4);
+            probe_fill_targets_kernel<<<blocks, thr>>>(tgt, n_rec, 1000000u);
+            probe_fill_targets_kernel<<<blocks, thr>>>((int32_t*)offs, n_offs, (uint32_t)(n_rec / 8));
+            cudaFuncSetAttribute(probe_tiled_deliver_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(tile * 4));
+            probe_tiled_deliver_kernel<<<grid, cthr, tile * 4>>>(offs, n_offs, tgt, w, tile, 100, (float*)sink);
+            cudaEventRecord(e0);
+            probe_tiled_deliver_kernel<<<grid, cthr, tile * 4>>>(offs, n_offs, tgt, w, tile, per, (float*)sink);
+            cudaEventRecord(e1);
+            units = (double)grid * cthr * per;                          // events (8 lanes x one run each per item)
         } else if (kind >= 3) {
             // plane of footprint_bytes spread over the shared memory of one cluster: 200 KB per CTA, 1..16 CTAs (power of two)
             const int64_t tile_bytes = 200 * 1024;

@@ -1768,6 +1768,29 @@ __global__ void probe_dsmem_red_kernel(float* ring, uint32_t M, uint32_t tile, u
     asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
     if (probe_tile[threadIdx.x % tile] == -1.f) ring[0] = 1.f;
 }
+// kind 5: the access shape of a target-tiled delivery (item 0): per work item one dependent 4-byte
+// lookup in a 256 MB offset table, then an 8-record run (32 B of targets + 32 B of weights at a random 32-byte-aligned
+// place in 2 GiB of records) read by 8 lanes and reduced into the CTA's own shared-memory tile
+__global__ void probe_tiled_deliver_kernel(const uint32_t* __restrict__ offs, uint32_t n_offs, const int32_t* __restrict__ tgt,
+                                           const float* __restrict__ w, uint32_t tile, int per_group, float* sink) {
+    extern __shared__ float probe_tile[];
+    for (uint32_t i = threadIdx.x; i < tile; i += blockDim.x) probe_tile[i] = 0.f;
+    __syncthreads();
+    const uint32_t base = (uint32_t)__cvta_generic_to_shared(probe_tile), lane8 = threadIdx.x & 7;
+    uint32_t s = probe_hash(((blockIdx.x * blockDim.x + threadIdx.x) >> 3) * 2654435761u + 1u);
+    for (int i = 0; i < per_group; i += 4) {
+        uint32_t run[4]; int32_t t[4]; float ww[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { s = s * 1664525u + 1013904223u; run[u] = __ldg(offs + __umulhi(probe_hash(s), n_offs)); }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { t[u] = __ldg(tgt + (size_t)run[u] * 8 + lane8); ww[u] = __ldg(w + (size_t)run[u] * 8 + lane8); }
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+            asm volatile("red.shared::cta.add.f32 [%0], %1;" ::"r"(base + ((uint32_t)t[u] % tile) * 4u), "f"(ww[u]) : "memory");
+    }
+    __syncthreads();
+    if (probe_tile[threadIdx.x % tile] == -1.f) *sink = 1.f;
+}
 __global__ void probe_fill_targets_kernel(int32_t* t, long long n, uint32_t M) {
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
