@@ -215,6 +215,8 @@ def run_probes(device=0):
         out[f"dsmem_red_per_s_cluster{cs}"] = B.probe(3, cs * 200 * 1024, device)
         out[f"dsmem_plus_global_red_per_s_cluster{cs}"] = B.probe(4, cs * 200 * 1024, device)
     out["tiled_delivery_shape_events_per_s"] = B.probe(5, 200 * 1024, device)
+    for K in (100, 1000):                       # append half of a per-delay event queue, rows of K records
+        out[f"queue_append_events_per_s_K{K}"] = B.probe(6, 8 * K, device)
     return out
 
 

@@ -296,6 +296,9 @@ int32_t ng_get_trace(ng_sim* sim, uint64_t* out_host, int64_t capacity, int64_t*
  *   kind 5: the access shape of a target-tiled delivery: per item one dependent 4-byte lookup in a 256 MB table, then an
  *           8-record run (32 B targets + 32 B weights, random place in 2 GiB) reduced into the CTA's own shared-memory tile
  *           of footprint_bytes (<= 200 KB)                                                     -> events per second
+ *   kind 6: the append half of a per-delay event queue: whole source rows of footprint_bytes (8 x out-degree, >= 64) read
+ *           coalesced at random places in 2 GiB, binned by delay in shared memory, appended as (target, weight) pairs to
+ *           64 global queues with one atomic per (4096-record batch, delay)                       -> events per second
  * Allocates its own scratch with cudaMalloc and frees it.  Errors: INVALID_ARG, OOM, CUDA. */
 int32_t ng_probe(int32_t device, int32_t kind, int64_t footprint_bytes, double* per_second_out);
 

@@ -970,7 +970,7 @@ int32_t ng_get_trace(ng_sim* s, uint64_t* out_host, int64_t capacity, int64_t* c
 
 // ng_probe: see include/ng.h.  Allocates with cudaMalloc, runs on the legacy stream, frees everything.
 extern "C" int32_t ng_probe(int32_t device, int32_t kind, int64_t footprint_bytes, double* per_second_out) {
-    if (!per_second_out || kind < 0 || kind > 5 || footprint_bytes < 4096) return NG_ERR_INVALID_ARG;
+    if (!per_second_out || kind < 0 || kind > 6 || footprint_bytes < (kind == 6 ? 64 : 4096)) return NG_ERR_INVALID_ARG;
     if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return NG_ERR_CUDA; }
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return NG_ERR_CUDA;
@@ -999,6 +999,26 @@ extern "C" int32_t ng_probe(int32_t device, int32_t kind, int64_t footprint_byte
             probe_red_kernel<<<blocks, thr>>>(ring, M, 2000);
             cudaEventRecord(e1);
             units = (double)blocks * thr * 2000;                        // reductions
+        } else if (kind == 6) {
+            const uint32_t K = (uint32_t)std::min<int64_t>(footprint_bytes / 8, 4096), cap_mask = (1u << 22) - 1;   // 64 queues x 4 Mi events
+            const uint32_t n_rows = (uint32_t)(n_rec / K);
+            const int grid = prop.multiProcessorCount, batches = 64;
+            unsigned long long* tails = nullptr; int2* queues = nullptr;
+            if (cudaMalloc(&tgt, n_rec * 4) != cudaSuccess || cudaMalloc(&w, n_rec * 4) != cudaSuccess ||
+                cudaMalloc(&ring, 64 * 128) != cudaSuccess) { rc = NG_ERR_OOM; break; }
+            if (cudaMalloc(&queues, (size_t)64 * (cap_mask + 1) * 8) != cudaSuccess) { rc = NG_ERR_OOM; break; }
+            tails = (unsigned long long*)ring;
+            cudaMemset(tails, 0, 64 * 128); cudaMemset(w, 0, n_rec * 4);
+            probe_fill_targets_kernel<<<blocks, thr>>>(tgt, n_rec, 1000000u);
+            probe_queue_append_kernel<<<grid, 1024>>>(tgt, w, n_rows, K, tails, queues, cap_mask, 4);
+            cudaEventRecord(e0);
+            probe_queue_append_kernel<<<grid, 1024>>>(tgt, w, n_rows, K, tails, queues, cap_mask, batches);
+            cudaEventRecord(e1);
+            units = (double)grid * batches * 4096;                      // events appended
+            if (cudaDeviceSynchronize() != cudaSuccess) rc = NG_ERR_CUDA;
+            else { cudaEventElapsedTime(&ms, e0, e1); *per_second_out = units / (ms * 1e-3); }
+            cudaFree(queues);
+            break;
         } else if (kind == 5) {
             const uint32_t n_offs = 1u << 26, tile = (uint32_t)std::min<int64_t>(footprint_bytes / 4, 50 * 1024);
             const int grid = prop.multiProcessorCount, cthr = 1024, per = 2000;

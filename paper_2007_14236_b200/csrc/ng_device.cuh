@@ -1791,6 +1791,52 @@ __global__ void probe_tiled_deliver_kernel(const uint32_t* __restrict__ offs, ui
     __syncthreads();
     if (probe_tile[threadIdx.x % tile] == -1.f) *sink = 1.f;
 }
+// kind 6: the append half of a per-delay event queue (item 0): a CTA takes batches of 4096 records
+// from whole source rows of K records at random places in 2 GiB (coalesced), bins them by delay (64 delays, rows
+// delay-grouped: record r of a row has delay r*64/K) in shared memory, claims a range in each of 64 global queues with
+// one atomic per (batch, delay) and stores (target, weight) pairs there; the drain half is kind 2
+__global__ void probe_queue_append_kernel(const int32_t* __restrict__ tgt, const float* __restrict__ w, uint32_t n_rows, uint32_t K,
+                                          unsigned long long* tails, int2* queues, uint32_t cap_mask, int batches) {
+    __shared__ uint32_t hist[64], base[64], sbase[65];
+    __shared__ int2 staged[4096];
+    if (threadIdx.x < 64) hist[threadIdx.x] = 0;
+    __syncthreads();
+    uint32_t seed = probe_hash(blockIdx.x * 2654435761u + 1u);
+    for (int b = 0; b < batches; ++b) {
+        int32_t t[4]; float ww[4]; uint32_t d[4], rank[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const uint32_t rec = threadIdx.x + u * 1024u, row_in_batch = rec / K, r = rec - row_in_batch * K;
+            const uint32_t row = __umulhi(probe_hash(seed + (uint32_t)b * 4099u + row_in_batch), n_rows);
+            t[u] = __ldg(tgt + (size_t)row * K + r); ww[u] = __ldg(w + (size_t)row * K + r);
+            d[u] = (uint32_t)(((unsigned long long)r * 64u) / K);
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) rank[u] = atomicAdd(&hist[d[u]], 1u);
+        __syncthreads();
+        if (threadIdx.x < 64) {                                    // exclusive scan of the 64 bins + one queue claim per bin
+            uint32_t acc = 0;
+            for (uint32_t k = 0; k < threadIdx.x; ++k) acc += hist[k];
+            sbase[threadIdx.x] = acc;
+            if (threadIdx.x == 63) sbase[64] = acc + hist[63];
+            base[threadIdx.x] = (uint32_t)atomicAdd(tails + threadIdx.x * 16, (unsigned long long)hist[threadIdx.x]);   // one 128-byte line per tail
+        }
+        __syncthreads();
+        if (threadIdx.x < 64) hist[threadIdx.x] = 0;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) staged[sbase[d[u]] + rank[u]] = make_int2(t[u], __float_as_int(ww[u]));
+        __syncthreads();
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {                              // sorted by delay: consecutive threads store consecutive queue cells
+            const uint32_t p = threadIdx.x + u * 1024u;
+            uint32_t lo = 0;
+#pragma unroll
+            for (uint32_t step = 32; step > 0; step >>= 1) if (sbase[lo + step] <= p) lo += step;
+            queues[(size_t)lo * (cap_mask + 1u) + ((base[lo] + (p - sbase[lo])) & cap_mask)] = staged[p];
+        }
+        __syncthreads();
+    }
+}
 __global__ void probe_fill_targets_kernel(int32_t* t, long long n, uint32_t M) {
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
