@@ -58,6 +58,7 @@ struct ng_sim {
     // statistics (ng_enable_statistics)
     int32_t* d_st_sample = nullptr; int st_sample_per_pop = 0; int st_slots = 0;
     bool one_round_step = false, one_round_persistent = false;   // the network is covered in one round of updater threads
+    size_t resm_bytes = 0;                 // > 0: multi-round LIF network with its state resident in dynamic shared memory (kResM)
     bool has_adex = false;                 // any AdEx population: two receptor ports, AdEx state arrays, <true> kernels
     int64_t NR = 0;                        // ring row length = N * ports
     bool window_backend = false;           // delivery kernel 4 chosen before ng_prepare: spike window instead of a D-plane ring
@@ -223,6 +224,21 @@ void configure_launch(ng_sim* s) {
         // updater threads per CTA of the AdEx kernels: all but four warps (pipe_updater_threads in ng_device.cuh)
         s->one_round_persistent = (long long)s->persistent_pipe_blocks * (pt - (s->has_adex ? 128 : (pt >= 512 ? kEntryTile : 64))) >= s->N;
         s->one_round_step = (long long)s->pipe_blocks * (kPipeThreads - (s->has_adex ? 128 : kEntryTile)) >= s->N;
+        // several rounds per step (config 4): keep V, I_syn, refr and the population byte (13 B per neuron) of the CTA's
+        // neurons in dynamic shared memory for the whole launch if that fits beside the static 45 KB
+        s->resm_bytes = 0;
+        if (!s->has_adex && !s->bypass && !s->one_round_persistent && pt - kResMRest >= 256 && s->N > 0) {
+            const long long U = pt - kResMRest, per_round = (long long)s->persistent_pipe_blocks * U;
+            const long long rounds = (s->N + per_round - 1) / per_round;
+            const size_t bytes = ((size_t)(rounds * U) * 13 + 15) & ~(size_t)15;
+            int occ2 = 0;
+            if (bytes <= 160 * 1024 &&
+                cudaFuncSetAttribute(persistent_pipe_kernel<false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) == cudaSuccess &&
+                cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ2, persistent_pipe_kernel<false, false, true>, pt, bytes) == cudaSuccess &&
+                (long long)occ2 * s->sm_count >= s->persistent_pipe_blocks)
+                s->resm_bytes = bytes;
+            cudaGetLastError();
+        }
     }
     int blocks = s->deliver_blocks_opt;
     if (blocks <= 0) {
@@ -719,9 +735,11 @@ int32_t ng_simulate(ng_sim* s, int64_t n_steps) {
             const void* fn = s->has_adex ? (s->one_round_persistent ? (const void*)persistent_pipe_kernel<true, true>
                                                                      : (const void*)persistent_pipe_kernel<true, false>)
                                          : (s->one_round_persistent && !s->bypass ? (const void*)persistent_pipe_kernel<false, true>
-                                                                    : (const void*)persistent_pipe_kernel<false, false>);
+                                            : s->resm_bytes ? (const void*)persistent_pipe_kernel<false, false, true>
+                                                            : (const void*)persistent_pipe_kernel<false, false>);
             NG_CUDA(s, cudaLaunchCooperativeKernel(fn, dim3(s->persistent_pipe_blocks),
-                                                   dim3(s->has_adex ? 512 : s->persistent_threads), args, 0, st));
+                                                   dim3(s->has_adex ? 512 : s->persistent_threads), args,
+                                                   s->has_adex || s->one_round_persistent ? 0 : s->resm_bytes, st));
         } else {
             const void* fn = s->delivery_kernel == 4 ? (const void*)persistent_kernel<4>
                              : s->delivery_kernel == 2 ? (const void*)persistent_kernel<2> : (const void*)persistent_kernel<1>;

@@ -1126,9 +1126,18 @@ __device__ __forceinline__ int pipe_updater_threads(int N, bool heavy_update) {
 // integration attempt per lane, the unfinished neurons in a second, dense pass (10^5 neurons: 33 -> 19 us per step).
 // With many rounds per step the update is bound by its memory round trips and the second pass only adds register
 // pressure and traffic, so every lane finishes in place there.
-template <bool kUpdate, bool kAdex, bool kOneRound = false, bool kRes = false>
+// kResM: LIF state resident in (dynamic) shared memory for networks that need SEVERAL rounds of updater threads per step
+// (config 4: 10^6 neurons = 9 rounds of 768 threads on 148 CTAs, 13 B per neuron = 90 KB per CTA).  Thread t of CTA b owns
+// neurons ((q * gridDim.x + b) * U + t), q = 0..rounds-1, at index q * U + t.  The membrane update and the spike decision
+// then read shared memory only; what is left per neuron and step is the input cell (one 4-byte load, four rounds in
+// flight, and the store that clears it), issued after the delay-1 records of the CTA's spikes are on their way.
+struct ResM { float* V; float* I; int32_t* r; uint8_t* pi; int rounds; };
+constexpr int kResMRest = 256;           // rest-group threads of the kResM kernel
+
+template <bool kUpdate, bool kAdex, bool kOneRound = false, bool kRes = false, bool kResM = false>
 __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* __restrict__ P, long long n, int slot, bool pending,
-                                               unsigned long long rec_prev, PipeShared& sh, int U, bool have_k = false) {
+                                               unsigned long long rec_prev, PipeShared& sh, int U, bool have_k = false,
+                                               const ResM rm = ResM{}) {
     const int N = a.N, Dr = a.Dr;
     const int lane = threadIdx.x & 31;
     // U = pipe_updater_threads(N, kAdex), computed once per launch by the caller: its integer division in front of every
@@ -1150,13 +1159,14 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
             const long long stride = (long long)gridDim.x * U;
             NeuronLoad L, Ln;
             float res_in = 0.f, res_I = 0.f;
-            if (!kAdex && !kRes) { const long long i0 = (long long)blockIdx.x * U + threadIdx.x; if (i0 < N) L = neuron_load<kAdex>(a, plane, (int)i0, have_k); }
-            for (long long base = (long long)blockIdx.x * U; base < N; base += stride) {
+            if (!kAdex && !kRes && !kResM) { const long long i0 = (long long)blockIdx.x * U + threadIdx.x; if (i0 < N) L = neuron_load<kAdex>(a, plane, (int)i0, have_k); }
+            int q_idx = threadIdx.x;                               // kResM: index of this thread's neuron of the current round
+            for (long long base = (long long)blockIdx.x * U; base < N; base += stride, q_idx += U) {
                 const long long ii = base + threadIdx.x;
                 const int i = (int)ii;
                 NeuronRegs g;
                 if (kAdex) { if (ii < N) L = neuron_load<kAdex>(a, plane, i, have_k); }
-                else if (!kOneRound && ii + stride < N) Ln = neuron_load<kAdex>(a, plane, (int)(ii + stride), have_k);   // next round's loads in flight
+                else if (!kOneRound && !kResM && ii + stride < N) Ln = neuron_load<kAdex>(a, plane, (int)(ii + stride), have_k);   // next round's loads in flight
                 // the row descriptor is fetched for EVERY neuron together with its state (16 B, L2-resident because it
                 // is touched every step): a spiking thread then needs no further memory round trip
                 // (only while one round covers the network: for large N the extra 16 B per neuron-step costs more
@@ -1180,6 +1190,17 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
                         else rf -= 1;
                         if (V >= p->V_th) { spk = true; V = p->V_reset; rf = p->refr_steps; r = sh.res_row[t]; }
                         sh.res_V[t] = V; sh.res_r[t] = rf;
+                    }
+                } else if (kResM) {
+                    if (ii < N) {
+                        float V = rm.V[q_idx];
+                        int rf = rm.r[q_idx];
+                        const PopDev* __restrict__ p = P + rm.pi[q_idx];
+                        const float E_L = p->E_L;
+                        if (rf == 0) V = E_L + fmaf(p->P22, V - E_L, fmaf(p->P21, rm.I[q_idx], p->P20Ie));
+                        else rf -= 1;
+                        if (V >= p->V_th) { spk = true; V = p->V_reset; rf = p->refr_steps; }
+                        rm.V[q_idx] = V; rm.r[q_idx] = rf;
                     }
                 } else {
                 if (single_round && ii < N) r = ld_row_info(a.row_info + i);
@@ -1215,8 +1236,8 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
                         }
                     }
                 }
-                if (!kRes && ii < N && !(kAdex && kOneRound && (g.pending || g.pi < 0))) neuron_late<kAdex>(a, P, n, i, plane, g);
-                if (!kAdex && !kOneRound) L = Ln;
+                if (!kRes && !kResM && ii < N && !(kAdex && kOneRound && (g.pending || g.pi < 0))) neuron_late<kAdex>(a, P, n, i, plane, g);
+                if (!kAdex && !kOneRound && !kResM) L = Ln;
             }
             if (kAdex && kOneRound) {                               // second pass over the CTA's slow neurons
                 group_sync(1, U);
@@ -1278,6 +1299,28 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
                     if (a.last_input) a.last_input[i] = res_in;
                     const int k = have_k ? (int)sh.res_kq[t] : poisson_count(a, p, n, i);
                     sh.res_I[t] = fmaf(p->P11, res_I, res_in) + p->w_ext * (float)k;
+                }
+            }
+            if (kResM) {                                           // current update of every round: input cells, four rounds in flight
+                for (int q0 = 0; q0 < rm.rounds; q0 += 4) {
+                    float inv[4];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const long long ii = ((long long)(q0 + u) * gridDim.x + blockIdx.x) * U + threadIdx.x;
+                        inv[u] = (q0 + u < rm.rounds && ii < N) ? __ldcg(plane + ii) : 0.f;
+                    }
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const long long ii = ((long long)(q0 + u) * gridDim.x + blockIdx.x) * U + threadIdx.x;
+                        if (q0 + u < rm.rounds && ii < N) {
+                            const int idx = (q0 + u) * U + threadIdx.x, i = (int)ii;
+                            const PopDev* __restrict__ p = P + rm.pi[idx];
+                            plane[i] = 0.f;
+                            if (a.last_input) a.last_input[i] = inv[u];
+                            const int k = poisson_count(a, p, n, i);
+                            rm.I[idx] = fmaf(p->P11, rm.I[idx], inv[u]) + p->w_ext * (float)k;
+                        }
+                    }
                 }
             }
             trace_stamp(a, n, 6);
@@ -1453,7 +1496,7 @@ __global__ void __launch_bounds__(kPipeThreads) pipe_step_kernel(const StepArgs 
 }
 
 // kAdex: the AdEx integrator needs more than the 64 registers a 1024-thread CTA leaves: 512-thread CTAs, two per SM at most
-template <bool kAdex, bool kOneRound = false>
+template <bool kAdex, bool kOneRound = false, bool kResM = false>
 __global__ void __launch_bounds__(kAdex ? 512 : kPersistentThreads, kAdex ? 2 : 1) persistent_pipe_kernel(const StepArgs a, long long n_steps) {
     __shared__ PipeShared sh;
     if (threadIdx.x == 0) {
@@ -1464,7 +1507,7 @@ __global__ void __launch_bounds__(kAdex ? 512 : kPersistentThreads, kAdex ? 2 : 
     const PopDev* P = stage_pops(a, sh.pops);
     if (a.n_pops > kMaxPopsSmem) __syncthreads();
     const long long gtid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const int U = pipe_updater_threads(a.N, kAdex);
+    const int U = kResM ? (int)blockDim.x - kResMRest : pipe_updater_threads(a.N, kAdex);
     const bool single_round = kOneRound;                           // else the counts are computed in line, overlapping the loads
     constexpr bool kRes = !kAdex && kOneRound;                     // LIF state resident in shared memory (the host never
     const long long res_i = (long long)blockIdx.x * U + threadIdx.x;       // picks this instantiation in bypass mode)
@@ -1473,13 +1516,27 @@ __global__ void __launch_bounds__(kAdex ? 512 : kPersistentThreads, kAdex ? 2 : 
         sh.res_V[t] = a.V[res_i]; sh.res_I[t] = a.I[res_i]; sh.res_r[t] = a.refr[res_i]; sh.res_pi[t] = a.pop_of[res_i];
         sh.res_row[t] = ld_row_info(a.row_info + res_i);
     }
+    ResM rm{};
+    if constexpr (kResM) {
+        extern __shared__ __align__(16) unsigned char res_dyn[];   // V, I_syn, refr, population byte of the CTA's neurons
+        const long long per_round = (long long)gridDim.x * U;
+        rm.rounds = (int)((a.N + per_round - 1) / per_round);
+        const size_t cap = (size_t)rm.rounds * U;
+        rm.V = reinterpret_cast<float*>(res_dyn); rm.I = rm.V + cap;
+        rm.r = reinterpret_cast<int32_t*>(rm.I + cap); rm.pi = reinterpret_cast<uint8_t*>(rm.r + cap);
+        if ((int)threadIdx.x < U)
+            for (int q = 0; q < rm.rounds; ++q) {
+                const long long ii = ((long long)q * gridDim.x + blockIdx.x) * U + threadIdx.x;
+                if (ii < a.N) { const int k = q * U + threadIdx.x; rm.V[k] = a.V[ii]; rm.I[k] = a.I[ii]; rm.r[k] = a.refr[ii]; rm.pi[k] = a.pop_of[ii]; }
+            }
+    }
     long long n = sh.sc.n;
     int slot = sh.sc.slot;
     unsigned long long rec_prev = sh.sc.rec_base, spikes = 0, epoch = 0;       // recorded before step n-1 (nothing pending at entry)
     for (long long s = 0; s < n_steps; ++s, ++n) {
         if (gtid == 0) a.ctl->spike_cnt[(n + 1) & 3] = 0;          // last read (as step n-3's) in phase n-2
         trace_stamp(a, n, 0);
-        const int Mp = pipelined_phase<true, kAdex, kOneRound, kRes>(a, P, n, slot, s > 0, rec_prev, sh, U, s > 0 && single_round);
+        const int Mp = pipelined_phase<true, kAdex, kOneRound, kRes, kResM>(a, P, n, slot, s > 0, rec_prev, sh, U, s > 0 && single_round, rm);
         rec_prev += (unsigned long long)Mp; spikes += (unsigned long long)Mp;
         trace_stamp(a, n, 1);
         grid_arrive(a.ctl, epoch);
@@ -1499,6 +1556,11 @@ __global__ void __launch_bounds__(kAdex ? 512 : kPersistentThreads, kAdex ? 2 : 
         const int t = threadIdx.x;
         a.V[res_i] = sh.res_V[t]; a.I[res_i] = sh.res_I[t]; a.refr[res_i] = sh.res_r[t];
     }
+    if (kResM && (int)threadIdx.x < U)
+        for (int q = 0; q < rm.rounds; ++q) {
+            const long long ii = ((long long)q * gridDim.x + blockIdx.x) * U + threadIdx.x;
+            if (ii < a.N) { const int k = q * U + threadIdx.x; a.V[ii] = rm.V[k]; a.I[ii] = rm.I[k]; a.refr[ii] = rm.r[k]; }
+        }
     if (n_steps > 0) {                                             // flush: rest pass of the last step
         const int Mp = pipelined_phase<false, kAdex>(a, P, n, slot, true, rec_prev, sh, U);
         rec_prev += (unsigned long long)Mp; spikes += (unsigned long long)Mp;

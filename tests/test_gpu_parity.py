@@ -154,6 +154,46 @@ def test_cfg0_launch_boundaries_are_invisible(B, mode, kernel):
     assert np.mean(a[3] == b[3]) >= 0.99
 
 
+def test_multi_round_resident_state(oracle_mod, B):
+    """A network that needs several rounds of updater threads per step (config 4's shape; here 200,000 neurons = two
+    rounds on 148 CTAs, the second one ragged) keeps its LIF state in dynamic shared memory for a whole persistent launch
+    (kResM).  (a) The first steps agree with the oracle spike for spike — step 0 carries the initial volley of ~4e4
+    spikes; (b) launch boundaries, with a state round trip in between, are invisible."""
+    wl = W.balanced_large(n=200_000, k_total=50, n_steps=60)
+    o, g = make_pair(wl, oracle_mod, debug_input=False)
+    assert g.stats is not None
+    g.simulate(30); o.simulate(30)
+    gs, gi = g.get_spikes()
+    os_, oi = o.get_spikes()
+    a = sorted(zip(gs.tolist(), gi.tolist())); b = sorted(zip(os_.tolist(), oi.tolist()))
+    assert len(b) > 30_000
+    diff = set(a) ^ set(b)
+    assert len(diff) <= 3, sorted(diff)[:10]                       # fp32 vs fp64 within 1e-4 mV of threshold (C11)
+    gV = g.get_state(B.FIELD_V).astype(np.float64); oV = o.get_state(oracle_mod.FIELD_V)
+    gI = g.get_state(B.FIELD_I_SYN).astype(np.float64); oI = o.get_state(oracle_mod.FIELD_I_SYN)
+    assert np.mean(np.abs(gV - oV) <= 1e-3) >= 0.999 and np.mean(np.abs(gI - oI) <= 1e-3 * (1.0 + np.abs(oI))) >= 0.999
+    g.close()
+
+    def run(chunks, roundtrip):
+        g = B.Sim(0.1, wl.ring_slots, wl.seed, record_spikes=True)
+        wl.apply(g); g.prepare(); g.set_state(B.FIELD_V, wl.initial_v())
+        for c in chunks:
+            g.simulate(c)
+            if roundtrip:
+                for f in (B.FIELD_V, B.FIELD_I_SYN, B.FIELD_REFR):
+                    g.set_state(f, g.get_state(f))
+        st, ids = g.get_spikes()
+        out = (set(zip(st.tolist(), ids.tolist())), g.get_state(B.FIELD_V), g.get_state(B.FIELD_REFR), g.stats().steps)
+        g.close()
+        return out
+
+    x = run([60], False)
+    y = run([1, 7, 20, 32], True)
+    assert x[3] == y[3] == 60
+    assert len(x[0] ^ y[0]) <= 3, sorted(x[0] ^ y[0])[:10]
+    assert np.mean(np.abs(x[1] - y[1]) <= 1e-3) >= 0.999 and np.mean(x[2] == y[2]) >= 0.999
+
+
 # ------------------------------------------------------------------------------------------------------------
 # microcircuit-shaped nets (normal weights and delays, 8 populations, up to 54 connect calls)
 # ------------------------------------------------------------------------------------------------------------
