@@ -234,6 +234,8 @@ def run_ours(args):
     wl = make_workload(args.workload, seed_offset=rank)       # replicas: independent seeds, no exchange
     g = B.Sim(DT_MS, wl.ring_slots, wl.seed, record_spikes=True, max_recorded_spikes=1 << 24, device=local)
     wl.apply(g)
+    if args.delivery_kernel == 4:
+        g.set_option(B.OPT_DELIVERY_KERNEL, 4)                # before prepare: the spike-buffer backend changes what is allocated
     t0 = time.time(); g.prepare(); build_wall = time.time() - t0
     g.set_option(B.OPT_STEP_MODE, args.step_mode)
     g.set_option(B.OPT_DELIVERY_KERNEL, args.delivery_kernel)
