@@ -30,6 +30,7 @@ import numpy as np
 TIME_STEPS_PER_BENCH_STEP = 1000
 DT_MS = 0.1
 NCU_DRAM_BYTES_PER_LAUNCH_CFG2 = 895.8e6     # profiles/r01f_cfg2_full_summary.csv
+NCU_DRAM_BYTES_PER_LAUNCH_CFG4 = 36.33e9     # profiles/r01h_cfg4_full_summary.csv (13.5 GB read + 22.8 GB written)
 PAPER_RTF_2080TI = 1.055          # PAPER.md:248, full-scale microcircuit, NeuronGPU on RTX 2080 Ti (context, other hardware)
 PAPER_RTF_ADEX_1M = 70.0          # PAPER.md:16, balanced network of 1e6 AdEx neurons / 1e9 synapses on an RTX 2080 Ti (context)
 BYTES_PER_EVENT = 8               # 4 B target + 4 B weight per synaptic event
@@ -321,7 +322,9 @@ def run_ours(args):
     # dram__bytes_read.sum + dram__bytes_write.sum of one launch of this kernel in this configuration, from the committed
     # `ncu --set full` capture (profiles/r01f_cfg2_full_summary.csv: 890.4 MB + 5.4 MB per 1000 time steps); below the
     # algorithmic bytes because the 33 B per neuron-step never leave the chip (state resident in shared memory / L2)
-    traffic = NCU_DRAM_BYTES_PER_LAUNCH_CFG2 if (args.workload == "cfg2" and kern == "persistent_pipe_kernel" and T == 1000) else None
+    traffic = None
+    if kern == "persistent_pipe_kernel" and T == 1000 and args.delivery_kernel in (0, 3):
+        traffic = {"cfg2": NCU_DRAM_BYTES_PER_LAUNCH_CFG2, "cfg4": NCU_DRAM_BYTES_PER_LAUNCH_CFG4}.get(args.workload)
     roofline = {"bound": "hbm", "kernel": kern, "achieved": achieved, "peak": peak_gbs, "unit": "GB/s",
                 "frac": achieved / peak_gbs, "traffic": traffic, "peak_source": peak_src,
                 "avg_launch_us": us, "algorithmic_bytes_per_launch": alg_bytes,
