@@ -212,12 +212,6 @@ def run_probes(device=0):
     for mb in (4, 16, 64, 256):
         out[f"scattered_red_per_s_{mb}MB"] = B.probe(1, mb << 20, device)
         out[f"records_plus_red_events_per_s_{mb}MB"] = B.probe(2, mb << 20, device)
-    for cs in (1, 2, 4, 8, 16):                 # reduction target in the distributed shared memory of a cs-CTA cluster (200 KB per CTA)
-        out[f"dsmem_red_per_s_cluster{cs}"] = B.probe(3, cs * 200 * 1024, device)
-        out[f"dsmem_plus_global_red_per_s_cluster{cs}"] = B.probe(4, cs * 200 * 1024, device)
-    out["tiled_delivery_shape_events_per_s"] = B.probe(5, 200 * 1024, device)
-    for K in (100, 1000):                       # append half of a per-delay event queue, rows of K records
-        out[f"queue_append_events_per_s_K{K}"] = B.probe(6, 8 * K, device)
     return out
 
 

@@ -290,15 +290,6 @@ int32_t ng_get_trace(ng_sim* sim, uint64_t* out_host, int64_t capacity, int64_t*
  *   kind 0: a coalesced 128-bit read stream over 2 GiB                        -> bytes per second
  *   kind 1: red.global.add.f32 to uniformly random cells of a footprint_bytes array -> reductions per second
  *   kind 2: streamed 8-byte records + one random reduction per record (the shape of a3) -> events per second
- *   kind 3: red.shared::cluster.add.f32 to uniformly random cells of a footprint_bytes plane spread over the shared
- *           memory of one thread-block cluster (200 KB per CTA, so footprint_bytes <= 3,276,800 = 16 CTAs)  -> reductions per second
- *   kind 4: kind 3 alternating with red.global.add.f32 into a 4 MB plane (whether the two paths add up) -> reductions per second
- *   kind 5: the access shape of a target-tiled delivery: per item one dependent 4-byte lookup in a 256 MB table, then an
- *           8-record run (32 B targets + 32 B weights, random place in 2 GiB) reduced into the CTA's own shared-memory tile
- *           of footprint_bytes (<= 200 KB)                                                     -> events per second
- *   kind 6: the append half of a per-delay event queue: whole source rows of footprint_bytes (8 x out-degree, >= 64) read
- *           coalesced at random places in 2 GiB, binned by delay in shared memory, appended as (target, weight) pairs to
- *           64 global queues with one atomic per (4096-record batch, delay)                       -> events per second
  * Allocates its own scratch with cudaMalloc and frees it.  Errors: INVALID_ARG, OOM, CUDA. */
 int32_t ng_probe(int32_t device, int32_t kind, int64_t footprint_bytes, double* per_second_out);
 

@@ -231,6 +231,9 @@ int prepare(Sim& s) {
     const int32_t N = s.N;
     // 1. draw every connection in call order, endpoint ascending, k ascending
     s.conns.clear();
+    size_t total = 0;                     // storage only: one allocation instead of doubling (1e9 records at config 4)
+    for (const ConnectCall& c : s.calls) total += (size_t)((c.rule == RULE_FIXED_INDEGREE) ? c.tgt_n : c.src_n) * (size_t)c.K;
+    s.conns.reserve(total);
     for (int32_t ci = 0; ci < (int32_t)s.calls.size(); ++ci) {
         const ConnectCall& c = s.calls[ci];
         int32_t e_first = (c.rule == RULE_FIXED_INDEGREE) ? c.tgt_first : c.src_first;

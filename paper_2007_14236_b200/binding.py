@@ -134,10 +134,7 @@ def load_library(path: str | None = None):
 
 
 def probe(kind: int, footprint_bytes: int = 4 << 20, device: int = 0) -> float:
-    """ng_probe: kind 0 stream bytes/s, 1 scattered reductions/s, 2 streamed records + reductions events/s,
-    3 cluster shared-memory reductions/s, 4 the same alternating with global reductions,
-    5 target-tiled delivery shape (lookup + 8-record run + own-tile shared-memory reductions) events/s,
-    6 event-queue append shape (footprint_bytes = bytes of one source row) events/s."""
+    """ng_probe: kind 0 stream bytes/s, 1 scattered reductions/s, 2 streamed records + reductions events/s."""
     out = C.c_double()
     rc = load_library().ng_probe(device, kind, footprint_bytes, C.byref(out))
     if rc != NG_OK:

@@ -185,7 +185,7 @@ void launch_pipe(ng_sim* s) {
     else if (s->one_round_step) pipe_step_kernel<true, false, true><<<s->pipe_blocks, kPipeThreads, 0, s->stream>>>(s->a);
     else pipe_step_kernel<true, false, false><<<s->pipe_blocks, kPipeThreads, 0, s->stream>>>(s->a);
 }
-// rest pass of the last step of an ng_simulate call (delivery kernel 4): leaves nothing pending between API calls
+// rest pass of the last step of an ng_simulate call (pipelined delivery kernel 3): leaves nothing pending between API calls
 void launch_pipe_flush(ng_sim* s) {
     if (s->has_adex) pipe_step_kernel<false, true><<<s->pipe_blocks, kPipeThreads, 0, s->stream>>>(s->a);
     else pipe_step_kernel<false, false><<<s->pipe_blocks, kPipeThreads, 0, s->stream>>>(s->a);
@@ -484,6 +484,7 @@ int32_t ng_set_option(ng_sim* s, int32_t option, int64_t value) {
             s->sort_segments = value ? 1 : 0; break;
         case NG_OPT_TRACE:
             if (value && !s->prepared) return fail(s, NG_ERR_STATE, "NG_OPT_TRACE before ng_prepare");
+            if (value && !s->a.trace && s->trace_saved) { s->a.trace = s->trace_saved; s->trace_saved = nullptr; }   // switched back on
             if (value && !s->a.trace) {
                 const size_t words = (size_t)kTraceSteps * (size_t)s->sm_count * 32 * kTraceStamps;
                 if (!dev_alloc_t(s, &s->a.trace, words)) return fail(s, NG_ERR_OOM, "trace buffer");
@@ -491,7 +492,6 @@ int32_t ng_set_option(ng_sim* s, int32_t option, int64_t value) {
                 s->trace_on = true;
             }
             if (!value && s->a.trace) { s->trace_saved = s->a.trace; s->a.trace = nullptr; }
-            else if (value && !s->a.trace) s->a.trace = s->trace_saved;
             break;
         case NG_OPT_PERSISTENT_THREADS:
             if (value != 512 && value != 1024) return fail(s, NG_ERR_INVALID_ARG, "persistent threads: 512 or 1024");
@@ -518,6 +518,15 @@ int32_t ng_prepare(ng_sim* s) {
     s->has_adex = false;
     for (const HostPop& hp : s->pops) s->has_adex = s->has_adex || hp.dev.model == 1;
     s->NR = (int64_t)N * (s->has_adex ? 2 : 1);
+    // Receptor port 1 is the inhibitory conductance of AdEx neurons: it exists only in networks with an AdEx population
+    // (two-port ring planes), and only AdEx targets read it — a LIF target would silently drop such input.
+    for (const CallDev& c : s->calls) {
+        if (c.port != 1) continue;
+        if (!s->has_adex) return fail(s, NG_ERR_INVALID_ARG, "receptor port 1 needs an AdEx population (LIF-only network has one port)");
+        for (const HostPop& hp : s->pops)
+            if (hp.dev.model != 1 && hp.first < c.tgt_first + c.tgt_n && c.tgt_first < hp.first + hp.n)
+                return fail(s, NG_ERR_INVALID_ARG, "receptor port 1 onto a target range that holds LIF neurons (they have one port)");
+    }
     const size_t NRs = (size_t)s->NR;
     s->S = 0;
     for (const CallDev& c : s->calls) s->S += (int64_t)(c.rule == kRuleIndegree ? c.tgt_n : c.src_n) * c.K;
@@ -611,9 +620,14 @@ int32_t ng_prepare(ng_sim* s) {
                                                                    s->d_row_off, s->d_grp_rel, s->d_tgt, s->d_w, s->d_dly, N);
         s->launches_other++;
     }
+    long long* d_long = nullptr;
     if (s->sort_segments) {
-        build_sort_groups_kernel<<<s->sm_count * 8, 256, 0, st>>>(N, D, s->d_row_off, s->d_grp_rel, s->d_tgt, s->d_w);
-        s->launches_other++;
+        // groups beyond the warp sort's shared-memory tile go to a list; there are at most S / kSortMax of them
+        const uint32_t long_cap = (uint32_t)std::min<int64_t>(s->S / kSortMax + 1, 0x7fffffff);
+        if (!dev_alloc_t(s, &d_long, (size_t)long_cap)) return fail(s, NG_ERR_OOM, "device allocation failed (long-group list)");
+        build_sort_groups_kernel<<<s->sm_count * 8, 256, 0, st>>>(N, D, s->d_row_off, s->d_grp_rel, s->d_tgt, s->d_w, d_long, long_cap, s->d_ctl);
+        build_sort_long_groups_kernel<<<s->sm_count * 2, 1024, 0, st>>>(D, s->d_row_off, s->d_grp_rel, s->d_tgt, s->d_w, d_long, long_cap, s->d_ctl);
+        s->launches_other += 2;
     }
     NG_CUDA(s, cudaEventRecord(e1, st));
     NG_CUDA(s, cudaStreamSynchronize(st));
@@ -625,6 +639,7 @@ int32_t ng_prepare(ng_sim* s) {
     // the per-(source, delay) counters and the row lengths are builder scratch
     dev_free(s, s->d_cnt); s->d_cnt = nullptr;
     dev_free(s, s->d_row_len); s->d_row_len = nullptr;
+    dev_free(s, d_long);
 
     // ---- step arguments ----
     s->a.NR = (int32_t)s->NR; s->a.dt_ms = (float)s->cfg.dt_ms; s->a.has_adex = s->has_adex ? 1 : 0;
@@ -988,7 +1003,7 @@ int32_t ng_get_trace(ng_sim* s, uint64_t* out_host, int64_t capacity, int64_t* c
 
 // ng_probe: see include/ng.h.  Allocates with cudaMalloc, runs on the legacy stream, frees everything.
 extern "C" int32_t ng_probe(int32_t device, int32_t kind, int64_t footprint_bytes, double* per_second_out) {
-    if (!per_second_out || kind < 0 || kind > 6 || footprint_bytes < (kind == 6 ? 64 : 4096)) return NG_ERR_INVALID_ARG;
+    if (!per_second_out || kind < 0 || kind > 2 || footprint_bytes < 4096) return NG_ERR_INVALID_ARG;
     if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return NG_ERR_CUDA; }
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return NG_ERR_CUDA;
@@ -1017,66 +1032,6 @@ extern "C" int32_t ng_probe(int32_t device, int32_t kind, int64_t footprint_byte
             probe_red_kernel<<<blocks, thr>>>(ring, M, 2000);
             cudaEventRecord(e1);
             units = (double)blocks * thr * 2000;                        // reductions
-        } else if (kind == 6) {
-            const uint32_t K = (uint32_t)std::min<int64_t>(footprint_bytes / 8, 4096), cap_mask = (1u << 22) - 1;   // 64 queues x 4 Mi events
-            const uint32_t n_rows = (uint32_t)(n_rec / K);
-            const int grid = prop.multiProcessorCount, batches = 64;
-            unsigned long long* tails = nullptr; int2* queues = nullptr;
-            if (cudaMalloc(&tgt, n_rec * 4) != cudaSuccess || cudaMalloc(&w, n_rec * 4) != cudaSuccess ||
-                cudaMalloc(&ring, 64 * 128) != cudaSuccess) { rc = NG_ERR_OOM; break; }
-            if (cudaMalloc(&queues, (size_t)64 * (cap_mask + 1) * 8) != cudaSuccess) { rc = NG_ERR_OOM; break; }
-            tails = (unsigned long long*)ring;
-            cudaMemset(tails, 0, 64 * 128); cudaMemset(w, 0, n_rec * 4);
-            probe_fill_targets_kernel<<<blocks, thr>>>(tgt, n_rec, 1000000u);
-            probe_queue_append_kernel<<<grid, 1024>>>(tgt, w, n_rows, K, tails, queues, cap_mask, 4);
-            cudaEventRecord(e0);
-            probe_queue_append_kernel<<<grid, 1024>>>(tgt, w, n_rows, K, tails, queues, cap_mask, batches);
-            cudaEventRecord(e1);
-            units = (double)grid * batches * 4096;                      // events appended
-            if (cudaDeviceSynchronize() != cudaSuccess) rc = NG_ERR_CUDA;
-            else { cudaEventElapsedTime(&ms, e0, e1); *per_second_out = units / (ms * 1e-3); }
-            cudaFree(queues);
-            break;
-        } else if (kind == 5) {
-            const uint32_t n_offs = 1u << 26, tile = (uint32_t)std::min<int64_t>(footprint_bytes / 4, 50 * 1024);
-            const int grid = prop.multiProcessorCount, cthr = 1024, per = 2000;
-            uint32_t* offs = nullptr;
-            if (cudaMalloc(&ring, (size_t)n_offs * 4) != cudaSuccess || cudaMalloc(&tgt, n_rec * 4) != cudaSuccess ||
-                cudaMalloc(&w, n_rec * 4) != cudaSuccess) { rc = NG_ERR_OOM; break; }
-            offs = (uint32_t*)ring;
-            cudaMemset(w, 0, n_rec * 4);
-            probe_fill_targets_kernel<<<blocks, thr>>>(tgt, n_rec, 1000000u);
-            probe_fill_targets_kernel<<<blocks, thr>>>((int32_t*)offs, n_offs, (uint32_t)(n_rec / 8));
-            cudaFuncSetAttribute(probe_tiled_deliver_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(tile * 4));
-            probe_tiled_deliver_kernel<<<grid, cthr, tile * 4>>>(offs, n_offs, tgt, w, tile, 100, (float*)sink);
-            cudaEventRecord(e0);
-            probe_tiled_deliver_kernel<<<grid, cthr, tile * 4>>>(offs, n_offs, tgt, w, tile, per, (float*)sink);
-            cudaEventRecord(e1);
-            units = (double)grid * cthr * per;                          // events (8 lanes x one run each per item)
-        } else if (kind >= 3) {
-            // plane of footprint_bytes spread over the shared memory of one cluster: 200 KB per CTA, 1..16 CTAs (power of two)
-            const int64_t tile_bytes = 200 * 1024;
-            unsigned csize = 1;
-            while ((int64_t)csize * tile_bytes < footprint_bytes && csize < 32) csize *= 2;
-            if (csize > 16) { rc = NG_ERR_INVALID_ARG; break; }
-            const uint32_t tile = (uint32_t)((footprint_bytes / 4 + csize - 1) / csize), Mg = 1000000;   // global plane: 4 MB
-            const int grid = prop.multiProcessorCount / (int)csize * (int)csize, cthr = 1024, per = 2000;
-            if (cudaMalloc(&ring, (size_t)Mg * 4) != cudaSuccess) { rc = NG_ERR_OOM; break; }
-            cudaMemset(ring, 0, (size_t)Mg * 4);
-            auto kern = kind == 3 ? probe_dsmem_red_kernel<false> : probe_dsmem_red_kernel<true>;
-            cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(tile * 4));
-            cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
-            cudaLaunchConfig_t lc = {};
-            lc.gridDim = dim3(grid); lc.blockDim = dim3(cthr); lc.dynamicSmemBytes = (size_t)tile * 4;
-            cudaLaunchAttribute at[1];
-            at[0].id = cudaLaunchAttributeClusterDimension;
-            at[0].val.clusterDim.x = csize; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
-            lc.attrs = at; lc.numAttrs = 1;
-            if (cudaLaunchKernelEx(&lc, kern, ring, Mg, tile, (uint32_t)csize, 100) != cudaSuccess) { rc = NG_ERR_CUDA; break; }
-            cudaEventRecord(e0);
-            if (cudaLaunchKernelEx(&lc, kern, ring, Mg, tile, (uint32_t)csize, per) != cudaSuccess) { rc = NG_ERR_CUDA; break; }
-            cudaEventRecord(e1);
-            units = (double)grid * cthr * per;                          // reductions
         } else {
             if (cudaMalloc(&ring, (size_t)M * 4) != cudaSuccess || cudaMalloc(&tgt, n_rec * 4) != cudaSuccess ||
                 cudaMalloc(&w, n_rec * 4) != cudaSuccess) { rc = NG_ERR_OOM; break; }

@@ -65,6 +65,7 @@ struct Ctl {
     int32_t slot_d;                        // step_d mod Dr: written by update, read by deliver (like step_d) — the delivery
                                            // kernel's bookkeeping advances `slot` while later CTAs of the same launch still start
     int32_t err_window;                    // spike-buffer backend: the spike window overflowed its capacity
+    uint32_t n_long_groups;                // builder: (source, delay) groups longer than kSortMax, listed for the CTA-wide sort
     // line 1: spike counters (atomics of the appending warps / CTAs)
     alignas(128) int32_t spike_cnt[4];     // length of the spike array of step n, indexed n & 3 (the list itself by n & 1)
     // line 2: event counter (one atomic per CTA and step)
@@ -296,11 +297,13 @@ build_fill_kernel(const CallDev* __restrict__ calls, int call_idx, uint32_t seed
 // Order the records of every (source, delay) group by (target, weight bits): the fill order above depends on
 // atomic arrival order; after this pass the structure is a deterministic function of the seed.
 // One warp per group; groups are short (1..~1e3 records), so an in-place odd-even transposition over
-// lane-strided elements is enough.  Groups longer than kSortMax records are left as filled.
+// lane-strided elements is enough.  Groups longer than kSortMax records (out-degree >= 1000 with a constant delay,
+// say) are listed in `long_list` and sorted by build_sort_long_groups_kernel, one CTA each.
 constexpr int kSortMax = 768;    // 8 warps x 768 x 8 B = 48 KB of static shared memory
 __global__ void __launch_bounds__(256)
 build_sort_groups_kernel(int N, int D, const long long* __restrict__ row_off, const uint32_t* __restrict__ grp_rel,
-                         int32_t* __restrict__ tgt, float* __restrict__ w) {
+                         int32_t* __restrict__ tgt, float* __restrict__ w, long long* __restrict__ long_list,
+                         uint32_t long_cap, Ctl* __restrict__ ctl) {
     __shared__ unsigned long long keys[8][kSortMax];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const long long n_groups = (long long)N * D;
@@ -309,7 +312,11 @@ build_sort_groups_kernel(int N, int D, const long long* __restrict__ row_off, co
         const int j = (int)(g / D), d = (int)(g % D);
         const uint32_t a = grp_rel[(size_t)j * (D + 1) + d], b = grp_rel[(size_t)j * (D + 1) + d + 1];
         const int len = (int)(b - a);
-        if (len < 2 || len > kSortMax) continue;
+        if (len < 2) continue;
+        if (len > kSortMax) {
+            if (lane == 0) { const uint32_t k = atomicAdd(&ctl->n_long_groups, 1u); if (k < long_cap) long_list[k] = g; }
+            continue;
+        }
         const long long base = row_off[j] + a;
         unsigned long long* K = keys[wib];
         for (int i = lane; i < len; i += 32)
@@ -327,6 +334,46 @@ build_sort_groups_kernel(int N, int D, const long long* __restrict__ row_off, co
             w[base + i] = __uint_as_float((uint32_t)K[i]);
         }
         __syncwarp();
+    }
+}
+
+// Long groups: one CTA per listed group sorts it in place in global memory with a bitonic network whose merges all run
+// in ascending direction (first stage of a merge of size k pairs i with i ^ (k - 1), the others i with i ^ j), so a
+// length that is not a power of two needs no padding: the cells beyond the end behave as +infinity and never move.
+__global__ void __launch_bounds__(1024)
+build_sort_long_groups_kernel(int D, const long long* __restrict__ row_off, const uint32_t* __restrict__ grp_rel,
+                              int32_t* __restrict__ tgt, float* __restrict__ w, const long long* __restrict__ long_list,
+                              uint32_t long_cap, const Ctl* __restrict__ ctl) {
+    const uint32_t n_long = min(ctl->n_long_groups, long_cap);
+    for (uint32_t k = blockIdx.x; k < n_long; k += gridDim.x) {
+        const long long g = long_list[k];
+        const int j = (int)(g / D), d = (int)(g % D);
+        const uint32_t a = grp_rel[(size_t)j * (D + 1) + d], b = grp_rel[(size_t)j * (D + 1) + d + 1];
+        const uint32_t len = b - a;
+        int32_t* __restrict__ T = tgt + row_off[j] + a;
+        float* __restrict__ W = w + row_off[j] + a;
+        auto cmpx = [&](uint32_t i, uint32_t l) {              // ascending compare-exchange of cells i < l < len
+            const unsigned long long x = ((unsigned long long)(uint32_t)T[i] << 32) | __float_as_uint(W[i]);
+            const unsigned long long y = ((unsigned long long)(uint32_t)T[l] << 32) | __float_as_uint(W[l]);
+            if (x > y) {
+                T[i] = (int32_t)(uint32_t)(y >> 32); W[i] = __uint_as_float((uint32_t)y);
+                T[l] = (int32_t)(uint32_t)(x >> 32); W[l] = __uint_as_float((uint32_t)x);
+            }
+        };
+        for (uint32_t kk = 2; (kk >> 1) < len; kk <<= 1) {
+            for (uint32_t i = threadIdx.x; i < len; i += blockDim.x) {
+                const uint32_t l = i ^ (kk - 1);
+                if (l > i && l < len) cmpx(i, l);
+            }
+            __syncthreads();
+            for (uint32_t jj = kk >> 2; jj > 0; jj >>= 1) {
+                for (uint32_t i = threadIdx.x; i < len; i += blockDim.x) {
+                    const uint32_t l = i ^ jj;
+                    if (l > i && l < len) cmpx(i, l);
+                }
+                __syncthreads();
+            }
+        }
     }
 }
 
@@ -408,7 +455,7 @@ __device__ __forceinline__ void stat_on_spike(const StepArgs& a, int i, long lon
 __device__ __forceinline__ void prefetch_row(const StepArgs& a, const RowInfo& r) {
     const int len = padded_len(r.deg);
     const long long bytes4 = (long long)len * 4;
-    const uint32_t head = (uint32_t)(((long long)r.d1 * 4 + 15) & ~15LL);      // delay-1 records: needed first (kernel 4)
+    const uint32_t head = (uint32_t)(((long long)r.d1 * 4 + 15) & ~15LL);      // delay-1 records: needed first (pipelined kernel 3)
     if (head > 0 && head < 32768) {
         prefetch_l2_bulk(reinterpret_cast<const char*>(a.tgt + r.r0), head);
         prefetch_l2_bulk(reinterpret_cast<const char*>(a.w + r.r0), head);
@@ -1016,7 +1063,7 @@ struct StepScalars { long long n; unsigned long long rec_base; int M; int slot; 
 constexpr int kPersistentThreads = 1024;
 
 // ---------------------------------------------------------------------------------------
-// Delivery kernel 4: the pipelined step — ONE grid-wide dependency per time step instead of two.
+// Delivery kernel 3: the pipelined step — ONE grid-wide dependency per time step instead of two.
 //   Only the delay-1 records of a spike of step n must land before update(n+1) starts; every other record
 //   (delay d >= 2, slot n+d) is not consumed before step n+2.  A step is therefore cut differently:
 //     phase n = [ update(n), then the CTA delivers the delay-1 records of ITS OWN spikes ]   (critical path)
@@ -1806,97 +1853,6 @@ __global__ void probe_deliver_kernel(const int4* __restrict__ tgt, const float4*
         const float4 ww = ld_stream_f32x4((const float*)(w + i));
         red_add_f32(ring + t.x, ww.x); red_add_f32(ring + t.y, ww.y);
         red_add_f32(ring + t.z, ww.z); red_add_f32(ring + t.w, ww.w);
-    }
-}
-// kinds 3, 4: the reduction target held in the distributed shared memory of a thread-block cluster (`tile` cells per CTA,
-// csize CTAs): `per_thread` red.shared::cluster.add.f32 per thread to uniformly random cells of the cluster's plane;
-// kMix alternates them with red.global.add.f32 into ring[0..M) (do the two reduction paths add up?)
-template <bool kMix>
-__global__ void probe_dsmem_red_kernel(float* ring, uint32_t M, uint32_t tile, uint32_t csize, int per_thread) {
-    extern __shared__ float probe_tile[];
-    for (uint32_t i = threadIdx.x; i < tile; i += blockDim.x) probe_tile[i] = 0.f;
-    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
-    const uint32_t base = (uint32_t)__cvta_generic_to_shared(probe_tile), cells = tile * csize;
-    uint32_t s = probe_hash((blockIdx.x * blockDim.x + threadIdx.x) * 2654435761u + 1u);
-    for (int i = 0; i < per_thread; ++i) {
-        s = s * 1664525u + 1013904223u;
-        const uint32_t r = probe_hash(s);
-        if (kMix && (i & 1)) { red_add_f32(ring + __umulhi(r, M), 1.0f); continue; }
-        const uint32_t c = __umulhi(r, cells), rank = c / tile;
-        uint32_t remote;
-        asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(base + (c - rank * tile) * 4u), "r"(rank));
-        asm volatile("red.shared::cluster.add.f32 [%0], %1;" ::"r"(remote), "f"(1.0f) : "memory");
-    }
-    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
-    if (probe_tile[threadIdx.x % tile] == -1.f) ring[0] = 1.f;
-}
-// kind 5: the access shape of a target-tiled delivery (item 0): per work item one dependent 4-byte
-// lookup in a 256 MB offset table, then an 8-record run (32 B of targets + 32 B of weights at a random 32-byte-aligned
-// place in 2 GiB of records) read by 8 lanes and reduced into the CTA's own shared-memory tile
-__global__ void probe_tiled_deliver_kernel(const uint32_t* __restrict__ offs, uint32_t n_offs, const int32_t* __restrict__ tgt,
-                                           const float* __restrict__ w, uint32_t tile, int per_group, float* sink) {
-    extern __shared__ float probe_tile[];
-    for (uint32_t i = threadIdx.x; i < tile; i += blockDim.x) probe_tile[i] = 0.f;
-    __syncthreads();
-    const uint32_t base = (uint32_t)__cvta_generic_to_shared(probe_tile), lane8 = threadIdx.x & 7;
-    uint32_t s = probe_hash(((blockIdx.x * blockDim.x + threadIdx.x) >> 3) * 2654435761u + 1u);
-    for (int i = 0; i < per_group; i += 4) {
-        uint32_t run[4]; int32_t t[4]; float ww[4];
-#pragma unroll
-        for (int u = 0; u < 4; ++u) { s = s * 1664525u + 1013904223u; run[u] = __ldg(offs + __umulhi(probe_hash(s), n_offs)); }
-#pragma unroll
-        for (int u = 0; u < 4; ++u) { t[u] = __ldg(tgt + (size_t)run[u] * 8 + lane8); ww[u] = __ldg(w + (size_t)run[u] * 8 + lane8); }
-#pragma unroll
-        for (int u = 0; u < 4; ++u)
-            asm volatile("red.shared::cta.add.f32 [%0], %1;" ::"r"(base + ((uint32_t)t[u] % tile) * 4u), "f"(ww[u]) : "memory");
-    }
-    __syncthreads();
-    if (probe_tile[threadIdx.x % tile] == -1.f) *sink = 1.f;
-}
-// kind 6: the append half of a per-delay event queue (item 0): a CTA takes batches of 4096 records
-// from whole source rows of K records at random places in 2 GiB (coalesced), bins them by delay (64 delays, rows
-// delay-grouped: record r of a row has delay r*64/K) in shared memory, claims a range in each of 64 global queues with
-// one atomic per (batch, delay) and stores (target, weight) pairs there; the drain half is kind 2
-__global__ void probe_queue_append_kernel(const int32_t* __restrict__ tgt, const float* __restrict__ w, uint32_t n_rows, uint32_t K,
-                                          unsigned long long* tails, int2* queues, uint32_t cap_mask, int batches) {
-    __shared__ uint32_t hist[64], base[64], sbase[65];
-    __shared__ int2 staged[4096];
-    if (threadIdx.x < 64) hist[threadIdx.x] = 0;
-    __syncthreads();
-    uint32_t seed = probe_hash(blockIdx.x * 2654435761u + 1u);
-    for (int b = 0; b < batches; ++b) {
-        int32_t t[4]; float ww[4]; uint32_t d[4], rank[4];
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            const uint32_t rec = threadIdx.x + u * 1024u, row_in_batch = rec / K, r = rec - row_in_batch * K;
-            const uint32_t row = __umulhi(probe_hash(seed + (uint32_t)b * 4099u + row_in_batch), n_rows);
-            t[u] = __ldg(tgt + (size_t)row * K + r); ww[u] = __ldg(w + (size_t)row * K + r);
-            d[u] = (uint32_t)(((unsigned long long)r * 64u) / K);
-        }
-#pragma unroll
-        for (int u = 0; u < 4; ++u) rank[u] = atomicAdd(&hist[d[u]], 1u);
-        __syncthreads();
-        if (threadIdx.x < 64) {                                    // exclusive scan of the 64 bins + one queue claim per bin
-            uint32_t acc = 0;
-            for (uint32_t k = 0; k < threadIdx.x; ++k) acc += hist[k];
-            sbase[threadIdx.x] = acc;
-            if (threadIdx.x == 63) sbase[64] = acc + hist[63];
-            base[threadIdx.x] = (uint32_t)atomicAdd(tails + threadIdx.x * 16, (unsigned long long)hist[threadIdx.x]);   // one 128-byte line per tail
-        }
-        __syncthreads();
-        if (threadIdx.x < 64) hist[threadIdx.x] = 0;
-#pragma unroll
-        for (int u = 0; u < 4; ++u) staged[sbase[d[u]] + rank[u]] = make_int2(t[u], __float_as_int(ww[u]));
-        __syncthreads();
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {                              // sorted by delay: consecutive threads store consecutive queue cells
-            const uint32_t p = threadIdx.x + u * 1024u;
-            uint32_t lo = 0;
-#pragma unroll
-            for (uint32_t step = 32; step > 0; step >>= 1) if (sbase[lo + step] <= p) lo += step;
-            queues[(size_t)lo * (cap_mask + 1u) + ((base[lo] + (p - sbase[lo])) & cap_mask)] = staged[p];
-        }
-        __syncthreads();
     }
 }
 __global__ void probe_fill_targets_kernel(int32_t* t, long long n, uint32_t M) {

@@ -172,7 +172,7 @@ def balanced_large(n=1_000_000, k_total=1000, n_steps=10000, seed=1) -> Workload
 # not in the paper (readings C23, C24)
 ADEX = dict(model="adex", C_m=281.0, g_L=30.0, E_L=-70.6, V_T=-50.4, Delta_T=2.0, tau_w=144.0, a=4.0, b=80.5, V_reset=-60.0,
             V_peak=0.0, E_ex=0.0, E_in=-85.0, tau_syn=1.0, I_e=0.0,
-            tol=(2e-4, 2e-3, 2e-5, 2e-4, 2e-5, 2e-4), h_min=1e-2)
+            tol=(2e-4, 2e-3, 2e-5, 2e-4, 2e-5, 2e-4), h_min=1e-3)
 
 
 def balanced_adex(n=1_000_000, k_total=1000, n_steps=10000, seed=1) -> Workload:

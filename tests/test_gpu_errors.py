@@ -65,3 +65,47 @@ def test_spike_record_overflow_keeps_simulating(B):
     g.simulate(2, allow_overflow=True)
     assert g.get_state(B.FIELD_STEP) == 7 and g.stats().events == g.stats().spikes * 10
     g.close()
+
+
+def test_receptor_port_1_needs_adex_targets(B):
+    """Port 1 is the inhibitory conductance of AdEx neurons.  In a LIF-only network the ring has one port, so a port-1
+    record would land in the next delay plane (or past the ring); onto LIF targets of a mixed network it would be dropped
+    silently.  Both are rejected by ng_prepare."""
+    g = B.Sim(0.1, 20, 1)
+    g.create_population(100, W.LIF | dict(poisson_rate_hz=800.0, poisson_weight=87.8))
+    g.connect_fixed_indegree(0, 100, 0, 100, 5, ("const", 1.0), ("uniform_int", 1, 20), port=1)
+    assert code(B, g.prepare) == B.NG_ERR_INVALID_ARG
+    g.close()
+    ax = dict(W.ADEX); ax.update(poisson_rate_hz=20000.0, poisson_weight=0.37)
+    g = B.Sim(0.1, 20, 1)
+    g.create_population(100, W.LIF | dict(poisson_rate_hz=800.0, poisson_weight=87.8))
+    g.create_population(100, ax)
+    g.connect_fixed_indegree(0, 200, 50, 150, 5, ("const", 0.35), ("uniform_int", 1, 20), port=1)     # targets 50..199: half LIF
+    assert code(B, g.prepare) == B.NG_ERR_INVALID_ARG
+    g.close()
+    g = B.Sim(0.1, 20, 1)
+    g.create_population(100, W.LIF | dict(poisson_rate_hz=800.0, poisson_weight=87.8))
+    g.create_population(100, ax)
+    g.connect_fixed_indegree(0, 200, 100, 100, 5, ("const", 0.35), ("uniform_int", 1, 20), port=1)    # AdEx targets only
+    g.connect_fixed_indegree(0, 200, 0, 100, 5, ("const", 50.0), ("uniform_int", 1, 20))
+    g.prepare()
+    g.simulate(30)
+    assert g.get_state(B.FIELD_STEP) == 30
+    g.close()
+
+
+def test_trace_option_can_be_switched_off_and_on(B):
+    wl = W.brunel_tiny(n_steps=50)
+    g = B.Sim(0.1, wl.ring_slots, wl.seed)
+    wl.apply(g); g.prepare()
+    before = None
+    for k in range(3):
+        g.set_option(B.OPT_TRACE, 1)
+        if before is None:
+            before = len(g._tensors)
+        assert len(g._tensors) == before               # the saved buffer is reused, nothing new is allocated
+        g.simulate(10)
+        assert g.trace().shape[0] == 64
+        g.set_option(B.OPT_TRACE, 0)
+        g.simulate(10)
+    g.close()

@@ -194,6 +194,37 @@ def test_multi_round_resident_state(oracle_mod, B):
     assert np.mean(np.abs(x[1] - y[1]) <= 1e-3) >= 0.999 and np.mean(x[2] == y[2]) >= 0.999
 
 
+def test_long_delay_groups_are_sorted_deterministically(oracle_mod, B):
+    """(source, delay) groups beyond the warp sort's 768-record tile (here: out-degree 2500 with ONE delay, and 1800 + 700
+    records per source over two delays in a second population) are sorted by a CTA-wide pass: the stored structure is a
+    deterministic function of the seed (two builds bit-identical, reading C18) and equals the oracle's canonical form."""
+    wl = W.Workload("long_groups", ring_slots=8, seed=7, n_steps=10)
+    lif = W.LIF | dict(poisson_rate_hz=0.0, poisson_weight=0.0)
+    wl.populations = [("A", 300, lif), ("B", 200, lif)]
+    wl.calls = [("out", 0, 0, 2500, ("normal", 87.8, 8.78), ("const", 3)),
+                ("out", 1, 0, 1800, ("normal", 87.8, 8.78), ("const", 5)),
+                ("out", 1, 1, 700, ("const", -351.2), ("const", 2)),
+                ("out", 1, 1, 40, ("const", 10.0), ("uniform_int", 1, 8))]
+    o, g = make_pair(wl, oracle_mod)
+    assert check_structure(g, o, max_weight_ulp_mismatch=4) <= 4
+    assert raw_layout_ok(g)
+    ro = g.row_offsets(); go = g.group_offsets().astype(np.int64); tgt, w, d = g.records()
+    n_long = 0
+    for j in range(wl.n_neurons):
+        for dd in range(wl.ring_slots):
+            a, b = ro[j] + go[j, dd], ro[j] + go[j, dd + 1]
+            if b - a > 768:
+                n_long += 1
+                key = (tgt[a:b].astype(np.int64) << 32) | w[a:b].view(np.uint32).astype(np.int64)
+                assert np.all(np.diff(key) >= 0), (j, dd)
+    assert n_long == 300 + 200
+    g2 = B.Sim(0.1, wl.ring_slots, wl.seed)
+    wl.apply(g2); g2.prepare()
+    t2, w2, d2 = g2.records()
+    assert np.array_equal(tgt, t2) and np.array_equal(w.view(np.uint32), w2.view(np.uint32)) and np.array_equal(d, d2)
+    g.close(); g2.close()
+
+
 # ------------------------------------------------------------------------------------------------------------
 # microcircuit-shaped nets (normal weights and delays, 8 populations, up to 54 connect calls)
 # ------------------------------------------------------------------------------------------------------------

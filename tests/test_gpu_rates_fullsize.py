@@ -1,0 +1,115 @@
+"""Free-running population firing rates at the sizes bench.py times, against the oracle (north_star: "free-running
+population firing rates agree within 5 % over 10 s of biological time"; 11 s simulated, the first second
+discarded).
+
+The oracle needs ~12 minutes for 11 s of the full-scale microcircuit and ~20 minutes for 1 s of the 1e6-neuron network,
+so its spike counts per population and per 100 ms window are stored (tests/golden/oracle_rates_cfg2.txt / _cfg4.txt,
+written by tests/golden/make_oracle_rates.py from oracle/ alone; tests/test_oracle_golden.py regenerates prefixes).
+The GPU runs the same seeded network in the default launch configuration (one persistent cooperative kernel per
+ng_simulate call, pipelined delivery kernel 3 — what bench.py times).
+
+  * window 0 (it holds the initial volley: both sides start from the same fp32 V) within 3 % per population;
+  * per population, the rate over the analysis interval within max(5 %, 0.1 Hz) of the oracle's (reading C17);
+  * the on-device statistics at the paper's own sample size — 200 neurons per population, 2 ms bins,
+    full scale — equal oracle/stats.py evaluated on the spike record of the same run.
+"""
+import os
+import sys
+
+import numpy as np
+import pytest
+
+from oracle import stats as S
+from paper_2007_14236_b200 import workloads as W
+
+sys.path.insert(0, os.path.join(os.path.dirname(__file__), "golden"))
+import make_oracle_rates as G  # noqa: E402
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2007_14236_b200 import binding
+    return binding
+
+
+def gpu_window_counts(g, wl, n_windows, ws, chunk_windows):
+    """Spike counts [n_windows, n_pops] of the free-running GPU simulation; returns them with the whole spike record."""
+    edges = np.array([r[0] for r in wl.pop_ranges()] + [wl.n_neurons])
+    counts = np.zeros((n_windows, len(wl.populations)), np.int64)
+    all_s, all_i = [], []
+    for k0 in range(0, n_windows, chunk_windows):
+        nw = min(chunk_windows, n_windows - k0)
+        g.simulate(nw * ws)                                   # ONE launch of nw * ws time steps
+        s, i = g.get_spikes()
+        all_s.append(s); all_i.append(i)
+        for k in range(k0, k0 + nw):
+            sel = (s >= k * ws) & (s < (k + 1) * ws)
+            counts[k] = np.histogram(i[sel], bins=edges)[0]
+    return counts, np.concatenate(all_s), np.concatenate(all_i)
+
+
+def compare_rates(wl, counts, ocounts, skip, ws, names):
+    sizes = np.array([p[1] for p in wl.populations], np.float64)
+    T = (counts.shape[0] - skip) * ws * 1e-4
+    rg = counts[skip:].sum(axis=0) / sizes / T
+    ro = ocounts[skip:].sum(axis=0) / sizes / T
+    for name, a, b in zip(names, rg, ro):
+        print(f"{name}: gpu {a:.4f} Hz, oracle {b:.4f} Hz, diff {100 * (a - b) / b:+.2f} %")
+    assert np.all(np.abs(rg - ro) <= np.maximum(0.05 * ro, 0.1)), (rg, ro)
+    return rg, ro
+
+
+def test_cfg2_free_running_rates_10s(B):
+    """BASELINE.json configs[2]: 77,169 neurons, 298,905,266 connections, 11 s simulated, rates over the last 10 s."""
+    ws, sizes, ocounts = G.read_file(G.golden_path("cfg2"))
+    wl = W.microcircuit(1)
+    assert sizes == [p[1] for p in wl.populations] and ocounts.shape[0] == 110
+    g = B.Sim(0.1, wl.ring_slots, wl.seed, record_spikes=True, max_recorded_spikes=1 << 23)
+    wl.apply(g); g.prepare()
+    g.set_state(B.FIELD_V, wl.initial_v())
+    st = g.stats()
+    assert st.n_connections == 298_905_266 and st.step_mode == B.STEP_PERSISTENT and st.delivery_kernel == 3
+    start, bin_steps, ns = 10_000, 20, 200                   # discard 1 s; 2 ms bins; 200 neurons
+    g.enable_statistics(start_step=start, bin_steps=bin_steps, sample_per_pop=ns, max_bins=5000)
+    counts, steps, ids = gpu_window_counts(g, wl, 110, ws, chunk_windows=10)       # 11 launches of 10,000 steps
+    assert g.get_state(B.FIELD_STEP) == 110_000 and g.stats().spikes == steps.size
+    # the initial volley is the same set of neurons on both sides (same fp32 V0, same Poisson counts)
+    assert np.all(np.abs(counts[0] - ocounts[0]) <= np.maximum(3, 0.03 * ocounts[0])), (counts[0], ocounts[0])
+    compare_rates(wl, counts, ocounts, 10, ws, W.PD_NAMES)
+    # on-device statistics, full scale, the paper's sample size
+    N, end = wl.n_neurons, 110_000
+    rate, cv = g.rate_cv()
+    o_rate, o_cv = S.rate_cv(steps, ids, N, start, end, 0.1)
+    assert np.allclose(rate, o_rate, rtol=1e-6, atol=0)
+    assert np.array_equal(np.isnan(cv), np.isnan(o_cv)) and np.count_nonzero(~np.isnan(cv)) > N // 2
+    ok = ~np.isnan(o_cv)
+    assert np.allclose(cv[ok], o_cv[ok], rtol=1e-5, atol=1e-6)
+    n_bins = (end - start) // bin_steps
+    for p in (0, 5):                                         # L2/3E (largest) and L5I (highest rate)
+        first, _ = wl.pop_ranges()[p]
+        Cg = g.correlations(p)
+        Co = S.correlation(S.binned_trains(steps, ids, list(range(first, first + ns)), start, n_bins, bin_steps))
+        assert Cg.shape == Co.shape == (ns, ns) and np.array_equal(np.isnan(Cg), np.isnan(Co))
+        okc = ~np.isnan(Co)
+        assert okc.sum() > ns * ns // 2 and np.allclose(Cg[okc], Co[okc], atol=2e-6)
+    g.close()
+
+
+def test_cfg4_free_running_rates_1s(B):
+    """BASELINE.json configs[4]: 1e6 neurons, 1e9 connections, "1 s of biological time"; rates over the last 0.9 s (the
+    first 100 ms hold the initial volley — reading C17)."""
+    ws, sizes, ocounts = G.read_file(G.golden_path("cfg4"))
+    wl = W.balanced_large()
+    assert sizes == [p[1] for p in wl.populations] and ocounts.shape[0] == 10
+    g = B.Sim(0.1, wl.ring_slots, wl.seed, record_spikes=True, max_recorded_spikes=1 << 25)
+    wl.apply(g); g.prepare()
+    g.set_state(B.FIELD_V, wl.initial_v())
+    st = g.stats()
+    assert st.n_connections == 10**9 and st.step_mode == B.STEP_PERSISTENT and st.delivery_kernel == 3
+    counts, steps, ids = gpu_window_counts(g, wl, 10, ws, chunk_windows=5)         # 2 launches of 5,000 steps
+    assert g.get_state(B.FIELD_STEP) == 10_000 and g.stats().spikes == steps.size
+    assert np.all(np.abs(counts[0] - ocounts[0]) <= np.maximum(3, 0.03 * ocounts[0])), (counts[0], ocounts[0])
+    compare_rates(wl, counts, ocounts, 1, ws, ["E", "I"])
+    g.close()

@@ -94,6 +94,76 @@ def test_single_neuron_700pA_against_scipy(oracle_mod):
     assert np.all(np.diff(np.diff(spikes)) > 0)
 
 
+def reference_spike_times(p, T):
+    """Spike times of one AdEx neuron under a constant current: scipy DOP853 (rtol 1e-11) with a terminal event at V_peak,
+    reset (V -> V_r, w -> w + b) by hand.  Independent of the oracle's integrator, controller and sub-step floor."""
+    f = scipy_rhs(p, clamp=False)
+    ev = lambda t, y: y[0] - p["V_peak"]
+    ev.terminal = True; ev.direction = 1
+    t0, y0, out = 0.0, [p["E_L"], 0, 0, 0, 0, 0], []
+    while t0 < T:
+        sol = solve_ivp(f, (t0, T), y0, method="DOP853", rtol=1e-11, atol=1e-12, events=ev)
+        if sol.status != 1:
+            break
+        t0 = sol.t_events[0][0]; out.append(t0)
+        y0 = sol.y[:, -1].copy(); y0[0] = p["V_reset"]; y0[1] += p["b"]
+    return out
+
+
+def oracle_spike_steps(oracle_mod, p, T):
+    y = np.array([p["E_L"], 0, 0, 0, 0, 0.0]); h = 0.1
+    out = []
+    for k in range(int(round(T / 0.1))):
+        y, h, s = oracle_mod.adex_step(p, y, h, 0.1)
+        if s:
+            out.append(k)
+    return out
+
+
+@pytest.mark.parametrize("I_e,n_min", [(700.0, 9), (1000.0, 30)])
+def test_spike_steps_and_sub_step_floor(oracle_mod, I_e, n_min):
+    """Reading C23 fixes the smallest sub-step h_min of the adaptive integrator (the paper names none).  On
+    the single-neuron constant-current protocol of PAPER.md:252 (700 pA; 1000 pA as a faster-firing second case), over a
+    full second, EVERY spike of the oracle with the recipe's h_min = 1e-3 ms must fall in the time step that contains the
+    event-located DOP853 crossing (the next step only if the crossing lies in the last tenth of its step: the integrator's
+    own phase error is a few 1e-3 ms) and the lag must not accumulate — spike steps and inter-spike intervals, not only the
+    subthreshold trace.  The looser floor 1e-2 ms (used for speed during round 1) does not meet this: sub-steps at the
+    floor are accepted unconditionally, each spike is found ~0.01 ms late and the lag grows to whole steps; asserted here
+    so that the choice stays on evidence."""
+    assert W.ADEX["h_min"] == 1e-3
+    T = 1000.0
+    ref = np.array(reference_spike_times(params(I_e=I_e), T))
+    assert ref.size >= n_min
+    ref_steps = np.floor(ref / 0.1).astype(int)
+    phase = ref / 0.1 - ref_steps
+    fine = np.array(oracle_spike_steps(oracle_mod, params(I_e=I_e), T))
+    assert fine.size == ref.size
+    lag = fine - ref_steps
+    assert np.all((lag == 0) | ((lag == 1) & (phase > 0.9))), (lag, phase)
+    assert np.all(np.abs(np.diff(fine) - np.diff(ref_steps)) <= 1) and lag[-1] == 0
+    assert np.mean(lag == 0) >= 0.9
+    coarse = np.array(oracle_spike_steps(oracle_mod, params(I_e=I_e, h_min=1e-2), T))
+    assert coarse.size == ref.size
+    lag_c = coarse - ref_steps
+    assert lag_c.min() >= 0 and lag_c[-1] >= 1 and np.mean(lag_c >= 1) >= 0.5, lag_c          # it accumulates
+
+
+def test_network_rate_is_insensitive_to_the_floor(oracle_mod):
+    """The 2000-neuron balanced network of the rate pin below at both floors: same mean rate within 1 %.  (The floor moves
+    single spikes by a step after tens of spikes; it does not change the population activity.)"""
+    rates = {}
+    for hm in (1e-3, 1e-2):
+        wl = W.balanced_adex(n=2000, k_total=200, n_steps=3000, seed=5)
+        wl.populations = [(name, n, dict(p, h_min=hm)) for name, n, p in wl.populations]
+        o = oracle_mod.Oracle(0.1, wl.ring_slots, wl.seed)
+        wl.apply(o); o.prepare()
+        o.set_state(oracle_mod.FIELD_V, wl.initial_v().astype(np.float64))
+        o.simulate(3000)
+        st, ids = o.get_spikes()
+        rates[hm] = np.sum(st >= 500) / 2000 / 0.25
+    assert abs(rates[1e-3] - rates[1e-2]) <= 0.01 * rates[1e-3], rates
+
+
 def test_fixed_point_and_step_size_state(oracle_mod):
     """No drive: the resting point of Eqs. (3), (5) is stationary; the sub-step size grows to the whole step."""
     p = params()
