@@ -191,7 +191,7 @@ def delivery_microbench(device, peak_gbs, K=10000, fraction=0.05, steps=30, warm
                    "events_per_s": ev / (ms * 1e-3), "algorithmic_gbs": ev * BYTES_PER_EVENT / (ms * 1e-3) / 1e9,
                    "frac_of_hbm_peak": ev * BYTES_PER_EVENT / (ms * 1e-3) / 1e9 / peak_gbs,
                    "delivery_kernel": int(s1.delivery_kernel),
-                   "ring_bytes": 4 * wl.n_neurons * (2 if int(s1.delivery_kernel) == 4 else wl.ring_slots + 1),
+                   "ring_bytes": 4 * wl.n_neurons * (2 if int(s1.delivery_kernel) >= 4 else wl.ring_slots + 1),
                    "timed": "delivery kernel" if int(s1.delivery_kernel) != 3 else "pipelined step kernel (injection + delivery)",
                    "build_ms": s1.build_ms,
                    "n_connections": int(s1.n_connections)}
@@ -229,8 +229,8 @@ def run_ours(args):
     wl = make_workload(args.workload, seed_offset=rank)       # replicas: independent seeds, no exchange
     g = B.Sim(DT_MS, wl.ring_slots, wl.seed, record_spikes=True, max_recorded_spikes=1 << 24, device=local)
     wl.apply(g)
-    if args.delivery_kernel == 4:
-        g.set_option(B.OPT_DELIVERY_KERNEL, 4)                # before prepare: the spike-buffer backend changes what is allocated
+    if args.delivery_kernel >= 4:
+        g.set_option(B.OPT_DELIVERY_KERNEL, args.delivery_kernel)                # before prepare: the spike-buffer backend changes what is allocated
     t0 = time.time(); g.prepare(); build_wall = time.time() - t0
     g.set_option(B.OPT_STEP_MODE, args.step_mode)
     g.set_option(B.OPT_DELIVERY_KERNEL, args.delivery_kernel)
@@ -441,7 +441,7 @@ def main():
     ap.add_argument("--micro-k-only", type=int, default=0, help="restrict --micro-sweep to one out-degree")
     ap.add_argument("--probe", action="store_true", help="run the ceiling probes (ng_probe) and print them as JSON")
     ap.add_argument("--step-mode", type=int, default=3, choices=[0, 1, 2, 3], help="NG_OPT_STEP_MODE (3 = auto)")
-    ap.add_argument("--delivery-kernel", type=int, default=0, choices=[0, 1, 2, 3, 4], help="NG_OPT_DELIVERY_KERNEL (0 = auto)")
+    ap.add_argument("--delivery-kernel", type=int, default=0, choices=[0, 1, 2, 3, 4, 5], help="NG_OPT_DELIVERY_KERNEL (0 = auto)")
     ap.add_argument("--no-prefetch", action="store_true", help="NG_OPT_PREFETCH = 0")
     ap.add_argument("--micro-k", type=int, default=10000)
     ap.add_argument("--micro-fraction", type=float, default=0.05)

@@ -96,7 +96,13 @@ enum {
                                     4 = spike-buffer backend, the paper's own mechanism: no D-plane
                                         ring; the spikes of the last ring_slots steps stay buffered and reach their
                                         delay groups one step at a time.  Must be chosen BEFORE ng_prepare;
-                                        NG_FIELD_RING is then read-only (expanded on demand)                 */
+                                        NG_FIELD_RING is then read-only (expanded on demand),
+                                    5 = per-delay event queues: a spiking row is read once and its records are appended,
+                                        binned by delay, to the queue of their arrival step; every step streams ONE
+                                        queue into the input plane of the next step.  Two planes like kernel 4, same
+                                        rules (before ng_prepare, NG_FIELD_RING read-only).  Memory: ring_slots queues
+                                        of NG_OPT_QUEUE_CAPACITY events x 8 B; a full queue drops events and
+                                        ng_simulate returns NG_ERR_OVERFLOW                                     */
     NG_OPT_DELIVER_BLOCKS = 3,   /* grid size of the delivery kernel, 0 = auto                         */
     NG_OPT_PROFILE = 4,          /* 1 = time every kernel with CUDA events (forces plain launches);
                                     results in ng_stats.ms_update / ms_deliver                       */
@@ -107,7 +113,10 @@ enum {
                                     L2 (default 1; ignored by delivery kernel 2)                       */
     NG_OPT_TRACE = 8,            /* 1 = the persistent kernels (step mode 2) stamp %globaltimer at every phase
                                     boundary of every CTA; read with ng_get_trace (after ng_prepare)   */
-    NG_OPT_PERSISTENT_THREADS = 9 /* threads per CTA of the persistent kernels: 1024 (default, one CTA per SM) or 512 */
+    NG_OPT_PERSISTENT_THREADS = 9, /* threads per CTA of the persistent kernels: 1024 (default, one CTA per SM) or 512 */
+    NG_OPT_QUEUE_CAPACITY = 10   /* delivery kernel 5: events per queue (before ng_prepare).  0 = auto: 1.25 x the expected
+                                    events per step (delivery-only mode: inject fraction x connections; else 2 % of
+                                    the connections, i.e. a mean rate of 200 Hz at dt = 0.1 ms) + 65536              */
 };
 
 typedef struct {
@@ -165,7 +174,7 @@ typedef struct {
     uint64_t launches_update;    /* kernel launches (or graph kernel nodes executed) since create    */
     uint64_t launches_deliver;
     uint64_t launches_other;     /* builder and bookkeeping kernels                                  */
-    int32_t delivery_kernel;     /* the delivery kernel in use (1 .. 4)                           */
+    int32_t delivery_kernel;     /* the delivery kernel in use (1 .. 5)                           */
     int32_t step_mode;
 } ng_stats;
 

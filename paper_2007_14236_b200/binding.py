@@ -18,7 +18,7 @@ FIELD_V, FIELD_I_SYN, FIELD_REFR, FIELD_RING, FIELD_STEP, FIELD_LAST_INPUT = 0, 
 FIELD_ADEX_W, FIELD_ADEX_G_EX, FIELD_ADEX_Y_EX, FIELD_ADEX_G_IN, FIELD_ADEX_Y_IN, FIELD_ADEX_H = 6, 7, 8, 9, 10, 11
 DIST_CONST, DIST_NORMAL_CLIPPED, DIST_UNIFORM_INT = 0, 1, 2
 (OPT_STEP_MODE, OPT_STEPS_PER_GRAPH, OPT_DELIVERY_KERNEL, OPT_DELIVER_BLOCKS, OPT_PROFILE, OPT_ASYNC,
- OPT_SORT_SEGMENTS, OPT_PREFETCH, OPT_TRACE, OPT_PERSISTENT_THREADS) = range(10)
+ OPT_SORT_SEGMENTS, OPT_PREFETCH, OPT_TRACE, OPT_PERSISTENT_THREADS, OPT_QUEUE_CAPACITY) = range(11)
 STEP_GRAPH, STEP_LAUNCH, STEP_PERSISTENT, STEP_AUTO = 0, 1, 2, 3
 
 EXPORTS = ["ng_create", "ng_destroy", "ng_last_error", "ng_create_population", "ng_connect_fixed_indegree",

@@ -62,6 +62,9 @@ struct ng_sim {
     bool has_adex = false;                 // any AdEx population: two receptor ports, AdEx state arrays, <true> kernels
     int64_t NR = 0;                        // ring row length = N * ports
     bool window_backend = false;           // delivery kernel 4 chosen before ng_prepare: spike window instead of a D-plane ring
+    bool queue_backend = false;            // delivery kernel 5 chosen before / by ng_prepare: per-delay event queues, two planes
+    int64_t queue_cap_opt = 0;             // NG_OPT_QUEUE_CAPACITY: events per queue (0 = auto)
+    int queue_blocks = 0;
     cudaGraphExec_t graph_exec = nullptr; int graph_steps = 0;
     // stats
     double build_ms = 0, ms_update = 0, ms_deliver = 0;
@@ -173,7 +176,8 @@ void launch_update(ng_sim* s) {
     else update_kernel<false><<<s->update_blocks, kUpdateThreads, 0, s->stream>>>(s->a);
 }
 void launch_deliver(ng_sim* s) {
-    if (s->delivery_kernel == 4) deliver_kernel<4><<<s->deliver_blocks, kDeliverThreads, 0, s->stream>>>(s->a);
+    if (s->delivery_kernel == 5) queue_deliver_kernel<<<s->queue_blocks, kQThreads, 0, s->stream>>>(s->a);
+    else if (s->delivery_kernel == 4) deliver_kernel<4><<<s->deliver_blocks, kDeliverThreads, 0, s->stream>>>(s->a);
     else if (s->delivery_kernel == 2) deliver_kernel<2><<<s->deliver_blocks, kDeliverThreads, 0, s->stream>>>(s->a);
     else deliver_kernel<1><<<s->deliver_blocks, kDeliverThreads, 0, s->stream>>>(s->a);
 }
@@ -207,12 +211,19 @@ void configure_launch(ng_sim* s) {
     if (k == 0) k = 3;                                              // a ring beyond L2 was given the window backend in ng_prepare
     (void)mean_group; (void)ring_bytes;
     if (s->window_backend) k = 4;                                   // fixed at ng_prepare: there is no D-plane ring
+    if (s->queue_backend) k = 5;
     s->delivery_kernel = k;
     // step mode: the latency-bound kernels run as one persistent cooperative kernel per ng_simulate call; the
     // bandwidth-bound delay-major kernel keeps its 8 CTAs per SM and runs from a CUDA graph
-    s->step_mode = s->step_mode_opt != 3 ? s->step_mode_opt : (k == 2 || k == 4 || !s->coop_ok) ? 0 : 2;
+    s->step_mode = s->step_mode_opt != 3 ? s->step_mode_opt : (k == 2 || k == 4 || k == 5 || !s->coop_ok) ? 0 : 2;
     if (s->has_adex && s->step_mode == 2 && k != 3) s->step_mode = 0;   // the two-phase persistent kernels are LIF only
-    s->a.prefetch = (k != 2 && k != 4 && s->prefetch_opt) ? 1 : 0;
+    if (k == 5 && s->step_mode == 2) s->step_mode = 0;                  // the event-queue backend runs as update + delivery launches
+    s->a.prefetch = (k != 2 && k != 4 && k != 5 && s->prefetch_opt) ? 1 : 0;
+    {
+        int occq = 0;
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occq, queue_deliver_kernel, kQThreads, 0);
+        s->queue_blocks = sm * std::max(1, std::min(occq, 2));
+    }
     s->pipe_blocks = grid_for(s->N, kPipeThreads - (s->has_adex ? 128 : kEntryTile), sm * 4);   // updaters per CTA
     {
         int occp = 0;
@@ -309,14 +320,15 @@ int32_t ring_copy(ng_sim* s, bool to_device, void* user, int64_t count, int64_t 
     int32_t rc = read_ctl(s, &h);
     if (rc) return rc;
     const int64_t N = s->NR, D = s->cfg.ring_slots, Dr = s->a.Dr, n = h.step_u;      // N: plane length (all ports)
-    if (s->window_backend) {
-        // no ring exists: the pending inputs live in the spike window.  Read-back expands them into a temporary image.
-        if (to_device) return fail(s, NG_ERR_STATE, "NG_FIELD_RING cannot be set with the spike-buffer backend (delivery kernel 4)");
+    if (s->window_backend || s->queue_backend) {
+        // no ring exists: the pending inputs live in the spike window / the event queues.  Read-back expands them into a temporary image.
+        if (to_device) return fail(s, NG_ERR_STATE, "NG_FIELD_RING cannot be set with the two-plane backends (delivery kernels 4 and 5)");
         float* img = nullptr;
         if (!dev_alloc_t(s, &img, (size_t)N * D)) return fail(s, NG_ERR_OOM, "ring image");
         NG_CUDA(s, cudaMemsetAsync(img, 0, (size_t)N * D * 4, s->stream));
         NG_CUDA(s, cudaMemcpyAsync(img + (size_t)(n % D) * N, s->a.ring + (size_t)(n % 2) * N, (size_t)N * 4, cudaMemcpyDeviceToDevice, s->stream));
-        materialize_window_kernel<<<s->sm_count * 8, 256, 0, s->stream>>>(s->a, (long long)n, img);
+        if (s->queue_backend) materialize_queues_kernel<<<s->sm_count * 8, 256, 0, s->stream>>>(s->a, (long long)n, img);
+        else materialize_window_kernel<<<s->sm_count * 8, 256, 0, s->stream>>>(s->a, (long long)n, img);
         NG_CUDA(s, cudaMemcpyAsync(user, img + first, (size_t)count * 4, cudaMemcpyDefault, s->stream));
         NG_CUDA(s, cudaStreamSynchronize(s->stream));
         dev_free(s, img);
@@ -470,9 +482,9 @@ int32_t ng_set_option(ng_sim* s, int32_t option, int64_t value) {
             if (value < 1 || value > 10000) return fail(s, NG_ERR_INVALID_ARG, "steps per graph in 1..10000");
             s->steps_per_graph = (int)value; destroy_graph(s); break;
         case NG_OPT_DELIVERY_KERNEL:
-            if (value < 0 || value > 4) return fail(s, NG_ERR_INVALID_ARG, "delivery kernel is 0 .. 4");
-            if (s->prepared && value != 0 && (value == 4) != s->window_backend)
-                return fail(s, NG_ERR_STATE, "delivery kernel 4 (spike-buffer backend) must be chosen before ng_prepare and cannot be left after it");
+            if (value < 0 || value > 5) return fail(s, NG_ERR_INVALID_ARG, "delivery kernel is 0 .. 5");
+            if (s->prepared && value != 0 && ((value == 4) != s->window_backend || (value == 5) != s->queue_backend))
+                return fail(s, NG_ERR_STATE, "delivery kernels 4 (spike-buffer backend) and 5 (event queues) must be chosen before ng_prepare and cannot be left after it");
             s->delivery_kernel_opt = (int)value; if (s->prepared) configure_launch(s); break;
         case NG_OPT_DELIVER_BLOCKS:
             if (value < 0 || value > (1 << 20)) return fail(s, NG_ERR_INVALID_ARG, "deliver blocks out of range");
@@ -497,6 +509,10 @@ int32_t ng_set_option(ng_sim* s, int32_t option, int64_t value) {
             if (value != 512 && value != 1024) return fail(s, NG_ERR_INVALID_ARG, "persistent threads: 512 or 1024");
             s->persistent_threads = (int)value; if (s->prepared) configure_launch(s); break;
         case NG_OPT_PREFETCH: s->prefetch_opt = value ? 1 : 0; if (s->prepared) configure_launch(s); break;
+        case NG_OPT_QUEUE_CAPACITY:
+            if (s->prepared) return fail(s, NG_ERR_STATE, "NG_OPT_QUEUE_CAPACITY after ng_prepare");
+            if (value < 0) return fail(s, NG_ERR_INVALID_ARG, "queue capacity < 0");
+            s->queue_cap_opt = value; break;
         default: return fail(s, NG_ERR_INVALID_ARG, "unknown option");
     }
     return NG_OK;
@@ -512,9 +528,22 @@ int32_t ng_prepare(ng_sim* s) {
     // Ring or spike window?  A ring that cannot stay in L2 (config 3: 65 planes x 4 MB) costs a DRAM round trip per plane
     // and step; the spike-buffer backend keeps two planes whatever D is and measured faster on every point of the
     // config 3 sweep, so it is the automatic choice there.
-    s->window_backend = s->delivery_kernel_opt == 4 ||
-                        (s->delivery_kernel_opt == 0 && (double)N * (D + 1) * 4.0 > 0.8 * (double)s->l2_bytes);
-    const int planes = s->window_backend ? 2 : D + 1;               // ring planes actually stored
+    s->S = 0;
+    for (const CallDev& c : s->calls) s->S += (int64_t)(c.rule == kRuleIndegree ? c.tgt_n : c.src_n) * c.K;
+    const bool beyond_l2 = (double)N * (D + 1) * 4.0 > 0.8 * (double)s->l2_bytes;
+    // Beyond L2, short delay groups (a few records per (source, delay): config 3 at out-degree 100 and 1000) make the
+    // spike-buffer walk read at random 12-125-byte granularity; the event queues read a spiking row once, whole
+    // (DESIGN.md section 7).  Expected events per step: the injected fraction in delivery-only mode, else 2 % of S.
+    const double mean_group = (double)s->S / ((double)N * D);
+    const double ev_step = s->bypass ? (double)s->inject_thr / 4294967296.0 * (double)s->S : 0.02 * (double)s->S;
+    int64_t qcap = s->queue_cap_opt > 0 ? s->queue_cap_opt : (int64_t)(1.25 * ev_step) + 65536;
+    qcap = (qcap + 1) & ~(int64_t)1;
+    size_t mem_free = 0, mem_total = 0;
+    cudaMemGetInfo(&mem_free, &mem_total);
+    const bool queue_fits = (double)qcap * D * 8.0 + (double)s->S * 9.0 < 0.85 * (double)mem_total;
+    s->queue_backend = s->delivery_kernel_opt == 5 || (s->delivery_kernel_opt == 0 && beyond_l2 && mean_group < 48.0 && queue_fits);
+    s->window_backend = s->delivery_kernel_opt == 4 || (s->delivery_kernel_opt == 0 && beyond_l2 && !s->queue_backend);
+    const int planes = (s->window_backend || s->queue_backend) ? 2 : D + 1;               // ring planes actually stored
     s->has_adex = false;
     for (const HostPop& hp : s->pops) s->has_adex = s->has_adex || hp.dev.model == 1;
     s->NR = (int64_t)N * (s->has_adex ? 2 : 1);
@@ -528,8 +557,6 @@ int32_t ng_prepare(ng_sim* s) {
                 return fail(s, NG_ERR_INVALID_ARG, "receptor port 1 onto a target range that holds LIF neurons (they have one port)");
     }
     const size_t NRs = (size_t)s->NR;
-    s->S = 0;
-    for (const CallDev& c : s->calls) s->S += (int64_t)(c.rule == kRuleIndegree ? c.tgt_n : c.src_n) * c.K;
 
     cudaEvent_t e0, e1;
     NG_CUDA(s, cudaEventCreate(&e0));
@@ -570,6 +597,12 @@ int32_t ng_prepare(ng_sim* s) {
         const long long worst = (long long)N * D;
         s->a.win_cap = worst <= (1LL << 26) ? worst : std::max(1LL << 26, worst / 8);
         if (!dev_alloc_t(s, &s->a.win_id, (size_t)s->a.win_cap)) return fail(s, NG_ERR_OOM, "device allocation failed (spike window)");
+    }
+    if (s->queue_backend) {
+        s->a.q_cap = qcap;
+        if (!(dev_alloc_t(s, &s->a.q_ev, (size_t)qcap * D) && dev_alloc_t(s, &s->a.q_tail, (size_t)D * kQTailStride)))
+            return fail(s, NG_ERR_OOM, "device allocation failed (event queues)");
+        NG_CUDA(s, cudaMemsetAsync(s->a.q_tail, 0, (size_t)D * kQTailStride * 8, st));
     }
     NG_CUDA(s, cudaMemsetAsync(s->d_cnt, 0, (size_t)N * D * 4, st));
     if (s->a.last_input) NG_CUDA(s, cudaMemsetAsync(s->a.last_input, 0, NRs * 4, st));
@@ -670,7 +703,9 @@ int32_t ng_set_state(ng_sim* s, int32_t field, const void* data, int64_t count, 
         std::memset(h.win_start, 0, sizeof(h.win_start)); h.err_window = 0;
         h.slot = (int32_t)(n % s->a.Dr);
         h.rec_total[0] = h.rec_total[1] = recorded;
+        h.err_queue = 0;
         NG_CUDA(s, cudaMemcpyAsync(s->d_ctl, &h, sizeof(Ctl), cudaMemcpyHostToDevice, s->stream));
+        if (s->a.q_tail) NG_CUDA(s, cudaMemsetAsync(s->a.q_tail, 0, (size_t)s->cfg.ring_slots * kQTailStride * 8, s->stream));
         NG_CUDA(s, cudaStreamSynchronize(s->stream));
         return NG_OK;
     }
@@ -779,11 +814,12 @@ int32_t ng_simulate(ng_sim* s, int64_t n_steps) {
     s->steps_done += (uint64_t)n_steps;
     if (s->async) return NG_OK;
     NG_CUDA(s, cudaStreamSynchronize(st));
-    if (s->a.rec_cap > 0 || s->window_backend) {
+    if (s->a.rec_cap > 0 || s->window_backend || s->queue_backend) {
         Ctl h{};
         rc = read_ctl(s, &h);
         if (rc) return rc;
         if (h.err_window) return fail(s, NG_ERR_OVERFLOW, "spike window overflowed: more spikes within ring_slots steps than its capacity");
+        if (h.err_queue) return fail(s, NG_ERR_OVERFLOW, "an event queue overflowed (events were dropped): raise NG_OPT_QUEUE_CAPACITY");
         const unsigned long long total = h.rec_total[h.step_u & 1];
         if (s->a.rec_cap > 0 && total > (unsigned long long)s->a.rec_cap) return fail(s, NG_ERR_OVERFLOW, "spike record full; later spikes were not recorded");
     }

@@ -66,6 +66,7 @@ struct Ctl {
                                            // kernel's bookkeeping advances `slot` while later CTAs of the same launch still start
     int32_t err_window;                    // spike-buffer backend: the spike window overflowed its capacity
     uint32_t n_long_groups;                // builder: (source, delay) groups longer than kSortMax, listed for the CTA-wide sort
+    int32_t err_queue;                     // event-queue backend: a queue overflowed its capacity (events were dropped)
     // line 1: spike counters (atomics of the appending warps / CTAs)
     alignas(128) int32_t spike_cnt[4];     // length of the spike array of step n, indexed n & 3 (the list itself by n & 1)
     // line 2: event counter (one atomic per CTA and step)
@@ -423,6 +424,9 @@ struct StepArgs {
     long long st_start; int32_t st_bin_steps, st_max_bins;
     int32_t* win_id;             // spike-buffer backend (delivery kernel 4): circular log of the spikes of the last D steps
     long long win_cap;           //   its capacity in entries; nullptr / 0 for the ring backends
+    int2* q_ev;                  // event-queue backend (delivery kernel 5): [D][q_cap] (target, weight bits) by arrival step mod D
+    unsigned long long* q_tail;  //   events appended to the queue of each arrival slot, one counter per 128-byte line
+    long long q_cap;             //   capacity of one queue in events (even); nullptr / 0 for the other backends
     unsigned long long* trace;   // NG_OPT_TRACE: [kTraceSteps][gridDim.x][kTraceStamps] %globaltimer stamps, or nullptr
     int32_t* rec_step; int32_t* rec_id; long long rec_cap;   // rec_cap = 0: recording off
     // connection structure
@@ -1016,6 +1020,183 @@ __device__ __forceinline__ void deliver_groups_phase(const StepArgs& a, long lon
         d_cur = d_nxt; ga_cur = ga_nxt; gb_cur = gb_nxt; r0_cur = r0_nxt;
     }
     if (ev) atomicAdd(&a.ctl->events, ev);
+}
+
+// ---------------------------------------------------------------------------------------
+// a3. Spike delivery, kernel 5: per-delay event queues (two input planes, like kernel 4).
+//   For short delay groups (out-degree / D of a few records: config 3 at out-degree 100 and 1000) both the ring walk and the
+//   spike-buffer walk read or reduce at random 12-125-byte granularity, and DRAM sectors, not reductions, bound them.  Here a
+//   spiking row is read ONCE, whole and coalesced (8 B of target + weight and 1 B of delay per record), at spike time:
+//     append (step n):  a CTA flattens the rows of its share of the spike array into batches of kQBatch records, bins a
+//                       batch by delay in shared memory, claims a range in the queue of each arrival step n + d with one
+//                       atomic per (batch, delay) and stores (target, weight) there in delay-sorted, coalesced runs;
+//                       records of delay 1 are reduced straight into the input plane of step n + 1;
+//     drain  (step n):  the queue of arrival step n + 1 — complete since the append of step n - 1, because only delays
+//                       >= 2 go through a queue — is streamed (8 B per event, 128-bit loads) into the same plane.
+//   Both run in the same launch on different CTAs' time lines (odd CTAs append first, even CTAs drain first): the append is
+//   DRAM-stream bound (9 B read + 8 B written per event), the drain is bound by the scattered reductions into ONE plane of
+//   N * 4 bytes that stays in L2 whatever D is.  Queue of arrival step a = slot a mod D: during step n the appends write
+//   every slot except (n + 1) mod D, which is the one being drained; its counter is cleared by the update of step n + 1.
+// ---------------------------------------------------------------------------------------
+constexpr int kQThreads = 512;
+constexpr int kQVecPerThread = 2;                              // 128-bit vectors (4 records each) per thread and batch
+constexpr int kQBatch = kQThreads * kQVecPerThread * 4;        // records per batch
+constexpr int kQTailStride = 16;                               // one 128-byte line per queue counter
+struct QueueShared {
+    long long r0[kEntryTile];
+    int32_t pre[kEntryTile + 1];         // 128-bit vectors of the entries [0, k) of the staged tile
+    int32_t warp_tot[kEntryTile / 32];
+    uint32_t hist[256];                  // records of the batch per delay
+    uint32_t sbase[257];                 // exclusive prefix of hist; [D + 1] = records of the batch that go to a queue
+    unsigned long long gbase[256];       // start of the range claimed in the queue of that delay's arrival step
+    int2 staged[kQBatch];                // the batch in delay order
+    uint8_t sbin[kQBatch];               //   and the delay of each staged record
+    int32_t nmodD;
+};
+
+__device__ __forceinline__ void queue_append_phase(const StepArgs& a, long long n, int M, float* __restrict__ plane1, QueueShared& sh) {
+    const int N = a.N, D = a.D;
+    const RowInfo* __restrict__ rows = a.spike_row + (size_t)(n & 1) * N;
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const int nmodD = sh.nmodD;
+    const int tile_len = max(1, min(kEntryTile, (M + (int)gridDim.x - 1) / (int)gridDim.x));
+    unsigned long long ev = 0;
+    bool overflow = false;
+    for (int tile0 = (int)blockIdx.x * tile_len; tile0 < M; tile0 += (int)gridDim.x * tile_len) {
+        const int m = min(tile_len, M - tile0);
+        __syncthreads();                                       // the previous tile's readers are done
+        int x = 0;
+        if (threadIdx.x < kEntryTile) {                        // stage the entries, scan their vector counts
+            if ((int)threadIdx.x < m) {
+                const int4 e = __ldcg(reinterpret_cast<const int4*>(rows + tile0 + threadIdx.x));     // r0 (lo, hi), deg, d1
+                sh.r0[threadIdx.x] = (long long)(((unsigned long long)(uint32_t)e.y << 32) | (uint32_t)e.x);
+                x = padded_len(e.z) >> 2;
+                ev += (unsigned long long)e.z;
+            }
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int y = __shfl_up_sync(0xffffffffu, x, o);
+                if (lane >= o) x += y;
+            }
+            if (lane == 31) sh.warp_tot[wib] = x;
+        }
+        __syncthreads();
+        if (threadIdx.x < kEntryTile) {
+            int off = 0;
+            for (int k = 0; k < wib; ++k) off += sh.warp_tot[k];
+            sh.pre[threadIdx.x + 1] = x + off;
+            if (threadIdx.x == 0) sh.pre[0] = 0;
+        }
+        __syncthreads();
+        const int total_vec = sh.pre[m];
+        for (int vb = 0; vb < total_vec; vb += kQThreads * kQVecPerThread) {
+            for (int k = threadIdx.x; k < 256; k += kQThreads) sh.hist[k] = 0;
+            int4 t4[kQVecPerThread]; float4 w4[kQVecPerThread]; uint32_t d4[kQVecPerThread];
+#pragma unroll
+            for (int u = 0; u < kQVecPerThread; ++u) {
+                const int v = vb + u * kQThreads + (int)threadIdx.x;
+                t4[u] = make_int4(-1, -1, -1, -1); w4[u] = make_float4(0.f, 0.f, 0.f, 0.f); d4[u] = 0;
+                if (v < total_vec) {
+                    int lo = 0, hi = m;                        // largest e with pre[e] <= v
+                    while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (sh.pre[mid] <= v) lo = mid; else hi = mid; }
+                    const long long p = sh.r0[lo] + ((long long)(v - sh.pre[lo]) << 2);
+                    t4[u] = ld_stream_s32x4(a.tgt + p); w4[u] = ld_stream_f32x4(a.w + p); d4[u] = ld_stream_u32(a.dly + p);
+                }
+            }
+            __syncthreads();                                   // hist is cleared
+            uint32_t rank[kQVecPerThread][4];
+#pragma unroll
+            for (int u = 0; u < kQVecPerThread; ++u) {
+                const int tt[4] = {t4[u].x, t4[u].y, t4[u].z, t4[u].w};
+                const float ww[4] = {w4[u].x, w4[u].y, w4[u].z, w4[u].w};
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    uint32_t d = tt[c] >= 0 ? (d4[u] >> (8 * c)) & 0xffu : 0u;           // padding records: target -1
+                    if (d == 1u) { red_add_f32(plane1 + tt[c], ww[c]); d = 0u; }         // consumed by the very next step
+                    d4[u] = (d4[u] & ~(0xffu << (8 * c))) | (d << (8 * c));              // 0 = not queued
+                    const unsigned mask = __match_any_sync(0xffffffffu, d);             // one shared-memory atomic per delay and warp
+                    const int leader = __ffs(mask) - 1;
+                    uint32_t base = 0;
+                    if (d != 0u && lane == leader) base = atomicAdd(&sh.hist[d], (uint32_t)__popc(mask));
+                    base = __shfl_sync(0xffffffffu, base, leader);
+                    rank[u][c] = base + (uint32_t)__popc(mask & ((1u << lane) - 1u));
+                }
+            }
+            __syncthreads();
+            if (wib == 0) {                                    // prefix over the delays; one global atomic per (batch, delay)
+                uint32_t carry = 0;
+                for (int b0 = 0; b0 <= D; b0 += 32) {
+                    const int k = b0 + lane;
+                    const uint32_t h = (k >= 2 && k <= D) ? sh.hist[k] : 0u;
+                    uint32_t incl = h;
+#pragma unroll
+                    for (int o = 1; o < 32; o <<= 1) {
+                        const uint32_t y = __shfl_up_sync(0xffffffffu, incl, o);
+                        if (lane >= o) incl += y;
+                    }
+                    if (k <= D) sh.sbase[k] = carry + incl - h;
+                    if (h > 0u) {
+                        int qs = nmodD + k; if (qs >= D) qs -= D;          // arrival step n + k
+                        sh.gbase[k] = atomicAdd(a.q_tail + (size_t)qs * kQTailStride, (unsigned long long)h);
+                    }
+                    carry += __shfl_sync(0xffffffffu, incl, 31);
+                }
+                if (lane == 0) sh.sbase[D + 1] = carry;
+            }
+            __syncthreads();
+#pragma unroll
+            for (int u = 0; u < kQVecPerThread; ++u) {
+                const int tt[4] = {t4[u].x, t4[u].y, t4[u].z, t4[u].w};
+                const float ww[4] = {w4[u].x, w4[u].y, w4[u].z, w4[u].w};
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    const uint32_t d = (d4[u] >> (8 * c)) & 0xffu;
+                    if (d != 0u) {
+                        const uint32_t pos = sh.sbase[d] + rank[u][c];
+                        sh.staged[pos] = make_int2(tt[c], __float_as_int(ww[c]));
+                        sh.sbin[pos] = (uint8_t)d;
+                    }
+                }
+            }
+            __syncthreads();
+            const int total = (int)sh.sbase[D + 1];
+            for (int p = threadIdx.x; p < total; p += kQThreads) {    // delay-sorted: consecutive threads, consecutive queue cells
+                const int d = sh.sbin[p];
+                int qs = nmodD + d; if (qs >= D) qs -= D;
+                const unsigned long long pos = sh.gbase[d] + (unsigned long long)(p - (int)sh.sbase[d]);
+                if (pos < (unsigned long long)a.q_cap) a.q_ev[(size_t)qs * (size_t)a.q_cap + pos] = sh.staged[p];
+                else overflow = true;
+            }
+            __syncthreads();                                   // staged / hist are rewritten by the next batch
+        }
+    }
+    if (overflow) a.ctl->err_queue = 1;
+    // event counter: one atomic per CTA
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) ev += __shfl_xor_sync(0xffffffffu, ev, o);
+    __syncthreads();
+    if (lane == 0 && wib < kEntryTile / 32) sh.gbase[wib] = ev;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned long long tot = 0;
+        for (int k = 0; k < kEntryTile / 32; ++k) tot += sh.gbase[k];
+        if (tot) atomicAdd(&a.ctl->events, tot);
+    }
+}
+
+__device__ __forceinline__ void queue_drain_phase(const StepArgs& a, float* __restrict__ plane1, const QueueShared& sh) {
+    const int D = a.D;
+    int qs = sh.nmodD + 1; if (qs >= D) qs -= D;               // arrival step n + 1
+    const unsigned long long T0 = __ldcg(a.q_tail + (size_t)qs * kQTailStride);
+    const long long T = (long long)(T0 < (unsigned long long)a.q_cap ? T0 : (unsigned long long)a.q_cap);
+    const int2* __restrict__ q = a.q_ev + (size_t)qs * (size_t)a.q_cap;
+    const long long gtid = (long long)blockIdx.x * blockDim.x + threadIdx.x, gthreads = (long long)gridDim.x * blockDim.x;
+    for (long long i = gtid; i < (T >> 1); i += gthreads) {    // two events per 128-bit load
+        const int4 v = ld_stream_s32x4(reinterpret_cast<const int32_t*>(q + 2 * i));
+        red_add_f32(plane1 + v.x, __int_as_float(v.y));
+        red_add_f32(plane1 + v.z, __int_as_float(v.w));
+    }
+    if ((T & 1) && gtid == 0) { const int2 v = q[T - 1]; red_add_f32(plane1 + v.x, __int_as_float(v.y)); }
 }
 
 // ---------------------------------------------------------------------------------------
@@ -1653,7 +1834,12 @@ __global__ void __launch_bounds__(kUpdateThreads) update_kernel(const StepArgs a
         sc.slot = __ldcg(&a.ctl->slot);
         sc.rec_base = __ldcg(&a.ctl->rec_total[sc.n & 1]);
         win_base = a.win_id ? __ldcg(&a.ctl->win_start[(unsigned long long)sc.n % (unsigned)(a.D + 1)]) : 0ULL;
-        if (blockIdx.x == 0) { a.ctl->step_d = sc.n; a.ctl->slot_d = sc.slot; }
+        if (blockIdx.x == 0) {
+            a.ctl->step_d = sc.n; a.ctl->slot_d = sc.slot;
+            // event-queue backend: the queue of arrival step n was drained by the delivery of step n-1 and is appended
+            // to again (as arrival step n + D) by the delivery of this step
+            if (a.q_tail) a.q_tail[(size_t)(sc.n % a.D) * kQTailStride] = 0ULL;
+        }
     }
     const PopDev* P = stage_pops(a, sh_pops);              // contains the __syncthreads that publishes sc
     if (a.n_pops > kMaxPopsSmem) __syncthreads();
@@ -1685,6 +1871,39 @@ __global__ void __launch_bounds__(kDeliverThreads, 3) deliver_kernel(const StepA
         if (gtid == 0) window_bookkeeping(a, sc.n, ws);
     }
     if (gtid == 0) bookkeeping_scalar(a, sc.n, sc.slot, M, __ldcg(&a.ctl->rec_total[sc.n & 1]));
+}
+
+// Delivery kernel 5 as a stand-alone launch (one per time step, after update_kernel).
+__global__ void __launch_bounds__(kQThreads, 2) queue_deliver_kernel(const StepArgs a) {
+    __shared__ QueueShared sh;
+    __shared__ StepScalars sc;
+    if (threadIdx.x == 0) {
+        sc.n = __ldcg(&a.ctl->step_d);
+        sc.slot = __ldcg(&a.ctl->slot_d);
+        sc.M = __ldcg(&a.ctl->spike_cnt[sc.n & 3]);
+        sh.nmodD = (int)(sc.n % a.D);
+    }
+    __syncthreads();
+    float* __restrict__ plane1 = a.ring + (size_t)(sc.slot == 0 ? 1 : 0) * a.NR;       // two planes: this step's and the next step's input
+    if (blockIdx.x & 1) { queue_append_phase(a, sc.n, sc.M, plane1, sh); queue_drain_phase(a, plane1, sh); }
+    else { queue_drain_phase(a, plane1, sh); queue_append_phase(a, sc.n, sc.M, plane1, sh); }
+    if (blockIdx.x == 0 && threadIdx.x == 0) bookkeeping_scalar(a, sc.n, sc.slot, sc.M, __ldcg(&a.ctl->rec_total[sc.n & 1]));
+}
+
+// Event-queue backend, read-back only (NG_FIELD_RING): add the queued events of the pending arrival steps n+1 .. n+D-1 to
+// a [D][NR] ring image (the plane of step n itself is copied by the host).
+__global__ void materialize_queues_kernel(const StepArgs a, long long n, float* __restrict__ out) {
+    const int D = a.D;
+    const long long gtid = (long long)blockIdx.x * blockDim.x + threadIdx.x, gthreads = (long long)gridDim.x * blockDim.x;
+    for (int k = 1; k < D; ++k) {
+        const int qs = (int)((n + k) % D);
+        const unsigned long long T0 = a.q_tail[(size_t)qs * kQTailStride];
+        const long long T = (long long)(T0 < (unsigned long long)a.q_cap ? T0 : (unsigned long long)a.q_cap);
+        for (long long i = gtid; i < T; i += gthreads) {
+            const int2 e = a.q_ev[(size_t)qs * (size_t)a.q_cap + i];
+            atomicAdd(out + (size_t)qs * a.NR + e.x, __int_as_float(e.y));
+        }
+    }
 }
 
 // One persistent cooperative kernel for n_steps steps: the two phases separated by grid-wide barriers (grid_barrier)

@@ -1,9 +1,18 @@
 """GPU parity of the AdEx path (the model of the paper's balanced network) against the fp64 oracle.
 
-Bars: connectivity with receptor ports bit-exact; lockstep (the GPU is fed the oracle's state, rounded to fp32, every
-step): spike lists identical except neurons on the exponential upswing (V > -45 mV before the step: "away from the
-peaks", logged); V within 5e-3 mV, w within 5e-2 pA, conductances within 1e-4 relative; delivered inputs per
-port within 1e-5 of their L1 mass (C12); free-running population rates within 5 % (C17)."""
+Bars.  Connectivity with receptor ports bit-exact.  Lockstep (the GPU is fed the oracle's state, rounded to fp32, every
+step; the GPU integrates in fp32 with __expf / __powf, "single precision"): tolerances are twice the largest
+error measured over 2.4e6 neuron-steps of this protocol (C23; the paper reports "a few 1e-4 mV" against NEST
+away from the peaks):
+  V      2e-5 mV   while the oracle's V after the step is more than 42 mV below V_peak,
+         2e-3 mV   between 42 and 30 mV below V_peak (the exponential term amplifies any rounding difference there);
+                   within 30 mV of V_peak the neuron crosses the peak within microseconds: exempt, logged;
+  w      2e-4 pA;  g_ex, y_ex 1.5e-5;  g_in, y_in 4e-6 (nS, nS/ms); each plus 2e-6 relative (33 fp32 ulp);
+  neurons that spiked in the step on both sides reset on different sub-step boundaries: V within 1e-2 mV, w within 5e-3 pA
+  (measured 4.1e-3 / 2.2e-3);
+  spike lists identical, except a neuron for which the side that did NOT spike ends the step within 30 mV of V_peak
+  (its spike falls into the next step): logged, at most 3 per run;
+  delivered inputs per port within 1e-5 of their L1 mass (C12); free-running population rates within 5 % (C17)."""
 import numpy as np
 import pytest
 
@@ -18,6 +27,9 @@ pytestmark = pytest.mark.gpu
 def B():
     from paper_2007_14236_b200 import binding
     return binding
+
+
+SPIKED_V_TOL, SPIKED_W_TOL = 1e-2, 5e-3       # neurons that spiked in the step (both sides), mV / pA: see the module docstring
 
 
 def adex_fields(B, oracle_mod):
@@ -43,7 +55,7 @@ def structure_with_ports(g, o, N):
     return src[keep][go], port[go]
 
 
-@pytest.mark.parametrize("mode,kernel", [(2, 3), (0, 3), (0, 1), (0, 4)])
+@pytest.mark.parametrize("mode,kernel", [(2, 3), (0, 3), (0, 1), (0, 4), (0, 5)])
 def test_adex_lockstep(oracle_mod, B, mode, kernel):
     wl = W.balanced_adex(n=2000, k_total=100, n_steps=400, seed=3)
     o, g = make_adex_pair(wl, oracle_mod, B, pre_options={B.OPT_DELIVERY_KERNEL: kernel, B.OPT_STEP_MODE: mode})
@@ -55,7 +67,8 @@ def test_adex_lockstep(oracle_mod, B, mode, kernel):
     osrc, otgt, ow, od, oro = o.get_connections()
     oport = np.where(osrc < 1600, 0, 1)
     mass = np.zeros((D, 2, N))
-    n_spk, logged = 0, []
+    n_spk, logged, n_exempt = 0, [], 0
+    V_PEAK = wl.populations[0][2]["V_peak"]
     for n in range(400):
         st = {}
         for gf, of in fields:
@@ -63,21 +76,29 @@ def test_adex_lockstep(oracle_mod, B, mode, kernel):
             g.set_state(gf, st[of].astype(np.float32))
         in_or = o.get_state(oracle_mod.FIELD_RING, 2 * N, first=(n % D) * 2 * N).reshape(2, N)
         m_in = mass[n % D].copy(); mass[n % D] = 0.0
-        upswing = st[oracle_mod.FIELD_V] > -45.0
         g.simulate(1); o.simulate(1, record=False)
         gs = np.sort(g.last_spikes()); os_ = np.sort(o.last_spikes())
         diff = np.setxor1d(gs, os_)
-        assert np.all(upswing[diff]), (n, diff[~upswing[diff]][:10])
-        logged += diff.tolist(); n_spk += os_.size
+        oV = o.get_state(oracle_mod.FIELD_V); gV = g.get_state(B.FIELD_V).astype(np.float64)
+        v_other = np.where(np.isin(diff, os_), gV[diff], oV[diff])      # V after the step on the side that did not spike
+        assert np.all(v_other >= V_PEAK - 30.0), (n, diff, v_other)
+        logged += [(n, int(i), float(v)) for i, v in zip(diff, v_other)]; n_spk += os_.size
         gin = g.get_state(B.FIELD_LAST_INPUT).astype(np.float64).reshape(2, N)
         assert np.all(np.abs(gin - in_or) <= 1e-5 * m_in + 1e-12), (n, float(np.abs(gin - in_or).max()))
-        calm = ~upswing
-        calm[diff] = False
-        for (gf, of), tol_abs, tol_rel in zip(fields, (5e-3, 5e-2, 1e-6, 1e-5, 1e-6, 1e-5, 0), (0, 0, 1e-4, 1e-4, 1e-4, 1e-4, 0)):
-            if gf == B.FIELD_ADEX_H:
-                continue                                   # the controller may take different sub-steps in fp32
+        same = np.ones(N, bool); same[diff] = False
+        both = np.intersect1d(gs, os_)                     # spiked on both sides: reset on different sub-step boundaries
+        same[both] = False
+        assert np.all(np.abs(gV - oV)[both] <= SPIKED_V_TOL), (n, float(np.abs(gV - oV)[both].max()))
+        gw, ow_ = g.get_state(B.FIELD_ADEX_W).astype(np.float64), o.get_state(oracle_mod.FIELD_W)
+        assert np.all(np.abs(gw - ow_)[both] <= SPIKED_W_TOL), (n, float(np.abs(gw - ow_)[both].max()))
+        calm = same & (oV < V_PEAK - 42.0)
+        rising = same & (oV >= V_PEAK - 42.0) & (oV < V_PEAK - 30.0)
+        n_exempt += int(np.sum(same & (oV >= V_PEAK - 30.0)))
+        assert np.all(np.abs(gV - oV)[calm] <= 2e-5), (n, float(np.abs(gV - oV)[calm].max()))
+        assert np.all(np.abs(gV - oV)[rising] <= 2e-3), (n, float(np.abs(gV - oV)[rising].max()))
+        for (gf, of), tol in zip(fields[1:6], (2e-4, 1.5e-5, 1.5e-5, 4e-6, 4e-6)):
             a, b = g.get_state(gf).astype(np.float64), o.get_state(of)
-            assert np.all(np.abs(a - b)[calm] <= tol_abs + tol_rel * np.abs(b)[calm]), (n, gf, float(np.abs(a - b)[calm].max()))
+            assert np.all(np.abs(a - b)[same] <= tol + 2e-6 * np.abs(b)[same]), (n, gf, float(np.abs(a - b)[same].max()))
         for j in os_.tolist():
             lo, hi = oro[j], oro[j + 1]
             np.add.at(mass, ((n + od[lo:hi].astype(np.int64)) % D, oport[lo:hi], otgt[lo:hi]), np.abs(ow[lo:hi].astype(np.float64)))
@@ -86,7 +107,8 @@ def test_adex_lockstep(oracle_mod, B, mode, kernel):
                 g.set_state(B.FIELD_RING, o.get_state(oracle_mod.FIELD_RING).astype(np.float32))
             except B.NgError:
                 break
-    assert n_spk > 50 and len(logged) <= max(3, n_spk // 20), (n_spk, logged)
+    print(f"adex lockstep: {n_spk} spikes, mismatches logged {logged}, neuron-steps exempt from the V bound {n_exempt}")
+    assert n_spk > 50 and len(logged) <= 3 and n_exempt <= 400, (n_spk, logged, n_exempt)
     g.close()
 
 

@@ -36,11 +36,12 @@ def ring_mass(o, wl, oracle_mod, n_steps, spikes_by_step):
     (100, 0.05, 3, 0), (1000, 0.01, 3, 1), (1000, 0.002, 3, 2), (37, 0.03, 3, 2), (3, 0.5, 3, 0), (1500, 0.3, 3, 0),
     (1500, 0.3, 3, 2), (1000, 0.05, 1, 0),
     (100, 0.05, 4, 0), (1000, 0.01, 4, 1), (1000, 0.002, 4, 2), (37, 0.03, 4, 2), (3, 0.5, 4, 0), (1500, 0.3, 4, 0),
+    (100, 0.05, 5, 0), (1000, 0.01, 5, 1), (1000, 0.002, 5, 0), (37, 0.03, 5, 1), (3, 0.5, 5, 0), (1500, 0.3, 5, 0),
 ])
 def test_delivery_only_matches_oracle(oracle_mod, B, K, fraction, kernel, mode):
     n, steps = 20000, 70                       # 70 > D = 64: the ring wraps
     wl = W.delivery_microbench(n=n, K=K, fraction=fraction, n_steps=steps, seed=5)
-    o, g = make_pair(wl, oracle_mod, debug_input=False, pre_options={B.OPT_DELIVERY_KERNEL: kernel} if kernel == 4 else None)
+    o, g = make_pair(wl, oracle_mod, debug_input=False, pre_options={B.OPT_DELIVERY_KERNEL: kernel} if kernel >= 4 else None)
     g.set_option(B.OPT_DELIVERY_KERNEL, kernel)
     g.set_option(B.OPT_STEP_MODE, mode)
     g.simulate(steps)
@@ -205,12 +206,13 @@ def test_cfg3_full_size_sampled(oracle_mod, B, K, fraction):
     g.close()
 
 
-def test_spike_buffer_backend_api(B):
-    """Delivery kernel 4 must be chosen before ng_prepare, cannot be left afterwards, and NG_FIELD_RING is read-only."""
+@pytest.mark.parametrize("kernel", [4, 5])
+def test_spike_buffer_backend_api(B, kernel):
+    """Delivery kernels 4 and 5 must be chosen before ng_prepare, cannot be left afterwards, and NG_FIELD_RING is read-only."""
     wl = W.delivery_microbench(n=5000, K=50, fraction=0.05, n_steps=10, seed=2)
     g = B.Sim(0.1, wl.ring_slots, wl.seed, record_spikes=True)
-    wl.apply(g); g.set_option(B.OPT_DELIVERY_KERNEL, 4); g.prepare()
-    assert g.stats().delivery_kernel == 4
+    wl.apply(g); g.set_option(B.OPT_DELIVERY_KERNEL, kernel); g.prepare()
+    assert g.stats().delivery_kernel == kernel
     with pytest.raises(B.NgError):
         g.set_option(B.OPT_DELIVERY_KERNEL, 1)
     g.simulate(5)
@@ -222,5 +224,21 @@ def test_spike_buffer_backend_api(B):
     g2 = B.Sim(0.1, wl.ring_slots, wl.seed)
     wl.apply(g2); g2.prepare()
     with pytest.raises(B.NgError):
-        g2.set_option(B.OPT_DELIVERY_KERNEL, 4)
+        g2.set_option(B.OPT_DELIVERY_KERNEL, kernel)
     g2.close()
+
+
+def test_event_queue_overflow_is_reported(B):
+    """Delivery kernel 5 with queues too small for the load: ng_simulate returns NG_ERR_OVERFLOW (events were dropped),
+    nothing is written out of bounds, and the simulator keeps running."""
+    wl = W.delivery_microbench(n=20000, K=200, fraction=0.2, n_steps=10, seed=2)      # 8e5 events per step
+    g = B.Sim(0.1, wl.ring_slots, wl.seed, record_spikes=False)
+    wl.apply(g); g.set_option(B.OPT_DELIVERY_KERNEL, 5); g.set_option(B.OPT_QUEUE_CAPACITY, 20000); g.prepare()
+    with pytest.raises(B.NgError) as e:
+        g.simulate(10)
+    assert e.value.code == B.NG_ERR_OVERFLOW
+    g.simulate(3, allow_overflow=True)
+    assert g.get_state(B.FIELD_STEP) == 13
+    ring = g.get_state(B.FIELD_RING)
+    assert np.all(np.isfinite(ring)) and np.count_nonzero(ring) > 0
+    g.close()
