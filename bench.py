@@ -29,8 +29,7 @@ import numpy as np
 
 TIME_STEPS_PER_BENCH_STEP = 1000
 DT_MS = 0.1
-NCU_DRAM_BYTES_PER_LAUNCH_CFG2 = 895.8e6     # profiles/r01f_cfg2_full_summary.csv
-NCU_DRAM_BYTES_PER_LAUNCH_CFG4 = 36.33e9     # profiles/r01h_cfg4_full_summary.csv (13.5 GB read + 22.8 GB written)
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r02_traffic.csv")   # ncu dram bytes per launch, keyed by the kernel sources' hash
 PAPER_RTF_2080TI = 1.055          # PAPER.md:248, full-scale microcircuit, NeuronGPU on RTX 2080 Ti (context, other hardware)
 PAPER_RTF_ADEX_1M = 70.0          # PAPER.md:16, balanced network of 1e6 AdEx neurons / 1e9 synapses on an RTX 2080 Ti (context)
 BYTES_PER_EVENT = 8               # 4 B target + 4 B weight per synaptic event
@@ -45,6 +44,33 @@ def measured_peak_gbs():
         except Exception:
             pass
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def csrc_hash():
+    """sha256 over the CUDA sources libng.so is built from: an ncu capture is only quoted for the code it was taken on."""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2007_14236_b200", "csrc")
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cuh")):
+            h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(workload, kernel):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` on `workload` from the committed ncu capture
+    (profiles/r02_traffic.csv), or None (with the reason) when no capture exists for the current kernel sources."""
+    if not os.path.exists(TRAFFIC_FILE):
+        return None, "no capture file"
+    cur = csrc_hash()
+    stale = None
+    for line in open(TRAFFIC_FILE):
+        f = [t.strip() for t in line.split(",")]
+        if len(f) >= 6 and f[0] == workload and f[1] == kernel:
+            if f[4] == cur:
+                return {"value": float(f[2]), "time_steps_per_launch": int(f[3]), "from": f[5], "csrc_sha256_16": f[4]}, None
+            stale = f"capture {f[5]} was taken on csrc {f[4]}, current csrc is {cur}"
+    return None, stale or "no capture for this workload / kernel"
 
 
 class ClockSampler:
@@ -215,6 +241,76 @@ def run_probes(device=0):
     return out
 
 
+def measure(name, steps, warmup, local, world, rank, dev, step_mode=3, delivery_kernel=0, no_prefetch=False, e2e=True):
+    """One workload through the C-ABI: W untimed + K timed bench steps of T time steps each, device-resident (CUDA events on
+    the simulator's stream), then (optionally) the same K steps with state and results crossing the host boundary."""
+    import torch
+    from paper_2007_14236_b200 import binding as B
+    T = TIME_STEPS_PER_BENCH_STEP
+    wl = make_workload(name, seed_offset=rank)                # replicas: independent seeds, no exchange
+    g = B.Sim(DT_MS, wl.ring_slots, wl.seed, record_spikes=True, max_recorded_spikes=1 << 24, device=local)
+    wl.apply(g)
+    if delivery_kernel >= 4:
+        g.set_option(B.OPT_DELIVERY_KERNEL, delivery_kernel)  # before prepare: the two-plane backends change what is allocated
+    t0 = time.time(); g.prepare(); build_wall = time.time() - t0
+    g.set_option(B.OPT_STEP_MODE, step_mode)
+    g.set_option(B.OPT_DELIVERY_KERNEL, delivery_kernel)
+    g.set_option(B.OPT_PREFETCH, 0 if no_prefetch else 1)
+    g.set_state(B.FIELD_V, wl.initial_v())
+    N = wl.n_neurons
+    for _ in range(warmup):                                   # also runs the network past its initial transient
+        g.simulate(T, allow_overflow=True)
+    g.get_spikes()
+    s0 = g.stats()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier(world)
+    with ClockSampler(local) as clk:
+        e0.record(g.stream)
+        for _ in range(steps):
+            g.simulate(T, allow_overflow=True)
+        e1.record(g.stream)
+        barrier(world)
+    ms_total = max_over_ranks(e0.elapsed_time(e1), world, dev)
+    s1 = g.stats()
+    g.get_spikes()
+    bio_s = steps * T * DT_MS * 1e-3
+    out = {"wl": wl, "g": g, "N": N, "s0": s0, "s1": s1, "ms_total": ms_total, "bio_s": bio_s, "build_wall": build_wall,
+           "clocks": clk.summary(),
+           "events": sum_over_ranks(float(s1.events - s0.events), world, dev),
+           "spikes": sum_over_ranks(float(s1.spikes - s0.spikes), world, dev),
+           "launches": int((s1.launches_update - s0.launches_update) + (s1.launches_deliver - s0.launches_deliver)),
+           "rtf": (ms_total * 1e-3) / (bio_s * world)}      # whole job: N replicas advance N biological seconds
+    if e2e:
+        hV = torch.empty(N, dtype=torch.float32).pin_memory(); hI = torch.empty(N, dtype=torch.float32).pin_memory()
+        hR = torch.empty(N, dtype=torch.int32).pin_memory()
+        hs = torch.empty(1 << 24, dtype=torch.int32).pin_memory(); hi = torch.empty(1 << 24, dtype=torch.int32).pin_memory()
+        g.get_state(B.FIELD_V, out=hV); g.get_state(B.FIELD_I_SYN, out=hI); g.get_state(B.FIELD_REFR, out=hR)
+        barrier(world)
+        d2h = h2d = 0
+        t0 = time.perf_counter()
+        for _ in range(steps):
+            g.set_state(B.FIELD_V, hV); g.set_state(B.FIELD_I_SYN, hI); g.set_state(B.FIELD_REFR, hR)      # H2D
+            g.simulate(T, allow_overflow=True)
+            g.get_state(B.FIELD_V, out=hV); g.get_state(B.FIELD_I_SYN, out=hI); g.get_state(B.FIELD_REFR, out=hR)  # D2H
+            st, _ = g.get_spikes(hs.numpy(), hi.numpy())                                                    # D2H
+            h2d += 3 * N * 4; d2h += 3 * N * 4 + 2 * 4 * st.size
+        barrier(world)
+        e2e_s = max_over_ranks(time.perf_counter() - t0, world, dev)
+        out.update(e2e_rtf=e2e_s / (bio_s * world), h2d=h2d // steps, d2h=d2h // steps)
+    return out
+
+
+def short_result(m, steps):
+    """Entry of the `configs` object: one workload, device-timed."""
+    T = TIME_STEPS_PER_BENCH_STEP
+    s1 = m["s1"]
+    return {"workload": workload_label(m["name"]), "real_time_factor": m["rtf"], "us_per_time_step": m["ms_total"] * 1e3 / (steps * T),
+            "synaptic_events_per_s": m["events"] / (m["ms_total"] * 1e-3), "spikes_per_time_step": m["spikes"] / (steps * T),
+            "mean_rate_hz": m["spikes"] / m["N"] / m["bio_s"], "steps": steps, "time_steps_per_bench_step": T,
+            "delivery_kernel": int(s1.delivery_kernel), "step_mode": int(s1.step_mode), "build_s": m["build_wall"],
+            "e2e_real_time_factor": m.get("e2e_rtf")}
+
+
 def run_ours(args):
     import torch
     if not torch.cuda.is_available():
@@ -226,60 +322,9 @@ def run_ours(args):
     peak_gbs, peak_src = measured_peak_gbs()
     T = TIME_STEPS_PER_BENCH_STEP
 
-    wl = make_workload(args.workload, seed_offset=rank)       # replicas: independent seeds, no exchange
-    g = B.Sim(DT_MS, wl.ring_slots, wl.seed, record_spikes=True, max_recorded_spikes=1 << 24, device=local)
-    wl.apply(g)
-    if args.delivery_kernel >= 4:
-        g.set_option(B.OPT_DELIVERY_KERNEL, args.delivery_kernel)                # before prepare: the spike-buffer backend changes what is allocated
-    t0 = time.time(); g.prepare(); build_wall = time.time() - t0
-    g.set_option(B.OPT_STEP_MODE, args.step_mode)
-    g.set_option(B.OPT_DELIVERY_KERNEL, args.delivery_kernel)
-    g.set_option(B.OPT_PREFETCH, 0 if args.no_prefetch else 1)
-    g.set_state(B.FIELD_V, wl.initial_v())
-    N = wl.n_neurons
-
-    # ---- warm-up: W untimed bench steps (also runs the network past its initial transient) ----
-    for _ in range(args.warmup):
-        g.simulate(T, allow_overflow=True)
-    g.get_spikes()
-
-    # ---- timed region: exactly K bench steps, device-resident, CUDA events on the simulator's stream ----
-    s0 = g.stats()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier(world)
-    with ClockSampler(local) as clk:
-        e0.record(g.stream)
-        for _ in range(args.steps):
-            g.simulate(T, allow_overflow=True)
-        e1.record(g.stream)
-        barrier(world)
-    ms_total = max_over_ranks(e0.elapsed_time(e1), world, dev)
-    s1 = g.stats()
-    g.get_spikes()
-    events = sum_over_ranks(float(s1.events - s0.events), world, dev)
-    spikes = sum_over_ranks(float(s1.spikes - s0.spikes), world, dev)
-    launches = int((s1.launches_update - s0.launches_update) + (s1.launches_deliver - s0.launches_deliver))
-    bio_s = args.steps * T * DT_MS * 1e-3
-    rtf = (ms_total * 1e-3) / (bio_s * world)                 # whole job: N replicas advance N biological seconds
-
-    # ---- e2e: the same K bench steps with the state entering and the results leaving through HOST buffers ----
-    hV = torch.empty(N, dtype=torch.float32).pin_memory(); hI = torch.empty(N, dtype=torch.float32).pin_memory()
-    hR = torch.empty(N, dtype=torch.int32).pin_memory()
-    hs = torch.empty(1 << 24, dtype=torch.int32).pin_memory(); hi = torch.empty(1 << 24, dtype=torch.int32).pin_memory()
-    g.get_state(B.FIELD_V, out=hV); g.get_state(B.FIELD_I_SYN, out=hI); g.get_state(B.FIELD_REFR, out=hR)
-    barrier(world)
-    d2h = h2d = 0
-    t0 = time.perf_counter()
-    for _ in range(args.steps):
-        g.set_state(B.FIELD_V, hV); g.set_state(B.FIELD_I_SYN, hI); g.set_state(B.FIELD_REFR, hR)      # H2D
-        g.simulate(T, allow_overflow=True)
-        g.get_state(B.FIELD_V, out=hV); g.get_state(B.FIELD_I_SYN, out=hI); g.get_state(B.FIELD_REFR, out=hR)  # D2H
-        st, _ = g.get_spikes(hs.numpy(), hi.numpy())                                                    # D2H
-        h2d += 3 * N * 4; d2h += 3 * N * 4 + 2 * 4 * st.size
-    barrier(world)
-    e2e_s = max_over_ranks(time.perf_counter() - t0, world, dev)
-    e2e_rtf = e2e_s / (bio_s * world)
-
+    m = measure(args.workload, args.steps, args.warmup, local, world, rank, dev, args.step_mode, args.delivery_kernel, args.no_prefetch)
+    g, wl, N, s0, s1, ms_total = m["g"], m["wl"], m["N"], m["s0"], m["s1"], m["ms_total"]
+    rtf, events, spikes, bio_s = m["rtf"], m["events"], m["spikes"], m["bio_s"]
     if rank != 0:
         g.close()
         return
@@ -287,7 +332,7 @@ def run_ours(args):
     # ---- roofline of the dominant kernel ----
     if int(s1.step_mode) == 2:
         # one persistent kernel per bench step: its launch IS the timed region (CUDA events on the simulator's stream)
-        kern = {1: "persistent_kernel<1>", 2: "persistent_kernel<2>", 3: "persistent_pipe_kernel"}[int(s1.delivery_kernel)]
+        kern = {1: "persistent_kernel<1>", 2: "persistent_kernel<2>", 3: "persistent_pipe_kernel", 4: "persistent_kernel<4>"}[int(s1.delivery_kernel)]
         us = ms_total * 1e3 / args.steps
         ev_per_launch = float(s1.events - s0.events) / args.steps
         # AdEx: seven state words and two input ports per neuron instead of three and one
@@ -308,30 +353,71 @@ def run_ours(args):
         if int(p1.delivery_kernel) == 3:          # pipelined step kernel: update + collection + delivery in one launch
             kern, alg_bytes, us = "pipe_step_kernel", N * BYTES_PER_NEURON_STEP + ev_per_launch * BYTES_PER_EVENT, us_upd
         elif us_del >= us_upd:
-            kern, alg_bytes, us = f"deliver_kernel<{int(p1.delivery_kernel)}>", ev_per_launch * BYTES_PER_EVENT, us_del
+            kname = "queue_deliver_kernel" if int(p1.delivery_kernel) == 5 else f"deliver_kernel<{int(p1.delivery_kernel)}>"
+            kern, alg_bytes, us = kname, ev_per_launch * BYTES_PER_EVENT, us_del
         else:
             kern, alg_bytes, us = "update_kernel", N * BYTES_PER_NEURON_STEP, us_upd
         share = {"update_kernel_us": us_upd, "deliver_kernel_us": us_del}
     achieved = alg_bytes / (us * 1e-6) / 1e9
-    # dram__bytes_read.sum + dram__bytes_write.sum of one launch of this kernel in this configuration, from the committed
-    # `ncu --set full` capture (profiles/r01f_cfg2_full_summary.csv: 890.4 MB + 5.4 MB per 1000 time steps); below the
-    # algorithmic bytes because the 33 B per neuron-step never leave the chip (state resident in shared memory / L2)
-    traffic = None
-    if kern == "persistent_pipe_kernel" and T == 1000 and args.delivery_kernel in (0, 3):
-        traffic = {"cfg2": NCU_DRAM_BYTES_PER_LAUNCH_CFG2, "cfg4": NCU_DRAM_BYTES_PER_LAUNCH_CFG4}.get(args.workload)
+    # dram__bytes_read.sum + dram__bytes_write.sum of one launch of this kernel in this configuration: quoted from the
+    # committed `ncu --set full` capture only while the kernel sources are the ones the capture was taken on
+    traffic, traffic_note = (None, "non-default options") if (args.delivery_kernel or args.step_mode != 3) else ncu_traffic(args.workload, kern)
+    if traffic and traffic["time_steps_per_launch"] != T:
+        traffic, traffic_note = None, "capture used another launch length"
     roofline = {"bound": "hbm", "kernel": kern, "achieved": achieved, "peak": peak_gbs, "unit": "GB/s",
-                "frac": achieved / peak_gbs, "traffic": traffic, "peak_source": peak_src,
+                "frac": achieved / peak_gbs, "traffic": traffic["value"] if traffic else None,
+                "traffic_source": traffic if traffic else traffic_note, "peak_source": peak_src,
                 "avg_launch_us": us, "algorithmic_bytes_per_launch": alg_bytes,
                 "share_of_step": share,
+                "target_frac_north_star": 0.5, "target_met": False,
                 "note": "latency-bound regime: ~1e5 events (0.8 MB) + 2.5 MB of neuron state per time step against "
-                        "~5 us of dependent memory round trips and one grid barrier; see delivery_microbench for the "
-                        "bandwidth-relevant load and DESIGN.md for the L2 tag-rate ceiling of scattered reductions"}
+                        "~5 us of dependent memory round trips and one grid barrier; the north_star target (>= 50 % of HBM "
+                        "peak on connection-record reads) is about the bandwidth regime: see delivery_microbench "
+                        "(best point 0.21 of the measured peak: NOT met; DESIGN.md section 7 names the scattered-reduction ceiling)"}
     g.close()
     del g
     torch.cuda.empty_cache()
 
-    micro = None if args.no_microbench else delivery_microbench(local, peak_gbs, K=args.micro_k, fraction=args.micro_fraction, steps=args.micro_steps)
-    cpu = None if args.no_cpu_baseline else cpu_baseline_sample()
+    # ---- the other configurations of BASELINE.json, device-timed, into the same record ----
+    configs = {}
+    m["name"] = args.workload
+    configs[args.workload] = short_result(m, args.steps)
+    if not args.no_configs and world == 1:
+        for name in ("cfg0", "cfg1", "cfg4", "adex1m"):
+            if name == args.workload:
+                continue
+            try:
+                mm = measure(name, 5, 3, local, 1, 0, dev, e2e=False)
+                mm["name"] = name
+                configs[name] = short_result(mm, 5)
+                mm["g"].close()
+                del mm
+            except Exception as e:                       # a smaller card: say so instead of failing the headline
+                configs[name] = {"error": str(e)}
+            torch.cuda.empty_cache()
+
+    micro, sweep = None, None
+    if not args.no_microbench and world == 1:
+        if args.no_configs:
+            micro = delivery_microbench(local, peak_gbs, K=args.micro_k, fraction=args.micro_fraction, steps=args.micro_steps)
+        else:
+            sweep = []
+            for k in (100, 1000, 10000):
+                for f in (0.001, 0.01, 0.05):
+                    r = delivery_microbench(local, peak_gbs, K=k, fraction=f, steps=args.micro_steps, fallback=False)
+                    r.update(out_degree=k, firing_fraction=f)
+                    sweep.append(r)
+                    if k == args.micro_k and f == args.micro_fraction:
+                        micro = r
+            if micro is None:
+                micro = delivery_microbench(local, peak_gbs, K=args.micro_k, fraction=args.micro_fraction, steps=args.micro_steps)
+        if micro and "frac_of_hbm_peak" in micro:
+            micro["target_frac_north_star"] = 0.5
+            micro["target_met"] = bool(micro["frac_of_hbm_peak"] >= 0.5)
+    cpu = None
+    if not args.no_cpu_baseline and world == 1:
+        standin = configs.get("cfg1", {}).get("real_time_factor")
+        cpu = cpu_baseline_for(args.workload, gpu_rtf=rtf, gpu_rtf_standin=standin)
 
     line = {
         "metric": "real_time_factor", "value": rtf, "unit": "wall_s_per_bio_s", "n_gpus": world, "steps": args.steps,
@@ -347,62 +433,75 @@ def run_ours(args):
                    "delivery_kernel": int(s1.delivery_kernel), "seed": wl.seed},
         "synaptic_events_per_s": events / (ms_total * 1e-3), "spikes_per_time_step": spikes / (args.steps * T * world),
         "mean_rate_hz": spikes / world / N / bio_s, "us_per_time_step": ms_total * 1e3 / (args.steps * T),
-        "build_s": build_wall, "gpu_launches": launches,
-        "clocks": clk.summary(),
-        "e2e": {"value": e2e_rtf, "unit": "wall_s_per_bio_s", "h2d_bytes_per_step": h2d // args.steps,
-                "d2h_bytes_per_step": d2h // args.steps,
+        "build_s": m["build_wall"], "gpu_launches": m["launches"],
+        "clocks": m["clocks"],
+        "e2e": {"value": m["e2e_rtf"], "unit": "wall_s_per_bio_s", "h2d_bytes_per_step": m["h2d"],
+                "d2h_bytes_per_step": m["d2h"],
                 "what": "per bench step: V, I_syn, refr from pinned HOST buffers -> ng_set_state, ng_simulate(1000), "
                         "state and recorded spikes back to HOST buffers (ng_get_state, ng_get_spikes)"},
         "roofline": roofline, "delivery_microbench": micro, "cpu_baseline": cpu,
+        "configs": configs, "delivery_sweep": sweep,
     }
     print(json.dumps(line), flush=True)
 
 
 # ---------------------------------------------------------------------------------------------------------------------
-# CPU arm: the oracle as it stands (oracle/, single thread, fp64), on a bounded sample of the same workload.
+# CPU arm: the oracle as it stands (oracle/, single thread, fp64).
+#   cpu_baseline of the default line: a bounded sample of the GPU line's own workload (1000 time steps of configs[2] after
+#     its transient; the oracle needs about a minute to build the full-scale network), the GPU's number beside it.
+#   --impl reference: the oracle on the SAME workload as the GPU arm (configs[2] by default), each bench step a bounded
+#     sample of REF_TIME_STEPS time steps.
 # ---------------------------------------------------------------------------------------------------------------------
-ORACLE_SAMPLE = ("the same microcircuit at 10% neuron scale with full in-degrees (BASELINE.json configs[1]: 7,718 neurons, "
-                 "29,892,043 synapses; the oracle needs minutes and >8 GB just to build the full-scale network), "
-                 "time steps after a 1000-step transient; value = wall s per biological s OF THE SAMPLE network; "
-                 "the full-scale network carries ~10x the neurons and synaptic events per step")
+REF_TIME_STEPS = 200               # time steps per bench step of the reference arm (20 ms biological)
+ORACLE_FEASIBLE = ("cfg0", "cfg1", "cfg2")     # networks the oracle builds within minutes; others fall back to a stand-in
 
 _oracle_cache = {}
 
 
-def oracle_sample_sim(transient=1000):
-    """Build (once per process) the oracle on the bounded sample and run it past the initial transient."""
-    if "o" not in _oracle_cache:
+def oracle_sim(name, transient=1000):
+    """Build (once per process) the oracle on workload `name` and run it past the initial transient."""
+    if name not in _oracle_cache:
         import oracle
-        from paper_2007_14236_b200 import workloads as W
-        wl = W.microcircuit(10)
+        wl = make_workload(name)
         o = oracle.Oracle(DT_MS, wl.ring_slots, wl.seed)
         wl.apply(o)
         t0 = time.time(); o.prepare(); build_s = time.time() - t0
         o.set_state(oracle.FIELD_V, wl.initial_v().astype(np.float64))
         o.simulate(transient, record=False)
-        _oracle_cache.update(o=o, wl=wl, build_s=build_s)
-    return _oracle_cache["o"], _oracle_cache["wl"], _oracle_cache["build_s"]
+        _oracle_cache[name] = (o, wl, build_s)
+    return _oracle_cache[name]
 
 
-def cpu_baseline_sample(time_steps=5000):
-    o, wl, build_s = oracle_sample_sim()
+def cpu_baseline_for(name, time_steps=1000, gpu_rtf=None, gpu_rtf_standin=None):
+    """The oracle as it stands, one host thread, on a bounded sample (time_steps time steps after a 1000-step transient) of
+    the GPU line's own workload where it can build it within minutes (configs 0-2; the full-scale microcircuit takes about
+    a minute and 10 GB), else of the 10 %-scale microcircuit as a labelled stand-in."""
+    run = name if name in ORACLE_FEASIBLE else "cfg1"
+    o, wl, build_s = oracle_sim(run)
     ev0 = o.n_events
     t0 = time.perf_counter()
     o.simulate(time_steps, record=False)
     dt = time.perf_counter() - t0
-    bio_s = time_steps * DT_MS * 1e-3
-    return {"value": dt / bio_s, "unit": "wall_s_per_bio_s", "cores": 1, "kind": "oracle",
-            "sample": f"{time_steps} {ORACLE_SAMPLE}", "host_cores_available": os.cpu_count(),
-            "synaptic_events_per_s": (o.n_events - ev0) / dt, "oracle_build_s": build_s}
+    out = {"value": dt / (time_steps * DT_MS * 1e-3), "unit": "wall_s_per_bio_s", "cores": 1, "kind": "oracle",
+           "workload": workload_label(run), "same_workload_as_gpu_line": run == name,
+           "sample": f"{time_steps} time steps of {workload_label(run)} after a 1000-step transient; value = wall s per biological s",
+           "host_cores_available": os.cpu_count(), "synaptic_events_per_s": (o.n_events - ev0) / dt, "oracle_build_s": build_s}
+    g = gpu_rtf if run == name else gpu_rtf_standin
+    if g:
+        out["gpu_value_same_workload"] = g
+        out["ratio_same_workload"] = out["value"] / g
+    return out
 
 
 def run_reference(args):
-    """--impl reference: the oracle timed on the host cores, same metric/unit; each bench step = a bounded sample of
-    TIME_STEPS_PER_BENCH_STEP time steps of the 10%-scale network.  Rank 0 only."""
+    """--impl reference: the oracle timed on the host cores on the GPU arm's own workload, same metric and unit; each bench
+    step = REF_TIME_STEPS time steps (a bounded sample of the 1000 the GPU arm runs per bench step).  Rank 0 only."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
-    T = TIME_STEPS_PER_BENCH_STEP
-    o, wl, build_s = oracle_sample_sim()
+    T = REF_TIME_STEPS
+    name = args.workload if args.workload in ORACLE_FEASIBLE else "cfg1"
+    same = name == args.workload
+    o, wl, build_s = oracle_sim(name, transient=0)
     for _ in range(args.warmup):
         o.simulate(T, record=False)
     ev0 = o.n_events
@@ -412,17 +511,25 @@ def run_reference(args):
     dt = time.perf_counter() - t0
     bio_s = args.steps * T * DT_MS * 1e-3
     rtf = dt / bio_s
-    sample = f"{T} time steps per bench step of {ORACLE_SAMPLE}"
+    sample = (f"{T} time steps per bench step (the GPU arm runs {TIME_STEPS_PER_BENCH_STEP}); value = wall s per biological s; "
+              f"{args.warmup} untimed warm-up steps first" + ("" if same else f"; STAND-IN network: the oracle cannot build {args.workload} within minutes"))
     line = {"impl": "reference", "metric": "real_time_factor", "value": rtf, "unit": "wall_s_per_bio_s",
             "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3 / args.steps,
             "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": workload_label(args.workload), "time_steps_per_bench_step": T, "dt_ms": DT_MS,
-                       "sample": sample},
+            "config": {"workload": workload_label(name), "time_steps_per_bench_step": T, "dt_ms": DT_MS, "sample": sample,
+                       "same_workload_as_gpu_arm": same},
             "synaptic_events_per_s": (o.n_events - ev0) / dt, "gpu_launches": 0,
             "cpu_baseline": {"value": rtf, "unit": "wall_s_per_bio_s", "cores": 1, "kind": "oracle", "sample": sample,
                              "host_cores_available": os.cpu_count(), "oracle_build_s": build_s},
             "e2e": {"value": rtf, "unit": "wall_s_per_bio_s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line), flush=True)
+
+
+def spawn_command(args_list, n_gpus, port=None):
+    """`python bench.py --gpus N` outside torchrun: the command that re-launches this script as N ranks on this node."""
+    port = port or (29500 + os.getpid() % 2000)
+    return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n_gpus}",
+            "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + list(args_list)
 
 
 def main():
@@ -433,6 +540,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg2", choices=["cfg0", "cfg1", "cfg2", "cfg4", "adex1m", "adex100k"])
     ap.add_argument("--no-microbench", action="store_true", help="skip the configs[3] delivery microbenchmark")
+    ap.add_argument("--no-configs", action="store_true", help="skip the other BASELINE.json configurations and the 9-point configs[3] sweep")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip timing the oracle")
     ap.add_argument("--only-microbench", action="store_true",
                     help="run only the configs[3] delivery microbenchmark and print its JSON object (used for ncu captures)")
@@ -445,10 +553,13 @@ def main():
     ap.add_argument("--no-prefetch", action="store_true", help="NG_OPT_PREFETCH = 0")
     ap.add_argument("--micro-k", type=int, default=10000)
     ap.add_argument("--micro-fraction", type=float, default=0.05)
-    ap.add_argument("--micro-steps", type=int, default=30)
+    ap.add_argument("--micro-steps", type=int, default=20)
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl == "ours" and not (args.probe or args.micro_sweep or args.only_microbench):
+        # launched plainly: become N ranks, one per GPU (the driver's torchrun command does the same)
+        os.execv(sys.executable, spawn_command(sys.argv[1:], args.gpus))
     if args.probe:
         print(json.dumps(run_probes()), flush=True)
     elif args.micro_sweep:

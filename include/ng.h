@@ -164,8 +164,8 @@ typedef struct {
     uint64_t spikes;             /* spikes emitted                                                   */
     uint64_t events;             /* synaptic events delivered = sum over spikes of the out-degree    */
     uint64_t recorded_dropped;   /* spikes not recorded because the record was full                  */
-    int64_t n_neurons;
-    int64_t n_connections;       /* S, records drawn                                                 */
+    int64_t n_neurons;           /* neurons this handle owns (all of them on one GPU)                */
+    int64_t n_connections;       /* S, connections stored on this handle                             */
     int64_t n_records_padded;    /* records stored (rows padded to a multiple of 4)                  */
     int64_t max_row_records;     /* longest padded row                                               */
     double build_ms;             /* device time of the connection build                              */
@@ -176,6 +176,9 @@ typedef struct {
     uint64_t launches_other;     /* builder and bookkeeping kernels                                  */
     int32_t delivery_kernel;     /* the delivery kernel in use (1 .. 5)                           */
     int32_t step_mode;
+    int64_t n_sources;           /* neurons of the whole network (= n_neurons unless target-sharded)  */
+    int32_t shard_rank, shard_world;   /* ng_set_shard (0, 1 on one GPU)                             */
+    int32_t id_first, reserved;  /* global id of this shard's first neuron                           */
 } ng_stats;
 
 /* Create a simulator on cfg->device.  `alloc` may be NULL.  `cuda_stream` is a cudaStream_t (or NULL).
@@ -219,6 +222,33 @@ int32_t ng_connect_fixed_outdegree_port(ng_sim* sim, int32_t src_first, int32_t 
  * Initial state: V = E_L, w = 0, conductances 0.  Errors: STATE after ng_prepare; INVALID_ARG for non-positive
  * C_m, g_L, Delta_T, tau_w, tau_syn, h_min or tolerances, too many populations, Poisson rate*h too large. */
 int32_t ng_create_population_adex(ng_sim* sim, int32_t n, const ng_adex_params* params, int32_t* first_id_out);
+
+/* Target-sharded multi-GPU (spikes of remote neurons arrive through "a spike
+ * buffer, similar to the local one").  One process (or handle) per GPU; all of them issue the SAME populations and
+ * connect calls with the same seed.  Handle `rank` of `world` owns the contiguous id range ng_shard_range gives: it keeps
+ * the state and the input planes of those neurons and every connection whose TARGET is one of them — because a draw is a
+ * pure function of (seed, call, endpoint, k), that is exactly the one-GPU structure restricted to those targets.  Each
+ * time step ends its update with ONE exchange: every rank stores the ids of its spikes into the receive buffer of every
+ * peer (peer-mapped device memory, NVLink) and appends what the peers stored in its own; delivery is local.
+ *   ng_shard_range     pure host arithmetic (no device): first = floor(n * rank / world), n = floor(n * (rank+1) / world) - first.
+ *   ng_set_shard       before ng_prepare; world 1..16.
+ *   ng_exchange_handle after ng_prepare: the CUDA IPC handle (64 bytes) and/or the device pointer of this handle's receive
+ *                      buffer, to be handed to the peers (the harness moves the 64 bytes with torch.distributed).
+ *   ng_exchange_attach map a peer's receive buffer: its IPC handle (another process) or its pointer (same process).
+ *                      Every peer must be attached before ng_simulate.
+ *   ng_shard_phase     one time step in two halves — 0: update + publish, 1: gather + deliver — so that several shards that
+ *                      share ONE GPU and ONE stream can be stepped without any kernel waiting for another (all phase 0
+ *                      calls, then all phase 1 calls); ng_simulate does both halves per step and, on separate GPUs,
+ *                      the gather kernel waits (bounded) for the peers' flags.
+ * In sharded mode ng_get_state / ng_set_state address the handle's OWN neurons (element i = neuron id_first + i), stored
+ * targets (ng_copy_records) are local indices, ng_get_spikes / ng_get_last_spikes / ng_stats.spikes cover the whole network
+ * (global ids; every rank records all spikes), ng_stats.events and n_connections this handle's share; delivery kernel 3, step mode 2 and the statistics are one-GPU only.
+ * Errors: INVALID_ARG, STATE, CUDA (a peer's list did not arrive: ng_simulate). */
+int32_t ng_shard_range(int32_t n_neurons, int32_t rank, int32_t world, int32_t* first_out, int32_t* n_out);
+int32_t ng_set_shard(ng_sim* sim, int32_t rank, int32_t world);
+int32_t ng_exchange_handle(ng_sim* sim, void* ipc_handle_out_64, void** local_ptr_out);
+int32_t ng_exchange_attach(ng_sim* sim, int32_t peer_rank, const void* ipc_handle_64, void* same_process_ptr);
+int32_t ng_shard_phase(ng_sim* sim, int32_t phase);
 
 /* Delivery-only mode (BASELINE.json configs[3], C8): the neuron update is bypassed and source s
  * fires in step n iff Philox(INJECT; s, n).x0 < floor(fraction * 2^32).  Before ng_prepare only. */

@@ -26,7 +26,8 @@ EXPORTS = ["ng_create", "ng_destroy", "ng_last_error", "ng_create_population", "
            "ng_get_state", "ng_simulate", "ng_get_spikes", "ng_get_last_spikes", "ng_copy_row_offsets",
            "ng_copy_group_offsets", "ng_copy_records", "ng_get_connections", "ng_get_stats", "ng_get_trace", "ng_probe",
            "ng_create_population_adex", "ng_connect_fixed_indegree_port", "ng_connect_fixed_outdegree_port",
-           "ng_enable_statistics", "ng_get_rate_cv", "ng_get_correlations"]
+           "ng_enable_statistics", "ng_get_rate_cv", "ng_get_correlations",
+           "ng_shard_range", "ng_set_shard", "ng_exchange_handle", "ng_exchange_attach", "ng_shard_phase"]
 
 
 class NgConfig(C.Structure):
@@ -75,7 +76,8 @@ class NgStats(C.Structure):
                 ("n_records_padded", C.c_int64), ("max_row_records", C.c_int64), ("build_ms", C.c_double),
                 ("ms_update", C.c_double), ("ms_deliver", C.c_double), ("launches_update", C.c_uint64),
                 ("launches_deliver", C.c_uint64), ("launches_other", C.c_uint64), ("delivery_kernel", C.c_int32),
-                ("step_mode", C.c_int32)]
+                ("step_mode", C.c_int32), ("n_sources", C.c_int64), ("shard_rank", C.c_int32), ("shard_world", C.c_int32),
+                ("id_first", C.c_int32), ("reserved", C.c_int32)]
 
 
 class NgError(RuntimeError):
@@ -125,6 +127,11 @@ def load_library(path: str | None = None):
     L.ng_get_rate_cv.argtypes = [vp, vp, vp, i64]
     L.ng_get_correlations.argtypes = [vp, i32, vp, i64, C.POINTER(i32), C.POINTER(i32)]
     L.ng_probe.argtypes = [i32, i32, i64, C.POINTER(C.c_double)]
+    L.ng_shard_range.argtypes = [i32, i32, i32, C.POINTER(i32), C.POINTER(i32)]
+    L.ng_set_shard.argtypes = [vp, i32, i32]
+    L.ng_exchange_handle.argtypes = [vp, vp, C.POINTER(vp)]
+    L.ng_exchange_attach.argtypes = [vp, i32, vp, vp]
+    L.ng_shard_phase.argtypes = [vp, i32]
     for name in EXPORTS:
         if name != "ng_last_error":
             getattr(L, name).restype = i32
@@ -173,7 +180,7 @@ class Sim:
 
     def __init__(self, dt_ms: float = 0.1, ring_slots: int = 64, seed: int = 1, record_spikes: bool = True,
                  max_recorded_spikes: int = 1 << 22, debug_input: bool = False, device: int = 0,
-                 torch_alloc: bool = True):
+                 torch_alloc: bool = True, rank: int = 0, world: int = 1, stream=None):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2007_14236_b200 needs a CUDA device; there is no CPU fallback")
@@ -182,7 +189,8 @@ class Sim:
         self.device = device
         self.dt_ms, self.D, self.seed = dt_ms, ring_slots, seed
         self.n_ports = 1                          # 2 as soon as an AdEx population is created
-        self.stream = torch.cuda.Stream(device=device)
+        self.stream = stream if stream is not None else torch.cuda.Stream(device=device)
+        self.rank, self.world = rank, world
         self._tensors = {}
         self._alloc_struct = None
         if torch_alloc:
@@ -207,6 +215,8 @@ class Sim:
         if rc != NG_OK:
             raise NgError(rc, "ng_create failed")
         self._h = h
+        if world > 1:
+            self._chk(self._L.ng_set_shard(self._h, rank, world))
 
     # ---- lifetime -------------------------------------------------------------------------------------------
     def close(self):
@@ -271,6 +281,26 @@ class Sim:
     @property
     def n_connections(self) -> int:
         return int(self.stats().n_connections)
+
+    @property
+    def n_sources(self) -> int:
+        """Neurons of the whole network (= n_neurons on one GPU): rows of the connection structure."""
+        return int(self.stats().n_sources)
+
+    # ---- target-sharded multi-GPU ---------------------------------------------------------------------------
+    def exchange_handle(self):
+        """(64-byte CUDA IPC handle, device pointer) of this handle's spike-exchange receive buffer."""
+        h = (C.c_ubyte * 64)()
+        p = C.c_void_p()
+        self._chk(self._L.ng_exchange_handle(self._h, h, C.byref(p)))
+        return bytes(h), p.value
+
+    def exchange_attach(self, peer_rank: int, ipc_handle: bytes | None = None, ptr: int | None = None):
+        buf = (C.c_ubyte * 64).from_buffer_copy(ipc_handle) if ipc_handle is not None else None
+        self._chk(self._L.ng_exchange_attach(self._h, peer_rank, buf, C.c_void_p(ptr) if ptr is not None else None))
+
+    def shard_phase(self, phase: int):
+        self._chk(self._L.ng_shard_phase(self._h, phase))
 
     def set_state(self, field: int, data, first: int = 0):
         """data: numpy array or torch tensor (host or device) of the field's element type."""
@@ -350,12 +380,12 @@ class Sim:
 
     # ---- connection structure read-back (parity checks) --------------------------------------------------------
     def row_offsets(self) -> np.ndarray:
-        out = np.empty(self.n_neurons + 1, np.int64)
+        out = np.empty(self.n_sources + 1, np.int64)
         self._chk(self._L.ng_copy_row_offsets(self._h, out.ctypes.data))
         return out
 
     def group_offsets(self) -> np.ndarray:
-        out = np.empty((self.n_neurons, self.D + 1), np.uint32)
+        out = np.empty((self.n_sources, self.D + 1), np.uint32)
         self._chk(self._L.ng_copy_group_offsets(self._h, out.ctypes.data))
         return out
 
@@ -375,3 +405,136 @@ class Sim:
             self._chk(self._L.ng_get_connections(self._h, src_id, tgt.ctypes.data, w.ctypes.data, d.ctypes.data, n,
                                                  C.byref(cnt)))
         return tgt, w, d
+
+
+def shard_range(n_neurons: int, rank: int, world: int):
+    """ng_shard_range: (first id, count) of the neurons rank `rank` of `world` owns.  Pure host arithmetic."""
+    first, n = C.c_int32(), C.c_int32()
+    rc = load_library().ng_shard_range(n_neurons, rank, world, C.byref(first), C.byref(n))
+    if rc != NG_OK:
+        raise NgError(rc, "ng_shard_range: bad arguments")
+    return first.value, n.value
+
+
+def connect_peers(sim: "Sim", dist=None, group=None):
+    """Multi-process plumbing of the spike exchange: all-gather the ranks' 64-byte IPC handles with torch.distributed
+    (any backend) and map every peer's receive buffer.  Marshalling only — the exchange itself runs in the kernels."""
+    import torch.distributed as td
+    dist = dist or td
+    mine, _ = sim.exchange_handle()
+    handles = [None] * sim.world
+    dist.all_gather_object(handles, mine, group=group)
+    for q, h in enumerate(handles):
+        if q != sim.rank:
+            sim.exchange_attach(q, ipc_handle=h)
+
+
+class ShardGroup:
+    """All `world` shards of one network as handles of ONE process on ONE device and ONE stream (tests; a box with fewer
+    GPUs than ranks).  Steps are issued half by half over all shards (ng_shard_phase), so no kernel ever waits for another.
+    Exposes the calls of `Sim` the parity helpers use, with global ids and whole-network arrays."""
+
+    def __init__(self, world: int, dt_ms: float = 0.1, ring_slots: int = 64, seed: int = 1, device: int = 0, **kw):
+        import torch
+        self.stream = torch.cuda.Stream(device=device)
+        self.world, self.D = world, ring_slots
+        self.shards = [Sim(dt_ms, ring_slots, seed, device=device, rank=r, world=world, stream=self.stream, **kw) for r in range(world)]
+
+    # network description: the same calls on every shard
+    def create_population(self, n, params):
+        return [g.create_population(n, params) for g in self.shards][0]
+
+    def connect_fixed_indegree(self, *a, **k):
+        for g in self.shards:
+            g.connect_fixed_indegree(*a, **k)
+
+    def connect_fixed_outdegree(self, *a, **k):
+        for g in self.shards:
+            g.connect_fixed_outdegree(*a, **k)
+
+    def set_bypass(self, *a):
+        for g in self.shards:
+            g.set_bypass(*a)
+
+    def set_option(self, option, value):
+        for g in self.shards:
+            g.set_option(option, value)
+
+    def prepare(self):
+        for g in self.shards:
+            g.prepare()
+        ptrs = [g.exchange_handle()[1] for g in self.shards]
+        for g in self.shards:
+            for q, p in enumerate(ptrs):
+                if q != g.rank:
+                    g.exchange_attach(q, ptr=p)
+        self.ranges = [(int(g.stats().id_first), int(g.stats().n_neurons)) for g in self.shards]
+        self.n_ports = self.shards[0].n_ports
+
+    @property
+    def n_neurons(self):
+        return sum(n for _, n in self.ranges)
+
+    def stats(self):
+        return [g.stats() for g in self.shards]
+
+    def simulate(self, n_steps: int):
+        for _ in range(n_steps):
+            for g in self.shards:
+                g.shard_phase(0)
+            for g in self.shards:
+                g.shard_phase(1)
+        self._torch_sync()
+
+    def _torch_sync(self):
+        self.stream.synchronize()
+
+    def set_state(self, field, data, first: int = 0):
+        if field == FIELD_STEP:
+            for g in self.shards:
+                g.set_state(field, data)
+            return
+        a = np.ascontiguousarray(data)
+        assert first == 0 and field != FIELD_RING
+        for g, (f0, n) in zip(self.shards, self.ranges):
+            g.set_state(field, a[f0:f0 + n])
+
+    def get_state(self, field, n=None, first: int = 0):
+        if field == FIELD_STEP:
+            vals = {g.get_state(field) for g in self.shards}
+            assert len(vals) == 1
+            return vals.pop()
+        parts = [g.get_state(field) for g in self.shards]
+        if field in (FIELD_RING, FIELD_LAST_INPUT):          # [slots][ports][local N] per shard -> [slots][ports][N]
+            rows = [p.reshape(-1, nloc) for p, (_, nloc) in zip(parts, self.ranges)]
+            return np.concatenate(rows, axis=1).reshape(-1)
+        return np.concatenate(parts)
+
+    def last_spikes(self):
+        ids = [np.sort(g.last_spikes()) for g in self.shards]
+        for other in ids[1:]:
+            assert np.array_equal(ids[0], other), "shards disagree on the spike array"
+        return ids[0]
+
+    def get_spikes(self):
+        rec = [g.get_spikes() for g in self.shards]
+        key0 = np.lexsort((rec[0][1], rec[0][0]))
+        for s_, i_ in rec[1:]:
+            k = np.lexsort((i_, s_))
+            assert np.array_equal(rec[0][0][key0], s_[k]) and np.array_equal(rec[0][1][key0], i_[k]), "shards disagree on the spike record"
+        return rec[0][0][key0], rec[0][1][key0]
+
+    def connections(self):
+        """(src, tgt, weight, delay) of the whole network with GLOBAL target ids, concatenated over the shards (padding removed)."""
+        out = []
+        for g, (f0, nloc) in zip(self.shards, self.ranges):
+            ro = g.row_offsets(); tgt, w, d = g.records()
+            src = np.repeat(np.arange(ro.size - 1, dtype=np.int32), np.diff(ro))
+            keep = tgt >= 0
+            port = tgt[keep] // nloc
+            out.append((src[keep], (tgt[keep] % nloc) + f0, w[keep], d[keep], port))
+        return tuple(np.concatenate([o[k] for o in out]) for k in range(5))
+
+    def close(self):
+        for g in self.shards:
+            g.close()

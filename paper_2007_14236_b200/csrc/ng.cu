@@ -18,6 +18,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -62,6 +63,9 @@ struct ng_sim {
     bool has_adex = false;                 // any AdEx population: two receptor ports, AdEx state arrays, <true> kernels
     int64_t NR = 0;                        // ring row length = N * ports
     bool window_backend = false;           // delivery kernel 4 chosen before ng_prepare: spike window instead of a D-plane ring
+    // target-sharded multi-GPU (ng_set_shard): this handle owns the neurons [id_first, id_first + NL)
+    int shard_rank = 0, shard_world = 1; int32_t id_first = 0; int32_t NL = 0;
+    unsigned char* xchg_own = nullptr; size_t xchg_bytes = 0; bool xchg_ipc_open[16] = {};
     bool queue_backend = false;            // delivery kernel 5 chosen before / by ng_prepare: per-delay event queues, two planes
     int64_t queue_cap_opt = 0;             // NG_OPT_QUEUE_CAPACITY: events per queue (0 = auto)
     int queue_blocks = 0;
@@ -194,21 +198,25 @@ void launch_pipe_flush(ng_sim* s) {
     if (s->has_adex) pipe_step_kernel<false, true><<<s->pipe_blocks, kPipeThreads, 0, s->stream>>>(s->a);
     else pipe_step_kernel<false, false><<<s->pipe_blocks, kPipeThreads, 0, s->stream>>>(s->a);
 }
+void launch_exchange_publish(ng_sim* s) { xchg_publish_kernel<<<s->shard_world, 256, 0, s->stream>>>(s->a); }
+void launch_exchange_gather(ng_sim* s) { xchg_gather_kernel<<<s->shard_world, 256, 0, s->stream>>>(s->a); }
 void launch_step(ng_sim* s) {
     if (s->delivery_kernel == 3) launch_pipe(s);
+    else if (s->shard_world > 1) { launch_update(s); launch_exchange_publish(s); launch_exchange_gather(s); launch_deliver(s); }
     else { launch_update(s); launch_deliver(s); }
 }
 // choose launch shapes from the built network (static per simulation; no per-step host decisions)
 void configure_launch(ng_sim* s) {
     const int sm = s->sm_count;
-    s->update_blocks = grid_for(s->N, kUpdateThreads, sm * 32);
+    s->update_blocks = grid_for(s->NL, kUpdateThreads, sm * 32);
     // delivery kernel: delay-major segment walk pays off when the ring is too big to stay in L2 next to the
     // streamed records and groups are long enough to fill a warp's 128-bit loads; otherwise walk whole rows.
     const double ring_bytes = (double)s->N * s->cfg.ring_slots * 4.0;
     const double mean_group = s->N > 0 ? (double)s->S / ((double)s->N * s->cfg.ring_slots) : 0.0;
     int k = s->delivery_kernel_opt;
     // otherwise the step is latency-bound: rows are walked whole (kernel 1) or by the pipelined step kernel (3).
-    if (k == 0) k = 3;                                              // a ring beyond L2 was given the window backend in ng_prepare
+    if (k == 0) k = s->shard_world > 1 ? 1 : 3;                     // a ring beyond L2 was given a two-plane backend in ng_prepare
+    if (k == 3 && s->shard_world > 1) k = 1;                        // the pipelined kernel delivers a CTA's own spikes: one GPU only
     (void)mean_group; (void)ring_bytes;
     if (s->window_backend) k = 4;                                   // fixed at ng_prepare: there is no D-plane ring
     if (s->queue_backend) k = 5;
@@ -218,6 +226,7 @@ void configure_launch(ng_sim* s) {
     s->step_mode = s->step_mode_opt != 3 ? s->step_mode_opt : (k == 2 || k == 4 || k == 5 || !s->coop_ok) ? 0 : 2;
     if (s->has_adex && s->step_mode == 2 && k != 3) s->step_mode = 0;   // the two-phase persistent kernels are LIF only
     if (k == 5 && s->step_mode == 2) s->step_mode = 0;                  // the event-queue backend runs as update + delivery launches
+    if (s->shard_world > 1 && s->step_mode == 2) s->step_mode = 0;      // sharded: update, exchange and delivery are separate launches
     s->a.prefetch = (k != 2 && k != 4 && k != 5 && s->prefetch_opt) ? 1 : 0;
     {
         int occq = 0;
@@ -234,6 +243,10 @@ void configure_launch(ng_sim* s) {
         s->persistent_pipe_blocks = sm * std::min(occp, kPersistentThreads / pt);
         // updater threads per CTA of the AdEx kernels: all but four warps (pipe_updater_threads in ng_device.cuh)
         s->one_round_persistent = (long long)s->persistent_pipe_blocks * (pt - (s->has_adex ? 128 : (pt >= 512 ? kEntryTile : 64))) >= s->N;
+        // AdEx: the two-pass update (one integration attempt per lane, the unfinished neurons — on the exponential
+        // upswing, up to thirty sub-steps — finished by dense warps from a CTA list) pays for any number of rounds:
+        // 10^6 neurons 116 -> 105 us per step (profiles/r02_adex1m.md)
+        if (s->has_adex) s->one_round_persistent = true;
         s->one_round_step = (long long)s->pipe_blocks * (kPipeThreads - (s->has_adex ? 128 : kEntryTile)) >= s->N;
         // several rounds per step (config 4): keep V, I_syn, refr and the population byte (13 B per neuron) of the CTA's
         // neurons in dynamic shared memory for the whole launch if that fits beside the static 45 KB
@@ -295,9 +308,9 @@ int32_t read_ctl(ng_sim* s, Ctl* out) {
 
 int32_t field_info(ng_sim* s, int32_t field, void** base, size_t* elem, int64_t* len) {
     switch (field) {
-        case NG_FIELD_V: *base = s->a.V; *elem = 4; *len = s->N; return NG_OK;
-        case NG_FIELD_I_SYN: *base = s->a.I; *elem = 4; *len = s->N; return NG_OK;
-        case NG_FIELD_REFR: *base = s->a.refr; *elem = 4; *len = s->N; return NG_OK;
+        case NG_FIELD_V: *base = s->a.V; *elem = 4; *len = s->NL; return NG_OK;
+        case NG_FIELD_I_SYN: *base = s->a.I; *elem = 4; *len = s->NL; return NG_OK;
+        case NG_FIELD_REFR: *base = s->a.refr; *elem = 4; *len = s->NL; return NG_OK;
         case NG_FIELD_RING: *base = s->a.ring; *elem = 4; *len = s->NR * s->cfg.ring_slots; return NG_OK;   // see ring_copy
         case NG_FIELD_LAST_INPUT:
             if (!s->a.last_input) return fail(s, NG_ERR_STATE, "NG_FIELD_LAST_INPUT needs NG_DEBUG_INPUT");
@@ -306,7 +319,7 @@ int32_t field_info(ng_sim* s, int32_t field, void** base, size_t* elem, int64_t*
         case NG_FIELD_ADEX_H: {
             if (!s->has_adex) return fail(s, NG_ERR_STATE, "no AdEx population");
             float* arr[] = {s->a.ax_w, s->a.ax_gx, s->a.ax_yx, s->a.ax_gi, s->a.ax_yi, s->a.ax_h};
-            *base = arr[field - NG_FIELD_ADEX_W]; *elem = 4; *len = s->N; return NG_OK;
+            *base = arr[field - NG_FIELD_ADEX_W]; *elem = 4; *len = s->NL; return NG_OK;
         }
         default: return fail(s, NG_ERR_INVALID_ARG, "unknown field");
     }
@@ -384,6 +397,8 @@ int32_t ng_destroy(ng_sim* s) {
     destroy_graph(s);
     std::vector<void*> all = s->allocs;
     for (void* p : all) dev_free(s, p);
+    for (int q = 0; q < 16; ++q) if (s->xchg_ipc_open[q] && s->a.xchg[q]) cudaIpcCloseMemHandle(s->a.xchg[q]);
+    if (s->xchg_own) cudaFree(s->xchg_own);
     if (s->own_stream) cudaStreamDestroy(s->stream);
     delete s;
     return NG_OK;
@@ -459,6 +474,78 @@ int32_t ng_create_population_adex(ng_sim* s, int32_t n, const ng_adex_params* p,
     return NG_OK;
 }
 
+int32_t ng_shard_range(int32_t n_neurons, int32_t rank, int32_t world, int32_t* first_out, int32_t* n_out) {
+    if (n_neurons < 0 || world < 1 || world > kMaxShards || rank < 0 || rank >= world || !first_out || !n_out) return NG_ERR_INVALID_ARG;
+    const int32_t first = (int32_t)((int64_t)n_neurons * rank / world);
+    *first_out = first;
+    *n_out = (int32_t)((int64_t)n_neurons * (rank + 1) / world) - first;
+    return NG_OK;
+}
+
+int32_t ng_set_shard(ng_sim* s, int32_t rank, int32_t world) {
+    if (!s) return NG_ERR_INVALID_ARG;
+    if (s->prepared) return fail(s, NG_ERR_STATE, "ng_set_shard after ng_prepare");
+    if (world < 1 || world > kMaxShards || rank < 0 || rank >= world) return fail(s, NG_ERR_INVALID_ARG, "shard rank / world (1..16)");
+    s->shard_rank = rank; s->shard_world = world;
+    return NG_OK;
+}
+
+int32_t ng_exchange_handle(ng_sim* s, void* handle_out_64, void** local_ptr_out) {
+    if (!s) return NG_ERR_INVALID_ARG;
+    if (!s->prepared || s->shard_world < 2) return fail(s, NG_ERR_STATE, "no exchange buffer: ng_set_shard with world > 1, then ng_prepare");
+    NG_CUDA(s, cudaSetDevice(s->cfg.device));
+    if (local_ptr_out) *local_ptr_out = s->xchg_own;
+    if (handle_out_64) {
+        static_assert(sizeof(cudaIpcMemHandle_t) == 64, "CUDA IPC handle size");
+        cudaIpcMemHandle_t h;
+        NG_CUDA(s, cudaIpcGetMemHandle(&h, s->xchg_own));
+        std::memcpy(handle_out_64, &h, 64);
+    }
+    return NG_OK;
+}
+
+int32_t ng_exchange_attach(ng_sim* s, int32_t peer_rank, const void* ipc_handle_64, void* same_process_ptr) {
+    if (!s) return NG_ERR_INVALID_ARG;
+    if (!s->prepared || s->shard_world < 2) return fail(s, NG_ERR_STATE, "no exchange buffer: ng_set_shard with world > 1, then ng_prepare");
+    if (peer_rank < 0 || peer_rank >= s->shard_world || peer_rank == s->shard_rank) return fail(s, NG_ERR_INVALID_ARG, "peer rank");
+    if ((ipc_handle_64 == nullptr) == (same_process_ptr == nullptr)) return fail(s, NG_ERR_INVALID_ARG, "give the IPC handle or the pointer, not both");
+    NG_CUDA(s, cudaSetDevice(s->cfg.device));
+    if (s->a.xchg[peer_rank]) return fail(s, NG_ERR_STATE, "peer already attached");
+    if (ipc_handle_64) {
+        cudaIpcMemHandle_t h;
+        std::memcpy(&h, ipc_handle_64, 64);
+        void* p = nullptr;
+        NG_CUDA(s, cudaIpcOpenMemHandle(&p, h, cudaIpcMemLazyEnablePeerAccess));
+        s->a.xchg[peer_rank] = (unsigned char*)p; s->xchg_ipc_open[peer_rank] = true;
+    } else {
+        // a buffer of another handle in this process: on another device it needs peer access (NVLink / NVSwitch)
+        cudaPointerAttributes at{};
+        NG_CUDA(s, cudaPointerGetAttributes(&at, same_process_ptr));
+        if (at.type != cudaMemoryTypeDevice) return fail(s, NG_ERR_INVALID_ARG, "not a device pointer");
+        if (at.device != s->cfg.device) {
+            cudaError_t e = cudaDeviceEnablePeerAccess(at.device, 0);
+            if (e != cudaSuccess && e != cudaErrorPeerAccessAlreadyEnabled) return fail(s, NG_ERR_CUDA, std::string("cudaDeviceEnablePeerAccess: ") + cudaGetErrorString(e));
+            cudaGetLastError();
+        }
+        s->a.xchg[peer_rank] = (unsigned char*)same_process_ptr;
+    }
+    destroy_graph(s);                                              // the kernels' argument block changed
+    return NG_OK;
+}
+
+int32_t ng_shard_phase(ng_sim* s, int32_t phase) {
+    if (!s) return NG_ERR_INVALID_ARG;
+    if (!s->prepared || s->shard_world < 2) return fail(s, NG_ERR_STATE, "ng_shard_phase needs a prepared target-sharded handle");
+    if (phase != 0 && phase != 1) return fail(s, NG_ERR_INVALID_ARG, "phase is 0 (update + publish) or 1 (gather + deliver)");
+    for (int q = 0; q < s->shard_world; ++q)
+        if (!s->a.xchg[q]) return fail(s, NG_ERR_STATE, "target-sharded mode: ng_exchange_attach every peer first");
+    NG_CUDA(s, cudaSetDevice(s->cfg.device));
+    if (phase == 0) { launch_update(s); launch_exchange_publish(s); s->launches_update += 1; }
+    else { launch_exchange_gather(s); launch_deliver(s); s->launches_deliver += 1; s->steps_done += 1; }
+    NG_CUDA(s, cudaGetLastError());
+    return NG_OK;
+}
+
 int32_t ng_set_bypass(ng_sim* s, int32_t bypass, double fraction) {
     if (!s) return NG_ERR_INVALID_ARG;
     if (s->prepared) return fail(s, NG_ERR_STATE, "ng_set_bypass after ng_prepare");
@@ -483,6 +570,7 @@ int32_t ng_set_option(ng_sim* s, int32_t option, int64_t value) {
             s->steps_per_graph = (int)value; destroy_graph(s); break;
         case NG_OPT_DELIVERY_KERNEL:
             if (value < 0 || value > 5) return fail(s, NG_ERR_INVALID_ARG, "delivery kernel is 0 .. 5");
+            if (value == 3 && s->shard_world > 1) return fail(s, NG_ERR_INVALID_ARG, "delivery kernel 3 (pipelined) runs on one GPU only");
             if (s->prepared && value != 0 && ((value == 4) != s->window_backend || (value == 5) != s->queue_backend))
                 return fail(s, NG_ERR_STATE, "delivery kernels 4 (spike-buffer backend) and 5 (event queues) must be chosen before ng_prepare and cannot be left after it");
             s->delivery_kernel_opt = (int)value; if (s->prepared) configure_launch(s); break;
@@ -523,14 +611,21 @@ int32_t ng_prepare(ng_sim* s) {
     if (s->prepared) return NG_OK;
     if (s->N <= 0) return fail(s, NG_ERR_STATE, "no population");
     NG_CUDA(s, cudaSetDevice(s->cfg.device));
-    const int N = s->N, D = s->cfg.ring_slots;
+    const int N = s->N, D = s->cfg.ring_slots;               // N: neurons of the whole network = sources = rows
+    // target-sharded mode: this handle owns the contiguous id range [id_first, id_first + NL) (ng_shard_range)
+    s->id_first = (int32_t)((int64_t)N * s->shard_rank / s->shard_world);
+    s->NL = (int32_t)((int64_t)N * (s->shard_rank + 1) / s->shard_world) - s->id_first;
+    const int NL = s->NL;
+    if (NL <= 0) return fail(s, NG_ERR_INVALID_ARG, "more shards than neurons");
     cudaStream_t st = s->stream;
     // Ring or spike window?  A ring that cannot stay in L2 (config 3: 65 planes x 4 MB) costs a DRAM round trip per plane
     // and step; the spike-buffer backend keeps two planes whatever D is and measured faster on every point of the
     // config 3 sweep, so it is the automatic choice there.
     s->S = 0;
     for (const CallDev& c : s->calls) s->S += (int64_t)(c.rule == kRuleIndegree ? c.tgt_n : c.src_n) * c.K;
-    const bool beyond_l2 = (double)N * (D + 1) * 4.0 > 0.8 * (double)s->l2_bytes;
+    const int64_t S_all = s->S;
+    s->S = S_all / s->shard_world;                              // estimate until the build has counted this shard's records
+    const bool beyond_l2 = (double)NL * (D + 1) * 4.0 > 0.8 * (double)s->l2_bytes;
     // Beyond L2, short delay groups (a few records per (source, delay): config 3 at out-degree 100 and 1000) make the
     // spike-buffer walk read at random 12-125-byte granularity; the event queues read a spiking row once, whole
     // (DESIGN.md section 7).  Expected events per step: the injected fraction in delivery-only mode, else 2 % of S.
@@ -546,7 +641,7 @@ int32_t ng_prepare(ng_sim* s) {
     const int planes = (s->window_backend || s->queue_backend) ? 2 : D + 1;               // ring planes actually stored
     s->has_adex = false;
     for (const HostPop& hp : s->pops) s->has_adex = s->has_adex || hp.dev.model == 1;
-    s->NR = (int64_t)N * (s->has_adex ? 2 : 1);
+    s->NR = (int64_t)NL * (s->has_adex ? 2 : 1);
     // Receptor port 1 is the inhibitory conductance of AdEx neurons: it exists only in networks with an AdEx population
     // (two-port ring planes), and only AdEx targets read it — a LIF target would silently drop such input.
     for (const CallDev& c : s->calls) {
@@ -565,17 +660,17 @@ int32_t ng_prepare(ng_sim* s) {
 
     // ---- control block, populations, state ----
     bool ok = dev_alloc_t(s, &s->d_ctl, 1) && dev_alloc_t(s, &s->d_pops, s->pops.size()) &&
-              dev_alloc_t(s, &s->d_pop_of, (size_t)N) && dev_alloc_t(s, &s->a.V, (size_t)N) &&
-              dev_alloc_t(s, &s->a.I, (size_t)N) && dev_alloc_t(s, &s->a.refr, (size_t)N) &&
+              dev_alloc_t(s, &s->d_pop_of, (size_t)NL) && dev_alloc_t(s, &s->a.V, (size_t)NL) &&
+              dev_alloc_t(s, &s->a.I, (size_t)NL) && dev_alloc_t(s, &s->a.refr, (size_t)NL) &&
               dev_alloc_t(s, &s->a.ring, NRs * planes) && dev_alloc_t(s, &s->a.spike_list, (size_t)2 * N) &&
-              dev_alloc_t(s, &s->a.spike_row, (size_t)2 * N) && dev_alloc_t(s, &s->a.pois_k, (size_t)N) && dev_alloc_t(s, &s->d_row_info, (size_t)N) &&
+              dev_alloc_t(s, &s->a.spike_row, (size_t)2 * N) && dev_alloc_t(s, &s->a.pois_k, (size_t)NL) && dev_alloc_t(s, &s->d_row_info, (size_t)N) &&
               dev_alloc_t(s, &s->d_calls, std::max<size_t>(1, s->calls.size())) &&
               dev_alloc_t(s, &s->d_cnt, (size_t)N * D) && dev_alloc_t(s, &s->d_row_len, (size_t)N) &&
               dev_alloc_t(s, &s->d_row_off, (size_t)N + 1) && dev_alloc_t(s, &s->d_grp_rel, (size_t)N * (D + 1));
     if (ok && (s->cfg.flags & NG_DEBUG_INPUT)) ok = dev_alloc_t(s, &s->a.last_input, NRs);
     if (ok && s->has_adex)
-        ok = dev_alloc_t(s, &s->a.ax_w, (size_t)N) && dev_alloc_t(s, &s->a.ax_gx, (size_t)N) && dev_alloc_t(s, &s->a.ax_yx, (size_t)N) &&
-             dev_alloc_t(s, &s->a.ax_gi, (size_t)N) && dev_alloc_t(s, &s->a.ax_yi, (size_t)N) && dev_alloc_t(s, &s->a.ax_h, (size_t)N);
+        ok = dev_alloc_t(s, &s->a.ax_w, (size_t)NL) && dev_alloc_t(s, &s->a.ax_gx, (size_t)NL) && dev_alloc_t(s, &s->a.ax_yx, (size_t)NL) &&
+             dev_alloc_t(s, &s->a.ax_gi, (size_t)NL) && dev_alloc_t(s, &s->a.ax_yi, (size_t)NL) && dev_alloc_t(s, &s->a.ax_h, (size_t)NL);
     if (ok && (s->cfg.flags & NG_RECORD_SPIKES) && s->cfg.max_recorded_spikes > 0) {
         ok = dev_alloc_t(s, &s->a.rec_step, (size_t)s->cfg.max_recorded_spikes) &&
              dev_alloc_t(s, &s->a.rec_id, (size_t)s->cfg.max_recorded_spikes);
@@ -583,13 +678,13 @@ int32_t ng_prepare(ng_sim* s) {
     }
     if (!ok) return fail(s, NG_ERR_OOM, "device allocation failed (state)");
     NG_CUDA(s, cudaMemsetAsync(s->d_ctl, 0, sizeof(Ctl), st));
-    NG_CUDA(s, cudaMemsetAsync(s->a.I, 0, (size_t)N * 4, st));
-    NG_CUDA(s, cudaMemsetAsync(s->a.refr, 0, (size_t)N * 4, st));
+    NG_CUDA(s, cudaMemsetAsync(s->a.I, 0, (size_t)NL * 4, st));
+    NG_CUDA(s, cudaMemsetAsync(s->a.refr, 0, (size_t)NL * 4, st));
     NG_CUDA(s, cudaMemsetAsync(s->a.ring, 0, NRs * planes * 4, st));
     if (s->has_adex) {
-        for (float* p : {s->a.ax_w, s->a.ax_gx, s->a.ax_yx, s->a.ax_gi, s->a.ax_yi}) NG_CUDA(s, cudaMemsetAsync(p, 0, (size_t)N * 4, st));
-        std::vector<float> h0((size_t)N, (float)s->cfg.dt_ms);     // sub-step size starts at the whole time step
-        NG_CUDA(s, cudaMemcpyAsync(s->a.ax_h, h0.data(), (size_t)N * 4, cudaMemcpyHostToDevice, st));
+        for (float* p : {s->a.ax_w, s->a.ax_gx, s->a.ax_yx, s->a.ax_gi, s->a.ax_yi}) NG_CUDA(s, cudaMemsetAsync(p, 0, (size_t)NL * 4, st));
+        std::vector<float> h0((size_t)NL, (float)s->cfg.dt_ms);    // sub-step size starts at the whole time step
+        NG_CUDA(s, cudaMemcpyAsync(s->a.ax_h, h0.data(), (size_t)NL * 4, cudaMemcpyHostToDevice, st));
         NG_CUDA(s, cudaStreamSynchronize(st));
     }
     if (s->window_backend) {
@@ -611,20 +706,38 @@ int32_t ng_prepare(ng_sim* s) {
     NG_CUDA(s, cudaMemcpyAsync(s->d_pops, pd.data(), pd.size() * sizeof(PopDev), cudaMemcpyHostToDevice, st));
     if (!s->calls.empty())
         NG_CUDA(s, cudaMemcpyAsync(s->d_calls, s->calls.data(), s->calls.size() * sizeof(CallDev), cudaMemcpyHostToDevice, st));
-    for (size_t i = 0; i < s->pops.size(); ++i) {
+    for (size_t i = 0; i < s->pops.size(); ++i) {                  // the part of each population this shard owns
         const HostPop& hp = s->pops[i];
-        fill_pop_of_kernel<<<(hp.n + 255) / 256, 256, 0, st>>>(s->d_pop_of, s->a.V, hp.first, hp.n, (uint8_t)i, hp.dev.E_L);
+        const int lo = std::max(hp.first, s->id_first), hi = std::min(hp.first + hp.n, s->id_first + NL);
+        if (hi <= lo) continue;
+        fill_pop_of_kernel<<<(hi - lo + 255) / 256, 256, 0, st>>>(s->d_pop_of, s->a.V, lo - s->id_first, hi - lo, (uint8_t)i, hp.dev.E_L);
         s->launches_other++;
+    }
+    if (s->shard_world > 1) {
+        // receive buffer of the per-step spike exchange: plain cudaMalloc (it is exported to the peers as a CUDA IPC
+        // handle, which the pooled allocations of the caller's allocator cannot be)
+        s->a.xchg_cap = (int32_t)(((int64_t)N + s->shard_world - 1) / s->shard_world + 1);
+        s->xchg_bytes = (size_t)kXchgHeaderBytes + (size_t)2 * s->shard_world * (size_t)s->a.xchg_cap * 4;
+        if (cudaMalloc((void**)&s->xchg_own, s->xchg_bytes) != cudaSuccess) { cudaGetLastError(); return fail(s, NG_ERR_OOM, "device allocation failed (exchange buffer)"); }
+        NG_CUDA(s, cudaMemsetAsync(s->xchg_own, 0, s->xchg_bytes, st));
+        s->a.xchg[s->shard_rank] = s->xchg_own;
+        s->a.xchg_rank = s->shard_rank; s->a.xchg_world = s->shard_world;
     }
 
     // ---- connection build (a0) ----
     const uint32_t seed_lo = (uint32_t)s->cfg.seed, seed_hi = (uint32_t)(s->cfg.seed >> 32);
     const int cap = s->sm_count * 16;
+    // draws the build kernels of this shard regenerate for one call: fixed in-degree -> the local targets only
+    auto call_draws = [&](const CallDev& c) -> long long {
+        if (c.rule != kRuleIndegree) return (long long)c.src_n * c.K;
+        const int lo = std::max(c.tgt_first, s->id_first), hi = std::min(c.tgt_first + c.tgt_n, s->id_first + NL);
+        return (long long)std::max(0, hi - lo) * c.K;
+    };
     for (size_t ci = 0; ci < s->calls.size(); ++ci) {
         const CallDev& c = s->calls[ci];
-        const long long total = (long long)(c.rule == kRuleIndegree ? c.tgt_n : c.src_n) * c.K;
+        const long long total = call_draws(c);
         if (total == 0) continue;
-        build_count_kernel<<<grid_for(total, 256, cap), 256, 0, st>>>(s->d_calls, (int)ci, seed_lo, seed_hi, D, s->d_cnt, s->d_ctl);
+        build_count_kernel<<<grid_for(total, 256, cap), 256, 0, st>>>(s->d_calls, (int)ci, seed_lo, seed_hi, D, s->d_cnt, s->d_ctl, s->id_first, NL);
         s->launches_other++;
     }
     build_rowlen_kernel<<<(N + 255) / 256, 256, 0, st>>>(s->d_cnt, N, D, s->d_row_len, s->d_ctl);
@@ -639,6 +752,8 @@ int32_t ng_prepare(ng_sim* s) {
     if (h.err_delay) return fail(s, NG_ERR_OVERFLOW, "a drawn delay fell outside [1, ring_slots]");
     s->n_padded = (int64_t)h.n_padded;
     s->max_row_records = h.max_row_records;
+    s->S = (int64_t)h.n_records;                                    // connections stored on this shard (= all of them on one GPU)
+    if (s->shard_world == 1 && s->S != S_all) return fail(s, NG_ERR_CUDA, "builder lost records");
     const size_t np = (size_t)std::max<int64_t>(s->n_padded, 4);
     if (!(dev_alloc_t(s, &s->d_tgt, np) && dev_alloc_t(s, &s->d_w, np) && dev_alloc_t(s, &s->d_dly, np + 16)))
         return fail(s, NG_ERR_OOM, "device allocation failed (connection records)");
@@ -647,10 +762,10 @@ int32_t ng_prepare(ng_sim* s) {
     NG_CUDA(s, cudaMemsetAsync(s->d_dly, 0, np, st));
     for (size_t ci = 0; ci < s->calls.size(); ++ci) {
         const CallDev& c = s->calls[ci];
-        const long long total = (long long)(c.rule == kRuleIndegree ? c.tgt_n : c.src_n) * c.K;
+        const long long total = call_draws(c);
         if (total == 0) continue;
         build_fill_kernel<<<grid_for(total, 256, cap), 256, 0, st>>>(s->d_calls, (int)ci, seed_lo, seed_hi, D, s->d_cnt,
-                                                                   s->d_row_off, s->d_grp_rel, s->d_tgt, s->d_w, s->d_dly, N);
+                                                                   s->d_row_off, s->d_grp_rel, s->d_tgt, s->d_w, s->d_dly, NL, s->id_first);
         s->launches_other++;
     }
     long long* d_long = nullptr;
@@ -676,7 +791,7 @@ int32_t ng_prepare(ng_sim* s) {
 
     // ---- step arguments ----
     s->a.NR = (int32_t)s->NR; s->a.dt_ms = (float)s->cfg.dt_ms; s->a.has_adex = s->has_adex ? 1 : 0;
-    s->a.N = N; s->a.D = D; s->a.Dr = planes; s->a.n_pops = (int32_t)s->pops.size(); s->a.seed_lo = seed_lo; s->a.seed_hi = seed_hi;
+    s->a.N = NL; s->a.NS = N; s->a.id_first = s->id_first; s->a.D = D; s->a.Dr = planes; s->a.n_pops = (int32_t)s->pops.size(); s->a.seed_lo = seed_lo; s->a.seed_hi = seed_hi;
     s->a.pop_of = s->d_pop_of; s->a.pops = s->d_pops;
     s->a.row_info = s->d_row_info;
     s->a.row_off = s->d_row_off; s->a.grp_rel = s->d_grp_rel; s->a.tgt = s->d_tgt; s->a.w = s->d_w; s->a.dly = s->d_dly;
@@ -750,6 +865,9 @@ int32_t ng_simulate(ng_sim* s, int64_t n_steps) {
     if (rc) return rc;
     NG_CUDA(s, cudaSetDevice(s->cfg.device));
     if (n_steps == 0) return NG_OK;
+    if (s->shard_world > 1)
+        for (int q = 0; q < s->shard_world; ++q)
+            if (!s->a.xchg[q]) return fail(s, NG_ERR_STATE, "target-sharded mode: ng_exchange_attach every peer before ng_simulate");
     cudaStream_t st = s->stream;
     if (s->profile) {
         // per-kernel device times: events around every launch, read back in batches
@@ -761,6 +879,7 @@ int32_t ng_simulate(ng_sim* s, int64_t n_steps) {
             for (int i = 0; i < b; ++i) {
                 cudaEventRecord(ev[3 * i], st);
                 if (s->delivery_kernel == 3) launch_pipe(s); else launch_update(s);
+                if (s->shard_world > 1) { launch_exchange_publish(s); launch_exchange_gather(s); }
                 cudaEventRecord(ev[3 * i + 1], st);
                 if (s->delivery_kernel != 3) launch_deliver(s);
                 cudaEventRecord(ev[3 * i + 2], st);
@@ -814,10 +933,11 @@ int32_t ng_simulate(ng_sim* s, int64_t n_steps) {
     s->steps_done += (uint64_t)n_steps;
     if (s->async) return NG_OK;
     NG_CUDA(s, cudaStreamSynchronize(st));
-    if (s->a.rec_cap > 0 || s->window_backend || s->queue_backend) {
+    if (s->a.rec_cap > 0 || s->window_backend || s->queue_backend || s->shard_world > 1) {
         Ctl h{};
         rc = read_ctl(s, &h);
         if (rc) return rc;
+        if (h.err_xchg) return fail(s, NG_ERR_CUDA, "spike exchange: a peer's spike list did not arrive within the bounded wait");
         if (h.err_window) return fail(s, NG_ERR_OVERFLOW, "spike window overflowed: more spikes within ring_slots steps than its capacity");
         if (h.err_queue) return fail(s, NG_ERR_OVERFLOW, "an event queue overflowed (events were dropped): raise NG_OPT_QUEUE_CAPACITY");
         const unsigned long long total = h.rec_total[h.step_u & 1];
@@ -927,7 +1047,8 @@ int32_t ng_get_connections(ng_sim* s, int32_t src_id, int32_t* tgt_host, float* 
 int32_t ng_get_stats(ng_sim* s, ng_stats* out) {
     if (!s || !out) return NG_ERR_INVALID_ARG;
     std::memset(out, 0, sizeof(*out));
-    out->n_neurons = s->N;
+    out->n_neurons = s->prepared ? s->NL : s->N;
+    out->n_sources = s->N; out->shard_rank = s->shard_rank; out->shard_world = s->shard_world; out->id_first = s->id_first;
     out->step_mode = s->step_mode;
     if (!s->prepared) return NG_OK;
     NG_CUDA(s, cudaSetDevice(s->cfg.device));
@@ -948,6 +1069,7 @@ int32_t ng_enable_statistics(ng_sim* s, int64_t start_step, int32_t bin_steps, i
     if (!s) return NG_ERR_INVALID_ARG;
     if (!s->prepared) return fail(s, NG_ERR_STATE, "ng_enable_statistics before ng_prepare");
     if (s->a.st_cnt) return fail(s, NG_ERR_STATE, "statistics are already enabled");
+    if (s->shard_world > 1) return fail(s, NG_ERR_STATE, "on-device statistics are not available in target-sharded mode");
     if (start_step < 0 || bin_steps < 1 || sample_per_pop < 0 || max_bins < 1 || max_bins > (1 << 24))
         return fail(s, NG_ERR_INVALID_ARG, "start_step < 0, bin_steps < 1, sample_per_pop < 0 or max_bins outside 1..2^24");
     NG_CUDA(s, cudaSetDevice(s->cfg.device));

@@ -67,6 +67,8 @@ struct Ctl {
     int32_t err_window;                    // spike-buffer backend: the spike window overflowed its capacity
     uint32_t n_long_groups;                // builder: (source, delay) groups longer than kSortMax, listed for the CTA-wide sort
     int32_t err_queue;                     // event-queue backend: a queue overflowed its capacity (events were dropped)
+    int32_t err_xchg;                      // target-sharded mode: a peer's spike list did not arrive (bounded wait expired)
+    unsigned long long n_records;          // builder: records stored on this shard (unpadded)
     // line 1: spike counters (atomics of the appending warps / CTAs)
     alignas(128) int32_t spike_cnt[4];     // length of the spike array of step n, indexed n & 3 (the list itself by n & 1)
     // line 2: event counter (one atomic per CTA and step)
@@ -169,16 +171,20 @@ __device__ __forceinline__ Draw draw_connection(const CallDev& c, uint32_t seed_
 // ---------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
 build_count_kernel(const CallDev* __restrict__ calls, int call_idx, uint32_t seed_lo, uint32_t seed_hi, int D,
-                   uint32_t* __restrict__ cnt, Ctl* __restrict__ ctl) {
+                   uint32_t* __restrict__ cnt, Ctl* __restrict__ ctl, int32_t id_first, int32_t id_n) {
     const CallDev c = calls[call_idx];
-    const int32_t e_first = c.rule == kRuleIndegree ? c.tgt_first : c.src_first;
-    const int32_t e_n = c.rule == kRuleIndegree ? c.tgt_n : c.src_n;
+    // target-sharded build: this GPU stores the connections whose TARGET is in [id_first, id_first + id_n).
+    // A draw is a pure function of (seed, call, endpoint, k), so the shard's structure is the one-GPU structure
+    // restricted to those targets.  Fixed in-degree: the endpoint is the target, so only local endpoints are drawn.
+    const int32_t e_first = c.rule == kRuleIndegree ? max(c.tgt_first, id_first) : c.src_first;
+    const int32_t e_n = c.rule == kRuleIndegree ? max(0, min(c.tgt_first + c.tgt_n, id_first + id_n) - e_first) : c.src_n;
     const long long total = (long long)e_n * c.K;
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += stride) {
         const int32_t e = e_first + (int32_t)(idx / c.K);
         const int32_t k = (int32_t)(idx % c.K);
         const Draw dr = draw_connection<false>(c, seed_lo, seed_hi, e, k);
+        if (dr.tgt < id_first || dr.tgt >= id_first + id_n) continue;
         if (dr.delay < 1 || dr.delay > D) { ctl->err_delay = 1; continue; }
         atomicAdd(&cnt[(size_t)dr.src * D + (dr.delay - 1)], 1u);
     }
@@ -190,18 +196,21 @@ __global__ void build_rowlen_kernel(const uint32_t* __restrict__ cnt, int N, int
                                     Ctl* __restrict__ ctl) {
     const int j = blockIdx.x * blockDim.x + threadIdx.x;
     int len = 0;
+    int deg = 0;
     if (j < N) {
-        for (int d = 0; d < D; ++d) len += (int)cnt[(size_t)j * D + d];
-        len = (len + 3) & ~3;
+        for (int d = 0; d < D; ++d) deg += (int)cnt[(size_t)j * D + d];
+        len = (deg + 3) & ~3;
         row_len[j] = len;
     }
-    // block max -> one atomic per block
+    // block max and block sum -> one atomic each per block
     __shared__ int smax;
-    if (threadIdx.x == 0) smax = 0;
+    __shared__ unsigned long long ssum;
+    if (threadIdx.x == 0) { smax = 0; ssum = 0; }
     __syncthreads();
     atomicMax(&smax, len);
+    if (deg) atomicAdd(&ssum, (unsigned long long)deg);
     __syncthreads();
-    if (threadIdx.x == 0) atomicMax(&ctl->max_row_records, smax);
+    if (threadIdx.x == 0) { atomicMax(&ctl->max_row_records, smax); if (ssum) atomicAdd(&ctl->n_records, ssum); }
 }
 
 // Exclusive scan of int64 values, one CTA of 1024 threads walking the array tile by tile.  N <= a few 1e6
@@ -276,20 +285,22 @@ __global__ void __launch_bounds__(256)
 build_fill_kernel(const CallDev* __restrict__ calls, int call_idx, uint32_t seed_lo, uint32_t seed_hi, int D,
                   uint32_t* __restrict__ cursor, const long long* __restrict__ row_off,
                   const uint32_t* __restrict__ grp_rel, int32_t* __restrict__ tgt, float* __restrict__ w,
-                  uint8_t* __restrict__ dly, int n_neurons) {
+                  uint8_t* __restrict__ dly, int n_neurons, int32_t id_first) {
     const CallDev c = calls[call_idx];
-    const int32_t e_first = c.rule == kRuleIndegree ? c.tgt_first : c.src_first;
-    const int32_t e_n = c.rule == kRuleIndegree ? c.tgt_n : c.src_n;
+    const int32_t id_n = n_neurons;                           // n_neurons = neurons of this shard
+    const int32_t e_first = c.rule == kRuleIndegree ? max(c.tgt_first, id_first) : c.src_first;
+    const int32_t e_n = c.rule == kRuleIndegree ? max(0, min(c.tgt_first + c.tgt_n, id_first + id_n) - e_first) : c.src_n;
     const long long total = (long long)e_n * c.K;
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += stride) {
         const int32_t e = e_first + (int32_t)(idx / c.K);
         const int32_t k = (int32_t)(idx % c.K);
         const Draw dr = draw_connection<true>(c, seed_lo, seed_hi, e, k);
+        if (dr.tgt < id_first || dr.tgt >= id_first + id_n) continue;
         if (dr.delay < 1 || dr.delay > D) continue;
         const uint32_t p = atomicAdd(&cursor[(size_t)dr.src * D + (dr.delay - 1)], 1u);
         const long long pos = row_off[dr.src] + grp_rel[(size_t)dr.src * (D + 1) + (dr.delay - 1)] + p;
-        tgt[pos] = dr.tgt + c.port * n_neurons;             // receptor port folded into the ring column
+        tgt[pos] = dr.tgt - id_first + c.port * n_neurons;  // local target index; receptor port folded into the ring column
         w[pos] = dr.w;
         dly[pos] = (uint8_t)dr.delay;
     }
@@ -393,15 +404,88 @@ __device__ __forceinline__ RowInfo ld_row_info(const RowInfo* p) {
 __device__ __forceinline__ void st_row_info(RowInfo* p, const RowInfo& r) {
     *reinterpret_cast<int4*>(p) = make_int4((int)(uint32_t)(unsigned long long)r.r0, (int)(uint32_t)((unsigned long long)r.r0 >> 32), r.deg, r.d1);
 }
+// L2 eviction priorities: connection records are read once per spike and never again soon (evict first), the input
+// ring is written by the reductions and read back by the update a few steps later (evict last), so that streaming
+// gigabytes of records does not push ring planes out of the 126 MB L2.
+#if defined(NG_EVICT_HINTS)
+__device__ __forceinline__ uint64_t l2_policy_stream() { uint64_t p; asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p)); return p; }
+__device__ __forceinline__ uint64_t l2_policy_keep() { uint64_t p; asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p)); return p; }
+#endif
+__device__ __forceinline__ void red_add_f32(float* addr, float v) {
+#if defined(NG_EVICT_HINTS) && NG_EVICT_HINTS >= 2
+    asm volatile("red.global.add.L2::cache_hint.f32 [%0], %1, %2;" ::"l"(addr), "f"(v), "l"(l2_policy_keep()) : "memory");
+#else
+    asm volatile("red.global.add.f32 [%0], %1;" ::"l"(addr), "f"(v) : "memory");
+#endif
+}
+// input cell of the ring: read at L2 (it is written by red.global from other SMs) and cleared
+__device__ __forceinline__ float ld_plane(const float* p) {
+    float v;
+#if defined(NG_EVICT_HINTS) && NG_EVICT_HINTS >= 3
+    asm volatile("ld.global.cg.L2::cache_hint.f32 %0, [%1], %2;" : "=f"(v) : "l"(p), "l"(l2_policy_keep()));
+#else
+    asm volatile("ld.global.cg.f32 %0, [%1];" : "=f"(v) : "l"(p));
+#endif
+    return v;
+}
+__device__ __forceinline__ void clear_plane(float* p) {
+#if defined(NG_EVICT_HINTS) && NG_EVICT_HINTS >= 3
+    asm volatile("st.global.L2::cache_hint.f32 [%0], %1, %2;" ::"l"(p), "f"(0.f), "l"(l2_policy_keep()) : "memory");
+#else
+    *p = 0.f;
+#endif
+}
+__device__ __forceinline__ int4 ld_stream_s32x4(const int32_t* p) {
+    int4 r;
+#if defined(NG_EVICT_HINTS)
+    asm("ld.global.nc.L1::no_allocate.L2::cache_hint.v4.s32 {%0,%1,%2,%3}, [%4], %5;"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p), "l"(l2_policy_stream()));
+#else
+    asm("ld.global.nc.L1::no_allocate.v4.s32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+#endif
+    return r;
+}
+__device__ __forceinline__ float4 ld_stream_f32x4(const float* p) {
+    float4 r;
+#if defined(NG_EVICT_HINTS)
+    asm("ld.global.nc.L1::no_allocate.L2::cache_hint.v4.f32 {%0,%1,%2,%3}, [%4], %5;"
+                 : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p), "l"(l2_policy_stream()));
+#else
+    asm("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];"
+                 : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p));
+#endif
+    return r;
+}
+__device__ __forceinline__ uint32_t ld_stream_u32(const void* p) {
+    uint32_t r;
+#if defined(NG_EVICT_HINTS)
+    asm("ld.global.nc.L1::no_allocate.L2::cache_hint.u32 %0, [%1], %2;" : "=r"(r) : "l"(p), "l"(l2_policy_stream()));
+#else
+    asm("ld.global.nc.L1::no_allocate.u32 %0, [%1];" : "=r"(r) : "l"(p));
+#endif
+    return r;
+}
+
 // TMA-unit bulk prefetch into L2 (no destination): p 16-byte aligned, bytes a multiple of 16
 __device__ __forceinline__ void prefetch_l2_bulk(const void* p, uint32_t bytes) {
+#if defined(NG_EVICT_HINTS)
+    uint64_t pol;
+    asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    asm volatile("cp.async.bulk.prefetch.L2.global.L2::cache_hint [%0], %1, %2;" ::"l"(p), "r"(bytes), "l"(pol) : "memory");
+#else
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+#endif
 }
 struct StepArgs;
 __device__ __forceinline__ void prefetch_row(const StepArgs& a, const RowInfo& r);
 
 struct StepArgs {
-    int32_t N, D;                // D = ring_slots of the C-ABI = largest legal delay
+    int32_t N, D;                // N = neurons of THIS shard (all neurons on one GPU); D = ring_slots = largest legal delay
+    int32_t NS, id_first;        // NS = sources = neurons of the whole network (rows, spike array); global id of local
+                                 // neuron i = id_first + i.  One GPU: NS = N, id_first = 0.
+    unsigned char* xchg[16];     // target-sharded mode: receive buffers of all ranks as seen from this device ([rank] = own)
+    int32_t xchg_rank, xchg_world, xchg_cap, xchg_pad;
     int32_t Dr, n_pops;          // Dr = D + 1 planes are stored (see update_phase); number of populations
     int32_t NR, pad_nr;          // ring row length = N * receptor ports (2 as soon as an AdEx population exists):
                                  // plane of (slot, port) = ring + (slot * NR + port * N); records store target + port * N
@@ -477,10 +561,11 @@ __device__ __forceinline__ void prefetch_row(const StepArgs& a, const RowInfo& r
 // `rec_base` = number of spikes recorded before step n: the spiking thread also writes the spike record (a2,
 // PAPER.md:181 "all spike times of all neurons recorded").  The atomic is issued before the row lookup and the
 // prefetches so that all three overlap.
-__device__ __forceinline__ void append_spike(const StepArgs& a, bool spk, int32_t id, long long n, unsigned long long rec_base,
+__device__ __forceinline__ void append_spike(const StepArgs& a, bool spk, int32_t i_local, long long n, unsigned long long rec_base,
                                              unsigned long long win_base = 0) {
     const unsigned m = __ballot_sync(0xffffffffu, spk);
     if (m == 0) return;
+    const int32_t id = a.id_first + i_local;                  // the spike array, the record and the rows use global ids
     const int lane = threadIdx.x & 31;
     const int leader = __ffs(m) - 1;
     int base = 0;
@@ -490,13 +575,13 @@ __device__ __forceinline__ void append_spike(const StepArgs& a, bool spk, int32_
     base = __shfl_sync(0xffffffffu, base, leader);
     if (spk) {
         const int idx = base + __popc(m & ((1u << lane) - 1u));
-        const size_t k = (size_t)(n & 1) * a.N + idx;
+        const size_t k = (size_t)(n & 1) * a.NS + idx;
         a.spike_list[k] = id;
         st_row_info(a.spike_row + k, r);
         const unsigned long long pos = rec_base + (unsigned long long)idx;
         if (pos < (unsigned long long)a.rec_cap) { a.rec_id[pos] = id; a.rec_step[pos] = (int32_t)n; }
         if (a.win_id) a.win_id[(win_base + (unsigned long long)idx) % (unsigned long long)a.win_cap] = id;
-        stat_on_spike(a, id, n);
+        stat_on_spike(a, i_local, n);
     }
 }
 
@@ -543,29 +628,33 @@ __device__ __forceinline__ int poisson_count(const StepArgs& a, const PopDev* __
 // Cash-Karp 5(4), controller and spike rule as readings C23-C25 state them.  fp32 throughout.
 // ---------------------------------------------------------------------------------------
 struct AdexY { float V, w, gx, yx, gi, yi; };
+struct AdexK { float V, w; };
 
-__device__ __forceinline__ AdexY adex_rhs(const AdexDev& p, const AdexY& y) {
-    const float V = fminf(y.V, p.V_peak);                                           // C24
+// Right-hand side of Eqs. (3) and (5) for given conductances (Eq. (4) with reading C21).
+__device__ __forceinline__ AdexK adex_rhs_vw(const AdexDev& p, float Vs, float ws, float gx, float gi) {
+    const float V = fminf(Vs, p.V_peak);                                            // C24
     const float I_spike = p.gL_DeltaT * __expf((V - p.V_T) * p.inv_DeltaT);
-    const float I_syn = fmaf(y.gx, p.E_ex - V, y.gi * (p.E_in - V));                // C21
-    AdexY f;
-    f.V = (fmaf(-p.g_L, V - p.E_L, I_spike) + I_syn - y.w + p.I_e) * p.inv_C;
-    f.w = (p.a * (V - p.E_L) - y.w) * p.inv_tau_w;
-    f.gx = fmaf(-y.gx, p.inv_tau_syn, y.yx);
-    f.yx = -y.yx * p.inv_tau_syn;
-    f.gi = fmaf(-y.gi, p.inv_tau_syn, y.yi);
-    f.yi = -y.yi * p.inv_tau_syn;
+    const float I_syn = fmaf(gx, p.E_ex - V, gi * (p.E_in - V));                    // C21
+    AdexK f;
+    f.V = (fmaf(-p.g_L, V - p.E_L, I_spike) + I_syn - ws + p.I_e) * p.inv_C;
+    f.w = (p.a * (V - p.E_L) - ws) * p.inv_tau_w;
     return f;
 }
-#define NG_AXPY(out, y, h, expr) \
-    out.V = fmaf(h, expr(V), y.V); out.w = fmaf(h, expr(w), y.w); out.gx = fmaf(h, expr(gx), y.gx); \
-    out.yx = fmaf(h, expr(yx), y.yx); out.gi = fmaf(h, expr(gi), y.gi); out.yi = fmaf(h, expr(yi), y.yi);
 
 // One time step of one neuron (C23, C24), resumable: at most max_iter attempts of the controller loop; t (time reached
 // inside the step) and spiked carry over.  Returns true when the step is complete.  The pipelined kernel gives every
 // neuron ONE attempt in its own lane (99 % finish: the sub-step is the whole time step) and collects the others —
-// neurons on the exponential upswing, up to ten sub-steps — in a CTA list that is worked off by dense warps
+// neurons on the exponential upswing, up to thirty sub-steps — in a CTA list that is worked off by dense warps
 // afterwards, so that a warp does not wait for its slowest lane.
+//
+// The embedded Cash-Karp 5(4) step is applied to the six-component system, as the oracle does, but only V and w carry
+// their six stage derivatives in registers: the alpha-conductance pair u = (g, y) of a port obeys the LINEAR autonomous
+// system u' = A u, A = -1/tau I + N (N nilpotent), for which every Runge-Kutta stage value is a polynomial in x = -h/tau
+// applied to u:   y_i = s_i(x) y,   g_i = s_i(x) g + h s_i'(x) y,
+// with s_1 = 1, s_i(x) = 1 + x sum_{j<i} b_ij s_j(x); the 5th-order result uses p(x) = 1 + x sum_j c_j s_j(x) and the
+// error estimate e(x) = x sum_j (c_j - c*_j) s_j(x) in the same way.  (Coefficients below: exact rationals of the
+// Cash-Karp tableau.)  Same arithmetic as the six-component stage loop up to fp32 rounding, 24 fewer live registers — the
+// 64-register budget of two 512-thread CTAs per SM is then met without local-memory spills.
 template <bool kOneAttempt>
 __device__ __forceinline__ bool adex_advance(const AdexDev& p, AdexY& y, float& h_int, float& t, bool& spiked, float h_step) {
     for (int it = 0; t < h_step; ++it) {
@@ -573,40 +662,54 @@ __device__ __forceinline__ bool adex_advance(const AdexDev& p, AdexY& y, float& 
         const float h = fmaxf(h_int, p.h_min);
         const bool clipped = h > h_step - t;
         const float ht = clipped ? h_step - t : h;
-        AdexY k1 = adex_rhs(p, y), tmp, k2, k3, k4, k5, k6;
-#define E2(c) (0.2f * k1.c)
-        NG_AXPY(tmp, y, ht, E2) k2 = adex_rhs(p, tmp);
-#define E3(c) (0.075f * k1.c + 0.225f * k2.c)
-        NG_AXPY(tmp, y, ht, E3) k3 = adex_rhs(p, tmp);
-#define E4(c) (0.3f * k1.c - 0.9f * k2.c + 1.2f * k3.c)
-        NG_AXPY(tmp, y, ht, E4) k4 = adex_rhs(p, tmp);
+        const float x = -ht * p.inv_tau_syn;
+        // stage conductances g_i = s_i(x) g + h s_i'(x) y of both ports
+#define NG_G(si, dsi) const float s_ = (si), hd_ = ht * (dsi); const float gx_ = fmaf(s_, y.gx, hd_ * y.yx), gi_ = fmaf(s_, y.gi, hd_ * y.yi);
+        const AdexK k1 = adex_rhs_vw(p, y.V, y.w, y.gx, y.gi);
+        AdexK k2, k3, k4, k5, k6;
+        { NG_G(fmaf(0.2f, x, 1.f), 0.2f)
+          k2 = adex_rhs_vw(p, fmaf(ht, 0.2f * k1.V, y.V), fmaf(ht, 0.2f * k1.w, y.w), gx_, gi_); }
+        { NG_G(fmaf(x, fmaf(0.045f, x, 0.3f), 1.f), fmaf(0.09f, x, 0.3f))
+          k3 = adex_rhs_vw(p, fmaf(ht, 0.075f * k1.V + 0.225f * k2.V, y.V), fmaf(ht, 0.075f * k1.w + 0.225f * k2.w, y.w), gx_, gi_); }
+        { NG_G(fmaf(x, fmaf(x, fmaf(0.054f, x, 0.18f), 0.6f), 1.f), fmaf(x, fmaf(0.162f, x, 0.36f), 0.6f))
+          k4 = adex_rhs_vw(p, fmaf(ht, 0.3f * k1.V - 0.9f * k2.V + 1.2f * k3.V, y.V), fmaf(ht, 0.3f * k1.w - 0.9f * k2.w + 1.2f * k3.w, y.w), gx_, gi_); }
+        { NG_G(fmaf(x, fmaf(x, fmaf(x, fmaf(0.07f, x, 7.f / 60.f), 0.5f), 1.f), 1.f), fmaf(x, fmaf(x, fmaf(0.28f, x, 0.35f), 1.f), 1.f))
 #define E5(c) ((-11.f / 54.f) * k1.c + 2.5f * k2.c - (70.f / 27.f) * k3.c + (35.f / 27.f) * k4.c)
-        NG_AXPY(tmp, y, ht, E5) k5 = adex_rhs(p, tmp);
+          k5 = adex_rhs_vw(p, fmaf(ht, E5(V), y.V), fmaf(ht, E5(w), y.w), gx_, gi_); }
+        { NG_G(fmaf(x, fmaf(x, fmaf(x, fmaf(x, fmaf(1771.f / 409600.f, x, 1771.f / 61440.f), 161.f / 1536.f), 49.f / 128.f), 0.875f), 1.f),
+               fmaf(x, fmaf(x, fmaf(x, fmaf(1771.f / 81920.f, x, 1771.f / 15360.f), 161.f / 512.f), 49.f / 64.f), 0.875f))
 #define E6(c) ((1631.f / 55296.f) * k1.c + (175.f / 512.f) * k2.c + (575.f / 13824.f) * k3.c + (44275.f / 110592.f) * k4.c + (253.f / 4096.f) * k5.c)
-        NG_AXPY(tmp, y, ht, E6) k6 = adex_rhs(p, tmp);
+          k6 = adex_rhs_vw(p, fmaf(ht, E6(V), y.V), fmaf(ht, E6(w), y.w), gx_, gi_); }
         // 5th-order weights and the difference to the embedded 4th-order ones
 #define Y5(c) ((37.f / 378.f) * k1.c + (250.f / 621.f) * k3.c + (125.f / 594.f) * k4.c + (512.f / 1771.f) * k6.c)
 #define ER(c) ((37.f / 378.f - 2825.f / 27648.f) * k1.c + (250.f / 621.f - 18575.f / 48384.f) * k3.c + \
                (125.f / 594.f - 13525.f / 55296.f) * k4.c - (277.f / 14336.f) * k5.c + (512.f / 1771.f - 0.25f) * k6.c)
+        // error polynomial of the linear pair: e(x) = x^5 (-277/1228800 + 277/1638400 x), h e'(x) likewise
+        const float x2 = x * x, x4 = x2 * x2;
+        const float eP = x4 * x * fmaf(277.f / 1638400.f, x, -277.f / 1228800.f);
+        const float hdE = ht * x4 * fmaf(831.f / 819200.f, x, -277.f / 245760.f);
         float e = fabsf(ht * ER(V)) * p.inv_tol[0];
         e = fmaxf(e, fabsf(ht * ER(w)) * p.inv_tol[1]);
-        e = fmaxf(e, fabsf(ht * ER(gx)) * p.inv_tol[2]);
-        e = fmaxf(e, fabsf(ht * ER(yx)) * p.inv_tol[3]);
-        e = fmaxf(e, fabsf(ht * ER(gi)) * p.inv_tol[4]);
-        e = fmaxf(e, fabsf(ht * ER(yi)) * p.inv_tol[5]);
+        e = fmaxf(e, fabsf(fmaf(eP, y.gx, hdE * y.yx)) * p.inv_tol[2]);
+        e = fmaxf(e, fabsf(eP * y.yx) * p.inv_tol[3]);
+        e = fmaxf(e, fabsf(fmaf(eP, y.gi, hdE * y.yi)) * p.inv_tol[4]);
+        e = fmaxf(e, fabsf(eP * y.yi) * p.inv_tol[5]);
         const bool accept = e <= 1.f || ht <= p.h_min;
         float fac = e > 0.f ? 0.9f * __powf(e, -0.2f) : 5.f;
         fac = fminf(5.f, fmaxf(0.2f, fac));
         if (!clipped || !accept) h_int = fminf(h_step, ht * fac);
         if (accept) {
-            NG_AXPY(tmp, y, ht, Y5)
-            y = tmp;
+            // p(x) = 1 + x + x^2/2 + x^3/6 + x^4/24 + x^5/120 + x^6/800 and h p'(x)
+            const float P = fmaf(x, fmaf(x, fmaf(x, fmaf(x, fmaf(x, fmaf(1.f / 800.f, x, 1.f / 120.f), 1.f / 24.f), 1.f / 6.f), 0.5f), 1.f), 1.f);
+            const float hdP = ht * fmaf(x, fmaf(x, fmaf(x, fmaf(x, fmaf(3.f / 400.f, x, 1.f / 24.f), 1.f / 6.f), 0.5f), 1.f), 1.f);
+            y.V = fmaf(ht, Y5(V), y.V);
+            y.w = fmaf(ht, Y5(w), y.w);
+            y.gx = fmaf(P, y.gx, hdP * y.yx); y.yx = P * y.yx;
+            y.gi = fmaf(P, y.gi, hdP * y.yi); y.yi = P * y.yi;
             t = clipped ? h_step : t + ht;
             if (y.V >= p.V_peak) { y.V = p.V_reset; y.w += p.b; spiked = true; }     // C24; a 2nd crossing is not recorded (C20)
         }
-#undef E2
-#undef E3
-#undef E4
+#undef NG_G
 #undef E5
 #undef E6
 #undef Y5
@@ -614,7 +717,6 @@ __device__ __forceinline__ bool adex_advance(const AdexDev& p, AdexY& y, float& 
     }
     return true;
 }
-#undef NG_AXPY
 __device__ __forceinline__ bool adex_step(const AdexDev& p, AdexY& y, float& h_int, float h_step) {
     float t = 0.f;
     bool spiked = false;
@@ -631,8 +733,8 @@ struct NeuronLoad { float in, in1, V, I; int r, pi, kq; };
 template <bool kAdex>
 __device__ __forceinline__ NeuronLoad neuron_load(const StepArgs& a, const float* __restrict__ plane, int i, bool have_k) {
     NeuronLoad L;
-    L.in = __ldcg(plane + i);                    // written by red.global from other SMs: read at L2
-    L.in1 = kAdex ? __ldcg(plane + a.N + i) : 0.f;          // inhibitory port
+    L.in = ld_plane(plane + i);                  // written by red.global from other SMs: read at L2
+    L.in1 = kAdex ? ld_plane(plane + a.N + i) : 0.f;          // inhibitory port
     L.kq = have_k ? (int)a.pois_k[i] : 0xff;
     L.V = 0.f; L.I = 0.f; L.r = 0; L.pi = 0;
     if (!a.bypass) { L.V = a.V[i]; L.I = a.I[i]; L.r = a.refr[i]; L.pi = a.pop_of[i]; }
@@ -644,7 +746,7 @@ __device__ __forceinline__ bool neuron_early(const StepArgs& a, const PopDev* __
                                              NeuronRegs& g, const NeuronLoad& L) {
     g.in = L.in; g.in1 = L.in1; g.kq = L.kq; g.adex = false; g.pending = false;
     if (a.bypass) {                                          // DESIGN.md C8: delivery-only mode
-        const uint4 x = philox4x32_10(a.seed_lo, a.seed_hi, (uint32_t)i, (uint32_t)n, (uint32_t)(n >> 32), kTagInject);
+        const uint4 x = philox4x32_10(a.seed_lo, a.seed_hi, (uint32_t)(a.id_first + i), (uint32_t)n, (uint32_t)(n >> 32), kTagInject);
         return x.x < a.inject_thr;
     }
     float V = L.V;
@@ -676,12 +778,12 @@ __device__ __forceinline__ bool neuron_early(const StepArgs& a, const PopDev* __
 template <bool kAdex>
 __device__ __forceinline__ void neuron_late(const StepArgs& a, const PopDev* __restrict__ P, long long n, int i,
                                             float* __restrict__ plane, const NeuronRegs& g) {
-    plane[i] = 0.f;
-    if (kAdex) plane[a.N + i] = 0.f;
+    clear_plane(plane + i);
+    if (kAdex) clear_plane(plane + a.N + i);
     if (a.last_input) { a.last_input[i] = g.in; if (kAdex) a.last_input[a.N + i] = g.in1; }
     if (a.bypass) return;
     const PopDev* __restrict__ p = P + g.pi;
-    const int k = g.kq != 0xff ? g.kq : poisson_count(a, p, n, i);
+    const int k = g.kq != 0xff ? g.kq : poisson_count(a, p, n, a.id_first + i);
     if (kAdex && g.adex) {                       // g.I carries y_ex after the integration; Poisson drive on the excitatory port
         a.ax_yx[i] = fmaf(p->ax.jump, fmaf(p->w_ext, (float)k, g.in), g.I);
         return;
@@ -696,13 +798,13 @@ __device__ __noinline__ bool adex_resume(const StepArgs& a, const PopDev* __rest
     const PopDev* __restrict__ p = P + a.pop_of[i];
     AdexY y; y.V = a.V[i]; y.w = a.ax_w[i]; y.gx = a.ax_gx[i]; y.yx = a.ax_yx[i]; y.gi = a.ax_gi[i]; y.yi = a.ax_yi[i];
     float h_int = a.ax_h[i];
-    const float in = __ldcg(plane + i), in1 = __ldcg(plane + a.N + i);
+    const float in = ld_plane(plane + i), in1 = ld_plane(plane + a.N + i);
     adex_advance<false>(p->ax, y, h_int, t, spiked, a.dt_ms);
-    const int k = poisson_count(a, p, n, i);
+    const int k = poisson_count(a, p, n, a.id_first + i);
     a.V[i] = y.V; a.ax_w[i] = y.w; a.ax_gx[i] = y.gx; a.ax_gi[i] = y.gi; a.ax_h[i] = h_int;
     a.ax_yx[i] = fmaf(p->ax.jump, fmaf(p->w_ext, (float)k, in), y.yx);       // C25
     a.ax_yi[i] = fmaf(p->ax.jump, in1, y.yi);
-    plane[i] = 0.f; plane[a.N + i] = 0.f;
+    clear_plane(plane + i); clear_plane(plane + a.N + i);
     if (a.last_input) { a.last_input[i] = in; a.last_input[a.N + i] = in1; }
     return spiked;
 }
@@ -723,27 +825,6 @@ __device__ __forceinline__ void update_phase(const StepArgs& a, const PopDev* __
         append_spike(a, spk, i, n, rec_base, win_base);
         if (i < N) neuron_late<kAdex>(a, P, n, i, plane, g);
     }
-}
-
-__device__ __forceinline__ void red_add_f32(float* addr, float v) {
-    asm volatile("red.global.add.f32 [%0], %1;" ::"l"(addr), "f"(v) : "memory");
-}
-__device__ __forceinline__ int4 ld_stream_s32x4(const int32_t* p) {
-    int4 r;
-    asm("ld.global.nc.L1::no_allocate.v4.s32 {%0,%1,%2,%3}, [%4];"
-                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
-    return r;
-}
-__device__ __forceinline__ float4 ld_stream_f32x4(const float* p) {
-    float4 r;
-    asm("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];"
-                 : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p));
-    return r;
-}
-__device__ __forceinline__ uint32_t ld_stream_u32(const void* p) {
-    uint32_t r;
-    asm("ld.global.nc.L1::no_allocate.u32 %0, [%1];" : "=r"(r) : "l"(p));
-    return r;
 }
 
 // Step bookkeeping of the stand-alone delivery kernels (a4), one thread: publish the next step index, clear the
@@ -822,7 +903,7 @@ __device__ __forceinline__ void deliver_item(const StepArgs& a, int nmod, long l
 // Returns M, the number of spikes of step n.  Thread 0 reads M while the first kEntryTile threads already load the
 // first tile of entries speculatively (one L2 round trip instead of two).
 __device__ __forceinline__ int deliver_rows_phase(const StepArgs& a, long long n, int nmod, DeliverShared& sh) {
-    const int N = a.N;
+    const int N = a.NS;
     const RowInfo* __restrict__ rows = a.spike_row + (size_t)(n & 1) * N;
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5, wpb = blockDim.x >> 5;
     const int gwarp = blockIdx.x * wpb + wib, gwarps = gridDim.x * wpb;
@@ -939,7 +1020,7 @@ __device__ __forceinline__ void red_vec(const StepArgs& a, const VecRef& r, cons
 template <bool kWindow>
 __device__ __forceinline__ void deliver_groups_phase(const StepArgs& a, long long n, int nmod, int M, long long gwarp,
                                                      long long gwarps, int lane, const unsigned long long* off = nullptr, int W = 0) {
-    const int N = a.N, D = a.D, Dr = a.Dr;
+    const int N = a.NS, D = a.D, Dr = a.Dr;
     const int32_t* __restrict__ list = a.spike_list + (size_t)(n & 1) * N;
     const long long items = kWindow ? (long long)(off[W] - off[0]) : (long long)M * D;
     if (items == 0) return;
@@ -1055,13 +1136,14 @@ struct QueueShared {
 };
 
 __device__ __forceinline__ void queue_append_phase(const StepArgs& a, long long n, int M, float* __restrict__ plane1, QueueShared& sh) {
-    const int N = a.N, D = a.D;
+    const int N = a.NS, D = a.D;
     const RowInfo* __restrict__ rows = a.spike_row + (size_t)(n & 1) * N;
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const int nmodD = sh.nmodD;
     const int tile_len = max(1, min(kEntryTile, (M + (int)gridDim.x - 1) / (int)gridDim.x));
     unsigned long long ev = 0;
     bool overflow = false;
+    if (threadIdx.x < 256) sh.hist[threadIdx.x] = 0;
     for (int tile0 = (int)blockIdx.x * tile_len; tile0 < M; tile0 += (int)gridDim.x * tile_len) {
         const int m = min(tile_len, M - tile0);
         __syncthreads();                                       // the previous tile's readers are done
@@ -1090,7 +1172,6 @@ __device__ __forceinline__ void queue_append_phase(const StepArgs& a, long long 
         __syncthreads();
         const int total_vec = sh.pre[m];
         for (int vb = 0; vb < total_vec; vb += kQThreads * kQVecPerThread) {
-            for (int k = threadIdx.x; k < 256; k += kQThreads) sh.hist[k] = 0;
             int4 t4[kQVecPerThread]; float4 w4[kQVecPerThread]; uint32_t d4[kQVecPerThread];
 #pragma unroll
             for (int u = 0; u < kQVecPerThread; ++u) {
@@ -1103,7 +1184,7 @@ __device__ __forceinline__ void queue_append_phase(const StepArgs& a, long long 
                     t4[u] = ld_stream_s32x4(a.tgt + p); w4[u] = ld_stream_f32x4(a.w + p); d4[u] = ld_stream_u32(a.dly + p);
                 }
             }
-            __syncthreads();                                   // hist is cleared
+            // hist is zero here: cleared before the first batch and in the staging phase of every batch
             uint32_t rank[kQVecPerThread][4];
 #pragma unroll
             for (int u = 0; u < kQVecPerThread; ++u) {
@@ -1114,36 +1195,46 @@ __device__ __forceinline__ void queue_append_phase(const StepArgs& a, long long 
                     uint32_t d = tt[c] >= 0 ? (d4[u] >> (8 * c)) & 0xffu : 0u;           // padding records: target -1
                     if (d == 1u) { red_add_f32(plane1 + tt[c], ww[c]); d = 0u; }         // consumed by the very next step
                     d4[u] = (d4[u] & ~(0xffu << (8 * c))) | (d << (8 * c));              // 0 = not queued
+#ifdef NG_Q_MATCH
                     const unsigned mask = __match_any_sync(0xffffffffu, d);             // one shared-memory atomic per delay and warp
                     const int leader = __ffs(mask) - 1;
                     uint32_t base = 0;
                     if (d != 0u && lane == leader) base = atomicAdd(&sh.hist[d], (uint32_t)__popc(mask));
                     base = __shfl_sync(0xffffffffu, base, leader);
                     rank[u][c] = base + (uint32_t)__popc(mask & ((1u << lane) - 1u));
+#else
+                    rank[u][c] = d != 0u ? atomicAdd(&sh.hist[d], 1u) : 0u;             // the order inside a queue is free
+#endif
                 }
             }
-            __syncthreads();
-            if (wib == 0) {                                    // prefix over the delays; one global atomic per (batch, delay)
-                uint32_t carry = 0;
-                for (int b0 = 0; b0 <= D; b0 += 32) {
-                    const int k = b0 + lane;
-                    const uint32_t h = (k >= 2 && k <= D) ? sh.hist[k] : 0u;
-                    uint32_t incl = h;
+            __syncthreads();                                   // (A) the histogram of the batch is complete
+            if (threadIdx.x < 256) {                           // one global atomic per (batch, delay), all in flight together
+                const int k = threadIdx.x;
+                const uint32_t h = (k >= 2 && k <= D) ? sh.hist[k] : 0u;
+                if (h > 0u) {
+                    int qs = nmodD + k; if (qs >= D) qs -= D;  // arrival step n + k
+                    sh.gbase[k] = atomicAdd(a.q_tail + (size_t)qs * kQTailStride, (unsigned long long)h);
+                }
+            } else if (wib == 8) {                             // meanwhile one warp prefix-sums the 256 bins, 8 per lane
+                uint32_t loc[8], sum = 0;
 #pragma unroll
-                    for (int o = 1; o < 32; o <<= 1) {
-                        const uint32_t y = __shfl_up_sync(0xffffffffu, incl, o);
-                        if (lane >= o) incl += y;
-                    }
-                    if (k <= D) sh.sbase[k] = carry + incl - h;
-                    if (h > 0u) {
-                        int qs = nmodD + k; if (qs >= D) qs -= D;          // arrival step n + k
-                        sh.gbase[k] = atomicAdd(a.q_tail + (size_t)qs * kQTailStride, (unsigned long long)h);
-                    }
-                    carry += __shfl_sync(0xffffffffu, incl, 31);
+                for (int j = 0; j < 8; ++j) {
+                    const int k = lane * 8 + j;
+                    loc[j] = sum;
+                    sum += (k >= 2 && k <= D) ? sh.hist[k] : 0u;
                 }
-                if (lane == 0) sh.sbase[D + 1] = carry;
+                uint32_t incl = sum;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const uint32_t y = __shfl_up_sync(0xffffffffu, incl, o);
+                    if (lane >= o) incl += y;
+                }
+#pragma unroll
+                for (int j = 0; j < 8; ++j) sh.sbase[lane * 8 + j] = incl - sum + loc[j];
+                if (lane == 31) sh.sbase[256] = incl;          // sbase[D + 1] = records of the batch that go to a queue
             }
-            __syncthreads();
+            __syncthreads();                                   // (B) sbase and gbase are known
+            if (threadIdx.x < 256) sh.hist[threadIdx.x] = 0;   // for the next batch
 #pragma unroll
             for (int u = 0; u < kQVecPerThread; ++u) {
                 const int tt[4] = {t4[u].x, t4[u].y, t4[u].z, t4[u].w};
@@ -1158,16 +1249,16 @@ __device__ __forceinline__ void queue_append_phase(const StepArgs& a, long long 
                     }
                 }
             }
-            __syncthreads();
+            __syncthreads();                                   // (C) the batch is staged in delay order
             const int total = (int)sh.sbase[D + 1];
-            for (int p = threadIdx.x; p < total; p += kQThreads) {    // delay-sorted: consecutive threads, consecutive queue cells
+            for (int p = threadIdx.x; p < total; p += kQThreads) {    // consecutive threads, consecutive queue cells
                 const int d = sh.sbin[p];
                 int qs = nmodD + d; if (qs >= D) qs -= D;
                 const unsigned long long pos = sh.gbase[d] + (unsigned long long)(p - (int)sh.sbase[d]);
                 if (pos < (unsigned long long)a.q_cap) a.q_ev[(size_t)qs * (size_t)a.q_cap + pos] = sh.staged[p];
                 else overflow = true;
             }
-            __syncthreads();                                   // staged / hist are rewritten by the next batch
+            // no barrier here: the next batch touches only hist before its (A), sbase / gbase after (A), staged after (B)
         }
     }
     if (overflow) a.ctl->err_queue = 1;
@@ -1191,10 +1282,17 @@ __device__ __forceinline__ void queue_drain_phase(const StepArgs& a, float* __re
     const long long T = (long long)(T0 < (unsigned long long)a.q_cap ? T0 : (unsigned long long)a.q_cap);
     const int2* __restrict__ q = a.q_ev + (size_t)qs * (size_t)a.q_cap;
     const long long gtid = (long long)blockIdx.x * blockDim.x + threadIdx.x, gthreads = (long long)gridDim.x * blockDim.x;
-    for (long long i = gtid; i < (T >> 1); i += gthreads) {    // two events per 128-bit load
-        const int4 v = ld_stream_s32x4(reinterpret_cast<const int32_t*>(q + 2 * i));
-        red_add_f32(plane1 + v.x, __int_as_float(v.y));
-        red_add_f32(plane1 + v.z, __int_as_float(v.w));
+    const long long pairs = T >> 1;                            // two events per 128-bit load, four loads in flight per thread
+    for (long long i = gtid; i < pairs; i += 4 * gthreads) {
+        int4 v[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+            v[u] = i + u * gthreads < pairs ? ld_stream_s32x4(reinterpret_cast<const int32_t*>(q + 2 * (i + u * gthreads))) : make_int4(-1, 0, -1, 0);
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            if (v[u].x >= 0) red_add_f32(plane1 + v[u].x, __int_as_float(v[u].y));
+            if (v[u].z >= 0) red_add_f32(plane1 + v[u].z, __int_as_float(v[u].w));
+        }
     }
     if ((T & 1) && gtid == 0) { const int2 v = q[T - 1]; red_add_f32(plane1 + v.x, __int_as_float(v.y)); }
 }
@@ -1408,7 +1506,7 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
                     // reds) overlaps all of it and is waited for only by the current update at the end.
                     const int t = threadIdx.x;
                     if (ii < N) {
-                        asm volatile("ld.global.cg.f32 %0, [%1];" : "=f"(res_in) : "l"(plane + i));      // first: the one long latency
+                        res_in = ld_plane(plane + i);                  // first: the one long latency
                         float V = sh.res_V[t];
                         int rf = sh.res_r[t];
                         res_I = sh.res_I[t];
@@ -1523,7 +1621,7 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
                 if (ii < N) {
                     const int t = threadIdx.x, i = (int)ii;
                     const PopDev* __restrict__ p = P + sh.res_pi[t];
-                    plane[i] = 0.f;
+                    clear_plane(plane + i);
                     if (a.last_input) a.last_input[i] = res_in;
                     const int k = have_k ? (int)sh.res_kq[t] : poisson_count(a, p, n, i);
                     sh.res_I[t] = fmaf(p->P11, res_I, res_in) + p->w_ext * (float)k;
@@ -1535,7 +1633,7 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
 #pragma unroll
                     for (int u = 0; u < 4; ++u) {
                         const long long ii = ((long long)(q0 + u) * gridDim.x + blockIdx.x) * U + threadIdx.x;
-                        inv[u] = (q0 + u < rm.rounds && ii < N) ? __ldcg(plane + ii) : 0.f;
+                        inv[u] = (q0 + u < rm.rounds && ii < N) ? ld_plane(plane + ii) : 0.f;
                     }
 #pragma unroll
                     for (int u = 0; u < 4; ++u) {
@@ -1543,7 +1641,7 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
                         if (q0 + u < rm.rounds && ii < N) {
                             const int idx = (q0 + u) * U + threadIdx.x, i = (int)ii;
                             const PopDev* __restrict__ p = P + rm.pi[idx];
-                            plane[i] = 0.f;
+                            clear_plane(plane + i);
                             if (a.last_input) a.last_input[i] = inv[u];
                             const int k = poisson_count(a, p, n, i);
                             rm.I[idx] = fmaf(p->P11, rm.I[idx], inv[u]) + p->w_ext * (float)k;
@@ -1873,6 +1971,81 @@ __global__ void __launch_bounds__(kDeliverThreads, 3) deliver_kernel(const StepA
     if (gtid == 0) bookkeeping_scalar(a, sc.n, sc.slot, M, __ldcg(&a.ctl->rec_total[sc.n & 1]));
 }
 
+// ---------------------------------------------------------------------------------------
+// Target-sharded multi-GPU ("a spike buffer, similar to the local one, is
+// created in the remote host"): rank r owns the neurons [id_first, id_first + N) — their state, their input planes and
+// every connection onto them, stored source-major over ALL sources.  One exchange per time step: after update(n) every
+// rank stores the ids of ITS spikes straight into the receive buffer of every peer (peer-mapped device memory over
+// NVLink: plain stores, then a system-scope release of a step-stamped flag) and then appends what the peers stored in its
+// own buffer to its spike array (acquire-poll on the flags); delivery is local.  No collective library call, no host
+// round trip.  Receive buffer of a rank: header { int64 flag[2][16]; int32 cnt[2][16]; } padded to 512 B, then
+// int32 ids[2][world][cap], indexed by step parity and SOURCE rank.  Two parities suffice: rank s can publish step n+2
+// only after it gathered step n+1, i.e. after this rank published n+1, i.e. after this rank gathered step n.
+// ---------------------------------------------------------------------------------------
+constexpr int kMaxShards = 16;
+constexpr int kXchgHeaderBytes = 512;
+__device__ __forceinline__ long long* xchg_flag(unsigned char* base, int parity, int src) { return reinterpret_cast<long long*>(base) + parity * kMaxShards + src; }
+__device__ __forceinline__ int32_t* xchg_cnt(unsigned char* base, int parity, int src) { return reinterpret_cast<int32_t*>(base + 256) + parity * kMaxShards + src; }
+__device__ __forceinline__ int32_t* xchg_ids(unsigned char* base, int parity, int src, int world, int cap) {
+    return reinterpret_cast<int32_t*>(base + kXchgHeaderBytes) + ((size_t)parity * world + src) * (size_t)cap;
+}
+
+// one CTA per peer: this rank's spikes of step n -> the peer's receive buffer
+__global__ void __launch_bounds__(256) xchg_publish_kernel(const StepArgs a) {
+    const int q = blockIdx.x;
+    if (q == a.xchg_rank) return;
+    __shared__ long long n_s; __shared__ int M_s;
+    if (threadIdx.x == 0) { n_s = __ldcg(&a.ctl->step_d); M_s = __ldcg(&a.ctl->spike_cnt[n_s & 3]); }
+    __syncthreads();
+    const long long n = n_s; const int M = M_s, par = (int)(n & 1);
+    const int32_t* __restrict__ list = a.spike_list + (size_t)par * a.NS;
+    int32_t* dst = xchg_ids(a.xchg[q], par, a.xchg_rank, a.xchg_world, a.xchg_cap);
+    for (int i = threadIdx.x; i < M; i += blockDim.x) dst[i] = __ldcg(list + i);
+    __threadfence_system();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        *xchg_cnt(a.xchg[q], par, a.xchg_rank) = M;
+        const long long stamp = n + 1;
+        asm volatile("st.release.sys.global.s64 [%0], %1;" ::"l"(xchg_flag(a.xchg[q], par, a.xchg_rank)), "l"(stamp) : "memory");
+    }
+}
+
+// one CTA per peer: the peer's spikes of step n, from this rank's own receive buffer, appended to the spike array
+__global__ void __launch_bounds__(256) xchg_gather_kernel(const StepArgs a) {
+    const int src = blockIdx.x;
+    if (src == a.xchg_rank) return;
+    __shared__ long long n_s; __shared__ int M_s, base_s; __shared__ unsigned long long win_s, rec_s;
+    unsigned char* own = a.xchg[a.xchg_rank];
+    if (threadIdx.x == 0) {
+        const long long n = __ldcg(&a.ctl->step_d);
+        const int par = (int)(n & 1);
+        long long v = 0;
+        const long long t0 = clock64();
+        do {                                                   // bounded: a lost peer must not hang the GPU
+            asm volatile("ld.acquire.sys.global.s64 %0, [%1];" : "=l"(v) : "l"(xchg_flag(own, par, src)) : "memory");
+        } while (v != n + 1 && clock64() - t0 < 20000000000LL);
+        int M = 0;
+        if (v == n + 1) M = *reinterpret_cast<volatile int32_t*>(xchg_cnt(own, par, src)); else a.ctl->err_xchg = 1;
+        n_s = n; M_s = M;
+        base_s = M > 0 ? atomicAdd(&a.ctl->spike_cnt[n & 3], M) : 0;
+        win_s = a.win_id ? __ldcg(&a.ctl->win_start[(unsigned long long)n % (unsigned)(a.D + 1)]) : 0ULL;
+        rec_s = __ldcg(&a.ctl->rec_total[n & 1]);
+    }
+    __syncthreads();
+    const long long n = n_s; const int M = M_s, base = base_s, par = (int)(n & 1);
+    const int32_t* ids = xchg_ids(own, par, src, a.xchg_world, a.xchg_cap);
+    for (int i = threadIdx.x; i < M; i += blockDim.x) {
+        const int32_t id = __ldcv(ids + i);
+        const size_t k = (size_t)par * a.NS + base + i;
+        a.spike_list[k] = id;
+        st_row_info(a.spike_row + k, ld_row_info(a.row_info + id));
+        if (a.win_id) a.win_id[(win_s + (unsigned long long)(base + i)) % (unsigned long long)a.win_cap] = id;
+        // the spike record of every rank holds the spikes of the whole network (the step bookkeeping counts all of them)
+        const unsigned long long pos = rec_s + (unsigned long long)(base + i);
+        if (pos < (unsigned long long)a.rec_cap) { a.rec_id[pos] = id; a.rec_step[pos] = (int32_t)n; }
+    }
+}
+
 // Delivery kernel 5 as a stand-alone launch (one per time step, after update_kernel).
 __global__ void __launch_bounds__(kQThreads, 2) queue_deliver_kernel(const StepArgs a) {
     __shared__ QueueShared sh;
@@ -1885,8 +2058,12 @@ __global__ void __launch_bounds__(kQThreads, 2) queue_deliver_kernel(const StepA
     }
     __syncthreads();
     float* __restrict__ plane1 = a.ring + (size_t)(sc.slot == 0 ? 1 : 0) * a.NR;       // two planes: this step's and the next step's input
+#ifdef NG_Q_SKIP_DRAIN
+    queue_append_phase(a, sc.n, sc.M, plane1, sh);
+#else
     if (blockIdx.x & 1) { queue_append_phase(a, sc.n, sc.M, plane1, sh); queue_drain_phase(a, plane1, sh); }
     else { queue_drain_phase(a, plane1, sh); queue_append_phase(a, sc.n, sc.M, plane1, sh); }
+#endif
     if (blockIdx.x == 0 && threadIdx.x == 0) bookkeeping_scalar(a, sc.n, sc.slot, sc.M, __ldcg(&a.ctl->rec_total[sc.n & 1]));
 }
 

@@ -40,7 +40,7 @@ def test_struct_layouts_match_header():
             printf("%zu %zu %zu %zu\n", offsetof(ng_config, seed), offsetof(ng_config, device), offsetof(ng_stats, build_ms), offsetof(ng_stats, delivery_kernel));
             printf("%d %d %d %d %d %d\n", NG_OK, NG_ERR_INVALID_ARG, NG_ERR_STATE, NG_ERR_OOM, NG_ERR_CUDA, NG_ERR_OVERFLOW);
             printf("%d %d %d %d %d %d\n", NG_FIELD_V, NG_FIELD_I_SYN, NG_FIELD_REFR, NG_FIELD_RING, NG_FIELD_STEP, NG_FIELD_LAST_INPUT);
-            printf("%d %d %d %d %d %d %d %d %d %d\n", NG_OPT_STEP_MODE, NG_OPT_STEPS_PER_GRAPH, NG_OPT_DELIVERY_KERNEL, NG_OPT_DELIVER_BLOCKS, NG_OPT_PROFILE, NG_OPT_ASYNC, NG_OPT_SORT_SEGMENTS, NG_OPT_PREFETCH, NG_OPT_TRACE, NG_OPT_PERSISTENT_THREADS);
+            printf("%d %d %d %d %d %d %d %d %d %d %d\n", NG_OPT_STEP_MODE, NG_OPT_STEPS_PER_GRAPH, NG_OPT_DELIVERY_KERNEL, NG_OPT_DELIVER_BLOCKS, NG_OPT_PROFILE, NG_OPT_ASYNC, NG_OPT_SORT_SEGMENTS, NG_OPT_PREFETCH, NG_OPT_TRACE, NG_OPT_PERSISTENT_THREADS, NG_OPT_QUEUE_CAPACITY);
             return 0;
         }''')
     import tempfile
@@ -56,7 +56,8 @@ def test_struct_layouts_match_header():
     assert list(map(int, out[2].split())) == [B.NG_OK, B.NG_ERR_INVALID_ARG, B.NG_ERR_STATE, B.NG_ERR_OOM, B.NG_ERR_CUDA, B.NG_ERR_OVERFLOW]
     assert list(map(int, out[3].split())) == [B.FIELD_V, B.FIELD_I_SYN, B.FIELD_REFR, B.FIELD_RING, B.FIELD_STEP, B.FIELD_LAST_INPUT]
     assert list(map(int, out[4].split())) == [B.OPT_STEP_MODE, B.OPT_STEPS_PER_GRAPH, B.OPT_DELIVERY_KERNEL, B.OPT_DELIVER_BLOCKS,
-                                              B.OPT_PROFILE, B.OPT_ASYNC, B.OPT_SORT_SEGMENTS, B.OPT_PREFETCH, B.OPT_TRACE, B.OPT_PERSISTENT_THREADS]
+                                              B.OPT_PROFILE, B.OPT_ASYNC, B.OPT_SORT_SEGMENTS, B.OPT_PREFETCH, B.OPT_TRACE, B.OPT_PERSISTENT_THREADS,
+                                              B.OPT_QUEUE_CAPACITY]
 
 
 def test_argument_validation_without_a_gpu():
@@ -127,3 +128,26 @@ def test_replica_aggregation_world_size_2_gloo(tmp_path):
     out = subprocess.run(cmd, capture_output=True, text=True, timeout=240)
     assert out.returncode == 0, out.stderr[-2000:]
     assert "ok 0" in out.stdout and "ok 1" in out.stdout
+
+
+def test_bench_spawns_its_own_ranks_and_quotes_only_matching_captures(tmp_path, monkeypatch):
+    """`python bench.py --gpus N` outside torchrun re-launches itself as N ranks on 127.0.0.1; roofline.traffic is quoted
+    from the committed ncu capture only while the kernel sources hash to what the capture was taken on."""
+    sys.path.insert(0, ROOT)
+    import bench
+    cmd = bench.spawn_command(["--gpus", "4", "--steps", "2"], 4, port=29777)
+    assert cmd[1:4] == ["-m", "torch.distributed.run", "--nnodes=1"] and "--nproc-per-node=4" in cmd
+    assert cmd[cmd.index("--master-addr") + 1] == "127.0.0.1" and cmd[cmd.index("--master-port") + 1] == "29777"
+    assert cmd[-4:] == ["--gpus", "4", "--steps", "2"] and cmd[-5].endswith("bench.py")
+    h = bench.csrc_hash()
+    f = tmp_path / "t.csv"
+    f.write_text(f"# workload,kernel,dram_bytes_per_launch,time_steps_per_launch,csrc_sha256_16,capture\n"
+                 f"cfg2,persistent_pipe_kernel,9.0e8,1000,{h},profiles/x.csv\n"
+                 f"cfg4,persistent_pipe_kernel,3.6e10,1000,0123456789abcdef,profiles/y.csv\n")
+    monkeypatch.setattr(bench, "TRAFFIC_FILE", str(f))
+    t, note = bench.ncu_traffic("cfg2", "persistent_pipe_kernel")
+    assert t["value"] == 9.0e8 and t["from"] == "profiles/x.csv" and note is None
+    t, note = bench.ncu_traffic("cfg4", "persistent_pipe_kernel")
+    assert t is None and "0123456789abcdef" in note
+    t, note = bench.ncu_traffic("cfg0", "persistent_pipe_kernel")
+    assert t is None and note
