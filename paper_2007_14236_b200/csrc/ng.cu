@@ -231,7 +231,7 @@ void configure_launch(ng_sim* s) {
     {
         int occq = 0;
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occq, queue_deliver_kernel, kQThreads, 0);
-        s->queue_blocks = sm * std::max(1, std::min(occq, 2));
+        s->queue_blocks = sm * std::max(1, std::min(occq, 1024 / kQThreads));
     }
     s->pipe_blocks = grid_for(s->N, kPipeThreads - (s->has_adex ? 128 : kEntryTile), sm * 4);   // updaters per CTA
     {
@@ -821,6 +821,8 @@ int32_t ng_set_state(ng_sim* s, int32_t field, const void* data, int64_t count, 
         h.err_queue = 0;
         NG_CUDA(s, cudaMemcpyAsync(s->d_ctl, &h, sizeof(Ctl), cudaMemcpyHostToDevice, s->stream));
         if (s->a.q_tail) NG_CUDA(s, cudaMemsetAsync(s->a.q_tail, 0, (size_t)s->cfg.ring_slots * kQTailStride * 8, s->stream));
+        // target-sharded mode: forget the step stamps of the exchange (every rank must set the same step while all are idle)
+        if (s->xchg_own) NG_CUDA(s, cudaMemsetAsync(s->xchg_own, 0, kXchgHeaderBytes, s->stream));
         NG_CUDA(s, cudaStreamSynchronize(s->stream));
         return NG_OK;
     }

@@ -9,6 +9,9 @@
 #include <cstdint>
 #include <cuda_runtime.h>
 
+#ifndef NG_GC
+#define NG_GC __grid_constant__     // kernel parameter block addressable without a local copy (noinline callees take it by reference)
+#endif
 namespace ng {
 namespace cg = cooperative_groups;
 
@@ -1119,7 +1122,10 @@ __device__ __forceinline__ void deliver_groups_phase(const StepArgs& a, long lon
 //   N * 4 bytes that stays in L2 whatever D is.  Queue of arrival step a = slot a mod D: during step n the appends write
 //   every slot except (n + 1) mod D, which is the one being drained; its counter is cleared by the update of step n + 1.
 // ---------------------------------------------------------------------------------------
-constexpr int kQThreads = 512;
+#ifndef NG_Q_THREADS
+#define NG_Q_THREADS 256
+#endif
+constexpr int kQThreads = NG_Q_THREADS;                       // threads per CTA; 1024 / kQThreads CTAs per SM
 constexpr int kQVecPerThread = 2;                              // 128-bit vectors (4 records each) per thread and batch
 constexpr int kQBatch = kQThreads * kQVecPerThread * 4;        // records per batch
 constexpr int kQTailStride = 16;                               // one 128-byte line per queue counter
@@ -1208,14 +1214,7 @@ __device__ __forceinline__ void queue_append_phase(const StepArgs& a, long long 
                 }
             }
             __syncthreads();                                   // (A) the histogram of the batch is complete
-            if (threadIdx.x < 256) {                           // one global atomic per (batch, delay), all in flight together
-                const int k = threadIdx.x;
-                const uint32_t h = (k >= 2 && k <= D) ? sh.hist[k] : 0u;
-                if (h > 0u) {
-                    int qs = nmodD + k; if (qs >= D) qs -= D;  // arrival step n + k
-                    sh.gbase[k] = atomicAdd(a.q_tail + (size_t)qs * kQTailStride, (unsigned long long)h);
-                }
-            } else if (wib == 8) {                             // meanwhile one warp prefix-sums the 256 bins, 8 per lane
+            if (wib == kQThreads / 32 - 1) {                   // the last warp prefix-sums the 256 bins, 8 per lane, while ...
                 uint32_t loc[8], sum = 0;
 #pragma unroll
                 for (int j = 0; j < 8; ++j) {
@@ -1232,6 +1231,13 @@ __device__ __forceinline__ void queue_append_phase(const StepArgs& a, long long 
 #pragma unroll
                 for (int j = 0; j < 8; ++j) sh.sbase[lane * 8 + j] = incl - sum + loc[j];
                 if (lane == 31) sh.sbase[256] = incl;          // sbase[D + 1] = records of the batch that go to a queue
+            }
+            for (int k = threadIdx.x; k < 256; k += kQThreads) {   // ... one global atomic per (batch, delay), all in flight together
+                const uint32_t h = (k >= 2 && k <= D) ? sh.hist[k] : 0u;
+                if (h > 0u) {
+                    int qs = nmodD + k; if (qs >= D) qs -= D;  // arrival step n + k
+                    sh.gbase[k] = atomicAdd(a.q_tail + (size_t)qs * kQTailStride, (unsigned long long)h);
+                }
             }
             __syncthreads();                                   // (B) sbase and gbase are known
             if (threadIdx.x < 256) sh.hist[threadIdx.x] = 0;   // for the next batch
@@ -1491,7 +1497,19 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
                 const long long ii = base + threadIdx.x;
                 const int i = (int)ii;
                 NeuronRegs g;
-                if (kAdex) { if (ii < N) L = neuron_load<kAdex>(a, plane, i, have_k); }
+                if (kAdex) {
+                    // the state of the next round (ten words per neuron, one 128-byte line per warp and array) is requested
+                    // now, so that the round after this one finds it in L1 (state: only this SM touches it) / L2 (input cells)
+                    if (lane < 10 && ii - lane + stride < N) {
+                        const long long nx = ii - lane + stride;
+                        const float* arr = lane == 0 ? a.V : lane == 1 ? a.ax_w : lane == 2 ? a.ax_gx : lane == 3 ? a.ax_yx : lane == 4 ? a.ax_gi
+                                           : lane == 5 ? a.ax_yi : lane == 6 ? a.ax_h : lane == 7 ? plane : lane == 8 ? plane + a.N
+                                           : reinterpret_cast<const float*>(a.pop_of) - (nx - nx / 4);   // byte array: element nx / 4 of a float view
+                        if (lane == 7 || lane == 8) asm volatile("prefetch.global.L2 [%0];" ::"l"(arr + nx));
+                        else asm volatile("prefetch.global.L1 [%0];" ::"l"(arr + nx));
+                    }
+                    if (ii < N) L = neuron_load<kAdex>(a, plane, i, have_k);
+                }
                 else if (!kOneRound && !kResM && ii + stride < N) Ln = neuron_load<kAdex>(a, plane, (int)(ii + stride), have_k);   // next round's loads in flight
                 // the row descriptor is fetched for EVERY neuron together with its state (16 B, L2-resident because it
                 // is touched every step): a spiking thread then needs no further memory round trip
@@ -1788,7 +1806,7 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
 // publishes the next step index (a4) and marks the rest pass of this step as pending.
 constexpr int kPipeThreads = 512;        // 256 updaters + 256 rest-pass threads
 template <bool kUpdate, bool kAdex, bool kOneRound = false>
-__global__ void __launch_bounds__(kPipeThreads) pipe_step_kernel(const StepArgs a) {
+__global__ void __launch_bounds__(kPipeThreads) pipe_step_kernel(const NG_GC StepArgs a) {
     __shared__ PipeShared sh;
     if (threadIdx.x == 0) {
         sh.sc.n = __ldcg(&a.ctl->step_u);
@@ -1823,7 +1841,7 @@ __global__ void __launch_bounds__(kPipeThreads) pipe_step_kernel(const StepArgs 
 
 // kAdex: the AdEx integrator needs more than the 64 registers a 1024-thread CTA leaves: 512-thread CTAs, two per SM at most
 template <bool kAdex, bool kOneRound = false, bool kResM = false>
-__global__ void __launch_bounds__(kAdex ? 512 : kPersistentThreads, kAdex ? 2 : 1) persistent_pipe_kernel(const StepArgs a, long long n_steps) {
+__global__ void __launch_bounds__(kAdex ? 512 : kPersistentThreads, kAdex ? 2 : 1) persistent_pipe_kernel(const NG_GC StepArgs a, long long n_steps) {
     __shared__ PipeShared sh;
     if (threadIdx.x == 0) {
         sh.sc.n = __ldcg(&a.ctl->step_u);
@@ -1923,7 +1941,7 @@ __device__ __forceinline__ void window_bookkeeping(const StepArgs& a, long long 
 }
 
 template <bool kAdex>
-__global__ void __launch_bounds__(kUpdateThreads) update_kernel(const StepArgs a) {
+__global__ void __launch_bounds__(kUpdateThreads) update_kernel(const NG_GC StepArgs a) {
     __shared__ PopDev sh_pops[kMaxPopsSmem];
     __shared__ StepScalars sc;
     __shared__ unsigned long long win_base;
@@ -1947,7 +1965,7 @@ __global__ void __launch_bounds__(kUpdateThreads) update_kernel(const StepArgs a
 
 // kKernel 1: row-chunk walk, 2: delay-major segment walk, 4: spike-buffer backend (segment walk over the spike window)
 template <int kKernel>
-__global__ void __launch_bounds__(kDeliverThreads, 3) deliver_kernel(const StepArgs a) {
+__global__ void __launch_bounds__(kDeliverThreads, 3) deliver_kernel(const NG_GC StepArgs a) {
     __shared__ DeliverShared sh;
     __shared__ StepScalars sc;
     __shared__ WindowShared ws;
@@ -2047,7 +2065,7 @@ __global__ void __launch_bounds__(256) xchg_gather_kernel(const StepArgs a) {
 }
 
 // Delivery kernel 5 as a stand-alone launch (one per time step, after update_kernel).
-__global__ void __launch_bounds__(kQThreads, 2) queue_deliver_kernel(const StepArgs a) {
+__global__ void __launch_bounds__(kQThreads, 1024 / kQThreads) queue_deliver_kernel(const NG_GC StepArgs a) {
     __shared__ QueueShared sh;
     __shared__ StepScalars sc;
     if (threadIdx.x == 0) {
@@ -2087,7 +2105,7 @@ __global__ void materialize_queues_kernel(const StepArgs a, long long n, float* 
 // instead of kernel boundaries (the per-step work of the microcircuit is a few microseconds).
 // One CTA per SM keeps the number of barrier arrivals (atomics on one address) at the SM count.
 template <int kKernel>
-__global__ void __launch_bounds__(kPersistentThreads, 1) persistent_kernel(const StepArgs a, long long n_steps) {
+__global__ void __launch_bounds__(kPersistentThreads, 1) persistent_kernel(const NG_GC StepArgs a, long long n_steps) {
     const long long gtid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const long long gthreads = (long long)gridDim.x * blockDim.x;
     __shared__ PopDev sh_pops[kMaxPopsSmem];
