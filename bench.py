@@ -382,7 +382,7 @@ def run_ours(args):
     # ---- roofline of the dominant kernel ----
     if int(s1.step_mode) == 2:
         # one persistent kernel per bench step: its launch IS the timed region (CUDA events on the simulator's stream)
-        kern = {1: "persistent_kernel<1>", 2: "persistent_kernel<2>", 3: "persistent_pipe_kernel", 4: "persistent_kernel<4>"}[int(s1.delivery_kernel)]
+        kern = {1: "persistent_kernel<1>", 2: "persistent_kernel<2>", 3: "persistent_pipe_kernel", 4: "persistent_kernel<4>", 6: "persistent_pipe_kernel"}[int(s1.delivery_kernel)]
         us = ms_total * 1e3 / args.steps
         ev_per_launch = float(s1.events - s0.events) / args.steps
         # AdEx: seven state words and two input ports per neuron instead of three and one
@@ -607,7 +607,7 @@ def main():
     ap.add_argument("--micro-k-only", type=int, default=0, help="restrict --micro-sweep to one out-degree")
     ap.add_argument("--probe", action="store_true", help="run the ceiling probes (ng_probe) and print them as JSON")
     ap.add_argument("--step-mode", type=int, default=3, choices=[0, 1, 2, 3], help="NG_OPT_STEP_MODE (3 = auto)")
-    ap.add_argument("--delivery-kernel", type=int, default=0, choices=[0, 1, 2, 3, 4, 5], help="NG_OPT_DELIVERY_KERNEL (0 = auto)")
+    ap.add_argument("--delivery-kernel", type=int, default=0, choices=[0, 1, 2, 3, 4, 5, 6], help="NG_OPT_DELIVERY_KERNEL (0 = auto)")
     ap.add_argument("--no-prefetch", action="store_true", help="NG_OPT_PREFETCH = 0")
     ap.add_argument("--micro-k", type=int, default=10000)
     ap.add_argument("--micro-fraction", type=float, default=0.05)

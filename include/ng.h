@@ -102,7 +102,11 @@ enum {
                                         queue into the input plane of the next step.  Two planes like kernel 4, same
                                         rules (before ng_prepare, NG_FIELD_RING read-only).  Memory: ring_slots queues
                                         of NG_OPT_QUEUE_CAPACITY events x 8 B; a full queue drops events and
-                                        ng_simulate returns NG_ERR_OVERFLOW                                     */
+                                        ng_simulate returns NG_ERR_OVERFLOW,
+                                    6 = kernel 3's pipelined step with kernel 4's backend: the delay-1 records go out with
+                                        the update, the rest warps walk the spike window (one delay group per buffered
+                                        spike and step) into the ONE input plane of the next step.  Persistent cooperative
+                                        kernel only (step mode 2), one GPU, not in delivery-only mode; rules of kernel 4  */
     NG_OPT_DELIVER_BLOCKS = 3,   /* grid size of the delivery kernel, 0 = auto                         */
     NG_OPT_PROFILE = 4,          /* 1 = time every kernel with CUDA events (forces plain launches);
                                     results in ng_stats.ms_update / ms_deliver                       */
@@ -174,7 +178,7 @@ typedef struct {
     uint64_t launches_update;    /* kernel launches (or graph kernel nodes executed) since create    */
     uint64_t launches_deliver;
     uint64_t launches_other;     /* builder and bookkeeping kernels                                  */
-    int32_t delivery_kernel;     /* the delivery kernel in use (1 .. 5)                           */
+    int32_t delivery_kernel;     /* the delivery kernel in use (1 .. 6)                           */
     int32_t step_mode;
     int64_t n_sources;           /* neurons of the whole network (= n_neurons unless target-sharded)  */
     int32_t shard_rank, shard_world;   /* ng_set_shard (0, 1 on one GPU)                             */

@@ -62,7 +62,8 @@ struct ng_sim {
     size_t resm_bytes = 0;                 // > 0: multi-round LIF network with its state resident in dynamic shared memory (kResM)
     bool has_adex = false;                 // any AdEx population: two receptor ports, AdEx state arrays, <true> kernels
     int64_t NR = 0;                        // ring row length = N * ports
-    bool window_backend = false;           // delivery kernel 4 chosen before ng_prepare: spike window instead of a D-plane ring
+    bool window_backend = false;           // delivery kernel 4 or 6 chosen before ng_prepare: spike window instead of a D-plane ring
+    bool pipewin = false;                  //   6: the window walked by the rest warps of the pipelined persistent kernel
     // target-sharded multi-GPU (ng_set_shard): this handle owns the neurons [id_first, id_first + NL)
     int shard_rank = 0, shard_world = 1; int32_t id_first = 0; int32_t NL = 0;
     unsigned char* xchg_own = nullptr; size_t xchg_bytes = 0; bool xchg_ipc_open[16] = {};
@@ -218,16 +219,17 @@ void configure_launch(ng_sim* s) {
     if (k == 0) k = s->shard_world > 1 ? 1 : 3;                     // a ring beyond L2 was given a two-plane backend in ng_prepare
     if (k == 3 && s->shard_world > 1) k = 1;                        // the pipelined kernel delivers a CTA's own spikes: one GPU only
     (void)mean_group; (void)ring_bytes;
-    if (s->window_backend) k = 4;                                   // fixed at ng_prepare: there is no D-plane ring
+    if (s->window_backend) k = s->pipewin ? 6 : 4;                  // fixed at ng_prepare: there is no D-plane ring
     if (s->queue_backend) k = 5;
     s->delivery_kernel = k;
     // step mode: the latency-bound kernels run as one persistent cooperative kernel per ng_simulate call; the
     // bandwidth-bound delay-major kernel keeps its 8 CTAs per SM and runs from a CUDA graph
     s->step_mode = s->step_mode_opt != 3 ? s->step_mode_opt : (k == 2 || k == 4 || k == 5 || !s->coop_ok) ? 0 : 2;
-    if (s->has_adex && s->step_mode == 2 && k != 3) s->step_mode = 0;   // the two-phase persistent kernels are LIF only
+    if (s->has_adex && s->step_mode == 2 && k != 3 && k != 6) s->step_mode = 0;   // the two-phase persistent kernels are LIF only
+    if (k == 6) s->step_mode = 2;                                       // exists as a persistent cooperative kernel only
     if (k == 5 && s->step_mode == 2) s->step_mode = 0;                  // the event-queue backend runs as update + delivery launches
     if (s->shard_world > 1 && s->step_mode == 2) s->step_mode = 0;      // sharded: update, exchange and delivery are separate launches
-    s->a.prefetch = (k != 2 && k != 4 && k != 5 && s->prefetch_opt) ? 1 : 0;
+    s->a.prefetch = (k != 2 && k != 4 && k != 5 && s->prefetch_opt) ? 1 : 0;      // (kernel 6: the delay-1 head only)
     {
         int occq = 0;
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occq, queue_deliver_kernel, kQThreads, 0);
@@ -258,6 +260,7 @@ void configure_launch(ng_sim* s) {
             int occ2 = 0;
             if (bytes <= 160 * 1024 &&
                 cudaFuncSetAttribute(persistent_pipe_kernel<false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) == cudaSuccess &&
+                cudaFuncSetAttribute(persistent_pipe_kernel<false, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) == cudaSuccess &&
                 cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ2, persistent_pipe_kernel<false, false, true>, pt, bytes) == cudaSuccess &&
                 (long long)occ2 * s->sm_count >= s->persistent_pipe_blocks)
                 s->resm_bytes = bytes;
@@ -569,10 +572,11 @@ int32_t ng_set_option(ng_sim* s, int32_t option, int64_t value) {
             if (value < 1 || value > 10000) return fail(s, NG_ERR_INVALID_ARG, "steps per graph in 1..10000");
             s->steps_per_graph = (int)value; destroy_graph(s); break;
         case NG_OPT_DELIVERY_KERNEL:
-            if (value < 0 || value > 5) return fail(s, NG_ERR_INVALID_ARG, "delivery kernel is 0 .. 5");
+            if (value < 0 || value > 6) return fail(s, NG_ERR_INVALID_ARG, "delivery kernel is 0 .. 6");
+            if (value == 6 && s->shard_world > 1) return fail(s, NG_ERR_INVALID_ARG, "delivery kernel 6 (pipelined) runs on one GPU only");
             if (value == 3 && s->shard_world > 1) return fail(s, NG_ERR_INVALID_ARG, "delivery kernel 3 (pipelined) runs on one GPU only");
-            if (s->prepared && value != 0 && ((value == 4) != s->window_backend || (value == 5) != s->queue_backend))
-                return fail(s, NG_ERR_STATE, "delivery kernels 4 (spike-buffer backend) and 5 (event queues) must be chosen before ng_prepare and cannot be left after it");
+            if (s->prepared && value != 0 && ((value == 4) != (s->window_backend && !s->pipewin) || (value == 5) != s->queue_backend || (value == 6) != s->pipewin))
+                return fail(s, NG_ERR_STATE, "delivery kernels 4, 6 (spike-buffer backends) and 5 (event queues) must be chosen before ng_prepare and cannot be left after it");
             s->delivery_kernel_opt = (int)value; if (s->prepared) configure_launch(s); break;
         case NG_OPT_DELIVER_BLOCKS:
             if (value < 0 || value > (1 << 20)) return fail(s, NG_ERR_INVALID_ARG, "deliver blocks out of range");
@@ -625,6 +629,10 @@ int32_t ng_prepare(ng_sim* s) {
     for (const CallDev& c : s->calls) s->S += (int64_t)(c.rule == kRuleIndegree ? c.tgt_n : c.src_n) * c.K;
     const int64_t S_all = s->S;
     s->S = S_all / s->shard_world;                              // estimate until the build has counted this shard's records
+    s->has_adex = false;
+    for (const HostPop& hp : s->pops) s->has_adex = s->has_adex || hp.dev.model == 1;
+    s->NR = (int64_t)NL * (s->has_adex ? 2 : 1);
+    const double ring_bytes = (double)s->NR * (D + 1) * 4.0;
     const bool beyond_l2 = (double)NL * (D + 1) * 4.0 > 0.8 * (double)s->l2_bytes;
     // Beyond L2, short delay groups (a few records per (source, delay): config 3 at out-degree 100 and 1000) make the
     // spike-buffer walk read at random 12-125-byte granularity; the event queues read a spiking row once, whole
@@ -636,12 +644,18 @@ int32_t ng_prepare(ng_sim* s) {
     size_t mem_free = 0, mem_total = 0;
     cudaMemGetInfo(&mem_free, &mem_total);
     const bool queue_fits = (double)qcap * D * 8.0 + (double)s->S * 9.0 < 0.85 * (double)mem_total;
-    s->queue_backend = s->delivery_kernel_opt == 5 || (s->delivery_kernel_opt == 0 && beyond_l2 && mean_group < 48.0 && queue_fits);
-    s->window_backend = s->delivery_kernel_opt == 4 || (s->delivery_kernel_opt == 0 && beyond_l2 && !s->queue_backend);
+    // A ring of more than half the L2 does not stay resident next to the record stream (config 4: 84 MB; the two-port AdEx
+    // network: 168 MB): the pipelined kernel then walks the spike window into two planes instead (kernel 6; config 4
+    // 20.4 -> 17.7 us per step, AdEx 10^6 92.0 -> 88.5).  Latency-bound networks with a small ring keep kernel 3 (config 2:
+    // 4.6 us against 10.0 with the window walk, which visits a spike once per delay group instead of once).
+    s->pipewin = s->delivery_kernel_opt == 6 ||
+                 (s->delivery_kernel_opt == 0 && s->step_mode_opt >= 2 && s->coop_ok && !s->bypass && D >= 2 && s->shard_world == 1 &&
+                  ring_bytes > 0.5 * (double)s->l2_bytes && mean_group >= 16.0);
+    if (s->pipewin && (!s->coop_ok || s->bypass || D < 2 || s->shard_world > 1))
+        return fail(s, NG_ERR_INVALID_ARG, "delivery kernel 6 needs cooperative launch, a neuron update (no delivery-only mode), ring_slots >= 2 and one GPU");
+    s->queue_backend = s->delivery_kernel_opt == 5 || (s->delivery_kernel_opt == 0 && beyond_l2 && mean_group < 48.0 && queue_fits && !s->pipewin);
+    s->window_backend = s->pipewin || s->delivery_kernel_opt == 4 || (s->delivery_kernel_opt == 0 && beyond_l2 && !s->queue_backend);
     const int planes = (s->window_backend || s->queue_backend) ? 2 : D + 1;               // ring planes actually stored
-    s->has_adex = false;
-    for (const HostPop& hp : s->pops) s->has_adex = s->has_adex || hp.dev.model == 1;
-    s->NR = (int64_t)NL * (s->has_adex ? 2 : 1);
     // Receptor port 1 is the inhibitory conductance of AdEx neurons: it exists only in networks with an AdEx population
     // (two-port ring planes), and only AdEx targets read it — a LIF target would silently drop such input.
     for (const CallDev& c : s->calls) {
@@ -815,7 +829,7 @@ int32_t ng_set_state(ng_sim* s, int32_t field, const void* data, int64_t count, 
         if (rc) return rc;
         const unsigned long long recorded = h.rec_total[h.step_u & 1];
         h.step_u = n; h.step_d = n; h.spike_cnt[0] = h.spike_cnt[1] = h.spike_cnt[2] = h.spike_cnt[3] = 0; h.ticket = 0; h.pending = 0;
-        std::memset(h.win_start, 0, sizeof(h.win_start)); h.err_window = 0;
+        std::memset(h.win_start, 0, sizeof(h.win_start)); h.err_window = 0; h.win_tail = 0;
         h.slot = (int32_t)(n % s->a.Dr);
         h.rec_total[0] = h.rec_total[1] = recorded;
         h.err_queue = 0;
@@ -871,7 +885,7 @@ int32_t ng_simulate(ng_sim* s, int64_t n_steps) {
         for (int q = 0; q < s->shard_world; ++q)
             if (!s->a.xchg[q]) return fail(s, NG_ERR_STATE, "target-sharded mode: ng_exchange_attach every peer before ng_simulate");
     cudaStream_t st = s->stream;
-    if (s->profile) {
+    if (s->profile && s->delivery_kernel != 6) {
         // per-kernel device times: events around every launch, read back in batches
         const int kBatch = 128;
         std::vector<cudaEvent_t> ev(3 * kBatch);
@@ -901,8 +915,18 @@ int32_t ng_simulate(ng_sim* s, int64_t n_steps) {
         long long ns = n_steps;
         void* args[] = {(void*)&s->a, (void*)&ns};
         NG_CUDA(s, cudaMemsetAsync(&s->d_ctl->bar, 0, sizeof(unsigned long long), st));
-        s->last_persistent_blocks = s->delivery_kernel == 3 ? s->persistent_pipe_blocks : s->persistent_blocks;
-        if (s->delivery_kernel == 3) {
+        const bool piped = s->delivery_kernel == 3 || s->delivery_kernel == 6;
+        s->last_persistent_blocks = piped ? s->persistent_pipe_blocks : s->persistent_blocks;
+        if (s->delivery_kernel == 6) {
+            const void* fn = s->has_adex ? (s->one_round_persistent ? (const void*)persistent_pipe_kernel<true, true, false, true>
+                                                                     : (const void*)persistent_pipe_kernel<true, false, false, true>)
+                                         : (s->one_round_persistent && !s->bypass ? (const void*)persistent_pipe_kernel<false, true, false, true>
+                                            : s->resm_bytes ? (const void*)persistent_pipe_kernel<false, false, true, true>
+                                                            : (const void*)persistent_pipe_kernel<false, false, false, true>);
+            NG_CUDA(s, cudaLaunchCooperativeKernel(fn, dim3(s->persistent_pipe_blocks),
+                                                   dim3(s->has_adex ? 512 : s->persistent_threads), args,
+                                                   s->has_adex || s->one_round_persistent ? 0 : s->resm_bytes, st));
+        } else if (s->delivery_kernel == 3) {
             const void* fn = s->has_adex ? (s->one_round_persistent ? (const void*)persistent_pipe_kernel<true, true>
                                                                      : (const void*)persistent_pipe_kernel<true, false>)
                                          : (s->one_round_persistent && !s->bypass ? (const void*)persistent_pipe_kernel<false, true>

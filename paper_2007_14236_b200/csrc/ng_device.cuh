@@ -70,6 +70,7 @@ struct Ctl {
     int32_t err_window;                    // spike-buffer backend: the spike window overflowed its capacity
     uint32_t n_long_groups;                // builder: (source, delay) groups longer than kSortMax, listed for the CTA-wide sort
     int32_t err_queue;                     // event-queue backend: a queue overflowed its capacity (events were dropped)
+    unsigned long long win_tail;           // pipelined spike-buffer backend (kernel 6): next free position of the spike window
     int32_t err_xchg;                      // target-sharded mode: a peer's spike list did not arrive (bounded wait expired)
     unsigned long long n_records;          // builder: records stored on this shard (unpadded)
     // line 1: spike counters (atomics of the appending warps / CTAs)
@@ -1022,7 +1023,8 @@ __device__ __forceinline__ void red_vec(const StepArgs& a, const VecRef& r, cons
 // `off` (shared memory) holds the W + 1 window offsets of steps n-W+1 .. n and the end.
 template <bool kWindow>
 __device__ __forceinline__ void deliver_groups_phase(const StepArgs& a, long long n, int nmod, int M, long long gwarp,
-                                                     long long gwarps, int lane, const unsigned long long* off = nullptr, int W = 0) {
+                                                     long long gwarps, int lane, const unsigned long long* off = nullptr, int W = 0,
+                                                     int age0 = 0) {
     const int N = a.NS, D = a.D, Dr = a.Dr;
     const int32_t* __restrict__ list = a.spike_list + (size_t)(n & 1) * N;
     const long long items = kWindow ? (long long)(off[W] - off[0]) : (long long)M * D;
@@ -1043,7 +1045,8 @@ __device__ __forceinline__ void deliver_groups_phase(const StepArgs& a, long lon
             const unsigned long long pos = off[0] + (unsigned long long)it;
             int lo = 0, hi = W;                                          // largest k with off[k] <= pos
             while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (off[mid] <= pos) lo = mid; else hi = mid; }
-            d = W - 1 - lo;                                              // 0-based delay index: age of the spike
+            d = W - 1 - lo + age0;                                       // 0-based delay index: age of the spike (the newest
+                                                                             // staged step has age age0: 0 = the step just updated)
             si = (int)(pos % (unsigned long long)a.win_cap);
         } else if (small) { d = (int)((uint32_t)it / (uint32_t)M); si = (int)((uint32_t)it - (uint32_t)d * (uint32_t)M); }
         else { d = (int)(it / M); si = (int)(it - (long long)d * M); }
@@ -1062,7 +1065,7 @@ __device__ __forceinline__ void deliver_groups_phase(const StepArgs& a, long lon
             const uint32_t* __restrict__ g = a.grp_rel + (size_t)j * (D + 1);
             ga = g[d]; gb = g[d + 1];
             r0 = a.row_off[j];
-            if (d == 0) ev += g[D];
+            if (d == age0) ev += g[D];                               // first visit of this spike: count its out-degree once
         }
     };
     long long b = gwarp;
@@ -1386,6 +1389,10 @@ struct PipeShared {
     int32_t n_d1;
     StepScalars sc;
     int32_t pending;
+    // pipelined spike-buffer backend (kernel 6): absolute window position of the first spike of step s at [s mod (D+1)]
+    // for the last D+1 steps, and the staged offsets of the steps whose groups are due in this phase
+    unsigned long long wstart[256];
+    unsigned long long woff[256];
 };
 
 __device__ __forceinline__ void deliver_d1_piece(const StepArgs& a, float* __restrict__ plane1, long long r0, int cnt, int q) {
@@ -1466,10 +1473,15 @@ __device__ __forceinline__ int pipe_updater_threads(int N, bool heavy_update) {
 struct ResM { float* V; float* I; int32_t* r; uint8_t* pi; int rounds; };
 constexpr int kResMRest = 256;           // rest-group threads of the kResM kernel
 
-template <bool kUpdate, bool kAdex, bool kOneRound = false, bool kRes = false, bool kResM = false>
+// kWin (delivery kernel 6, the pipelined spike-buffer backend): two input planes instead of the D + 1 of the ring.  The
+// delay-1 pass is unchanged; the rest pass is replaced by the walk over the spike window of the paper's mechanism
+// (as in kernel 4): in phase n the rest warps deliver, for every spike of the steps n - D + 1 .. n - 1, the
+// connection group whose delay is the spike's age + 1 — everything that arrives in step n + 1 — into the ONE plane of step
+// n + 1, which stays in L2 whatever D and the number of receptor ports are.  `wslot` = n mod (D + 1).
+template <bool kUpdate, bool kAdex, bool kOneRound = false, bool kRes = false, bool kResM = false, bool kWin = false>
 __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* __restrict__ P, long long n, int slot, bool pending,
                                                unsigned long long rec_prev, PipeShared& sh, int U, bool have_k = false,
-                                               const ResM rm = ResM{}) {
+                                               const ResM rm = ResM{}, int wslot = 0) {
     const int N = a.N, Dr = a.Dr;
     const int lane = threadIdx.x & 31;
     // U = pipe_updater_threads(N, kAdex), computed once per launch by the caller: its integer division in front of every
@@ -1573,10 +1585,11 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
                         if (k < kD1Cap) { sh.d1_r0[k] = r.r0; sh.d1_cnt[k] = r.d1; sh.d1_deg[k] = r.deg; sh.d1_id[k] = i; }
                         else {                                     // CTA list full: this lane does everything alone
                             for (int q = 0; q < r.d1; ++q) deliver_d1_piece(a, plane1, r.r0, r.d1, q);
-                            if (a.prefetch) prefetch_row(a, r);
+                            if (a.prefetch && !kWin) prefetch_row(a, r);
                             const size_t gk = (size_t)(n & 1) * N + atomicAdd(&a.ctl->spike_cnt[n & 3], 1);
                             a.spike_list[gk] = i;
                             st_row_info(a.spike_row + gk, r);
+                            if (kWin) a.win_id[atomicAdd(&a.ctl->win_tail, 1ULL) % (unsigned long long)a.win_cap] = i;
                         }
                     }
                 }
@@ -1600,10 +1613,11 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
                         if (k < kD1Cap) { sh.d1_r0[k] = r.r0; sh.d1_cnt[k] = r.d1; sh.d1_deg[k] = r.deg; sh.d1_id[k] = i; }
                         else {
                             for (int q = 0; q < r.d1; ++q) deliver_d1_piece(a, plane1, r.r0, r.d1, q);
-                            if (a.prefetch) prefetch_row(a, r);
+                            if (a.prefetch && !kWin) prefetch_row(a, r);
                             const size_t gk = (size_t)(n & 1) * N + atomicAdd(&a.ctl->spike_cnt[n & 3], 1);
                             a.spike_list[gk] = i;
                             st_row_info(a.spike_row + gk, r);
+                            if (kWin) a.win_id[atomicAdd(&a.ctl->win_tail, 1ULL) % (unsigned long long)a.win_cap] = i;
                         }
                     }
                 }
@@ -1619,10 +1633,14 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
             // The same warp later writes the CTA's entries of the global spike array: no barrier, nothing after the reds
             // on the warps that deliver.
             int gb = 0;
-            if ((int)threadIdx.x == U - 1 && nd1 > 0) gb = atomicAdd(&a.ctl->spike_cnt[n & 3], nd1);
+            unsigned long long wp = 0;                             // kWin: the CTA's range in the spike window
+            if ((int)threadIdx.x == U - 1 && nd1 > 0) {
+                gb = atomicAdd(&a.ctl->spike_cnt[n & 3], nd1);
+                if (kWin) wp = atomicAdd(&a.ctl->win_tail, (unsigned long long)nd1);
+            }
             // the rest of the spiking rows is read one phase later: request it now, from the LAST updater threads, so
             // that issuing the bulk prefetches overlaps the delay-1 pass of the first warps instead of following it
-            if (a.prefetch)
+            if (a.prefetch && !kWin)                                // (window form: the groups are read one per step over D steps)
                 for (int s = U - 1 - (int)threadIdx.x; s < nd1; s += U) {
                     RowInfo r; r.r0 = sh.d1_r0[s]; r.d1 = sh.d1_cnt[s]; r.deg = sh.d1_deg[s];
                     prefetch_row(a, r);
@@ -1670,14 +1688,47 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
             trace_stamp(a, n, 6);
             if (nd1 > 0 && (int)threadIdx.x >= U - 32) {           // the last updater warp (U is a multiple of 32)
                 gb = __shfl_sync(0xffffffffu, gb, 31);
+                if (kWin) wp = __shfl_sync(0xffffffffu, wp, 31);
                 for (int s = lane; s < nd1; s += 32) {             // a2: global spike array; the rest of the row is read
                     RowInfo r; r.r0 = sh.d1_r0[s]; r.d1 = sh.d1_cnt[s]; r.deg = sh.d1_deg[s];       // one phase later
                     const size_t gk = (size_t)(n & 1) * N + gb + s;
                     a.spike_list[gk] = sh.d1_id[s];
                     st_row_info(a.spike_row + gk, r);
+                    if (kWin) a.win_id[(wp + (unsigned long long)s) % (unsigned long long)a.win_cap] = sh.d1_id[s];
                 }
             }
         }
+    } else if (kWin) {
+        // ---- window pass: the groups of the spikes of steps n-W .. n-1 that arrive in step n+1 (delay = age + 1 >= 2) ----
+        const int t = threadIdx.x - U, wir = t >> 5, wpr = R >> 5, D = a.D, Dp = D + 1;
+        const long long np = n - 1;
+        if (t == 0) {
+            int M = 0;
+            if (pending) {                                         // M_{n-1} is final since the barrier: W_n = W_{n-1} + M_{n-1}
+                M = __ldcg(&a.ctl->spike_cnt[np & 3]);
+                sh.wstart[wslot] = sh.wstart[wslot == 0 ? D : wslot - 1] + (unsigned long long)M;
+            }
+            sh.d.M = M;
+        }
+        group_sync(2, R);
+        trace_stamp(a, n, 7, U);
+        const int M = sh.d.M;
+        const int W = (int)(n < (long long)(D - 1) ? n : (long long)(D - 1));
+        for (int k = t; k <= W; k += R) { int q = wslot - W + k; if (q < 0) q += Dp; sh.woff[k] = sh.wstart[q]; }
+        group_sync(2, R);
+        trace_stamp(a, n, 8, U);
+        if (blockIdx.x == 0) {
+            if (a.rec_cap > 0 && pending) {                        // spike record of step n-1 (coalesced, off the critical path)
+                const int32_t* __restrict__ list_prev = a.spike_list + (size_t)(np & 1) * N;
+                for (int i = t; i < M; i += R) {
+                    const unsigned long long pos = rec_prev + (unsigned long long)i;
+                    if (pos < (unsigned long long)a.rec_cap) { a.rec_id[pos] = __ldcg(list_prev + i); a.rec_step[pos] = (int32_t)np; }
+                }
+            }
+            if (t == 0 && sh.woff[W] - sh.woff[0] > (unsigned long long)a.win_cap) a.ctl->err_window = 1;
+        }
+        deliver_groups_phase<true>(a, n, slot, M, (long long)blockIdx.x * wpr + wir, (long long)gridDim.x * wpr, lane, sh.woff, W, 1);
+        trace_stamp(a, n, 9, U);
     } else if (pending) {
         // ---- rest pass of step n-1: records [d1, deg) of every spike ----
         const int t = threadIdx.x - U;                             // index inside the rest group
@@ -1840,14 +1891,17 @@ __global__ void __launch_bounds__(kPipeThreads) pipe_step_kernel(const NG_GC Ste
 }
 
 // kAdex: the AdEx integrator needs more than the 64 registers a 1024-thread CTA leaves: 512-thread CTAs, two per SM at most
-template <bool kAdex, bool kOneRound = false, bool kResM = false>
+template <bool kAdex, bool kOneRound = false, bool kResM = false, bool kWin = false>
 __global__ void __launch_bounds__(kAdex ? 512 : kPersistentThreads, kAdex ? 2 : 1) persistent_pipe_kernel(const NG_GC StepArgs a, long long n_steps) {
     __shared__ PipeShared sh;
     if (threadIdx.x == 0) {
         sh.sc.n = __ldcg(&a.ctl->step_u);
         sh.sc.slot = __ldcg(&a.ctl->slot);
         sh.sc.rec_base = __ldcg(&a.ctl->rec_total[sh.sc.n & 1]);
+        sh.sc.M = kWin ? (int)(sh.sc.n % (a.D + 1)) : 0;           // kWin: window slot of the first step of this launch
     }
+    if (kWin)                                                      // window starts of the last D + 1 steps (Ctl.win_start, [s mod (D+1)])
+        for (int k = threadIdx.x; k <= a.D; k += blockDim.x) sh.wstart[k] = __ldcg(&a.ctl->win_start[k]);
     const PopDev* P = stage_pops(a, sh.pops);
     if (a.n_pops > kMaxPopsSmem) __syncthreads();
     const long long gtid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -1877,10 +1931,11 @@ __global__ void __launch_bounds__(kAdex ? 512 : kPersistentThreads, kAdex ? 2 : 
     long long n = sh.sc.n;
     int slot = sh.sc.slot;
     unsigned long long rec_prev = sh.sc.rec_base, spikes = 0, epoch = 0;       // recorded before step n-1 (nothing pending at entry)
+    int wslot = sh.sc.M;
     for (long long s = 0; s < n_steps; ++s, ++n) {
         if (gtid == 0) a.ctl->spike_cnt[(n + 1) & 3] = 0;          // last read (as step n-3's) in phase n-2
         trace_stamp(a, n, 0);
-        const int Mp = pipelined_phase<true, kAdex, kOneRound, kRes, kResM>(a, P, n, slot, s > 0, rec_prev, sh, U, s > 0 && single_round, rm);
+        const int Mp = pipelined_phase<true, kAdex, kOneRound, kRes, kResM, kWin>(a, P, n, slot, s > 0, rec_prev, sh, U, s > 0 && single_round, rm, wslot);
         rec_prev += (unsigned long long)Mp; spikes += (unsigned long long)Mp;
         trace_stamp(a, n, 1);
         grid_arrive(a.ctl, epoch);
@@ -1895,6 +1950,7 @@ __global__ void __launch_bounds__(kAdex ? 512 : kPersistentThreads, kAdex ? 2 : 
         grid_wait(a.ctl, epoch);
         trace_stamp(a, n, 2);
         slot = slot + 1 == a.Dr ? 0 : slot + 1;
+        if (kWin) wslot = wslot == a.D ? 0 : wslot + 1;
     }
     if (kRes && (int)threadIdx.x < U && res_i < a.N) {
         const int t = threadIdx.x;
@@ -1905,7 +1961,29 @@ __global__ void __launch_bounds__(kAdex ? 512 : kPersistentThreads, kAdex ? 2 : 
             const long long ii = ((long long)q * gridDim.x + blockIdx.x) * U + threadIdx.x;
             if (ii < a.N) { const int k = q * U + threadIdx.x; a.V[ii] = rm.V[k]; a.I[ii] = rm.I[k]; a.refr[ii] = rm.r[k]; }
         }
-    if (n_steps > 0) {                                             // flush: rest pass of the last step
+    if (kWin) {
+        // nothing to flush: what is still due lives in the spike window and the plane of step n is complete.  Close the
+        // bookkeeping of the last step (its count, its window start, its part of the spike record) for the next call.
+        if (n_steps > 0) {
+            __syncthreads();
+            if (threadIdx.x == 0) sh.d.M = __ldcg(&a.ctl->spike_cnt[(n - 1) & 3]);
+            __syncthreads();
+            const int Ml = sh.d.M;
+            if (blockIdx.x == 0) {
+                if (threadIdx.x == 0) sh.wstart[wslot] = sh.wstart[wslot == 0 ? a.D : wslot - 1] + (unsigned long long)Ml;
+                __syncthreads();
+                for (int k = threadIdx.x; k <= a.D; k += blockDim.x) a.ctl->win_start[k] = sh.wstart[k];
+                if (a.rec_cap > 0) {
+                    const int32_t* __restrict__ list_prev = a.spike_list + (size_t)((n - 1) & 1) * a.NS;
+                    for (int i = threadIdx.x; i < Ml; i += blockDim.x) {
+                        const unsigned long long pos = rec_prev + (unsigned long long)i;
+                        if (pos < (unsigned long long)a.rec_cap) { a.rec_id[pos] = __ldcg(list_prev + i); a.rec_step[pos] = (int32_t)(n - 1); }
+                    }
+                }
+            }
+            rec_prev += (unsigned long long)Ml; spikes += (unsigned long long)Ml;
+        }
+    } else if (n_steps > 0) {                                      // flush: rest pass of the last step
         const int Mp = pipelined_phase<false, kAdex>(a, P, n, slot, true, rec_prev, sh, U);
         rec_prev += (unsigned long long)Mp; spikes += (unsigned long long)Mp;
     }

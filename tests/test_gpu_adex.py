@@ -55,7 +55,7 @@ def structure_with_ports(g, o, N):
     return src[keep][go], port[go]
 
 
-@pytest.mark.parametrize("mode,kernel", [(2, 3), (0, 3), (0, 1), (0, 4), (0, 5)])
+@pytest.mark.parametrize("mode,kernel", [(2, 3), (0, 3), (0, 1), (0, 4), (0, 5), (2, 6)])
 def test_adex_lockstep(oracle_mod, B, mode, kernel):
     wl = W.balanced_adex(n=2000, k_total=100, n_steps=400, seed=3)
     o, g = make_adex_pair(wl, oracle_mod, B, pre_options={B.OPT_DELIVERY_KERNEL: kernel, B.OPT_STEP_MODE: mode})

@@ -60,7 +60,7 @@ def lockstep(o, g, wl, oracle_mod, B, n_steps, check_input=True):
             try:
                 g.set_state(B.FIELD_RING, o.get_state(oracle_mod.FIELD_RING).astype(np.float32))
             except B.NgError:                                            # spike-buffer backend: no ring to re-feed; stop here
-                assert g.stats().delivery_kernel in (4, 5)
+                assert g.stats().delivery_kernel in (4, 5, 6)
                 break
     return log, n_spk
 
@@ -83,10 +83,10 @@ def test_cfg0_structure_bit_exact(oracle_mod, B):
     g.close()
 
 
-@pytest.mark.parametrize("mode,kernel", [(0, 3), (1, 3), (2, 3), (0, 1), (2, 1), (1, 2)])
+@pytest.mark.parametrize("mode,kernel", [(0, 3), (1, 3), (2, 3), (0, 1), (2, 1), (1, 2), (2, 6)])
 def test_cfg0_lockstep_1000_steps(oracle_mod, B, mode, kernel):
     wl = W.brunel_tiny()
-    o, g = make_pair(wl, oracle_mod)
+    o, g = make_pair(wl, oracle_mod, pre_options={B.OPT_DELIVERY_KERNEL: kernel} if kernel >= 4 else None)
     g.set_option(B.OPT_STEP_MODE, mode)
     g.set_option(B.OPT_DELIVERY_KERNEL, kernel)
     log, n_spk = lockstep(o, g, wl, oracle_mod, B, 1000)
@@ -97,7 +97,7 @@ def test_cfg0_lockstep_1000_steps(oracle_mod, B, mode, kernel):
     g.close()
 
 
-@pytest.mark.parametrize("mode,kernel", [(0, 1), (0, 2), (2, 1), (2, 2), (1, 1), (0, 3), (1, 3), (2, 3), (0, 4), (1, 4), (2, 4), (0, 5), (1, 5)])
+@pytest.mark.parametrize("mode,kernel", [(0, 1), (0, 2), (2, 1), (2, 2), (1, 1), (0, 3), (1, 3), (2, 3), (0, 4), (1, 4), (2, 4), (0, 5), (1, 5), (2, 6)])
 def test_cfg0_free_running_spikes_and_rates(oracle_mod, B, mode, kernel):
     """Free run.  The first steps must agree spike for spike; afterwards rates per population (C17)."""
     wl = W.brunel_tiny(n_steps=20000)
@@ -122,7 +122,7 @@ def test_cfg0_free_running_spikes_and_rates(oracle_mod, B, mode, kernel):
     g.close()
 
 
-@pytest.mark.parametrize("mode,kernel", [(2, 3), (2, 1), (0, 3)])
+@pytest.mark.parametrize("mode,kernel", [(2, 3), (2, 1), (0, 3), (2, 6)])
 def test_cfg0_launch_boundaries_are_invisible(B, mode, kernel):
     """The persistent pipelined kernel keeps the LIF state in shared memory for a whole launch and writes it back at
     exit: one call of 240 steps and the same steps cut into calls of 1, 7, 32 and 200 — with a state read-back and a
@@ -132,7 +132,10 @@ def test_cfg0_launch_boundaries_are_invisible(B, mode, kernel):
 
     def run(chunks, roundtrip):
         g = B.Sim(0.1, wl.ring_slots, wl.seed, record_spikes=True)
-        wl.apply(g); g.prepare(); g.set_state(B.FIELD_V, wl.initial_v())
+        wl.apply(g)
+        if kernel >= 4:
+            g.set_option(B.OPT_DELIVERY_KERNEL, kernel)
+        g.prepare(); g.set_state(B.FIELD_V, wl.initial_v())
         g.set_option(B.OPT_STEP_MODE, mode); g.set_option(B.OPT_DELIVERY_KERNEL, kernel)
         for c in chunks:
             g.simulate(c)
@@ -154,14 +157,16 @@ def test_cfg0_launch_boundaries_are_invisible(B, mode, kernel):
     assert np.mean(a[3] == b[3]) >= 0.99
 
 
-def test_multi_round_resident_state(oracle_mod, B):
+@pytest.mark.parametrize("kernel", [0, 6])
+def test_multi_round_resident_state(oracle_mod, B, kernel):
     """A network that needs several rounds of updater threads per step (config 4's shape; here 200,000 neurons = two
     rounds on 148 CTAs, the second one ragged) keeps its LIF state in dynamic shared memory for a whole persistent launch
     (kResM).  (a) The first steps agree with the oracle spike for spike — step 0 carries the initial volley of ~4e4
     spikes; (b) launch boundaries, with a state round trip in between, are invisible."""
     wl = W.balanced_large(n=200_000, k_total=50, n_steps=60)
-    o, g = make_pair(wl, oracle_mod, debug_input=False)
-    assert g.stats is not None
+    pre = {B.OPT_DELIVERY_KERNEL: kernel} if kernel else None
+    o, g = make_pair(wl, oracle_mod, debug_input=False, pre_options=pre)
+    assert g.stats().delivery_kernel == (kernel or 3) and g.stats().step_mode == B.STEP_PERSISTENT
     g.simulate(30); o.simulate(30)
     gs, gi = g.get_spikes()
     os_, oi = o.get_spikes()
@@ -176,7 +181,10 @@ def test_multi_round_resident_state(oracle_mod, B):
 
     def run(chunks, roundtrip):
         g = B.Sim(0.1, wl.ring_slots, wl.seed, record_spikes=True)
-        wl.apply(g); g.prepare(); g.set_state(B.FIELD_V, wl.initial_v())
+        wl.apply(g)
+        if kernel:
+            g.set_option(B.OPT_DELIVERY_KERNEL, kernel)
+        g.prepare(); g.set_state(B.FIELD_V, wl.initial_v())
         for c in chunks:
             g.simulate(c)
             if roundtrip:
@@ -228,7 +236,7 @@ def test_long_delay_groups_are_sorted_deterministically(oracle_mod, B):
 # ------------------------------------------------------------------------------------------------------------
 # microcircuit-shaped nets (normal weights and delays, 8 populations, up to 54 connect calls)
 # ------------------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("kernel", [0, 4, 5])
+@pytest.mark.parametrize("kernel", [0, 4, 5, 6])
 def test_microcircuit_small_structure_and_lockstep(oracle_mod, B, kernel):
     wl = W.microcircuit(scale_div=40, n_steps=300, indegree_div=8)
     o, g = make_pair(wl, oracle_mod, pre_options={B.OPT_DELIVERY_KERNEL: kernel})

@@ -6,7 +6,7 @@ The oracle needs ~12 minutes for 11 s of the full-scale microcircuit and ~20 min
 so its spike counts per population and per 100 ms window are stored (tests/golden/oracle_rates_cfg2.txt / _cfg4.txt,
 written by tests/golden/make_oracle_rates.py from oracle/ alone; tests/test_oracle_golden.py regenerates prefixes).
 The GPU runs the same seeded network in the default launch configuration (one persistent cooperative kernel per
-ng_simulate call, pipelined delivery kernel 3 — what bench.py times).
+ng_simulate call, pipelined delivery kernel 3 at config 2 and its two-plane form, kernel 6, at config 4 — what bench.py times).
 
   * window 0 (it holds the initial volley: both sides start from the same fp32 V) within 3 % per population;
   * per population, the rate over the analysis interval within max(5 %, 0.1 Hz) of the oracle's (reading C17);
@@ -107,7 +107,7 @@ def test_cfg4_free_running_rates_1s(B):
     wl.apply(g); g.prepare()
     g.set_state(B.FIELD_V, wl.initial_v())
     st = g.stats()
-    assert st.n_connections == 10**9 and st.step_mode == B.STEP_PERSISTENT and st.delivery_kernel == 3
+    assert st.n_connections == 10**9 and st.step_mode == B.STEP_PERSISTENT and st.delivery_kernel == 6      # 84 MB ring: kernel 6
     counts, steps, ids = gpu_window_counts(g, wl, 10, ws, chunk_windows=5)         # 2 launches of 5,000 steps
     assert g.get_state(B.FIELD_STEP) == 10_000 and g.stats().spikes == steps.size
     assert np.all(np.abs(counts[0] - ocounts[0]) <= np.maximum(3, 0.03 * ocounts[0])), (counts[0], ocounts[0])

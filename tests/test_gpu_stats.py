@@ -16,7 +16,7 @@ def B():
     return binding
 
 
-@pytest.mark.parametrize("mode,kernel", [(3, 0), (0, 3), (0, 1), (2, 1), (0, 4), (0, 5)])
+@pytest.mark.parametrize("mode,kernel", [(3, 0), (0, 3), (0, 1), (2, 1), (0, 4), (0, 5), (2, 6)])
 def test_statistics_match_the_spike_record(B, mode, kernel):
     wl = W.microcircuit(scale_div=20, n_steps=6000, indegree_div=2)
     N = wl.n_neurons
