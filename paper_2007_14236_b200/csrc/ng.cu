@@ -235,7 +235,7 @@ void configure_launch(ng_sim* s) {
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occq, queue_deliver_kernel, kQThreads, 0);
         s->queue_blocks = sm * std::max(1, std::min(occq, 1024 / kQThreads));
     }
-    s->pipe_blocks = grid_for(s->N, kPipeThreads - (s->has_adex ? 128 : kEntryTile), sm * 4);   // updaters per CTA
+    s->pipe_blocks = grid_for(s->N, kPipeThreads - (s->has_adex ? kAdexRest : kEntryTile), sm * 4);   // updaters per CTA
     {
         int occp = 0;
         const int pt = s->has_adex ? 512 : s->persistent_threads;      // AdEx kernels are compiled for 512-thread CTAs
@@ -244,12 +244,12 @@ void configure_launch(ng_sim* s) {
         if (occp < 1) occp = 1;
         s->persistent_pipe_blocks = sm * std::min(occp, kPersistentThreads / pt);
         // updater threads per CTA of the AdEx kernels: all but four warps (pipe_updater_threads in ng_device.cuh)
-        s->one_round_persistent = (long long)s->persistent_pipe_blocks * (pt - (s->has_adex ? 128 : (pt >= 512 ? kEntryTile : 64))) >= s->N;
+        s->one_round_persistent = (long long)s->persistent_pipe_blocks * (pt - (s->has_adex ? kAdexRest : (pt >= 512 ? kEntryTile : 64))) >= s->N;
         // AdEx: the two-pass update (one integration attempt per lane, the unfinished neurons — on the exponential
         // upswing, up to thirty sub-steps — finished by dense warps from a CTA list) pays for any number of rounds:
         // 10^6 neurons 116 -> 105 us per step (profiles/r02_adex1m.md)
         if (s->has_adex) s->one_round_persistent = true;
-        s->one_round_step = (long long)s->pipe_blocks * (kPipeThreads - (s->has_adex ? 128 : kEntryTile)) >= s->N;
+        s->one_round_step = (long long)s->pipe_blocks * (kPipeThreads - (s->has_adex ? kAdexRest : kEntryTile)) >= s->N;
         // several rounds per step (config 4): keep V, I_syn, refr and the population byte (13 B per neuron) of the CTA's
         // neurons in dynamic shared memory for the whole launch if that fits beside the static 45 KB
         s->resm_bytes = 0;

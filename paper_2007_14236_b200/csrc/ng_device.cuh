@@ -617,7 +617,7 @@ __device__ __forceinline__ int poisson_count(const StepArgs& a, const PopDev* __
     const int nT = p->n_T;
     if (nT > 0) {
         const uint4 x = philox4x32_10(a.seed_lo, a.seed_hi, (uint32_t)i, (uint32_t)n, (uint32_t)(n >> 32), kTagPoisson);
-        while (k < nT && x.x >= p->T[k]) ++k;
+while (k < nT && x.x >= p->T[k]) ++k;
     }
     return k;
 }
@@ -1363,6 +1363,10 @@ constexpr int kPersistentThreads = 1024;
 //   writes plane n+1, the rest pass of step n-1 writes planes n+1 .. n-1+D (Dr = D + 1 planes).
 //   The spike record of step n-1 is written by CTA 0 during the rest pass (coalesced, off the critical path).
 // ---------------------------------------------------------------------------------------
+#ifndef NG_ADEX_REST
+#define NG_ADEX_REST 64
+#endif
+constexpr int kAdexRest = NG_ADEX_REST;   // rest-group threads of the AdEx kernels (the integrator is the step: most warps update)
 constexpr int kD1Cap = 256;
 constexpr int kResCap = 768;             // updater threads of a 1024-thread CTA at most (pipe_updater_threads)
 constexpr int kSlowCap = 512;
@@ -1455,7 +1459,7 @@ __device__ __forceinline__ void pipe_one_item(const StepArgs& a, int nmod, PipeS
 __device__ __forceinline__ int pipe_updater_threads(int N, bool heavy_update) {
     const unsigned per_cta = ((unsigned)N + gridDim.x - 1u) / gridDim.x;          // 32-bit: no 64-bit division on the step path
     const int need = (int)((per_cta + 31u) & ~31u);
-    const int cap = (int)blockDim.x - (blockDim.x < 512 ? 64 : heavy_update ? 128 : kEntryTile);
+    const int cap = (int)blockDim.x - (blockDim.x < 512 ? 64 : heavy_update ? kAdexRest : kEntryTile);
     return (int)per_cta <= cap ? max(need, 32) : cap;
 }
 
@@ -1471,7 +1475,10 @@ __device__ __forceinline__ int pipe_updater_threads(int N, bool heavy_update) {
 // then read shared memory only; what is left per neuron and step is the input cell (one 4-byte load, four rounds in
 // flight, and the store that clears it), issued after the delay-1 records of the CTA's spikes are on their way.
 struct ResM { float* V; float* I; int32_t* r; uint8_t* pi; int rounds; };
-constexpr int kResMRest = 256;           // rest-group threads of the kResM kernel
+#ifndef NG_RESM_REST
+#define NG_RESM_REST 256
+#endif
+constexpr int kResMRest = NG_RESM_REST;           // rest-group threads of the kResM kernel
 
 // kWin (delivery kernel 6, the pipelined spike-buffer backend): two input planes instead of the D + 1 of the ring.  The
 // delay-1 pass is unchanged; the rest pass is replaced by the walk over the spike window of the paper's mechanism
