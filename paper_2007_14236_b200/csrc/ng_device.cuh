@@ -617,7 +617,7 @@ __device__ __forceinline__ int poisson_count(const StepArgs& a, const PopDev* __
     const int nT = p->n_T;
     if (nT > 0) {
         const uint4 x = philox4x32_10(a.seed_lo, a.seed_hi, (uint32_t)i, (uint32_t)n, (uint32_t)(n >> 32), kTagPoisson);
-while (k < nT && x.x >= p->T[k]) ++k;
+        while (k < nT && x.x >= p->T[k]) ++k;
     }
     return k;
 }
