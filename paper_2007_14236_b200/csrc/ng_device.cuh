@@ -1566,7 +1566,7 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
                         rm.V[q_idx] = V; rm.r[q_idx] = rf;
                     }
                 } else {
-                if (single_round && ii < N) r = ld_row_info(a.row_info + i);
+                if (single_round && !kAdex && ii < N) r = ld_row_info(a.row_info + i);     // (AdEx: four registers live across the integrator)
                 spk = ii < N && neuron_early<kAdex, kAdex && kOneRound>(a, P, n, i, g, L);
                 }
                 if (kAdex && kOneRound && ii < N && g.pending) {            // first attempt did not finish: second pass, dense warps
@@ -1574,7 +1574,7 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
                     if (ks < kSlowCap) { sh.slow_id[ks] = i | (g.spiked ? (1 << 30) : 0); sh.slow_t[ks] = g.t; }
                     else { spk = adex_resume(a, P, n, i, g.t, g.spiked, plane); g.pending = false; g.adex = false; g.pi = -1; }
                 }
-                if (!single_round && spk) r = ld_row_info(a.row_info + i);
+                if ((!single_round || kAdex) && spk) r = ld_row_info(a.row_info + i);
                 const unsigned m = __ballot_sync(0xffffffffu, spk);
                 if (m) {                                           // warp-aggregated append to the CTA's own list
                     const int leader = __ffs(m) - 1;
