@@ -109,3 +109,37 @@ def test_trace_option_can_be_switched_off_and_on(B):
         g.set_option(B.OPT_TRACE, 0)
         g.simulate(10)
     g.close()
+
+
+def test_pipelined_window_backend_rules(B):
+    """Delivery kernel 6 exists as a persistent cooperative kernel with a neuron update: not in delivery-only mode, not
+    with ring_slots = 1, not sharded, and — like kernels 4 and 5 — only when chosen before ng_prepare."""
+    wl = W.delivery_microbench(n=5000, K=50, fraction=0.05, n_steps=10, seed=2)
+    g = B.Sim(0.1, wl.ring_slots, wl.seed)
+    wl.apply(g); g.set_option(B.OPT_DELIVERY_KERNEL, 6)
+    assert code(B, g.prepare) == B.NG_ERR_INVALID_ARG                                   # delivery-only mode
+    g.close()
+    g = B.Sim(0.1, 1, 1)
+    g.create_population(100, W.LIF | dict(poisson_rate_hz=800.0, poisson_weight=87.8))
+    g.connect_fixed_indegree(0, 100, 0, 100, 5, ("const", 50.0), ("const", 1))
+    g.set_option(B.OPT_DELIVERY_KERNEL, 6)
+    assert code(B, g.prepare) == B.NG_ERR_INVALID_ARG                                   # one ring slot: no delay >= 2 exists
+    g.close()
+    g = B.Sim(0.1, 20, 1, rank=0, world=2)
+    assert code(B, g.set_option, B.OPT_DELIVERY_KERNEL, 6) == B.NG_ERR_INVALID_ARG      # one GPU only
+    g.close()
+    wl = W.brunel_tiny(n_steps=50)
+    g = B.Sim(0.1, wl.ring_slots, wl.seed)
+    wl.apply(g); g.prepare()
+    assert code(B, g.set_option, B.OPT_DELIVERY_KERNEL, 6) == B.NG_ERR_STATE            # after ng_prepare
+    g.close()
+    g = B.Sim(0.1, wl.ring_slots, wl.seed)
+    wl.apply(g); g.set_option(B.OPT_DELIVERY_KERNEL, 6); g.prepare()
+    g.set_option(B.OPT_STEP_MODE, 0)                                                    # ignored: kernel 6 is persistent only
+    g.set_state(B.FIELD_V, wl.initial_v())
+    g.simulate(50)
+    st = g.stats()
+    assert st.delivery_kernel == 6 and st.step_mode == B.STEP_PERSISTENT and st.spikes > 150
+    assert code(B, g.set_state, B.FIELD_RING, np.zeros(1000 * 20, np.float32)) == B.NG_ERR_STATE   # two planes: read-only
+    assert g.get_state(B.FIELD_RING).size == 1000 * 20
+    g.close()
