@@ -47,13 +47,14 @@ def measured_peak_gbs():
 
 
 def csrc_hash():
-    """sha256 over the CUDA sources libng.so is built from: an ncu capture is only quoted for the code it was taken on."""
+    """sha256 over the CUDA sources the simulation kernels are built from (ng.cu + ng_device.cuh; ng_noalloc.cu holds a
+    separate entry point with kernels of its own that bench.py never launches): an ncu capture is only quoted for the
+    code it was taken on."""
     import hashlib
     h = hashlib.sha256()
     d = os.path.join(ROOT, "paper_2007_14236_b200", "csrc")
-    for f in sorted(os.listdir(d)):
-        if f.endswith((".cu", ".cuh")):
-            h.update(open(os.path.join(d, f), "rb").read())
+    for f in ("ng.cu", "ng_device.cuh"):
+        h.update(open(os.path.join(d, f), "rb").read())
     return h.hexdigest()[:16]
 
 

@@ -336,6 +336,39 @@ int32_t ng_get_trace(ng_sim* sim, uint64_t* out_host, int64_t capacity, int64_t*
  * Allocates its own scratch with cudaMalloc and frees it.  Errors: INVALID_ARG, OOM, CUDA. */
 int32_t ng_probe(int32_t device, int32_t kind, int64_t footprint_bytes, double* per_second_out);
 
+/* ---- Spike delivery that allocates nothing (csrc/ng_noalloc.cu) --------------------------------------------------
+ * For callers that cannot call cudaMalloc: code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * it.  One step n of a3 (every connection (j -> i, w, d) of a neuron j that spiked in step n adds w to
+ * ring slot (n + d) mod D of target i) on caller-owned DEVICE arrays, with the ring — the only scratch the step
+ * needs — in a static device array of the library instead of allocated memory:
+ *     NG_NOALLOC_MAX_CELLS = 4,194,304 float cells = 16 MiB, held by every GPU that loads libng.so until exit;
+ *     n_targets * ring_slots beyond it is rejected with NG_ERR_INVALID_ARG (use ng_create / ng_simulate there).
+ * What one call does, in stream order on cuda_stream (NULL = legacy default stream) of the CURRENT device:
+ *     reset != 0: the ring is cleared first (the array keeps the last call's contents: pass reset on the first call
+ *                 of a sequence, and whenever the network or the step sequence changes);
+ *     input_out_dev[i] = ring[(step mod D) * n_targets + i], i < n_targets — the input arriving at step n, what
+ *                 the neuron update of step n consumes (NG_FIELD_LAST_INPUT) — and that plane is cleared;
+ *     for every s < n_spikes, j = spike_ids_dev[s], every record r in [row_offsets_dev[j], row_offsets_dev[j+1]):
+ *                 ring[((step + delay_dev[r]) mod D) * n_targets + tgt_dev[r]] += w_dev[r]   (red.global.add.f32).
+ * The connection arrays have the layout ng_copy_row_offsets / ng_copy_records return (source-major rows, int64
+ * offsets [n_sources + 1], records with tgt < 0 are padding and skipped); rows that start and end on multiples of
+ * 4 records in 16-byte aligned arrays are read with 128-bit loads, any other layout with scalar loads.  A record whose
+ * target is >= n_targets or whose delay is outside [1, ring_slots], and a spike id outside [0, n_sources), is
+ * skipped and counted; ng_deliver_noalloc_check synchronises the stream, returns the count since the last check
+ * (n_bad_out may be NULL) and NG_ERR_OVERFLOW if it is not zero.
+ * The call enqueues two kernels (and one memset with reset) and returns without synchronising; it calls no
+ * cudaMalloc, cudaFree or allocating library routine.  Ownership: all arrays stay the caller's.
+ * ALL calls on one GPU share the one static ring: calls that overlap on the GPU (two streams, two host threads, two
+ * simulations interleaved step by step) race on it — one sequence of steps at a time per GPU.
+ * Errors: INVALID_ARG (sizes, NULL arrays), CUDA.  ng_noalloc_last_error() gives the message of the calling
+ * thread's last failing ng_deliver_noalloc* call ("" if none). */
+#define NG_NOALLOC_MAX_CELLS (1 << 22)
+int32_t ng_deliver_noalloc(void* cuda_stream, const int64_t* row_offsets_dev, const int32_t* tgt_dev, const float* w_dev,
+                           const uint8_t* delay_dev, int32_t n_sources, const int32_t* spike_ids_dev, int32_t n_spikes,
+                           int32_t n_targets, int32_t ring_slots, int64_t step, int32_t reset, float* input_out_dev);
+int32_t ng_deliver_noalloc_check(void* cuda_stream, int64_t* n_bad_out);
+const char* ng_noalloc_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

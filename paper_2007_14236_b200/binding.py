@@ -27,7 +27,9 @@ EXPORTS = ["ng_create", "ng_destroy", "ng_last_error", "ng_create_population", "
            "ng_copy_group_offsets", "ng_copy_records", "ng_get_connections", "ng_get_stats", "ng_get_trace", "ng_probe",
            "ng_create_population_adex", "ng_connect_fixed_indegree_port", "ng_connect_fixed_outdegree_port",
            "ng_enable_statistics", "ng_get_rate_cv", "ng_get_correlations",
-           "ng_shard_range", "ng_set_shard", "ng_exchange_handle", "ng_exchange_attach", "ng_shard_phase"]
+           "ng_shard_range", "ng_set_shard", "ng_exchange_handle", "ng_exchange_attach", "ng_shard_phase",
+           "ng_deliver_noalloc", "ng_deliver_noalloc_check", "ng_noalloc_last_error"]
+NOALLOC_MAX_CELLS = 1 << 22
 
 
 class NgConfig(C.Structure):
@@ -132,8 +134,12 @@ def load_library(path: str | None = None):
     L.ng_exchange_handle.argtypes = [vp, vp, C.POINTER(vp)]
     L.ng_exchange_attach.argtypes = [vp, i32, vp, vp]
     L.ng_shard_phase.argtypes = [vp, i32]
+    L.ng_deliver_noalloc.argtypes = [vp, vp, vp, vp, vp, i32, vp, i32, i32, i32, i64, i32, vp]
+    L.ng_deliver_noalloc_check.argtypes = [vp, C.POINTER(i64)]
+    L.ng_noalloc_last_error.argtypes = []
+    L.ng_noalloc_last_error.restype = C.c_char_p
     for name in EXPORTS:
-        if name != "ng_last_error":
+        if name not in ("ng_last_error", "ng_noalloc_last_error"):
             getattr(L, name).restype = i32
     if path is None:
         _lib = L
@@ -147,6 +153,33 @@ def probe(kind: int, footprint_bytes: int = 4 << 20, device: int = 0) -> float:
     if rc != NG_OK:
         raise NgError(rc, "ng_probe failed")
     return out.value
+
+
+def _dev_ptr(t):
+    return 0 if t is None else t.data_ptr()
+
+
+def deliver_noalloc(row_offsets, tgt, w, delay, spike_ids, n_spikes: int, n_targets: int, ring_slots: int, step: int,
+                    input_out, reset: bool = False, stream: int = 0) -> None:
+    """ng_deliver_noalloc: one delivery step on caller-owned DEVICE tensors (int64 row offsets, int32 targets, float32
+    weights, uint8 delays, int32 spike ids, float32 output), the ring in the library's static 16 MiB device array.
+    Enqueues on `stream` (a raw cudaStream_t, 0 = default) of the current device and returns; allocates nothing."""
+    L = load_library()
+    rc = L.ng_deliver_noalloc(stream, _dev_ptr(row_offsets), _dev_ptr(tgt), _dev_ptr(w), _dev_ptr(delay),
+                              0 if row_offsets is None else row_offsets.numel() - 1, _dev_ptr(spike_ids), n_spikes,
+                              n_targets, ring_slots, step, int(bool(reset)), _dev_ptr(input_out))
+    if rc != NG_OK:
+        raise NgError(rc, L.ng_noalloc_last_error().decode())
+
+
+def deliver_noalloc_check(stream: int = 0) -> int:
+    """ng_deliver_noalloc_check: synchronises; raises if records or spike ids were skipped as out of range since the last check."""
+    L = load_library()
+    bad = C.c_int64()
+    rc = L.ng_deliver_noalloc_check(stream, C.byref(bad))
+    if rc != NG_OK:
+        raise NgError(rc, L.ng_noalloc_last_error().decode())
+    return bad.value
 
 
 def _lif(params: dict) -> NgLifParams:
