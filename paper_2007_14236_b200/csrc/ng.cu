@@ -290,6 +290,16 @@ void configure_launch(ng_sim* s) {
     destroy_graph(s);
 }
 
+// Resident one-round LIF kernel: take the spike decisions of step n + 1 in the barrier shadow of step n (kEarly,
+// ng_device.cuh)?  It pays once a CTA holds enough neurons for spikes to be frequent; with a handful of neurons per CTA
+// the step is the barrier itself and the work in front of the poll only delays it (config 0: 2.52 -> 2.55-2.68 us).
+#ifndef NG_EARLY_MIN_PER_CTA
+#define NG_EARLY_MIN_PER_CTA 32
+#endif
+bool early_decision(const ng_sim* s) {
+    return !s->has_adex && (long long)s->N >= (long long)NG_EARLY_MIN_PER_CTA * s->persistent_pipe_blocks;
+}
+
 int32_t build_graph(ng_sim* s, int steps) {
     destroy_graph(s);
     cudaGraph_t graph = nullptr;
@@ -929,7 +939,9 @@ int32_t ng_simulate(ng_sim* s, int64_t n_steps) {
         } else if (s->delivery_kernel == 3) {
             const void* fn = s->has_adex ? (s->one_round_persistent ? (const void*)persistent_pipe_kernel<true, true>
                                                                      : (const void*)persistent_pipe_kernel<true, false>)
-                                         : (s->one_round_persistent && !s->bypass ? (const void*)persistent_pipe_kernel<false, true>
+                                         : (s->one_round_persistent && !s->bypass
+                                                ? (early_decision(s) ? (const void*)persistent_pipe_kernel<false, true, false, false, true>
+                                                                     : (const void*)persistent_pipe_kernel<false, true>)
                                             : s->resm_bytes ? (const void*)persistent_pipe_kernel<false, false, true>
                                                             : (const void*)persistent_pipe_kernel<false, false>);
             NG_CUDA(s, cudaLaunchCooperativeKernel(fn, dim3(s->persistent_pipe_blocks),

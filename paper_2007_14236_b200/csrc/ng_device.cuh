@@ -1391,6 +1391,7 @@ struct PipeShared {
     uint8_t res_kq[kResCap];               // Poisson count of the next step (barrier shadow)
     int32_t n_slow;
     int32_t n_d1;
+    int32_t n_d1x[2];                      // kEarly: spikes of step m on the CTA list at [m & 1] (counted one phase ahead)
     StepScalars sc;
     int32_t pending;
     // pipelined spike-buffer backend (kernel 6): absolute window position of the first spike of step s at [s mod (D+1)]
@@ -1480,15 +1481,108 @@ struct ResM { float* V; float* I; int32_t* r; uint8_t* pi; int rounds; };
 #endif
 constexpr int kResMRest = NG_RESM_REST;           // rest-group threads of the kResM kernel
 
+// kEarly (resident LIF state, ring backend): the membrane update of a step needs nothing that the grid barrier in front of
+// it publishes — V_{m+1} = f(V_m, I_m), both final in shared memory when the CTA arrives at the barrier of step m - 1;
+// only the CURRENT update reads the input cell.  The spike decision of step m is therefore taken between arrival and
+// release of barrier m - 1 (resident_decide), where the CTA would only poll: the CTA list of step m is complete and the
+// spiking rows are on their way from DRAM when the phase starts, and the phase itself (resident_late) begins with the
+// delay-1 reductions.  Arithmetic and order per neuron are those of the in-phase form: bit-identical results.
+#ifndef NG_EARLY_POISSON_LATE_U
+#define NG_EARLY_POISSON_LATE_U 256      // updater threads per CTA from which the next step's Poisson counts are drawn at the
+#endif                                   // end of the phase instead of in the barrier shadow (measured: DESIGN.md section 6)
+__device__ __forceinline__ bool resident_decide(const StepArgs& a, const PopDev* __restrict__ P, long long m, PipeShared& sh, int U) {
+    const int t = threadIdx.x, lane = t & 31;
+    const long long ii = (long long)blockIdx.x * U + t;
+    bool spk = false, ovf = false;
+    RowInfo r;
+    if (ii < a.N) {
+        float V = sh.res_V[t];
+        int rf = sh.res_r[t];
+        const PopDev* __restrict__ p = P + sh.res_pi[t];
+        const float E_L = p->E_L;
+        if (rf == 0) V = E_L + fmaf(p->P22, V - E_L, fmaf(p->P21, sh.res_I[t], p->P20Ie));
+        else rf -= 1;
+        if (V >= p->V_th) { spk = true; V = p->V_reset; rf = p->refr_steps; r = sh.res_row[t]; }
+        sh.res_V[t] = V; sh.res_r[t] = rf;
+    }
+    const unsigned mk = __ballot_sync(0xffffffffu, spk);
+    if (mk) {                                                  // warp-aggregated append to the CTA's list of step m
+        const int leader = __ffs(mk) - 1;
+        int lb = 0;
+        if (lane == leader) lb = atomicAdd(&sh.n_d1x[m & 1], __popc(mk));
+        if (spk && a.prefetch) prefetch_row(a, r);             // delay-1 head first, then the whole row: a barrier ahead of its use
+        lb = __shfl_sync(0xffffffffu, lb, leader);
+        if (spk) {
+            stat_on_spike(a, (int)ii, m);
+            const int k = lb + __popc(mk & ((1u << lane) - 1u));
+            if (k < kD1Cap) { sh.d1_r0[k] = r.r0; sh.d1_cnt[k] = r.d1; sh.d1_deg[k] = r.deg; sh.d1_id[k] = (int)ii; }
+            else ovf = true;                                   // CTA list full: this thread delivers alone in the phase
+        }
+    }
+    return ovf;
+}
+
+// Phase n of the updater threads when the spikes of step n were decided ahead (resident_decide): reserve the CTA's slots in
+// the global spike array, deliver the delay-1 records, then the current update — the only reader of the input cell.
+__device__ __forceinline__ void resident_late(const StepArgs& a, const PopDev* __restrict__ P, long long n, int slot, PipeShared& sh,
+                                              int U, bool have_k, bool ovf, bool pois_late) {
+    const int N = a.N, Dr = a.Dr, t = threadIdx.x, lane = t & 31, wib = t >> 5, wpu = U >> 5;
+    float* __restrict__ plane = a.ring + (size_t)slot * a.NR;
+    float* __restrict__ plane1 = a.ring + (size_t)(slot + 1 == Dr ? 0 : slot + 1) * a.NR;
+    const long long ii = (long long)blockIdx.x * U + t;
+    const int i = (int)ii;
+    float res_in = 0.f;
+    if (ii < N) res_in = ld_plane(plane + i);                  // first: the one long latency of the phase
+    const int nd1 = min(sh.n_d1x[n & 1], kD1Cap);
+    if (t == 0) sh.n_d1x[(n + 1) & 1] = 0;                     // last read in phase n - 1; next written after this phase's last barrier
+    trace_stamp(a, n, 4);
+    int gb = 0;
+    if (t == U - 1 && nd1 > 0) gb = atomicAdd(&a.ctl->spike_cnt[n & 3], nd1);
+    if (ovf) {
+        const RowInfo r = sh.res_row[t];
+        for (int q = 0; q < r.d1; ++q) deliver_d1_piece(a, plane1, r.r0, r.d1, q);
+        const size_t gk = (size_t)(n & 1) * N + atomicAdd(&a.ctl->spike_cnt[n & 3], 1);
+        a.spike_list[gk] = i;
+        st_row_info(a.spike_row + gk, r);
+    }
+    if (nd1 <= 2) {                                            // latency regime: one or two spikes, 32 records per warp
+        for (int s = 0; s < nd1; ++s) {
+            const long long r0 = sh.d1_r0[s];
+            const int cnt = sh.d1_cnt[s];
+            for (int q = wib * 32 + lane; q < cnt; q += wpu * 32) deliver_d1_piece(a, plane1, r0, cnt, q);
+        }
+    } else d1_flat_pass(a, sh, plane1, nd1, U);
+    if (ii < N) {                                              // the current update
+        const PopDev* __restrict__ p = P + sh.res_pi[t];
+        clear_plane(plane + i);
+        if (a.last_input) a.last_input[i] = res_in;
+        const int k = have_k ? (int)sh.res_kq[t] : poisson_count(a, p, n, i);
+        sh.res_I[t] = fmaf(p->P11, sh.res_I[t], res_in) + p->w_ext * (float)k;
+    }
+    trace_stamp(a, n, 6);
+    if (nd1 > 0 && t >= U - 32) {                              // the last updater warp: a2, the global spike array
+        gb = __shfl_sync(0xffffffffu, gb, 31);
+        for (int s = lane; s < nd1; s += 32) {
+            RowInfo r; r.r0 = sh.d1_r0[s]; r.d1 = sh.d1_cnt[s]; r.deg = sh.d1_deg[s];
+            const size_t gk = (size_t)(n & 1) * N + gb + s;
+            a.spike_list[gk] = sh.d1_id[s];
+            st_row_info(a.spike_row + gk, r);
+        }
+    }
+    // Poisson count of step n + 1 (wide CTAs: here, behind the reductions, instead of in front of the barrier poll)
+    if (pois_late && ii < N) sh.res_kq[t] = (uint8_t)poisson_count(a, P + sh.res_pi[t], n + 1, i);
+}
+
 // kWin (delivery kernel 6, the pipelined spike-buffer backend): two input planes instead of the D + 1 of the ring.  The
 // delay-1 pass is unchanged; the rest pass is replaced by the walk over the spike window of the paper's mechanism
 // (as in kernel 4): in phase n the rest warps deliver, for every spike of the steps n - D + 1 .. n - 1, the
 // connection group whose delay is the spike's age + 1 — everything that arrives in step n + 1 — into the ONE plane of step
 // n + 1, which stays in L2 whatever D and the number of receptor ports are.  `wslot` = n mod (D + 1).
-template <bool kUpdate, bool kAdex, bool kOneRound = false, bool kRes = false, bool kResM = false, bool kWin = false>
+template <bool kUpdate, bool kAdex, bool kOneRound = false, bool kRes = false, bool kResM = false, bool kWin = false, bool kEarly = false>
 __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* __restrict__ P, long long n, int slot, bool pending,
                                                unsigned long long rec_prev, PipeShared& sh, int U, bool have_k = false,
-                                               const ResM rm = ResM{}, int wslot = 0) {
+                                               const ResM rm = ResM{}, int wslot = 0, bool ovf = false) {
+    static_assert(!kEarly || (kRes && !kWin), "kEarly: resident one-round LIF state on the ring backend");
     const int N = a.N, Dr = a.Dr;
     const int lane = threadIdx.x & 31;
     // U = pipe_updater_threads(N, kAdex), computed once per launch by the caller: its integer division in front of every
@@ -1502,7 +1596,8 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
 
     if ((int)threadIdx.x < U) {
         // ---- update(n), spike collection, then the delay-1 records of this CTA's spikes ----
-        if (kUpdate) {
+        if (kUpdate && kEarly) resident_late(a, P, n, slot, sh, U, have_k, ovf, U >= NG_EARLY_POISSON_LATE_U);
+        else if (kUpdate) {
             const int wib = threadIdx.x >> 5, wpu = U >> 5;
             float* __restrict__ plane = a.ring + (size_t)slot * a.NR;
             float* __restrict__ plane1 = a.ring + (size_t)(slot + 1 == Dr ? 0 : slot + 1) * a.NR;
@@ -1898,7 +1993,7 @@ __global__ void __launch_bounds__(kPipeThreads) pipe_step_kernel(const NG_GC Ste
 }
 
 // kAdex: the AdEx integrator needs more than the 64 registers a 1024-thread CTA leaves: 512-thread CTAs, two per SM at most
-template <bool kAdex, bool kOneRound = false, bool kResM = false, bool kWin = false>
+template <bool kAdex, bool kOneRound = false, bool kResM = false, bool kWin = false, bool kEarly = false>
 __global__ void __launch_bounds__(kAdex ? 512 : kPersistentThreads, kAdex ? 2 : 1) persistent_pipe_kernel(const NG_GC StepArgs a, long long n_steps) {
     __shared__ PipeShared sh;
     if (threadIdx.x == 0) {
@@ -1939,15 +2034,25 @@ __global__ void __launch_bounds__(kAdex ? 512 : kPersistentThreads, kAdex ? 2 : 
     int slot = sh.sc.slot;
     unsigned long long rec_prev = sh.sc.rec_base, spikes = 0, epoch = 0;       // recorded before step n-1 (nothing pending at entry)
     int wslot = sh.sc.M;
+    bool ovf = false;                                              // kEarly: this thread's spike of the coming step is not on the CTA list
+    if (kEarly && n_steps > 0) {                                   // spikes of the first step of the launch
+        if (threadIdx.x < 2) sh.n_d1x[threadIdx.x] = 0;
+        __syncthreads();
+        if ((int)threadIdx.x < U) ovf = resident_decide(a, P, n, sh, U);
+    }
     for (long long s = 0; s < n_steps; ++s, ++n) {
         if (gtid == 0) a.ctl->spike_cnt[(n + 1) & 3] = 0;          // last read (as step n-3's) in phase n-2
         trace_stamp(a, n, 0);
-        const int Mp = pipelined_phase<true, kAdex, kOneRound, kRes, kResM, kWin>(a, P, n, slot, s > 0, rec_prev, sh, U, s > 0 && single_round, rm, wslot);
+        const int Mp = pipelined_phase<true, kAdex, kOneRound, kRes, kResM, kWin, kEarly>(a, P, n, slot, s > 0, rec_prev, sh, U, s > 0 && single_round, rm, wslot, ovf);
         rec_prev += (unsigned long long)Mp; spikes += (unsigned long long)Mp;
         trace_stamp(a, n, 1);
         grid_arrive(a.ctl, epoch);
         if (s + 1 < n_steps && !a.bypass && single_round && (int)threadIdx.x < U) {    // barrier shadow: Poisson counts of step n+1
-            if (kRes) {                                            // thread t owns neuron blockIdx.x * U + t for the whole launch
+            if (kEarly) {                                          // ... and, first, its spikes
+                ovf = resident_decide(a, P, n + 1, sh, U);
+                const long long ii = (long long)blockIdx.x * U + threadIdx.x;
+                if (U < NG_EARLY_POISSON_LATE_U && ii < a.N) sh.res_kq[threadIdx.x] = (uint8_t)poisson_count(a, P + sh.res_pi[threadIdx.x], n + 1, (int)ii);
+            } else if (kRes) {                                     // thread t owns neuron blockIdx.x * U + t for the whole launch
                 const long long ii = (long long)blockIdx.x * U + threadIdx.x;
                 if (ii < a.N) sh.res_kq[threadIdx.x] = (uint8_t)poisson_count(a, P + sh.res_pi[threadIdx.x], n + 1, (int)ii);
             } else
