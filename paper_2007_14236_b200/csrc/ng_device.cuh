@@ -1856,7 +1856,9 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
         group_sync(2, R);
         trace_stamp(a, n, 7, U);
         const int M = sh.d.M;
-        const int gwarp = blockIdx.x * wpr + wir, gwarps = gridDim.x * wpr;      // items are dealt to the rest warps of the grid
+        // items are dealt to the rest warps of the grid, CTA by CTA: a light step has fewer items than rest warps, and an SM
+        // issues the scattered reductions of its items one address at a time — every SM should get its share
+        const int gwarp = wir * gridDim.x + blockIdx.x, gwarps = gridDim.x * wpr;
         // item size: the smallest of 32 / 64 / 128 records with about one item per rest warp or fewer — a warp's items
         // are serial (every scattered red holds it for an L2 round trip), so the phase ends with the warp that has most
         const long long est = (long long)M * a.mean_row_records;
