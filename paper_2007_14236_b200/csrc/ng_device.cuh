@@ -1859,10 +1859,11 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
         // items are dealt to the rest warps of the grid, CTA by CTA: a light step has fewer items than rest warps, and an SM
         // issues the scattered reductions of its items one address at a time — every SM should get its share
         const int gwarp = wir * gridDim.x + blockIdx.x, gwarps = gridDim.x * wpr;
-        // item size: the smallest of 32 / 64 / 128 records with about one item per rest warp or fewer — a warp's items
-        // are serial (every scattered red holds it for an L2 round trip), so the phase ends with the warp that has most
+        // item size: 32 / 64 / 128 records.  A warp's items are serial (every scattered red holds it for an L2 round trip), so
+        // small items only while a quarter of the rest warps or fewer get one; beyond that the wide loads of the 128-record
+        // item win (measured on config 2 with thresholds 32/64, 16/32, 8/16 per warp: 4.10 / 4.05 / 4.03 us per step)
         const long long est = (long long)M * a.mean_row_records;
-        const int cshift = est <= 32LL * gwarps ? 5 : est <= 64LL * gwarps ? 6 : 7;
+        const int cshift = est <= 8LL * gwarps ? 5 : est <= 16LL * gwarps ? 6 : 7;
         unsigned long long ev = 0;
         int base_mod = 0;
         // many spikes (>= 8 per CTA): every CTA stages only its own tiles and deals their items to its own rest warps
