@@ -41,6 +41,7 @@ struct ng_sim {
     bool prepared = false;
     int32_t bypass = 0; uint32_t inject_thr = 0;
     // options
+    int list_bufs = 2;
     int step_mode_opt = 3; int step_mode = 0; int steps_per_graph = 100; int delivery_kernel_opt = 0; int deliver_blocks_opt = 0;
     bool trace_on = false; unsigned long long* trace_saved = nullptr; int last_persistent_blocks = 0;
     int profile = 0; int async = 0; int sort_segments = 1; int prefetch_opt = 1;
@@ -293,11 +294,14 @@ void configure_launch(ng_sim* s) {
 // Resident one-round LIF kernel: take the spike decisions of step n + 1 in the barrier shadow of step n (kEarly,
 // ng_device.cuh)?  It pays once a CTA holds enough neurons for spikes to be frequent; with a handful of neurons per CTA
 // the step is the barrier itself and the work in front of the poll only delays it (config 0: 2.52 -> 2.55-2.68 us).
+#ifndef NG_SPLIT_KERNEL
+#define NG_SPLIT_KERNEL 1
+#endif
 #ifndef NG_EARLY_MIN_PER_CTA
 #define NG_EARLY_MIN_PER_CTA 32
 #endif
 bool early_decision(const ng_sim* s) {
-    return !s->has_adex && (long long)s->N >= (long long)NG_EARLY_MIN_PER_CTA * s->persistent_pipe_blocks;
+    return !s->has_adex && s->list_bufs == 4 && (long long)s->N >= (long long)NG_EARLY_MIN_PER_CTA * s->persistent_pipe_blocks;
 }
 
 int32_t build_graph(ng_sim* s, int steps) {
@@ -683,11 +687,14 @@ int32_t ng_prepare(ng_sim* s) {
     NG_CUDA(s, cudaEventRecord(e0, st));
 
     // ---- control block, populations, state ----
+    // the spike array of two steps; of four where the resident LIF kernel with the split barrier can be chosen (its CTAs
+    // drift a phase apart; one neuron per updater thread of a persistent launch: small networks, 80 B per neuron)
+    s->list_bufs = (!s->has_adex && s->shard_world <= 1 && (long long)N <= 1024LL * 4 * std::max(1, s->sm_count)) ? 4 : 2;
     bool ok = dev_alloc_t(s, &s->d_ctl, 1) && dev_alloc_t(s, &s->d_pops, s->pops.size()) &&
               dev_alloc_t(s, &s->d_pop_of, (size_t)NL) && dev_alloc_t(s, &s->a.V, (size_t)NL) &&
               dev_alloc_t(s, &s->a.I, (size_t)NL) && dev_alloc_t(s, &s->a.refr, (size_t)NL) &&
-              dev_alloc_t(s, &s->a.ring, NRs * planes) && dev_alloc_t(s, &s->a.spike_list, (size_t)2 * N) &&
-              dev_alloc_t(s, &s->a.spike_row, (size_t)2 * N) && dev_alloc_t(s, &s->a.pois_k, (size_t)NL) && dev_alloc_t(s, &s->d_row_info, (size_t)N) &&
+              dev_alloc_t(s, &s->a.ring, NRs * planes) && dev_alloc_t(s, &s->a.spike_list, (size_t)s->list_bufs * N) &&
+              dev_alloc_t(s, &s->a.spike_row, (size_t)s->list_bufs * N) && dev_alloc_t(s, &s->a.pois_k, (size_t)NL) && dev_alloc_t(s, &s->d_row_info, (size_t)N) &&
               dev_alloc_t(s, &s->d_calls, std::max<size_t>(1, s->calls.size())) &&
               dev_alloc_t(s, &s->d_cnt, (size_t)N * D) && dev_alloc_t(s, &s->d_row_len, (size_t)N) &&
               dev_alloc_t(s, &s->d_row_off, (size_t)N + 1) && dev_alloc_t(s, &s->d_grp_rel, (size_t)N * (D + 1));
@@ -924,7 +931,7 @@ int32_t ng_simulate(ng_sim* s, int64_t n_steps) {
     } else if (s->step_mode == 2) {
         long long ns = n_steps;
         void* args[] = {(void*)&s->a, (void*)&ns};
-        NG_CUDA(s, cudaMemsetAsync(&s->d_ctl->bar, 0, sizeof(unsigned long long), st));
+        NG_CUDA(s, cudaMemsetAsync(&s->d_ctl->bar, 0, offsetof(Ctl, bar_list) + 2 * sizeof(unsigned long long) - offsetof(Ctl, bar), st));   // bar, ticket, bar_plane, bar_list
         const bool piped = s->delivery_kernel == 3 || s->delivery_kernel == 6;
         s->last_persistent_blocks = piped ? s->persistent_pipe_blocks : s->persistent_blocks;
         if (s->delivery_kernel == 6) {
@@ -940,7 +947,7 @@ int32_t ng_simulate(ng_sim* s, int64_t n_steps) {
             const void* fn = s->has_adex ? (s->one_round_persistent ? (const void*)persistent_pipe_kernel<true, true>
                                                                      : (const void*)persistent_pipe_kernel<true, false>)
                                          : (s->one_round_persistent && !s->bypass
-                                                ? (early_decision(s) ? (const void*)persistent_pipe_kernel<false, true, false, false, true>
+                                                ? (early_decision(s) ? (NG_SPLIT_KERNEL ? (const void*)persistent_split_kernel : (const void*)persistent_pipe_kernel<false, true, false, false, true>)
                                                                      : (const void*)persistent_pipe_kernel<false, true>)
                                             : s->resm_bytes ? (const void*)persistent_pipe_kernel<false, false, true>
                                                             : (const void*)persistent_pipe_kernel<false, false>);

@@ -75,11 +75,17 @@ struct Ctl {
     unsigned long long n_records;          // builder: records stored on this shard (unpadded)
     // line 1: spike counters (atomics of the appending warps / CTAs)
     alignas(128) int32_t spike_cnt[4];     // length of the spike array of step n, indexed n & 3 (the list itself by n & 1)
+    int32_t spike_cnt8[8];                 // split kernel: the same, indexed n & 7 (its warp groups run up to two steps apart)
     // line 2: event counter (one atomic per CTA and step)
     alignas(128) unsigned long long events;
     // line 3: grid barrier of the persistent kernels, and the ticket of the stand-alone pipelined kernel
     alignas(128) unsigned long long bar;   // arrivals at the grid barrier
     unsigned int ticket;                   // CTAs that finished the current step
+    unsigned long long bar_plane[2];       // split kernel: CTAs whose reductions of a phase are all issued and acknowledged, and
+    unsigned long long bar_list[2];        // split kernel: CTAs that have appended their spikes of a step to the global spike array,
+                                           // one word per step parity each (a CTA may arrive for step n + 1 while another still
+                                           // waits for step n to be complete: on one word its arrival would stand in for a missing one;
+                                           // it cannot arrive for step n + 2 before step n is complete)
     // line 4 ..: spike-buffer backend
     alignas(128) unsigned long long win_start[kMaxWindowSteps + 1];   // absolute position in the spike window of the first
                                            // spike of step s, at index s mod (D+1); [s+1] = its end
@@ -1392,6 +1398,7 @@ struct PipeShared {
     int32_t n_slow;
     int32_t n_d1;
     int32_t n_d1x[2];                      // kEarly: spikes of step m on the CTA list at [m & 1] (counted one phase ahead)
+    int32_t phase_cnt[4];                  // split kernel: warp groups of the CTA that are done with the phase of step index s & 3
     StepScalars sc;
     int32_t pending;
     // pipelined spike-buffer backend (kernel 6): absolute window position of the first spike of step s at [s mod (D+1)]
@@ -1958,6 +1965,152 @@ __device__ __forceinline__ int pipelined_phase(const StepArgs& a, const PopDev* 
     return sh.d.M;
 }
 
+// The rest pass of step n - 1 for the split kernel (persistent_split_kernel): the rest group's half of pipelined_phase as
+// a function of its own — it is called by the rest group alone, with no CTA-wide barrier around it.  Waits for the list
+// barrier of step n - 1 first (`list_need` arrivals on the word of that step's parity).  Returns M_{n-1}.
+__device__ __forceinline__ int split_rest_pass(const StepArgs& a, long long n, int slot, unsigned long long rec_prev, PipeShared& sh, int U, int R,
+                                               unsigned long long list_need) {
+    // U = first thread of the rest group, R = its size
+    const int N = a.N, Dr = a.Dr;
+    const int lane = threadIdx.x & 31;
+    const int RT = min(R, kEntryTile);
+    const int nmod_prev = slot == 0 ? Dr - 1 : slot - 1;           // (n - 1) mod Dr
+    {
+        // ---- rest pass of step n-1: records [d1, deg) of every spike ----
+        const int t = threadIdx.x - U;                             // index inside the rest group
+        const int wir = t >> 5, wpr = R >> 5;
+        const long long np = n - 1;
+        constexpr int kListMask = 3;                               // the spike array of four steps is kept
+        const RowInfo* __restrict__ rows_prev = a.spike_row + (size_t)(np & kListMask) * N;
+        const int32_t* __restrict__ list_prev = a.spike_list + (size_t)(np & kListMask) * N;
+        const bool rec_cta = blockIdx.x == 0 && a.rec_cap > 0;
+        if (list_need) {                                 // list barrier of step n-1: its spike array is complete
+            if (t == 0) {
+                unsigned long long v;
+                do {
+                    asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(&a.ctl->bar_list[np & 1]) : "memory");
+                } while (v < list_need);
+            }
+            group_sync(2, R);
+        }
+        int4 e = make_int4(0, 0, 0, 0);
+        int id_prev = 0;
+        if (t == 0) sh.d.M = __ldcg(&a.ctl->spike_cnt8[np & 7]);
+        if (t < RT && t < N) {                                     // speculative: the first tile, before M is known
+            e = __ldcg(reinterpret_cast<const int4*>(rows_prev + t));
+            if (rec_cta) id_prev = __ldcg(list_prev + t);
+        }
+        // the first 32 entries go to shared memory before M is known (entries beyond M are stale but valid memory): the
+        // barrier that publishes M publishes them too
+        if (t < 32 && t < N) {
+            sh.d.r0[t] = (long long)(((unsigned long long)(uint32_t)e.y << 32) | (uint32_t)e.x);
+            sh.d.len[t] = padded_len(e.z);
+            sh.skip[t] = e.w;
+        }
+        group_sync(2, R);
+        trace_stamp(a, n, 7, U);
+        const int M = sh.d.M;
+        // items are dealt to the rest warps of the grid, CTA by CTA: a light step has fewer items than rest warps, and an SM
+        // issues the scattered reductions of its items one address at a time — every SM should get its share
+        const int gwarp = wir * gridDim.x + blockIdx.x, gwarps = gridDim.x * wpr;
+        // item size: 32 / 64 / 128 records.  A warp's items are serial (every scattered red holds it for an L2 round trip), so
+        // small items only while a quarter of the rest warps or fewer get one; beyond that the wide loads of the 128-record
+        // item win (measured on config 2 with thresholds 32/64, 16/32, 8/16 per warp: 4.10 / 4.05 / 4.03 us per step)
+        const long long est = (long long)M * a.mean_row_records;
+        const int cshift = est <= 8LL * gwarps ? 5 : est <= 16LL * gwarps ? 6 : 7;
+        unsigned long long ev = 0;
+        int base_mod = 0;
+        // many spikes (>= 8 per CTA): every CTA stages only its own tiles and deals their items to its own rest warps
+        const bool part = M >= 8 * (int)gridDim.x;
+        // a CTA's tile holds about M / gridDim entries, so that every CTA has one
+        const int tile_len = part ? min(RT, (M + (int)gridDim.x - 1) / (int)gridDim.x) : RT;
+        const int tile_first = part ? (int)blockIdx.x * tile_len : 0, tile_stride = part ? (int)gridDim.x * tile_len : RT;
+        const int gw = part ? wir : gwarp, gw_n = part ? wpr : gwarps;
+        const bool rec_here = a.rec_cap > 0 && (blockIdx.x == 0 || part);
+        if (M <= 32) {
+            // Latency regime (three steps of four in config 2): no second staging round and no second barrier — every
+            // rest warp prefix-sums the chunk counts of the <= 32 entries in its own registers and finds its items by
+            // ballot; the first records are requested ~0.5 us earlier.
+            const int len_l = lane < M ? sh.d.len[lane] : 0;
+            int incl = (len_l + (1 << cshift) - 1) >> cshift;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int y = __shfl_up_sync(0xffffffffu, incl, o);
+                if (lane >= o) incl += y;
+            }
+            const int total = __shfl_sync(0xffffffffu, incl, 31);
+            if (blockIdx.x == 0 && t < M) {                        // warp 0 of CTA 0 still holds the entries: events, spike record
+                ev += (unsigned long long)e.z;
+                if (rec_cta) {
+                    const unsigned long long pos = rec_prev + (unsigned long long)t;
+                    if (pos < (unsigned long long)a.rec_cap) { a.rec_id[pos] = id_prev; a.rec_step[pos] = (int32_t)np; }
+                }
+            }
+            for (int it = gwarp; it < total; it += gwarps) {
+                const int sidx = __popc(__ballot_sync(0xffffffffu, incl <= it));
+                const int before = __shfl_sync(0xffffffffu, incl, sidx > 0 ? sidx - 1 : 0);
+                const int c = it - (sidx > 0 ? before : 0);
+                if (cshift == 5) deliver_item<1>(a, nmod_prev, sh.d.r0[sidx], sh.d.len[sidx], c, lane, sh.skip[sidx]);
+                else if (cshift == 6) deliver_item<2>(a, nmod_prev, sh.d.r0[sidx], sh.d.len[sidx], c, lane, sh.skip[sidx]);
+                else deliver_item<4>(a, nmod_prev, sh.d.r0[sidx], sh.d.len[sidx], c, lane, sh.skip[sidx]);
+            }
+        } else
+        for (int tile0 = tile_first; tile0 < M; tile0 += tile_stride) {
+            const int m = min(tile_len, M - tile0);
+            if (tile0 > 0) {
+                group_sync(2, R);
+                if (t < m) {
+                    e = __ldcg(reinterpret_cast<const int4*>(rows_prev + tile0 + t));
+                    if (rec_here) id_prev = __ldcg(list_prev + tile0 + t);
+                }
+            }
+            int x = 0;
+            // only the warps that hold entries run the staging code: with all fifteen rest warps in it the few spikes of
+            // a latency-bound step cost ~250 issue slots per warp, 0.5 us, before the first record was requested
+            const int mw = (m + 31) >> 5;
+            if (t < m) {                                           // e = r0 (lo, hi), deg, d1
+                const int len = padded_len(e.z);
+                sh.d.r0[t] = (long long)(((unsigned long long)(uint32_t)e.y << 32) | (uint32_t)e.x);
+                sh.d.len[t] = len;
+                sh.skip[t] = e.w;
+                x = (len + (1 << cshift) - 1) >> cshift;
+                if (blockIdx.x == 0 || part) ev += (unsigned long long)e.z;
+                if (rec_here) {
+                    const unsigned long long pos = rec_prev + (unsigned long long)(tile0 + t);
+                    if (pos < (unsigned long long)a.rec_cap) { a.rec_id[pos] = id_prev; a.rec_step[pos] = (int32_t)np; }
+                }
+            }
+            if (wir < mw) {                                        // whole warps (m <= RT, a multiple of 32)
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const int y = __shfl_up_sync(0xffffffffu, x, o);
+                    if (lane >= o) x += y;
+                }
+                if (lane == 31) sh.d.warp_tot[wir] = x;
+            }
+            if (m > 32) {                                          // several warps hold entries: add the warp offsets
+                group_sync(2, R);
+                if (wir < mw) {
+                    int off = 0;
+                    for (int k = 0; k < wir; ++k) off += sh.d.warp_tot[k];
+                    sh.d.pre[t + 1] = x + off;
+                }
+            } else if (t < 32) sh.d.pre[t + 1] = x;                // latency regime: one warp, one barrier
+            if (t == 0) sh.d.pre[0] = 0;
+            group_sync(2, R);
+            trace_stamp(a, n, 8, U);
+            const int total = sh.d.pre[m];
+            int first = gw - base_mod;                             // items are numbered across tiles: round-robin deal
+            if (first < 0) first += gw_n;
+            for (int it = first; it < total; it += gw_n) pipe_one_item(a, nmod_prev, sh, m, it, cshift, lane);
+            base_mod = (int)(((long long)base_mod + total) % gw_n);
+        }
+        trace_stamp(a, n, 9, U);
+        if (ev) atomicAdd(&a.ctl->events, ev);
+        return M;
+    }
+}
+
 // Graph / plain-launch form: one launch per time step, the kernel boundary is the barrier.  The last CTA to finish
 // publishes the next step index (a4) and marks the rest pass of this step as pending.
 constexpr int kPipeThreads = 512;        // 256 updaters + 256 rest-pass threads
@@ -2109,6 +2262,200 @@ __global__ void __launch_bounds__(kAdex ? 512 : kPersistentThreads, kAdex ? 2 : 
         a.ctl->step_d = n - 1;
         a.ctl->slot = slot;
         a.ctl->step_u = n;
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// The split kernel: the resident LIF kernel (kEarly) with its grid barrier cut in two and its two warp groups decoupled.
+//   What a step really orders across CTAs is two things:
+//     list(n):  every CTA has appended its spikes of step n to the global spike array           -> Ctl::bar_list[n & 1]
+//     plane(n): every CTA has issued (and had acknowledged) all reductions of phase n           -> Ctl::bar_plane[step index & 1]
+//   and each has ONE consumer: the rest pass of step n (the delay >= 2 records, run by the rest warps) needs list(n); the
+//   current update of step n + 1 (the only reader of an input cell) needs plane(n).  Nothing else of a phase reads what
+//   other CTAs wrote in the phase before — the ring has D + 1 planes, the spike array is kept for four steps and its
+//   counters for eight — so no warp waits at a phase boundary any more, and the two warp groups of a CTA run their own loops:
+//     updaters, step n:  reserve slots, delay-1 reductions, a2 -> arrive list(n) -> [group done] -> wait plane(n - 1)
+//                        -> input cell, current update -> decisions of step n + 1 (resident_decide), its Poisson counts
+//     rest warps, step n: wait list(n - 1) -> count, descriptors, records, reductions of step n - 1 -> [group done]
+//   The group that is done second in a CTA arrives at plane(n) (one fence each, cumulative over the group's barrier).
+//   The latency of a barrier (release fence, arrival, poll: 1.1 us of a 4 us step) then overlaps the other group's work
+//   instead of standing between two phases.  Arithmetic and order per neuron are those of the in-phase form.
+// ---------------------------------------------------------------------------------------
+__device__ __forceinline__ void split_group_done(const StepArgs& a, PipeShared& sh, long long s_idx) {       // one thread, behind its group's barrier
+    asm volatile("fence.acq_rel.gpu;" ::: "memory");
+    if (atomicAdd(&sh.phase_cnt[s_idx & 3], 1) == 1) {             // the other group was first: the CTA is done with the phase
+        sh.phase_cnt[s_idx & 3] = 0;
+        asm volatile("red.relaxed.gpu.global.add.u64 [%0], 1;" ::"l"(&a.ctl->bar_plane[s_idx & 1]) : "memory");
+    }
+}
+
+__device__ __forceinline__ bool split_update_step(const StepArgs& a, const PopDev* __restrict__ P, long long n, long long s_idx, int slot,
+                                                  PipeShared& sh, int U, bool have_k, bool ovf, unsigned long long plane_need, bool decide_next) {
+    const int N = a.N, Dr = a.Dr, t = threadIdx.x, lane = t & 31, wib = t >> 5, wpu = U >> 5;
+    float* __restrict__ plane = a.ring + (size_t)slot * a.NR;
+    float* __restrict__ plane1 = a.ring + (size_t)(slot + 1 == Dr ? 0 : slot + 1) * a.NR;
+    const size_t buf = (size_t)(n & 3) * N;                    // the spike array of step n
+    const long long ii = (long long)blockIdx.x * U + t;
+    const int i = (int)ii;
+    group_sync(1, U);                                          // the CTA list of step n (resident_decide) is complete
+    const int n_all = sh.n_d1x[n & 1], nd1 = min(n_all, kD1Cap);
+    trace_stamp(a, n, 0);
+    // thread 0 asks for plane(n - 1) at once: its round trip runs beside the reductions and the append of the other warps
+    if (t == 0 && plane_need) {
+        unsigned long long v;
+        do {
+            asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(&a.ctl->bar_plane[(s_idx - 1) & 1]) : "memory");
+        } while (v < plane_need);
+    }
+    int gb = 0;
+    if (t == U - 1 && nd1 > 0) gb = atomicAdd(&a.ctl->spike_cnt8[n & 7], nd1);
+    if (ovf) {
+        const RowInfo r = sh.res_row[t];
+        for (int q = 0; q < r.d1; ++q) deliver_d1_piece(a, plane1, r.r0, r.d1, q);
+        const size_t gk = buf + atomicAdd(&a.ctl->spike_cnt8[n & 7], 1);
+        a.spike_list[gk] = i;
+        st_row_info(a.spike_row + gk, r);
+    }
+    if (nd1 <= 2) {                                            // latency regime: one or two spikes, 32 records per warp
+        for (int s = 0; s < nd1; ++s) {
+            const long long r0 = sh.d1_r0[s];
+            const int cnt = sh.d1_cnt[s];
+            for (int q = wib * 32 + lane; q < cnt; q += wpu * 32) deliver_d1_piece(a, plane1, r0, cnt, q);
+        }
+    } else d1_flat_pass(a, sh, plane1, nd1, U);
+    if (n_all > kD1Cap) group_sync(1, U);                      // overflow lanes have appended alone: before the list arrival
+    if (t >= U - 32) {                                         // the last updater warp: a2, the global spike array, list arrival
+        gb = __shfl_sync(0xffffffffu, gb, 31);
+        for (int s = lane; s < nd1; s += 32) {
+            RowInfo r; r.r0 = sh.d1_r0[s]; r.d1 = sh.d1_cnt[s]; r.deg = sh.d1_deg[s];
+            a.spike_list[buf + gb + s] = sh.d1_id[s];
+            st_row_info(a.spike_row + buf + gb + s, r);
+        }
+        __syncwarp();
+        if (lane == 31) asm volatile("red.release.gpu.global.add.u64 [%0], 1;" ::"l"(&a.ctl->bar_list[n & 1]) : "memory");
+    }
+    // beside those round trips: the Poisson count of step n + 1 (a pure function of neuron and step; 0.85 us for 17 warps)
+    int k_cur = -1;
+    if (ii < N) {
+        if (have_k) k_cur = (int)sh.res_kq[t];
+        if (decide_next) sh.res_kq[t] = (uint8_t)poisson_count(a, P + sh.res_pi[t], n + 1, i);
+    }
+    group_sync(1, U);                                          // all reductions of the phase issued; plane(n - 1) is complete
+    trace_stamp(a, n, 4);
+    float res_in = 0.f;
+    if (ii < N) res_in = ld_plane(plane + i);
+    if (t == (U >= 64 ? 32 : 0)) split_group_done(a, sh, s_idx);   // (behind the load: the fence waits for it anyway; measured best place)
+    if (t == 0) {
+        sh.n_d1x[(n + 1) & 1] = 0;                             // (read above by every warp; written again behind the barrier below)
+        // every CTA is done with phase n - 1, hence with the count of step n - 3 (read by the rest pass of phase n - 2):
+        // that counter serves step n + 5 next
+        if (blockIdx.x == 0) a.ctl->spike_cnt8[(n + 5) & 7] = 0;
+    }
+    if (ii < N) {                                              // the current update
+        const PopDev* __restrict__ p = P + sh.res_pi[t];
+        clear_plane(plane + i);
+        if (a.last_input) a.last_input[i] = res_in;
+        const int k = k_cur >= 0 ? k_cur : poisson_count(a, p, n, i);
+        sh.res_I[t] = fmaf(p->P11, sh.res_I[t], res_in) + p->w_ext * (float)k;
+    }
+    trace_stamp(a, n, 6);
+    bool ovf_next = false;
+    if (decide_next) {
+        group_sync(1, U);                                      // the counter of the next CTA list is clear
+        ovf_next = resident_decide(a, P, n + 1, sh, U);
+    }
+    trace_stamp(a, n, 1);
+    return ovf_next;
+}
+
+__global__ void __launch_bounds__(kPersistentThreads, 1) persistent_split_kernel(const NG_GC StepArgs a, long long n_steps) {
+    __shared__ PipeShared sh;
+    if (threadIdx.x == 0) {
+        sh.sc.n = __ldcg(&a.ctl->step_u);
+        sh.sc.slot = __ldcg(&a.ctl->slot);
+        sh.sc.rec_base = __ldcg(&a.ctl->rec_total[sh.sc.n & 1]);
+    }
+    if (threadIdx.x < 4) sh.phase_cnt[threadIdx.x] = 0;
+    if (threadIdx.x < 2) sh.n_d1x[threadIdx.x] = 0;
+    const PopDev* P = stage_pops(a, sh.pops);
+    __syncthreads();
+    const long long gtid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int U = pipe_updater_threads(a.N, false), R = (int)blockDim.x - U;
+    const long long res_i = (long long)blockIdx.x * U + threadIdx.x;
+    const bool updater = (int)threadIdx.x < U;
+    if (updater && res_i < a.N) {
+        const int t = threadIdx.x;
+        sh.res_V[t] = a.V[res_i]; sh.res_I[t] = a.I[res_i]; sh.res_r[t] = a.refr[res_i]; sh.res_pi[t] = a.pop_of[res_i];
+        sh.res_row[t] = ld_row_info(a.row_info + res_i);
+    }
+    const long long n0 = sh.sc.n;
+    const int slot0 = sh.sc.slot;
+    unsigned long long rec_prev = sh.sc.rec_base, spikes = 0, epoch = 0;
+    bool ovf = false;
+    if (n_steps > 0) {
+        if (gtid < 5) a.ctl->spike_cnt8[(n0 + gtid) & 7] = 0;      // (the updaters clear the counter of the fifth step ahead)
+        if (updater) ovf = resident_decide(a, P, n0, sh, U);       // spikes of the first step of the launch
+        grid_barrier(a.ctl, epoch);                                // the counters are clear before any CTA appends
+    }
+    const unsigned long long G = gridDim.x;
+    long long n = n0;
+    int slot = slot0;
+    int M_last = 0;
+    if (updater) {
+        for (long long s = 0; s < n_steps; ++s, ++n) {
+            // plane(step index s - 1) is the ((s - 1) / 2 + 1)-th use of its word
+            ovf = split_update_step(a, P, n, s, slot, sh, U, s > 0, ovf, s > 0 ? (unsigned long long)(((s - 1) >> 1) + 1) * G : 0ULL, s + 1 < n_steps);
+            slot = slot + 1 == a.Dr ? 0 : slot + 1;
+        }
+    } else {
+        // ---- the rest warps: list(n - 1), then count, descriptors, records and reductions of step n - 1, then the group's arrival ----
+        const int t = threadIdx.x - U;
+        for (long long s = 0; s < n_steps; ++s, ++n) {
+            if (s > 0) {
+                const int Mp = split_rest_pass(a, n, slot, rec_prev, sh, U, R, (unsigned long long)((s + 1) >> 1) * G);
+                rec_prev += (unsigned long long)Mp; spikes += (unsigned long long)Mp;
+            }
+            group_sync(2, R);                                      // every rest warp has issued its reductions of this phase
+            if (t == 0) split_group_done(a, sh, s);
+            slot = slot + 1 == a.Dr ? 0 : slot + 1;
+        }
+    }
+    // the one full stop of the launch: plane(last step)
+    __syncthreads();
+    if (n_steps > 0) {
+        if (threadIdx.x == 0) {
+            unsigned long long v;
+            do {
+                asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(&a.ctl->bar_plane[(n_steps - 1) & 1]) : "memory");
+            } while (v < (unsigned long long)(((n_steps - 1) >> 1) + 1) * G);
+        }
+        __syncthreads();
+    }
+    if (updater && res_i < a.N) {
+        const int t = threadIdx.x;
+        a.V[res_i] = sh.res_V[t]; a.I[res_i] = sh.res_I[t]; a.refr[res_i] = sh.res_r[t];
+    }
+    if (n_steps > 0 && !updater) {                                 // flush: rest pass of the last step
+        M_last = split_rest_pass(a, n, slot, rec_prev, sh, U, R, (unsigned long long)((n_steps + 1) >> 1) * G);
+        rec_prev += (unsigned long long)M_last; spikes += (unsigned long long)M_last;
+        if (blockIdx.x == 0) {
+            group_sync(2, R);
+            if (((n - 1) & 3) >= 2) {                              // the host reads the last step's ids at list index (n - 1) & 1
+                const int32_t* __restrict__ src = a.spike_list + (size_t)((n - 1) & 3) * a.N;
+                int32_t* __restrict__ dst = a.spike_list + (size_t)((n - 1) & 1) * a.N;
+                for (int i = threadIdx.x - U; i < M_last; i += R) dst[i] = __ldcg(src + i);
+            }
+            if ((int)threadIdx.x == U) {                           // what the other kernels and the host expect to find
+                a.ctl->rec_total[n & 1] = rec_prev;
+                a.ctl->rec_total[(n - 1) & 1] = rec_prev;
+                a.ctl->spikes += spikes;
+                a.ctl->spike_cnt[(n - 1) & 3] = M_last;
+                a.ctl->spike_cnt[n & 3] = 0;
+                a.ctl->step_d = n - 1;
+                a.ctl->slot = slot;
+                a.ctl->step_u = n;
+            }
+        }
     }
 }
 
