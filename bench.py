@@ -384,6 +384,8 @@ def run_ours(args):
     if int(s1.step_mode) == 2:
         # one persistent kernel per bench step: its launch IS the timed region (CUDA events on the simulator's stream)
         kern = {1: "persistent_kernel<1>", 2: "persistent_kernel<2>", 3: "persistent_pipe_kernel", 4: "persistent_kernel<4>", 6: "persistent_pipe_kernel"}[int(s1.delivery_kernel)]
+        if int(s1.step_kernel) == 3:
+            kern = "persistent_split_kernel"             # ng_stats.step_kernel: what ng_simulate launched
         us = ms_total * 1e3 / args.steps
         ev_per_launch = float(s1.events - s0.events) / args.steps
         # AdEx: seven state words and two input ports per neuron instead of three and one

@@ -182,7 +182,10 @@ typedef struct {
     int32_t step_mode;
     int64_t n_sources;           /* neurons of the whole network (= n_neurons unless target-sharded)  */
     int32_t shard_rank, shard_world;   /* ng_set_shard (0, 1 on one GPU)                             */
-    int32_t id_first, reserved;  /* global id of this shard's first neuron                           */
+    int32_t id_first;            /* global id of this shard's first neuron                           */
+    int32_t step_kernel;         /* persistent kernel of the last ng_simulate call in step mode 2: 0 = none / two-phase
+                                    (persistent_kernel<k>), 1 = persistent_pipe_kernel, 2 = the same with the spike decisions in
+                                    the barrier shadow, 3 = persistent_split_kernel (list / plane barriers, decoupled warp groups) */
 } ng_stats;
 
 /* Create a simulator on cfg->device.  `alloc` may be NULL.  `cuda_stream` is a cudaStream_t (or NULL).

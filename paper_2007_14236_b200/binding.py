@@ -79,7 +79,7 @@ class NgStats(C.Structure):
                 ("ms_update", C.c_double), ("ms_deliver", C.c_double), ("launches_update", C.c_uint64),
                 ("launches_deliver", C.c_uint64), ("launches_other", C.c_uint64), ("delivery_kernel", C.c_int32),
                 ("step_mode", C.c_int32), ("n_sources", C.c_int64), ("shard_rank", C.c_int32), ("shard_world", C.c_int32),
-                ("id_first", C.c_int32), ("reserved", C.c_int32)]
+                ("id_first", C.c_int32), ("step_kernel", C.c_int32)]
 
 
 class NgError(RuntimeError):

@@ -42,6 +42,7 @@ struct ng_sim {
     int32_t bypass = 0; uint32_t inject_thr = 0;
     // options
     int list_bufs = 2;
+    int step_kernel = 0;
     int step_mode_opt = 3; int step_mode = 0; int steps_per_graph = 100; int delivery_kernel_opt = 0; int deliver_blocks_opt = 0;
     bool trace_on = false; unsigned long long* trace_saved = nullptr; int last_persistent_blocks = 0;
     int profile = 0; int async = 0; int sort_segments = 1; int prefetch_opt = 1;
@@ -934,7 +935,9 @@ int32_t ng_simulate(ng_sim* s, int64_t n_steps) {
         NG_CUDA(s, cudaMemsetAsync(&s->d_ctl->bar, 0, offsetof(Ctl, bar_list) + 2 * sizeof(unsigned long long) - offsetof(Ctl, bar), st));   // bar, ticket, bar_plane, bar_list
         const bool piped = s->delivery_kernel == 3 || s->delivery_kernel == 6;
         s->last_persistent_blocks = piped ? s->persistent_pipe_blocks : s->persistent_blocks;
+        s->step_kernel = 0;
         if (s->delivery_kernel == 6) {
+            s->step_kernel = 1;
             const void* fn = s->has_adex ? (s->one_round_persistent ? (const void*)persistent_pipe_kernel<true, true, false, true>
                                                                      : (const void*)persistent_pipe_kernel<true, false, false, true>)
                                          : (s->one_round_persistent && !s->bypass ? (const void*)persistent_pipe_kernel<false, true, false, true>
@@ -944,6 +947,7 @@ int32_t ng_simulate(ng_sim* s, int64_t n_steps) {
                                                    dim3(s->has_adex ? 512 : s->persistent_threads), args,
                                                    s->has_adex || s->one_round_persistent ? 0 : s->resm_bytes, st));
         } else if (s->delivery_kernel == 3) {
+            s->step_kernel = s->has_adex || !(s->one_round_persistent && !s->bypass) || !early_decision(s) ? 1 : NG_SPLIT_KERNEL ? 3 : 2;
             const void* fn = s->has_adex ? (s->one_round_persistent ? (const void*)persistent_pipe_kernel<true, true>
                                                                      : (const void*)persistent_pipe_kernel<true, false>)
                                          : (s->one_round_persistent && !s->bypass
@@ -1093,7 +1097,7 @@ int32_t ng_get_stats(ng_sim* s, ng_stats* out) {
     if (!s || !out) return NG_ERR_INVALID_ARG;
     std::memset(out, 0, sizeof(*out));
     out->n_neurons = s->prepared ? s->NL : s->N;
-    out->n_sources = s->N; out->shard_rank = s->shard_rank; out->shard_world = s->shard_world; out->id_first = s->id_first;
+    out->n_sources = s->N; out->shard_rank = s->shard_rank; out->shard_world = s->shard_world; out->id_first = s->id_first; out->step_kernel = s->step_kernel;
     out->step_mode = s->step_mode;
     if (!s->prepared) return NG_OK;
     NG_CUDA(s, cudaSetDevice(s->cfg.device));
