@@ -284,3 +284,38 @@ def test_cfg1_free_running_rates_10s(oracle_mod, B):
         print(f"{name}: gpu {rg:.3f} Hz oracle {ro:.3f} Hz")
         assert abs(rg - ro) <= max(0.05 * ro, 0.1), (name, rg, ro)
     g.close()
+
+
+def test_split_kernel_cta_list_overflow(oracle_mod, B):
+    """The split kernel (resident LIF state, list / plane barriers) keeps at most 256 spikes per CTA and step on the CTA's
+    list; a thread whose spike does not fit delivers its delay-1 records and appends to the global spike array alone.
+    Here EVERY neuron starts above threshold: 80,000 neurons on 148 CTAs = 541 spikes per CTA in step 0 (and again whenever
+    the synchronised population comes out of refractoriness) — spike for spike against the oracle, across launch
+    boundaries, and the last step's spike array where the host reads it."""
+    wl = W.balanced_large(n=80_000, k_total=20, n_steps=60)
+    o, g = make_pair(wl, oracle_mod, debug_input=False)
+    v0 = np.full(wl.n_neurons, -40.0, np.float32)                 # V_th = -50 mV
+    o.set_state(oracle_mod.FIELD_V, v0.astype(np.float64)); g.set_state(B.FIELD_V, v0)
+    for c in (1, 24, 5):
+        g.simulate(c); o.simulate(c)
+        assert g.stats().step_kernel == 3 and g.stats().delivery_kernel == 3
+        assert np.array_equal(np.sort(g.last_spikes()), np.sort(o.last_spikes()))
+    # a second volley in the MIDDLE of a launch (the decision is then taken inside the step loop, not in the launch prologue):
+    # every neuron a few mV below threshold with a synaptic current that carries it across within two or three steps
+    v1 = np.full(wl.n_neurons, -53.0, np.float32); i1 = np.full(wl.n_neurons, 5000.0, np.float32)
+    zr = np.zeros(wl.n_neurons, np.int32)
+    o.set_state(oracle_mod.FIELD_V, v1.astype(np.float64)); g.set_state(B.FIELD_V, v1)
+    o.set_state(oracle_mod.FIELD_I_SYN, i1.astype(np.float64)); g.set_state(B.FIELD_I_SYN, i1)
+    o.set_state(oracle_mod.FIELD_REFR, zr); g.set_state(B.FIELD_REFR, zr)
+    g.simulate(10); o.simulate(10)
+    assert np.array_equal(np.sort(g.last_spikes()), np.sort(o.last_spikes()))
+    gs, gi = g.get_spikes()
+    os_, oi = o.get_spikes()
+    a = set(zip(gs.tolist(), gi.tolist())); b = set(zip(os_.tolist(), oi.tolist()))
+    per_step = np.bincount(os_, minlength=40)
+    assert per_step[0] == wl.n_neurons and per_step[30] < 256 * 148 and np.count_nonzero(per_step[31:] > 256 * 148) >= 1, per_step
+    assert len(a ^ b) <= 3, sorted(a ^ b)[:10]                     # fp32 vs fp64 within 1e-4 mV of threshold (C11)
+    assert g.stats().events == o.n_events or abs(g.stats().events - o.n_events) <= 3 * 20
+    gV = g.get_state(B.FIELD_V).astype(np.float64); oV = o.get_state(oracle_mod.FIELD_V)
+    assert np.mean(np.abs(gV - oV) <= 1e-3) >= 0.999
+    g.close()
