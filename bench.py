@@ -424,7 +424,7 @@ def run_ours(args):
                 "share_of_step": share,
                 "target_frac_north_star": 0.5, "target_met": False,
                 "note": "latency-bound regime: ~1e5 events (0.8 MB) + 2.5 MB of neuron state per time step against "
-                        "~5 us of dependent memory round trips and one grid barrier; the north_star target (>= 50 % of HBM "
+                        "~4 us of dependent memory round trips and grid-wide list / plane barriers; the north_star target (>= 50 % of HBM "
                         "peak on connection-record reads) is about the bandwidth regime: see delivery_microbench "
                         "(best point 0.21 of the measured peak: NOT met; DESIGN.md section 7 names the scattered-reduction ceiling)"}
     g.close()
