@@ -932,7 +932,7 @@ int32_t ng_simulate(ng_sim* s, int64_t n_steps) {
     } else if (s->step_mode == 2) {
         long long ns = n_steps;
         void* args[] = {(void*)&s->a, (void*)&ns};
-        NG_CUDA(s, cudaMemsetAsync(&s->d_ctl->bar, 0, offsetof(Ctl, bar_list) + 2 * sizeof(unsigned long long) - offsetof(Ctl, bar), st));   // bar, ticket, bar_plane, bar_list
+        NG_CUDA(s, cudaMemsetAsync(&s->d_ctl->bar, 0, offsetof(Ctl, bar_list) + 2 * sizeof(BarWord) - offsetof(Ctl, bar), st));   // bar, ticket, bar_plane, bar_list
         const bool piped = s->delivery_kernel == 3 || s->delivery_kernel == 6;
         s->last_persistent_blocks = piped ? s->persistent_pipe_blocks : s->persistent_blocks;
         s->step_kernel = 0;

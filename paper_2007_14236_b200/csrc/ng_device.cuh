@@ -54,6 +54,8 @@ struct PopDev {                // per-population constants of the update (fp32 c
 // Device-resident control block; see ng.cu for the update/deliver handshake.  Words with different traffic live on
 // different 128-byte lines: the barrier counter is polled by every CTA while late CTAs still append spikes
 // (atomics on spike_cnt) and count events — on one line those requests queue at the same L2 slice.
+struct alignas(128) BarWord { unsigned long long v; };   // one barrier word per 128-byte line: polls and arrivals of different
+                                                           // barriers do not queue at one L2 slice
 struct Ctl {
     // line 0: step bookkeeping, written once per step by one thread
     alignas(128) long long step_u;         // written by deliver, read by update: index of the next step
@@ -81,8 +83,8 @@ struct Ctl {
     // line 3: grid barrier of the persistent kernels, and the ticket of the stand-alone pipelined kernel
     alignas(128) unsigned long long bar;   // arrivals at the grid barrier
     unsigned int ticket;                   // CTAs that finished the current step
-    unsigned long long bar_plane[2];       // split kernel: CTAs whose reductions of a phase are all issued and acknowledged, and
-    unsigned long long bar_list[2];        // split kernel: CTAs that have appended their spikes of a step to the global spike array,
+    BarWord bar_plane[2];                  // split kernel: CTAs whose reductions of a phase are all issued and acknowledged, and
+    BarWord bar_list[2];                   // split kernel: CTAs that have appended their spikes of a step to the global spike array,
                                            // one word per step parity each (a CTA may arrive for step n + 1 while another still
                                            // waits for step n to be complete: on one word its arrival would stand in for a missing one;
                                            // it cannot arrive for step n + 2 before step n is complete)
@@ -1988,7 +1990,7 @@ __device__ __forceinline__ int split_rest_pass(const StepArgs& a, long long n, i
             if (t == 0) {
                 unsigned long long v;
                 do {
-                    asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(&a.ctl->bar_list[np & 1]) : "memory");
+                    asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(&a.ctl->bar_list[np & 1].v) : "memory");
                 } while (v < list_need);
             }
             group_sync(2, R);
@@ -2285,7 +2287,7 @@ __device__ __forceinline__ void split_group_done(const StepArgs& a, PipeShared& 
     asm volatile("fence.acq_rel.gpu;" ::: "memory");
     if (atomicAdd(&sh.phase_cnt[s_idx & 3], 1) == 1) {             // the other group was first: the CTA is done with the phase
         sh.phase_cnt[s_idx & 3] = 0;
-        asm volatile("red.relaxed.gpu.global.add.u64 [%0], 1;" ::"l"(&a.ctl->bar_plane[s_idx & 1]) : "memory");
+        asm volatile("red.relaxed.gpu.global.add.u64 [%0], 1;" ::"l"(&a.ctl->bar_plane[s_idx & 1].v) : "memory");
     }
 }
 
@@ -2304,7 +2306,7 @@ __device__ __forceinline__ bool split_update_step(const StepArgs& a, const PopDe
     if (t == 0 && plane_need) {
         unsigned long long v;
         do {
-            asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(&a.ctl->bar_plane[(s_idx - 1) & 1]) : "memory");
+            asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(&a.ctl->bar_plane[(s_idx - 1) & 1].v) : "memory");
         } while (v < plane_need);
     }
     int gb = 0;
@@ -2332,7 +2334,7 @@ __device__ __forceinline__ bool split_update_step(const StepArgs& a, const PopDe
             st_row_info(a.spike_row + buf + gb + s, r);
         }
         __syncwarp();
-        if (lane == 31) asm volatile("red.release.gpu.global.add.u64 [%0], 1;" ::"l"(&a.ctl->bar_list[n & 1]) : "memory");
+        if (lane == 31) asm volatile("red.release.gpu.global.add.u64 [%0], 1;" ::"l"(&a.ctl->bar_list[n & 1].v) : "memory");
     }
     // beside those round trips: the Poisson count of step n + 1 (a pure function of neuron and step; 0.85 us for 17 warps)
     int k_cur = -1;
@@ -2426,7 +2428,7 @@ __global__ void __launch_bounds__(kPersistentThreads, 1) persistent_split_kernel
         if (threadIdx.x == 0) {
             unsigned long long v;
             do {
-                asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(&a.ctl->bar_plane[(n_steps - 1) & 1]) : "memory");
+                asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(&a.ctl->bar_plane[(n_steps - 1) & 1].v) : "memory");
             } while (v < (unsigned long long)(((n_steps - 1) >> 1) + 1) * G);
         }
         __syncthreads();
