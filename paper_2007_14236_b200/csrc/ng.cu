@@ -292,14 +292,15 @@ void configure_launch(ng_sim* s) {
     destroy_graph(s);
 }
 
-// Resident one-round LIF kernel: take the spike decisions of step n + 1 in the barrier shadow of step n (kEarly,
-// ng_device.cuh)?  It pays once a CTA holds enough neurons for spikes to be frequent; with a handful of neurons per CTA
-// the step is the barrier itself and the work in front of the poll only delays it (config 0: 2.52 -> 2.55-2.68 us).
+// Resident one-round LIF networks: the split kernel (persistent_split_kernel: spike decisions a step ahead, list / plane
+// barriers, decoupled warp groups) instead of the pipelined kernel with one grid barrier per step?  Yes as soon as every CTA
+// holds a neuron (config 0, five neurons per CTA: 2.50 -> 2.38 us per step; the kEarly form of the one-barrier kernel, kept
+// behind -DNG_SPLIT_KERNEL=0, only paid from 32 neurons per CTA on: 2.52 -> 2.55-2.68 us at config 0).
 #ifndef NG_SPLIT_KERNEL
 #define NG_SPLIT_KERNEL 1
 #endif
 #ifndef NG_EARLY_MIN_PER_CTA
-#define NG_EARLY_MIN_PER_CTA 32
+#define NG_EARLY_MIN_PER_CTA (NG_SPLIT_KERNEL ? 1 : 32)
 #endif
 bool early_decision(const ng_sim* s) {
     return !s->has_adex && s->list_bufs == 4 && (long long)s->N >= (long long)NG_EARLY_MIN_PER_CTA * s->persistent_pipe_blocks;
